@@ -1,0 +1,464 @@
+// gf_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, obviously-correct CPU evaluation of the hot path of
+// arXiv:1205.0752 (Windisch, Alkofer, Haase, Liebmann): for every complex
+// x = p^2 of a grid, the regularised d=4 one-loop integral eq. (14)/(15)
+// as a non-adaptive radial x angular quadrature (Step 5,
+// PAPER.md:109-113; Kernel 2) of the Taylor-subtracted
+// integrand eq. (12)/(20).
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+// reference legs may build, load or call this file.  It shares no code, header,
+// table or constant generator with paper_1205_0752_b200/csrc (the CUDA path)
+// and neither includes the other.
+//
+// What is computed:
+//
+//   G(x) = c0 * sum_seg sum_i  Wr(seg,i;x) * y_i * sum_j w'_j * F_sub(x, y_i, z_j)
+//
+//   F     = D1(y) * D2(u),   u = x + y - 2 sqrt(x) sqrt(y) z = (p-k)^2   eq. (10),(19)
+//   F_sub = (1 - t^0) F = D1(y) * [ D2(u) - D2(y) ]                      eq. (12),(13),(20)
+//
+// The loops run in the paper's order (sub-contour, radial node, angular node),
+// every term is evaluated in std::complex<double> arithmetic in the combined
+// form the paper itself prints in eq. (20) (so that G(0) = 0 exactly), and the
+// sums are accumulated in long double (accum=0, the parity variant) or double
+// (accum=1, the timed variant).  No blocking, pairing, fusion or reordering.
+//
+// Pins (tests/test_oracle_pins.py): closed form CF1 of the equal-mass bubble,
+// the paper's eq. (18) for masses^2 = +-i/2, the Feynman-parameter form CF3 for
+// the rational propagator, G(0)=0, conjugation symmetry, cutoff independence,
+// line-swap symmetry, rule independence, exactness degree of the quadrature
+// rules, brute-force high-order quadrature.  Unpinned: values of RAY_ARC inside
+// the wedge around the negative real axis and of REAL outside the parabola R2
+// (DESIGN.md "parity unpinned"), where no closed form applies.
+//
+// Build: g++ -O2 -std=c++17 -shared -fPIC -pthread (no -ffast-math).
+
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstring>
+#include <thread>
+#include <vector>
+
+namespace {
+
+typedef std::complex<double> cplx;
+typedef long double ld;
+
+const double kPi = 3.14159265358979323846264338327950288;
+
+// ---- enums (values are part of the oracle's own C interface) -------------
+enum { QUAD_GAUSS_LEGENDRE = 0, QUAD_GAUSS_CHEB2 = 1, QUAD_TANH_SINH = 2 };
+enum { MEASURE_PLAIN = 0, MEASURE_SQRT1MZ2 = 1 };
+enum { PROP_MASSIVE = 0, PROP_RATIONAL = 1 };
+enum { CONTOUR_REAL = 0, CONTOUR_RAY_ARC = 1, CONTOUR_THREAD = 2, CONTOUR_AUTO = 3 };
+enum { SPACING_UNIFORM = 0, SPACING_LOG_ABS_IM = 1 };
+
+struct Propagator {
+  int kind;
+  double m2_re, m2_im;  // MASSIVE: 1/(u + m2)
+  double M2, a, b;      // RATIONAL: (u + M2)/(u^2 + a u + b)
+};
+
+struct Params {
+  Propagator line_k;   // D1(y), carries k        (eq. (19))
+  Propagator line_pk;  // D2(u), carries p-k
+  double cutoff2;      // Lambda^2
+  double sub_re, sub_im;
+  int taylor_order;
+  double prefactor;    // c0; 2/pi reproduces eq. (21)
+  double map_scale;    // s0 of the shifted-log radial map
+  int contour;
+  int precision;
+};
+
+// ---- quadrature rules on [-1,1] ----------------------------
+
+// Gauss-Legendre: roots of P_n by Newton iteration, weights 2/((1-x^2)P_n'(x)^2)
+// (Abramowitz-Stegun 25.4.29; the paper's radial rule, ref. [18]).
+void gauss_legendre(int n, double* x, double* w) {
+  for (int k = 0; k < (n + 1) / 2; ++k) {
+    ld t = std::cos((ld)kPi * ((ld)k + 0.75L) / ((ld)n + 0.5L));
+    ld dp = 0;
+    for (int it = 0; it < 100; ++it) {
+      ld p0 = 1, p1 = t;
+      for (int l = 2; l <= n; ++l) {
+        ld p2 = ((2 * l - 1) * t * p1 - (l - 1) * p0) / l;
+        p0 = p1;
+        p1 = p2;
+      }
+      if (n == 1) { p0 = 1; p1 = t; }
+      dp = n * (t * p1 - p0) / (t * t - 1);
+      ld dt = p1 / dp;
+      t -= dt;
+      if (std::fabs(dt) < 1e-19L) break;
+    }
+    // recompute the derivative at the converged root
+    {
+      ld p0 = 1, p1 = t;
+      for (int l = 2; l <= n; ++l) {
+        ld p2 = ((2 * l - 1) * t * p1 - (l - 1) * p0) / l;
+        p0 = p1;
+        p1 = p2;
+      }
+      dp = n * (t * p1 - p0) / (t * t - 1);
+    }
+    ld wt = 2 / ((1 - t * t) * dp * dp);
+    // k = 0 is the largest root; store ascending
+    x[n - 1 - k] = (double)t;
+    x[k] = -(double)t;
+    w[n - 1 - k] = (double)wt;
+    w[k] = (double)wt;
+  }
+  if (n % 2 == 1) x[n / 2] = 0.0;
+}
+
+int make_quadrature(int kind, int n, double step, int measure, double* x, double* w) {
+  if (n < 1 || !x || !w) return 1;
+  if (kind == QUAD_GAUSS_LEGENDRE) {
+    gauss_legendre(n, x, w);
+    if (measure == MEASURE_SQRT1MZ2)
+      for (int j = 0; j < n; ++j) w[j] *= std::sqrt((1.0 - x[j]) * (1.0 + x[j]));
+    return 0;
+  }
+  if (kind == QUAD_GAUSS_CHEB2) {
+    // Gauss-Chebyshev, 2nd kind: exact Gauss rule for the weight sqrt(1-z^2)
+    // (Abramowitz-Stegun 25.4.40; the paper's check rule).
+    for (int j = 0; j < n; ++j) {
+      ld th = (ld)kPi * (ld)(n - j) / (ld)(n + 1);  // ascending z
+      ld s = std::sin(th);
+      x[j] = (double)std::cos(th);
+      ld ww = (ld)kPi / (ld)(n + 1) * s * s;  // includes sqrt(1-z^2)
+      w[j] = (double)(measure == MEASURE_SQRT1MZ2 ? ww : ww / s);
+    }
+    if (n % 2 == 1) x[n / 2] = 0.0;
+    return 0;
+  }
+  if (kind == QUAD_TANH_SINH) {
+    // Takahasi-Mori double exponential rule (the paper's angular rule, ref. [19]):
+    // z_k = tanh(pi/2 sinh(kh)), w_k = pi/2 h cosh(kh) / cosh^2(pi/2 sinh(kh)),
+    // k = -(n-1)/2 .. (n-1)/2.  Step h: reading G8, 2.9/((n-1)/2).
+    ld h = step > 0 ? (ld)step : (n > 1 ? 2.9L / (((ld)n - 1) / 2) : 1.0L);
+    for (int j = 0; j < n; ++j) {
+      ld k = (ld)j - ((ld)n - 1) / 2;
+      ld a = 0.5L * (ld)kPi * std::sinh(k * h);
+      ld ch = std::cosh(a);
+      x[j] = (double)std::tanh(a);
+      ld ww = 0.5L * (ld)kPi * h * std::cosh(k * h) / (ch * ch);
+      // sqrt(1 - tanh^2) = sech, computed without cancellation
+      w[j] = (double)(measure == MEASURE_SQRT1MZ2 ? ww / ch : ww);
+    }
+    if (n % 2 == 1) x[n / 2] = 0.0;
+    return 0;
+  }
+  return 2;
+}
+
+// ---- Step 4 / Kernel 1: the grid ------------------
+// Endpoint-inclusive homogeneous distribution (reading G9).  Two-sided: the
+// lower half counts up from min, the upper half counts down from max, so a
+// range symmetric about 0 gives exactly mirrored values.
+double lin_two_sided(double lo, double hi, int n, int i) {
+  if (n == 1) return lo;
+  double d = (hi - lo) / (double)(n - 1);
+  if (2 * i <= n - 1) return std::fma((double)i, d, lo);
+  return std::fma(-(double)(n - 1 - i), d, hi);
+}
+
+int make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
+              int spacing, double im_abs_min, double* x) {
+  if (!x) return 1;
+  if (n_re < 1 || n_im < 1) return 2;
+  if (spacing == SPACING_LOG_ABS_IM) {
+    // reading G10: |Im x| log-spaced in [im_abs_min, im_max], both signs, ascending Im
+    if (n_im % 2 != 0 || !(im_abs_min > 0) || !(im_max > im_abs_min) || im_min != -im_max) return 2;
+  } else if (spacing != SPACING_UNIFORM) {
+    return 2;
+  }
+  for (int j = 0; j < n_im; ++j) {
+    double im;
+    if (spacing == SPACING_UNIFORM) {
+      im = lin_two_sided(im_min, im_max, n_im, j);
+    } else {
+      int half = n_im / 2;
+      int k = j >= half ? j - half : half - 1 - j;
+      double v;
+      if (k == 0) v = im_abs_min;
+      else if (k == half - 1) v = im_max;
+      else {
+        double l0 = std::log(im_abs_min), l1 = std::log(im_max);
+        v = std::exp(std::fma((double)k / (double)(half - 1), l1 - l0, l0));
+      }
+      im = j >= half ? v : -v;
+    }
+    for (int i = 0; i < n_re; ++i) {
+      x[2 * ((size_t)j * n_re + i) + 0] = lin_two_sided(re_min, re_max, n_re, i);
+      x[2 * ((size_t)j * n_re + i) + 1] = im;
+    }
+  }
+  return 0;
+}
+
+// ---- propagators ---------------------------------------------------------
+cplx prop(const Propagator& P, cplx u) {
+  if (P.kind == PROP_MASSIVE) return 1.0 / (u + cplx(P.m2_re, P.m2_im));
+  return (u + P.M2) / (u * u + P.a * u + P.b);
+}
+
+// D2(u) - D2(y) with u = y + d, in the combined form of eq. (20)
+// (PAPER.md:198-203): the factor d = x - 2 sqrt(x) sqrt(y) z is explicit, so
+// the difference is exactly 0 at x = 0 and keeps full relative accuracy at
+// small |x| (a numerical difference of two nearly equal numbers would not).
+cplx prop_diff(const Propagator& P, cplx y, cplx d) {
+  cplx u = y + d;
+  if (P.kind == PROP_MASSIVE) {
+    cplx c = y + cplx(P.m2_re, P.m2_im);
+    return -d / ((c + d) * c);
+  }
+  // (u+M2)/Q(u) - (y+M2)/Q(y) = -d [u y + M2 (u+y) + a M2 - b] / (Q(u) Q(y))
+  cplx Qu = u * u + P.a * u + P.b;
+  cplx Qy = y * y + P.a * y + P.b;
+  return -d * (u * y + P.M2 * (u + y) + (P.a * P.M2 - P.b)) / (Qu * Qy);
+}
+
+// scale of the singular structure of line 2 in the y-plane: |m2^2| for a
+// massive line, the largest pole modulus sqrt(b)... of Q(u)=u^2+au+b for a
+// rational one (used only to size contours).
+double line2_scale(const Propagator& P) {
+  if (P.kind == PROP_MASSIVE) return std::hypot(P.m2_re, P.m2_im);
+  double disc = P.a * P.a - 4.0 * P.b;
+  if (disc < 0) return std::sqrt(P.b);  // complex-conjugate pair, |u_r|^2 = b
+  double r = std::sqrt(disc);
+  return std::fmax(std::fabs(-P.a + r), std::fabs(-P.a - r)) / 2.0;
+}
+
+// ---- contours (Step 3; the IF-THEN-ELSE of Kernel 2,
+//      PAPER.md:162,310).  DESIGN.md "Contour policies" states each one. -----
+struct RNode { cplx y; cplx wy; };  // node and (rule weight) x dy/dt
+
+struct Rule { const double* t; const double* w; int n; };
+
+// level l of the radial pyramid: Gauss-Legendre rule of order n_rad >> l
+// ("n arrays for the radial nodes"), stored back to back.
+Rule level(const double* nodes, const double* weights, int n_rad, int l) {
+  int off = 0, n = n_rad;
+  for (int k = 0; k < l; ++k) { off += n; n /= 2; }
+  Rule r = { nodes + off, weights + off, n };
+  return r;
+}
+
+// shifted-log map of a real segment [a,b] (readings G3/G4):
+//   y(u) = a + (a+s0) expm1(u L),  L = ln((b+s0)/(a+s0)),  dy/du = L (y+s0)
+void seg_logreal(double a, double b, double s0, cplx dir, Rule R, std::vector<RNode>& out) {
+  double L = std::log((b + s0) / (a + s0));
+  for (int i = 0; i < R.n; ++i) {
+    double u = 0.5 * (R.t[i] + 1.0);
+    double r = a + (a + s0) * std::expm1(u * L);
+    double dr = 0.5 * R.w[i] * L * (r + s0);
+    RNode nd = { dir * r, dir * dr };
+    out.push_back(nd);
+  }
+}
+
+void seg_line(cplx a, cplx b, Rule R, std::vector<RNode>& out) {
+  for (int i = 0; i < R.n; ++i) {
+    double u = 0.5 * (R.t[i] + 1.0);
+    RNode nd = { a + (b - a) * u, (b - a) * (0.5 * R.w[i]) };
+    out.push_back(nd);
+  }
+}
+
+void seg_arc(double Rad, double th0, double th1, Rule R, std::vector<RNode>& out) {
+  for (int i = 0; i < R.n; ++i) {
+    double u = 0.5 * (R.t[i] + 1.0);
+    double th = th0 + (th1 - th0) * u;
+    cplx y = Rad * cplx(std::cos(th), std::sin(th));
+    RNode nd = { y, cplx(0, 1) * y * ((th1 - th0) * 0.5 * R.w[i]) };
+    out.push_back(nd);
+  }
+}
+
+void contour_real(const Params& P, const double* rn, const double* rw, int n_rad, std::vector<RNode>& out) {
+  seg_logreal(0.0, P.cutoff2, P.map_scale, cplx(1, 0), level(rn, rw, n_rad, 0), out);
+}
+
+void contour_ray_arc(const Params& P, cplx x, const double* rn, const double* rw, int n_rad,
+                     std::vector<RNode>& out) {
+  double ax = std::sqrt(std::fma(x.real(), x.real(), x.imag() * x.imag()));
+  double phi = std::atan2(x.imag(), x.real());
+  double sc = line2_scale(P.line_pk);
+  double q = std::sqrt(ax) + std::sqrt(ax + sc);
+  double Rad = std::fmin(1.5 * q * q, 0.5 * P.cutoff2);
+  cplx dir(std::cos(phi), std::sin(phi));
+  seg_logreal(0.0, Rad, P.map_scale, dir, level(rn, rw, n_rad, 1), out);
+  seg_arc(Rad, phi, 0.0, level(rn, rw, n_rad, 2), out);
+  seg_logreal(Rad, P.cutoff2, P.map_scale, cplx(1, 0), level(rn, rw, n_rad, 2), out);
+}
+
+// THREAD: equal real masses, Re x < -4 m^2, near the negative axis.
+void contour_thread(const Params& P, cplx x, const double* rn, const double* rw, int n_rad,
+                    std::vector<RNode>& out) {
+  bool mirror = x.imag() < 0;
+  cplx xx = mirror ? std::conj(x) : x;
+  double m2 = P.line_pk.m2_re, m = std::sqrt(m2);
+  double s = std::sqrt(std::fma(xx.real(), xx.real(), xx.imag() * xx.imag()));
+  double phi = std::atan2(xx.imag(), xx.real());
+  double rs = std::sqrt(s);
+  double Aa = (rs - m) * (rs - m), Bb = (rs + m) * (rs + m);
+  double r0 = std::abs(xx + m2);
+  cplx e(std::cos(phi), std::sin(phi));
+  cplx W[6];
+  W[0] = 0.0;
+  W[1] = cplx(-m2, 0.5 * (Aa - m2));
+  W[2] = 0.5 * (Aa + m2) * e;
+  W[3] = cplx(-0.5 * (Aa + r0), -0.5 * (r0 - Aa));
+  W[4] = r0 * e;
+  double Rad = std::fmin(1.5 * Bb, 0.5 * P.cutoff2);
+  double th5 = 0.75 * kPi;
+  W[5] = Rad * cplx(std::cos(th5), std::sin(th5));
+  size_t first = out.size();
+  for (int k = 0; k < 5; ++k) seg_line(W[k], W[k + 1], level(rn, rw, n_rad, 3), out);
+  seg_arc(Rad, th5, 0.0, level(rn, rw, n_rad, 3), out);
+  seg_logreal(Rad, P.cutoff2, P.map_scale, cplx(1, 0), level(rn, rw, n_rad, 2), out);
+  if (mirror)
+    for (size_t k = first; k < out.size(); ++k) {
+      out[k].y = std::conj(out[k].y);
+      out[k].wy = std::conj(out[k].wy);
+    }
+}
+
+bool thread_applicable(const Params& P) {
+  return P.line_k.kind == PROP_MASSIVE && P.line_pk.kind == PROP_MASSIVE && P.line_k.m2_im == 0 &&
+         P.line_pk.m2_im == 0 && P.line_k.m2_re == P.line_pk.m2_re && P.line_pk.m2_re > 0;
+}
+
+// AUTO: per-point choice, half-open tests exactly as DESIGN.md writes them.
+int auto_policy(const Params& P, cplx x, int n_ang) {
+  double sc = line2_scale(P.line_pk);
+  double ax2 = std::fma(x.real(), x.real(), x.imag() * x.imag());
+  bool wedge = (x.real() < -sc) && (std::fabs(x.imag()) * ((double)n_ang * sc) < 5.0 * ax2);
+  if (!wedge) return CONTOUR_RAY_ARC;
+  if (thread_applicable(P) && x.real() <= -4.1 * sc) return CONTOUR_THREAD;
+  return CONTOUR_REAL;
+}
+
+// ---- Step 5 / Kernel 2: the double sum for one x ---------------------------
+template <typename ACC>
+cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int n_rad,
+                const double* z, const double* wz, int n_ang, std::vector<RNode>& nodes) {
+  nodes.clear();
+  int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, x, n_ang) : P.contour;
+  if (pol == CONTOUR_REAL) contour_real(P, rn, rw, n_rad, nodes);
+  else if (pol == CONTOUR_RAY_ARC) contour_ray_arc(P, x, rn, rw, n_rad, nodes);
+  else contour_thread(P, x, rn, rw, n_rad, nodes);
+
+  cplx sx = std::sqrt(x);  // principal branch
+  ACC gr = 0, gi = 0;
+  for (size_t i = 0; i < nodes.size(); ++i) {
+    cplx y = nodes[i].y;
+    cplx B = 2.0 * sx * std::sqrt(y);
+    cplx D1 = prop(P.line_k, y);
+    ACC sr = 0, si = 0;
+    for (int j = 0; j < n_ang; ++j) {
+      cplx d = x - B * z[j];                                   // u - y
+      cplx f = D1 * prop_diff(P.line_pk, y, d);                // F_sub, eq. (20)
+      sr += (ACC)(wz[j] * f.real());
+      si += (ACC)(wz[j] * f.imag());
+    }
+    cplx S((double)sr, (double)si);
+    cplx term = nodes[i].wy * y * S;                           // dy y (...), eq. (14)
+    gr += (ACC)term.real();
+    gi += (ACC)term.imag();
+  }
+  return P.prefactor * cplx((double)gr, (double)gi);
+}
+
+int check_params(const Params& P, int n_rad, int n_ang) {
+  if (n_rad < 1 || n_ang < 1) return 2;
+  if (!(P.cutoff2 > 0) || !(P.map_scale > 0)) return 2;
+  if (P.taylor_order != 0 || P.sub_re != 0 || P.sub_im != 0) return 3;
+  if (P.contour < 0 || P.contour > 3) return 2;
+  if (P.contour != CONTOUR_REAL && n_rad % 8 != 0) return 2;
+  if (P.contour == CONTOUR_THREAD && !thread_applicable(P)) return 3;
+  return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gfo_make_quadrature(int kind, int n, double step, int measure, double* nodes, double* weights) {
+  return make_quadrature(kind, n, step, measure, nodes, weights);
+}
+
+int gfo_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
+                  int spacing, double im_abs_min, double* x) {
+  return make_grid(re_min, re_max, n_re, im_min, im_max, n_im, spacing, im_abs_min, x);
+}
+
+// x, out: interleaved (re, im) doubles.  accum: 0 = long double sums (parity),
+// 1 = double sums (the timed variant).  n_threads <= 0: hardware concurrency.
+// Returns 0 on success; fills *threads_used.
+int gfo_eval_grid(const void* params, const double* rad_nodes, const double* rad_weights, int n_rad,
+                  const double* ang_nodes, const double* ang_weights, int n_ang, const double* x,
+                  long long n_points, double* out, int n_threads, int accum, int* threads_used) {
+  if (!params || !rad_nodes || !rad_weights || !ang_nodes || !ang_weights || (!x && n_points) ||
+      (!out && n_points))
+    return 1;
+  Params P;
+  std::memcpy(&P, params, sizeof(Params));
+  int rc = check_params(P, n_rad, n_ang);
+  if (rc) return rc;
+  if (n_points < 0) return 2;
+  int nt = n_threads > 0 ? n_threads : (int)std::thread::hardware_concurrency();
+  if (nt < 1) nt = 1;
+  if ((long long)nt > n_points) nt = n_points > 0 ? (int)n_points : 1;
+  if (threads_used) *threads_used = nt;
+  auto work = [&](int tid) {
+    std::vector<RNode> nodes;
+    nodes.reserve((size_t)n_rad);
+    for (long long p = tid; p < n_points; p += nt) {
+      cplx xx(x[2 * p], x[2 * p + 1]);
+      cplx g = accum == 0
+                   ? eval_point<ld>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
+                   : eval_point<double>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes);
+      out[2 * p] = g.real();
+      out[2 * p + 1] = g.imag();
+    }
+  };
+  if (nt == 1) {
+    work(0);
+  } else {
+    std::vector<std::thread> th;
+    for (int t = 0; t < nt; ++t) th.emplace_back(work, t);
+    for (auto& t : th) t.join();
+  }
+  return 0;
+}
+
+// the contour of one point, for tests and plots: fills y (2*n doubles) and
+// wy (2*n doubles); returns the policy used (0..2) or a negative error.
+int gfo_contour_nodes(const void* params, double x_re, double x_im, const double* rad_nodes,
+                      const double* rad_weights, int n_rad, int n_ang, double* y, double* wy, int* n_out) {
+  Params P;
+  std::memcpy(&P, params, sizeof(Params));
+  if (check_params(P, n_rad, n_ang)) return -1;
+  cplx x(x_re, x_im);
+  std::vector<RNode> nodes;
+  int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, x, n_ang) : P.contour;
+  if (pol == CONTOUR_REAL) contour_real(P, rad_nodes, rad_weights, n_rad, nodes);
+  else if (pol == CONTOUR_RAY_ARC) contour_ray_arc(P, x, rad_nodes, rad_weights, n_rad, nodes);
+  else contour_thread(P, x, rad_nodes, rad_weights, n_rad, nodes);
+  for (size_t i = 0; i < nodes.size(); ++i) {
+    y[2 * i] = nodes[i].y.real(); y[2 * i + 1] = nodes[i].y.imag();
+    wy[2 * i] = nodes[i].wy.real(); wy[2 * i + 1] = nodes[i].wy.imag();
+  }
+  *n_out = (int)nodes.size();
+  return pol;
+}
+
+int gfo_params_size(void) { return (int)sizeof(Params); }
+
+}  // extern "C"

@@ -1,0 +1,391 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU).
+
+Each test names the plausible mistake it would catch.  Nothing here compares the
+oracle with itself through the same formula: references are closed forms evaluated
+with mpmath (tests/closed_forms.py), numpy's own Gauss-Legendre routine, exact
+moments, and invariants.
+"""
+import math
+import os
+
+import mpmath as mp
+import numpy as np
+import pytest
+
+import gf_workloads as W
+from tests import closed_forms as CF
+
+BUB = {"kind": "massive", "m2": 1.0}
+RAT = {"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2}
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "closed_form_samples.txt")
+
+
+def relerr(g, ref):
+    ref = np.asarray(ref, dtype=complex)
+    g = np.asarray(g, dtype=complex)
+    den = np.where(np.abs(ref) == 0, 1.0, np.abs(ref))
+    return np.abs(g - ref) / den
+
+
+def tables(O, n_rad, n_ang, ang="gauss_legendre", levels=4):
+    rn, rw = O.make_radial_pyramid(n_rad, levels=levels)
+    z, wz = O.make_quadrature(ang, n_ang, measure="sqrt1mz2")
+    return rn, rw, z, wz
+
+
+def G(O, xs, line_k=BUB, line_pk=BUB, cutoff2=1e6, n_rad=256, n_ang=128, ang="gauss_cheb2",
+      contour="real", **kw):
+    P = O.make_params(line_k, line_pk, cutoff2, contour=contour, **kw)
+    rn, rw, z, wz = tables(O, n_rad, n_ang, ang)
+    g, _ = O.eval_grid(P, rn, rw, n_rad, z, wz, np.asarray(xs, dtype=complex))
+    return g
+
+
+# ---------------------------------------------------------------- closed forms themselves
+def test_closed_forms_match_survey_samples():
+    """The mpmath closed forms reproduce the independently computed sample values."""
+    for line in open(GOLD):
+        if line.startswith("#") or not line.strip():
+            continue
+        form, xr, xi, gr, gi = line.split()
+        x = complex(float(xr), float(xi))
+        if form == "CF1":
+            v = CF.cf1(x)
+        elif form == "CF2":
+            v = CF.cf2_paper_eq18(x)
+        else:
+            v = CF.cf3_rational(x, 1.0, 2.0, 0.5, 1.2)
+        assert abs(complex(v) - complex(float(gr), float(gi))) < 2e-10, (form, x)
+
+
+def test_cf1_series_and_threshold():
+    # small-x series -tau/6 + tau^2/60 - tau^3/420 and G(-4 m^2) = 2
+    x = mp.mpf("1e-3")
+    assert abs(CF.cf1(x) - (-x / 6 + x ** 2 / 60 - x ** 3 / 420)) < 1e-13
+    assert abs(CF.cf1(-4) - 2) < 1e-25
+
+
+# ---------------------------------------------------------------- quadrature tables (a2)
+@pytest.mark.parametrize("n", [1, 2, 5, 32, 64, 255, 512])
+def test_gauss_legendre_matches_numpy_and_is_exact(oracle, n):
+    """Catches wrong roots/weights, ordering, asymmetry (A-S 25.4.29)."""
+    x, w = oracle.make_quadrature("gauss_legendre", n)
+    xr, wr = np.polynomial.legendre.leggauss(n)
+    assert np.max(np.abs(x - xr)) < 4e-16
+    assert np.max(np.abs(w - wr) / wr) < 1e-9   # numpy's own end weights are only ~1e-10 at n=512
+    if n >= 2:  # 40-digit reference for a few nodes: weights to a few ulp
+        mp40 = mp.mp.clone()
+        mp40.dps = 40
+        for k in sorted({0, 1, n // 3, (n - 1) // 2}):
+            r = mp40.findroot(lambda t: mp40.legendre(n, t), mp40.mpf(float(x[k])), tol=1e-30)
+            dpn = n * (r * mp40.legendre(n, r) - mp40.legendre(n - 1, r)) / (r * r - 1)
+            wk = 2 / ((1 - r * r) * dpn * dpn)
+            assert abs(r - float(x[k])) < 3e-16 and abs(wk - float(w[k])) / wk < 1e-14
+    assert np.all(np.diff(x) > 0) or n == 1
+    assert np.array_equal(x, -x[::-1]) and np.array_equal(w, w[::-1])
+    for k in range(0, min(2 * n, 40), 2):  # exact for degree <= 2n-1
+        assert abs(np.sum(w * x ** k) - 2.0 / (k + 1)) < 1e-14
+
+
+@pytest.mark.parametrize("n", [3, 32, 128])
+def test_cheb2_moments(oracle, n):
+    """int sqrt(1-z^2) z^(2k) dz = pi (2k)! / (2^(2k+1) k! (k+1)!) exactly for 2k <= 2n-1."""
+    z, w = oracle.make_quadrature("gauss_cheb2", n, measure="sqrt1mz2")
+    for k in range(0, min(n, 12)):
+        exact = math.pi * math.factorial(2 * k) / (2 ** (2 * k + 1) * math.factorial(k) * math.factorial(k + 1))
+        assert abs(np.sum(w * z ** (2 * k)) - exact) < 1e-14
+    zp, wp = oracle.make_quadrature("gauss_cheb2", n, measure="plain")
+    assert np.allclose(wp * np.sqrt(1 - zp ** 2), w, rtol=1e-13)
+
+
+def test_tanh_sinh_rule(oracle):
+    """n = 49 (the paper's ndbl) with the default step integrates the d=4
+    angular measure and a smooth integrand to ~1e-12 (reading G8)."""
+    z, w = oracle.make_quadrature("tanh_sinh", 49, measure="sqrt1mz2")
+    assert abs(np.sum(w) - math.pi / 2) < 1e-11
+    a, b = 3.0, 1.0  # int sqrt(1-z^2)/(a - b z) dz = pi (a - sqrt(a^2-b^2)) / b^2
+    assert abs(np.sum(w / (a - b * z)) - math.pi * (a - math.sqrt(a * a - b * b)) / b ** 2) < 1e-11
+    zp, wp = oracle.make_quadrature("tanh_sinh", 49, measure="plain")
+    assert abs(np.sum(wp * zp ** 2) - 2.0 / 3.0) < 1e-11
+    assert np.array_equal(z, -z[::-1])
+
+
+def test_angular_measure_of_gl(oracle):
+    z, w = oracle.make_quadrature("gauss_legendre", 64, measure="sqrt1mz2")
+    zp, wp = oracle.make_quadrature("gauss_legendre", 64, measure="plain")
+    assert np.allclose(w, wp * np.sqrt(1 - zp ** 2), rtol=1e-14)
+
+
+# ---------------------------------------------------------------- grid (a1)
+def test_grid_uniform(oracle):
+    """Endpoint-inclusive, re index fastest, exactly mirrored rows (reading G9)."""
+    x = oracle.make_grid(-5.0, 1.0, 64, -2.0, 2.0, 64)
+    assert x.shape == (64, 64)
+    assert x[0, 0] == complex(-5, -2) and x[-1, -1] == complex(1, 2)
+    assert np.max(np.abs(x[0].real - np.linspace(-5, 1, 64))) < 2e-15
+    assert np.max(np.abs(x[:, 0].imag - np.linspace(-2, 2, 64))) < 2e-15
+    assert np.array_equal(x[::-1].imag, -x.imag)          # rows j <-> N-1-j are conjugates
+    assert np.all(x.imag != 0)                              # even N: Im x = 0 never occurs
+    assert np.array_equal(x[3].real, x[40].real)
+    one = oracle.make_grid(0.25, 9.0, 1, -1.0, 7.0, 1)
+    assert one[0, 0] == complex(0.25, -1.0)
+
+
+def test_grid_log_abs_im(oracle):
+    """Config 5 (reading G10): ascending Im, 128 log-spaced |Im| per sign in [1e-6, 1e-3]."""
+    x = oracle.make_grid(-10.0, -3.0, 16, -1e-3, 1e-3, 256, spacing="log_abs_im", im_abs_min=1e-6)
+    im = x[:, 0].imag
+    assert im[0] == -1e-3 and im[127] == -1e-6 and im[128] == 1e-6 and im[255] == 1e-3
+    assert np.all(np.diff(im) > 0)
+    assert np.array_equal(im[::-1], -im)
+    ratio = im[129:] / im[128:-1]
+    assert np.allclose(ratio, (1e3) ** (1 / 127), rtol=1e-12)
+    with pytest.raises(ValueError):
+        oracle.make_grid(-10.0, -3.0, 16, -1e-3, 1e-3, 255, spacing="log_abs_im", im_abs_min=1e-6)
+
+
+# ---------------------------------------------------------------- the double sum vs closed forms
+def test_cf1_tight_cheb2(oracle):
+    """Pins measure (y dy, sqrt(1-z^2)), prefactor 2/pi, the shifted-log map and its Jacobian,
+    the subtraction term and u = x+y-2 sqrt(x) sqrt(y) z, to 1e-10 (Chebyshev angular rule)."""
+    xs = [0.5 + 0.2j, 1 + 2j, 0.3 - 0.1j, 1.5 + 0j, -0.5 + 0.5j, 1e-3 + 2e-3j, 1e-5 - 1e-5j]
+    assert all(CF.in_parabola_R2(x) for x in xs)
+    g = G(oracle, xs)
+    ref = [complex(CF.cf1(x)) for x in xs]
+    assert np.max(relerr(g, ref)) < 1e-10
+
+
+def test_cf1_other_mass(oracle):
+    """m^2 = 2.5 on both lines: catches a mass that is hard-wired to 1."""
+    xs = [0.7 + 0.4j, 2 - 1j]
+    m = {"kind": "massive", "m2": 2.5}
+    g = G(oracle, xs, line_k=m, line_pk=m)
+    assert np.max(relerr(g, [complex(CF.cf1(x, 2.5)) for x in xs])) < 1e-10
+
+
+@pytest.mark.parametrize("name,tol", [("cfg1_tiny", 2e-4), ("cfg2_mid", 3e-6)])
+def test_configs_vs_cf1_inside_parabola(oracle, name, tol):
+    """Configs 1 and 2 as BASELINE.json states them (Gauss-Legendre angular rule, REAL contour)
+    on the mask 'parabola R2 shrunk by 0.5' (measured: 1.03e-4 / 1.40e-6; with a shrink of 0.25
+    the points next to the parabola reach 4.2e-4 / 5.3e-6); the bound is the GL angular
+    quadrature error (reading G5)."""
+    c = W.CONFIGS[name]
+    x = oracle.make_grid(c["re"][0], c["re"][1], c["n_re"], c["im"][0], c["im"][1], c["n_im"])
+    step = max(1, c["n_re"] // 48)
+    xs = x[::step, ::step].ravel()
+    xs = np.array([v for v in xs if CF.in_parabola_R2(v, shrink=0.5)])
+    assert xs.size > 100
+    g = G(oracle, xs, cutoff2=c["cutoff2"], n_rad=c["n_rad"], n_ang=c["n_ang"], ang="gauss_legendre")
+    err = relerr(g, [complex(CF.cf1(v)) for v in xs])
+    assert np.max(err) < tol
+    assert np.max(err) > tol / 50   # the error really is the GL angular error, not something else
+
+
+def test_cf2_paper_example(oracle):
+    """The paper's worked example eq. (19)-(21) against its eq. (18) in
+    region 1 (Re x > (Im x)^2 - 1/4).  Catches swapped lines / wrong sign of a complex mass."""
+    k = {"kind": "massive", "m2": 0.5j}
+    pk = {"kind": "massive", "m2": -0.5j}
+    xs = [0.5 + 0.2j, 2 + 1j, 3 + 0j, 1 - 0.5j, 0.2 + 0.1j]
+    assert all(x.real > x.imag ** 2 - 0.25 for x in xs)
+    g = G(oracle, xs, line_k=k, line_pk=pk, cutoff2=1e8, n_rad=512)
+    ref = [complex(CF.cf2_paper_eq18(x)) for x in xs]
+    assert np.max(relerr(g, ref)) < 1e-10
+    # a wrong sign of one mass is a different function (a line SWAP is not: invariant I4)
+    g_wrong = G(oracle, xs, line_k=k, line_pk=k, cutoff2=1e8, n_rad=512)
+    assert np.min(relerr(g_wrong, ref)) > 1e-2
+
+
+def test_finite_cutoff_against_adaptive_integration(oracle):
+    """eq. (14) at a SMALL cutoff, Lambda^2 = 50, where the two lines are
+    distinguishable (O(Lambda^-4) = 1e-4): mpmath's adaptive integrator over y of the plain
+    difference D1(y) [ <D2(u)> - <D2(y)> ], the angular average taken analytically,
+    int sqrt(1-z^2)/(A - B z) dz = pi (A - sqrt(A^2-B^2))/B^2.  Pins which line carries which
+    mass, the finite cutoff, and the radial map with its Jacobian."""
+    ma, mb = 1.0, 3.0
+    a, b = {"kind": "massive", "m2": ma}, {"kind": "massive", "m2": mb}
+    xs = [0.5 + 0.2j, 1.0 - 0.3j]
+
+    def direct(x, m1, m2_, lam2):
+        x = mp.mpc(x)
+
+        def f(y):
+            A = x + y + m2_
+            B2 = 4 * x * y
+            ang_u = mp.pi * (A - A * mp.sqrt(1 - B2 / (A * A))) / B2
+            ang_y = mp.pi / (2 * (y + m2_))
+            return y / (y + m1) * (ang_u - ang_y)
+        return 2 / mp.pi * mp.quad(f, [0, 1, 5, 20, lam2])
+
+    g_ab = G(oracle, xs, line_k=a, line_pk=b, cutoff2=50.0, n_rad=256)
+    g_ba = G(oracle, xs, line_k=b, line_pk=a, cutoff2=50.0, n_rad=256)
+    ref_ab = [complex(direct(x, ma, mb, 50)) for x in xs]
+    ref_ba = [complex(direct(x, mb, ma, 50)) for x in xs]
+    assert np.max(relerr(g_ab, ref_ab)) < 1e-10 and np.max(relerr(g_ba, ref_ba)) < 1e-10
+    assert np.min(relerr(g_ab, ref_ba)) > 1e-5      # the assignment matters at this cutoff
+
+
+def test_cf3_rational_line(oracle):
+    """Config 4's integrand (reading G11: line 2 rational) against the Feynman-parameter form
+    on the REAL mask Re x >= 0.25, |Im x| <= 1.25."""
+    xs = [0.5 + 0.2j, 1 + 1j, 2 - 1j, 0.3 + 0j]
+    g = G(oracle, xs, line_pk=RAT, cutoff2=1e8, n_rad=512)
+    ref = [complex(CF.cf3_rational(x, 1.0, 2.0, 0.5, 1.2)) for x in xs]
+    assert np.max(relerr(g, ref)) < 1e-10
+    # rational on line 1 instead (line swap): same G up to O(Lambda^-4)
+    g_sw = G(oracle, xs, line_k=RAT, line_pk=BUB, cutoff2=1e8, n_rad=512)
+    assert np.max(relerr(g_sw, ref)) < 1e-10
+
+
+def test_cf3_unequal_real_masses(oracle):
+    a, b = {"kind": "massive", "m2": 1.0}, {"kind": "massive", "m2": 3.0}
+    xs = [0.5 + 0.2j, 2 + 0.5j]
+    g = G(oracle, xs, line_k=a, line_pk=b, cutoff2=1e8, n_rad=512)
+    ref = [complex(CF.cf3_feynman(x, 1.0, 3.0)) for x in xs]
+    assert np.max(relerr(g, ref)) < 1e-10
+
+
+# ---------------------------------------------------------------- invariants
+def test_I1_G_of_zero_is_exactly_zero(oracle):
+    for contour in ["real", "ray_arc"]:
+        g = G(oracle, [0j], contour=contour, ang="gauss_legendre")
+        assert g[0] == 0
+    assert G(oracle, [0j], line_pk=RAT)[0] == 0
+
+
+def test_I2_conjugation_symmetry_bitwise(oracle):
+    """G(conj x) = conj G(x) bitwise for real-coefficient propagators (real tables, principal sqrt)."""
+    xs = np.array([0.5 + 0.2j, -3 + 0.5j, 2 - 4j, -7 + 1e-3j, 1e-4 + 3j])
+    for kw in [dict(), dict(line_pk=RAT), dict(contour="ray_arc"), dict(contour="auto")]:
+        g = G(oracle, xs, ang="gauss_legendre", **kw)
+        gc = G(oracle, np.conj(xs), ang="gauss_legendre", **kw)
+        assert np.array_equal(gc, np.conj(g)), kw
+
+
+def test_I2_complex_masses_swap_under_conjugation(oracle):
+    k = {"kind": "massive", "m2": 0.5j}
+    pk = {"kind": "massive", "m2": -0.5j}
+    xs = np.array([0.5 + 0.2j, 2 + 1j])
+    g = G(oracle, xs, line_k=k, line_pk=pk)
+    gc = G(oracle, np.conj(xs), line_k=pk, line_pk=k)
+    assert np.array_equal(gc, np.conj(g))
+
+
+def test_I3_cutoff_independence(oracle):
+    """BPHZ subtraction makes the result cutoff independent: error ~ Lambda^-4."""
+    x = [0.5 + 0.2j]
+    ref = complex(CF.cf1(x[0]))
+    e4 = relerr(G(oracle, x, cutoff2=1e4), [ref])[0]
+    e6 = relerr(G(oracle, x, cutoff2=1e6), [ref])[0]
+    e8 = relerr(G(oracle, x, cutoff2=1e8, n_rad=512), [ref])[0]
+    assert 1e-8 < e4 < 1e-7 and e6 < 2e-11 and e8 < 1e-12
+    assert 5e3 < e4 / max(e6, 1e-30) < 2e4 or e6 < 5e-12  # ~ (1e6/1e4)^2 = 1e4
+
+
+def test_I4_line_swap(oracle):
+    """k <-> p-k (shift invariance of eq. (4)): unequal masses, O(Lambda^-4)."""
+    a, b = {"kind": "massive", "m2": 1.0}, {"kind": "massive", "m2": 3.0}
+    xs = [0.5 + 0.2j, 1 + 1j]
+    g1 = G(oracle, xs, line_k=a, line_pk=b, cutoff2=1e8, n_rad=512)
+    g2 = G(oracle, xs, line_k=b, line_pk=a, cutoff2=1e8, n_rad=512)
+    assert np.max(relerr(g1, g2)) < 1e-11
+
+
+def test_I5_rule_independence(oracle):
+    """The paper's own check: tanh-sinh vs Gauss-Chebyshev angular integration."""
+    xs = [0.5 + 0.2j, 1 + 2j]
+    g_ch = G(oracle, xs, ang="gauss_cheb2", n_ang=128)
+    g_ts = G(oracle, xs, ang="tanh_sinh", n_ang=49)
+    g_gl = G(oracle, xs, ang="gauss_legendre", n_ang=128)
+    assert np.max(relerr(g_ts, g_ch)) < 1e-10
+    assert 1e-7 < np.max(relerr(g_gl, g_ch)) < 3e-6
+
+
+def test_I6_brute_force_high_order(oracle):
+    """2048 x 1024 Chebyshev nodes, Lambda^2 = 1e8, 8x8 grid: <= 1e-12 inside the masks."""
+    re, im = np.meshgrid(np.linspace(0.1, 2.0, 8), np.linspace(-1.0, 1.0, 8))
+    xs = (re + 1j * im).ravel()
+    g = G(oracle, xs, cutoff2=1e8, n_rad=2048, n_ang=1024)
+    ref = [complex(CF.cf1(x)) for x in xs]
+    assert np.max(relerr(g, ref)) < 1e-12
+
+
+def test_accum_variants_agree(oracle):
+    P = oracle.make_params(BUB, BUB, 1e6)
+    rn, rw, z, wz = tables(oracle, 256, 128)
+    xs = np.array([0.5 + 0.2j, -3 + 0.5j, 2e-3 + 1e-3j])
+    g_ld, _ = oracle.eval_grid(P, rn, rw, 256, z, wz, xs, accum="long_double")
+    g_d, _ = oracle.eval_grid(P, rn, rw, 256, z, wz, xs, accum="double", n_threads=2)
+    assert np.max(relerr(g_d, g_ld)) < 1e-12
+
+
+# ---------------------------------------------------------------- contours (a3)
+def test_real_contour_fails_outside_parabola(oracle):
+    """R2: outside the parabola the REAL sum is NOT the continuation."""
+    x = [2 - 4j]
+    assert not CF.in_parabola_R2(x[0])
+    assert relerr(G(oracle, x), [complex(CF.cf1(x[0]))])[0] > 0.03
+
+
+def test_ray_arc_reaches_outside_parabola(oracle):
+    """Generalised region-2/5 contour reproduces CF1 where REAL cannot."""
+    xs = [2 - 4j, -3 + 2j, -8 + 4j, 0.5 + 0.2j, -1 + 3j, 4 + 6j]
+    g = G(oracle, xs, contour="ray_arc")
+    assert np.max(relerr(g, [complex(CF.cf1(x)) for x in xs])) < 2e-9
+
+
+def test_contour_geometry(oracle):
+    """Every policy connects 0 with Lambda^2: sum of (weight x dy/dt) = Lambda^2 (up to the
+    quadrature error of integrating dy/dt), and the node counts follow the pyramid."""
+    rn, rw = oracle.make_radial_pyramid(256)
+    for contour, x in [("real", 1 + 1j), ("ray_arc", -3 + 2j), ("thread", -6 + 0.1j), ("thread", -6 - 0.1j)]:
+        P = oracle.make_params(BUB, BUB, 1e6, contour=contour)
+        pol, y, wy = oracle.contour_nodes(P, x, rn, rw, 256, 128)
+        assert y.size == 256
+        assert abs(np.sum(wy) - 1e6) / 1e6 < 1e-9
+    P = oracle.make_params(BUB, BUB, 1e6, contour="ray_arc")
+    _, y, _ = oracle.contour_nodes(P, -3 + 2j, rn, rw, 256, 128)
+    assert np.allclose(np.angle(y[:128]), np.angle(-3 + 2j))        # the ray
+    assert np.allclose(np.abs(y[128:192]), np.abs(y[128]))          # the arc
+    assert np.all(y[192:].imag == 0) and y[-1].real < 1e6           # the real tail
+
+
+def test_auto_policy_regions(oracle):
+    rn, rw = oracle.make_radial_pyramid(64)
+    P = oracle.make_params(BUB, BUB, 1e6, contour="auto")
+    pol = lambda x: oracle.contour_nodes(P, x, rn, rw, 64, 128)[0]
+    assert pol(1 + 1j) == 1 and pol(-3 + 2j) == 1        # RAY_ARC outside the wedge
+    assert pol(-6 + 0.01j) == 2 and pol(-6 - 0.01j) == 2  # THREAD near the cut
+    assert pol(-3 + 0.01j) == 0                           # REAL in the strip -4.1 < Re x < -1
+    assert pol(-0.5 + 0.001j) == 1                        # Re x >= -m^2: not in the wedge
+
+
+def test_thread_contour_and_discontinuity(oracle):
+    """Analogue of the paper's region-3/4 polylines.  Moderately close to the
+    cut it matches CF1; very close it reproduces the discontinuity -2 pi i sqrt(1-4/s) within 20%."""
+    g = G(oracle, [-6 + 1j, -8 + 0.5j], contour="thread", n_rad=1024, n_ang=512, ang="gauss_legendre")
+    ref = [complex(CF.cf1(-6 + 1j)), complex(CF.cf1(-8 + 0.5j))]
+    assert np.max(relerr(g, ref)) < 1e-4
+    for s in [5.0, 7.0, 10.0]:
+        gp, gm = G(oracle, [-s + 1e-4j, -s - 1e-4j], contour="thread", n_rad=1024, n_ang=512,
+                   ang="gauss_legendre")
+        exact = math.pi * math.sqrt(1 - 4 / s)
+        assert gp.imag < 0 < gm.imag                       # sign of Im G opposite to sign of Im x
+        assert abs(-gp.imag / exact - 1) < 0.2 and abs(gm.imag / exact - 1) < 0.2
+    # under REAL the strip shows no cut at all
+    gp, gm = G(oracle, [-6 + 1e-4j, -6 - 1e-4j], contour="real", n_rad=1024, n_ang=512, ang="gauss_legendre")
+    assert abs(gp.imag) < 1e-2
+
+
+# ---------------------------------------------------------------- argument checks
+def test_oracle_rejects_unsupported(oracle):
+    rn, rw, z, wz = tables(oracle, 64, 32)
+    xs = np.array([1 + 1j])
+    with pytest.raises(ValueError):
+        oracle.eval_grid(oracle.make_params(BUB, BUB, 1e6, taylor_order=1), rn, rw, 64, z, wz, xs)
+    with pytest.raises(ValueError):
+        oracle.eval_grid(oracle.make_params(BUB, BUB, -1.0), rn, rw, 64, z, wz, xs)
+    with pytest.raises(ValueError):
+        oracle.eval_grid(oracle.make_params(BUB, RAT, 1e6, contour="thread"), rn, rw, 64, z, wz, xs)
+    g, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e6), rn, rw, 64, z, wz, np.zeros(0, dtype=complex))
+    assert g.size == 0
