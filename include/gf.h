@@ -1,0 +1,166 @@
+/* gf.h -- C ABI of libgf_b200: complex-plane scans of regularised one-loop integrals on B200.
+ *
+ * The data-parallel hot path of arXiv:1205.0752 (Windisch, Alkofer, Haase, Liebmann,
+ * "Examining the Analytic Structure of Green's Functions: Massive Parallel Complex Integration
+ * using GPUs"), citations are lines of the paper text PAPER.md:
+ *
+ *   for every point x = p^2 of a grid in the complex plane (Step 4) evaluate
+ *
+ *     G(x) = c0 * int_C dy y  int_-1^1 dz sqrt(1-z^2)  F_sub(x, y, sqrt(x) sqrt(y) z)     eq. (14)/(15)
+ *
+ *   by non-adaptive quadrature (Step 5), where F = D1(y) D2(u),
+ *   u = x + y - 2 sqrt(x) sqrt(y) z = (p-k)^2 (eq. (10),(19)), and F_sub = (1 - t^0) F is the
+ *   BPHZ-like Taylor-subtracted integrand (eq. (12),(13),(20)).  Every grid point is independent.
+ *
+ * Conventions
+ *   - All entry points are extern "C", return a gf_status, and never throw.
+ *   - "d_" arguments are DEVICE pointers (CUDA global memory of the current device), "h_"
+ *     arguments are HOST pointers.  `stream` is a cudaStream_t passed as void* (NULL = the
+ *     legacy default stream).  Unless stated otherwise a call only ENQUEUES work on `stream`
+ *     and returns; the caller synchronises.
+ *   - Ownership: the caller owns every buffer.  The library keeps no device memory between
+ *     calls and frees nothing it did not allocate inside the same call.
+ *   - Complex arrays are interleaved (re, im) pairs: complex<double> = 2 doubles (16 bytes,
+ *     16-byte aligned), complex<float> = 2 floats (8 bytes, 8-byte aligned).
+ *   - Grids are stored [n_im][n_re], the real index fastest (the paper's X(M,N) with M along
+ *     the real axis, Fortran order).
+ *   - Errors: GF_ERR_NULL for a null pointer, GF_ERR_ARG for a value out of range,
+ *     GF_ERR_UNSUPPORTED for a combination the method does not define (taylor_order != 0, a
+ *     subtraction point other than 0, the THREAD contour with unequal or complex masses, a
+ *     rational propagator with a double pole), GF_ERR_CUDA when the CUDA runtime reports an
+ *     error (no device, launch failure).  gf_last_error() describes the last failure of the
+ *     calling thread.  A denominator that vanishes at a quadrature node yields IEEE inf/NaN in
+ *     that output entry, not an error (the paper has no convention).
+ */
+#ifndef GF_B200_H_
+#define GF_B200_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { GF_OK = 0, GF_ERR_NULL = 1, GF_ERR_ARG = 2, GF_ERR_UNSUPPORTED = 3, GF_ERR_CUDA = 4 } gf_status;
+
+/* Quadrature rules on [-1,1]: Gauss-Legendre (the paper's radial rule, and the
+ * angular rule of BASELINE.json's configs), Gauss-Chebyshev of the 2nd kind (the paper's check
+ * rule; the exact Gauss rule for the d=4 angular measure), tanh-sinh (the paper's angular rule). */
+typedef enum { GF_QUAD_GAUSS_LEGENDRE = 0, GF_QUAD_GAUSS_CHEB2 = 1, GF_QUAD_TANH_SINH = 2 } gf_quad_kind;
+
+/* Which measure the returned weights integrate against: dz (radial rules), or the d=4
+ * hyperspherical angular measure sqrt(1-z^2) dz of eq. (9)/(11). */
+typedef enum { GF_MEASURE_PLAIN = 0, GF_MEASURE_SQRT1MZ2 = 1 } gf_measure;
+
+/* Propagators.  MASSIVE: 1/(u + m2), m2 complex (the paper's example uses m2 = +-i/2, eq. (19)).
+ * RATIONAL: (u + M2)/(u^2 + a u + b) with real M2, a, b (BASELINE.json config 4). */
+typedef enum { GF_PROP_MASSIVE = 0, GF_PROP_RATIONAL = 1 } gf_prop_kind;
+typedef struct {
+  int kind;            /* gf_prop_kind */
+  double m2_re, m2_im; /* MASSIVE */
+  double M2, a, b;     /* RATIONAL */
+} gf_propagator;
+
+/* Radial contour C of eq. (15) (Step 3), chosen per grid point inside the
+ * evaluation kernel like the IF-THEN-ELSE of the paper's Kernel 2:
+ *   REAL     the positive real axis [0, Lambda^2] of eq. (14);
+ *   RAY_ARC  ray along arg x, arc back to the real axis, real tail (generalises the paper's
+ *            region-2/5 contour);
+ *   THREAD   polyline through the opening of the cut for Re x < -4 m^2 next to the negative
+ *            axis, equal real masses only (analogue of the region-3/4 contours);
+ *   AUTO     per-point choice among the three. */
+typedef enum { GF_CONTOUR_REAL = 0, GF_CONTOUR_RAY_ARC = 1, GF_CONTOUR_THREAD = 2, GF_CONTOUR_AUTO = 3 } gf_contour;
+
+typedef enum { GF_SPACING_UNIFORM = 0, GF_SPACING_LOG_ABS_IM = 1 } gf_spacing;
+
+typedef struct {
+  gf_propagator line_k;  /* D1(y): the line carrying k      (eq. (19)) */
+  gf_propagator line_pk; /* D2(u): the line carrying p - k */
+  double cutoff2;        /* Lambda^2 > 0, upper limit of the radial integral */
+  double sub_re, sub_im; /* subtraction point x0 of t^n; only 0 is supported (eq. (13)) */
+  int taylor_order;      /* n of t^n; only 0 is supported (log-divergent integrals) */
+  double prefactor;      /* c0; 1/(2 pi)^3 is eq. (14), 2/pi the rescaled eq. (21) */
+  double map_scale;      /* s0 > 0 of the shifted-log radial map y(u) = a + (a+s0) expm1(u L) */
+  int contour;           /* gf_contour */
+  int precision;         /* 64: complex<double> output (the contract); 32: the FP32 comparison
+                            variant, complex<float> output */
+} gf_params;
+
+/* Step 4 / Kernel 1: fill d_x[n_im][n_re] (complex<double>) with the
+ * homogeneous, endpoint-inclusive distribution of points over [re_min,re_max] x [im_min,im_max].
+ * Each axis is two-sided: v_i = min + i*d for 2i <= n-1 and max - (n-1-i)*d above, d = (max-min)/(n-1),
+ * each with one fused multiply-add, so a range symmetric about 0 is mirrored exactly.  n = 1 gives min.
+ * GF_SPACING_LOG_ABS_IM (n_im even, im_min == -im_max, 0 < im_abs_min < im_max): |Im x| takes n_im/2
+ * log-spaced values from im_abs_min to im_max on each side of the real axis, ascending in Im x.
+ * Asynchronous on `stream`. */
+int gf_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
+                 int spacing, double im_abs_min, void* d_x, void* stream);
+
+/* "Preparation": nodes t_i in (-1,1), ascending, and weights of an n-point rule
+ * into caller-allocated DEVICE arrays of n doubles each.  Tables are computed on the host in extended
+ * precision (as in the paper) and copied with cudaMemcpyAsync on `stream`; the host staging copy is
+ * complete on return.  `step` is the tanh-sinh step h (0 = default 2.9/((n-1)/2)); ignored otherwise.
+ * `measure` is a gf_measure.  Rules are exactly symmetric: t[n-1-i] == -t[i], w[n-1-i] == w[i]. */
+int gf_make_quadrature(int kind, int n, double step, int measure, double* d_nodes, double* d_weights,
+                       void* stream);
+
+/* The same tables into HOST arrays (no CUDA call is made). */
+int gf_make_quadrature_host(int kind, int n, double step, int measure, double* h_nodes, double* h_weights);
+
+/* Doubles needed for the radial tables of a contour policy: n_rad for REAL; for the other policies
+ * the pyramid n_rad + n_rad/2 + n_rad/4 + n_rad/8 (rules of those orders back to back -- the paper's
+ * "n arrays for the radial nodes"), which requires n_rad % 8 == 0.  Returns -1 on error. */
+long long gf_radial_table_size(int contour, int n_rad);
+
+/* Step 5 / Kernel 2: G at every point of d_x.
+ *   d_rad_nodes/d_rad_weights  radial rule(s), measure PLAIN, gf_radial_table_size() doubles each;
+ *                              nodes strictly inside (-1,1)
+ *   d_ang_nodes/d_ang_weights  angular rule of n_ang nodes whose weights include the measure
+ *                              sqrt(1-z^2) (GF_MEASURE_SQRT1MZ2).  The rule must be symmetric
+ *                              (z[n-1-j] = -z[j], equal weights): the kernel folds +-z pairs.  A rule
+ *                              that is not makes every output NaN.
+ *   d_x      n_points complex<double>
+ *   d_out    n_points complex<double> (precision 64) or complex<float> (precision 32)
+ * Domain: x = 0 gives exactly 0; |x| up to 1e100.  Asynchronous on `stream`; n_points = 0 is a no-op. */
+int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                 const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
+                 long long n_points, void* d_out, void* stream);
+
+/* The same call on HOST buffers (the end-to-end path): allocates device scratch on `stream`, copies
+ * tables and x host->device, runs the kernels, copies the result device->host and synchronises
+ * `stream` before returning.  Pinned host memory makes the copies asynchronous but is not required. */
+int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const double* h_rad_weights, int n_rad,
+                      const double* h_ang_nodes, const double* h_ang_weights, int n_ang, const void* h_x,
+                      long long n_points, void* h_out, void* stream);
+
+/* How gf_eval_grid would launch, and its arithmetic per launch (for benchmarks and roofline numbers;
+ * makes no CUDA call).  fp64_inst / fp32_inst are executed warp-level-uniform per-thread instruction
+ * counts of the evaluation kernel summed over all threads (DFMA, DMUL and DADD each count 1), flops
+ * counts an FMA as 2; both follow the SASS of the inner loop and the per-node set-up. */
+typedef struct {
+  int block_threads;      /* threads per CTA */
+  long long grid_blocks;  /* CTAs */
+  int split;              /* lanes sharing one grid point (radial nodes dealt round-robin) */
+  int smem_bytes;         /* dynamic shared memory per CTA */
+  int n_pairs;            /* folded angular nodes: ceil(n_ang/2) */
+  int n_terms;            /* simple-pole terms of line 2 (1 massive, 2 rational) */
+  double fp64_inst;       /* FP64-pipe thread-instructions per launch */
+  double fp32_inst;       /* FP32-pipe thread-instructions of the inner loop (precision 32) */
+  double flops;           /* floating-point operations per launch */
+  double evals;           /* nominal integrand evaluations: n_points * n_rad * n_ang */
+} gf_launch_info;
+int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_points, gf_launch_info* out);
+
+/* Diagnostics used by bench.py to measure the denominators it reports against (not on the hot path).
+ * gf_diag_fp64_peak: enqueue a kernel of `blocks` x `threads` threads, each running `iters` rounds of 8
+ *   independent DFMA chains (16*iters flops per thread per round... see DESIGN.md); writes one double
+ *   per thread to d_sink (blocks*threads doubles) so the work cannot be removed.
+ * gf_diag_rcp_seed: for n doubles in d_in, writes the raw MUFU.RCP64H seed to d_out. */
+int gf_diag_fp64_peak(int blocks, int threads, long long iters, double* d_sink, void* stream);
+int gf_diag_rcp_seed(const double* d_in, double* d_out, long long n, void* stream);
+
+const char* gf_last_error(void);
+const char* gf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GF_B200_H_ */

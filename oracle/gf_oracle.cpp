@@ -47,7 +47,7 @@ namespace {
 typedef std::complex<double> cplx;
 typedef long double ld;
 
-const double kPi = 3.14159265358979323846264338327950288;
+const long double kPi = 3.14159265358979323846264338327950288L;
 
 // ---- enums (values are part of the oracle's own C interface) -------------
 enum { QUAD_GAUSS_LEGENDRE = 0, QUAD_GAUSS_CHEB2 = 1, QUAD_TANH_SINH = 2 };
@@ -316,7 +316,7 @@ void contour_thread(const Params& P, cplx x, const double* rn, const double* rw,
   W[3] = cplx(-0.5 * (Aa + r0), -0.5 * (r0 - Aa));
   W[4] = r0 * e;
   double Rad = std::fmin(1.5 * Bb, 0.5 * P.cutoff2);
-  double th5 = 0.75 * kPi;
+  double th5 = (double)(0.75L * kPi);
   W[5] = Rad * cplx(std::cos(th5), std::sin(th5));
   size_t first = out.size();
   for (int k = 0; k < 5; ++k) seg_line(W[k], W[k + 1], level(rn, rw, n_rad, 3), out);

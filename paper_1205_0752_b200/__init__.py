@@ -1,0 +1,252 @@
+"""paper_1205_0752_b200 -- thin Python binding of libgf_b200 (include/gf.h).
+
+Argument marshalling only: every step of the hot path (grid fill, evaluation of the double integral,
+reductions, stores) runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and
+streams.  There is no CPU fallback: if the shared library is missing, importing works but the first
+call raises; if no CUDA device is present the library returns GF_ERR_CUDA and the call raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libgf_b200.so")
+
+QUAD = {"gauss_legendre": 0, "gauss_cheb2": 1, "tanh_sinh": 2}
+MEASURE = {"plain": 0, "sqrt1mz2": 1}
+PROP = {"massive": 0, "rational": 1}
+CONTOUR = {"real": 0, "ray_arc": 1, "thread": 2, "auto": 3}
+SPACING = {"uniform": 0, "log_abs_im": 1}
+STATUS = {0: "GF_OK", 1: "GF_ERR_NULL", 2: "GF_ERR_ARG", 3: "GF_ERR_UNSUPPORTED", 4: "GF_ERR_CUDA"}
+
+
+class GfError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("%s: %s" % (STATUS.get(status, status), message))
+        self.status = status
+
+
+class gf_propagator(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int), ("m2_re", ctypes.c_double), ("m2_im", ctypes.c_double),
+                ("M2", ctypes.c_double), ("a", ctypes.c_double), ("b", ctypes.c_double)]
+
+
+class gf_params(ctypes.Structure):
+    _fields_ = [("line_k", gf_propagator), ("line_pk", gf_propagator), ("cutoff2", ctypes.c_double),
+                ("sub_re", ctypes.c_double), ("sub_im", ctypes.c_double), ("taylor_order", ctypes.c_int),
+                ("prefactor", ctypes.c_double), ("map_scale", ctypes.c_double), ("contour", ctypes.c_int),
+                ("precision", ctypes.c_int)]
+
+
+class gf_launch_info(ctypes.Structure):
+    _fields_ = [("block_threads", ctypes.c_int), ("grid_blocks", ctypes.c_longlong), ("split", ctypes.c_int),
+                ("smem_bytes", ctypes.c_int), ("n_pairs", ctypes.c_int), ("n_terms", ctypes.c_int),
+                ("fp64_inst", ctypes.c_double), ("fp32_inst", ctypes.c_double), ("flops", ctypes.c_double),
+                ("evals", ctypes.c_double)]
+
+
+_lib = None
+_vp, _dbl, _int, _ll = ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.c_longlong
+_SIGNATURES = {
+    "gf_make_grid": [_dbl, _dbl, _int, _dbl, _dbl, _int, _int, _dbl, _vp, _vp],
+    "gf_make_quadrature": [_int, _int, _dbl, _int, _vp, _vp, _vp],
+    "gf_make_quadrature_host": [_int, _int, _dbl, _int, _vp, _vp],
+    "gf_radial_table_size": [_int, _int],
+    "gf_eval_grid": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
+    "gf_eval_grid_host": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
+    "gf_eval_launch_info": [ctypes.POINTER(gf_params), _int, _int, _ll, ctypes.POINTER(gf_launch_info)],
+    "gf_diag_fp64_peak": [_int, _int, _ll, _vp, _vp],
+    "gf_diag_rcp_seed": [_vp, _vp, _ll, _vp],
+    "gf_last_error": [],
+    "gf_version": [],
+}
+
+
+def lib():
+    """The loaded C-ABI library.  Raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libgf_b200.so is missing: run `python -m paper_1205_0752_b200.build` "
+                               "(nvcc, sm_100a).  There is no CPU fallback.")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, args in _SIGNATURES.items():
+            f = getattr(L, name)
+            f.argtypes = args
+            f.restype = _int
+        L.gf_radial_table_size.restype = _ll
+        L.gf_last_error.restype = ctypes.c_char_p
+        L.gf_version.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise GfError(rc, lib().gf_last_error().decode())
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def _device(device):
+    if not torch.cuda.is_available():
+        raise GfError(4, "no CUDA device: the hot path runs only in the sm_100a kernels (no CPU fallback)")
+    return torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+
+
+def _prop(d):
+    p = gf_propagator()
+    p.kind = PROP[d["kind"]]
+    m2 = complex(d.get("m2", 0.0))
+    p.m2_re, p.m2_im = m2.real, m2.imag
+    p.M2, p.a, p.b = float(d.get("M2", 0.0)), float(d.get("a", 0.0)), float(d.get("b", 0.0))
+    return p
+
+
+def make_params(line_k, line_pk, cutoff2, prefactor=2.0 / np.pi, map_scale=1.0, contour="real", sub=0.0,
+                taylor_order=0, precision=64):
+    """gf_params from plain Python values.  Propagators: {'kind': 'massive', 'm2': complex} or
+    {'kind': 'rational', 'M2': .., 'a': .., 'b': ..}."""
+    P = gf_params()
+    P.line_k, P.line_pk = _prop(line_k), _prop(line_pk)
+    P.cutoff2 = float(cutoff2)
+    s = complex(sub)
+    P.sub_re, P.sub_im = s.real, s.imag
+    P.taylor_order = int(taylor_order)
+    P.prefactor = float(prefactor)
+    P.map_scale = float(map_scale)
+    P.contour = CONTOUR[contour] if isinstance(contour, str) else int(contour)
+    P.precision = int(precision)
+    return P
+
+
+def make_grid(re_min, re_max, n_re, im_min, im_max, n_im, spacing="uniform", im_abs_min=0.0, device=None,
+              stream=None, out=None):
+    """gf_make_grid: complex128 tensor [n_im, n_re] on the device."""
+    dev = _device(device)
+    x = out if out is not None else torch.empty((n_im, n_re), dtype=torch.complex128, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib().gf_make_grid(re_min, re_max, n_re, im_min, im_max, n_im, SPACING[spacing], im_abs_min,
+                                  x.data_ptr(), _stream(stream)))
+    return x
+
+
+def make_quadrature(kind, n, step=0.0, measure="plain", device=None, stream=None):
+    """gf_make_quadrature: (nodes, weights) float64 tensors on the device."""
+    dev = _device(device)
+    nodes = torch.empty(n, dtype=torch.float64, device=dev)
+    weights = torch.empty(n, dtype=torch.float64, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib().gf_make_quadrature(QUAD[kind], n, step, MEASURE[measure], nodes.data_ptr(),
+                                        weights.data_ptr(), _stream(stream)))
+    return nodes, weights
+
+
+def make_quadrature_host(kind, n, step=0.0, measure="plain"):
+    """gf_make_quadrature_host: (nodes, weights) numpy arrays (no CUDA call)."""
+    nodes = np.empty(n, dtype=np.float64)
+    weights = np.empty(n, dtype=np.float64)
+    _check(lib().gf_make_quadrature_host(QUAD[kind], n, step, MEASURE[measure], nodes.ctypes.data,
+                                         weights.ctypes.data))
+    return nodes, weights
+
+
+def radial_table_size(contour, n_rad):
+    c = CONTOUR[contour] if isinstance(contour, str) else int(contour)
+    return int(lib().gf_radial_table_size(c, n_rad))
+
+
+def _levels(contour, n_rad):
+    size = radial_table_size(contour, n_rad)
+    if size < 0:
+        raise GfError(2, "bad contour / n_rad (deformed contours need n_rad % 8 == 0)")
+    return [n_rad] if size == n_rad else [n_rad, n_rad // 2, n_rad // 4, n_rad // 8]
+
+
+def make_radial_tables(contour, n_rad, kind="gauss_legendre", device=None, stream=None):
+    """The radial rule(s) gf_eval_grid expects for `contour`: one gf_make_quadrature call per level."""
+    dev = _device(device)
+    levels = _levels(contour, n_rad)
+    nodes = torch.empty(sum(levels), dtype=torch.float64, device=dev)
+    weights = torch.empty(sum(levels), dtype=torch.float64, device=dev)
+    off = 0
+    with torch.cuda.device(dev):
+        for n in levels:
+            _check(lib().gf_make_quadrature(QUAD[kind], n, 0.0, MEASURE["plain"], nodes[off:].data_ptr(),
+                                            weights[off:].data_ptr(), _stream(stream)))
+            off += n
+    return nodes, weights
+
+
+def make_radial_tables_host(contour, n_rad, kind="gauss_legendre"):
+    xs, ws = zip(*[make_quadrature_host(kind, n) for n in _levels(contour, n_rad)])
+    return np.concatenate(xs), np.concatenate(ws)
+
+
+def eval_grid(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out=None, stream=None):
+    """gf_eval_grid on device tensors.  x: complex128, any shape; returns complex128 (precision 64) or
+    complex64 (precision 32) of the same shape.  Asynchronous on the current stream."""
+    if not x.is_cuda:
+        raise GfError(2, "eval_grid takes device tensors; use eval_grid_host for host buffers")
+    assert x.dtype == torch.complex128 and x.is_contiguous()
+    for t in (rad_nodes, rad_weights, ang_nodes, ang_weights):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+    assert ang_nodes.numel() == ang_weights.numel()
+    need = radial_table_size(params.contour, n_rad)
+    assert rad_nodes.numel() >= need and rad_weights.numel() >= need, "radial tables too short for this contour"
+    odt = torch.complex64 if params.precision == 32 else torch.complex128
+    if out is None:
+        out = torch.empty(x.shape, dtype=odt, device=x.device)
+    assert out.dtype == odt and out.is_contiguous() and out.numel() == x.numel()
+    with torch.cuda.device(x.device):
+        _check(lib().gf_eval_grid(ctypes.byref(params), rad_nodes.data_ptr(), rad_weights.data_ptr(), n_rad,
+                                  ang_nodes.data_ptr(), ang_weights.data_ptr(), ang_nodes.numel(),
+                                  x.data_ptr(), x.numel(), out.data_ptr(), _stream(stream)))
+    return out
+
+
+def _host_ptr(a):
+    if isinstance(a, torch.Tensor):
+        assert not a.is_cuda and a.is_contiguous()
+        return a.data_ptr()
+    assert a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data
+
+
+def eval_grid_host(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out, stream=None):
+    """gf_eval_grid_host: every buffer is HOST memory (numpy arrays or CPU torch tensors, ideally pinned);
+    host<->device copies happen inside the call, which returns after `out` is complete."""
+    if not torch.cuda.is_available():
+        raise GfError(4, "no CUDA device (no CPU fallback)")
+    n_ang = int(ang_nodes.shape[0])
+    n_points = int(np.prod(x.shape))
+    _check(lib().gf_eval_grid_host(ctypes.byref(params), _host_ptr(rad_nodes), _host_ptr(rad_weights), n_rad,
+                                   _host_ptr(ang_nodes), _host_ptr(ang_weights), n_ang, _host_ptr(x),
+                                   n_points, _host_ptr(out), _stream(stream)))
+    return out
+
+
+def launch_info(params, n_rad, n_ang, n_points):
+    info = gf_launch_info()
+    _check(lib().gf_eval_launch_info(ctypes.byref(params), n_rad, n_ang, n_points, ctypes.byref(info)))
+    return {k: getattr(info, k) for k, _ in gf_launch_info._fields_}
+
+
+def diag_fp64_peak(blocks, threads, iters, sink, stream=None):
+    _check(lib().gf_diag_fp64_peak(blocks, threads, iters, sink.data_ptr(), _stream(stream)))
+
+
+def diag_rcp_seed(x, stream=None):
+    out = torch.empty_like(x)
+    _check(lib().gf_diag_rcp_seed(x.data_ptr(), out.data_ptr(), x.numel(), _stream(stream)))
+    return out
+
+
+def version():
+    return lib().gf_version().decode()

@@ -1,0 +1,250 @@
+// gf_api.cu -- the C ABI of include/gf.h: argument validation, host-side preparation (pole
+// decomposition of line 2, launch plan) and kernel launches.  No torch types, no exceptions.
+#include <cmath>
+#include <complex>
+#include <cstdarg>
+#include <cstdio>
+#include <vector>
+
+#include "gf_internal.h"
+
+namespace gf {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+int check_cuda(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return GF_OK;
+  set_error("%s: %s", what, cudaGetErrorString(e));
+  return GF_ERR_CUDA;
+}
+
+namespace {
+
+bool finite_prop(const gf_propagator& p) {
+  return std::isfinite(p.m2_re) && std::isfinite(p.m2_im) && std::isfinite(p.M2) && std::isfinite(p.a) &&
+         std::isfinite(p.b);
+}
+
+int check_prop(const gf_propagator& p, const char* name) {
+  if (p.kind != GF_PROP_MASSIVE && p.kind != GF_PROP_RATIONAL) {
+    set_error("%s: unknown propagator kind %d", name, p.kind);
+    return GF_ERR_ARG;
+  }
+  if (!finite_prop(p)) { set_error("%s: non-finite propagator parameter", name); return GF_ERR_ARG; }
+  return GF_OK;
+}
+
+// validate everything that does not need a pointer, and build the kernel arguments
+int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, EvalArgs* a) {
+  if (!p) { set_error("eval_grid: params is null"); return GF_ERR_NULL; }
+  int rc;
+  if ((rc = check_prop(p->line_k, "line_k"))) return rc;
+  if ((rc = check_prop(p->line_pk, "line_pk"))) return rc;
+  if (n_rad < 1 || n_ang < 1) { set_error("eval_grid: n_rad=%d, n_ang=%d must be >= 1", n_rad, n_ang); return GF_ERR_ARG; }
+  if (n_points < 0) { set_error("eval_grid: n_points < 0"); return GF_ERR_ARG; }
+  if (!(p->cutoff2 > 0) || !std::isfinite(p->cutoff2)) { set_error("eval_grid: cutoff2 must be > 0"); return GF_ERR_ARG; }
+  if (!(p->map_scale > 0) || !std::isfinite(p->map_scale)) { set_error("eval_grid: map_scale must be > 0"); return GF_ERR_ARG; }
+  if (!std::isfinite(p->prefactor)) { set_error("eval_grid: prefactor not finite"); return GF_ERR_ARG; }
+  if (p->precision != 64 && p->precision != 32) { set_error("eval_grid: precision must be 64 or 32"); return GF_ERR_ARG; }
+  if (p->contour < GF_CONTOUR_REAL || p->contour > GF_CONTOUR_AUTO) { set_error("eval_grid: unknown contour %d", p->contour); return GF_ERR_ARG; }
+  if (p->taylor_order != 0) { set_error("eval_grid: taylor_order %d unsupported (only t^0, eq. (13))", p->taylor_order); return GF_ERR_UNSUPPORTED; }
+  if (p->sub_re != 0 || p->sub_im != 0) { set_error("eval_grid: subtraction point must be 0 (eq. (13))"); return GF_ERR_UNSUPPORTED; }
+  if (p->contour != GF_CONTOUR_REAL && n_rad % 8 != 0) { set_error("eval_grid: deformed contours need n_rad %% 8 == 0"); return GF_ERR_ARG; }
+
+  *a = EvalArgs{};
+  a->n_points = n_points;
+  a->n_rad = n_rad;
+  a->n_ang = n_ang;
+  a->n_pairs = (n_ang + 1) / 2;
+  a->line_k = p->line_k;
+  a->cutoff2 = p->cutoff2;
+  a->s0 = p->map_scale;
+  a->c0 = p->prefactor;
+  a->contour = p->contour;
+
+  // line 2 as a sum of simple poles R_r/(u + mu_r)
+  const gf_propagator& q = p->line_pk;
+  if (q.kind == GF_PROP_MASSIVE) {
+    a->n_terms = 1;
+    a->term[0] = PoleTerm{1.0, 0.0, q.m2_re, q.m2_im};
+    a->line2_scale = std::hypot(q.m2_re, q.m2_im);
+  } else {
+    const double disc = q.a * q.a - 4.0 * q.b;
+    if (disc == 0.0) {
+      set_error("line_pk: rational propagator with a double pole (a^2 = 4b) is unsupported");
+      return GF_ERR_UNSUPPORTED;
+    }
+    typedef std::complex<double> C;
+    const C sq = std::sqrt(C(disc, 0.0));
+    const C u1 = 0.5 * (-q.a + sq), u2 = 0.5 * (-q.a - sq);
+    const C R1 = (u1 + q.M2) / (u1 - u2), R2 = (u2 + q.M2) / (u2 - u1);
+    a->n_terms = 2;
+    a->term[0] = PoleTerm{R1.real(), R1.imag(), -u1.real(), -u1.imag()};
+    a->term[1] = PoleTerm{R2.real(), R2.imag(), -u2.real(), -u2.imag()};
+    a->line2_scale = std::fmax(std::abs(u1), std::abs(u2));
+  }
+  a->thread_ok = p->line_k.kind == GF_PROP_MASSIVE && q.kind == GF_PROP_MASSIVE && p->line_k.m2_im == 0 &&
+                 q.m2_im == 0 && p->line_k.m2_re == q.m2_re && q.m2_re > 0;
+  if (p->contour == GF_CONTOUR_THREAD && !a->thread_ok) {
+    set_error("eval_grid: the THREAD contour needs equal real positive masses on both lines");
+    return GF_ERR_UNSUPPORTED;
+  }
+  return GF_OK;
+}
+
+long long radial_table_size(int contour, int n_rad) {
+  if (n_rad < 1) return -1;
+  if (contour == GF_CONTOUR_REAL) return n_rad;
+  if (contour < GF_CONTOUR_REAL || contour > GF_CONTOUR_AUTO || n_rad % 8 != 0) return -1;
+  return (long long)n_rad + n_rad / 2 + n_rad / 4 + n_rad / 8;
+}
+
+}  // namespace
+}  // namespace gf
+
+using namespace gf;
+
+extern "C" {
+
+const char* gf_last_error(void) { return g_err; }
+const char* gf_version(void) { return "gf_b200 0.1 (sm_100a)"; }
+
+int gf_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im, int spacing,
+                 double im_abs_min, void* d_x, void* stream) {
+  if (!d_x) { set_error("make_grid: d_x is null"); return GF_ERR_NULL; }
+  if (n_re < 1 || n_im < 1) { set_error("make_grid: n_re=%d, n_im=%d must be >= 1", n_re, n_im); return GF_ERR_ARG; }
+  if (!std::isfinite(re_min) || !std::isfinite(re_max) || !std::isfinite(im_min) || !std::isfinite(im_max)) {
+    set_error("make_grid: non-finite box");
+    return GF_ERR_ARG;
+  }
+  if (spacing == GF_SPACING_LOG_ABS_IM) {
+    if (n_im % 2 != 0 || !(im_abs_min > 0) || !(im_max > im_abs_min) || im_min != -im_max) {
+      set_error("make_grid: LOG_ABS_IM needs n_im even, im_min == -im_max, 0 < im_abs_min < im_max");
+      return GF_ERR_ARG;
+    }
+  } else if (spacing != GF_SPACING_UNIFORM) {
+    set_error("make_grid: unknown spacing %d", spacing);
+    return GF_ERR_ARG;
+  }
+  return launch_make_grid(re_min, re_max, n_re, im_min, im_max, n_im, spacing, im_abs_min,
+                          static_cast<double2*>(d_x), static_cast<cudaStream_t>(stream));
+}
+
+int gf_make_quadrature_host(int kind, int n, double step, int measure, double* h_nodes, double* h_weights) {
+  return make_rule_host(kind, n, step, measure, h_nodes, h_weights);
+}
+
+int gf_make_quadrature(int kind, int n, double step, int measure, double* d_nodes, double* d_weights, void* stream) {
+  if (!d_nodes || !d_weights) { set_error("make_quadrature: null device pointer"); return GF_ERR_NULL; }
+  if (n < 1 || n > (1 << 20)) { set_error("make_quadrature: n=%d out of range", n); return GF_ERR_ARG; }
+  std::vector<double> x(n), w(n);
+  int rc = make_rule_host(kind, n, step, measure, x.data(), w.data());
+  if (rc) return rc;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  // pageable source: the runtime stages the data before returning, so x, w may go out of scope
+  if ((rc = check_cuda(cudaMemcpyAsync(d_nodes, x.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy nodes"))) return rc;
+  return check_cuda(cudaMemcpyAsync(d_weights, w.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy weights");
+}
+
+long long gf_radial_table_size(int contour, int n_rad) { return radial_table_size(contour, n_rad); }
+
+int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                 const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
+                 long long n_points, void* d_out, void* stream) {
+  EvalArgs a;
+  int rc = build_args(p, n_rad, n_ang, n_points, &a);
+  if (rc) return rc;
+  if (!d_rad_nodes || !d_rad_weights || !d_ang_nodes || !d_ang_weights) { set_error("eval_grid: null table pointer"); return GF_ERR_NULL; }
+  if (n_points > 0 && (!d_x || !d_out)) { set_error("eval_grid: null grid/output pointer"); return GF_ERR_NULL; }
+  a.rad_nodes = d_rad_nodes;
+  a.rad_weights = d_rad_weights;
+  a.ang_nodes = d_ang_nodes;
+  a.ang_weights = d_ang_weights;
+  a.x = static_cast<const double2*>(d_x);
+  a.out = d_out;
+  return launch_eval(a, p->precision, static_cast<cudaStream_t>(stream));
+}
+
+int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const double* h_rad_weights, int n_rad,
+                      const double* h_ang_nodes, const double* h_ang_weights, int n_ang, const void* h_x,
+                      long long n_points, void* h_out, void* stream) {
+  EvalArgs a;
+  int rc = build_args(p, n_rad, n_ang, n_points, &a);
+  if (rc) return rc;
+  if (!h_rad_nodes || !h_rad_weights || !h_ang_nodes || !h_ang_weights) { set_error("eval_grid_host: null table pointer"); return GF_ERR_NULL; }
+  if (n_points > 0 && (!h_x || !h_out)) { set_error("eval_grid_host: null grid/output pointer"); return GF_ERR_NULL; }
+  if (n_points == 0) return GF_OK;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const size_t n_radtab = (size_t)radial_table_size(p->contour, n_rad);
+  const size_t out_elem = p->precision == 32 ? 8 : 16;
+  const size_t tab_bytes = (2 * n_radtab + 2 * (size_t)n_ang) * sizeof(double);
+  const size_t x_bytes = (size_t)n_points * 16, out_bytes = (size_t)n_points * out_elem;
+  // one scratch allocation: [tables | x | out], each part 256-byte aligned
+  auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+  const size_t off_x = up(tab_bytes), off_out = off_x + up(x_bytes), total = off_out + up(out_bytes);
+  unsigned char* d = nullptr;
+  if ((rc = check_cuda(cudaMallocAsync(reinterpret_cast<void**>(&d), total, s), "cudaMallocAsync(scratch)"))) return rc;
+  double* d_tab = reinterpret_cast<double*>(d);
+  double* d_rn = d_tab;
+  double* d_rw = d_rn + n_radtab;
+  double* d_an = d_rw + n_radtab;
+  double* d_aw = d_an + n_ang;
+  cudaError_t e = cudaSuccess;
+  auto cp = [&](void* dst, const void* src, size_t n, cudaMemcpyKind k) { if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, n, k, s); };
+  cp(d_rn, h_rad_nodes, n_radtab * 8, cudaMemcpyHostToDevice);
+  cp(d_rw, h_rad_weights, n_radtab * 8, cudaMemcpyHostToDevice);
+  cp(d_an, h_ang_nodes, (size_t)n_ang * 8, cudaMemcpyHostToDevice);
+  cp(d_aw, h_ang_weights, (size_t)n_ang * 8, cudaMemcpyHostToDevice);
+  cp(d + off_x, h_x, x_bytes, cudaMemcpyHostToDevice);
+  rc = check_cuda(e, "host->device copies");
+  if (!rc) {
+    a.rad_nodes = d_rn; a.rad_weights = d_rw; a.ang_nodes = d_an; a.ang_weights = d_aw;
+    a.x = reinterpret_cast<const double2*>(d + off_x);
+    a.out = d + off_out;
+    rc = launch_eval(a, p->precision, s);
+  }
+  if (!rc) rc = check_cuda(cudaMemcpyAsync(h_out, d + off_out, out_bytes, cudaMemcpyDeviceToHost, s), "device->host copy");
+  cudaFreeAsync(d, s);
+  int rc2 = check_cuda(cudaStreamSynchronize(s), "stream synchronize");
+  return rc ? rc : rc2;
+}
+
+int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_points, gf_launch_info* out) {
+  if (!out) { set_error("eval_launch_info: out is null"); return GF_ERR_NULL; }
+  EvalArgs a;
+  int rc = build_args(p, n_rad, n_ang, n_points, &a);
+  if (rc) return rc;
+  LaunchPlan plan;
+  if ((rc = plan_eval(a, p->precision, &plan))) return rc;
+  out->block_threads = plan.block_threads;
+  out->grid_blocks = plan.grid_blocks;
+  out->split = 1 << plan.split_log2;
+  out->smem_bytes = (int)plan.smem_bytes;
+  out->n_pairs = a.n_pairs;
+  out->n_terms = a.n_terms;
+  eval_inst_counts(a, p->precision, plan, &out->fp64_inst, &out->fp32_inst, &out->flops);
+  out->evals = (double)n_points * n_rad * n_ang;
+  return GF_OK;
+}
+
+int gf_diag_fp64_peak(int blocks, int threads, long long iters, double* d_sink, void* stream) {
+  if (!d_sink) { set_error("diag_fp64_peak: d_sink is null"); return GF_ERR_NULL; }
+  if (blocks < 1 || threads < 1 || threads > 1024 || iters < 0) { set_error("diag_fp64_peak: bad launch shape"); return GF_ERR_ARG; }
+  return launch_fp64_peak(blocks, threads, iters, d_sink, static_cast<cudaStream_t>(stream));
+}
+
+int gf_diag_rcp_seed(const double* d_in, double* d_out, long long n, void* stream) {
+  if (!d_in || !d_out) { set_error("diag_rcp_seed: null pointer"); return GF_ERR_NULL; }
+  if (n < 0) { set_error("diag_rcp_seed: n < 0"); return GF_ERR_ARG; }
+  if (n == 0) return GF_OK;
+  return launch_rcp_seed(d_in, d_out, n, static_cast<cudaStream_t>(stream));
+}
+
+}  // extern "C"
