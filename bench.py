@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the hot path of arXiv:1205.0752 on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg3_production]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the whole hot path over one synthetic scan: quadrature tables (a2:
+gf_make_quadrature, host generation + copy), grid fill (a1: gf_make_grid_rows), evaluation of the double
+integral with its reductions and stores (a3-a6: gf_eval_grid).  The workload at N=1 is BASELINE.json
+configs[2], the 2048x2048-point, 512x256-node FP64 production scan the headline target is quoted on.  With N
+ranks the grid keeps its box and 2048 columns and has 2048*N rows; each rank owns 2048 contiguous rows (weak
+scaling; grid points are independent; no data-path collective).
+
+value    = grid points/s of the whole job, inputs resident in HBM (the grid is produced on the device).
+e2e      = the same metric through gf_eval_grid_host on pinned HOST buffers (x in, G out), copies in the
+           timed region.
+roofline = the evaluation kernel against the FP64 pipe (bound "alu").
+cpu_baseline = the oracle as it stands, on the box's host cores, on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import gf_workloads as W
+
+METRIC = "grid_points_per_s"
+UNIT = "points/s"
+# 148 SMs x 64 FP64 FMA lanes x 2 flops x 1.965 GHz (clocks.max.sm)
+FP64_LANES_PER_SM = 64
+N_SM = 148
+# dram__bytes_read.sum + dram__bytes_write.sum of one eval kernel launch on cfg3 (profiles/, ncu --set full);
+# None until a capture is committed
+EVAL_KERNEL_DRAM_TRAFFIC_BYTES = None
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def workload_for(name, world):
+    """The per-job workload: cfg rows x world (weak scaling), and this is all the host logic there is."""
+    cfg = dict(W.CONFIGS[name])
+    cfg["n_im_global"] = cfg["n_im"] * world
+    return cfg
+
+
+def max_over_ranks(value, world, backend_device=None):
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=backend_device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, gpu_id):
+        self.rows, self.proc, self.thread = [], None, None
+        self.cmd = ["nvidia-smi", "-i", str(gpu_id), "--query-gpu=" + self.FIELDS, "--format=csv,noheader,nounits",
+                    "-lms", "100"]
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(self.cmd, stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], None, [], set()
+        for t, line in self.rows:
+            if not (t0 <= t <= t1 + 0.1):
+                continue
+            f = [c.strip() for c in line.split(",")]
+            try:
+                sm.append(float(f[0]))
+                smax = float(f[1])
+                power.append(float(f[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(self.NAMES, f[3:7]):
+                if v == "Active":
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax,
+                "power_w_max": max(power) if power else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------- oracle legs
+def oracle_sample(cfg, stride):
+    """Every `stride`-th index in each direction of the workload's grid (per-point cost is uniform)."""
+    from oracle import gf_oracle as O
+    X = O.make_grid(cfg["re"][0], cfg["re"][1], cfg["n_re"], cfg["im"][0], cfg["im"][1], cfg["n_im"],
+                    spacing=cfg["spacing"], im_abs_min=cfg["im_abs_min"])
+    return np.ascontiguousarray(X[::stride, ::stride]).ravel()
+
+
+def oracle_step(cfg, xs):
+    """One pass of the oracle over the sample: its own tables, then the triple loop (double accumulation,
+    the timed variant of oracle/gf_oracle.cpp).  Returns (seconds, threads used)."""
+    from oracle import gf_oracle as O
+    t = time.perf_counter()
+    P = O.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE)
+    rn, rw = O.make_quadrature(W.RADIAL_RULE, cfg["n_rad"])
+    z, wz = O.make_quadrature(W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
+    _, used = O.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, xs, accum="double")
+    return time.perf_counter() - t, used
+
+
+def cpu_baseline(cfg, stride=8):
+    xs = oracle_sample(cfg, stride)
+    dt, used = oracle_step(cfg, xs)
+    return {"value": xs.size / dt, "unit": UNIT, "cores": used, "kind": "oracle",
+            "evals_per_s": xs.size * cfg["n_rad"] * cfg["n_ang"] / dt,
+            "sample": "%s: every %dth index in each direction (%d of %d points, all %dx%d nodes), %.1f s, "
+                      "oracle/gf_oracle.cpp -O2, double accumulation, one thread per core"
+                      % (cfg["name"], stride, xs.size, cfg["n_re"] * cfg["n_im"], cfg["n_rad"], cfg["n_ang"], dt)}
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    cfg = dict(W.CONFIGS[args.workload], name=args.workload)
+    stride = 16
+    from oracle import gf_oracle as O
+    O.build()
+    xs = oracle_sample(cfg, stride)
+    for _ in range(args.warmup):
+        oracle_step(cfg, xs)
+    t = time.perf_counter()
+    used = 0
+    for _ in range(args.steps):
+        _, used = oracle_step(cfg, xs)
+    dt = time.perf_counter() - t
+    value = xs.size * args.steps / dt
+    sample = ("each step: every %dth index in each direction of %s (%d of %d points, all %dx%d nodes); "
+              "oracle/gf_oracle.cpp -O2, double accumulation, one thread per core"
+              % (stride, args.workload, xs.size, cfg["n_re"] * cfg["n_im"], cfg["n_rad"], cfg["n_ang"]))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg, 1, cfg["n_im"]),
+            "evals_per_s": value * cfg["n_rad"] * cfg["n_ang"],
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(cfg, world, rows_per_rank):
+    return {"workload": "%s: bubble m=1 once-subtracted at p^2=0, %dx%d grid over Re[%g,%g] Im[%g,%g], "
+                        "%d radial x %d angular Gauss-Legendre nodes, cutoff %g, REAL contour, complex128"
+                        % (cfg["name"], cfg["n_re"], rows_per_rank * world, cfg["re"][0], cfg["re"][1], cfg["im"][0],
+                           cfg["im"][1], cfg["n_rad"], cfg["n_ang"], cfg["cutoff2"]),
+            "n_points": cfg["n_re"] * rows_per_rank * world, "n_rad": cfg["n_rad"], "n_ang": cfg["n_ang"],
+            "parallelism": "rows x%d, no collective" % world,
+            "cache": "L2 flushed between steps (256 MiB write); x + G = 128 MiB per rank"}
+
+
+# ------------------------------------------------------------------------------------- the CUDA arm
+def run_ours(args):
+    import torch
+    import paper_1205_0752_b200 as gf
+    gf.lib()  # fails loudly when the extension is missing: there is no fallback
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path runs only in the sm_100a kernels")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = workload_for(args.workload, world)
+    cfg["name"] = args.workload
+    n_re, n_rows, n_rad, n_ang = cfg["n_re"], cfg["n_im"], cfg["n_rad"], cfg["n_ang"]
+    row_first, rows_local = W.row_partition(cfg["n_im_global"], world, rank)
+    assert rows_local == n_rows
+    n_points_local = n_re * rows_local
+    P = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
+                       contour="real", precision=64)
+    info = gf.launch_info(P, n_rad, n_ang, n_points_local)
+
+    x = torch.empty((rows_local, n_re), dtype=torch.complex128, device=dev)
+    out = torch.empty_like(x)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    ev_k0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev_k1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+
+    def step(k=None):
+        rn, rw = gf.make_radial_tables("real", n_rad, W.RADIAL_RULE)                    # a2
+        z, wz = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")           # a2
+        gf.make_grid_rows(cfg["re"][0], cfg["re"][1], n_re, cfg["im"][0], cfg["im"][1], cfg["n_im_global"],
+                          row_first, rows_local, spacing=cfg["spacing"], im_abs_min=cfg["im_abs_min"], out=x)  # a1
+        if k is not None:
+            ev_k0[k].record(stream)
+        gf.eval_grid(P, rn, rw, n_rad, z, wz, x, out=out)                                # a3-a6
+        if k is not None:
+            ev_k1[k].record(stream)
+        flush.zero_()                                                                    # L2 flush
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+
+    sampler = ClockSampler("GPU-" + str(torch.cuda.get_device_properties(dev).uuid).replace("GPU-", ""))
+    sampler.start()
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.perf_counter()
+    e0.record(stream)
+    for k in range(args.steps):
+        step(k)
+    e1.record(stream)
+    barrier()
+    t1 = time.perf_counter()
+    clocks = sampler.stop(t0, t1)
+    ms_total = max_over_ranks(e0.elapsed_time(e1), world, dev)
+    kernel_ms = float(np.mean([a.elapsed_time(b) for a, b in zip(ev_k0, ev_k1)]))
+    checksum = out.view(torch.float64).abs().sum().item()
+    assert np.isfinite(checksum) and checksum > 0
+
+    # ---- e2e: the host-buffer entry point, copies inside the timed region
+    xh = x.cpu().pin_memory()
+    outh = torch.empty(xh.shape, dtype=torch.complex128).pin_memory()
+    rn_h, rw_h = gf.make_radial_tables_host("real", n_rad, W.RADIAL_RULE)
+    z_h, wz_h = gf.make_quadrature_host(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+
+    def e2e_step():
+        gf.eval_grid_host(P, rn_h, rw_h, n_rad, z_h, wz_h, xh, outh)   # synchronises before returning
+        flush.zero_()
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    ee0, ee1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ee0.record(stream)
+    for _ in range(args.steps):
+        e2e_step()
+    ee1.record(stream)
+    barrier()
+    e2e_ms = max_over_ranks(ee0.elapsed_time(ee1), world, dev)
+    assert torch.equal(outh.view(torch.float64), out.cpu().view(torch.float64)), "e2e result differs from device path"
+    h2d = n_points_local * 16 + 8 * (2 * n_rad + 2 * n_ang)
+    d2h = n_points_local * 16
+
+    # ---- the measured FP64-pipe peak at the clocks this run saw (8 independent DFMA chains per thread)
+    peak_blocks, peak_threads, peak_iters = N_SM * 4, 512, 100000
+    sink = torch.empty(peak_blocks * peak_threads, dtype=torch.float64, device=dev)
+    best = float("inf")
+    for i in range(6):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        gf.diag_fp64_peak(peak_blocks, peak_threads, peak_iters, sink)
+        b.record(stream)
+        torch.cuda.synchronize()
+        if i:
+            best = min(best, a.elapsed_time(b))
+    dfma_tflops = 2.0 * 8 * peak_iters * peak_blocks * peak_threads / (best * 1e-3) / 1e12
+
+    if world > 1:
+        torch.distributed.barrier()
+    if rank != 0:
+        if world > 1:
+            torch.distributed.destroy_process_group()
+        return 0
+
+    sm_max = clocks["sm_max_mhz"] or 1965.0
+    peak_nominal = 2.0 * FP64_LANES_PER_SM * N_SM * sm_max * 1e6 / 1e12
+    achieved = info["flops"] / (kernel_ms * 1e-3) / 1e12
+    n_points_job = n_points_local * world
+    value = n_points_job * args.steps / (ms_total * 1e-3)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, world, rows_local),
+        "evals_per_s": value * n_rad * n_ang,
+        "e2e": {"value": n_points_job * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": h2d * world, "d2h_bytes_per_step": d2h * world},
+        "gpu_launches": 2 * args.steps,
+        "launch": {"kernel": "eval_real_kernel<double>", "grid_blocks": info["grid_blocks"],
+                   "block_threads": info["block_threads"], "smem_bytes": info["smem_bytes"], "lanes_per_point": info["split"]},
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
+                     "frac": achieved / peak_nominal, "traffic": EVAL_KERNEL_DRAM_TRAFFIC_BYTES,
+                     "peak_kind": "derived: %d SMs x %d FP64 lanes x 2 x %.0f MHz (DESIGN.md)" % (N_SM, FP64_LANES_PER_SM, sm_max),
+                     "peak_measured_dfma": dfma_tflops, "frac_of_measured_dfma": achieved / dfma_tflops,
+                     "kernel_ms": kernel_ms, "flops_per_launch": info["flops"],
+                     "fp64_inst_per_launch": info["fp64_inst"],
+                     "fp64_pipe_frac": info["fp64_inst"] / (kernel_ms * 1e-3) / (FP64_LANES_PER_SM * N_SM * sm_max * 1e6),
+                     "kernel_share_of_step": kernel_ms * args.steps / ms_total},
+        "clocks": clocks,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import gf_oracle as O
+        O.build()
+        line["cpu_baseline"] = cpu_baseline(dict(W.CONFIGS[args.workload], name=args.workload))
+    print(json.dumps(line))
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", default="cfg3_production", choices=list(W.CONFIGS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    _, _, world = dist_env()
+    if world != args.gpus and world > 1:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d" % (args.gpus, world))
+    if args.gpus > 1 and world == 1 and args.impl == "ours":
+        raise SystemExit("bench.py: launch N>1 with torch.distributed.run (one rank per GPU)")
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

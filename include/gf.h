@@ -94,6 +94,13 @@ typedef struct {
 int gf_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
                  int spacing, double im_abs_min, void* d_x, void* stream);
 
+/* Rows [row_first, row_first + n_rows) of the same grid into d_x[n_rows][n_re], bit-identical to the
+ * corresponding rows of gf_make_grid.  This is the multi-GPU partition: grid
+ * points are independent, each rank owns a contiguous block of rows, no exchange.
+ * n_rows = 0 is a no-op. */
+int gf_make_grid_rows(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
+                      int spacing, double im_abs_min, int row_first, int n_rows, void* d_x, void* stream);
+
 /* "Preparation": nodes t_i in (-1,1), ascending, and weights of an n-point rule
  * into caller-allocated DEVICE arrays of n doubles each.  Tables are computed on the host in extended
  * precision (as in the paper) and copied with cudaMemcpyAsync on `stream`; the host staging copy is

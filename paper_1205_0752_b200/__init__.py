@@ -51,6 +51,7 @@ _lib = None
 _vp, _dbl, _int, _ll = ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.c_longlong
 _SIGNATURES = {
     "gf_make_grid": [_dbl, _dbl, _int, _dbl, _dbl, _int, _int, _dbl, _vp, _vp],
+    "gf_make_grid_rows": [_dbl, _dbl, _int, _dbl, _dbl, _int, _int, _dbl, _int, _int, _vp, _vp],
     "gf_make_quadrature": [_int, _int, _dbl, _int, _vp, _vp, _vp],
     "gf_make_quadrature_host": [_int, _int, _dbl, _int, _vp, _vp],
     "gf_radial_table_size": [_int, _int],
@@ -134,6 +135,17 @@ def make_grid(re_min, re_max, n_re, im_min, im_max, n_im, spacing="uniform", im_
     with torch.cuda.device(dev):
         _check(lib().gf_make_grid(re_min, re_max, n_re, im_min, im_max, n_im, SPACING[spacing], im_abs_min,
                                   x.data_ptr(), _stream(stream)))
+    return x
+
+
+def make_grid_rows(re_min, re_max, n_re, im_min, im_max, n_im, row_first, n_rows, spacing="uniform",
+                   im_abs_min=0.0, device=None, stream=None, out=None):
+    """gf_make_grid_rows: rows [row_first, row_first+n_rows) of the grid, complex128 [n_rows, n_re]."""
+    dev = _device(device)
+    x = out if out is not None else torch.empty((n_rows, n_re), dtype=torch.complex128, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib().gf_make_grid_rows(re_min, re_max, n_re, im_min, im_max, n_im, SPACING[spacing], im_abs_min,
+                                       row_first, n_rows, x.data_ptr(), _stream(stream)))
     return x
 
 

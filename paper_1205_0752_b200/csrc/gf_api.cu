@@ -116,10 +116,14 @@ extern "C" {
 const char* gf_last_error(void) { return g_err; }
 const char* gf_version(void) { return "gf_b200 0.1 (sm_100a)"; }
 
-int gf_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im, int spacing,
-                 double im_abs_min, void* d_x, void* stream) {
-  if (!d_x) { set_error("make_grid: d_x is null"); return GF_ERR_NULL; }
+static int make_grid_rows(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
+                          int spacing, double im_abs_min, int row_first, int n_rows, void* d_x, void* stream) {
   if (n_re < 1 || n_im < 1) { set_error("make_grid: n_re=%d, n_im=%d must be >= 1", n_re, n_im); return GF_ERR_ARG; }
+  if (row_first < 0 || n_rows < 0 || (long long)row_first + n_rows > n_im) {
+    set_error("make_grid: rows [%d, %d+%d) outside the grid of %d rows", row_first, row_first, n_rows, n_im);
+    return GF_ERR_ARG;
+  }
+  if (!d_x && n_rows > 0) { set_error("make_grid: d_x is null"); return GF_ERR_NULL; }
   if (!std::isfinite(re_min) || !std::isfinite(re_max) || !std::isfinite(im_min) || !std::isfinite(im_max)) {
     set_error("make_grid: non-finite box");
     return GF_ERR_ARG;
@@ -133,8 +137,20 @@ int gf_make_grid(double re_min, double re_max, int n_re, double im_min, double i
     set_error("make_grid: unknown spacing %d", spacing);
     return GF_ERR_ARG;
   }
-  return launch_make_grid(re_min, re_max, n_re, im_min, im_max, n_im, spacing, im_abs_min,
+  return launch_make_grid(re_min, re_max, n_re, im_min, im_max, n_im, spacing, im_abs_min, row_first, n_rows,
                           static_cast<double2*>(d_x), static_cast<cudaStream_t>(stream));
+}
+
+int gf_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im, int spacing,
+                 double im_abs_min, void* d_x, void* stream) {
+  if (!d_x) { set_error("make_grid: d_x is null"); return GF_ERR_NULL; }
+  return make_grid_rows(re_min, re_max, n_re, im_min, im_max, n_im, spacing, im_abs_min, 0, n_im, d_x, stream);
+}
+
+int gf_make_grid_rows(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im, int spacing,
+                      double im_abs_min, int row_first, int n_rows, void* d_x, void* stream) {
+  return make_grid_rows(re_min, re_max, n_re, im_min, im_max, n_im, spacing, im_abs_min, row_first, n_rows, d_x,
+                        stream);
 }
 
 int gf_make_quadrature_host(int kind, int n, double step, int measure, double* h_nodes, double* h_weights) {

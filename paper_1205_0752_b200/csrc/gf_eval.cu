@@ -234,14 +234,17 @@ __global__ void __launch_bounds__(kBlockThreads, 2) eval_real_kernel(const __gri
     const double2 xv = a.x[point];
     x = {xv.x, xv.y};
   }
-  // G(0) = 0 exactly (invariant I1); for 0 < |x| < 2^-200 use G(x) = G(x 2^400) 2^-400, exact to
-  // O(|x|) because G is analytic at 0 with G(0) = 0 (keeps zeta = A^2/(4xy) inside the FP64 range).
+  // G(0) = 0 exactly (invariant I1); for 0 < |x| < 2^-200 use G(x) = G(x 2^k) 2^-k with |x 2^k| ~ 2^-200,
+  // exact to O(|x|) because the sum is analytic at 0 and vanishes there (keeps zeta = A^2/(4xy) and its
+  // square inside the FP64 range).
   const bool is_zero = (x.re == 0.0 && x.im == 0.0);
   double out_scale = 1.0;
+  const double xmax = fmax(fabs(x.re), fabs(x.im));
   if (is_zero) x = {1.0, 0.0};
-  else if (fmax(fabs(x.re), fabs(x.im)) < 0x1p-200) {
-    x = {x.re * 0x1p400, x.im * 0x1p400};
-    out_scale = 0x1p-400;
+  else if (xmax < 0x1p-200) {
+    const int k = -200 - ilogb(xmax);
+    x = {scalbn(x.re, k), scalbn(x.im, k)};
+    out_scale = scalbn(1.0, -k);
   }
   const cd xinv = cinv(x);
 

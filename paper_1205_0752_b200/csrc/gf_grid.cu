@@ -16,11 +16,13 @@ __device__ __forceinline__ double axis_value(double lo, double hi, double d, int
 __global__ void __launch_bounds__(256) make_grid_kernel(double re_min, double re_max, double d_re, int n_re,
                                                         double im_min, double im_max, double d_im, int n_im,
                                                         int spacing, double log_lo, double log_hi,
-                                                        double im_abs_min, double2* __restrict__ x) {
-  const long long total = (long long)n_re * n_im;
+                                                        double im_abs_min, int row_first, int n_rows,
+                                                        double2* __restrict__ x) {
+  const long long total = (long long)n_re * n_rows;
   for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < total;
        p += (long long)gridDim.x * blockDim.x) {
-    const int j = (int)(p / n_re), i = (int)(p - (long long)j * n_re);
+    const int jl = (int)(p / n_re), i = (int)(p - (long long)jl * n_re);
+    const int j = row_first + jl;  // row of the global grid
     double im;
     if (spacing == GF_SPACING_UNIFORM) {
       im = axis_value(im_min, im_max, d_im, n_im, j);
@@ -41,8 +43,10 @@ __global__ void __launch_bounds__(256) make_grid_kernel(double re_min, double re
 }  // namespace
 
 int launch_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
-                     int spacing, double im_abs_min, double2* d_x, cudaStream_t stream) {
-  const long long total = (long long)n_re * n_im;
+                     int spacing, double im_abs_min, int row_first, int n_rows, double2* d_x,
+                     cudaStream_t stream) {
+  const long long total = (long long)n_re * n_rows;
+  if (total == 0) return GF_OK;
   const double d_re = n_re > 1 ? (re_max - re_min) / (double)(n_re - 1) : 0.0;
   const double d_im = n_im > 1 ? (im_max - im_min) / (double)(n_im - 1) : 0.0;
   double log_lo = 0, log_hi = 0;
@@ -53,7 +57,7 @@ int launch_make_grid(double re_min, double re_max, int n_re, double im_min, doub
   long long blocks = (total + 255) / 256;
   if (blocks > 148LL * 16) blocks = 148LL * 16;  // grid-stride: 16 CTAs per SM
   make_grid_kernel<<<(unsigned)blocks, 256, 0, stream>>>(re_min, re_max, d_re, n_re, im_min, im_max, d_im, n_im,
-                                                         spacing, log_lo, log_hi, im_abs_min, d_x);
+                                                         spacing, log_lo, log_hi, im_abs_min, row_first, n_rows, d_x);
   return check_cuda(cudaGetLastError(), "make_grid launch");
 }
 

@@ -54,7 +54,8 @@ int make_rule_host(int kind, int n, double step, int measure, double* nodes, dou
 
 // gf_grid.cu
 int launch_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
-                     int spacing, double im_abs_min, double2* d_x, cudaStream_t stream);
+                     int spacing, double im_abs_min, int row_first, int n_rows, double2* d_x,
+                     cudaStream_t stream);
 
 // gf_eval.cu
 int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan);

@@ -1,0 +1,266 @@
+"""Parity of the CUDA path (through the C ABI, via the thin binding) with the CPU oracle, element by
+element on the same inputs.  Bars (BASELINE.json north_star):
+  FP64  max over points of |G_gpu - G_oracle| / |G_oracle|  <= 1e-11   (0/0 := 0, reading G17)
+  FP32  the same                                             <= 1e-4
+  grids: bit-exact;  quadrature tables: <= 4 ulp (independent generators, reading "parity safety").
+Each side builds its own grid and its own tables from the numbers in gf_workloads.py.
+"""
+import numpy as np
+import pytest
+import torch
+
+import gf_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-11
+TOL32 = 1e-4
+
+
+@pytest.fixture(scope="module")
+def gf():
+    import paper_1205_0752_b200 as gf
+    gf.lib()  # fails loudly if the extension is missing
+    assert torch.cuda.is_available()
+    return gf
+
+
+def relerr(g, ref):
+    g = np.asarray(g, dtype=np.complex128).ravel()
+    ref = np.asarray(ref, dtype=np.complex128).ravel()
+    both_zero = (ref == 0) & (g == 0)
+    den = np.where(ref == 0, 1.0, np.abs(ref))
+    e = np.abs(g - ref) / den
+    e[both_zero] = 0.0
+    return e
+
+
+def gpu_setup(gf, cfg, contour="real", ang=None, precision=64):
+    P = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR,
+                       map_scale=W.MAP_SCALE, contour=contour, precision=precision)
+    rn, rw = gf.make_radial_tables(contour, cfg["n_rad"], W.RADIAL_RULE)
+    z, wz = gf.make_quadrature(ang or W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
+    return P, rn, rw, z, wz
+
+
+def gpu_grid(gf, cfg):
+    return gf.make_grid(cfg["re"][0], cfg["re"][1], cfg["n_re"], cfg["im"][0], cfg["im"][1], cfg["n_im"],
+                        spacing=cfg["spacing"], im_abs_min=cfg["im_abs_min"])
+
+
+def oracle_setup(O, cfg, contour="real", ang=None):
+    P = O.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR,
+                      map_scale=W.MAP_SCALE, contour=contour)
+    rn, rw = O.make_radial_pyramid(cfg["n_rad"], levels=1 if contour == "real" else 4, kind=W.RADIAL_RULE)
+    z, wz = O.make_quadrature(ang or W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
+    return P, rn, rw, z, wz
+
+
+def oracle_grid(O, cfg):
+    return O.make_grid(cfg["re"][0], cfg["re"][1], cfg["n_re"], cfg["im"][0], cfg["im"][1], cfg["n_im"],
+                       spacing=cfg["spacing"], im_abs_min=cfg["im_abs_min"])
+
+
+def oracle_eval(O, cfg, xs, contour="real", ang=None):
+    P, rn, rw, z, wz = oracle_setup(O, cfg, contour, ang)
+    g, _ = O.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, xs)
+    return g
+
+
+# ------------------------------------------------------------------ a1: grid fill
+@pytest.mark.parametrize("name", list(W.CONFIGS))
+def test_grid_bit_exact(gf, oracle, name):
+    cfg = W.CONFIGS[name]
+    xg = gpu_grid(gf, cfg).cpu().numpy()
+    xo = oracle_grid(oracle, cfg)
+    assert xg.shape == (cfg["n_im"], cfg["n_re"])
+    assert np.array_equal(xg.view(np.float64), xo.view(np.float64))
+
+
+@pytest.mark.parametrize("shape", [(1, 1), (1, 7), (5, 1), (3, 1001), (257, 129)])
+def test_grid_ragged_shapes(gf, oracle, shape):
+    n_im, n_re = shape
+    xg = gf.make_grid(-3.0, 2.5, n_re, -1.25, 1.25, n_im).cpu().numpy()
+    xo = oracle.make_grid(-3.0, 2.5, n_re, -1.25, 1.25, n_im)
+    assert np.array_equal(xg.view(np.float64), xo.view(np.float64))
+
+
+# ------------------------------------------------------------------ a2: tables
+@pytest.mark.parametrize("kind", ["gauss_legendre", "gauss_cheb2", "tanh_sinh"])
+@pytest.mark.parametrize("n", [1, 2, 31, 32, 49, 256, 1024])
+@pytest.mark.parametrize("measure", ["plain", "sqrt1mz2"])
+def test_tables_match_oracle(gf, oracle, kind, n, measure):
+    xg, wg = (t.cpu().numpy() for t in gf.make_quadrature(kind, n, measure=measure))
+    xo, wo = oracle.make_quadrature(kind, n, measure=measure)
+    assert np.max(np.abs(xg - xo)) <= 4 * np.finfo(float).eps
+    assert np.max(np.abs(wg - wo) / np.abs(wo)) <= 64 * np.finfo(float).eps
+    xh, wh = gf.make_quadrature_host(kind, n, measure=measure)
+    assert np.array_equal(xh, xg) and np.array_equal(wh, wg)
+
+
+# ------------------------------------------------------------------ a3-a6: evaluation, REAL contour
+def test_cfg1_every_point(gf, oracle):
+    cfg = W.CONFIGS["cfg1_tiny"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
+    ref = oracle_eval(oracle, cfg, oracle_grid(oracle, cfg))
+    e = relerr(g, ref)
+    assert e.max() <= TOL64, (e.max(), x.cpu().numpy().ravel()[e.argmax()])
+
+
+def test_cfg2_every_point(gf, oracle):
+    cfg = W.CONFIGS["cfg2_mid"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
+    ref = oracle_eval(oracle, cfg, oracle_grid(oracle, cfg))
+    e = relerr(g, ref)
+    assert e.max() <= TOL64, (e.max(), x.cpu().numpy().ravel()[e.argmax()])
+
+
+@pytest.mark.parametrize("name,n_random", [("cfg3_production", 256), ("cfg4_rational", 256), ("cfg5_strip", 64)])
+def test_large_configs_sampled(gf, oracle, name, n_random):
+    """Full-size launch (the configuration bench.py times), compared on a seeded sample the oracle
+    can compute point by point."""
+    cfg = W.CONFIGS[name]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+    torch.cuda.synchronize()
+    idx = W.parity_sample(cfg, n_random=n_random, stride=max(cfg["n_re"], cfg["n_im"]) // 8)
+    gs = g.reshape(-1)[torch.from_numpy(idx).cuda()].cpu().numpy()
+    xs = oracle_grid(oracle, cfg).ravel()[idx]
+    ref = oracle_eval(oracle, cfg, xs)
+    e = relerr(gs, ref)
+    assert e.max() <= TOL64, (name, e.max(), xs[e.argmax()])
+    # property at full size: rows j and n_im-1-j are conjugates, bit for bit (invariant I2)
+    # (cfg4: conjugation also swaps the two conjugate poles of line 2, i.e. the order of two additions)
+    gn = g.cpu().numpy()
+    if name == "cfg4_rational":
+        assert relerr(np.conj(gn[::-1]), gn).max() <= 1e-12
+    else:
+        assert np.array_equal(gn[::-1].real, gn.real) and np.array_equal(gn[::-1].imag, -gn.imag)
+
+
+def test_fp32_variant(gf, oracle):
+    cfg = dict(W.CONFIGS["cfg2_mid"], n_re=128, n_im=96)
+    P, rn, rw, z, wz = gpu_setup(gf, cfg, precision=32)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+    assert g.dtype == torch.complex64
+    ref = oracle_eval(oracle, cfg, oracle_grid(oracle, cfg))
+    e = relerr(g.cpu().numpy(), ref)
+    assert e.max() <= TOL32, e.max()
+
+
+@pytest.mark.parametrize("ang,n_ang", [("gauss_cheb2", 33), ("tanh_sinh", 49), ("gauss_legendre", 1),
+                                       ("gauss_legendre", 7), ("gauss_cheb2", 130)])
+@pytest.mark.parametrize("n_rad", [1, 3, 64, 100])
+def test_ragged_orders_and_rules(gf, oracle, ang, n_ang, n_rad):
+    """Odd orders (middle node enters once), orders that are not multiples of the unroll, n = 1."""
+    cfg = dict(W.CONFIGS["cfg1_tiny"], n_re=37, n_im=11, n_rad=n_rad, n_ang=n_ang)
+    P, rn, rw, z, wz = gpu_setup(gf, cfg, ang=ang)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, n_rad, z, wz, x).cpu().numpy()
+    ref = oracle_eval(oracle, cfg, oracle_grid(oracle, cfg), ang=ang)
+    e = relerr(g, ref)
+    assert e.max() <= TOL64, e.max()
+
+
+@pytest.mark.parametrize("n_points", [1, 2, 31, 33, 255, 257, 4097, 75777])
+def test_ragged_point_counts(gf, oracle, n_points):
+    """Every lane-split (1..32 lanes per point) and a ragged last CTA."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    rng = np.random.default_rng(W.PARITY_SEED + n_points)
+    xs = rng.uniform(-5, 1, n_points) + 1j * rng.uniform(-2, 2, n_points)
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+    keep = slice(None) if n_points <= 4097 else slice(None, None, 37)
+    ref = oracle_eval(oracle, cfg, xs[keep])
+    assert relerr(g[keep], ref).max() <= TOL64
+
+
+def test_empty_input(gf):
+    cfg = W.CONFIGS["cfg1_tiny"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    x = torch.empty(0, dtype=torch.complex128, device="cuda")
+    assert gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).numel() == 0
+
+
+def test_degenerate_points(gf, oracle):
+    """x = 0 (exactly 0, invariant I1), tiny and huge |x|, x on the axes, points on the cut side."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    xs = np.array([0, 1e-300, 1e-250j, 1e-100 + 1e-100j, 1e-12, -1e-9j, 1e-5 + 1e-5j, 3e-3, 1.0, -0.5, 1j, -1j,
+                   -3.9 + 1e-3j, -0.999 + 0.01j, 250.0 + 1j, 1e6 + 3e5j, -1e6 + 1j, 1e12j, 1e40 - 1e39j,
+                   -5 + 2j, -5 - 2j], dtype=np.complex128)
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+    ref = oracle_eval(oracle, cfg, xs)
+    assert g[0] == 0 and ref[0] == 0
+    e = relerr(g, ref)
+    assert e.max() <= TOL64, (e.max(), xs[e.argmax()])
+
+
+def test_conjugation_symmetry_bitwise(gf):
+    cfg = W.CONFIGS["cfg1_tiny"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+    gc = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x.conj().resolve_conj().contiguous())
+    assert torch.equal(gc.real, g.real) and torch.equal(gc.imag, -g.imag)
+
+
+@pytest.mark.parametrize("lines", ["complex_masses", "unequal", "rational_k", "rational_both"])
+def test_other_propagators(gf, oracle, lines):
+    bub = {"kind": "massive", "m2": 1.0}
+    rat = {"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2}
+    rat_real = {"kind": "rational", "M2": 0.7, "a": 3.0, "b": 1.5}   # two real poles
+    lk, lpk = {
+        "complex_masses": ({"kind": "massive", "m2": 0.5j}, {"kind": "massive", "m2": -0.5j}),   # eq. (19)
+        "unequal": ({"kind": "massive", "m2": 0.3}, {"kind": "massive", "m2": 2.5}),
+        "rational_k": (rat, bub),
+        "rational_both": (rat, rat_real),
+    }[lines]
+    cfg = dict(W.CONFIGS["cfg2_mid"], line_k=lk, line_pk=lpk, n_re=48, n_im=40, n_rad=128, n_ang=64,
+               re=(-0.2, 4.0), im=(-1.0, 1.0))
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
+    ref = oracle_eval(oracle, cfg, oracle_grid(oracle, cfg))
+    e = relerr(g, ref)
+    assert e.max() <= TOL64, e.max()
+
+
+def test_asymmetric_rule_is_rejected_with_nan(gf):
+    cfg = W.CONFIGS["cfg1_tiny"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    z2 = z.clone()
+    z2[3] += 1e-3
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z2, wz, gpu_grid(gf, cfg))
+    assert torch.isnan(g.real).all()
+
+
+# ------------------------------------------------------------------ end-to-end host entry point
+def test_eval_grid_host_matches_device_path(gf):
+    cfg = W.CONFIGS["cfg1_tiny"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu()
+    out = torch.empty(x.shape, dtype=torch.complex128).pin_memory()
+    gf.eval_grid_host(P, rn.cpu().numpy(), rw.cpu().numpy(), cfg["n_rad"], z.cpu().numpy(), wz.cpu().numpy(),
+                      x.cpu().pin_memory(), out)
+    assert torch.equal(out.view(torch.float64), g.view(torch.float64))
+
+
+def test_runs_on_the_callers_stream(gf):
+    cfg = W.CONFIGS["cfg1_tiny"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    x = gpu_grid(gf, cfg)
+    ref = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+    s.synchronize()
+    assert torch.equal(g.view(torch.float64), ref.view(torch.float64))
