@@ -22,8 +22,12 @@
 // The loops run in the paper's order (sub-contour, radial node, angular node),
 // every term is evaluated in std::complex<double> arithmetic in the combined
 // form the paper itself prints in eq. (20) (so that G(0) = 0 exactly), and the
-// sums are accumulated in long double (accum=0, the parity variant) or double
-// (accum=1, the timed variant).  No blocking, pairing, fusion or reordering.
+// sums are accumulated in long double (accum=0) or double (accum=1, the timed
+// variant).  accum=2, the parity variant, runs the same loops with every term in
+// std::complex<long double> as well: at the rare points where the contour passes
+// within ~1e-5 of a singularity of the integrand, and at tiny |x| where the +-z
+// terms cancel to O(sqrt|x|), double terms are themselves only good to ~1e-11
+// (reading G18).  No blocking, pairing, fusion or reordering.
 //
 // Pins (tests/test_oracle_pins.py): closed form CF1 of the equal-mass bubble,
 // the paper's eq. (18) for masses^2 = +-i/2, the Feynman-parameter form CF3 for
@@ -202,25 +206,32 @@ int make_grid(double re_min, double re_max, int n_re, double im_min, double im_m
 }
 
 // ---- propagators ---------------------------------------------------------
-cplx prop(const Propagator& P, cplx u) {
-  if (P.kind == PROP_MASSIVE) return 1.0 / (u + cplx(P.m2_re, P.m2_im));
-  return (u + P.M2) / (u * u + P.a * u + P.b);
+// R is the real type the terms are evaluated in: double, or long double for the
+// variant whose own rounding error is negligible against the 1e-11 parity bar
+// even where a term is nearly singular or x is tiny (reading G18).
+template <typename R>
+std::complex<R> prop(const Propagator& P, std::complex<R> u) {
+  typedef std::complex<R> C;
+  if (P.kind == PROP_MASSIVE) return C(1) / (u + C((R)P.m2_re, (R)P.m2_im));
+  return (u + (R)P.M2) / (u * u + (R)P.a * u + (R)P.b);
 }
 
 // D2(u) - D2(y) with u = y + d, in the combined form of eq. (20)
 // (PAPER.md:198-203): the factor d = x - 2 sqrt(x) sqrt(y) z is explicit, so
 // the difference is exactly 0 at x = 0 and keeps full relative accuracy at
 // small |x| (a numerical difference of two nearly equal numbers would not).
-cplx prop_diff(const Propagator& P, cplx y, cplx d) {
-  cplx u = y + d;
+template <typename R>
+std::complex<R> prop_diff(const Propagator& P, std::complex<R> y, std::complex<R> d) {
+  typedef std::complex<R> C;
+  C u = y + d;
   if (P.kind == PROP_MASSIVE) {
-    cplx c = y + cplx(P.m2_re, P.m2_im);
+    C c = y + C((R)P.m2_re, (R)P.m2_im);
     return -d / ((c + d) * c);
   }
   // (u+M2)/Q(u) - (y+M2)/Q(y) = -d [u y + M2 (u+y) + a M2 - b] / (Q(u) Q(y))
-  cplx Qu = u * u + P.a * u + P.b;
-  cplx Qy = y * y + P.a * y + P.b;
-  return -d * (u * y + P.M2 * (u + y) + (P.a * P.M2 - P.b)) / (Qu * Qy);
+  C Qu = u * u + (R)P.a * u + (R)P.b;
+  C Qy = y * y + (R)P.a * y + (R)P.b;
+  return -d * (u * y + (R)P.M2 * (u + y) + ((R)P.a * (R)P.M2 - (R)P.b)) / (Qu * Qy);
 }
 
 // scale of the singular structure of line 2 in the y-plane: |m2^2| for a
@@ -345,30 +356,34 @@ int auto_policy(const Params& P, cplx x, int n_ang) {
 }
 
 // ---- Step 5 / Kernel 2: the double sum for one x ---------------------------
-template <typename ACC>
+// ACC: type of the two running sums; R: type every term is evaluated in.
+template <typename ACC, typename R>
 cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int n_rad,
                 const double* z, const double* wz, int n_ang, std::vector<RNode>& nodes) {
+  typedef std::complex<R> C;
   nodes.clear();
   int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, x, n_ang) : P.contour;
   if (pol == CONTOUR_REAL) contour_real(P, rn, rw, n_rad, nodes);
   else if (pol == CONTOUR_RAY_ARC) contour_ray_arc(P, x, rn, rw, n_rad, nodes);
   else contour_thread(P, x, rn, rw, n_rad, nodes);
 
-  cplx sx = std::sqrt(x);  // principal branch
+  C xx((R)x.real(), (R)x.imag());
+  C sx = std::sqrt(xx);  // principal branch
   ACC gr = 0, gi = 0;
   for (size_t i = 0; i < nodes.size(); ++i) {
-    cplx y = nodes[i].y;
-    cplx B = 2.0 * sx * std::sqrt(y);
-    cplx D1 = prop(P.line_k, y);
+    C y((R)nodes[i].y.real(), (R)nodes[i].y.imag());
+    C wy((R)nodes[i].wy.real(), (R)nodes[i].wy.imag());
+    C B = (R)2 * sx * std::sqrt(y);
+    C D1 = prop<R>(P.line_k, y);
     ACC sr = 0, si = 0;
     for (int j = 0; j < n_ang; ++j) {
-      cplx d = x - B * z[j];                                   // u - y
-      cplx f = D1 * prop_diff(P.line_pk, y, d);                // F_sub, eq. (20)
-      sr += (ACC)(wz[j] * f.real());
-      si += (ACC)(wz[j] * f.imag());
+      C d = xx - B * (R)z[j];                                  // u - y
+      C f = D1 * prop_diff<R>(P.line_pk, y, d);                // F_sub, eq. (20)
+      sr += (ACC)((R)wz[j] * f.real());
+      si += (ACC)((R)wz[j] * f.imag());
     }
-    cplx S((double)sr, (double)si);
-    cplx term = nodes[i].wy * y * S;                           // dy y (...), eq. (14)
+    C S((R)sr, (R)si);
+    C term = wy * y * S;                                       // dy y (...), eq. (14)
     gr += (ACC)term.real();
     gi += (ACC)term.imag();
   }
@@ -398,8 +413,9 @@ int gfo_make_grid(double re_min, double re_max, int n_re, double im_min, double 
   return make_grid(re_min, re_max, n_re, im_min, im_max, n_im, spacing, im_abs_min, x);
 }
 
-// x, out: interleaved (re, im) doubles.  accum: 0 = long double sums (parity),
-// 1 = double sums (the timed variant).  n_threads <= 0: hardware concurrency.
+// x, out: interleaved (re, im) doubles.  accum: 0 = double terms, long double sums;
+// 1 = double terms and sums (the timed variant); 2 = long double terms and sums (the
+// parity variant: own rounding error << 1e-11 at every point, reading G18).  n_threads <= 0: hardware concurrency.
 // Returns 0 on success; fills *threads_used.
 int gfo_eval_grid(const void* params, const double* rad_nodes, const double* rad_weights, int n_rad,
                   const double* ang_nodes, const double* ang_weights, int n_ang, const double* x,
@@ -422,8 +438,10 @@ int gfo_eval_grid(const void* params, const double* rad_nodes, const double* rad
     for (long long p = tid; p < n_points; p += nt) {
       cplx xx(x[2 * p], x[2 * p + 1]);
       cplx g = accum == 0
-                   ? eval_point<ld>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
-                   : eval_point<double>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes);
+                   ? eval_point<ld, double>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
+               : accum == 1
+                   ? eval_point<double, double>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
+                   : eval_point<ld, ld>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes);
       out[2 * p] = g.real();
       out[2 * p + 1] = g.imag();
     }

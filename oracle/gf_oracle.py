@@ -23,6 +23,9 @@ MEASURE = {"plain": 0, "sqrt1mz2": 1}
 PROP = {"massive": 0, "rational": 1}
 CONTOUR = {"real": 0, "ray_arc": 1, "thread": 2, "auto": 3}
 SPACING = {"uniform": 0, "log_abs_im": 1}
+# arithmetic variants of gfo_eval_grid: double terms + long double sums; all double (timed);
+# long double terms and sums (parity: own rounding error << 1e-11 everywhere, reading G18)
+ACCUM = {"long_double": 0, "double": 1, "extended": 2}
 
 
 class _Prop(ctypes.Structure):
@@ -134,7 +137,7 @@ def eval_grid(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, 
     rc = lib().gfo_eval_grid(ctypes.byref(params), _dp(rn), _dp(rw), int(n_rad), _dp(an), _dp(aw),
                              int(an.size), _dp(xf.view(np.float64)), ctypes.c_longlong(xf.size),
                              _dp(out.view(np.float64)), int(n_threads),
-                             0 if accum == "long_double" else 1, ctypes.byref(used))
+                             ACCUM[accum], ctypes.byref(used))
     if rc:
         raise ValueError("gfo_eval_grid failed: %d" % rc)
     return out.reshape(np.shape(x)), used.value
