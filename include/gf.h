@@ -138,10 +138,18 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
                       const double* h_ang_nodes, const double* h_ang_weights, int n_ang, const void* h_x,
                       long long n_points, void* h_out, void* stream);
 
-/* How gf_eval_grid would launch, and its arithmetic per launch (for benchmarks and roofline numbers;
- * makes no CUDA call).  fp64_inst / fp32_inst are executed warp-level-uniform per-thread instruction
- * counts of the evaluation kernel summed over all threads (DFMA, DMUL and DADD each count 1), flops
- * counts an FMA as 2; both follow the SASS of the inner loop and the per-node set-up. */
+/* The same evaluation, also counting the work by route for the roofline accounting.
+ * d_counters: 6 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
+ *   [0] NEAR pairs  [1] FAR series terms  [2] EXACT pairs  [3..5] (point, radial node, pole) triples
+ *   taken by the NEAR / FAR / EXACT route.  Results are identical to gf_eval_grid. */
+int gf_eval_grid_counted(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                         const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
+                         long long n_points, void* d_out, unsigned long long* d_counters, void* stream);
+
+/* How gf_eval_grid would launch, and the FP64-pipe instructions per unit of work of each route (for benchmarks
+ * and roofline numbers; makes no CUDA call).  Per unit: *_dfma counts DFMA (2 flops each), *_other counts
+ * DMUL + DADD (1 flop each); they follow the SASS of the loops.  Executed
+ * instructions per launch = sum over routes of (gf_eval_grid_counted's counters) x (these). */
 typedef struct {
   int block_threads;      /* threads per CTA */
   long long grid_blocks;  /* CTAs */
@@ -149,10 +157,14 @@ typedef struct {
   int smem_bytes;         /* dynamic shared memory per CTA */
   int n_pairs;            /* folded angular nodes: ceil(n_ang/2) */
   int n_terms;            /* simple-pole terms of line 2 (1 massive, 2 rational) */
-  double fp64_inst;       /* FP64-pipe thread-instructions per launch */
-  double fp32_inst;       /* FP32-pipe thread-instructions of the inner loop (precision 32) */
-  double flops;           /* floating-point operations per launch */
+  int far_terms_max;      /* longest far-field series */
   double evals;           /* nominal integrand evaluations: n_points * n_rad * n_ang */
+  double near_pair_dfma, near_pair_other, near_pair_fp32;   /* per NEAR pair (fp32: FP32-pipe, precision 32) */
+  double far_term_dfma, far_term_other;                     /* per FAR series term */
+  double exact_pair_dfma, exact_pair_other;                 /* per EXACT pair */
+  double node_near_dfma, node_near_other;                   /* per (point, node, pole) by route: set-up + finish */
+  double node_far_dfma, node_far_other;
+  double node_exact_dfma, node_exact_other;
 } gf_launch_info;
 int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_points, gf_launch_info* out);
 
@@ -163,6 +175,10 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
  * gf_diag_rcp_seed: for n doubles in d_in, writes the raw MUFU.RCP64H seed to d_out. */
 int gf_diag_fp64_peak(int blocks, int threads, long long iters, double* d_sink, void* stream);
 int gf_diag_rcp_seed(const double* d_in, double* d_out, long long n, void* stream);
+/* The radial nodes y_i = s0 expm1(u_i L), u_i = (t_i + 1)/2, L = ln((cutoff2 + s0)/s0), of the REAL contour
+ * exactly as the evaluation kernel makes them (double-double, correctly rounded), for the n rule nodes in
+ * d_nodes; tests compare them bit for bit with the oracle's. */
+int gf_diag_radial_map(double cutoff2, double map_scale, const double* d_nodes, int n, double* d_y, void* stream);
 
 const char* gf_last_error(void);
 const char* gf_version(void);

@@ -37,7 +37,9 @@
 // the wedge around the negative real axis and of REAL outside the parabola R2
 // (DESIGN.md "parity unpinned"), where no closed form applies.
 //
-// Build: g++ -O2 -std=c++17 -shared -fPIC -pthread (no -ffast-math).
+// Build: g++ -O2 -std=c++17 -shared -fPIC -pthread ... -lquadmath (no -ffast-math).
+
+#include <quadmath.h>
 
 #include <cmath>
 #include <complex>
@@ -262,12 +264,17 @@ Rule level(const double* nodes, const double* weights, int n_rad, int l) {
 
 // shifted-log map of a real segment [a,b] (readings G3/G4):
 //   y(u) = a + (a+s0) expm1(u L),  L = ln((b+s0)/(a+s0)),  dy/du = L (y+s0)
+// Node positions are evaluated in binary128 (libquadmath) and rounded once to double, like the
+// quadrature tables, which are made in extended precision: where the contour passes close to a
+// singularity of the integrand a 1-ulp difference of y_i (e.g. between two libm's expm1) changes
+// the sum by far more than 1e-11 (reading G18), so y_i must be THE correctly rounded value.
 void seg_logreal(double a, double b, double s0, cplx dir, Rule R, std::vector<RNode>& out) {
-  double L = std::log((b + s0) / (a + s0));
+  const __float128 as = (__float128)a + (__float128)s0;
+  const __float128 L = logq(((__float128)b + (__float128)s0) / as);
   for (int i = 0; i < R.n; ++i) {
     double u = 0.5 * (R.t[i] + 1.0);
-    double r = a + (a + s0) * std::expm1(u * L);
-    double dr = 0.5 * R.w[i] * L * (r + s0);
+    double r = (double)((__float128)a + as * expm1q((__float128)u * L));
+    double dr = (double)((__float128)(0.5 * R.w[i]) * L * ((__float128)r + (__float128)s0));
     RNode nd = { dir * r, dir * dr };
     out.push_back(nd);
   }

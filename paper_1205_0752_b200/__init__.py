@@ -43,8 +43,14 @@ class gf_params(ctypes.Structure):
 class gf_launch_info(ctypes.Structure):
     _fields_ = [("block_threads", ctypes.c_int), ("grid_blocks", ctypes.c_longlong), ("split", ctypes.c_int),
                 ("smem_bytes", ctypes.c_int), ("n_pairs", ctypes.c_int), ("n_terms", ctypes.c_int),
-                ("fp64_inst", ctypes.c_double), ("fp32_inst", ctypes.c_double), ("flops", ctypes.c_double),
-                ("evals", ctypes.c_double)]
+                ("far_terms_max", ctypes.c_int), ("evals", ctypes.c_double)] + [
+        (n, ctypes.c_double) for n in (
+            "near_pair_dfma", "near_pair_other", "near_pair_fp32", "far_term_dfma", "far_term_other",
+            "exact_pair_dfma", "exact_pair_other", "node_near_dfma", "node_near_other", "node_far_dfma",
+            "node_far_other", "node_exact_dfma", "node_exact_other")]
+
+
+COUNTER_NAMES = ("near_pairs", "far_terms", "exact_pairs", "near_nodes", "far_nodes", "exact_nodes")
 
 
 _lib = None
@@ -56,10 +62,12 @@ _SIGNATURES = {
     "gf_make_quadrature_host": [_int, _int, _dbl, _int, _vp, _vp],
     "gf_radial_table_size": [_int, _int],
     "gf_eval_grid": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
+    "gf_eval_grid_counted": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp, _vp],
     "gf_eval_grid_host": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
     "gf_eval_launch_info": [ctypes.POINTER(gf_params), _int, _int, _ll, ctypes.POINTER(gf_launch_info)],
     "gf_diag_fp64_peak": [_int, _int, _ll, _vp, _vp],
     "gf_diag_rcp_seed": [_vp, _vp, _ll, _vp],
+    "gf_diag_radial_map": [_dbl, _dbl, _vp, _int, _vp, _vp],
     "gf_last_error": [],
     "gf_version": [],
 }
@@ -201,9 +209,7 @@ def make_radial_tables_host(contour, n_rad, kind="gauss_legendre"):
     return np.concatenate(xs), np.concatenate(ws)
 
 
-def eval_grid(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out=None, stream=None):
-    """gf_eval_grid on device tensors.  x: complex128, any shape; returns complex128 (precision 64) or
-    complex64 (precision 32) of the same shape.  Asynchronous on the current stream."""
+def _eval_checks(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out):
     if not x.is_cuda:
         raise GfError(2, "eval_grid takes device tensors; use eval_grid_host for host buffers")
     assert x.dtype == torch.complex128 and x.is_contiguous()
@@ -216,11 +222,39 @@ def eval_grid(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, 
     if out is None:
         out = torch.empty(x.shape, dtype=odt, device=x.device)
     assert out.dtype == odt and out.is_contiguous() and out.numel() == x.numel()
+    return out
+
+
+def eval_grid(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out=None, stream=None):
+    """gf_eval_grid on device tensors.  x: complex128, any shape; returns complex128 (precision 64) or
+    complex64 (precision 32) of the same shape.  Asynchronous on the current stream."""
+    out = _eval_checks(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out)
     with torch.cuda.device(x.device):
         _check(lib().gf_eval_grid(ctypes.byref(params), rad_nodes.data_ptr(), rad_weights.data_ptr(), n_rad,
                                   ang_nodes.data_ptr(), ang_weights.data_ptr(), ang_nodes.numel(),
                                   x.data_ptr(), x.numel(), out.data_ptr(), _stream(stream)))
     return out
+
+
+def eval_grid_counted(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out=None, stream=None):
+    """gf_eval_grid_counted: (G, {route counter: value}).  Synchronises to read the counters."""
+    out = _eval_checks(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out)
+    counters = torch.zeros(len(COUNTER_NAMES), dtype=torch.int64, device=x.device)
+    with torch.cuda.device(x.device):
+        _check(lib().gf_eval_grid_counted(ctypes.byref(params), rad_nodes.data_ptr(), rad_weights.data_ptr(), n_rad,
+                                          ang_nodes.data_ptr(), ang_weights.data_ptr(), ang_nodes.numel(),
+                                          x.data_ptr(), x.numel(), out.data_ptr(), counters.data_ptr(),
+                                          _stream(stream)))
+    return out, dict(zip(COUNTER_NAMES, counters.cpu().tolist()))
+
+
+def executed_fp64(info, counters):
+    """(FP64-pipe thread-instructions, flops with FMA = 2) of one launch from its route counters."""
+    units = (("near_pair", "near_pairs"), ("far_term", "far_terms"), ("exact_pair", "exact_pairs"),
+             ("node_near", "near_nodes"), ("node_far", "far_nodes"), ("node_exact", "exact_nodes"))
+    inst = sum((info[u + "_dfma"] + info[u + "_other"]) * counters[c] for u, c in units)
+    flops = sum((2 * info[u + "_dfma"] + info[u + "_other"]) * counters[c] for u, c in units)
+    return float(inst), float(flops)
 
 
 def _host_ptr(a):
@@ -252,6 +286,12 @@ def launch_info(params, n_rad, n_ang, n_points):
 
 def diag_fp64_peak(blocks, threads, iters, sink, stream=None):
     _check(lib().gf_diag_fp64_peak(blocks, threads, iters, sink.data_ptr(), _stream(stream)))
+
+
+def diag_radial_map(cutoff2, map_scale, nodes, stream=None):
+    y = torch.empty_like(nodes)
+    _check(lib().gf_diag_radial_map(cutoff2, map_scale, nodes.data_ptr(), nodes.numel(), y.data_ptr(), _stream(stream)))
+    return y
 
 
 def diag_rcp_seed(x, stream=None):

@@ -11,7 +11,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libgf_b200.so")
 SOURCES = ["gf_api.cu", "gf_eval.cu", "gf_grid.cu", "gf_diag.cu", "gf_tables.cpp"]
-HEADERS = [os.path.join(CSRC, "gf_internal.h"), os.path.join(ROOT, "include", "gf.h")]
+HEADERS = [os.path.join(CSRC, "gf_internal.h"), os.path.join(CSRC, "gf_dd.cuh"), os.path.join(ROOT, "include", "gf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--threads", "4"]
 
@@ -38,7 +38,7 @@ def build(force=False, verbose=False):
     cmd = [_nvcc()] + NVCC_FLAGS + ["-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += [os.path.join(CSRC, s) for s in SOURCES]
+    cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-lquadmath"]
     subprocess.run(cmd, check=True)
     return LIB
 

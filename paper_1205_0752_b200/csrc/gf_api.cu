@@ -67,6 +67,7 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   a->cutoff2 = p->cutoff2;
   a->s0 = p->map_scale;
   a->c0 = p->prefactor;
+  log_ratio_dd(0.0, p->cutoff2, p->map_scale, &a->Llog_hi, &a->Llog_lo);  // REAL contour: [0, Lambda^2]
   a->contour = p->contour;
 
   // line 2 as a sum of simple poles R_r/(u + mu_r)
@@ -171,9 +172,9 @@ int gf_make_quadrature(int kind, int n, double step, int measure, double* d_node
 
 long long gf_radial_table_size(int contour, int n_rad) { return radial_table_size(contour, n_rad); }
 
-int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
-                 const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
-                 long long n_points, void* d_out, void* stream) {
+static int eval_grid_impl(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                          const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
+                          long long n_points, void* d_out, unsigned long long* d_counters, void* stream) {
   EvalArgs a;
   int rc = build_args(p, n_rad, n_ang, n_points, &a);
   if (rc) return rc;
@@ -185,7 +186,22 @@ int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_
   a.ang_weights = d_ang_weights;
   a.x = static_cast<const double2*>(d_x);
   a.out = d_out;
-  return launch_eval(a, p->precision, static_cast<cudaStream_t>(stream));
+  return launch_eval(a, p->precision, d_counters, static_cast<cudaStream_t>(stream));
+}
+
+int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                 const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
+                 long long n_points, void* d_out, void* stream) {
+  return eval_grid_impl(p, d_rad_nodes, d_rad_weights, n_rad, d_ang_nodes, d_ang_weights, n_ang, d_x, n_points,
+                        d_out, nullptr, stream);
+}
+
+int gf_eval_grid_counted(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                         const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
+                         long long n_points, void* d_out, unsigned long long* d_counters, void* stream) {
+  if (!d_counters) { set_error("eval_grid_counted: d_counters is null"); return GF_ERR_NULL; }
+  return eval_grid_impl(p, d_rad_nodes, d_rad_weights, n_rad, d_ang_nodes, d_ang_weights, n_ang, d_x, n_points,
+                        d_out, d_counters, stream);
 }
 
 int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const double* h_rad_weights, int n_rad,
@@ -224,7 +240,7 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
     a.rad_nodes = d_rn; a.rad_weights = d_rw; a.ang_nodes = d_an; a.ang_weights = d_aw;
     a.x = reinterpret_cast<const double2*>(d + off_x);
     a.out = d + off_out;
-    rc = launch_eval(a, p->precision, s);
+    rc = launch_eval(a, p->precision, nullptr, s);
   }
   if (!rc) rc = check_cuda(cudaMemcpyAsync(h_out, d + off_out, out_bytes, cudaMemcpyDeviceToHost, s), "device->host copy");
   cudaFreeAsync(d, s);
@@ -245,8 +261,18 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
   out->smem_bytes = (int)plan.smem_bytes;
   out->n_pairs = a.n_pairs;
   out->n_terms = a.n_terms;
-  eval_inst_counts(a, p->precision, plan, &out->fp64_inst, &out->fp32_inst, &out->flops);
+  out->far_terms_max = plan.layout.km;
   out->evals = (double)n_points * n_rad * n_ang;
+  // FP64-pipe instructions per unit of each route, read off the SASS of gf_eval.cu (DESIGN.md "Instruction
+  // counts"): NEAR pair 5 DFMA + 1 DMUL + 2 DADD; FAR term 6 DFMA + 2 DMUL; EXACT pair 4 DFMA + 2 DMUL +
+  // 3 DADD + a full-precision division (8 DFMA + 1 DMUL); per node-term: set-up and finish of each route.
+  const bool f32 = p->precision == 32;
+  out->near_pair_dfma = f32 ? 0 : 5; out->near_pair_other = f32 ? 0 : 3; out->near_pair_fp32 = f32 ? 5 : 0;
+  out->far_term_dfma = 6; out->far_term_other = 2;
+  out->exact_pair_dfma = 12; out->exact_pair_other = 6;
+  out->node_near_dfma = 10; out->node_near_other = 14;
+  out->node_far_dfma = 16; out->node_far_other = 18;
+  out->node_exact_dfma = 120; out->node_exact_other = 180;
   return GF_OK;
 }
 
@@ -254,6 +280,14 @@ int gf_diag_fp64_peak(int blocks, int threads, long long iters, double* d_sink, 
   if (!d_sink) { set_error("diag_fp64_peak: d_sink is null"); return GF_ERR_NULL; }
   if (blocks < 1 || threads < 1 || threads > 1024 || iters < 0) { set_error("diag_fp64_peak: bad launch shape"); return GF_ERR_ARG; }
   return launch_fp64_peak(blocks, threads, iters, d_sink, static_cast<cudaStream_t>(stream));
+}
+
+int gf_diag_radial_map(double cutoff2, double map_scale, const double* d_nodes, int n, double* d_y, void* stream) {
+  if (!d_nodes || !d_y) { set_error("diag_radial_map: null pointer"); return GF_ERR_NULL; }
+  if (n < 1 || !(cutoff2 > 0) || !(map_scale > 0)) { set_error("diag_radial_map: bad argument"); return GF_ERR_ARG; }
+  double hi, lo;
+  log_ratio_dd(0.0, cutoff2, map_scale, &hi, &lo);
+  return launch_radial_map(hi, lo, map_scale, d_nodes, n, d_y, static_cast<cudaStream_t>(stream));
 }
 
 int gf_diag_rcp_seed(const double* d_in, double* d_out, long long n, void* stream) {

@@ -31,10 +31,24 @@ struct EvalArgs {
   PoleTerm term[kMaxTerms];
   gf_propagator line_k;
   double cutoff2, s0, c0;
+  double Llog_hi, Llog_lo;  // ln((Lambda^2 + s0)/s0) as a double-double (host, binary128)
   double line2_scale;  // |m2^2| or the largest pole modulus: sizes the deformed contours
   int contour;         // gf_contour
   int thread_ok;       // THREAD applicable (equal real masses)
   int split_log2;      // lanes per grid point = 1 << split_log2
+};
+
+// Offsets (in doubles) of the prepared tables, as the preparation kernel writes them and every CTA of the
+// evaluation kernel copies them to shared memory (one 16-byte header first).
+struct BlobLayout {
+  int npad;                     // n_pairs rounded up to 4
+  int km;                       // far-field moments mu_0..mu_{km-1}, nu_0..nu_{km-1}
+  int off_t, off_tlo, off_w;    // folded angular rule: t = z^2 (hi, lo), weight
+  int off_mu, off_nu;
+  int off_y, off_q4;            // radial nodes y_i, 1/(4 y_i)
+  int off_pref;                 // double2 pref[n_terms][n_rad]
+  int off_f32;                  // float t[npad], w[npad] (FP32 variant) or -1
+  int n_doubles;                // total, even
 };
 
 struct LaunchPlan {
@@ -42,7 +56,8 @@ struct LaunchPlan {
   long long grid_blocks;
   int split_log2;
   size_t smem_bytes;
-  bool shared_nodes;  // REAL: per-node tables staged once per CTA
+  bool shared_nodes;  // REAL: per-node tables prepared once per launch
+  BlobLayout layout;
 };
 
 // host-side helpers (gf_api.cu)
@@ -51,6 +66,7 @@ int check_cuda(cudaError_t e, const char* what);
 
 // gf_tables.cpp
 int make_rule_host(int kind, int n, double step, int measure, double* nodes, double* weights);
+void log_ratio_dd(double a, double b, double s0, double* hi, double* lo);  // ln((b+s0)/(a+s0)), binary128 -> (hi, lo)
 
 // gf_grid.cu
 int launch_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
@@ -59,9 +75,9 @@ int launch_make_grid(double re_min, double re_max, int n_re, double im_min, doub
 
 // gf_eval.cu
 int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan);
-int launch_eval(const EvalArgs& a, int precision, cudaStream_t stream);
-void eval_inst_counts(const EvalArgs& a, int precision, const LaunchPlan& plan, double* fp64_inst,
-                      double* fp32_inst, double* flops);
+int launch_eval(const EvalArgs& a, int precision, unsigned long long* d_counters, cudaStream_t stream);
+int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d_nodes, int n, double* d_y,
+                      cudaStream_t stream);
 
 // gf_diag.cu
 int launch_fp64_peak(int blocks, int threads, long long iters, double* d_sink, cudaStream_t stream);

@@ -1,6 +1,8 @@
 // gf_tables.cpp -- host-side generation of the quadrature tables (row a2 of the hot-path table;
 // the paper's "Preparation": nodes and weights are calculated on the host).
 // Library code; shares nothing with oracle/.
+#include <quadmath.h>
+
 #include <cmath>
 #include <vector>
 
@@ -58,6 +60,15 @@ void gauss_legendre(int n, double* x, double* w) {
 }
 
 }  // namespace
+
+// L = ln((b + s0)/(a + s0)) of the shifted-log map of a real segment [a, b] (readings G3/G4), in binary128,
+// split into a double-double.  The map's node positions must not depend on a libm's last bit (DESIGN.md
+// reading G18), so L carries ~106 bits.
+void log_ratio_dd(double a, double b, double s0, double* hi, double* lo) {
+  const __float128 L = logq(((__float128)b + (__float128)s0) / ((__float128)a + (__float128)s0));
+  *hi = (double)L;
+  *lo = (double)(L - (__float128)*hi);
+}
 
 int make_rule_host(int kind, int n, double step, int measure, double* nodes, double* weights) {
   if (!nodes || !weights) { set_error("make_quadrature: null table pointer"); return GF_ERR_NULL; }

@@ -63,7 +63,8 @@ def oracle_grid(O, cfg):
 
 def oracle_eval(O, cfg, xs, contour="real", ang=None):
     P, rn, rw, z, wz = oracle_setup(O, cfg, contour, ang)
-    g, _ = O.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, xs)
+    # the parity variant: every term in long double (reading G18)
+    g, _ = O.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, xs, accum="extended")
     return g
 
 
@@ -96,6 +97,23 @@ def test_tables_match_oracle(gf, oracle, kind, n, measure):
     assert np.max(np.abs(wg - wo) / np.abs(wo)) <= 64 * np.finfo(float).eps
     xh, wh = gf.make_quadrature_host(kind, n, measure=measure)
     assert np.array_equal(xh, xg) and np.array_equal(wh, wg)
+
+
+def test_radial_map_bit_identical(gf, oracle):
+    """The REAL contour's nodes y_i = s0 expm1(u_i L): kernel (double-double) vs oracle (binary128), bit
+    for bit -- next to a singularity of the integrand a 1-ulp difference of y_i moves G by more than
+    1e-11 (reading G18)."""
+    for n_rad, cutoff2, s0 in [(64, 1e4, 1.0), (256, 1e6, 1.0), (512, 1e6, 1.0), (1024, 1e6, 1.0), (100, 3.7e8, 0.25),
+                               (33, 10.0, 2.0)]:
+        t, w = gf.make_quadrature("gauss_legendre", n_rad)
+        y = gf.diag_radial_map(cutoff2, s0, t).cpu().numpy()
+        bub = {"kind": "massive", "m2": 1.0}
+        P = oracle.make_params(bub, bub, cutoff2, map_scale=s0)
+        to, wo = oracle.make_quadrature("gauss_legendre", n_rad)
+        assert np.array_equal(to, t.cpu().numpy())
+        _, yo, _ = oracle.contour_nodes(P, 1.0 + 1.0j, to, wo, n_rad, 32)
+        assert np.array_equal(yo.imag, np.zeros(n_rad))
+        assert np.array_equal(yo.real, y), (n_rad, int((yo.real != y).sum()))
 
 
 # ------------------------------------------------------------------ a3-a6: evaluation, REAL contour
@@ -179,6 +197,21 @@ def test_ragged_point_counts(gf, oracle, n_points):
     keep = slice(None) if n_points <= 4097 else slice(None, None, 37)
     ref = oracle_eval(oracle, cfg, xs[keep])
     assert relerr(g[keep], ref).max() <= TOL64
+
+
+def test_route_counters(gf):
+    """Every (point, node, pole) triple takes exactly one route; the counted call returns the same G."""
+    cfg = W.CONFIGS["cfg2_mid"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+    g2, c = gf.eval_grid_counted(P, rn, rw, cfg["n_rad"], z, wz, x)
+    assert torch.equal(g.view(torch.float64), g2.view(torch.float64))
+    n_pairs = cfg["n_ang"] // 2
+    assert c["near_nodes"] + c["far_nodes"] + c["exact_nodes"] == x.numel() * cfg["n_rad"]
+    assert c["near_pairs"] == c["near_nodes"] * n_pairs and c["exact_pairs"] == c["exact_nodes"] * n_pairs
+    assert 2 * c["far_nodes"] <= c["far_terms"] <= 59 * c["far_nodes"]
+    assert 0 < c["exact_nodes"] < 1e-2 * c["near_nodes"] and c["far_nodes"] > c["near_nodes"]
 
 
 def test_empty_input(gf):
