@@ -260,6 +260,15 @@ def run_ours(args):
     checksum = out.view(torch.float64).abs().sum().item()
     assert np.isfinite(checksum) and checksum > 0
 
+    # ---- executed FP64 work of one launch: the kernel's own route counters (an untimed, counted launch
+    #      with identical results) x the per-unit instruction counts of the SASS (gf_eval_launch_info)
+    rn_c, rw_c = gf.make_radial_tables("real", n_rad, W.RADIAL_RULE)
+    z_c, wz_c = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    out_c, counters = gf.eval_grid_counted(P, rn_c, rw_c, n_rad, z_c, wz_c, x)
+    assert torch.equal(out_c.view(torch.float64), out.view(torch.float64)), "counted launch differs"
+    fp64_inst, fp64_flops = gf.executed_fp64(info, counters)
+    del out_c
+
     # ---- e2e: the host-buffer entry point, copies inside the timed region
     xh = x.cpu().pin_memory()
     outh = torch.empty(xh.shape, dtype=torch.complex128).pin_memory()
@@ -307,7 +316,7 @@ def run_ours(args):
 
     sm_max = clocks["sm_max_mhz"] or 1965.0
     peak_nominal = 2.0 * FP64_LANES_PER_SM * N_SM * sm_max * 1e6 / 1e12
-    achieved = info["flops"] / (kernel_ms * 1e-3) / 1e12
+    achieved = fp64_flops / (kernel_ms * 1e-3) / 1e12
     n_points_job = n_points_local * world
     value = n_points_job * args.steps / (ms_total * 1e-3)
     line = {
@@ -317,16 +326,16 @@ def run_ours(args):
         "evals_per_s": value * n_rad * n_ang,
         "e2e": {"value": n_points_job * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
                 "h2d_bytes_per_step": h2d * world, "d2h_bytes_per_step": d2h * world},
-        "gpu_launches": 2 * args.steps,
+        "gpu_launches": 3 * args.steps,  # make_grid, prep_real, eval_real per step
         "launch": {"kernel": "eval_real_kernel<double>", "grid_blocks": info["grid_blocks"],
                    "block_threads": info["block_threads"], "smem_bytes": info["smem_bytes"], "lanes_per_point": info["split"]},
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                      "frac": achieved / peak_nominal, "traffic": EVAL_KERNEL_DRAM_TRAFFIC_BYTES,
                      "peak_kind": "derived: %d SMs x %d FP64 lanes x 2 x %.0f MHz (DESIGN.md)" % (N_SM, FP64_LANES_PER_SM, sm_max),
                      "peak_measured_dfma": dfma_tflops, "frac_of_measured_dfma": achieved / dfma_tflops,
-                     "kernel_ms": kernel_ms, "flops_per_launch": info["flops"],
-                     "fp64_inst_per_launch": info["fp64_inst"],
-                     "fp64_pipe_frac": info["fp64_inst"] / (kernel_ms * 1e-3) / (FP64_LANES_PER_SM * N_SM * sm_max * 1e6),
+                     "kernel_ms": kernel_ms, "flops_per_launch": fp64_flops,
+                     "fp64_inst_per_launch": fp64_inst, "routes": counters,
+                     "fp64_pipe_frac": fp64_inst / (kernel_ms * 1e-3) / (FP64_LANES_PER_SM * N_SM * sm_max * 1e6),
                      "kernel_share_of_step": kernel_ms * args.steps / ms_total},
         "clocks": clocks,
     }

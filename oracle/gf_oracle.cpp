@@ -27,7 +27,10 @@
 // std::complex<long double> as well: at the rare points where the contour passes
 // within ~1e-5 of a singularity of the integrand, and at tiny |x| where the +-z
 // terms cancel to O(sqrt|x|), double terms are themselves only good to ~1e-11
-// (reading G18).  No blocking, pairing, fusion or reordering.
+// (reading G18); below |x| = 2^-10 it runs them in binary128, because there the +-z
+// terms cancel by a factor 2 sqrt(y/|x|).  Domain of the parity variant: x = 0 or |x| >~ 1e-30
+// (below that no fixed-width type can form the plain sum; tests use tests/mp_reference.py, the
+// same sum at 400 digits).  No blocking, pairing, fusion or reordering.
 //
 // Pins (tests/test_oracle_pins.py): closed form CF1 of the equal-mass bubble,
 // the paper's eq. (18) for masses^2 = +-i/2, the Feynman-parameter form CF3 for
@@ -362,6 +365,18 @@ int auto_policy(const Params& P, cplx x, int n_ang) {
   return CONTOUR_REAL;
 }
 
+// principal square root in the term type (libstdc++ has no std::sqrt for complex<__float128>)
+template <typename R>
+std::complex<R> psqrt(std::complex<R> v) { return std::sqrt(v); }
+template <>
+std::complex<__float128> psqrt(std::complex<__float128> v) {
+  __complex128 c;
+  __real__ c = v.real();
+  __imag__ c = v.imag();
+  c = csqrtq(c);
+  return std::complex<__float128>(__real__ c, __imag__ c);
+}
+
 // ---- Step 5 / Kernel 2: the double sum for one x ---------------------------
 // ACC: type of the two running sums; R: type every term is evaluated in.
 template <typename ACC, typename R>
@@ -375,12 +390,12 @@ cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int
   else contour_thread(P, x, rn, rw, n_rad, nodes);
 
   C xx((R)x.real(), (R)x.imag());
-  C sx = std::sqrt(xx);  // principal branch
+  C sx = psqrt<R>(xx);  // principal branch
   ACC gr = 0, gi = 0;
   for (size_t i = 0; i < nodes.size(); ++i) {
     C y((R)nodes[i].y.real(), (R)nodes[i].y.imag());
     C wy((R)nodes[i].wy.real(), (R)nodes[i].wy.imag());
-    C B = (R)2 * sx * std::sqrt(y);
+    C B = (R)2 * sx * psqrt<R>(y);
     C D1 = prop<R>(P.line_k, y);
     ACC sr = 0, si = 0;
     for (int j = 0; j < n_ang; ++j) {
@@ -421,8 +436,12 @@ int gfo_make_grid(double re_min, double re_max, int n_re, double im_min, double 
 }
 
 // x, out: interleaved (re, im) doubles.  accum: 0 = double terms, long double sums;
-// 1 = double terms and sums (the timed variant); 2 = long double terms and sums (the
-// parity variant: own rounding error << 1e-11 at every point, reading G18).  n_threads <= 0: hardware concurrency.
+// 1 = double terms and sums (the timed variant); 2 = the parity variant, whose own rounding error
+// is << 1e-11 at every point (reading G18): long double terms and sums, and binary128 (libquadmath)
+// terms and sums where |x| < 2^-10 -- there the +-z terms, each O(sqrt|x y|), cancel to O(|x|), which
+// costs even long double a factor 2 sqrt(y/|x|) (measured against a 60-digit evaluation of the same
+// sum: 7e-9 at |x| = 1e-16); 3 = binary128 everywhere (slow; checks variant 2).
+// n_threads <= 0: hardware concurrency.
 // Returns 0 on success; fills *threads_used.
 int gfo_eval_grid(const void* params, const double* rad_nodes, const double* rad_weights, int n_rad,
                   const double* ang_nodes, const double* ang_weights, int n_ang, const double* x,
@@ -448,7 +467,10 @@ int gfo_eval_grid(const void* params, const double* rad_nodes, const double* rad
                    ? eval_point<ld, double>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
                : accum == 1
                    ? eval_point<double, double>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
-                   : eval_point<ld, ld>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes);
+               : (accum == 2 && std::fmax(std::fabs(xx.real()), std::fabs(xx.imag())) >= 0x1p-10)
+                   ? eval_point<ld, ld>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
+                   : eval_point<__float128, __float128>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights,
+                                                        n_ang, nodes);
       out[2 * p] = g.real();
       out[2 * p + 1] = g.imag();
     }

@@ -24,8 +24,9 @@ PROP = {"massive": 0, "rational": 1}
 CONTOUR = {"real": 0, "ray_arc": 1, "thread": 2, "auto": 3}
 SPACING = {"uniform": 0, "log_abs_im": 1}
 # arithmetic variants of gfo_eval_grid: double terms + long double sums; all double (timed);
-# long double terms and sums (parity: own rounding error << 1e-11 everywhere, reading G18)
-ACCUM = {"long_double": 0, "double": 1, "extended": 2}
+# long double terms and sums, binary128 for |x| < 2^-10 (parity: own rounding error << 1e-11
+# everywhere, reading G18); binary128 everywhere (slow, checks "extended")
+ACCUM = {"long_double": 0, "double": 1, "extended": 2, "quad": 3}
 
 
 class _Prop(ctypes.Structure):

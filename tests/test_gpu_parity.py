@@ -211,7 +211,7 @@ def test_route_counters(gf):
     assert c["near_nodes"] + c["far_nodes"] + c["exact_nodes"] == x.numel() * cfg["n_rad"]
     assert c["near_pairs"] == c["near_nodes"] * n_pairs and c["exact_pairs"] == c["exact_nodes"] * n_pairs
     assert 2 * c["far_nodes"] <= c["far_terms"] <= 59 * c["far_nodes"]
-    assert 0 < c["exact_nodes"] < 1e-2 * c["near_nodes"] and c["far_nodes"] > c["near_nodes"]
+    assert 0 < c["exact_nodes"] < 5e-2 * c["near_nodes"] and c["far_nodes"] > c["near_nodes"]
 
 
 def test_empty_input(gf):
@@ -230,6 +230,12 @@ def test_degenerate_points(gf, oracle):
     P, rn, rw, z, wz = gpu_setup(gf, cfg)
     g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
     ref = oracle_eval(oracle, cfg, xs)
+    # below |x| ~ 1e-30 no fixed-width arithmetic can form the plain sum (the +-z terms cancel by
+    # 2 sqrt(y/|x|)): the reference there is the same sum at 400 digits (tests/mp_reference.py)
+    from tests import mp_reference as MPR
+    Po, rno, rwo, zo, wzo = oracle_setup(oracle, cfg)
+    for k in np.nonzero((np.abs(xs) < 1e-30) & (xs != 0))[0]:
+        ref[k] = MPR.finite_sum(oracle, Po, xs[k], rno, rwo, cfg["n_rad"], zo, wzo, digits=400)
     assert g[0] == 0 and ref[0] == 0
     e = relerr(g, ref)
     assert e.max() <= TOL64, (e.max(), xs[e.argmax()])

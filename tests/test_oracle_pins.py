@@ -14,6 +14,7 @@ import pytest
 
 import gf_workloads as W
 from tests import closed_forms as CF
+from tests import mp_reference as MPR
 
 BUB = {"kind": "massive", "m2": 1.0}
 RAT = {"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2}
@@ -317,6 +318,22 @@ def test_accum_variants_agree(oracle):
     g_ld, _ = oracle.eval_grid(P, rn, rw, 256, z, wz, xs, accum="long_double")
     g_d, _ = oracle.eval_grid(P, rn, rw, 256, z, wz, xs, accum="double", n_threads=2)
     assert np.max(relerr(g_d, g_ld)) < 1e-12
+
+
+@pytest.mark.parametrize("x", [5.551115123125783e-17 + 1.1102230246251565e-16j, 1e-9 - 3e-10j, -7e-4 + 2e-4j,
+                               1.2e-3 + 0j, 0.3 - 0.1j, -1.3112 - 1.6986j])
+def test_parity_variant_rounding_error_is_negligible(oracle, x):
+    """Reading G18: the variant GPU parity is measured against carries << 1e-11 of its own error, also
+    at tiny |x| (where the +-z terms cancel; binary128 below |x| = 2^-10) and next to a zero of a
+    denominator (x = -1.3112 - 1.6986i, outside the parabola R2)."""
+    P = oracle.make_params(BUB, BUB, 1e4)
+    rn, rw = oracle.make_quadrature("gauss_legendre", 24)
+    z, wz = oracle.make_quadrature("gauss_cheb2", 33, measure="sqrt1mz2")
+    ref = MPR.finite_sum(oracle, P, x, rn, rw, 24, z, wz, digits=60)
+    g, _ = oracle.eval_grid(P, rn, rw, 24, z, wz, np.array([x]), accum="extended")
+    assert relerr(g, [ref])[0] < 2e-14
+    gq, _ = oracle.eval_grid(P, rn, rw, 24, z, wz, np.array([x]), accum="quad")
+    assert relerr(gq, [ref])[0] < 1e-15
 
 
 # ---------------------------------------------------------------- contours (a3)
