@@ -41,7 +41,7 @@ FP64_LANES_PER_SM = 64
 N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of one eval kernel launch on cfg3 (profiles/, ncu --set full);
 # None until a capture is committed
-EVAL_KERNEL_DRAM_TRAFFIC_BYTES = None
+EVAL_KERNEL_DRAM_TRAFFIC_BYTES = 95.5e6  # r01b: 69.2 MB read + 26.3 MB written
 
 
 def dist_env():
