@@ -27,7 +27,7 @@
  *   - Errors: GF_ERR_NULL for a null pointer, GF_ERR_ARG for a value out of range,
  *     GF_ERR_UNSUPPORTED for a combination the method does not define (taylor_order != 0, a
  *     subtraction point other than 0, the THREAD contour with unequal or complex masses, a
- *     rational propagator with a double pole), GF_ERR_CUDA when the CUDA runtime reports an
+ *     rational propagator with a double pole, precision 32 on a contour other than REAL), GF_ERR_CUDA when the CUDA runtime reports an
  *     error (no device, launch failure).  gf_last_error() describes the last failure of the
  *     calling thread.  A denominator that vanishes at a quadrature node yields IEEE inf/NaN in
  *     that output entry, not an error (the paper has no convention).
@@ -66,7 +66,17 @@ typedef struct {
  *            region-2/5 contour);
  *   THREAD   polyline through the opening of the cut for Re x < -4 m^2 next to the negative
  *            axis, equal real masses only (analogue of the region-3/4 contours);
- *   AUTO     per-point choice among the three. */
+ *   AUTO     per-point choice among the three.
+ * With sc = |m2^2| of line 2 (largest pole modulus for a rational line), phi = arg x:
+ *   RAY_ARC  = ray r e^{i phi}, r in [0,R] shifted-log, n_rad/2 nodes; arc R e^{i theta}, theta: phi -> 0,
+ *              n_rad/4; real [R, Lambda^2] shifted-log, n_rad/4; R = min(1.5 (sqrt|x| + sqrt(|x|+sc))^2, Lambda^2/2).
+ *   THREAD   (Im x >= 0, mirrored otherwise; s = |x|, |A| = (sqrt s - m)^2, |B| = (sqrt s + m)^2, r0 = |x + m^2|)
+ *              straight pieces 0 -> -m^2 + i(|A|-m^2)/2 -> (|A|+m^2)/2 e^{i phi} -> -(|A|+r0)/2 - i(r0-|A|)/2
+ *              -> r0 e^{i phi} -> R e^{3 pi i/4}, arc to R, n_rad/8 nodes each; real [R, Lambda^2], n_rad/4;
+ *              R = min(1.5 |B|, Lambda^2/2).
+ *   AUTO     wedge W = {Re x < -sc, |Im x| n_ang sc < 5 |x|^2}: outside W RAY_ARC; inside W THREAD if it
+ *              applies and Re x <= -4.1 sc, else REAL.
+ * Every piece carries the Gauss-Legendre rule of its order from the pyramid of gf_radial_table_size(). */
 typedef enum { GF_CONTOUR_REAL = 0, GF_CONTOUR_RAY_ARC = 1, GF_CONTOUR_THREAD = 2, GF_CONTOUR_AUTO = 3 } gf_contour;
 
 typedef enum { GF_SPACING_UNIFORM = 0, GF_SPACING_LOG_ABS_IM = 1 } gf_spacing;
@@ -125,7 +135,7 @@ long long gf_radial_table_size(int contour, int n_rad);
  *                              (z[n-1-j] = -z[j], equal weights): the kernel folds +-z pairs.  A rule
  *                              that is not makes every output NaN.
  *   d_x      n_points complex<double>
- *   d_out    n_points complex<double> (precision 64) or complex<float> (precision 32)
+ *   d_out    n_points complex<double> (precision 64) or complex<float> (precision 32; REAL contour only)
  * Domain: x = 0 gives exactly 0; |x| up to 1e100.  Asynchronous on `stream`; n_points = 0 is a no-op. */
 int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
                  const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,

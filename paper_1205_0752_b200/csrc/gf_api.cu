@@ -69,6 +69,9 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   a->c0 = p->prefactor;
   log_ratio_dd(0.0, p->cutoff2, p->map_scale, &a->Llog_hi, &a->Llog_lo);  // REAL contour: [0, Lambda^2]
   a->contour = p->contour;
+  a->th5 = 0.75 * 3.14159265358979323846;  // 3 pi/4, correctly rounded
+  a->cos_th5 = std::cos(a->th5);
+  a->sin_th5 = std::sin(a->th5);
 
   // line 2 as a sum of simple poles R_r/(u + mu_r)
   const gf_propagator& q = p->line_pk;
@@ -89,7 +92,10 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
     a->n_terms = 2;
     a->term[0] = PoleTerm{R1.real(), R1.imag(), -u1.real(), -u1.imag()};
     a->term[1] = PoleTerm{R2.real(), R2.imag(), -u2.real(), -u2.imag()};
-    a->line2_scale = std::fmax(std::abs(u1), std::abs(u2));
+    // size of the singular structure of line 2 in the y-plane, the largest pole modulus: sqrt(b) for a
+    // complex-conjugate pair (|u_r|^2 = b), else max |(-a +- sqrt(disc))/2|
+    a->line2_scale = disc < 0 ? std::sqrt(q.b)
+                              : std::fmax(std::fabs(-q.a + std::sqrt(disc)), std::fabs(-q.a - std::sqrt(disc))) / 2.0;
   }
   a->thread_ok = p->line_k.kind == GF_PROP_MASSIVE && q.kind == GF_PROP_MASSIVE && p->line_k.m2_im == 0 &&
                  q.m2_im == 0 && p->line_k.m2_re == q.m2_re && q.m2_re > 0;

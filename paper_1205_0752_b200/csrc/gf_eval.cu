@@ -43,207 +43,10 @@
 
 #include "gf_dd.cuh"
 #include "gf_internal.h"
+#include "gf_routes.cuh"
 
 namespace gf {
 namespace {
-
-constexpr int kKmCap = 60;           // most far-field terms ever used (|zeta| >= 2 -> K <= 59)
-constexpr int kFarBits = 116;        // 2 * 58: K = kFarBits / (2 ilogb|zeta|) + 1
-constexpr double kTau64 = 0x1p-8;    // EXACT route inside this distance of [0,1] (FP64)
-constexpr double kTau32 = 0x1p-4;    // the FP32 variant's NEAR loop is only good further away
-
-struct cd {
-  double re, im;
-};
-__device__ __forceinline__ cd cmul(cd a, cd b) {
-  return {fma(a.re, b.re, -(a.im * b.im)), fma(a.re, b.im, a.im * b.re)};
-}
-__device__ __forceinline__ cd cscale(cd a, double s) { return {a.re * s, a.im * s}; }
-__device__ __forceinline__ cd cinv(cd a) {
-  // set-up code only (once per point / node): plain division, scaled against overflow
-  const double m = fmax(fabs(a.re), fabs(a.im));
-  const double ar = a.re / m, ai = a.im / m;
-  const double d = 1.0 / (m * fma(ar, ar, ai * ai));
-  return {ar * d, -ai * d};
-}
-
-__device__ __forceinline__ double rcp_seed(double s) {
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));  // MUFU.RCP64H
-  return r;
-}
-__device__ __forceinline__ float rcp_seed(float s) {
-  float r;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s));  // MUFU.RCP
-  return r;
-}
-
-// ---- 1-D TMA: one bulk copy global -> shared, completion on an mbarrier ------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                   smem_u32(dst)),
-               "l"(src), "r"(bytes), "r"(smem_u32(bar))
-               : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
-  uint32_t done = 0;
-  for (long long spin = 0; !done; ++spin) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done)
-        : "r"(smem_u32(bar)), "r"(phase)
-        : "memory");
-    if (spin > (1LL << 26)) __trap();  // a 20 KB copy that has not landed after seconds: fail, do not hang
-  }
-}
-
-// ---- NEAR: one folded angular pair: q = w/|zeta - t|^2 and the two sums ---------------------------
-__device__ __forceinline__ void pair_step(double zr, double zi2, double t, double w, double& u0, double& u1) {
-  const double a = zr - t;              // DADD
-  const double s = fma(a, a, zi2);      // DFMA  |zeta - t|^2
-  const double r0 = rcp_seed(s);        // MUFU.RCP64H
-  const double e = fma(-s, r0, 1.0);    // DFMA
-  const double p = fma(e, e, e);        // DFMA  e + e^2
-  const double v = r0 * w;              // DMUL
-  const double q = fma(v, p, v);        // DFMA  w/s (1 - e^3)
-  u0 += q;                              // DADD
-  u1 = fma(q, t, u1);                   // DFMA
-}
-__device__ __forceinline__ void pair_step(float zr, float zi2, float t, float w, float& u0, float& u1) {
-  const float a = zr - t;
-  const float s = fmaf(a, a, zi2);
-  const float q = w * rcp_seed(s);
-  u0 += q;
-  u1 = fmaf(q, t, u1);
-}
-
-template <typename T>
-struct Vec2;
-template <>
-struct Vec2<double> { typedef double2 type; };
-template <>
-struct Vec2<float> { typedef float2 type; };
-
-// S = mu0 - (zeta - eta)(conj(zeta) U0 - U1).  Two independent accumulator sets (even / odd pairs).
-template <typename T>
-__device__ __forceinline__ cd angular_near(cd eta, cd zeta, double mu0, const T* __restrict__ st,
-                                           const T* __restrict__ sw, int n_pairs) {
-  typedef typename Vec2<T>::type V2;
-  const T zr = (T)zeta.re;
-  const T zi2 = (T)(zeta.im * zeta.im);
-  T a0 = 0, a1 = 0, b0 = 0, b1 = 0;
-  int j = 0;
-#pragma unroll 1
-  for (; j + 4 <= n_pairs; j += 4) {
-    const V2 t01 = *reinterpret_cast<const V2*>(st + j), t23 = *reinterpret_cast<const V2*>(st + j + 2);
-    const V2 w01 = *reinterpret_cast<const V2*>(sw + j), w23 = *reinterpret_cast<const V2*>(sw + j + 2);
-    pair_step(zr, zi2, t01.x, w01.x, a0, a1);
-    pair_step(zr, zi2, t01.y, w01.y, b0, b1);
-    pair_step(zr, zi2, t23.x, w23.x, a0, a1);
-    pair_step(zr, zi2, t23.y, w23.y, b0, b1);
-  }
-  for (; j < n_pairs; ++j) pair_step(zr, zi2, st[j], sw[j], a0, a1);
-  const double u0 = (double)a0 + (double)b0, u1 = (double)a1 + (double)b1;
-  const double cr = fma(zeta.re, u0, -u1), ci = -zeta.im * u0;  // conj(zeta) U0 - U1
-  const double dr = zeta.re - eta.re, di = zeta.im - eta.im;
-  cd s;
-  s.re = mu0 - fma(dr, cr, -(di * ci));
-  s.im = -fma(dr, ci, di * cr);
-  return s;
-}
-
-// FAR: S = omega [ delta P(omega) + N(omega) ], K terms (Horner from the top).
-__device__ __forceinline__ cd angular_far(cd delta, cd zeta, int K, const double* __restrict__ smu,
-                                          const double* __restrict__ snu) {
-  const cd om = cinv(zeta);
-  double pr = smu[K - 1], pi = 0.0, nr = snu[K - 1], ni = 0.0;
-#pragma unroll 1
-  for (int k = K - 2; k >= 0; --k) {
-    const double m = smu[k], n = snu[k];
-    const double tpr = fma(pr, om.re, fma(-pi, om.im, m));
-    pi = fma(pr, om.im, pi * om.re);
-    pr = tpr;
-    const double tnr = fma(nr, om.re, fma(-ni, om.im, n));
-    ni = fma(nr, om.im, ni * om.re);
-    nr = tnr;
-  }
-  const cd acc = {fma(delta.re, pr, fma(-delta.im, pi, nr)), fma(delta.re, pi, fma(delta.im, pr, ni))};
-  return cmul(om, acc);
-}
-
-// EXACT: zeta = A^2/(4 x y) in double-double, A = x + y + mu; every term formed directly.
-__device__ __noinline__ cd angular_exact(double xr, double xi, double y, double mur, double mui, cd eta,
-                                         const double* __restrict__ st, const double* __restrict__ stlo,
-                                         const double* __restrict__ sw, int n_pairs) {
-  const dd Ar = dd_add_d(two_sum(xr, mur), y), Ai = two_sum(xi, mui);
-  const dd A2r = dd_add(dd_mul(Ar, Ar), dd_neg(dd_mul(Ai, Ai)));
-  const dd A2i = dd_scale2(dd_mul(Ar, Ai), 2.0);
-  // zeta = A^2 conj(x) / (4 y |x|^2)
-  const dd nr = dd_add(dd_mul_d(A2r, xr), dd_mul_d(A2i, xi));
-  const dd ni = dd_add(dd_mul_d(A2i, xr), dd_neg(dd_mul_d(A2r, xi)));
-  const dd den = dd_scale2(dd_mul_d(dd_add(two_prod(xr, xr), two_prod(xi, xi)), y), 4.0);
-  const dd zr = dd_div(nr, den), zi = dd_div(ni, den);
-  const double zi2 = fma(zi.hi, zi.hi, 2.0 * zi.hi * zi.lo);
-  double sr = 0.0, si = 0.0;
-#pragma unroll 1
-  for (int j = 0; j < n_pairs; ++j) {
-    const double t = st[j];
-    const double a = (zr.hi - t) + (zr.lo - stlo[j]);  // Re(zeta - t), accurate to an ulp of ITSELF
-    const double s = fma(a, a, zi2);
-    const double wq = sw[j] / s;
-    const double d = eta.re - t;
-    // (eta - t) conj(zeta - t)
-    sr = fma(wq, fma(d, a, eta.im * zi.hi), sr);
-    si = fma(wq, fma(eta.im, a, -(d * zi.hi)), si);
-  }
-  return {sr, si};
-}
-
-// Stage the folded angular rule: pair j = nodes (j, n_ang-1-j); t = z^2 (hi + lo exactly), weight =
-// w_j + w_mirror (the middle node of an odd rule enters once).  *bad is set if the rule is not symmetric.
-__device__ void prep_angular(const EvalArgs& a, const BlobLayout& L, double* blob, int* bad) {
-  float* tf = reinterpret_cast<float*>(blob + L.off_f32);
-  float* wf = tf + L.npad;
-  for (int j = threadIdx.x; j < L.npad; j += blockDim.x) {
-    double t = 0, tlo = 0, w = 0;
-    if (j < a.n_pairs) {
-      const int jm = a.n_ang - 1 - j;
-      const double zp = a.ang_nodes[jm], zm = a.ang_nodes[j];
-      const double wp = a.ang_weights[jm], wm = a.ang_weights[j];
-      const double tol = 16.0 * DBL_EPSILON;
-      const bool ok = (jm == j) ? (fabs(zp) <= 1e-15)
-                                : (fabs(zp + zm) <= tol * fabs(zp) && fabs(wp - wm) <= tol * fabs(wp));
-      if (!ok) atomicExch(bad, 1);
-      const dd tt = two_prod(zp, zp);
-      t = tt.hi;
-      tlo = tt.lo;
-      w = (jm == j) ? wp : wp + wm;
-    }
-    blob[L.off_t + j] = t;
-    blob[L.off_tlo + j] = tlo;
-    blob[L.off_w + j] = w;
-    if (L.off_f32 >= 0) {
-      tf[j] = (float)t;
-      wf[j] = (float)w;
-    }
-  }
-}
-
-__device__ __forceinline__ double powi(double t, int k) {
-  double r = 1.0;
-  while (k) {
-    if (k & 1) r *= t;
-    t *= t;
-    k >>= 1;
-  }
-  return r;
-}
 
 // D1(y) for real y (REAL contour): massive 1/(y + m2) or rational (y + M2)/(y^2 + a y + b).
 __device__ __forceinline__ cd line_k_real(const gf_propagator& p, double y) {
@@ -293,6 +96,11 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
       }
     }
   }
+  if (L.off_rt >= 0)  // point-dependent contours: the rule pyramid as given ("n arrays")
+    for (int i = threadIdx.x; i < L.n_tab; i += blockDim.x) {
+      blob[L.off_rt + i] = a.rad_nodes[i];
+      blob[L.off_rw + i] = a.rad_weights[i];
+    }
   __syncthreads();  // t, w written by this CTA are visible to it
   for (int k = threadIdx.x; k < L.km; k += blockDim.x) {
     dd mu = {0.0, 0.0}, nu = {0.0, 0.0};
@@ -385,7 +193,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
         s = angular_far(delta, zeta, K, smu, snu);
         if (COUNT) { c_far += K; ++n_far; }
       } else if (zeta.im * zeta.im < tau * tau && zeta.re > -tau && zeta.re < 1.0 + tau) {
-        s = angular_exact(x.re, x.im, y, mur, mui, eta, st, stlo, sw, a.n_pairs);
+        s = angular_exact(x.re, x.im, y, 0.0, mur, mui, eta, st, stlo, sw, a.n_pairs);
         if (COUNT) { c_exact += a.n_pairs; ++n_exact; }
       } else {
         s = angular_near<T>(eta, zeta, mu0, stT, swT, a.n_pairs);
@@ -419,7 +227,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   }
 }
 
-BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32) {
+BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid) {
   BlobLayout L;
   L.npad = (n_pairs + 3) & ~3;
   L.km = kKmCap;
@@ -434,6 +242,9 @@ BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32) {
   L.off_q4 = take(n_rad);
   L.off_pref = take(2 * n_terms * n_rad);
   L.off_f32 = f32 ? take(L.npad) : -1;  // 2 float tables of npad entries = npad doubles
+  L.n_tab = pyramid ? n_rad + n_rad / 2 + n_rad / 4 + n_rad / 8 : 0;
+  L.off_rt = pyramid ? take(L.n_tab) : -1;
+  L.off_rw = pyramid ? take(L.n_tab) : -1;
   L.n_doubles = o;
   return L;
 }
@@ -451,7 +262,7 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   plan->split_log2 = sl;
   const long long threads = a.n_points << sl;
   plan->grid_blocks = (threads + kBlockThreads - 1) / kBlockThreads;
-  plan->layout = make_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32);
+  plan->layout = make_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes);
   plan->smem_bytes = 16 + (size_t)plan->layout.n_doubles * sizeof(double);
   if (plan->smem_bytes > 200 * 1024) {
     set_error("eval_grid: tables need %zu bytes of shared memory (limit 200 KiB): reduce n_rad/n_ang",
@@ -489,8 +300,8 @@ int launch_eval(const EvalArgs& a_in, int precision, unsigned long long* d_count
   LaunchPlan plan;
   int rc = plan_eval(a_in, precision, &plan);
   if (rc) return rc;
-  if (!plan.shared_nodes) {
-    set_error("eval_grid: contour %d is not implemented yet", a_in.contour);
+  if (!plan.shared_nodes && precision == 32) {
+    set_error("eval_grid: the FP32 comparison variant exists for the REAL contour only");
     return GF_ERR_UNSUPPORTED;
   }
   EvalArgs a = a_in;
@@ -502,7 +313,9 @@ int launch_eval(const EvalArgs& a_in, int precision, unsigned long long* d_count
   if (rc) return rc;
   prep_real_kernel<<<1, 256, 0, stream>>>(a, plan.layout, blob);
   rc = check_cuda(cudaGetLastError(), "prep kernel launch");
-  if (!rc) {
+  if (!rc && !plan.shared_nodes) {
+    rc = launch_contour(a, plan, blob, d_counters, stream);
+  } else if (!rc) {
     if (d_counters)
       rc = precision == 32 ? launch_real<float, true>(a, plan, blob, d_counters, stream)
                            : launch_real<double, true>(a, plan, blob, d_counters, stream);

@@ -35,6 +35,7 @@ struct EvalArgs {
   double line2_scale;  // |m2^2| or the largest pole modulus: sizes the deformed contours
   int contour;         // gf_contour
   int thread_ok;       // THREAD applicable (equal real masses)
+  double th5, cos_th5, sin_th5;  // 3 pi/4 and its cos, sin as the host's libm rounds them (far waypoint of THREAD)
   int split_log2;      // lanes per grid point = 1 << split_log2
 };
 
@@ -48,6 +49,7 @@ struct BlobLayout {
   int off_y, off_q4;            // radial nodes y_i, 1/(4 y_i)
   int off_pref;                 // double2 pref[n_terms][n_rad]
   int off_f32;                  // float t[npad], w[npad] (FP32 variant) or -1
+  int off_rt, off_rw, n_tab;    // point-dependent contours: the radial rule pyramid (nodes, weights) or -1
   int n_doubles;                // total, even
 };
 
@@ -76,6 +78,9 @@ int launch_make_grid(double re_min, double re_max, int n_re, double im_min, doub
 // gf_eval.cu
 int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan);
 int launch_eval(const EvalArgs& a, int precision, unsigned long long* d_counters, cudaStream_t stream);
+// gf_contour.cu: evaluation kernel for contours that depend on the grid point (RAY_ARC, THREAD, AUTO)
+int launch_contour(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* d_counters,
+                   cudaStream_t stream);
 int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d_nodes, int n, double* d_y,
                       cudaStream_t stream);
 

@@ -280,6 +280,111 @@ def test_asymmetric_rule_is_rejected_with_nan(gf):
     assert torch.isnan(g.real).all()
 
 
+# ------------------------------------------------------------------ a3: contours that depend on the point
+@pytest.mark.parametrize("contour,over", [
+    ("ray_arc", {}), ("auto", {}),
+    ("thread", {"re": (-5.0, -4.2), "im": (-0.5, 0.5)}),          # where THREAD applies (Re x <= -4.1 m^2)
+    ("thread", {"re": (-9.0, -4.2), "im": (-1e-3, 1e-3), "n_re": 96, "n_im": 20}),
+])
+def test_cfg1_contours_every_point(gf, oracle, contour, over):
+    """Config 1 on each contour policy (contour selection is part of Kernel 2), every point."""
+    cfg = dict(W.CONFIGS["cfg1_tiny"], **over)
+    P, rn, rw, z, wz = gpu_setup(gf, cfg, contour=contour)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
+    ref = oracle_eval(oracle, cfg, oracle_grid(oracle, cfg), contour=contour)
+    e = relerr(g, ref)
+    assert e.max() <= TOL64, (e.max(), x.cpu().numpy().ravel()[e.argmax()])
+
+
+def test_cfg2_auto_every_point(gf, oracle):
+    cfg = W.CONFIGS["cfg2_mid"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg, contour="auto")
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
+    ref = oracle_eval(oracle, cfg, oracle_grid(oracle, cfg), contour="auto")
+    e = relerr(g, ref)
+    assert e.max() <= TOL64, (e.max(), x.cpu().numpy().ravel()[e.argmax()])
+    # rows j and n_im-1-j are conjugates (invariant I2); the mirrored THREAD contour makes it exact there,
+    # elsewhere sincos(-phi) = -sincos(phi) does
+    assert relerr(np.conj(g[::-1]), g).max() <= 1e-13
+
+
+@pytest.mark.parametrize("contour", ["auto", "thread"])
+def test_cfg5_strip_contours_sampled(gf, oracle, contour):
+    """The near-cut strip at full size under AUTO / THREAD, on the seeded sample; and the discontinuity
+    across the cut against the closed form (-+ pi sqrt(1 - 4 m^2/s)) within the 20 % the
+    non-adaptive rule reaches there (0.94-1.13 of the exact value)."""
+    cfg = W.CONFIGS["cfg5_strip"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg, contour=contour)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+    torch.cuda.synchronize()
+    idx = W.parity_sample(cfg, n_random=64, stride=max(cfg["n_re"], cfg["n_im"]) // 8)
+    gs = g.reshape(-1)[torch.from_numpy(idx).cuda()].cpu().numpy()
+    xs = oracle_grid(oracle, cfg).ravel()[idx]
+    ref = oracle_eval(oracle, cfg, xs, contour=contour)
+    e = relerr(gs, ref)
+    assert e.max() <= TOL64, (contour, e.max(), xs[e.argmax()])
+    gn, xn = g.cpu().numpy(), x.cpu().numpy()
+    # median over bands of Re x: single points where a node of the non-adaptive rule lands next to the
+    # cut's opening are off by O(1) (the oracle has the same outliers: parity above)
+    for lo, hi in [(-10.0, -8.0), (-8.0, -6.0), (-6.0, -5.0), (-5.0, -4.5), (-4.5, -4.2)]:
+        m = (xn.real > lo) & (xn.real <= hi)
+        exact = -np.sign(xn.imag[m]) * np.pi * np.sqrt(1.0 + 4.0 / xn.real[m])
+        assert abs(np.median(gn.imag[m] / exact) - 1.0) <= 0.1, (lo, hi)
+
+
+@pytest.mark.parametrize("contour", ["ray_arc", "auto"])
+def test_other_propagators_on_contours(gf, oracle, contour):
+    """Rational line 2 (config 4's integrand, two poles) and rational line 1 with complex y."""
+    rat = {"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2}
+    for lk, lpk in ((W.CONFIGS["cfg4_rational"]["line_k"], rat), (rat, {"kind": "massive", "m2": 0.7})):
+        cfg = dict(W.CONFIGS["cfg4_rational"], line_k=lk, line_pk=lpk, n_re=40, n_im=36, n_rad=128, n_ang=64)
+        P, rn, rw, z, wz = gpu_setup(gf, cfg, contour=contour)
+        x = gpu_grid(gf, cfg)
+        g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
+        ref = oracle_eval(oracle, cfg, oracle_grid(oracle, cfg), contour=contour)
+        e = relerr(g, ref)
+        assert e.max() <= TOL64, (e.max(), x.cpu().numpy().ravel()[e.argmax()])
+
+
+@pytest.mark.parametrize("n_points", [1, 33, 4097])
+def test_contours_ragged_point_counts(gf, oracle, n_points):
+    """Lane split (1..32 lanes per point walk one contour together) and a ragged last CTA under AUTO."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    rng = np.random.default_rng(W.PARITY_SEED + 7 * n_points)
+    xs = rng.uniform(-6, 1, n_points) + 1j * rng.uniform(-2, 2, n_points) * rng.choice([1.0, 1e-3], n_points)
+    xs[0] = 0.0
+    P, rn, rw, z, wz = gpu_setup(gf, cfg, contour="auto")
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+    ref = oracle_eval(oracle, cfg, xs, contour="auto")
+    assert g[0] == 0 and relerr(g, ref).max() <= TOL64
+
+
+def test_contours_reach_the_continuation(gf):
+    """What the deformation is for: outside the parabola R2 the REAL sum is not the continuation, RAY_ARC is
+    (closed form CF1, values from tests/golden via mpmath; Chebyshev angular rule, SURVEY 8(c) tolerances)."""
+    from tests import closed_forms as CF
+    cfg = dict(W.CONFIGS["cfg2_mid"])
+    xs = np.array([2 - 4j, -3 + 2j, -8 + 4j])
+    exact = np.array([complex(CF.cf1(v)) for v in xs])
+    out = {}
+    for contour in ("real", "ray_arc"):
+        P, rn, rw, z, wz = gpu_setup(gf, cfg, contour=contour, ang="gauss_cheb2")
+        out[contour] = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+    assert relerr(out["ray_arc"], exact).max() <= 1e-9
+    assert relerr(out["real"], exact).min() > 1e-2
+
+
+def test_fp32_variant_is_real_contour_only(gf):
+    cfg = W.CONFIGS["cfg1_tiny"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg, contour="auto", precision=32)
+    with pytest.raises(gf.GfError) as ei:
+        gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, gpu_grid(gf, cfg))
+    assert ei.value.status == 3
+
+
 # ------------------------------------------------------------------ end-to-end host entry point
 def test_eval_grid_host_matches_device_path(gf):
     cfg = W.CONFIGS["cfg1_tiny"]
