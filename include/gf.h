@@ -149,17 +149,20 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
                       long long n_points, void* h_out, void* stream);
 
 /* The same evaluation, also counting the work by route for the roofline accounting.
- * d_counters: 6 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
- *   [0] NEAR pairs  [1] FAR series terms  [2] EXACT pairs  [3..5] (point, radial node, pole) triples
- *   taken by the NEAR / FAR / EXACT route.  Results are identical to gf_eval_grid. */
+ * d_counters: 8 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
+ *   [0] NEAR pairs  [1] series terms EXECUTED (every lane of a warp runs its warp's longest series)
+ *   [2] EXACT pairs  [3] [4] [5] [6] (point, radial node, pole) triples taken by the NEAR / MOMENT / EXACT / CHEB
+ *   route  [7] series terms NEEDED (the sum over series triples of their own K).  Results are identical to
+ *   gf_eval_grid. */
 int gf_eval_grid_counted(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
                          const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
                          long long n_points, void* d_out, unsigned long long* d_counters, void* stream);
 
 /* How gf_eval_grid would launch, and the FP64-pipe instructions per unit of work of each route (for benchmarks
  * and roofline numbers; makes no CUDA call).  Per unit: *_dfma counts DFMA (2 flops each), *_other counts
- * DMUL + DADD (1 flop each); they follow the SASS of the loops.  Executed
- * instructions per launch = sum over routes of (gf_eval_grid_counted's counters) x (these). */
+ * DMUL + DADD (1 flop each), *_fp32 FP32-pipe instructions (precision 32); they follow the SASS of the loops
+ * (DESIGN.md "Instruction counts").  Executed instructions per launch = sum over routes of
+ * (gf_eval_grid_counted's counters) x (these). */
 typedef struct {
   int block_threads;      /* threads per CTA */
   long long grid_blocks;  /* CTAs */
@@ -167,13 +170,14 @@ typedef struct {
   int smem_bytes;         /* dynamic shared memory per CTA */
   int n_pairs;            /* folded angular nodes: ceil(n_ang/2) */
   int n_terms;            /* simple-pole terms of line 2 (1 massive, 2 rational) */
-  int far_terms_max;      /* longest far-field series */
+  int series_terms_max;   /* longest series (coefficients staged per table) */
   double evals;           /* nominal integrand evaluations: n_points * n_rad * n_ang */
-  double near_pair_dfma, near_pair_other, near_pair_fp32;   /* per NEAR pair (fp32: FP32-pipe, precision 32) */
-  double far_term_dfma, far_term_other;                     /* per FAR series term */
-  double exact_pair_dfma, exact_pair_other;                 /* per EXACT pair */
-  double node_near_dfma, node_near_other;                   /* per (point, node, pole) by route: set-up + finish */
-  double node_far_dfma, node_far_other;
+  double near_pair_dfma, near_pair_other, near_pair_fp32;         /* per NEAR pair */
+  double series_term_dfma, series_term_other, series_term_fp32;   /* per executed series term */
+  double exact_pair_dfma, exact_pair_other;                       /* per EXACT pair */
+  double node_near_dfma, node_near_other;                         /* per (point, node, pole) by route: set-up + finish */
+  double node_moment_dfma, node_moment_other;
+  double node_cheb_dfma, node_cheb_other;
   double node_exact_dfma, node_exact_other;
 } gf_launch_info;
 int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_points, gf_launch_info* out);

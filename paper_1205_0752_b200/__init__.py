@@ -43,14 +43,16 @@ class gf_params(ctypes.Structure):
 class gf_launch_info(ctypes.Structure):
     _fields_ = [("block_threads", ctypes.c_int), ("grid_blocks", ctypes.c_longlong), ("split", ctypes.c_int),
                 ("smem_bytes", ctypes.c_int), ("n_pairs", ctypes.c_int), ("n_terms", ctypes.c_int),
-                ("far_terms_max", ctypes.c_int), ("evals", ctypes.c_double)] + [
+                ("series_terms_max", ctypes.c_int), ("evals", ctypes.c_double)] + [
         (n, ctypes.c_double) for n in (
-            "near_pair_dfma", "near_pair_other", "near_pair_fp32", "far_term_dfma", "far_term_other",
-            "exact_pair_dfma", "exact_pair_other", "node_near_dfma", "node_near_other", "node_far_dfma",
-            "node_far_other", "node_exact_dfma", "node_exact_other")]
+            "near_pair_dfma", "near_pair_other", "near_pair_fp32", "series_term_dfma", "series_term_other",
+            "series_term_fp32", "exact_pair_dfma", "exact_pair_other", "node_near_dfma", "node_near_other",
+            "node_moment_dfma", "node_moment_other", "node_cheb_dfma", "node_cheb_other", "node_exact_dfma",
+            "node_exact_other")]
 
 
-COUNTER_NAMES = ("near_pairs", "far_terms", "exact_pairs", "near_nodes", "far_nodes", "exact_nodes")
+COUNTER_NAMES = ("near_pairs", "series_terms", "exact_pairs", "near_nodes", "moment_nodes", "exact_nodes",
+                 "cheb_nodes", "series_terms_needed")
 
 
 _lib = None
@@ -250,8 +252,9 @@ def eval_grid_counted(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weig
 
 def executed_fp64(info, counters):
     """(FP64-pipe thread-instructions, flops with FMA = 2) of one launch from its route counters."""
-    units = (("near_pair", "near_pairs"), ("far_term", "far_terms"), ("exact_pair", "exact_pairs"),
-             ("node_near", "near_nodes"), ("node_far", "far_nodes"), ("node_exact", "exact_nodes"))
+    units = (("near_pair", "near_pairs"), ("series_term", "series_terms"), ("exact_pair", "exact_pairs"),
+             ("node_near", "near_nodes"), ("node_moment", "moment_nodes"), ("node_exact", "exact_nodes"),
+             ("node_cheb", "cheb_nodes"))
     inst = sum((info[u + "_dfma"] + info[u + "_other"]) * counters[c] for u, c in units)
     flops = sum((2 * info[u + "_dfma"] + info[u + "_other"]) * counters[c] for u, c in units)
     return float(inst), float(flops)

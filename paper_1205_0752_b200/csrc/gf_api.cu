@@ -27,6 +27,10 @@ int check_cuda(cudaError_t e, const char* what) {
 
 namespace {
 
+// per (point, node, pole) FP64-pipe instructions of each route's set-up + finish (SASS of eval_real_kernel<double>)
+constexpr double kNodeNearDfma = 10, kNodeNearOther = 14, kNodeMomentDfma = 22, kNodeMomentOther = 12,
+                 kNodeChebDfma = 40, kNodeChebOther = 28;
+
 bool finite_prop(const gf_propagator& p) {
   return std::isfinite(p.m2_re) && std::isfinite(p.m2_im) && std::isfinite(p.M2) && std::isfinite(p.a) &&
          std::isfinite(p.b);
@@ -267,17 +271,18 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
   out->smem_bytes = (int)plan.smem_bytes;
   out->n_pairs = a.n_pairs;
   out->n_terms = a.n_terms;
-  out->far_terms_max = plan.layout.km;
+  out->series_terms_max = plan.layout.kmc;
   out->evals = (double)n_points * n_rad * n_ang;
   // FP64-pipe instructions per unit of each route, read off the SASS of gf_eval.cu (DESIGN.md "Instruction
-  // counts"): NEAR pair 5 DFMA + 1 DMUL + 2 DADD; FAR term 6 DFMA + 2 DMUL; EXACT pair 4 DFMA + 2 DMUL +
-  // 3 DADD + a full-precision division (8 DFMA + 1 DMUL); per node-term: set-up and finish of each route.
+  // counts"): NEAR pair 5 DFMA + 1 DMUL + 2 DADD; series term (both polynomials) 4 DFMA; EXACT pair 4 DFMA +
+  // 2 DMUL + 3 DADD + a full-precision division (8 DFMA + 1 DMUL); per node-term: set-up and finish of each route.
   const bool f32 = p->precision == 32;
   out->near_pair_dfma = f32 ? 0 : 5; out->near_pair_other = f32 ? 0 : 3; out->near_pair_fp32 = f32 ? 5 : 0;
-  out->far_term_dfma = 6; out->far_term_other = 2;
+  out->series_term_dfma = f32 ? 0 : 4; out->series_term_other = 0; out->series_term_fp32 = f32 ? 4 : 0;
   out->exact_pair_dfma = 12; out->exact_pair_other = 6;
-  out->node_near_dfma = 10; out->node_near_other = 14;
-  out->node_far_dfma = 16; out->node_far_other = 18;
+  out->node_near_dfma = kNodeNearDfma; out->node_near_other = kNodeNearOther;
+  out->node_moment_dfma = kNodeMomentDfma; out->node_moment_other = kNodeMomentOther;
+  out->node_cheb_dfma = kNodeChebDfma; out->node_cheb_other = kNodeChebOther;
   out->node_exact_dfma = 120; out->node_exact_other = 180;
   return GF_OK;
 }

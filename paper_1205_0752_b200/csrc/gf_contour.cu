@@ -149,18 +149,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   if (threadIdx.x == 0) bulk_load(sb, blob, (uint32_t)(L.n_doubles * sizeof(double)), bar);
   mbar_wait(bar, 0);
 
-  const double* st = sb + L.off_t;
-  const double* stlo = sb + L.off_tlo;
-  const double* sw = sb + L.off_w;
-  const double* smu = sb + L.off_mu;
-  const double* snu = sb + L.off_nu;
+  const Tabs<double> tb = make_tabs<double>(sb, L, a.n_pairs);
   const double* sy = sb + L.off_y;
   const double* sq4 = sb + L.off_q4;
   const double2* spref = reinterpret_cast<const double2*>(sb + L.off_pref);
   const double* srt = sb + L.off_rt;
   const double* srw = sb + L.off_rw;
   const bool bad_rule = sb[0] != 0.0;
-  const double mu0 = smu[0];
 
   const int S = 1 << a.split_log2;
   const long long gtid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -190,11 +185,14 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   const int pol = a.contour == GF_CONTOUR_AUTO ? auto_policy(a, x.re, x.im) : a.contour;
   const int n_seg = build_contour(a, pol, x.re, x.im, seg, &mirror);
 
-  unsigned long long c_near = 0, c_far = 0, c_exact = 0, n_near = 0, n_far = 0, n_exact = 0;
+  RouteCount rc;
   double g_re = 0.0, g_im = 0.0;
   int ks = 0;
+  // warp-synchronous node loop (node_term is warp-collective): a lane past the last node repeats it with weight 0
 #pragma unroll 1
-  for (int g = sub; g < a.n_rad; g += S) {
+  for (int g0 = 0; g0 < a.n_rad; g0 += S) {
+    const bool valid = g0 + sub < a.n_rad;
+    const int g = valid ? g0 + sub : a.n_rad - 1;
     while (ks + 1 < n_seg && g >= seg[ks].start + seg[ks].n) ++ks;
     const Seg& sg = seg[ks];
     const int i = g - sg.start;
@@ -233,27 +231,15 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
     }
     cd base = {0.0, 0.0};
     if (!table) base = cscale(cmul(cmul(wy, y), line_k_complex(a.line_k, y)), a.c0);
+    const cd xq = cmul(xinv, q4);                    // 1/(4 x y)
 #pragma unroll 1
     for (int r = 0; r < a.n_terms; ++r) {
       const double mur = a.term[r].mu_re, mui = a.term[r].mu_im;
       const cd xm = {x.re + mur, x.im + mui};
       const cd A = {xm.re + y.re, xm.im + y.im};
       const cd delta = cmul(xm, q4);                 // eta - 1/4
-      const cd eta = {0.25 + delta.re, delta.im};
-      const cd zeta = cmul(cmul(eta, A), xinv);
-      const int e2 = 2 * ilogb(fmax(fabs(zeta.re), fabs(zeta.im)));
-      const int K = e2 >= 2 ? (e2 >= kFarBits ? 2 : kFarBits / e2 + 1) : 0x7fffffff;
-      cd s;
-      if (K <= L.km && (K <= a.n_pairs || e2 > 6)) {
-        s = angular_far(delta, zeta, K, smu, snu);
-        if (COUNT) { c_far += K; ++n_far; }
-      } else if (zeta.im * zeta.im < kTau64 * kTau64 && zeta.re > -kTau64 && zeta.re < 1.0 + kTau64) {
-        s = angular_exact(x.re, x.im, y.re, y.im, mur, mui, eta, st, stlo, sw, a.n_pairs);
-        if (COUNT) { c_exact += a.n_pairs; ++n_exact; }
-      } else {
-        s = angular_near<double>(eta, zeta, mu0, st, sw, a.n_pairs);
-        if (COUNT) { c_near += a.n_pairs; ++n_near; }
-      }
+      const cd zeta = cmul(csqr(A), xq);
+      const cd s = node_term<double, COUNT>(tb, x, y, delta, zeta, mur, mui, rc);
       cd pr;
       if (table) {
         const double2 p2 = spref[r * a.n_rad + i];
@@ -262,6 +248,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
         const cd ic = cinv(cd{y.re + mur, y.im + mui});
         pr = cmul(cmul(base, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);
       }
+      if (!valid) pr = {0.0, 0.0};
       g_re = fma(pr.re, s.re, fma(-pr.im, s.im, g_re));
       g_im = fma(pr.re, s.im, fma(pr.im, s.re, g_im));
     }
@@ -277,14 +264,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
     if (bad_rule) { g_re = nan(""); g_im = nan(""); }
     reinterpret_cast<double2*>(a.out)[point] = make_double2(g_re, g_im);
   }
-  if (COUNT) {
-    if (!active) c_near = c_far = c_exact = n_near = n_far = n_exact = 0;
-    unsigned long long v[6] = {c_near, c_far, c_exact, n_near, n_far, n_exact};
-    for (int k = 0; k < 6; ++k) {
-      for (int o = 16; o; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
-      if ((threadIdx.x & 31) == 0 && v[k]) atomicAdd(counters + k, v[k]);
-    }
-  }
+  if (COUNT) flush_counters(rc, active, counters);
 }
 
 template <bool COUNT>

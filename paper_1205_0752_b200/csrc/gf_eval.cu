@@ -13,30 +13,36 @@
 //    angular rule folds into
 //        1/(A - Bz) + 1/(A + Bz) - 2/c = -(2/c) (eta - t)/(zeta - t),
 //        t = z^2,  eta = A/(4y) = 1/4 + delta,  delta = (x + mu)/(4y),  zeta = A^2/(4xy),
-//    which needs no square root.  Per (point, radial node, pole) the angular sum
+//    which needs no square root of x or y.  Per (point, radial node, pole) the angular sum
 //        S = sum_j w_j (eta - t_j)/(zeta - t_j)          (w_j: folded weights)
-//    is evaluated by one of three routes, chosen from zeta alone:
-//      FAR    |zeta| >= 2 and few enough terms: the finite geometric series in omega = 1/zeta,
-//             S = omega [ delta P(omega) + N(omega) ],  P = sum_k mu_k omega^k,  N = sum_k nu_k omega^k,
-//             mu_k = sum_j w_j t_j^k,  nu_k = sum_j w_j t_j^k (1/4 - t_j)  (moments of the rule, made once
-//             per launch).  K = ceil(58 / log2|zeta|) terms make the truncation < 2^-58.  Cancellation
-//             free, O(K) instead of O(N_a).  Most radial nodes of a log-mapped rule are FAR.
-//      NEAR   otherwise: q_j = w_j/|zeta - t_j|^2 by one real reciprocal per PAIR (MUFU.RCP64H seed + one
-//             cubic correction, 3 DFMA, no slow path), two real sums U0 = sum q_j, U1 = sum q_j t_j, and
-//             S = mu_0 - (zeta - eta)(conj(zeta) U0 - U1).  8 FP64 instructions per pair.  Its
-//             cancellation grows like |zeta|^2, which FAR bounds.
+//    is the Cauchy transform of a fixed discrete measure on [0,1], analytic in zeta off [0,1].  It is
+//    evaluated by one of four routes chosen from zeta alone (gf_routes.cuh, node_term):
+//      MOMENT |zeta| large: geometric series in s = 1/(zeta - 1/2) with the centred moments of the rule,
+//             at most 22 terms.
+//      CHEB   Chebyshev series in s = 1/(w + sqrt(w^2-1)), w = 2 zeta - 1: 1/(zeta - t) = 4/sqrt(w^2-1)
+//             sum'_k s^k T_k(2t-1), with the Chebyshev moments of the rule (made once per launch).  It
+//             converges like rho^-k, rho = 1/|s| the parameter of the ellipse with foci 0 and 1 through
+//             zeta, so K = 60/log2(rho) terms replace the N_a/2 pairs of the direct sum wherever the
+//             radial node is not next to the image of the cut (median rho over the production scan: 3).
+//             Both series have real coefficients and a complex argument and share one loop: the
+//             second-order (Goertzel) recurrence, 2 DFMA per coefficient, 4 per term for the two
+//             polynomials P (times delta) and N.  Cancellation free as x -> 0 and as y -> infinity.
+//      NEAR   zeta close to [0,1] (rho < ~1.2): q_j = w_j/|zeta - t_j|^2 by one real reciprocal per PAIR
+//             (MUFU.RCP64H seed + one cubic correction, 3 DFMA, no slow path), two real sums U0 = sum q_j,
+//             U1 = sum q_j t_j, and S = mu_0 - (zeta - eta)(conj(zeta) U0 - U1).  8 FP64 instructions per pair.
 //      EXACT  zeta within 2^-8 of the segment [0,1] (the radial contour passes next to a zero of a
 //             denominator): zeta is recomputed in double-double and each term is formed directly with
 //             a = (zeta_hi - t_hi) + (zeta_lo - t_lo), t_hi + t_lo = z^2 exactly.  Rare (a few nodes per
-//             point outside the parabola where REAL is the continuation), so its cost does not matter;
-//             without it such terms carry an error eps/dist (reading G18).
+//             point outside the parabola where REAL is the continuation); without it such terms carry an
+//             error eps/dist (reading G18).
 //  * x = 0 gives exactly 0 (invariant I1); 0 < |x| < 2^-200 is rescaled (the sum is analytic at 0).
 //  * A one-CTA preparation kernel makes every x-independent table once per launch (folded angular rule,
-//    moments, the radial map y_i in double-double so that it is correctly rounded, per-node prefactors);
-//    each CTA of the evaluation kernel pulls that block into shared memory with ONE bulk copy
+//    series coefficients, the radial map y_i in double-double so that it is correctly rounded, per-node
+//    prefactors); each CTA of the evaluation kernel pulls that block into shared memory with ONE bulk copy
 //    (cp.async.bulk + mbarrier, the 1-D TMA path) and reads it as warp-wide broadcasts.
 //  * One thread owns one grid point (or 1/S of its radial nodes when the grid is too small to fill 148
-//    SMs; the S lanes are merged with warp shuffles); results leave as coalesced 16-byte stores.
+//    SMs; the S lanes are merged with warp shuffles); the node loop is warp-synchronous (the series loop
+//    of node_term runs to the warp's longest series); results leave as coalesced 16-byte stores.
 #include <cfloat>
 #include <cmath>
 #include <cstdint>
@@ -68,8 +74,8 @@ __global__ void radial_map_kernel(double Lhi, double Llo, double s0, const doubl
 
 // ---------------------------------------------------------------------------------------------
 // Preparation (one CTA): everything that does not depend on x, for the REAL contour.
-//   header [0] = 1.0 if the angular rule is not symmetric;  t, t_lo, w (folded rule);
-//   mu_k, nu_k (moments);  y_i, 1/(4 y_i);  pref_{r,i} = c0 Wr_i y_i D1(y_i) (-R_r/(y_i + mu_r)).
+//   header [0] = 1.0 if the angular rule is not symmetric;  t, t_lo, w (folded rule);  series coefficients
+//   mom[k], cheb[k];  y_i, 1/(4 y_i);  pref_{r,i} = c0 Wr_i y_i D1(y_i) (-R_r/(y_i + mu_r)).
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ EvalArgs a,
                                                         const __grid_constant__ BlobLayout L,
@@ -78,6 +84,8 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
   if (threadIdx.x == 0) bad = 0;
   __syncthreads();
   prep_angular(a, L, blob, &bad);
+  __syncthreads();  // t, w written by this CTA are visible to it
+  prep_series_T(a, L, blob);
   {
     // shifted-log map of [0, Lambda^2] (readings G3/G4): y(u) = s0 expm1(u L), dy/du = L (y + s0),
     // L = ln((Lambda^2 + s0)/s0) as a double-double from the host; y_i correctly rounded.
@@ -101,17 +109,8 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
       blob[L.off_rt + i] = a.rad_nodes[i];
       blob[L.off_rw + i] = a.rad_weights[i];
     }
-  __syncthreads();  // t, w written by this CTA are visible to it
-  for (int k = threadIdx.x; k < L.km; k += blockDim.x) {
-    dd mu = {0.0, 0.0}, nu = {0.0, 0.0};
-    for (int j = 0; j < a.n_pairs; ++j) {
-      const double t = blob[L.off_t + j], wp = blob[L.off_w + j] * powi(t, k);
-      mu = dd_add_d(mu, wp);
-      nu = dd_add(nu, two_prod(wp, 0.25 - t));
-    }
-    blob[L.off_mu + k] = mu.hi;
-    blob[L.off_nu + k] = nu.hi;
-  }
+  __syncthreads();  // the T_k(s_j) matrix is complete
+  prep_series_sums(a, L, blob);
   if (threadIdx.x == 0) {
     blob[0] = bad ? 1.0 : 0.0;
     blob[1] = 0.0;
@@ -119,11 +118,10 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
 }
 
 // ---------------------------------------------------------------------------------------------
-// Evaluation, REAL contour.  counters (COUNT only): [0] NEAR pairs, [1] FAR terms, [2] EXACT pairs,
-// [3] NEAR node-terms, [4] FAR node-terms, [5] EXACT node-terms.
+// Evaluation, REAL contour.  counters (COUNT only): gf.h, gf_eval_grid_counted.
 // ---------------------------------------------------------------------------------------------
 template <typename T, bool COUNT>
-__global__ void __launch_bounds__(kBlockThreads, 2)
+__global__ void __launch_bounds__(kBlockThreads, 3)
     eval_real_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                      const double* __restrict__ blob, unsigned long long* __restrict__ counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -134,19 +132,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   if (threadIdx.x == 0) bulk_load(sb, blob, (uint32_t)(L.n_doubles * sizeof(double)), bar);
   mbar_wait(bar, 0);
 
-  const double* st = sb + L.off_t;
-  const double* stlo = sb + L.off_tlo;
-  const double* sw = sb + L.off_w;
-  const double* smu = sb + L.off_mu;
-  const double* snu = sb + L.off_nu;
+  const Tabs<T> tb = make_tabs<T>(sb, L, a.n_pairs);
   const double* sy = sb + L.off_y;
   const double* sq4 = sb + L.off_q4;
   const double2* spref = reinterpret_cast<const double2*>(sb + L.off_pref);
-  const T* stT = sizeof(T) == 8 ? reinterpret_cast<const T*>(st) : reinterpret_cast<const T*>(sb + L.off_f32);
-  const T* swT = sizeof(T) == 8 ? reinterpret_cast<const T*>(sw) : stT + L.npad;
   const bool bad_rule = sb[0] != 0.0;
-  const double mu0 = smu[0];
-  const double tau = sizeof(T) == 8 ? kTau64 : kTau32;
 
   const int S = 1 << a.split_log2;
   const long long gtid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -172,34 +162,26 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   }
   const cd xinv = cinv(x);
 
-  unsigned long long c_near = 0, c_far = 0, c_exact = 0, n_near = 0, n_far = 0, n_exact = 0;
+  RouteCount rc;
   double g_re = 0.0, g_im = 0.0;
+  // warp-synchronous node loop: every lane makes the same number of trips (node_term is warp-collective);
+  // a lane past the last node repeats it with weight 0
 #pragma unroll 1
-  for (int i = sub; i < a.n_rad; i += S) {
+  for (int i0 = 0; i0 < a.n_rad; i0 += S) {
+    const bool valid = i0 + sub < a.n_rad;
+    const int i = valid ? i0 + sub : a.n_rad - 1;
     const double y = sy[i], q4 = sq4[i];
+    const cd xq = cscale(xinv, q4);                  // 1/(4 x y)
 #pragma unroll 1
     for (int r = 0; r < a.n_terms; ++r) {
       const double mur = a.term[r].mu_re, mui = a.term[r].mu_im;
       const cd xm = {x.re + mur, x.im + mui};
       const cd A = {xm.re + y, xm.im};
       const cd delta = cscale(xm, q4);               // eta - 1/4
-      const cd eta = {0.25 + delta.re, delta.im};
-      const cd zeta = cmul(cmul(eta, A), xinv);
-      // 2 ilogb(max component) <= log2 |zeta|^2
-      const int e2 = 2 * ilogb(fmax(fabs(zeta.re), fabs(zeta.im)));
-      const int K = e2 >= 2 ? (e2 >= kFarBits ? 2 : kFarBits / e2 + 1) : 0x7fffffff;
-      cd s;
-      if (K <= L.km && (K <= a.n_pairs || e2 > 6)) {
-        s = angular_far(delta, zeta, K, smu, snu);
-        if (COUNT) { c_far += K; ++n_far; }
-      } else if (zeta.im * zeta.im < tau * tau && zeta.re > -tau && zeta.re < 1.0 + tau) {
-        s = angular_exact(x.re, x.im, y, 0.0, mur, mui, eta, st, stlo, sw, a.n_pairs);
-        if (COUNT) { c_exact += a.n_pairs; ++n_exact; }
-      } else {
-        s = angular_near<T>(eta, zeta, mu0, stT, swT, a.n_pairs);
-        if (COUNT) { c_near += a.n_pairs; ++n_near; }
-      }
-      const double2 pr = spref[r * a.n_rad + i];
+      const cd zeta = cmul(csqr(A), xq);
+      const cd s = node_term<T, COUNT>(tb, x, cd{y, 0.0}, delta, zeta, mur, mui, rc);
+      double2 pr = spref[r * a.n_rad + i];
+      if (!valid) pr = make_double2(0.0, 0.0);
       g_re = fma(pr.x, s.re, fma(-pr.y, s.im, g_re));
       g_im = fma(pr.x, s.im, fma(pr.y, s.re, g_im));
     }
@@ -217,35 +199,31 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
     if (sizeof(T) == 8) reinterpret_cast<double2*>(a.out)[point] = make_double2(g_re, g_im);
     else reinterpret_cast<float2*>(a.out)[point] = make_float2((float)g_re, (float)g_im);
   }
-  if (COUNT) {
-    if (!active) c_near = c_far = c_exact = n_near = n_far = n_exact = 0;
-    unsigned long long v[6] = {c_near, c_far, c_exact, n_near, n_far, n_exact};
-    for (int k = 0; k < 6; ++k) {
-      for (int o = 16; o; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
-      if ((threadIdx.x & 31) == 0 && v[k]) atomicAdd(counters + k, v[k]);
-    }
-  }
+  if (COUNT) flush_counters(rc, active, counters);
 }
 
 BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid) {
   BlobLayout L;
   L.npad = (n_pairs + 3) & ~3;
-  L.km = kKmCap;
+  L.kmc = kKmc;
   int o = 2;  // header
   auto take = [&](int n) { int at = o; o += (n + 1) & ~1; return at; };
   L.off_t = take(L.npad);
   L.off_tlo = take(L.npad);
   L.off_w = take(L.npad);
-  L.off_mu = take(L.km);
-  L.off_nu = take(L.km);
+  L.off_mom = take(2 * L.kmc);
+  L.off_cheb = take(2 * L.kmc);
   L.off_y = take(n_rad);
   L.off_q4 = take(n_rad);
   L.off_pref = take(2 * n_terms * n_rad);
-  L.off_f32 = f32 ? take(L.npad) : -1;  // 2 float tables of npad entries = npad doubles
+  // 2 float tables of npad entries = npad doubles; 2 float2 tables of kmc entries = 2 kmc doubles
+  L.off_f32 = f32 ? take(L.npad + 2 * L.kmc) : -1;
   L.n_tab = pyramid ? n_rad + n_rad / 2 + n_rad / 4 + n_rad / 8 : 0;
   L.off_rt = pyramid ? take(L.n_tab) : -1;
   L.off_rw = pyramid ? take(L.n_tab) : -1;
   L.n_doubles = o;
+  L.off_scratch = o;
+  L.n_total = o + L.kmc * L.npad;
   return L;
 }
 
@@ -308,7 +286,7 @@ int launch_eval(const EvalArgs& a_in, int precision, unsigned long long* d_count
   a.split_log2 = plan.split_log2;
   // scratch for the prepared tables: stream-ordered, freed in stream order after the evaluation
   double* blob = nullptr;
-  rc = check_cuda(cudaMallocAsync(reinterpret_cast<void**>(&blob), (size_t)plan.layout.n_doubles * sizeof(double), stream),
+  rc = check_cuda(cudaMallocAsync(reinterpret_cast<void**>(&blob), (size_t)plan.layout.n_total * sizeof(double), stream),
                   "cudaMallocAsync(tables)");
   if (rc) return rc;
   prep_real_kernel<<<1, 256, 0, stream>>>(a, plan.layout, blob);

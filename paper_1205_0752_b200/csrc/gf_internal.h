@@ -43,14 +43,16 @@ struct EvalArgs {
 // evaluation kernel copies them to shared memory (one 16-byte header first).
 struct BlobLayout {
   int npad;                     // n_pairs rounded up to 4
-  int km;                       // far-field moments mu_0..mu_{km-1}, nu_0..nu_{km-1}
+  int kmc;                      // series coefficients k = 0 .. kmc-1 (even)
   int off_t, off_tlo, off_w;    // folded angular rule: t = z^2 (hi, lo), weight
-  int off_mu, off_nu;
+  int off_mom, off_cheb;        // double2 (P_k, N_k)[kmc]: centred-moment series, Chebyshev series
   int off_y, off_q4;            // radial nodes y_i, 1/(4 y_i)
   int off_pref;                 // double2 pref[n_terms][n_rad]
-  int off_f32;                  // float t[npad], w[npad] (FP32 variant) or -1
+  int off_f32;                  // FP32 variant: float t[npad], w[npad], float2 mom[kmc], cheb[kmc]; or -1
   int off_rt, off_rw, n_tab;    // point-dependent contours: the radial rule pyramid (nodes, weights) or -1
-  int n_doubles;                // total, even
+  int n_doubles;                // doubles every CTA stages (even)
+  int off_scratch;              // preparation-only scratch after the staged block: T_k(s_j), [kmc][npad]
+  int n_total;                  // doubles to allocate
 };
 
 struct LaunchPlan {

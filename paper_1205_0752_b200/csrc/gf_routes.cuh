@@ -1,5 +1,5 @@
 // gf_routes.cuh -- device code shared by the two evaluation kernels (gf_eval.cu: REAL contour, nodes
-// prepared once per launch; gf_contour.cu: contours that depend on the grid point): the three routes that
+// prepared once per launch; gf_contour.cu: contours that depend on the grid point): the routes that
 // evaluate the folded angular sum S = sum_j w_j (eta - t_j)/(zeta - t_j) of one (point, radial node, pole),
 // the 1-D TMA staging of the prepared tables, and the folding of the angular rule.  See gf_eval.cu's
 // header for the algebra.  Everything here is internal to the translation unit that includes it.
@@ -14,10 +14,16 @@
 namespace gf {
 namespace {
 
-constexpr int kKmCap = 60;           // most far-field terms ever used (|zeta| >= 2 -> K <= 59)
-constexpr int kFarBits = 116;        // 2 * 58: K = kFarBits / (2 ilogb|zeta|) + 1
-constexpr double kTau64 = 0x1p-8;    // EXACT route inside this distance of [0,1] (FP64)
-constexpr double kTau32 = 0x1p-4;    // the FP32 variant's NEAR loop is only good further away
+constexpr int kKmc = 256;             // series coefficients staged per table (even)
+constexpr int kMomTerms = 32;         // genuine coefficients of the centred-moment series (zero beyond)
+constexpr double kMomentMin = 4.5;    // MOMENT route when max(|Re zeta|, |Im zeta|) >= this: |zeta - 1/2| >= 4
+constexpr double kTau64 = 0x1p-8;     // EXACT route inside this distance of [0,1] (FP64)
+constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only good further away
+// FP64-pipe instructions of the per-node code of each route (set-up + finish), used to pick the cheaper of
+// CHEB and NEAR; they only steer the choice, any value gives the same sum
+constexpr int kChebNodeCost = 76, kNearNodeCost = 24;
+
+enum { ROUTE_MOMENT = 0, ROUTE_CHEB = 1, ROUTE_NEAR = 2, ROUTE_EXACT = 3 };
 
 struct cd {
   double re, im;
@@ -25,6 +31,7 @@ struct cd {
 __device__ __forceinline__ cd cmul(cd a, cd b) {
   return {fma(a.re, b.re, -(a.im * b.im)), fma(a.re, b.im, a.im * b.re)};
 }
+__device__ __forceinline__ cd csqr(cd a) { return {fma(a.re, a.re, -(a.im * a.im)), (a.re + a.re) * a.im}; }
 __device__ __forceinline__ cd cscale(cd a, double s) { return {a.re * s, a.im * s}; }
 __device__ __forceinline__ cd cinv(cd a) {
   // set-up code only (once per point / node): plain division, scaled against overflow
@@ -43,6 +50,22 @@ __device__ __forceinline__ float rcp_seed(float s) {
   float r;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s));  // MUFU.RCP
   return r;
+}
+__device__ __forceinline__ double rsqrt_seed(double s) {
+  double r;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));  // MUFU.RSQ64H
+  return r;
+}
+// 1/s and 1/sqrt(s) for normal s well inside the exponent range: seed + one cubic correction, no slow path
+__device__ __forceinline__ double rcp_fast(double s) {
+  const double r0 = rcp_seed(s);
+  const double e = fma(-s, r0, 1.0);
+  return fma(r0, fma(e, e, e), r0);
+}
+__device__ __forceinline__ double rsqrt_fast(double s) {
+  const double r0 = rsqrt_seed(s);
+  const double e = fma(-s * r0, r0, 1.0);                // 1 - s r0^2
+  return fma(r0, e * fma(0.375, e, 0.5), r0);            // r0 (1 + e/2 + 3 e^2/8)
 }
 
 // ---- 1-D TMA: one bulk copy global -> shared, completion on an mbarrier ------------------------
@@ -66,9 +89,58 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
         : "=r"(done)
         : "r"(smem_u32(bar)), "r"(phase)
         : "memory");
-    if (spin > (1LL << 26)) __trap();  // a 20 KB copy that has not landed after seconds: fail, do not hang
+    if (spin > (1LL << 26)) __trap();  // a copy of a few KB that has not landed after seconds: fail, do not hang
   }
 }
+
+template <typename T>
+struct Vec2;
+template <>
+struct Vec2<double> { typedef double2 type; };
+template <>
+struct Vec2<float> { typedef float2 type; };
+
+// Shared-memory views of the staged tables
+template <typename T>
+struct Tabs {
+  const double *st, *stlo, *sw;                   // folded angular rule
+  const T *stT, *swT;                             // the same in the loop's type
+  const typename Vec2<T>::type *mom, *cheb;       // series coefficients (P_k, N_k), kmc entries each
+  double mu0;                                     // sum of the folded weights
+  double tau;                                     // EXACT inside this distance of [0,1]
+  int n_pairs, kmc;
+};
+template <typename T>
+__device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout& L, int n_pairs) {
+  Tabs<T> tb;
+  tb.st = sb + L.off_t;
+  tb.stlo = sb + L.off_tlo;
+  tb.sw = sb + L.off_w;
+  typedef typename Vec2<T>::type V2;
+  if (sizeof(T) == 8) {
+    tb.stT = reinterpret_cast<const T*>(tb.st);
+    tb.swT = reinterpret_cast<const T*>(tb.sw);
+    tb.mom = reinterpret_cast<const V2*>(sb + L.off_mom);
+    tb.cheb = reinterpret_cast<const V2*>(sb + L.off_cheb);
+  } else {
+    tb.stT = reinterpret_cast<const T*>(sb + L.off_f32);
+    tb.swT = tb.stT + L.npad;
+    tb.mom = reinterpret_cast<const V2*>(tb.swT + L.npad);
+    tb.cheb = tb.mom + L.kmc;
+  }
+  tb.mu0 = sb[L.off_mom];  // a_0 of the moment series = sum of the folded weights
+  tb.tau = sizeof(T) == 8 ? kTau64 : kTau32;
+  tb.n_pairs = n_pairs;
+  tb.kmc = L.kmc;
+  return tb;
+}
+
+// Work counters of one thread (COUNT launches only)
+struct RouteCount {
+  unsigned long long near_pairs = 0, series_exec = 0, exact_pairs = 0, n_near = 0, n_moment = 0, n_exact = 0,
+                     n_cheb = 0, series_used = 0;
+};
+constexpr int kNumCounters = 8;
 
 // ---- NEAR: one folded angular pair: q = w/|zeta - t|^2 and the two sums ---------------------------
 __device__ __forceinline__ void pair_step(double zr, double zi2, double t, double w, double& u0, double& u1) {
@@ -89,13 +161,6 @@ __device__ __forceinline__ void pair_step(float zr, float zi2, float t, float w,
   u0 += q;
   u1 = fmaf(q, t, u1);
 }
-
-template <typename T>
-struct Vec2;
-template <>
-struct Vec2<double> { typedef double2 type; };
-template <>
-struct Vec2<float> { typedef float2 type; };
 
 // S = mu0 - (zeta - eta)(conj(zeta) U0 - U1).  Two independent accumulator sets (even / odd pairs).
 template <typename T>
@@ -125,23 +190,25 @@ __device__ __forceinline__ cd angular_near(cd eta, cd zeta, double mu0, const T*
   return s;
 }
 
-// FAR: S = omega [ delta P(omega) + N(omega) ], K terms (Horner from the top).
-__device__ __forceinline__ cd angular_far(cd delta, cd zeta, int K, const double* __restrict__ smu,
-                                          const double* __restrict__ snu) {
-  const cd om = cinv(zeta);
-  double pr = smu[K - 1], pi = 0.0, nr = snu[K - 1], ni = 0.0;
-#pragma unroll 1
-  for (int k = K - 2; k >= 0; --k) {
-    const double m = smu[k], n = snu[k];
-    const double tpr = fma(pr, om.re, fma(-pi, om.im, m));
-    pi = fma(pr, om.im, pi * om.re);
-    pr = tpr;
-    const double tnr = fma(nr, om.re, fma(-ni, om.im, n));
-    ni = fma(nr, om.im, ni * om.re);
-    nr = tnr;
+// ---- series routes: P(s) = sum_k a_k s^k and N(s) = sum_k b_k s^k, real coefficients (a_k, b_k) =
+// tab[k], complex s, by the second-order (Goertzel) recurrence c_k = coef_k + r c_{k+1} - |s|^2 c_{k+2},
+// r = 2 Re s, run from k = Kw-1 down to 0 (Kw even): P(s) = c_0 - c_1 conj(s).  On return p1 = c_0,
+// p2 = c_1 (and n1, n2 for N).  Two real DFMA per coefficient instead of a complex multiply-add.
+template <typename T>
+__device__ __forceinline__ void goertzel_pair(const typename Vec2<T>::type* __restrict__ tab, int Kw, T r, T ns,
+                                              T& p1, T& p2, T& n1, T& n2) {
+  typedef typename Vec2<T>::type V2;
+  p1 = p2 = n1 = n2 = (T)0;
+  const V2* c = tab + Kw;
+#pragma unroll 2
+  for (int k = Kw; k > 0; k -= 2) {
+    c -= 2;
+    const V2 c1 = c[1], c0 = c[0];
+    p2 = fma(r, p1, fma(ns, p2, c1.x));
+    n2 = fma(r, n1, fma(ns, n2, c1.y));
+    p1 = fma(r, p2, fma(ns, p1, c0.x));
+    n1 = fma(r, n2, fma(ns, n1, c0.y));
   }
-  const cd acc = {fma(delta.re, pr, fma(-delta.im, pi, nr)), fma(delta.re, pi, fma(delta.im, pr, ni))};
-  return cmul(om, acc);
 }
 
 // EXACT: zeta = A^2/(4 x y) in double-double, A = x + y + mu (y complex on a deformed contour); every
@@ -175,6 +242,115 @@ __device__ __noinline__ cd angular_exact(double xr, double xi, double yr, double
   return {sr, si};
 }
 
+// ---------------------------------------------------------------------------------------------
+// One (point, radial node, pole): S(delta, zeta) by the route zeta selects.  delta = eta - 1/4.
+// WARP-COLLECTIVE: all 32 lanes must call it together (the series loop runs to the warp's longest
+// series, lanes on other routes idle through it; extra terms are below 2^-58 and harmless).
+//   MOMENT  max(|Re zeta|, |Im zeta|) >= 4.5: s = 1/(zeta - 1/2), S = s [delta P(s) - N(s)] with the moments
+//           a_k = sum_j w_j (t_j - 1/2)^k, b_k = sum_j w_j (t_j - 1/4)(t_j - 1/2)^k; |t - 1/2| <= 1/2 and
+//           |s| <= 1/4, so K = 58/(1 - log2|s|) + 2 <= 22 terms.
+//   CHEB    else, with w = 2 zeta - 1 and s = 1/(w + sqrt(w^2 - 1)) the smaller root of s + 1/s = 2w
+//           (|s| = 1/rho, rho the parameter of the ellipse with foci 0, 1 through zeta):
+//           1/(zeta - t) = 4/sqrt(w^2-1) sum'_k s^k T_k(2t-1), so S = 4/sqrt(w^2-1) [delta P(s) - N(s)] with the
+//           Chebyshev moments a_k = sum_j w_j T_k(2t_j-1), b_k = sum_j w_j (t_j - 1/4) T_k(2t_j-1) (k = 0 halved);
+//           K = 60/log2(rho) + 2 terms, taken when K <= kmc and cheaper than the NEAR loop.
+//   EXACT   zeta within tau of [0,1];   NEAR  the rest (zeta close to [0,1], or few angular nodes).
+// ---------------------------------------------------------------------------------------------
+template <typename T, bool COUNT>
+__device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta, cd zeta, double mur, double mui,
+                                        RouteCount& rc) {
+  typedef typename Vec2<T>::type V2;
+  const double mx = fmax(fabs(zeta.re), fabs(zeta.im));
+  int route, K = 0;
+  cd sg = {0.0, 0.0}, g = {0.0, 0.0};   // series argument s and prefactor
+  double ns = 0.0;                      // -|s|^2
+  if (mx >= kMomentMin) {
+    route = ROUTE_MOMENT;
+    const cd zc = {zeta.re - 0.5, zeta.im};
+    if (mx < 0x1p400) {
+      const double in = rcp_fast(fma(zc.re, zc.re, zc.im * zc.im));
+      sg = {zc.re * in, -zc.im * in};
+      ns = -in;
+    } else {
+      sg = cinv(zc);
+      ns = -fma(sg.re, sg.re, sg.im * sg.im);
+    }
+    g = sg;
+    const float l2 = __log2f((float)(-ns));        // log2 |s|^2 <= -4 (-inf when it underflows)
+    K = (int)(116.f / (2.f - l2)) + 2;             // (|s|/2)^K <= 2^-58
+  } else {
+    const float zr = (float)zeta.re, zi = (float)zeta.im, zi2 = zi * zi;
+    const float ssum = sqrtf(fmaf(zr, zr, zi2)) + sqrtf(fmaf(zr - 1.f, zr - 1.f, zi2));  // (rho + 1/rho)/2
+    const float rho = ssum + sqrtf(fmaxf(fmaf(ssum, ssum, -1.f), 0.f));
+    const float kc = 60.f / __log2f(rho);
+    K = kc < 4096.f ? (int)kc + 2 : 1 << 20;       // rho -> 1 (or NaN): never CHEB
+    if (K <= tb.kmc && 4 * K + kChebNodeCost < 8 * tb.n_pairs + kNearNodeCost) {
+      route = ROUTE_CHEB;
+      // root = sqrt(zeta (zeta - 1)) = sqrt(w^2 - 1)/2, sign such that |w + 2 root| >= 1
+      const double zm = zeta.re - 1.0, wr = fma(2.0, zeta.re, -1.0), wi = zeta.im + zeta.im;
+      const double qr = fma(zeta.re, zm, -(zeta.im * zeta.im)), qi = zeta.im * wr;
+      const double n2 = fma(qr, qr, qi * qi);
+      const double rm = rsqrt_fast(n2);            // 1/|q|
+      const double h2 = 0.5 * fma(n2, rm, fabs(qr));
+      const double rh = rsqrt_fast(h2);
+      const double h = h2 * rh, kk = 0.5 * qi * rh;
+      double ar = qr >= 0.0 ? h : fabs(kk);
+      double ai = qr >= 0.0 ? kk : copysign(h, qi);
+      if (fma(wr, ar, wi * ai) < 0.0) { ar = -ar; ai = -ai; }
+      const double Dr = fma(2.0, ar, wr), Di = fma(2.0, ai, wi);
+      const double in = rcp_fast(fma(Dr, Dr, Di * Di));
+      sg = {Dr * in, -Di * in};
+      ns = -in;
+      const double g2 = rm + rm;                   // 4/sqrt(w^2-1) = 2 conj(root)/|q|
+      g = {ar * g2, -ai * g2};
+    } else {
+      K = 0;
+      route = (zeta.im * zeta.im < tb.tau * tb.tau && zeta.re > -tb.tau && zeta.re < 1.0 + tb.tau) ? ROUTE_EXACT
+                                                                                                   : ROUTE_NEAR;
+    }
+  }
+  int Kw = __reduce_max_sync(0xffffffffu, K);
+  Kw = min((Kw + 1) & ~1, tb.kmc);
+  cd s = {0.0, 0.0};
+  if (Kw > 0) {  // warp-uniform
+    const V2* tab = route == ROUTE_CHEB ? tb.cheb : tb.mom;
+    T p1, p2, n1, n2;
+    goertzel_pair<T>(tab, Kw, (T)(sg.re + sg.re), (T)ns, p1, p2, n1, n2);
+    if (COUNT) rc.series_exec += Kw;
+    if (route <= ROUTE_CHEB) {
+      const double b0 = (double)p1, b1 = (double)p2, d0 = (double)n1, d1 = (double)n2;
+      const double Pr = fma(-b1, sg.re, b0), Pi = b1 * sg.im;     // c_0 - c_1 conj(s)
+      const double Nr = fma(-d1, sg.re, d0), Ni = d1 * sg.im;
+      const cd acc = {fma(delta.re, Pr, fma(-delta.im, Pi, -Nr)), fma(delta.re, Pi, fma(delta.im, Pr, -Ni))};
+      s = cmul(g, acc);
+      if (COUNT) {
+        rc.series_used += K;
+        if (route == ROUTE_CHEB) ++rc.n_cheb; else ++rc.n_moment;
+      }
+    }
+  }
+  if (route == ROUTE_EXACT) {
+    s = angular_exact(x.re, x.im, y.re, y.im, mur, mui, cd{__dadd_rn(0.25, delta.re), delta.im}, tb.st, tb.stlo, tb.sw,
+                      tb.n_pairs);
+    if (COUNT) { rc.exact_pairs += tb.n_pairs; ++rc.n_exact; }
+  } else if (route == ROUTE_NEAR) {
+    s = angular_near<T>(cd{__dadd_rn(0.25, delta.re), delta.im}, zeta, tb.mu0, tb.stT, tb.swT, tb.n_pairs);
+    if (COUNT) { rc.near_pairs += tb.n_pairs; ++rc.n_near; }
+  }
+  return s;
+}
+
+// Add this thread's counters to the launch's (one atomic per warp and counter)
+__device__ __forceinline__ void flush_counters(const RouteCount& rc, bool active, unsigned long long* counters) {
+  unsigned long long v[kNumCounters] = {rc.near_pairs, rc.series_exec, rc.exact_pairs, rc.n_near,
+                                        rc.n_moment,   rc.n_exact,     rc.n_cheb,      rc.series_used};
+  for (int k = 0; k < kNumCounters; ++k) {
+    if (!active) v[k] = 0;
+    for (int o = 16; o; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+    if ((threadIdx.x & 31) == 0 && v[k]) atomicAdd(counters + k, v[k]);
+  }
+}
+
 // Stage the folded angular rule: pair j = nodes (j, n_ang-1-j); t = z^2 (hi + lo exactly), weight =
 // w_j + w_mirror (the middle node of an odd rule enters once).  *bad is set if the rule is not symmetric.
 __device__ void prep_angular(const EvalArgs& a, const BlobLayout& L, double* blob, int* bad) {
@@ -205,6 +381,30 @@ __device__ void prep_angular(const EvalArgs& a, const BlobLayout& L, double* blo
   }
 }
 
+// The series coefficients of the folded rule (call after prep_angular and a __syncthreads()):
+//   phase 1 (prep_series_T): T_k(2 t_j - 1), k < kmc, by the three-term recurrence in double-double, one
+//            thread per node j, into the scratch matrix [j][k];
+//   phase 2 (prep_series_sums, after a __syncthreads()): one thread per k sums over the nodes with
+//            double-double accumulators.
+__device__ void prep_series_T(const EvalArgs& a, const BlobLayout& L, double* blob) {
+  double* scratch = blob + L.off_scratch;
+  for (int j = threadIdx.x; j < a.n_pairs; j += blockDim.x) {
+    // s = 2 t - 1 with t = hi + lo exactly
+    const dd s2 = dd_add_d(dd{2.0 * blob[L.off_t + j], 2.0 * blob[L.off_tlo + j]}, -1.0);
+    const dd twos = dd_scale2(s2, 2.0);
+    dd Tm = {1.0, 0.0}, Tk = s2;
+    double* row = scratch + (size_t)j * L.kmc;
+    row[0] = 1.0;
+    row[1] = Tk.hi;
+    for (int k = 2; k < L.kmc; ++k) {
+      const dd Tn = dd_add(dd_mul(twos, Tk), dd_neg(Tm));
+      Tm = Tk;
+      Tk = Tn;
+      row[k] = Tn.hi;
+    }
+  }
+}
+
 __device__ __forceinline__ double powi(double t, int k) {
   double r = 1.0;
   while (k) {
@@ -213,6 +413,38 @@ __device__ __forceinline__ double powi(double t, int k) {
     k >>= 1;
   }
   return r;
+}
+
+__device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double* blob) {
+  const double* scratch = blob + L.off_scratch;
+  float2* momf = L.off_f32 >= 0 ? reinterpret_cast<float2*>(reinterpret_cast<float*>(blob + L.off_f32) + 2 * L.npad)
+                                : nullptr;
+  float2* chebf = momf ? momf + L.kmc : nullptr;
+  for (int k = threadIdx.x; k < L.kmc; k += blockDim.x) {
+    dd tau = {0.0, 0.0}, nu = {0.0, 0.0}, mo = {0.0, 0.0}, no = {0.0, 0.0};
+    for (int j = 0; j < a.n_pairs; ++j) {
+      const double t = blob[L.off_t + j], w = blob[L.off_w + j], tq = t - 0.25;
+      const double wT = w * scratch[(size_t)j * L.kmc + k];
+      tau = dd_add_d(tau, wT);
+      nu = dd_add(nu, two_prod(wT, tq));
+      if (k < kMomTerms) {
+        const double wp = w * powi(t - 0.5, k);
+        mo = dd_add_d(mo, wp);
+        no = dd_add(no, two_prod(wp, tq));
+      }
+    }
+    const double half = k == 0 ? 0.5 : 1.0;   // sum' : the k = 0 term of a Chebyshev series is halved
+    const double c0 = half * tau.hi, c1 = half * nu.hi;
+    const double m0 = k < kMomTerms ? mo.hi : 0.0, m1 = k < kMomTerms ? no.hi : 0.0;
+    blob[L.off_cheb + 2 * k] = c0;
+    blob[L.off_cheb + 2 * k + 1] = c1;
+    blob[L.off_mom + 2 * k] = m0;
+    blob[L.off_mom + 2 * k + 1] = m1;
+    if (momf) {
+      chebf[k] = make_float2((float)c0, (float)c1);
+      momf[k] = make_float2((float)m0, (float)m1);
+    }
+  }
 }
 
 }  // namespace
