@@ -242,7 +242,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
       const cd s = node_term<double, COUNT>(tb, x, y, delta, zeta, mur, mui, rc);
       cd pr;
       if (table) {
-        const double2 p2 = spref[r * a.n_rad + i];
+        const double2 p2 = spref[r * L.n_rad_pad + i];
         pr = {p2.x, p2.y};
       } else {
         const cd ic = cinv(cd{y.re + mur, y.im + mui});

@@ -90,17 +90,18 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
     // shifted-log map of [0, Lambda^2] (readings G3/G4): y(u) = s0 expm1(u L), dy/du = L (y + s0),
     // L = ln((Lambda^2 + s0)/s0) as a double-double from the host; y_i correctly rounded.
     const dd Llog = {a.Llog_hi, a.Llog_lo};
-    for (int i = threadIdx.x; i < a.n_rad; i += blockDim.x) {
+    for (int ip = threadIdx.x; ip < L.n_rad_pad; ip += blockDim.x) {
+      const int i = min(ip, a.n_rad - 1);            // padding: the last node again, prefactor 0
       const double y = radial_node(a.rad_nodes[i], Llog, a.s0);
-      const double Wr = 0.5 * a.rad_weights[i] * a.Llog_hi * (y + a.s0);
-      blob[L.off_y + i] = y;
-      blob[L.off_q4 + i] = 0.25 / y;
+      const double Wr = ip < a.n_rad ? 0.5 * a.rad_weights[i] * a.Llog_hi * (y + a.s0) : 0.0;
+      blob[L.off_y + ip] = y;
+      blob[L.off_q4 + ip] = 0.25 / y;
       const cd d1 = cscale(line_k_real(a.line_k, y), a.c0 * Wr * y);
       for (int r = 0; r < a.n_terms; ++r) {
         const cd ic = cinv(cd{y + a.term[r].mu_re, a.term[r].mu_im});
         const cd pr = cmul(cmul(d1, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);
-        blob[L.off_pref + 2 * (r * a.n_rad + i)] = pr.re;
-        blob[L.off_pref + 2 * (r * a.n_rad + i) + 1] = pr.im;
+        blob[L.off_pref + 2 * (r * L.n_rad_pad + ip)] = pr.re;
+        blob[L.off_pref + 2 * (r * L.n_rad_pad + ip) + 1] = pr.im;
       }
     }
   }
@@ -120,7 +121,7 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
 // ---------------------------------------------------------------------------------------------
 // Evaluation, REAL contour.  counters (COUNT only): gf.h, gf_eval_grid_counted.
 // ---------------------------------------------------------------------------------------------
-template <typename T, bool COUNT>
+template <typename T, bool COUNT, int NT>
 __global__ void __launch_bounds__(kBlockThreads, 3)
     eval_real_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                      const double* __restrict__ blob, unsigned long long* __restrict__ counters) {
@@ -133,9 +134,6 @@ __global__ void __launch_bounds__(kBlockThreads, 3)
   mbar_wait(bar, 0);
 
   const Tabs<T> tb = make_tabs<T>(sb, L, a.n_pairs);
-  const double* sy = sb + L.off_y;
-  const double* sq4 = sb + L.off_q4;
-  const double2* spref = reinterpret_cast<const double2*>(sb + L.off_pref);
   const bool bad_rule = sb[0] != 0.0;
 
   const int S = 1 << a.split_log2;
@@ -161,27 +159,28 @@ __global__ void __launch_bounds__(kBlockThreads, 3)
     out_scale = scalbn(1.0, -k);
   }
   const cd xinv = cinv(x);
+  cd xm[NT];  // x + mu_r
+#pragma unroll
+  for (int r = 0; r < NT; ++r) xm[r] = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
 
   RouteCount rc;
   double g_re = 0.0, g_im = 0.0;
   // warp-synchronous node loop: every lane makes the same number of trips (node_term is warp-collective);
-  // a lane past the last node repeats it with weight 0
+  // the node tables are padded to a multiple of 32 with zero-weight copies of the last node
+  const double* py = sb + L.off_y + sub;
+  const double* pq4 = sb + L.off_q4 + sub;
+  const double2* ppref = reinterpret_cast<const double2*>(sb + L.off_pref) + sub;
 #pragma unroll 1
-  for (int i0 = 0; i0 < a.n_rad; i0 += S) {
-    const bool valid = i0 + sub < a.n_rad;
-    const int i = valid ? i0 + sub : a.n_rad - 1;
-    const double y = sy[i], q4 = sq4[i];
+  for (int i0 = 0; i0 < a.n_rad; i0 += S, py += S, pq4 += S, ppref += S) {
+    const double y = *py, q4 = *pq4;
     const cd xq = cscale(xinv, q4);                  // 1/(4 x y)
-#pragma unroll 1
-    for (int r = 0; r < a.n_terms; ++r) {
-      const double mur = a.term[r].mu_re, mui = a.term[r].mu_im;
-      const cd xm = {x.re + mur, x.im + mui};
-      const cd A = {xm.re + y, xm.im};
-      const cd delta = cscale(xm, q4);               // eta - 1/4
+#pragma unroll
+    for (int r = 0; r < NT; ++r) {
+      const cd A = {xm[r].re + y, xm[r].im};
+      const cd delta = cscale(xm[r], q4);            // eta - 1/4
       const cd zeta = cmul(csqr(A), xq);
-      const cd s = node_term<T, COUNT>(tb, x, cd{y, 0.0}, delta, zeta, mur, mui, rc);
-      double2 pr = spref[r * a.n_rad + i];
-      if (!valid) pr = make_double2(0.0, 0.0);
+      const cd s = node_term<T, COUNT>(tb, x, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc);
+      const double2 pr = ppref[r * L.n_rad_pad];
       g_re = fma(pr.x, s.re, fma(-pr.y, s.im, g_re));
       g_im = fma(pr.x, s.im, fma(pr.y, s.re, g_im));
     }
@@ -213,9 +212,10 @@ BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyram
   L.off_w = take(L.npad);
   L.off_mom = take(2 * L.kmc);
   L.off_cheb = take(2 * L.kmc);
-  L.off_y = take(n_rad);
-  L.off_q4 = take(n_rad);
-  L.off_pref = take(2 * n_terms * n_rad);
+  L.n_rad_pad = (n_rad + 31) & ~31;
+  L.off_y = take(L.n_rad_pad);
+  L.off_q4 = take(L.n_rad_pad);
+  L.off_pref = take(2 * n_terms * L.n_rad_pad);
   // 2 float tables of npad entries = npad doubles; 2 float2 tables of kmc entries = 2 kmc doubles
   L.off_f32 = f32 ? take(L.npad + 2 * L.kmc) : -1;
   L.n_tab = pyramid ? n_rad + n_rad / 2 + n_rad / 4 + n_rad / 8 : 0;
@@ -254,10 +254,10 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   return GF_OK;
 }
 
-template <typename T, bool COUNT>
-static int launch_real(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
-                       cudaStream_t stream) {
-  auto kern = eval_real_kernel<T, COUNT>;
+template <typename T, bool COUNT, int NT>
+static int launch_real_nt(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
+                          cudaStream_t stream) {
+  auto kern = eval_real_kernel<T, COUNT, NT>;
   if (plan.smem_bytes > 48 * 1024) {
     int rc = check_cuda(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes),
                         "cudaFuncSetAttribute(max dynamic shared memory)");
@@ -265,6 +265,12 @@ static int launch_real(const EvalArgs& a, const LaunchPlan& plan, const double* 
   }
   kern<<<(unsigned)plan.grid_blocks, plan.block_threads, plan.smem_bytes, stream>>>(a, plan.layout, blob, counters);
   return check_cuda(cudaGetLastError(), "eval kernel launch");
+}
+template <typename T, bool COUNT>
+static int launch_real(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
+                       cudaStream_t stream) {
+  return a.n_terms == 1 ? launch_real_nt<T, COUNT, 1>(a, plan, blob, counters, stream)
+                        : launch_real_nt<T, COUNT, 2>(a, plan, blob, counters, stream);
 }
 
 int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d_nodes, int n, double* d_y,

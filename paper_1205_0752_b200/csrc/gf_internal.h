@@ -46,8 +46,9 @@ struct BlobLayout {
   int kmc;                      // series coefficients k = 0 .. kmc-1 (even)
   int off_t, off_tlo, off_w;    // folded angular rule: t = z^2 (hi, lo), weight
   int off_mom, off_cheb;        // double2 (P_k, N_k)[kmc]: centred-moment series, Chebyshev series
-  int off_y, off_q4;            // radial nodes y_i, 1/(4 y_i)
-  int off_pref;                 // double2 pref[n_terms][n_rad]
+  int n_rad_pad;                // n_rad rounded up to 32: padding repeats the last node with prefactor 0
+  int off_y, off_q4;            // radial nodes y_i, 1/(4 y_i), n_rad_pad each
+  int off_pref;                 // double2 pref[n_terms][n_rad_pad]
   int off_f32;                  // FP32 variant: float t[npad], w[npad], float2 mom[kmc], cheb[kmc]; or -1
   int off_rt, off_rw, n_tab;    // point-dependent contours: the radial rule pyramid (nodes, weights) or -1
   int n_doubles;                // doubles every CTA stages (even)

@@ -260,51 +260,42 @@ template <typename T, bool COUNT>
 __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta, cd zeta, double mur, double mui,
                                         RouteCount& rc) {
   typedef typename Vec2<T>::type V2;
-  const double mx = fmax(fabs(zeta.re), fabs(zeta.im));
-  int route, K = 0;
-  cd sg = {0.0, 0.0}, g = {0.0, 0.0};   // series argument s and prefactor
-  double ns = 0.0;                      // -|s|^2
-  if (mx >= kMomentMin) {
+  int route, K;
+  cd sg, g;     // series argument s and prefactor
+  double ns;    // -|s|^2
+  if (fabs(zeta.re) >= kMomentMin || fabs(zeta.im) >= kMomentMin) {
     route = ROUTE_MOMENT;
-    const cd zc = {zeta.re - 0.5, zeta.im};
-    if (mx < 0x1p400) {
-      const double in = rcp_fast(fma(zc.re, zc.re, zc.im * zc.im));
-      sg = {zc.re * in, -zc.im * in};
-      ns = -in;
-    } else {
-      sg = cinv(zc);
-      ns = -fma(sg.re, sg.re, sg.im * sg.im);
-    }
+    const double zc = zeta.re - 0.5;
+    const double in = rcp_fast(fma(zc, zc, zeta.im * zeta.im));   // |zeta| < 2^500 (gf.h: domain)
+    sg = {zc * in, -zeta.im * in};
+    ns = -in;
     g = sg;
-    const float l2 = __log2f((float)(-ns));        // log2 |s|^2 <= -4 (-inf when it underflows)
-    K = (int)(116.f / (2.f - l2)) + 2;             // (|s|/2)^K <= 2^-58
+    // (|s|/2)^K <= 2^-58;  log2 |s|^2 <= -4 (-inf when it underflows in FP32: K = 2)
+    K = (int)__fdividef(116.f, 2.f - __log2f((float)in)) + 2;
   } else {
-    const float zr = (float)zeta.re, zi = (float)zeta.im, zi2 = zi * zi;
-    const float ssum = sqrtf(fmaf(zr, zr, zi2)) + sqrtf(fmaf(zr - 1.f, zr - 1.f, zi2));  // (rho + 1/rho)/2
-    const float rho = ssum + sqrtf(fmaxf(fmaf(ssum, ssum, -1.f), 0.f));
-    const float kc = 60.f / __log2f(rho);
-    K = kc < 4096.f ? (int)kc + 2 : 1 << 20;       // rho -> 1 (or NaN): never CHEB
-    if (K <= tb.kmc && 4 * K + kChebNodeCost < 8 * tb.n_pairs + kNearNodeCost) {
-      route = ROUTE_CHEB;
-      // root = sqrt(zeta (zeta - 1)) = sqrt(w^2 - 1)/2, sign such that |w + 2 root| >= 1
-      const double zm = zeta.re - 1.0, wr = fma(2.0, zeta.re, -1.0), wi = zeta.im + zeta.im;
-      const double qr = fma(zeta.re, zm, -(zeta.im * zeta.im)), qi = zeta.im * wr;
-      const double n2 = fma(qr, qr, qi * qi);
-      const double rm = rsqrt_fast(n2);            // 1/|q|
-      const double h2 = 0.5 * fma(n2, rm, fabs(qr));
-      const double rh = rsqrt_fast(h2);
-      const double h = h2 * rh, kk = 0.5 * qi * rh;
-      double ar = qr >= 0.0 ? h : fabs(kk);
-      double ai = qr >= 0.0 ? kk : copysign(h, qi);
-      if (fma(wr, ar, wi * ai) < 0.0) { ar = -ar; ai = -ai; }
-      const double Dr = fma(2.0, ar, wr), Di = fma(2.0, ai, wi);
-      const double in = rcp_fast(fma(Dr, Dr, Di * Di));
-      sg = {Dr * in, -Di * in};
-      ns = -in;
-      const double g2 = rm + rm;                   // 4/sqrt(w^2-1) = 2 conj(root)/|q|
-      g = {ar * g2, -ai * g2};
-    } else {
-      K = 0;
+    // root = sqrt(zeta (zeta - 1)) = sqrt(w^2 - 1)/2, sign such that |w + 2 root| >= 1
+    const double zm = zeta.re - 1.0, wr = fma(2.0, zeta.re, -1.0), wi = zeta.im + zeta.im;
+    const double qr = fma(zeta.re, zm, -(zeta.im * zeta.im)), qi = zeta.im * wr;
+    const double n2 = fma(qr, qr, qi * qi);
+    const double rm = rsqrt_fast(n2);            // 1/|q|
+    const double h2 = 0.5 * fma(n2, rm, fabs(qr));
+    const double rh = rsqrt_fast(h2);
+    const double h = h2 * rh, kk = 0.5 * qi * rh;
+    double ar = qr >= 0.0 ? h : fabs(kk);
+    double ai = qr >= 0.0 ? kk : copysign(h, qi);
+    if (fma(wr, ar, wi * ai) < 0.0) { ar = -ar; ai = -ai; }
+    const double Dr = fma(2.0, ar, wr), Di = fma(2.0, ai, wi);
+    const double in = rcp_fast(fma(Dr, Dr, Di * Di));   // 1/rho^2
+    sg = {Dr * in, -Di * in};
+    ns = -in;
+    const double g2 = rm + rm;                   // 4/sqrt(w^2-1) = 2 conj(root)/|q|
+    g = {ar * g2, -ai * g2};
+    // rho^-K <= 2^-60.  zeta on [0,1] itself gives rho = 1 or NaN: the comparison below fails, never CHEB
+    const float kc = __fdividef(-120.f, __log2f((float)in));
+    K = kc < 4096.f ? (int)kc + 2 : 1 << 20;
+    route = ROUTE_CHEB;
+    if (!(K <= tb.kmc && 4 * K + kChebNodeCost < 8 * tb.n_pairs + kNearNodeCost)) {
+      K = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
       route = (zeta.im * zeta.im < tb.tau * tb.tau && zeta.re > -tb.tau && zeta.re < 1.0 + tb.tau) ? ROUTE_EXACT
                                                                                                    : ROUTE_NEAR;
     }

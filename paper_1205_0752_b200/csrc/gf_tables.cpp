@@ -3,7 +3,10 @@
 // Library code; shares nothing with oracle/.
 #include <quadmath.h>
 
+#include <algorithm>
 #include <cmath>
+#include <functional>
+#include <thread>
 #include <vector>
 
 #include "gf_internal.h"
@@ -14,7 +17,7 @@ namespace {
 typedef long double real;
 const real PI = 3.141592653589793238462643383279502884L;
 
-// Legendre P_n(t) and P_{n-1}(t) by the three-term recurrence (Bonnet).
+// Legendre P_n(t) and P_{n-1}(t) by the three-term recurrence (Bonnet), extended precision.
 inline void legendre_pair(int n, real t, real* pn, real* pnm1) {
   real a = 1.0L, b = t;  // P_0, P_1
   if (n == 0) { *pn = a; *pnm1 = 0; return; }
@@ -27,29 +30,107 @@ inline void legendre_pair(int n, real t, real* pn, real* pnm1) {
   *pnm1 = a;
 }
 
-// Gauss-Legendre (ref. [18]).  Positive roots by Newton's method from Tricomi's
-// estimate; weights from w = 2 / ((1 - t^2) P_n'(t)^2) (A-S 25.4.29; the equivalent form with P_{n-1} is n
-// times more sensitive to the last-bit error of the root).  Mirrored, so the rule is exactly symmetric.
+// The same in double with the coefficients al_k = (2k+1)/(k+1), be_k = k/(k+1) tabulated (no division in
+// the loop): only used to bring Tricomi's estimate to a double-precision root quickly.
+struct BonnetD {
+  std::vector<double> al, be;
+  explicit BonnetD(int n) : al(n + 1), be(n + 1) {
+    for (int k = 0; k <= n; ++k) {
+      al[k] = (2.0 * k + 1.0) / (k + 1.0);
+      be[k] = (double)k / (k + 1.0);
+    }
+  }
+  void pair(int n, double t, double* pn, double* pnm1) const {
+    double a = 1, b = t;
+    for (int k = 1; k < n; ++k) {
+      const double c = al[k] * t * b - be[k] * a;
+      a = b;
+      b = c;
+    }
+    *pn = b;
+    *pnm1 = a;
+  }
+};
+
+// legendre_pair for kLanes points at once: the same operations per point in the same order (bit-identical
+// results), interleaved so that the divisions of independent recurrences overlap in the pipeline.
+constexpr int kLanes = 4;
+inline void legendre_pair_lanes(int n, const real* t, real* pn, real* pnm1) {
+  real a[kLanes], b[kLanes];
+  for (int l = 0; l < kLanes; ++l) { a[l] = 1.0L; b[l] = t[l]; }
+  for (int k = 1; k < n; ++k) {
+    for (int l = 0; l < kLanes; ++l) {
+      real c = ((2 * k + 1) * t[l] * b[l] - k * a[l]) / (k + 1);
+      a[l] = b[l];
+      b[l] = c;
+    }
+  }
+  for (int l = 0; l < kLanes; ++l) { pn[l] = b[l]; pnm1[l] = a[l]; }
+}
+
+// Positive roots m0 <= m < m1 (counted from the largest) of P_n and their weights.
+void gauss_legendre_roots(int n, int m0, int m1, const BonnetD& Bd, double* x, double* w) {
+  for (int mb = m0; mb < m1; mb += kLanes) {
+    real t[kLanes], pn[kLanes], pm[kLanes];
+    bool done[kLanes];
+    for (int l = 0; l < kLanes; ++l) {
+      const int m = mb + l < m1 ? mb + l : m1 - 1;   // a short last group repeats its last root
+      const double th = (double)(PI * (4 * (m + 1) - 1) / (4 * (real)n + 2));
+      const double dn = n, sn = std::sin(th);
+      double t0 = (1 - (dn - 1) / (8 * dn * dn * dn) - 1 / (384 * dn * dn * dn * dn) * (39 - 28 / (sn * sn))) * std::cos(th);
+      for (int it = 0; it < 20; ++it) {
+        double p, q;
+        Bd.pair(n, t0, &p, &q);
+        const double dt = p * (1 - t0 * t0) / (dn * (q - t0 * p));
+        t0 -= dt;
+        if (std::fabs(dt) <= 4e-16 * std::fabs(t0)) break;
+      }
+      t[l] = t0;
+      done[l] = false;
+    }
+    for (int it = 0; it < 50; ++it) {
+      legendre_pair_lanes(n, t, pn, pm);
+      bool all = true;
+      for (int l = 0; l < kLanes; ++l) {
+        if (done[l]) continue;
+        const real dpn = n * (pm[l] - t[l] * pn[l]) / (1 - t[l] * t[l]);
+        const real dt = pn[l] / dpn;
+        t[l] -= dt;
+        done[l] = fabsl(dt) <= 1e-12L * fabsl(t[l]);  // quadratic: the next correction is below 1e-21
+        all = all && done[l];
+      }
+      if (all) break;
+    }
+    legendre_pair_lanes(n, t, pn, pm);
+    for (int l = 0; l < kLanes && mb + l < m1; ++l) {
+      const int m = mb + l;
+      const real dpn = n * (pm[l] - t[l] * pn[l]) / (1 - t[l] * t[l]);
+      const real wt = 2 / ((1 - t[l] * t[l]) * dpn * dpn);
+      x[n - 1 - m] = (double)t[l];
+      x[m] = -(double)t[l];
+      w[n - 1 - m] = w[m] = (double)wt;
+    }
+  }
+}
+
+// Gauss-Legendre (ref. [18]).  Positive roots: Tricomi's estimate, Newton's method in double to
+// its limit, then Newton in extended precision (one step brings |dt| from ~1e-16 to ~1e-28); weights from
+// w = 2 / ((1 - t^2) P_n'(t)^2) (A-S 25.4.29; the equivalent form with P_{n-1} is n times more sensitive to
+// the last-bit error of the root) with P_n' from one more extended-precision evaluation at the final root.
+// Mirrored, so the rule is exactly symmetric.  Roots are independent: large rules are split over up to 8 threads.
 void gauss_legendre(int n, double* x, double* w) {
   const int half = n / 2;
-  for (int m = 0; m < half; ++m) {
-    // m-th positive root counted from the largest
-    real th = PI * (4 * (m + 1) - 1) / (4 * (real)n + 2);
-    real t = (1 - (real)(n - 1) / (8 * (real)n * n * n) - 1 / (384 * (real)n * n * n * n) * (39 - 28 / (sinl(th) * sinl(th)))) * cosl(th);
-    real pn, pm;
-    for (int it = 0; it < 50; ++it) {
-      legendre_pair(n, t, &pn, &pm);
-      real dpn = n * (pm - t * pn) / (1 - t * t);
-      real dt = pn / dpn;
-      t -= dt;
-      if (fabsl(dt) <= 2e-20L * fabsl(t)) break;
-    }
-    legendre_pair(n, t, &pn, &pm);
-    const real dpn = n * (pm - t * pn) / (1 - t * t);
-    real wt = 2 / ((1 - t * t) * dpn * dpn);
-    x[n - 1 - m] = (double)t;
-    x[m] = -(double)t;
-    w[n - 1 - m] = w[m] = (double)wt;
+  const BonnetD Bd(n);
+  const unsigned hw = std::thread::hardware_concurrency();
+  const int n_thr = half < 64 ? 1 : std::max(1, std::min({half / 32, 8, hw ? (int)hw : 4}));
+  if (n_thr == 1) {
+    gauss_legendre_roots(n, 0, half, Bd, x, w);
+  } else {
+    // roots near the ends need no more work than the others: equal blocks
+    std::vector<std::thread> pool;
+    for (int k = 0; k < n_thr; ++k)
+      pool.emplace_back(gauss_legendre_roots, n, half * k / n_thr, half * (k + 1) / n_thr, std::cref(Bd), x, w);
+    for (auto& th : pool) th.join();
   }
   if (n & 1) {
     real pn, pm;
