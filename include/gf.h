@@ -149,10 +149,11 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
                       long long n_points, void* h_out, void* stream);
 
 /* The same evaluation, also counting the work by route for the roofline accounting.
- * d_counters: 8 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
+ * d_counters: 9 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
  *   [0] NEAR pairs  [1] series terms EXECUTED (every lane of a warp runs its warp's longest series)
  *   [2] EXACT pairs  [3] [4] [5] [6] (point, radial node, pole) triples taken by the NEAR / MOMENT / EXACT / CHEB
- *   route  [7] series terms NEEDED (the sum over series triples of their own K).  Results are identical to
+ *   route (the triples of the large-y tail are not among them)  [7] series terms NEEDED (the sum over series
+ *   triples of their own K)  [8] tail series evaluated, one per (point, pole).  Results are identical to
  *   gf_eval_grid. */
 int gf_eval_grid_counted(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
                          const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
@@ -179,6 +180,7 @@ typedef struct {
   double node_moment_dfma, node_moment_other;
   double node_cheb_dfma, node_cheb_other;
   double node_exact_dfma, node_exact_other;
+  double tail_dfma, tail_other;                                   /* per tail series (point, pole) */
 } gf_launch_info;
 int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_points, gf_launch_info* out);
 

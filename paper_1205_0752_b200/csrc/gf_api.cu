@@ -284,6 +284,8 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
   out->node_moment_dfma = kNodeMomentDfma; out->node_moment_other = kNodeMomentOther;
   out->node_cheb_dfma = kNodeChebDfma; out->node_cheb_other = kNodeChebOther;
   out->node_exact_dfma = 120; out->node_exact_other = 180;
+  // tail: kTailN (kTailN + 1) DFMA in the recurrences + per n: 2 complex products, 1 complex multiply-add, P
+  out->tail_dfma = kTailN * (kTailN + 1) + 14.0 * kTailN; out->tail_other = 7.0 * kTailN + 30;
   return GF_OK;
 }
 

@@ -81,11 +81,13 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
                                                         const __grid_constant__ BlobLayout L,
                                                         double* __restrict__ blob) {
   __shared__ int bad;
+  __shared__ dd s_mu[kTailN], s_nu[kTailN];
   if (threadIdx.x == 0) bad = 0;
   __syncthreads();
   prep_angular(a, L, blob, &bad);
   __syncthreads();  // t, w written by this CTA are visible to it
   prep_series_T(a, L, blob);
+  if (L.off_gam >= 0) prep_tail_moments(a, L, blob, s_mu, s_nu);
   {
     // shifted-log map of [0, Lambda^2] (readings G3/G4): y(u) = s0 expm1(u L), dy/du = L (y + s0),
     // L = ln((Lambda^2 + s0)/s0) as a double-double from the host; y_i correctly rounded.
@@ -110,12 +112,61 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
       blob[L.off_rt + i] = a.rad_nodes[i];
       blob[L.off_rw + i] = a.rad_weights[i];
     }
-  __syncthreads();  // the T_k(s_j) matrix is complete
+  __syncthreads();  // the T_k(s_j) matrix, the monomial moments and the radial tables are complete
   prep_series_sums(a, L, blob);
+  if (L.off_gam >= 0) {
+    prep_tail_gamma(L, blob, s_mu, s_nu);
+    prep_tail_powers(a, L, blob);
+    __syncthreads();
+    prep_tail_sums(a, L, blob);
+  }
   if (threadIdx.x == 0) {
     blob[0] = bad ? 1.0 : 0.0;
     blob[1] = 0.0;
   }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Tail: all radial nodes with y_i >= Y0(x) at once.  With a = x + mu, eps = 1/y:
+//   S(x, y) = sum_k omega^(k+1) [delta mu_k - nu_k],  omega = 4 x eps/(1 + a eps)^2,  delta = a eps/4
+//           = sum_n eps^n X h_n(X, Z),   X = 4x, Z = -a,   h_n = sum_{k<n} gamma_{n,k} X^k Z^(n-1-k)
+// (binomial series of (1 + a eps)^(-2k-2); gamma_{n,k} in gf_routes.cuh).  The series converges absolutely,
+// term n below 4^-n, for y >= Y0 = 4 (sqrt|x| + sqrt(|x| + |a|))^2, so
+//   sum_{i >= i0} pref_i S(x, y_i) = X sum_n h_n sum_{i >= i0} pref_i y_i^-n = (X/y_i0) sum_n h_n(X/y_i0, Z/y_i0) Rhat_n(i0)
+// with the x-independent tables Rhat_n(i0) made once per launch.  h_n is a real-coefficient polynomial in the
+// ratio of X and Z (the smaller over the larger) and is evaluated by the same second-order recurrence as the
+// angular series.  A log-mapped radial rule has most of its nodes in this tail (about 60 % on the production
+// scan), and they cost kTailN (kTailN + 1) DFMA per point instead of a series each.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ cd tail_series(const double* __restrict__ gam, const double2* __restrict__ Rrow, cd x,
+                                          cd a, double invy0) {
+  const cd X = {4.0 * x.re * invy0, 4.0 * x.im * invy0}, Z = {-a.re * invy0, -a.im * invy0};
+  const double nX = fma(X.re, X.re, X.im * X.im), nZ = fma(Z.re, Z.re, Z.im * Z.im);
+  const bool fwd = nX <= nZ;                        // powers of X/Z, else of Z/X
+  const cd base = fwd ? Z : X, oth = fwd ? X : Z;
+  const double inb = 1.0 / (fwd ? nZ : nX);
+  const cd rho = {fma(oth.re, base.re, oth.im * base.im) * inb, fma(oth.im, base.re, -(oth.re * base.im)) * inb};
+  const double rr = rho.re + rho.re, ns = -fma(rho.re, rho.re, rho.im * rho.im);
+  cd pw = {1.0, 0.0}, acc = {0.0, 0.0};
+  const double* row = gam;
+#pragma unroll 1
+  for (int n = 1; n <= kTailN; ++n) {
+    double b0 = 0.0, b1 = 0.0;
+    const double* c = fwd ? row + n - 1 : row;      // highest power of the ratio first
+    const int step = fwd ? -1 : 1;
+#pragma unroll 1
+    for (int j = 0; j < n; ++j, c += step) {
+      const double t = fma(rr, b0, fma(ns, b1, *c));
+      b1 = b0;
+      b0 = t;
+    }
+    const cd P = {fma(-b1, rho.re, b0), b1 * rho.im};   // c_0 - c_1 conj(rho)
+    const double2 R = Rrow[n - 1];
+    acc = cadd(acc, cmul(cmul(P, pw), cd{R.x, R.y}));
+    pw = cmul(pw, base);
+    row += n;
+  }
+  return cmul(X, acc);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -163,6 +214,25 @@ __global__ void __launch_bounds__(kBlockThreads, 3)
 #pragma unroll
   for (int r = 0; r < NT; ++r) xm[r] = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
 
+  // where the tail series takes over: the first node with y_i >= Y0 = 4 (sqrt|x| + sqrt(|x| + |x + mu|))^2
+  int i_end = a.n_rad;
+  if (L.off_gam >= 0) {
+    const double ax = sqrt(fma(x.re, x.re, x.im * x.im));
+    double Y0 = 0.0;
+#pragma unroll
+    for (int r = 0; r < NT; ++r) {
+      const double q = sqrt(ax) + sqrt(ax + sqrt(fma(xm[r].re, xm[r].re, xm[r].im * xm[r].im)));
+      Y0 = fmax(Y0, 4.0 * q * q);
+    }
+    int lo = 0, hi = a.n_rad;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (sb[L.off_y + mid] < Y0) lo = mid + 1; else hi = mid;
+    }
+    i_end = lo;
+  }
+  const int i_stop = __reduce_max_sync(0xffffffffu, i_end);
+
   RouteCount rc;
   double g_re = 0.0, g_im = 0.0;
   // warp-synchronous node loop: every lane makes the same number of trips (node_term is warp-collective);
@@ -171,8 +241,9 @@ __global__ void __launch_bounds__(kBlockThreads, 3)
   const double* pq4 = sb + L.off_q4 + sub;
   const double2* ppref = reinterpret_cast<const double2*>(sb + L.off_pref) + sub;
 #pragma unroll 1
-  for (int i0 = 0; i0 < a.n_rad; i0 += S, py += S, pq4 += S, ppref += S) {
+  for (int i0 = 0; i0 < i_stop; i0 += S, py += S, pq4 += S, ppref += S) {
     const double y = *py, q4 = *pq4;
+    const bool on = i0 + sub < i_end;                // past its own i_end a lane idles with weight 0
     const cd xq = cscale(xinv, q4);                  // 1/(4 x y)
 #pragma unroll
     for (int r = 0; r < NT; ++r) {
@@ -180,9 +251,23 @@ __global__ void __launch_bounds__(kBlockThreads, 3)
       const cd delta = cscale(xm[r], q4);            // eta - 1/4
       const cd zeta = cmul(csqr(A), xq);
       const cd s = node_term<T, COUNT>(tb, x, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc);
-      const double2 pr = ppref[r * L.n_rad_pad];
+      double2 pr = ppref[r * L.n_rad_pad];
+      if (!on) pr = make_double2(0.0, 0.0);
       g_re = fma(pr.x, s.re, fma(-pr.y, s.im, g_re));
       g_im = fma(pr.x, s.im, fma(pr.y, s.re, g_im));
+    }
+  }
+  if (L.off_gam >= 0 && __any_sync(0xffffffffu, i_end < a.n_rad)) {
+    const double invy0 = 4.0 * sb[L.off_q4 + min(i_end, a.n_rad - 1)];
+    const double2* R = reinterpret_cast<const double2*>(blob + L.off_tail) + (size_t)i_end * kTailN;
+#pragma unroll
+    for (int r = 0; r < NT; ++r) {
+      const cd tl = tail_series(sb + L.off_gam, R + (size_t)r * (a.n_rad + 1) * kTailN, x, xm[r], invy0);
+      if (sub == 0) {
+        g_re += tl.re;
+        g_im += tl.im;
+      }
+      if (COUNT) ++rc.tails;
     }
   }
   // merge the S lanes that share a point
@@ -201,7 +286,7 @@ __global__ void __launch_bounds__(kBlockThreads, 3)
   if (COUNT) flush_counters(rc, active, counters);
 }
 
-BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid) {
+BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail) {
   BlobLayout L;
   L.npad = (n_pairs + 3) & ~3;
   L.kmc = kKmc;
@@ -221,9 +306,12 @@ BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyram
   L.n_tab = pyramid ? n_rad + n_rad / 2 + n_rad / 4 + n_rad / 8 : 0;
   L.off_rt = pyramid ? take(L.n_tab) : -1;
   L.off_rw = pyramid ? take(L.n_tab) : -1;
+  L.off_gam = tail ? take(kTailN * (kTailN + 1) / 2) : -1;
   L.n_doubles = o;
-  L.off_scratch = o;
-  L.n_total = o + L.kmc * L.npad;
+  L.off_tail = tail ? take(2 * n_terms * (n_rad + 1) * kTailN) : -1;
+  L.off_scratch = take(L.kmc * L.npad);
+  L.off_scratch2 = tail ? take(2 * kTailN * n_rad) : -1;
+  L.n_total = o;
   return L;
 }
 
@@ -240,7 +328,7 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   plan->split_log2 = sl;
   const long long threads = a.n_points << sl;
   plan->grid_blocks = (threads + kBlockThreads - 1) / kBlockThreads;
-  plan->layout = make_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes);
+  plan->layout = make_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes, plan->shared_nodes);
   plan->smem_bytes = 16 + (size_t)plan->layout.n_doubles * sizeof(double);
   if (plan->smem_bytes > 200 * 1024) {
     set_error("eval_grid: tables need %zu bytes of shared memory (limit 200 KiB): reduce n_rad/n_ang",

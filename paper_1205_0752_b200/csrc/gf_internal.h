@@ -16,6 +16,7 @@ struct PoleTerm {
 
 constexpr int kMaxTerms = 2;
 constexpr int kBlockThreads = 256;
+constexpr int kTailN = 32;  // terms of the large-y tail series (gf_eval.cu)
 
 // Everything the evaluation kernel needs, passed by value as a __grid_constant__.
 struct EvalArgs {
@@ -52,7 +53,10 @@ struct BlobLayout {
   int off_f32;                  // FP32 variant: float t[npad], w[npad], float2 mom[kmc], cheb[kmc]; or -1
   int off_rt, off_rw, n_tab;    // point-dependent contours: the radial rule pyramid (nodes, weights) or -1
   int n_doubles;                // doubles every CTA stages (even)
-  int off_scratch;              // preparation-only scratch after the staged block: T_k(s_j), [kmc][npad]
+  int off_gam;                  // tail series: gamma_{n,k}, row n = 1..kTailN at n(n-1)/2, staged; or -1 (no tail)
+  int off_tail;                 // NOT staged (global): double2 Rhat[n_terms][n_rad + 1][kTailN]
+  int off_scratch;              // preparation-only scratch: T_k(s_j) [npad][kmc]; tail: q_i^n (hi, lo) [kTailN][n_rad] x 2
+  int off_scratch2;
   int n_total;                  // doubles to allocate
 };
 

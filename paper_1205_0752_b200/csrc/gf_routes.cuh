@@ -33,6 +33,7 @@ __device__ __forceinline__ cd cmul(cd a, cd b) {
 }
 __device__ __forceinline__ cd csqr(cd a) { return {fma(a.re, a.re, -(a.im * a.im)), (a.re + a.re) * a.im}; }
 __device__ __forceinline__ cd cscale(cd a, double s) { return {a.re * s, a.im * s}; }
+__device__ __forceinline__ cd cadd(cd a, cd b) { return {a.re + b.re, a.im + b.im}; }
 __device__ __forceinline__ cd cinv(cd a) {
   // set-up code only (once per point / node): plain division, scaled against overflow
   const double m = fmax(fabs(a.re), fabs(a.im));
@@ -138,9 +139,9 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
 // Work counters of one thread (COUNT launches only)
 struct RouteCount {
   unsigned long long near_pairs = 0, series_exec = 0, exact_pairs = 0, n_near = 0, n_moment = 0, n_exact = 0,
-                     n_cheb = 0, series_used = 0;
+                     n_cheb = 0, series_used = 0, tails = 0;
 };
-constexpr int kNumCounters = 8;
+constexpr int kNumCounters = 9;
 
 // ---- NEAR: one folded angular pair: q = w/|zeta - t|^2 and the two sums ---------------------------
 __device__ __forceinline__ void pair_step(double zr, double zi2, double t, double w, double& u0, double& u1) {
@@ -334,7 +335,8 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
 // Add this thread's counters to the launch's (one atomic per warp and counter)
 __device__ __forceinline__ void flush_counters(const RouteCount& rc, bool active, unsigned long long* counters) {
   unsigned long long v[kNumCounters] = {rc.near_pairs, rc.series_exec, rc.exact_pairs, rc.n_near,
-                                        rc.n_moment,   rc.n_exact,     rc.n_cheb,      rc.series_used};
+                                        rc.n_moment,   rc.n_exact,     rc.n_cheb,      rc.series_used,
+                                        rc.tails};
   for (int k = 0; k < kNumCounters; ++k) {
     if (!active) v[k] = 0;
     for (int o = 16; o; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
@@ -434,6 +436,86 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
     if (momf) {
       chebf[k] = make_float2((float)c0, (float)c1);
       momf[k] = make_float2((float)m0, (float)m1);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Large-y tail (REAL contour; gf_eval.cu header "Tail"): tables that do not depend on x.
+//   gamma_{n,k} = -nu_k C(n+k, n-1-k) - (mu_k/4) C(n+k-1, n-2-k),  0 <= k < n <= kTailN, with the monomial
+//   moments mu_k = sum_j w_j t_j^k and nu_k = sum_j w_j (t_j - 1/4) t_j^k of the folded rule (double-double);
+//   Rhat_n(i0) = sum_{i >= i0} pref_i (y_i0 / y_i)^n by the downward recurrence
+//   Rhat_n(i) = pref_i + (y_i/y_{i+1})^n Rhat_n(i+1), the powers of q_i = y_i/y_{i+1} in double-double.
+// ---------------------------------------------------------------------------------------------
+__device__ dd dd_binom(int n, int k) {   // C(n, k) to double-double accuracy
+  if (k < 0 || k > n) return {0.0, 0.0};
+  if (k > n - k) k = n - k;
+  dd c = {1.0, 0.0};
+  for (int i = 1; i <= k; ++i) c = dd_div_d(dd_mul_d(c, (double)(n - k + i)), (double)i);
+  return c;
+}
+
+// phase A (after prep_angular + __syncthreads): thread k < kTailN computes mu_k, nu_k (dd) into shared arrays
+__device__ void prep_tail_moments(const EvalArgs& a, const BlobLayout& L, const double* blob, dd* s_mu, dd* s_nu) {
+  for (int k = threadIdx.x; k < kTailN; k += blockDim.x) {
+    dd mu = {0.0, 0.0}, nu = {0.0, 0.0};
+    for (int j = 0; j < a.n_pairs; ++j) {
+      const dd t = {blob[L.off_t + j], blob[L.off_tlo + j]};
+      dd p = {1.0, 0.0}, b = t;   // t^k
+      for (int e = k; e; e >>= 1) {
+        if (e & 1) p = dd_mul(p, b);
+        b = dd_mul(b, b);
+      }
+      const dd wp = dd_mul_d(p, blob[L.off_w + j]);
+      mu = dd_add(mu, wp);
+      nu = dd_add(nu, dd_mul(wp, dd_add_d(t, -0.25)));
+    }
+    s_mu[k] = mu;
+    s_nu[k] = nu;
+  }
+}
+// phase B (after a __syncthreads): gamma table
+__device__ void prep_tail_gamma(const BlobLayout& L, double* blob, const dd* s_mu, const dd* s_nu) {
+  for (int e = threadIdx.x; e < kTailN * (kTailN + 1) / 2; e += blockDim.x) {
+    int n = 1;
+    while (n * (n + 1) / 2 <= e) ++n;      // row n holds k = 0 .. n-1 at n(n-1)/2
+    const int k = e - n * (n - 1) / 2;
+    const dd t1 = dd_mul(s_nu[k], dd_binom(n + k, n - 1 - k));
+    const dd t2 = dd_scale2(dd_mul(s_mu[k], dd_binom(n + k - 1, n - 2 - k)), 0.25);
+    blob[L.off_gam + e] = dd_neg(dd_add(t1, t2)).hi;
+  }
+}
+// phase C: thread per node i: q_i^n, n = 1..kTailN, in double-double into the scratch (hi, lo) [n][i]
+__device__ void prep_tail_powers(const EvalArgs& a, const BlobLayout& L, double* blob) {
+  double* qhi = blob + L.off_scratch2;
+  double* qlo = qhi + (size_t)kTailN * a.n_rad;
+  for (int i = threadIdx.x; i < a.n_rad; i += blockDim.x) {
+    dd q = {1.0, 0.0};
+    if (i + 1 < a.n_rad) q = dd_div(dd{blob[L.off_y + i], 0.0}, dd{blob[L.off_y + i + 1], 0.0});
+    dd p = q;
+    for (int n = 0; n < kTailN; ++n) {
+      qhi[(size_t)n * a.n_rad + i] = p.hi;
+      qlo[(size_t)n * a.n_rad + i] = p.lo;
+      p = dd_mul(p, q);
+    }
+  }
+}
+// phase D (after a __syncthreads): thread per (pole r, n): the downward recurrence
+__device__ void prep_tail_sums(const EvalArgs& a, const BlobLayout& L, double* blob) {
+  const double* qhi = blob + L.off_scratch2;
+  const double* qlo = qhi + (size_t)kTailN * a.n_rad;
+  double2* R = reinterpret_cast<double2*>(blob + L.off_tail);
+  for (int e = threadIdx.x; e < a.n_terms * kTailN; e += blockDim.x) {
+    const int r = e / kTailN, n = e % kTailN;      // n + 1 is the power
+    double2* Rr = R + (size_t)r * (a.n_rad + 1) * kTailN;
+    Rr[(size_t)a.n_rad * kTailN + n] = make_double2(0.0, 0.0);
+    dd re = {0.0, 0.0}, im = {0.0, 0.0};
+    for (int i = a.n_rad - 1; i >= 0; --i) {
+      const dd q = {qhi[(size_t)n * a.n_rad + i], qlo[(size_t)n * a.n_rad + i]};
+      const double pr = blob[L.off_pref + 2 * (r * L.n_rad_pad + i)], pi = blob[L.off_pref + 2 * (r * L.n_rad_pad + i) + 1];
+      re = dd_add_d(dd_mul(re, q), pr);
+      im = dd_add_d(dd_mul(im, q), pi);
+      Rr[(size_t)i * kTailN + n] = make_double2(re.hi, im.hi);
     }
   }
 }
