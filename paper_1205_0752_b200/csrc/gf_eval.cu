@@ -114,6 +114,8 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
     }
   __syncthreads();  // the T_k(s_j) matrix, the monomial moments and the radial tables are complete
   prep_series_sums(a, L, blob);
+  __syncthreads();
+  prep_series_kreq(L, blob);
   if (L.off_gam >= 0) {
     prep_tail_gamma(L, blob, s_mu, s_nu);
     prep_tail_powers(a, L, blob);
@@ -297,6 +299,7 @@ BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyram
   L.off_w = take(L.npad);
   L.off_mom = take(2 * L.kmc);
   L.off_cheb = take(2 * L.kmc);
+  L.off_kreq = take(kKreqBins / 2);
   L.n_rad_pad = (n_rad + 31) & ~31;
   L.off_y = take(L.n_rad_pad);
   L.off_q4 = take(L.n_rad_pad);

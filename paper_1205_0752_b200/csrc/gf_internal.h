@@ -16,6 +16,7 @@ struct PoleTerm {
 
 constexpr int kMaxTerms = 2;
 constexpr int kBlockThreads = 256;
+constexpr int kKreqBins = 256;
 constexpr int kTailN = 32;  // terms of the large-y tail series (gf_eval.cu)
 
 // Everything the evaluation kernel needs, passed by value as a __grid_constant__.
@@ -47,6 +48,7 @@ struct BlobLayout {
   int kmc;                      // series coefficients k = 0 .. kmc-1 (even)
   int off_t, off_tlo, off_w;    // folded angular rule: t = z^2 (hi, lo), weight
   int off_mom, off_cheb;        // double2 (P_k, N_k)[kmc]: centred-moment series, Chebyshev series
+  int off_kreq;                 // int Kreq[kKreqBins]: Chebyshev terms needed per bin of log2(rho)
   int n_rad_pad;                // n_rad rounded up to 32: padding repeats the last node with prefactor 0
   int off_y, off_q4;            // radial nodes y_i, 1/(4 y_i), n_rad_pad each
   int off_pref;                 // double2 pref[n_terms][n_rad_pad]

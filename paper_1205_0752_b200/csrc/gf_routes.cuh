@@ -22,6 +22,8 @@ constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only go
 // FP64-pipe instructions of the per-node code of each route (set-up + finish), used to pick the cheaper of
 // CHEB and NEAR; they only steer the choice, any value gives the same sum
 constexpr int kChebNodeCost = 76, kNearNodeCost = 24;
+// Kreq table: bins of log2(rho) from kEllLo in steps of kEllStep (the lower edge of a bin decides, so K is safe)
+constexpr float kEllLo = 0.235f, kEllStep = 0.02f;
 
 enum { ROUTE_MOMENT = 0, ROUTE_CHEB = 1, ROUTE_NEAR = 2, ROUTE_EXACT = 3 };
 
@@ -107,6 +109,7 @@ struct Tabs {
   const double *st, *stlo, *sw;                   // folded angular rule
   const T *stT, *swT;                             // the same in the loop's type
   const typename Vec2<T>::type *mom, *cheb;       // series coefficients (P_k, N_k), kmc entries each
+  const int* kreq;                                // Chebyshev terms needed per bin of log2(rho)
   double mu0;                                     // sum of the folded weights
   double tau;                                     // EXACT inside this distance of [0,1]
   int n_pairs, kmc;
@@ -129,6 +132,7 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
     tb.mom = reinterpret_cast<const V2*>(tb.swT + L.npad);
     tb.cheb = tb.mom + L.kmc;
   }
+  tb.kreq = reinterpret_cast<const int*>(sb + L.off_kreq);
   tb.mu0 = sb[L.off_mom];  // a_0 of the moment series = sum of the folded weights
   tb.tau = sizeof(T) == 8 ? kTau64 : kTau32;
   tb.n_pairs = n_pairs;
@@ -291,9 +295,10 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
     ns = -in;
     const double g2 = rm + rm;                   // 4/sqrt(w^2-1) = 2 conj(root)/|q|
     g = {ar * g2, -ai * g2};
-    // rho^-K <= 2^-60.  zeta on [0,1] itself gives rho = 1 or NaN: the comparison below fails, never CHEB
-    const float kc = __fdividef(-120.f, __log2f((float)in));
-    K = kc < 4096.f ? (int)kc + 2 : 1 << 20;
+    // terms needed at this rho (table made from the coefficients themselves, prep_series_kreq).  zeta on [0,1]
+    // itself gives rho = 1 or NaN: the comparison fails, never CHEB
+    const float ell = -0.5f * __log2f((float)in);     // log2(rho)
+    K = ell >= kEllLo ? tb.kreq[min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)] : 1 << 20;
     route = ROUTE_CHEB;
     if (!(K <= tb.kmc && 4 * K + kChebNodeCost < 8 * tb.n_pairs + kNearNodeCost)) {
       K = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
@@ -437,6 +442,32 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
       chebf[k] = make_float2((float)c0, (float)c1);
       momf[k] = make_float2((float)m0, (float)m1);
     }
+  }
+}
+
+// Kreq[b]: the number of Chebyshev terms after which every dropped term is below 2^-62 of the leading
+// coefficient when log2(rho) >= kEllLo + b kEllStep: the smallest K with |c_j| rho^-j <= 2^-62 |c_0| for all
+// j >= K, c_j the larger of the two coefficients.  For a rule that integrates the measure well the c_j beyond
+// the first few are the rule's defect (~1e-7), so far fewer terms are needed than rho^-K <= 2^-60 asks for.
+// Coefficients beyond kmc are not known: a bin is usable only if rho^-kmc <= 2^-60.
+__device__ void prep_series_kreq(const BlobLayout& L, double* blob) {
+  int* kreq = reinterpret_cast<int*>(blob + L.off_kreq);
+  const double c00 = fmax(fabs(blob[L.off_cheb]), fabs(blob[L.off_cheb + 1]));
+  for (int b = threadIdx.x; b < kKreqBins; b += blockDim.x) {
+    const double ell = (double)kEllLo + (double)b * (double)kEllStep;
+    int K = 1 << 20;
+    if (ell * L.kmc >= 60.0) {
+      K = 4;
+      for (int j = L.kmc - 1; j >= 4; --j) {
+        const double c = fmax(fabs(blob[L.off_cheb + 2 * j]), fabs(blob[L.off_cheb + 2 * j + 1]));
+        if (log2(c / c00) - j * ell > -62.0) {   // c = 0 gives -inf: never needed
+          K = j + 1;
+          break;
+        }
+      }
+      K = (K + 3) & ~1;   // one spare term, even
+    }
+    kreq[b] = K;
   }
 }
 
