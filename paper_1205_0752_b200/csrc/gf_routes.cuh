@@ -16,6 +16,7 @@ namespace {
 
 constexpr int kKmc = 256;             // series coefficients staged per table (even)
 constexpr int kMomTerms = 32;         // genuine coefficients of the centred-moment series (zero beyond)
+constexpr float kSeriesBits = 54.f;    // series are cut where the dropped terms are below 2^-54 of the leading one
 constexpr double kMomentMin = 4.5;    // MOMENT route when max(|Re zeta|, |Im zeta|) >= this: |zeta - 1/2| >= 4
 constexpr double kTau64 = 0x1p-8;     // EXACT route inside this distance of [0,1] (FP64)
 constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only good further away
@@ -216,11 +217,11 @@ __device__ __forceinline__ void goertzel_pair(const typename Vec2<T>::type* __re
   }
 }
 
-// EXACT: zeta = A^2/(4 x y) in double-double, A = x + y + mu (y complex on a deformed contour); every
-// term formed directly.
-__device__ __noinline__ cd angular_exact(double xr, double xi, double yr, double yi, double mur, double mui, cd eta,
-                                         const double* __restrict__ st, const double* __restrict__ stlo,
-                                         const double* __restrict__ sw, int n_pairs) {
+// EXACT: zeta = A^2/(4 x y) in double-double, A = x + y + mu (y complex on a deformed contour).
+struct ZetaDD {
+  double re_hi, re_lo, im, im2;   // Re zeta = hi + lo, Im zeta, (Im zeta)^2
+};
+__device__ __noinline__ ZetaDD zeta_dd(double xr, double xi, double yr, double yi, double mur, double mui) {
   const dd Ar = dd_add_d(two_sum(xr, mur), yr), Ai = dd_add_d(two_sum(xi, mui), yi);
   const dd A2r = dd_add(dd_mul(Ar, Ar), dd_neg(dd_mul(Ai, Ai)));
   const dd A2i = dd_scale2(dd_mul(Ar, Ai), 2.0);
@@ -231,20 +232,46 @@ __device__ __noinline__ cd angular_exact(double xr, double xi, double yr, double
   const dd ni = dd_add(dd_mul(A2i, dr), dd_neg(dd_mul(A2r, di)));
   const dd den = dd_add(dd_mul(dr, dr), dd_mul(di, di));
   const dd zr = dd_div(nr, den), zi = dd_div(ni, den);
-  const double zi2 = fma(zi.hi, zi.hi, 2.0 * zi.hi * zi.lo);
-  double sr = 0.0, si = 0.0;
+  return {zr.hi, zr.lo, zi.hi, fma(zi.hi, zi.hi, 2.0 * zi.hi * zi.lo)};
+}
+
+// The direct sum with Re(zeta - t_j) formed from double-double zeta and t_j = z_j^2 = hi + lo exactly, so that it
+// is accurate to an ulp of ITSELF next to a zero of a denominator:  a_j = (zeta_hi - t_hi) + (zeta_lo - t_lo),
+// q_j = w_j/(a_j^2 + Im^2), U0 = sum q_j, Ua = sum q_j a_j, sum_j w_j/(zeta - t_j) = Ua - i Im U0, and
+// S = mu0 + (eta - zeta) (Ua - i Im U0).  10 FP64 instructions per pair (the reciprocal as in pair_step).
+// The FP64 kernel runs its NEAR lanes (zeta_lo = 0) and its EXACT lanes through this one loop.
+__device__ __forceinline__ void direct_step(double zh, double zl, double zi2, double t, double tlo, double w,
+                                            double& u0, double& ua) {
+  const double a = (zh - t) + (zl - tlo);
+  const double s = fma(a, a, zi2);
+  const double r0 = rcp_seed(s);
+  const double e = fma(-s, r0, 1.0);
+  const double p = fma(e, e, e);
+  const double v = r0 * w;
+  const double q = fma(v, p, v);
+  u0 += q;
+  ua = fma(q, a, ua);
+}
+__device__ __forceinline__ cd angular_direct(cd eta, ZetaDD z, double mu0, const double* __restrict__ st,
+                                             const double* __restrict__ stlo, const double* __restrict__ sw,
+                                             int n_pairs) {
+  double a0 = 0, a1 = 0, b0 = 0, b1 = 0;
+  int j = 0;
 #pragma unroll 1
-  for (int j = 0; j < n_pairs; ++j) {
-    const double t = st[j];
-    const double a = (zr.hi - t) + (zr.lo - stlo[j]);  // Re(zeta - t), accurate to an ulp of ITSELF
-    const double s = fma(a, a, zi2);
-    const double wq = sw[j] / s;
-    const double d = eta.re - t;
-    // (eta - t) conj(zeta - t)
-    sr = fma(wq, fma(d, a, eta.im * zi.hi), sr);
-    si = fma(wq, fma(eta.im, a, -(d * zi.hi)), si);
+  for (; j + 4 <= n_pairs; j += 4) {
+    const double2 t01 = *reinterpret_cast<const double2*>(st + j), t23 = *reinterpret_cast<const double2*>(st + j + 2);
+    const double2 l01 = *reinterpret_cast<const double2*>(stlo + j), l23 = *reinterpret_cast<const double2*>(stlo + j + 2);
+    const double2 w01 = *reinterpret_cast<const double2*>(sw + j), w23 = *reinterpret_cast<const double2*>(sw + j + 2);
+    direct_step(z.re_hi, z.re_lo, z.im2, t01.x, l01.x, w01.x, a0, a1);
+    direct_step(z.re_hi, z.re_lo, z.im2, t01.y, l01.y, w01.y, b0, b1);
+    direct_step(z.re_hi, z.re_lo, z.im2, t23.x, l23.x, w23.x, a0, a1);
+    direct_step(z.re_hi, z.re_lo, z.im2, t23.y, l23.y, w23.y, b0, b1);
   }
-  return {sr, si};
+  for (; j < n_pairs; ++j) direct_step(z.re_hi, z.re_lo, z.im2, st[j], stlo[j], sw[j], a0, a1);
+  const double u0 = a0 + b0, ua = a1 + b1;
+  const double cr = ua, ci = -z.im * u0;                       // sum_j w_j/(zeta - t_j)
+  const double dr = (eta.re - z.re_hi) - z.re_lo, di = eta.im - z.im;
+  return {mu0 + fma(dr, cr, -(di * ci)), fma(dr, ci, di * cr)};
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -275,8 +302,8 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
     sg = {zc * in, -zeta.im * in};
     ns = -in;
     g = sg;
-    // (|s|/2)^K <= 2^-58;  log2 |s|^2 <= -4 (-inf when it underflows in FP32: K = 2)
-    K = (int)__fdividef(116.f, 2.f - __log2f((float)in)) + 2;
+    // (|s|/2)^K <= 2^-kSeriesBits;  log2 |s|^2 <= -4 (-inf when it underflows in FP32: K = 2)
+    K = (int)__fdividef(2.f * kSeriesBits, 2.f - __log2f((float)in)) + 2;
   } else {
     // root = sqrt(zeta (zeta - 1)) = sqrt(w^2 - 1)/2, sign such that |w + 2 root| >= 1
     const double zm = zeta.re - 1.0, wr = fma(2.0, zeta.re, -1.0), wi = zeta.im + zeta.im;
@@ -326,13 +353,19 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
       }
     }
   }
-  if (route == ROUTE_EXACT) {
-    s = angular_exact(x.re, x.im, y.re, y.im, mur, mui, cd{__dadd_rn(0.25, delta.re), delta.im}, tb.st, tb.stlo, tb.sw,
-                      tb.n_pairs);
-    if (COUNT) { rc.exact_pairs += tb.n_pairs; ++rc.n_exact; }
-  } else if (route == ROUTE_NEAR) {
-    s = angular_near<T>(cd{__dadd_rn(0.25, delta.re), delta.im}, zeta, tb.mu0, tb.stT, tb.swT, tb.n_pairs);
-    if (COUNT) { rc.near_pairs += tb.n_pairs; ++rc.n_near; }
+  if (route >= ROUTE_NEAR) {
+    const cd eta = {__dadd_rn(0.25, delta.re), delta.im};
+    if (sizeof(T) == 8 || route == ROUTE_EXACT) {
+      ZetaDD z = {zeta.re, 0.0, zeta.im, zeta.im * zeta.im};
+      if (route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y.re, y.im, mur, mui);
+      s = angular_direct(eta, z, tb.mu0, tb.st, tb.stlo, tb.sw, tb.n_pairs);
+    } else {
+      s = angular_near<T>(eta, zeta, tb.mu0, tb.stT, tb.swT, tb.n_pairs);
+    }
+    if (COUNT) {
+      if (route == ROUTE_EXACT) { rc.exact_pairs += tb.n_pairs; ++rc.n_exact; }
+      else { rc.near_pairs += tb.n_pairs; ++rc.n_near; }
+    }
   }
   return s;
 }
@@ -445,8 +478,8 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
   }
 }
 
-// Kreq[b]: the number of Chebyshev terms after which every dropped term is below 2^-62 of the leading
-// coefficient when log2(rho) >= kEllLo + b kEllStep: the smallest K with |c_j| rho^-j <= 2^-62 |c_0| for all
+// Kreq[b]: the number of Chebyshev terms after which every dropped term is below 2^-(kSeriesBits+2) of the leading
+// coefficient when log2(rho) >= kEllLo + b kEllStep: the smallest K with |c_j| rho^-j <= 2^-(kSeriesBits+2) |c_0| for all
 // j >= K, c_j the larger of the two coefficients.  For a rule that integrates the measure well the c_j beyond
 // the first few are the rule's defect (~1e-7), so far fewer terms are needed than rho^-K <= 2^-60 asks for.
 // Coefficients beyond kmc are not known: a bin is usable only if rho^-kmc <= 2^-60.
@@ -460,7 +493,7 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob) {
       K = 4;
       for (int j = L.kmc - 1; j >= 4; --j) {
         const double c = fmax(fabs(blob[L.off_cheb + 2 * j]), fabs(blob[L.off_cheb + 2 * j + 1]));
-        if (log2(c / c00) - j * ell > -62.0) {   // c = 0 gives -inf: never needed
+        if (log2(c / c00) - j * ell > -(double)kSeriesBits - 2.0) {   // c = 0 gives -inf: never needed
           K = j + 1;
           break;
         }
