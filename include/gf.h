@@ -18,8 +18,10 @@
  *     arguments are HOST pointers.  `stream` is a cudaStream_t passed as void* (NULL = the
  *     legacy default stream).  Unless stated otherwise a call only ENQUEUES work on `stream`
  *     and returns; the caller synchronises.
- *   - Ownership: the caller owns every buffer.  The library keeps no device memory between
- *     calls and frees nothing it did not allocate inside the same call.
+ *   - Ownership: the caller owns every buffer.  Scratch a call needs is taken from, and returned
+ *     (in stream order, before the call returns) to, a stream-ordered memory pool of the library's
+ *     own, one per device; the pool keeps freed blocks for the next call until gf_trim_scratch().
+ *     Nothing else outlives a call.
  *   - Complex arrays are interleaved (re, im) pairs: complex<double> = 2 doubles (16 bytes,
  *     16-byte aligned), complex<float> = 2 floats (8 bytes, 8-byte aligned).
  *   - Grids are stored [n_im][n_re], the real index fastest (the paper's X(M,N) with M along
@@ -141,6 +143,20 @@ int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_
                  const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
                  long long n_points, void* d_out, void* stream);
 
+/* The two halves of gf_eval_grid, for callers that evaluate several grids with the same parameters and rules
+ * (and for benchmarks that time the evaluation kernel alone).  gf_eval_prepare makes every table that does not
+ * depend on x (folded angular rule, series coefficients, radial nodes and prefactors, tail tables) into the
+ * caller's DEVICE workspace of gf_eval_workspace_size() bytes (256-byte aligned; -1 on a bad argument; it does not
+ * depend on the number of points).  gf_eval_grid_prepared evaluates d_x from such a workspace; params, n_rad and
+ * n_ang must be the ones it was prepared with (not checked).  d_counters may be NULL (else as in
+ * gf_eval_grid_counted).  gf_eval_grid == workspace from cudaMallocAsync + these two + cudaFreeAsync. */
+long long gf_eval_workspace_size(const gf_params* p, int n_rad, int n_ang);
+int gf_eval_prepare(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                    const double* d_ang_nodes, const double* d_ang_weights, int n_ang, void* d_workspace,
+                    void* stream);
+int gf_eval_grid_prepared(const gf_params* p, int n_rad, int n_ang, const void* d_workspace, const void* d_x,
+                          long long n_points, void* d_out, unsigned long long* d_counters, void* stream);
+
 /* The same call on HOST buffers (the end-to-end path): allocates device scratch on `stream`, copies
  * tables and x host->device, runs the kernels, copies the result device->host and synchronises
  * `stream` before returning.  Pinned host memory makes the copies asynchronous but is not required. */
@@ -195,6 +211,9 @@ int gf_diag_rcp_seed(const double* d_in, double* d_out, long long n, void* strea
  * exactly as the evaluation kernel makes them (double-double, correctly rounded), for the n rule nodes in
  * d_nodes; tests compare them bit for bit with the oracle's. */
 int gf_diag_radial_map(double cutoff2, double map_scale, const double* d_nodes, int n, double* d_y, void* stream);
+
+/* Return the cached scratch of every device's pool to the driver (blocks still in use by enqueued work stay). */
+int gf_trim_scratch(void);
 
 const char* gf_last_error(void);
 const char* gf_version(void);

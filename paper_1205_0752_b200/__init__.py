@@ -66,10 +66,14 @@ _SIGNATURES = {
     "gf_eval_grid": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
     "gf_eval_grid_counted": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp, _vp],
     "gf_eval_grid_host": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
+    "gf_eval_workspace_size": [ctypes.POINTER(gf_params), _int, _int],
+    "gf_eval_prepare": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _vp],
+    "gf_eval_grid_prepared": [ctypes.POINTER(gf_params), _int, _int, _vp, _vp, _ll, _vp, _vp, _vp],
     "gf_eval_launch_info": [ctypes.POINTER(gf_params), _int, _int, _ll, ctypes.POINTER(gf_launch_info)],
     "gf_diag_fp64_peak": [_int, _int, _ll, _vp, _vp],
     "gf_diag_rcp_seed": [_vp, _vp, _ll, _vp],
     "gf_diag_radial_map": [_dbl, _dbl, _vp, _int, _vp, _vp],
+    "gf_trim_scratch": [],
     "gf_last_error": [],
     "gf_version": [],
 }
@@ -88,6 +92,7 @@ def lib():
             f.argtypes = args
             f.restype = _int
         L.gf_radial_table_size.restype = _ll
+        L.gf_eval_workspace_size.restype = _ll
         L.gf_last_error.restype = ctypes.c_char_p
         L.gf_version.restype = ctypes.c_char_p
         _lib = L
@@ -250,6 +255,33 @@ def eval_grid_counted(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weig
     return out, dict(zip(COUNTER_NAMES, counters.cpu().tolist()))
 
 
+def eval_prepare(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, stream=None):
+    """gf_eval_prepare: the x-independent tables into a fresh device workspace (a uint8 tensor)."""
+    n_ang = ang_nodes.numel()
+    size = int(lib().gf_eval_workspace_size(ctypes.byref(params), n_rad, n_ang))
+    if size < 0:
+        raise GfError(2, lib().gf_last_error().decode())
+    ws = torch.empty(size, dtype=torch.uint8, device=ang_nodes.device)
+    with torch.cuda.device(ws.device):
+        _check(lib().gf_eval_prepare(ctypes.byref(params), rad_nodes.data_ptr(), rad_weights.data_ptr(), n_rad,
+                                     ang_nodes.data_ptr(), ang_weights.data_ptr(), n_ang, ws.data_ptr(),
+                                     _stream(stream)))
+    return ws
+
+
+def eval_grid_prepared(params, n_rad, n_ang, workspace, x, out=None, stream=None):
+    """gf_eval_grid_prepared: G at x from a workspace made by eval_prepare with the same params and orders."""
+    assert x.is_cuda and x.dtype == torch.complex128 and x.is_contiguous()
+    odt = torch.complex64 if params.precision == 32 else torch.complex128
+    if out is None:
+        out = torch.empty(x.shape, dtype=odt, device=x.device)
+    assert out.dtype == odt and out.is_contiguous() and out.numel() == x.numel()
+    with torch.cuda.device(x.device):
+        _check(lib().gf_eval_grid_prepared(ctypes.byref(params), n_rad, n_ang, workspace.data_ptr(), x.data_ptr(),
+                                           x.numel(), out.data_ptr(), None, _stream(stream)))
+    return out
+
+
 def executed_fp64(info, counters):
     """(FP64-pipe thread-instructions, flops with FMA = 2) of one launch from its route counters."""
     units = (("near_pair", "near_pairs"), ("series_term", "series_terms"), ("exact_pair", "exact_pairs"),
@@ -301,6 +333,10 @@ def diag_rcp_seed(x, stream=None):
     out = torch.empty_like(x)
     _check(lib().gf_diag_rcp_seed(x.data_ptr(), out.data_ptr(), x.numel(), _stream(stream)))
     return out
+
+
+def trim_scratch():
+    _check(lib().gf_trim_scratch())
 
 
 def version():

@@ -35,7 +35,7 @@ def build(force=False, verbose=False):
     """Compile every CUDA source of the package into paper_1205_0752_b200/libgf_b200.so."""
     if not force and not stale():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + ["-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB]
+    cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("GF_NVCC_EXTRA", "").split() + ["-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB]
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-lquadmath"]

@@ -1,9 +1,11 @@
 // gf_api.cu -- the C ABI of include/gf.h: argument validation, host-side preparation (pole
 // decomposition of line 2, launch plan) and kernel launches.  No torch types, no exceptions.
+#include <algorithm>
 #include <cmath>
 #include <complex>
 #include <cstdarg>
 #include <cstdio>
+#include <mutex>
 #include <vector>
 
 #include "gf_internal.h"
@@ -23,6 +25,39 @@ int check_cuda(cudaError_t e, const char* what) {
   if (e == cudaSuccess) return GF_OK;
   set_error("%s: %s", what, cudaGetErrorString(e));
   return GF_ERR_CUDA;
+}
+
+// Scratch comes from a stream-ordered memory pool of the library's own (one per device) that keeps freed
+// blocks for the next call instead of returning them to the driver at every synchronisation (the default
+// pool does that, and mapping ~200 MB again costs milliseconds per call); gf_trim_scratch() empties it.
+static cudaMemPool_t g_pool[64] = {};
+static std::mutex g_pool_mutex;
+
+static int scratch_pool(cudaMemPool_t* pool) {
+  int dev = 0;
+  int rc = check_cuda(cudaGetDevice(&dev), "cudaGetDevice");
+  if (rc) return rc;
+  if (dev < 0 || dev >= 64) { set_error("device ordinal %d out of range", dev); return GF_ERR_CUDA; }
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  if (!g_pool[dev]) {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    if ((rc = check_cuda(cudaMemPoolCreate(&g_pool[dev], &props), "cudaMemPoolCreate"))) { g_pool[dev] = nullptr; return rc; }
+    unsigned long long keep = ~0ULL;
+    cudaMemPoolSetAttribute(g_pool[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+  }
+  *pool = g_pool[dev];
+  return GF_OK;
+}
+
+int scratch_alloc(void** ptr, size_t bytes, cudaStream_t stream) {
+  cudaMemPool_t pool;
+  int rc = scratch_pool(&pool);
+  if (rc) return rc;
+  return check_cuda(cudaMallocFromPoolAsync(ptr, bytes, pool, stream), "cudaMallocFromPoolAsync(scratch)");
 }
 
 namespace {
@@ -125,6 +160,17 @@ using namespace gf;
 extern "C" {
 
 const char* gf_last_error(void) { return g_err; }
+int gf_trim_scratch(void) {
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  int rc = GF_OK;
+  for (int dev = 0; dev < 64; ++dev)
+    if (g_pool[dev]) {
+      int r = check_cuda(cudaMemPoolTrimTo(g_pool[dev], 0), "cudaMemPoolTrimTo");
+      if (r) rc = r;
+    }
+  return rc;
+}
+
 const char* gf_version(void) { return "gf_b200 0.1 (sm_100a)"; }
 
 static int make_grid_rows(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
@@ -214,6 +260,42 @@ int gf_eval_grid_counted(const gf_params* p, const double* d_rad_nodes, const do
                         d_out, d_counters, stream);
 }
 
+long long gf_eval_workspace_size(const gf_params* p, int n_rad, int n_ang) {
+  EvalArgs a;
+  if (build_args(p, n_rad, n_ang, 1, &a)) return -1;
+  LaunchPlan plan;
+  if (plan_eval(a, p->precision, &plan)) return -1;
+  return (long long)plan.layout.n_total * (long long)sizeof(double);
+}
+
+int gf_eval_prepare(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                    const double* d_ang_nodes, const double* d_ang_weights, int n_ang, void* d_workspace,
+                    void* stream) {
+  EvalArgs a;
+  int rc = build_args(p, n_rad, n_ang, 1, &a);
+  if (rc) return rc;
+  if (!d_rad_nodes || !d_rad_weights || !d_ang_nodes || !d_ang_weights) { set_error("eval_prepare: null table pointer"); return GF_ERR_NULL; }
+  if (!d_workspace) { set_error("eval_prepare: d_workspace is null"); return GF_ERR_NULL; }
+  a.rad_nodes = d_rad_nodes;
+  a.rad_weights = d_rad_weights;
+  a.ang_nodes = d_ang_nodes;
+  a.ang_weights = d_ang_weights;
+  return launch_prepare(a, p->precision, static_cast<double*>(d_workspace), static_cast<cudaStream_t>(stream));
+}
+
+int gf_eval_grid_prepared(const gf_params* p, int n_rad, int n_ang, const void* d_workspace, const void* d_x,
+                          long long n_points, void* d_out, unsigned long long* d_counters, void* stream) {
+  EvalArgs a;
+  int rc = build_args(p, n_rad, n_ang, n_points, &a);
+  if (rc) return rc;
+  if (!d_workspace) { set_error("eval_grid_prepared: d_workspace is null"); return GF_ERR_NULL; }
+  if (n_points > 0 && (!d_x || !d_out)) { set_error("eval_grid_prepared: null grid/output pointer"); return GF_ERR_NULL; }
+  a.x = static_cast<const double2*>(d_x);
+  a.out = d_out;
+  return launch_prepared(a, p->precision, static_cast<const double*>(d_workspace), d_counters,
+                         static_cast<cudaStream_t>(stream));
+}
+
 int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const double* h_rad_weights, int n_rad,
                       const double* h_ang_nodes, const double* h_ang_weights, int n_ang, const void* h_x,
                       long long n_points, void* h_out, void* stream) {
@@ -228,33 +310,93 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
   const size_t out_elem = p->precision == 32 ? 8 : 16;
   const size_t tab_bytes = (2 * n_radtab + 2 * (size_t)n_ang) * sizeof(double);
   const size_t x_bytes = (size_t)n_points * 16, out_bytes = (size_t)n_points * out_elem;
-  // one scratch allocation: [tables | x | out], each part 256-byte aligned
+  // one scratch allocation: [tables | prepared workspace | x | out], each part 256-byte aligned
   auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
-  const size_t off_x = up(tab_bytes), off_out = off_x + up(x_bytes), total = off_out + up(out_bytes);
+  LaunchPlan plan0;
+  if ((rc = plan_eval(a, p->precision, &plan0))) return rc;
+  const size_t ws_bytes = (size_t)plan0.layout.n_total * sizeof(double);
+  const size_t off_ws = up(tab_bytes), off_x = off_ws + up(ws_bytes), off_out = off_x + up(x_bytes),
+               total = off_out + up(out_bytes);
   unsigned char* d = nullptr;
-  if ((rc = check_cuda(cudaMallocAsync(reinterpret_cast<void**>(&d), total, s), "cudaMallocAsync(scratch)"))) return rc;
+  if ((rc = scratch_alloc(reinterpret_cast<void**>(&d), total, s))) return rc;
   double* d_tab = reinterpret_cast<double*>(d);
   double* d_rn = d_tab;
   double* d_rw = d_rn + n_radtab;
   double* d_an = d_rw + n_radtab;
   double* d_aw = d_an + n_ang;
   cudaError_t e = cudaSuccess;
-  auto cp = [&](void* dst, const void* src, size_t n, cudaMemcpyKind k) { if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, n, k, s); };
-  cp(d_rn, h_rad_nodes, n_radtab * 8, cudaMemcpyHostToDevice);
-  cp(d_rw, h_rad_weights, n_radtab * 8, cudaMemcpyHostToDevice);
-  cp(d_an, h_ang_nodes, (size_t)n_ang * 8, cudaMemcpyHostToDevice);
-  cp(d_aw, h_ang_weights, (size_t)n_ang * 8, cudaMemcpyHostToDevice);
-  cp(d + off_x, h_x, x_bytes, cudaMemcpyHostToDevice);
-  rc = check_cuda(e, "host->device copies");
-  if (!rc) {
-    a.rad_nodes = d_rn; a.rad_weights = d_rw; a.ang_nodes = d_an; a.ang_weights = d_aw;
-    a.x = reinterpret_cast<const double2*>(d + off_x);
-    a.out = d + off_out;
-    rc = launch_eval(a, p->precision, nullptr, s);
+  auto cp = [&](void* dst, const void* src, size_t n, cudaMemcpyKind k, cudaStream_t st) { if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, n, k, st); };
+  cp(d_rn, h_rad_nodes, n_radtab * 8, cudaMemcpyHostToDevice, s);
+  cp(d_rw, h_rad_weights, n_radtab * 8, cudaMemcpyHostToDevice, s);
+  cp(d_an, h_ang_nodes, (size_t)n_ang * 8, cudaMemcpyHostToDevice, s);
+  cp(d_aw, h_ang_weights, (size_t)n_ang * 8, cudaMemcpyHostToDevice, s);
+  rc = check_cuda(e, "host->device copies (tables)");
+  a.rad_nodes = d_rn; a.rad_weights = d_rw; a.ang_nodes = d_an; a.ang_weights = d_aw;
+  double* d_ws = reinterpret_cast<double*>(d + off_ws);
+  if (!rc) rc = launch_prepare(a, p->precision, d_ws, s);
+
+  // x in, kernel, G out as a pipeline of chunks: copies in both directions overlap the evaluation
+  // (pinned host buffers; with pageable ones the copies serialise but the result is the same)
+  const int kMaxChunks = 4;
+  const long long min_chunk = 1 << 18;
+  int n_chunks = (int)std::min<long long>(kMaxChunks, std::max<long long>(1, n_points / min_chunk));
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaEvent_t ev_ready = nullptr, ev_in[kMaxChunks] = {}, ev_k[kMaxChunks] = {}, ev_done = nullptr;
+  auto ok = [&](cudaError_t err, const char* what) { if (!rc) rc = check_cuda(err, what); };
+  if (!rc && n_chunks > 1) {
+    ok(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking), "cudaStreamCreate");
+    ok(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking), "cudaStreamCreate");
+    ok(cudaEventCreateWithFlags(&ev_ready, cudaEventDisableTiming), "cudaEventCreate");
+    ok(cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming), "cudaEventCreate");
+    for (int c = 0; c < n_chunks; ++c) {
+      ok(cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming), "cudaEventCreate");
+      ok(cudaEventCreateWithFlags(&ev_k[c], cudaEventDisableTiming), "cudaEventCreate");
+    }
+    if (!rc) {
+      ok(cudaEventRecord(ev_ready, s), "cudaEventRecord");          // the scratch exists in stream order of s
+      ok(cudaStreamWaitEvent(s_in, ev_ready, 0), "cudaStreamWaitEvent");
+      ok(cudaStreamWaitEvent(s_out, ev_ready, 0), "cudaStreamWaitEvent");
+    }
   }
-  if (!rc) rc = check_cuda(cudaMemcpyAsync(h_out, d + off_out, out_bytes, cudaMemcpyDeviceToHost, s), "device->host copy");
+  for (int c = 0; c < n_chunks && !rc; ++c) {
+    // boundaries on multiples of the CTA size: every warp holds the same points as in one launch over all of x,
+    // so the chunked result is bit-identical to gf_eval_grid's (the series loop runs to the warp's longest series)
+    auto cut = [&](int k) { return k >= n_chunks ? n_points : (n_points * k / n_chunks) & ~(long long)(kBlockThreads - 1); };
+    const long long p0 = cut(c), p1 = cut(c + 1), np = p1 - p0;
+    cudaStream_t sin = n_chunks > 1 ? s_in : s, sout = n_chunks > 1 ? s_out : s;
+    ok(cudaMemcpyAsync(d + off_x + (size_t)p0 * 16, static_cast<const char*>(h_x) + (size_t)p0 * 16, (size_t)np * 16,
+                       cudaMemcpyHostToDevice, sin), "host->device copy (x)");
+    if (n_chunks > 1) {
+      ok(cudaEventRecord(ev_in[c], s_in), "cudaEventRecord");
+      ok(cudaStreamWaitEvent(s, ev_in[c], 0), "cudaStreamWaitEvent");
+    }
+    if (!rc) {
+      a.x = reinterpret_cast<const double2*>(d + off_x) + p0;
+      a.out = d + off_out + (size_t)p0 * out_elem;
+      a.n_points = np;
+      rc = launch_prepared(a, p->precision, d_ws, nullptr, s);
+    }
+    if (n_chunks > 1) {
+      ok(cudaEventRecord(ev_k[c], s), "cudaEventRecord");
+      ok(cudaStreamWaitEvent(s_out, ev_k[c], 0), "cudaStreamWaitEvent");
+    }
+    ok(cudaMemcpyAsync(static_cast<char*>(h_out) + (size_t)p0 * out_elem, d + off_out + (size_t)p0 * out_elem,
+                       (size_t)np * out_elem, cudaMemcpyDeviceToHost, sout), "device->host copy");
+  }
+  if (n_chunks > 1 && ev_done && s_out) {
+    cudaEventRecord(ev_done, s_out);
+    cudaStreamWaitEvent(s, ev_done, 0);   // the scratch is freed in stream order of s after the last copy out
+  }
   cudaFreeAsync(d, s);
   int rc2 = check_cuda(cudaStreamSynchronize(s), "stream synchronize");
+  if (s_in) { cudaStreamSynchronize(s_in); cudaStreamDestroy(s_in); }
+  if (s_out) { cudaStreamSynchronize(s_out); cudaStreamDestroy(s_out); }
+  if (ev_ready) cudaEventDestroy(ev_ready);
+  if (ev_done) cudaEventDestroy(ev_done);
+  for (int c = 0; c < kMaxChunks; ++c) {
+    if (ev_in[c]) cudaEventDestroy(ev_in[c]);
+    if (ev_k[c]) cudaEventDestroy(ev_k[c]);
+  }
   return rc ? rc : rc2;
 }
 

@@ -156,11 +156,14 @@ __device__ __forceinline__ cd tail_series(const double* __restrict__ gam, const 
     double b0 = 0.0, b1 = 0.0;
     const double* c = fwd ? row + n - 1 : row;      // highest power of the ratio first
     const int step = fwd ? -1 : 1;
-#pragma unroll 1
-    for (int j = 0; j < n; ++j, c += step) {
-      const double t = fma(rr, b0, fma(ns, b1, *c));
-      b1 = b0;
-      b0 = t;
+    if (n & 1) {
+      b0 = *c;
+      c += step;
+    }
+#pragma unroll 2
+    for (int j = n >> 1; j > 0; --j, c += 2 * step) {   // two coefficients per trip, roles of b0, b1 alternate
+      b1 = fma(rr, b0, fma(ns, b1, c[0]));
+      b0 = fma(rr, b1, fma(ns, b0, c[step]));
     }
     const cd P = {fma(-b1, rho.re, b0), b1 * rho.im};   // c_0 - c_1 conj(rho)
     const double2 R = Rrow[n - 1];
@@ -174,8 +177,11 @@ __device__ __forceinline__ cd tail_series(const double* __restrict__ gam, const 
 // ---------------------------------------------------------------------------------------------
 // Evaluation, REAL contour.  counters (COUNT only): gf.h, gf_eval_grid_counted.
 // ---------------------------------------------------------------------------------------------
+#ifndef GF_MIN_BLOCKS
+#define GF_MIN_BLOCKS 3
+#endif
 template <typename T, bool COUNT, int NT>
-__global__ void __launch_bounds__(kBlockThreads, 3)
+__global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
     eval_real_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                      const double* __restrict__ blob, unsigned long long* __restrict__ counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -370,34 +376,52 @@ int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d
   return check_cuda(cudaGetLastError(), "radial_map launch");
 }
 
-int launch_eval(const EvalArgs& a_in, int precision, unsigned long long* d_counters, cudaStream_t stream) {
-  if (a_in.n_points == 0) return GF_OK;
-  LaunchPlan plan;
-  int rc = plan_eval(a_in, precision, &plan);
-  if (rc) return rc;
+static int check_variant(const LaunchPlan& plan, int precision) {
   if (!plan.shared_nodes && precision == 32) {
     set_error("eval_grid: the FP32 comparison variant exists for the REAL contour only");
     return GF_ERR_UNSUPPORTED;
   }
+  return GF_OK;
+}
+
+// Preparation alone: the x-independent tables of this (params, rules) into `blob` (plan.layout.n_total doubles).
+int launch_prepare(const EvalArgs& a, int precision, double* blob, cudaStream_t stream) {
+  LaunchPlan plan;
+  int rc = plan_eval(a, precision, &plan);
+  if (rc) return rc;
+  if ((rc = check_variant(plan, precision))) return rc;
+  prep_real_kernel<<<1, 256, 0, stream>>>(a, plan.layout, blob);
+  return check_cuda(cudaGetLastError(), "prep kernel launch");
+}
+
+// Evaluation alone, from tables made by launch_prepare with the same params, orders and precision.
+int launch_prepared(const EvalArgs& a_in, int precision, const double* blob, unsigned long long* d_counters,
+                    cudaStream_t stream) {
+  if (a_in.n_points == 0) return GF_OK;
+  LaunchPlan plan;
+  int rc = plan_eval(a_in, precision, &plan);
+  if (rc) return rc;
+  if ((rc = check_variant(plan, precision))) return rc;
   EvalArgs a = a_in;
   a.split_log2 = plan.split_log2;
+  if (!plan.shared_nodes) return launch_contour(a, plan, blob, d_counters, stream);
+  if (d_counters)
+    return precision == 32 ? launch_real<float, true>(a, plan, blob, d_counters, stream)
+                           : launch_real<double, true>(a, plan, blob, d_counters, stream);
+  return precision == 32 ? launch_real<float, false>(a, plan, blob, nullptr, stream)
+                         : launch_real<double, false>(a, plan, blob, nullptr, stream);
+}
+
+int launch_eval(const EvalArgs& a, int precision, unsigned long long* d_counters, cudaStream_t stream) {
+  if (a.n_points == 0) return GF_OK;
+  LaunchPlan plan;
+  int rc = plan_eval(a, precision, &plan);
+  if (rc) return rc;
   // scratch for the prepared tables: stream-ordered, freed in stream order after the evaluation
   double* blob = nullptr;
-  rc = check_cuda(cudaMallocAsync(reinterpret_cast<void**>(&blob), (size_t)plan.layout.n_total * sizeof(double), stream),
-                  "cudaMallocAsync(tables)");
-  if (rc) return rc;
-  prep_real_kernel<<<1, 256, 0, stream>>>(a, plan.layout, blob);
-  rc = check_cuda(cudaGetLastError(), "prep kernel launch");
-  if (!rc && !plan.shared_nodes) {
-    rc = launch_contour(a, plan, blob, d_counters, stream);
-  } else if (!rc) {
-    if (d_counters)
-      rc = precision == 32 ? launch_real<float, true>(a, plan, blob, d_counters, stream)
-                           : launch_real<double, true>(a, plan, blob, d_counters, stream);
-    else
-      rc = precision == 32 ? launch_real<float, false>(a, plan, blob, nullptr, stream)
-                           : launch_real<double, false>(a, plan, blob, nullptr, stream);
-  }
+  if ((rc = scratch_alloc(reinterpret_cast<void**>(&blob), (size_t)plan.layout.n_total * sizeof(double), stream))) return rc;
+  rc = launch_prepare(a, precision, blob, stream);
+  if (!rc) rc = launch_prepared(a, precision, blob, d_counters, stream);
   cudaFreeAsync(blob, stream);
   return rc;
 }

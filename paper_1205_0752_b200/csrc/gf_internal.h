@@ -74,6 +74,7 @@ struct LaunchPlan {
 // host-side helpers (gf_api.cu)
 void set_error(const char* fmt, ...);
 int check_cuda(cudaError_t e, const char* what);
+int scratch_alloc(void** ptr, size_t bytes, cudaStream_t stream);  // from the library's own stream-ordered pool
 
 // gf_tables.cpp
 int make_rule_host(int kind, int n, double step, int measure, double* nodes, double* weights);
@@ -87,6 +88,9 @@ int launch_make_grid(double re_min, double re_max, int n_re, double im_min, doub
 // gf_eval.cu
 int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan);
 int launch_eval(const EvalArgs& a, int precision, unsigned long long* d_counters, cudaStream_t stream);
+int launch_prepare(const EvalArgs& a, int precision, double* blob, cudaStream_t stream);
+int launch_prepared(const EvalArgs& a, int precision, const double* blob, unsigned long long* d_counters,
+                    cudaStream_t stream);
 // gf_contour.cu: evaluation kernel for contours that depend on the grid point (RAY_ARC, THREAD, AUTO)
 int launch_contour(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* d_counters,
                    cudaStream_t stream);

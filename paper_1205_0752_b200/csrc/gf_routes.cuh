@@ -16,7 +16,10 @@ namespace {
 
 constexpr int kKmc = 256;             // series coefficients staged per table (even)
 constexpr int kMomTerms = 32;         // genuine coefficients of the centred-moment series (zero beyond)
-constexpr float kSeriesBits = 54.f;    // series are cut where the dropped terms are below 2^-54 of the leading one
+#ifndef GF_SERIES_BITS
+#define GF_SERIES_BITS 54
+#endif
+constexpr float kSeriesBits = GF_SERIES_BITS;    // series are cut where the dropped terms are below 2^-54 of the leading one
 constexpr double kMomentMin = 4.5;    // MOMENT route when max(|Re zeta|, |Im zeta|) >= this: |zeta - 1/2| >= 4
 constexpr double kTau64 = 0x1p-8;     // EXACT route inside this distance of [0,1] (FP64)
 constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only good further away
@@ -58,6 +61,17 @@ __device__ __forceinline__ float rcp_seed(float s) {
 __device__ __forceinline__ double rsqrt_seed(double s) {
   double r;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));  // MUFU.RSQ64H
+  return r;
+}
+// FP32 helpers for the term counts (flush-to-zero, approximate: one MUFU each)
+__device__ __forceinline__ float lg2_ftz(float s) {
+  float r;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s));
+  return r;
+}
+__device__ __forceinline__ float rcp_ftz(float s) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s));
   return r;
 }
 // 1/s and 1/sqrt(s) for normal s well inside the exponent range: seed + one cubic correction, no slow path
@@ -303,7 +317,7 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
     ns = -in;
     g = sg;
     // (|s|/2)^K <= 2^-kSeriesBits;  log2 |s|^2 <= -4 (-inf when it underflows in FP32: K = 2)
-    K = (int)__fdividef(2.f * kSeriesBits, 2.f - __log2f((float)in)) + 2;
+    K = (int)(2.f * kSeriesBits * rcp_ftz(2.f - lg2_ftz((float)in))) + 2;
   } else {
     // root = sqrt(zeta (zeta - 1)) = sqrt(w^2 - 1)/2, sign such that |w + 2 root| >= 1
     const double zm = zeta.re - 1.0, wr = fma(2.0, zeta.re, -1.0), wi = zeta.im + zeta.im;
@@ -324,7 +338,7 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
     g = {ar * g2, -ai * g2};
     // terms needed at this rho (table made from the coefficients themselves, prep_series_kreq).  zeta on [0,1]
     // itself gives rho = 1 or NaN: the comparison fails, never CHEB
-    const float ell = -0.5f * __log2f((float)in);     // log2(rho)
+    const float ell = -0.5f * lg2_ftz((float)in);     // log2(rho)
     K = ell >= kEllLo ? tb.kreq[min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)] : 1 << 20;
     route = ROUTE_CHEB;
     if (!(K <= tb.kmc && 4 * K + kChebNodeCost < 8 * tb.n_pairs + kNearNodeCost)) {
