@@ -81,13 +81,15 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
                                                         const __grid_constant__ BlobLayout L,
                                                         double* __restrict__ blob) {
   __shared__ int bad;
-  __shared__ dd s_mu[kTailN], s_nu[kTailN];
+  __shared__ dd s_mu[kTailN], s_nu[kTailN], s_part[8][2][kTailN];
+  __shared__ float s_lc[kKmc];
+  __shared__ dd s_cpart[8][2][kMomTerms];
   if (threadIdx.x == 0) bad = 0;
   __syncthreads();
   prep_angular(a, L, blob, &bad);
   __syncthreads();  // t, w written by this CTA are visible to it
   prep_series_T(a, L, blob);
-  if (L.off_gam >= 0) prep_tail_moments(a, L, blob, s_mu, s_nu);
+  if (L.off_gam >= 0) prep_tail_moments(a, L, blob, s_part);
   {
     // shifted-log map of [0, Lambda^2] (readings G3/G4): y(u) = s0 expm1(u L), dy/du = L (y + s0),
     // L = ln((Lambda^2 + s0)/s0) as a double-double from the host; y_i correctly rounded.
@@ -113,11 +115,11 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
       blob[L.off_rw + i] = a.rad_weights[i];
     }
   __syncthreads();  // the T_k(s_j) matrix, the monomial moments and the radial tables are complete
-  prep_series_sums(a, L, blob);
+  prep_series_sums(a, L, blob, s_cpart);
   __syncthreads();
-  prep_series_kreq(L, blob);
+  prep_series_kreq(L, blob, s_lc);
   if (L.off_gam >= 0) {
-    prep_tail_gamma(L, blob, s_mu, s_nu);
+    prep_tail_gamma(L, blob, s_part, s_mu, s_nu);
     prep_tail_powers(a, L, blob);
     __syncthreads();
     prep_tail_sums(a, L, blob);
@@ -320,6 +322,7 @@ BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyram
   L.off_tail = tail ? take(2 * n_terms * (n_rad + 1) * kTailN) : -1;
   L.off_scratch = take(L.kmc * L.npad);
   L.off_scratch2 = tail ? take(2 * kTailN * n_rad) : -1;
+  L.off_scratch3 = tail ? take(kTailN * n_rad + 2 * kTailChunks * (2 * n_terms * kTailN + kTailN)) : -1;
   L.n_total = o;
   return L;
 }

@@ -59,6 +59,7 @@ struct BlobLayout {
   int off_tail;                 // NOT staged (global): double2 Rhat[n_terms][n_rad + 1][kTailN]
   int off_scratch;              // preparation-only scratch: T_k(s_j) [npad][kmc]; tail: q_i^n (hi, lo) [kTailN][n_rad] x 2
   int off_scratch2;
+  int off_scratch3;             // tail: Q_c(i) [kTailN][n_rad], run starts (double-double)
   int n_total;                  // doubles to allocate
 };
 

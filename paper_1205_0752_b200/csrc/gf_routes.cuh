@@ -460,35 +460,56 @@ __device__ __forceinline__ double powi(double t, int k) {
   return r;
 }
 
-__device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double* blob) {
+__device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double* blob, dd (*s_cpart)[2][kMomTerms]) {
   const double* scratch = blob + L.off_scratch;
   float2* momf = L.off_f32 >= 0 ? reinterpret_cast<float2*>(reinterpret_cast<float*>(blob + L.off_f32) + 2 * L.npad)
                                 : nullptr;
   float2* chebf = momf ? momf + L.kmc : nullptr;
   for (int k = threadIdx.x; k < L.kmc; k += blockDim.x) {
-    dd tau = {0.0, 0.0}, nu = {0.0, 0.0}, mo = {0.0, 0.0}, no = {0.0, 0.0};
-    for (int j = 0; j < a.n_pairs; ++j) {
-      const double t = blob[L.off_t + j], w = blob[L.off_w + j], tq = t - 0.25;
-      const double wT = w * scratch[(size_t)j * L.kmc + k];
-      tau = dd_add_d(tau, wT);
-      nu = dd_add(nu, two_prod(wT, tq));
-      if (k < kMomTerms) {
-        const double wp = w * powi(t - 0.5, k);
-        mo = dd_add_d(mo, wp);
-        no = dd_add(no, two_prod(wp, tq));
+    dd tau = {0.0, 0.0}, nu = {0.0, 0.0}, tau1 = {0.0, 0.0}, nu1 = {0.0, 0.0}, mo = {0.0, 0.0}, no = {0.0, 0.0};
+    for (int j = 0; j < a.n_pairs; j += 2) {   // two independent accumulator chains (npad is even, padding has w = 0)
+      const double t0 = blob[L.off_t + j], w0 = blob[L.off_w + j], t1 = blob[L.off_t + j + 1], w1 = blob[L.off_w + j + 1];
+      const double wT0 = w0 * scratch[(size_t)j * L.kmc + k];
+      const double wT1 = j + 1 < a.n_pairs ? w1 * scratch[(size_t)(j + 1) * L.kmc + k] : 0.0;
+      tau = dd_add_d(tau, wT0);
+      tau1 = dd_add_d(tau1, wT1);
+      nu = dd_add(nu, two_prod(wT0, t0 - 0.25));
+      nu1 = dd_add(nu1, two_prod(wT1, t1 - 0.25));
+    }
+    tau = dd_add(tau, tau1);
+    nu = dd_add(nu, nu1);
+    {
+      // centred moments: thread k sums chunk k/32 of 8 of the nodes for the moment k%32; combined below
+      const int km = k % kMomTerms, c = (k / kMomTerms) % 8;
+      if (k < 8 * kMomTerms) {
+        for (int j = c; j < a.n_pairs; j += 8) {
+          const double t = blob[L.off_t + j];
+          const double wp = blob[L.off_w + j] * powi(t - 0.5, km);
+          mo = dd_add_d(mo, wp);
+          no = dd_add(no, two_prod(wp, t - 0.25));
+        }
+        s_cpart[c][0][km] = mo;
+        s_cpart[c][1][km] = no;
       }
     }
     const double half = k == 0 ? 0.5 : 1.0;   // sum' : the k = 0 term of a Chebyshev series is halved
     const double c0 = half * tau.hi, c1 = half * nu.hi;
-    const double m0 = k < kMomTerms ? mo.hi : 0.0, m1 = k < kMomTerms ? no.hi : 0.0;
     blob[L.off_cheb + 2 * k] = c0;
     blob[L.off_cheb + 2 * k + 1] = c1;
+    if (chebf) chebf[k] = make_float2((float)c0, (float)c1);
+  }
+  __syncthreads();
+  for (int k = threadIdx.x; k < L.kmc; k += blockDim.x) {
+    dd mo = {0.0, 0.0}, no = {0.0, 0.0};
+    if (k < kMomTerms)
+      for (int c = 0; c < 8; ++c) {
+        mo = dd_add(mo, s_cpart[c][0][k]);
+        no = dd_add(no, s_cpart[c][1][k]);
+      }
+    const double m0 = mo.hi, m1 = no.hi;     // zero beyond kMomTerms
     blob[L.off_mom + 2 * k] = m0;
     blob[L.off_mom + 2 * k + 1] = m1;
-    if (momf) {
-      chebf[k] = make_float2((float)c0, (float)c1);
-      momf[k] = make_float2((float)m0, (float)m1);
-    }
+    if (momf) momf[k] = make_float2((float)m0, (float)m1);
   }
 }
 
@@ -497,21 +518,22 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
 // j >= K, c_j the larger of the two coefficients.  For a rule that integrates the measure well the c_j beyond
 // the first few are the rule's defect (~1e-7), so far fewer terms are needed than rho^-K <= 2^-60 asks for.
 // Coefficients beyond kmc are not known: a bin is usable only if rho^-kmc <= 2^-60.
-__device__ void prep_series_kreq(const BlobLayout& L, double* blob) {
+__device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc /* [kKmc] shared */) {
   int* kreq = reinterpret_cast<int*>(blob + L.off_kreq);
   const double c00 = fmax(fabs(blob[L.off_cheb]), fabs(blob[L.off_cheb + 1]));
+  for (int j = threadIdx.x; j < L.kmc; j += blockDim.x)   // log2 |c_j / c_0|, rounded up a little (c = 0: -inf)
+    s_lc[j] = (float)log2(fmax(fabs(blob[L.off_cheb + 2 * j]), fabs(blob[L.off_cheb + 2 * j + 1])) / c00) + 1e-3f;
+  __syncthreads();
   for (int b = threadIdx.x; b < kKreqBins; b += blockDim.x) {
-    const double ell = (double)kEllLo + (double)b * (double)kEllStep;
+    const float ell = kEllLo + (float)b * kEllStep;
     int K = 1 << 20;
-    if (ell * L.kmc >= 60.0) {
+    if (ell * L.kmc >= 60.f) {
       K = 4;
-      for (int j = L.kmc - 1; j >= 4; --j) {
-        const double c = fmax(fabs(blob[L.off_cheb + 2 * j]), fabs(blob[L.off_cheb + 2 * j + 1]));
-        if (log2(c / c00) - j * ell > -(double)kSeriesBits - 2.0) {   // c = 0 gives -inf: never needed
+      for (int j = L.kmc - 1; j >= 4; --j)
+        if (s_lc[j] - (float)j * ell > -kSeriesBits - 2.f) {
           K = j + 1;
           break;
         }
-      }
       K = (K + 3) & ~1;   // one spare term, even
     }
     kreq[b] = K;
@@ -525,35 +547,48 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob) {
 //   Rhat_n(i0) = sum_{i >= i0} pref_i (y_i0 / y_i)^n by the downward recurrence
 //   Rhat_n(i) = pref_i + (y_i/y_{i+1})^n Rhat_n(i+1), the powers of q_i = y_i/y_{i+1} in double-double.
 // ---------------------------------------------------------------------------------------------
-__device__ dd dd_binom(int n, int k) {   // C(n, k) to double-double accuracy
+__device__ dd dd_binom(int n, int k) {   // C(n, k) for n <= 63, exact: every partial product fits 64 bits
   if (k < 0 || k > n) return {0.0, 0.0};
   if (k > n - k) k = n - k;
-  dd c = {1.0, 0.0};
-  for (int i = 1; i <= k; ++i) c = dd_div_d(dd_mul_d(c, (double)(n - k + i)), (double)i);
-  return c;
+  unsigned long long c = 1;
+  for (int i = 1; i <= k; ++i) {
+    const unsigned long long m = (unsigned long long)(n - k + i), d = (unsigned long long)i;
+    c = (c / d) * m + ((c % d) * m) / d;   // c m / d without forming c m (c m is divisible by d)
+  }
+  const double hi = (double)c;             // < 2^63; the remainder is exact in a double
+  const long long rem = (long long)c - (long long)hi;
+  return quick_two_sum(hi, (double)rem);
 }
 
-// phase A (after prep_angular + __syncthreads): thread k < kTailN computes mu_k, nu_k (dd) into shared arrays
-__device__ void prep_tail_moments(const EvalArgs& a, const BlobLayout& L, const double* blob, dd* s_mu, dd* s_nu) {
-  for (int k = threadIdx.x; k < kTailN; k += blockDim.x) {
+// phase A (after prep_angular + __syncthreads): thread (k, c) sums chunk c of 8 of the nodes into s_part[c][k]
+// (mu in [0], nu in [1]); phase B adds the 8 parts
+__device__ void prep_tail_moments(const EvalArgs& a, const BlobLayout& L, const double* blob, dd (*s_part)[2][kTailN]) {
+  for (int e = threadIdx.x; e < 8 * kTailN; e += blockDim.x) {
+    const int k = e % kTailN, c = e / kTailN;
     dd mu = {0.0, 0.0}, nu = {0.0, 0.0};
-    for (int j = 0; j < a.n_pairs; ++j) {
+    for (int j = c; j < a.n_pairs; j += 8) {
       const dd t = {blob[L.off_t + j], blob[L.off_tlo + j]};
       dd p = {1.0, 0.0}, b = t;   // t^k
-      for (int e = k; e; e >>= 1) {
-        if (e & 1) p = dd_mul(p, b);
+      for (int ex = k; ex; ex >>= 1) {
+        if (ex & 1) p = dd_mul(p, b);
         b = dd_mul(b, b);
       }
       const dd wp = dd_mul_d(p, blob[L.off_w + j]);
       mu = dd_add(mu, wp);
       nu = dd_add(nu, dd_mul(wp, dd_add_d(t, -0.25)));
     }
-    s_mu[k] = mu;
-    s_nu[k] = nu;
+    s_part[c][0][k] = mu;
+    s_part[c][1][k] = nu;
   }
 }
 // phase B (after a __syncthreads): gamma table
-__device__ void prep_tail_gamma(const BlobLayout& L, double* blob, const dd* s_mu, const dd* s_nu) {
+__device__ void prep_tail_gamma(const BlobLayout& L, double* blob, dd (*s_part)[2][kTailN], dd* s_mu, dd* s_nu) {
+  for (int k = threadIdx.x; k < 2 * kTailN; k += blockDim.x) {
+    dd acc = {0.0, 0.0};
+    for (int c = 0; c < 8; ++c) acc = dd_add(acc, s_part[c][k / kTailN][k % kTailN]);
+    (k < kTailN ? s_mu : s_nu)[k % kTailN] = acc;
+  }
+  __syncthreads();
   for (int e = threadIdx.x; e < kTailN * (kTailN + 1) / 2; e += blockDim.x) {
     int n = 1;
     while (n * (n + 1) / 2 <= e) ++n;      // row n holds k = 0 .. n-1 at n(n-1)/2
@@ -578,23 +613,51 @@ __device__ void prep_tail_powers(const EvalArgs& a, const BlobLayout& L, double*
     }
   }
 }
-// phase D (after a __syncthreads): thread per (pole r, n): the downward recurrence
+// phase D (after a __syncthreads): the downward recurrence, split into kTailChunks runs of nodes so that the CTA's
+// threads share it: item = (pole r, power n + 1, real / imaginary part), run c.  Pass 1 runs the recurrence inside
+// each run from 0 (L_c(i)) with the run's product of q (Q_c(i)); pass 2 folds the runs above c into the carry
+// Rhat(end of run c) in double-double and completes Rhat(i) = L_c(i) + Q_c(i) carry.
+constexpr int kTailChunks = 8;
 __device__ void prep_tail_sums(const EvalArgs& a, const BlobLayout& L, double* blob) {
   const double* qhi = blob + L.off_scratch2;
   const double* qlo = qhi + (size_t)kTailN * a.n_rad;
   double2* R = reinterpret_cast<double2*>(blob + L.off_tail);
-  for (int e = threadIdx.x; e < a.n_terms * kTailN; e += blockDim.x) {
-    const int r = e / kTailN, n = e % kTailN;      // n + 1 is the power
-    double2* Rr = R + (size_t)r * (a.n_rad + 1) * kTailN;
-    Rr[(size_t)a.n_rad * kTailN + n] = make_double2(0.0, 0.0);
-    dd re = {0.0, 0.0}, im = {0.0, 0.0};
-    for (int i = a.n_rad - 1; i >= 0; --i) {
+  const int n_items = 2 * a.n_terms * kTailN, CL = (a.n_rad + kTailChunks - 1) / kTailChunks;
+  double* Qs = blob + L.off_scratch3;                                   // Q_c(i), [kTailN][n_rad]
+  dd* Lstart = reinterpret_cast<dd*>(Qs + (size_t)kTailN * a.n_rad);    // [n_items][kTailChunks]
+  dd* Qstart = Lstart + (size_t)n_items * kTailChunks;                  // [kTailN][kTailChunks]
+  for (int w = threadIdx.x; w < n_items * kTailChunks; w += blockDim.x) {
+    const int e = w % n_items, c = w / n_items;
+    const int part = e / (a.n_terms * kTailN), r = (e / kTailN) % a.n_terms, n = e % kTailN;
+    double* Rr = reinterpret_cast<double*>(R + (size_t)r * (a.n_rad + 1) * kTailN) + part;
+    const bool owner = r == 0 && part == 0;
+    if (c == 0) Rr[2 * ((size_t)a.n_rad * kTailN + n)] = 0.0;
+    dd acc = {0.0, 0.0}, Q = {1.0, 0.0};
+    for (int i = min((c + 1) * CL, a.n_rad) - 1; i >= c * CL; --i) {
       const dd q = {qhi[(size_t)n * a.n_rad + i], qlo[(size_t)n * a.n_rad + i]};
-      const double pr = blob[L.off_pref + 2 * (r * L.n_rad_pad + i)], pi = blob[L.off_pref + 2 * (r * L.n_rad_pad + i) + 1];
-      re = dd_add_d(dd_mul(re, q), pr);
-      im = dd_add_d(dd_mul(im, q), pi);
-      Rr[(size_t)i * kTailN + n] = make_double2(re.hi, im.hi);
+      acc = dd_add_d(dd_mul(acc, q), blob[L.off_pref + 2 * (r * L.n_rad_pad + i) + part]);
+      Rr[2 * ((size_t)i * kTailN + n)] = acc.hi;
+      if (owner) {
+        Q = dd_mul(Q, q);
+        Qs[(size_t)n * a.n_rad + i] = Q.hi;
+      }
     }
+    Lstart[(size_t)e * kTailChunks + c] = acc;
+    if (owner) Qstart[(size_t)n * kTailChunks + c] = Q;
+  }
+  __syncthreads();
+  for (int w = threadIdx.x; w < n_items * kTailChunks; w += blockDim.x) {
+    const int e = w % n_items, c = w / n_items;
+    const int part = e / (a.n_terms * kTailN), r = (e / kTailN) % a.n_terms, n = e % kTailN;
+    double* Rr = reinterpret_cast<double*>(R + (size_t)r * (a.n_rad + 1) * kTailN) + part;
+    dd carry = {0.0, 0.0};
+    for (int cc = kTailChunks - 1; cc > c; --cc)
+      carry = dd_add(Lstart[(size_t)e * kTailChunks + cc], dd_mul(Qstart[(size_t)n * kTailChunks + cc], carry));
+    if (carry.hi != 0.0 || carry.lo != 0.0)
+      for (int i = min((c + 1) * CL, a.n_rad) - 1; i >= c * CL; --i) {
+        const size_t at = 2 * ((size_t)i * kTailN + n);
+        Rr[at] = dd_add_d(dd_mul_d(carry, Qs[(size_t)n * a.n_rad + i]), Rr[at]).hi;
+      }
   }
 }
 

@@ -402,6 +402,45 @@ def test_eval_grid_host_matches_device_path(gf):
     assert torch.equal(out.view(torch.float64), g.view(torch.float64))
 
 
+def test_eval_grid_host_pipeline_ragged(gf):
+    """The chunked copy/compute pipeline of the host path (>= 2^18 points per chunk, ragged total, pageable and
+    pinned buffers) returns bit for bit what one launch over the device-resident grid returns."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    n = 3 * (1 << 18) + 12345
+    rng = np.random.default_rng(W.PARITY_SEED)
+    xs = torch.from_numpy(rng.uniform(-5, 1, n) + 1j * rng.uniform(-2, 2, n))
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, xs.cuda()).cpu()
+    tabs = (rn.cpu().numpy(), rw.cpu().numpy(), cfg["n_rad"], z.cpu().numpy(), wz.cpu().numpy())
+    for pin in (True, False):
+        out = torch.empty(n, dtype=torch.complex128)
+        xin = xs.clone()
+        if pin:
+            out, xin = out.pin_memory(), xin.pin_memory()
+        gf.eval_grid_host(P, *tabs, xin, out)
+        assert torch.equal(out.view(torch.float64), g.view(torch.float64))
+    gf.trim_scratch()
+
+
+def test_prepare_then_evaluate_two_grids(gf, oracle):
+    """gf_eval_prepare once, gf_eval_grid_prepared on two grids: the same numbers as gf_eval_grid, on the FP64 and
+    the FP32 variant and on a deformed contour; parity of one of them against the oracle."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    x = gpu_grid(gf, cfg)
+    x2 = (0.5 * x + (0.25 - 0.125j)).contiguous()
+    for contour, prec in (("real", 64), ("real", 32), ("auto", 64)):
+        P, rn, rw, z, wz = gpu_setup(gf, cfg, contour=contour, precision=prec)
+        ws = gf.eval_prepare(P, rn, rw, cfg["n_rad"], z, wz)
+        for xx in (x, x2):
+            a = gf.eval_grid_prepared(P, cfg["n_rad"], cfg["n_ang"], ws, xx)
+            b = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, xx)
+            assert torch.equal(torch.view_as_real(a), torch.view_as_real(b))
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    ws = gf.eval_prepare(P, rn, rw, cfg["n_rad"], z, wz)
+    g2 = gf.eval_grid_prepared(P, cfg["n_rad"], cfg["n_ang"], ws, x2).cpu().numpy()
+    assert relerr(g2.ravel(), oracle_eval(oracle, cfg, x2.cpu().numpy().ravel())).max() <= TOL64
+
+
 def test_runs_on_the_callers_stream(gf):
     cfg = W.CONFIGS["cfg1_tiny"]
     P, rn, rw, z, wz = gpu_setup(gf, cfg)
