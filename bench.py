@@ -41,7 +41,7 @@ FP64_LANES_PER_SM = 64
 N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of one eval kernel launch on cfg3 (profiles/, ncu --set full);
 # None until a capture is committed
-EVAL_KERNEL_DRAM_TRAFFIC_BYTES = 95.5e6  # r01b: 69.2 MB read + 26.3 MB written
+EVAL_KERNEL_DRAM_TRAFFIC_BYTES = 94.8e6  # r01f: 68.2 MB read + 26.6 MB written
 
 
 def dist_env():
@@ -270,6 +270,24 @@ def run_ours(args):
     fp64_inst, fp64_flops = gf.executed_fp64(info, counters)
     del out_c
 
+    # ---- the FP32 comparison variant on the same scan (BASELINE.json configs[2]): untimed for `value`, own events
+    P32 = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
+                         contour="real", precision=32)
+    ws32 = gf.eval_prepare(P32, rn_c, rw_c, n_rad, z_c, wz_c)
+    out32 = torch.empty(x.shape, dtype=torch.complex64, device=dev)
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for i in range(3):
+        if i == 2:
+            f0.record(stream)
+        gf.eval_grid_prepared(P32, n_rad, n_ang, ws32, x, out=out32)
+    f1.record(stream)
+    torch.cuda.synchronize()
+    ref64 = out.to(torch.complex128)
+    err32 = ((out32.to(torch.complex128) - ref64).abs() / ref64.abs().clamp_min(1e-300)).max().item()
+    fp32_variant = {"kernel_ms": f0.elapsed_time(f1), "max_rel_diff_vs_fp64": err32,
+                    "note": "series and NEAR loops in float, per-node set-up, EXACT lanes and the tail in FP64"}
+    del out32, ref64, ws32
+
     # ---- e2e: the host-buffer entry point, copies inside the timed region
     xh = x.cpu().pin_memory()
     outh = torch.empty(xh.shape, dtype=torch.complex128).pin_memory()
@@ -338,6 +356,7 @@ def run_ours(args):
                      "fp64_inst_per_launch": fp64_inst, "routes": counters,
                      "fp64_pipe_frac": fp64_inst / (kernel_ms * 1e-3) / (FP64_LANES_PER_SM * N_SM * sm_max * 1e6),
                      "kernel_share_of_step": kernel_ms * args.steps / ms_total},
+        "fp32_variant": fp32_variant,
         "clocks": clocks,
     }
     if world == 1 and not args.no_cpu_baseline:

@@ -166,8 +166,9 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
 
 /* The same evaluation, also counting the work by route for the roofline accounting.
  * d_counters: 9 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
- *   [0] NEAR pairs  [1] series terms EXECUTED (every lane of a warp runs its warp's longest series)
- *   [2] EXACT pairs  [3] [4] [5] [6] (point, radial node, pole) triples taken by the NEAR / MOMENT / EXACT / CHEB
+ *   [0] pairs of the plain direct loop  [1] series terms EXECUTED (every lane of a warp runs its warp's longest
+ *   series)  [2] pairs of the double-double direct loop (EXACT lanes, and the NEAR lanes of their warps)
+ *   [3] [4] [5] [6] (point, radial node, pole) triples taken by the NEAR / MOMENT / EXACT / CHEB
  *   route (the triples of the large-y tail are not among them)  [7] series terms NEEDED (the sum over series
  *   triples of their own K)  [8] tail series evaluated, one per (point, pole).  Results are identical to
  *   gf_eval_grid. */

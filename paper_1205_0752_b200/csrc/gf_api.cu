@@ -63,8 +63,8 @@ int scratch_alloc(void** ptr, size_t bytes, cudaStream_t stream) {
 namespace {
 
 // per (point, node, pole) FP64-pipe instructions of each route's set-up + finish (SASS of eval_real_kernel<double>)
-constexpr double kNodeNearDfma = 9, kNodeNearOther = 19, kNodeMomentDfma = 19, kNodeMomentOther = 18,
-                 kNodeChebDfma = 32, kNodeChebOther = 38;
+constexpr double kNodeNearDfma = 12, kNodeNearOther = 13, kNodeMomentDfma = 21, kNodeMomentOther = 13,
+                 kNodeChebDfma = 34, kNodeChebOther = 33;
 
 bool finite_prop(const gf_propagator& p) {
   return std::isfinite(p.m2_re) && std::isfinite(p.m2_im) && std::isfinite(p.M2) && std::isfinite(p.a) &&
@@ -416,21 +416,22 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
   out->series_terms_max = plan.layout.kmc;
   out->evals = (double)n_points * n_rad * n_ang;
   // FP64-pipe instructions per unit of each route, counted per SASS region in the ncu source page of
-  // eval_real_kernel<double, false, 1> (profiles/r01e_eval_ncu_full.md; DSETP not counted: no flops):
-  //   direct pair (NEAR and EXACT lanes): 5 DFMA + 1 DMUL + 4 DADD;   series term (P and N): 4 DFMA;
-  //   every node-term: zeta, delta (3 DFMA + 7 DMUL + 2 DADD) and the accumulation into G (4 DFMA);
-  //   MOMENT adds 4 + 5 (set-up) and 8 + 4 (finish), CHEB 17 + 25 and 8 + 4, the direct loop 2 + 10,
+  // eval_real_kernel<double, false, 1> (profiles/r01f_eval_ncu_full.md; DSETP not counted: no flops):
+  //   pair of the plain direct loop 5 DFMA + 1 DMUL + 2 DADD, of the double-double loop 5 + 1 + 4;
+  //   series term (P and N): 4 DFMA;
+  //   every node-term: zeta, delta (5 DFMA + 3 DMUL + 1 DADD) and the accumulation into G (4 DFMA);
+  //   MOMENT adds 4 + 5 (set-up) and 8 + 4 (finish), CHEB 17 + 25 and 8 + 4, the direct loops 3 + 9,
   //   EXACT lanes the double-double zeta (29 + 217);
-  //   tail per (point, pole): 2 DFMA per coefficient (kTailN (kTailN + 1)), 7 + 9 per n, the per-point set-up.
+  //   tail per (point, pole): 2 DFMA per coefficient (kTailN (kTailN + 1)), 8 + 9 per n, the per-point set-up.
   const bool f32 = p->precision == 32;
-  out->near_pair_dfma = f32 ? 0 : 5; out->near_pair_other = f32 ? 0 : 5; out->near_pair_fp32 = f32 ? 5 : 0;
+  out->near_pair_dfma = f32 ? 0 : 5; out->near_pair_other = f32 ? 0 : 3; out->near_pair_fp32 = f32 ? 5 : 0;
   out->series_term_dfma = f32 ? 0 : 4; out->series_term_other = 0; out->series_term_fp32 = f32 ? 4 : 0;
   out->exact_pair_dfma = 5; out->exact_pair_other = 5;
   out->node_near_dfma = kNodeNearDfma; out->node_near_other = kNodeNearOther;
   out->node_moment_dfma = kNodeMomentDfma; out->node_moment_other = kNodeMomentOther;
   out->node_cheb_dfma = kNodeChebDfma; out->node_cheb_other = kNodeChebOther;
   out->node_exact_dfma = kNodeNearDfma + 29; out->node_exact_other = kNodeNearOther + 217;
-  out->tail_dfma = kTailN * (kTailN + 1) + 7.0 * kTailN + 42; out->tail_other = 9.0 * kTailN + 27;
+  out->tail_dfma = kTailN * (kTailN + 1) + 8.0 * kTailN + 45; out->tail_other = 9.0 * kTailN + 34;
   return GF_OK;
 }
 

@@ -18,11 +18,11 @@
 //    is the Cauchy transform of a fixed discrete measure on [0,1], analytic in zeta off [0,1].  It is
 //    evaluated by one of four routes chosen from zeta alone (gf_routes.cuh, node_term):
 //      MOMENT |zeta| large: geometric series in s = 1/(zeta - 1/2) with the centred moments of the rule,
-//             at most 22 terms.
+//             at most 20 terms.
 //      CHEB   Chebyshev series in s = 1/(w + sqrt(w^2-1)), w = 2 zeta - 1: 1/(zeta - t) = 4/sqrt(w^2-1)
 //             sum'_k s^k T_k(2t-1), with the Chebyshev moments of the rule (made once per launch).  It
 //             converges like rho^-k, rho = 1/|s| the parameter of the ellipse with foci 0 and 1 through
-//             zeta, so K = 60/log2(rho) terms replace the N_a/2 pairs of the direct sum wherever the
+//             zeta, so a few tens of terms replace the N_a/2 pairs of the direct sum wherever the
 //             radial node is not next to the image of the cut (median rho over the production scan: 3).
 //             Both series have real coefficients and a complex argument and share one loop: the
 //             second-order (Goertzel) recurrence, 2 DFMA per coefficient, 4 per term for the two
@@ -220,9 +220,17 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
     out_scale = scalbn(1.0, -k);
   }
   const cd xinv = cinv(x);
-  cd xm[NT];  // x + mu_r
+  // zeta = (x + mu + y)^2/(4 x y) = C1/y + C2 + C3 y with C1 = (x + mu)^2/(4x), C2 = (x + mu)/(2x), C3 = 1/(4x):
+  // four DFMA per node-term.  Its absolute error is an ulp of the largest of the three terms, which is O(1)
+  // wherever zeta is O(1) (the EXACT route recomputes zeta in double-double from x, y, mu anyway).
+  cd xm[NT], C1x4[NT], C2[NT];  // x + mu_r, 4 C1 (multiplies 1/(4y)), C2
+  const cd C3 = cscale(xinv, 0.25);
 #pragma unroll
-  for (int r = 0; r < NT; ++r) xm[r] = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
+  for (int r = 0; r < NT; ++r) {
+    xm[r] = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
+    C2[r] = cscale(cmul(xm[r], xinv), 0.5);
+    C1x4[r] = cscale(cmul(xm[r], C2[r]), 2.0);
+  }
 
   // where the tail series takes over: the first node with y_i >= Y0 = 4 (sqrt|x| + sqrt(|x| + |x + mu|))^2
   int i_end = a.n_rad;
@@ -254,12 +262,10 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
   for (int i0 = 0; i0 < i_stop; i0 += S, py += S, pq4 += S, ppref += S) {
     const double y = *py, q4 = *pq4;
     const bool on = i0 + sub < i_end;                // past its own i_end a lane idles with weight 0
-    const cd xq = cscale(xinv, q4);                  // 1/(4 x y)
 #pragma unroll
     for (int r = 0; r < NT; ++r) {
-      const cd A = {xm[r].re + y, xm[r].im};
       const cd delta = cscale(xm[r], q4);            // eta - 1/4
-      const cd zeta = cmul(csqr(A), xq);
+      const cd zeta = {fma(C1x4[r].re, q4, fma(C3.re, y, C2[r].re)), fma(C1x4[r].im, q4, fma(C3.im, y, C2[r].im))};
       const cd s = node_term<T, COUNT>(tb, x, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc);
       double2 pr = ppref[r * L.n_rad_pad];
       if (!on) pr = make_double2(0.0, 0.0);

@@ -17,9 +17,13 @@ namespace {
 constexpr int kKmc = 256;             // series coefficients staged per table (even)
 constexpr int kMomTerms = 32;         // genuine coefficients of the centred-moment series (zero beyond)
 #ifndef GF_SERIES_BITS
-#define GF_SERIES_BITS 54
+#define GF_SERIES_BITS 50
 #endif
-constexpr float kSeriesBits = GF_SERIES_BITS;    // series are cut where the dropped terms are below 2^-54 of the leading one
+constexpr float kSeriesBits = GF_SERIES_BITS;    // series are cut where the dropped terms are below 2^-50 of the leading one
+#ifndef GF_GOERTZEL_UNROLL
+#define GF_GOERTZEL_UNROLL 2
+#endif
+constexpr int kGoertzelUnroll = GF_GOERTZEL_UNROLL;   // trips of the series loop (2 terms each) unrolled
 constexpr double kMomentMin = 4.5;    // MOMENT route when max(|Re zeta|, |Im zeta|) >= this: |zeta - 1/2| >= 4
 constexpr double kTau64 = 0x1p-8;     // EXACT route inside this distance of [0,1] (FP64)
 constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only good further away
@@ -220,7 +224,7 @@ __device__ __forceinline__ void goertzel_pair(const typename Vec2<T>::type* __re
   typedef typename Vec2<T>::type V2;
   p1 = p2 = n1 = n2 = (T)0;
   const V2* c = tab + Kw;
-#pragma unroll 2
+#pragma unroll(kGoertzelUnroll)
   for (int k = Kw; k > 0; k -= 2) {
     c -= 2;
     const V2 c1 = c[1], c0 = c[0];
@@ -291,33 +295,36 @@ __device__ __forceinline__ cd angular_direct(cd eta, ZetaDD z, double mu0, const
 // ---------------------------------------------------------------------------------------------
 // One (point, radial node, pole): S(delta, zeta) by the route zeta selects.  delta = eta - 1/4.
 // WARP-COLLECTIVE: all 32 lanes must call it together (the series loop runs to the warp's longest
-// series, lanes on other routes idle through it; extra terms are below 2^-58 and harmless).
+// series, lanes on other routes idle through it; extra terms are below the cut and harmless).
 //   MOMENT  max(|Re zeta|, |Im zeta|) >= 4.5: s = 1/(zeta - 1/2), S = s [delta P(s) - N(s)] with the moments
 //           a_k = sum_j w_j (t_j - 1/2)^k, b_k = sum_j w_j (t_j - 1/4)(t_j - 1/2)^k; |t - 1/2| <= 1/2 and
-//           |s| <= 1/4, so K = 58/(1 - log2|s|) + 2 <= 22 terms.
+//           |s| <= 1/4, so K = kSeriesBits/(1 - log2|s|) + 2 <= 20 terms.
 //   CHEB    else, with w = 2 zeta - 1 and s = 1/(w + sqrt(w^2 - 1)) the smaller root of s + 1/s = 2w
 //           (|s| = 1/rho, rho the parameter of the ellipse with foci 0, 1 through zeta):
 //           1/(zeta - t) = 4/sqrt(w^2-1) sum'_k s^k T_k(2t-1), so S = 4/sqrt(w^2-1) [delta P(s) - N(s)] with the
 //           Chebyshev moments a_k = sum_j w_j T_k(2t_j-1), b_k = sum_j w_j (t_j - 1/4) T_k(2t_j-1) (k = 0 halved);
-//           K = 60/log2(rho) + 2 terms, taken when K <= kmc and cheaper than the NEAR loop.
+//           K terms from the Kreq table (prep_series_kreq), taken when K <= kmc and cheaper than the NEAR loop.
 //   EXACT   zeta within tau of [0,1];   NEAR  the rest (zeta close to [0,1], or few angular nodes).
 // ---------------------------------------------------------------------------------------------
-template <typename T, bool COUNT>
-__device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta, cd zeta, double mur, double mui,
-                                        RouteCount& rc) {
-  typedef typename Vec2<T>::type V2;
-  int route, K;
+// The series argument of one (point, radial node, pole), as route_setup leaves it
+struct SeriesArg {
   cd sg, g;     // series argument s and prefactor
   double ns;    // -|s|^2
+  int K, route;
+};
+
+template <typename T>
+__device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
+  SeriesArg o;
   if (fabs(zeta.re) >= kMomentMin || fabs(zeta.im) >= kMomentMin) {
-    route = ROUTE_MOMENT;
+    o.route = ROUTE_MOMENT;
     const double zc = zeta.re - 0.5;
     const double in = rcp_fast(fma(zc, zc, zeta.im * zeta.im));   // |zeta| < 2^500 (gf.h: domain)
-    sg = {zc * in, -zeta.im * in};
-    ns = -in;
-    g = sg;
+    o.sg = {zc * in, -zeta.im * in};
+    o.ns = -in;
+    o.g = o.sg;
     // (|s|/2)^K <= 2^-kSeriesBits;  log2 |s|^2 <= -4 (-inf when it underflows in FP32: K = 2)
-    K = (int)(2.f * kSeriesBits * rcp_ftz(2.f - lg2_ftz((float)in))) + 2;
+    o.K = (int)(2.f * kSeriesBits * rcp_ftz(2.f - lg2_ftz((float)in))) + 2;
   } else {
     // root = sqrt(zeta (zeta - 1)) = sqrt(w^2 - 1)/2, sign such that |w + 2 root| >= 1
     const double zm = zeta.re - 1.0, wr = fma(2.0, zeta.re, -1.0), wi = zeta.im + zeta.im;
@@ -332,55 +339,80 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
     if (fma(wr, ar, wi * ai) < 0.0) { ar = -ar; ai = -ai; }
     const double Dr = fma(2.0, ar, wr), Di = fma(2.0, ai, wi);
     const double in = rcp_fast(fma(Dr, Dr, Di * Di));   // 1/rho^2
-    sg = {Dr * in, -Di * in};
-    ns = -in;
+    o.sg = {Dr * in, -Di * in};
+    o.ns = -in;
     const double g2 = rm + rm;                   // 4/sqrt(w^2-1) = 2 conj(root)/|q|
-    g = {ar * g2, -ai * g2};
+    o.g = {ar * g2, -ai * g2};
     // terms needed at this rho (table made from the coefficients themselves, prep_series_kreq).  zeta on [0,1]
     // itself gives rho = 1 or NaN: the comparison fails, never CHEB
     const float ell = -0.5f * lg2_ftz((float)in);     // log2(rho)
-    K = ell >= kEllLo ? tb.kreq[min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)] : 1 << 20;
-    route = ROUTE_CHEB;
-    if (!(K <= tb.kmc && 4 * K + kChebNodeCost < 8 * tb.n_pairs + kNearNodeCost)) {
-      K = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
-      route = (zeta.im * zeta.im < tb.tau * tb.tau && zeta.re > -tb.tau && zeta.re < 1.0 + tb.tau) ? ROUTE_EXACT
-                                                                                                   : ROUTE_NEAR;
+    o.K = ell >= kEllLo ? tb.kreq[min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)] : 1 << 20;
+    o.route = ROUTE_CHEB;
+    if (!(o.K <= tb.kmc && 4 * o.K + kChebNodeCost < 8 * tb.n_pairs + kNearNodeCost)) {
+      o.K = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
+      o.route = (zeta.im * zeta.im < tb.tau * tb.tau && zeta.re > -tb.tau && zeta.re < 1.0 + tb.tau) ? ROUTE_EXACT
+                                                                                                     : ROUTE_NEAR;
     }
   }
-  int Kw = __reduce_max_sync(0xffffffffu, K);
+  return o;
+}
+
+// S = g [delta P(s) - N(s)] from the recurrence's last two values of each polynomial
+template <typename T, bool COUNT>
+__device__ __forceinline__ cd series_finish(const SeriesArg& o, cd delta, T p1, T p2, T n1, T n2, RouteCount& rc) {
+  const double b0 = (double)p1, b1 = (double)p2, d0 = (double)n1, d1 = (double)n2;
+  const double Pr = fma(-b1, o.sg.re, b0), Pi = b1 * o.sg.im;     // c_0 - c_1 conj(s)
+  const double Nr = fma(-d1, o.sg.re, d0), Ni = d1 * o.sg.im;
+  const cd acc = {fma(delta.re, Pr, fma(-delta.im, Pi, -Nr)), fma(delta.re, Pi, fma(delta.im, Pr, -Ni))};
+  if (COUNT) {
+    rc.series_used += o.K;
+    if (o.route == ROUTE_CHEB) ++rc.n_cheb; else ++rc.n_moment;
+  }
+  return cmul(o.g, acc);
+}
+
+// The direct loop for a lane on the NEAR or EXACT route
+template <typename T, bool COUNT>
+__device__ __forceinline__ cd direct_route(const Tabs<T>& tb, int route, cd x, cd y, cd delta, cd zeta, double mur,
+                                           double mui, RouteCount& rc) {
+  cd s;
+  const cd eta = {__dadd_rn(0.25, delta.re), delta.im};
+  bool dd_loop = true;
+  if (sizeof(T) == 8 && !__any_sync(__activemask(), route == ROUTE_EXACT)) {
+    // no EXACT lane among the lanes here: the 8-instruction pair (zeta in double is accurate enough for NEAR)
+    s = angular_near<T>(eta, zeta, tb.mu0, tb.stT, tb.swT, tb.n_pairs);
+    dd_loop = false;
+  } else if (sizeof(T) == 8 || route == ROUTE_EXACT) {
+    ZetaDD z = {zeta.re, 0.0, zeta.im, zeta.im * zeta.im};
+    if (route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y.re, y.im, mur, mui);
+    s = angular_direct(eta, z, tb.mu0, tb.st, tb.stlo, tb.sw, tb.n_pairs);
+  } else {
+    s = angular_near<T>(eta, zeta, tb.mu0, tb.stT, tb.swT, tb.n_pairs);
+    dd_loop = false;
+  }
+  if (COUNT) {
+    if (dd_loop) rc.exact_pairs += tb.n_pairs; else rc.near_pairs += tb.n_pairs;   // by loop, not by route
+    if (route == ROUTE_EXACT) ++rc.n_exact; else ++rc.n_near;
+  }
+  return s;
+}
+
+template <typename T, bool COUNT>
+__device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta, cd zeta, double mur, double mui,
+                                        RouteCount& rc) {
+  typedef typename Vec2<T>::type V2;
+  const SeriesArg o = route_setup<T>(tb, zeta);
+  int Kw = __reduce_max_sync(0xffffffffu, o.K);
   Kw = min((Kw + 1) & ~1, tb.kmc);
   cd s = {0.0, 0.0};
   if (Kw > 0) {  // warp-uniform
-    const V2* tab = route == ROUTE_CHEB ? tb.cheb : tb.mom;
+    const V2* tab = o.route == ROUTE_CHEB ? tb.cheb : tb.mom;
     T p1, p2, n1, n2;
-    goertzel_pair<T>(tab, Kw, (T)(sg.re + sg.re), (T)ns, p1, p2, n1, n2);
+    goertzel_pair<T>(tab, Kw, (T)(o.sg.re + o.sg.re), (T)o.ns, p1, p2, n1, n2);
     if (COUNT) rc.series_exec += Kw;
-    if (route <= ROUTE_CHEB) {
-      const double b0 = (double)p1, b1 = (double)p2, d0 = (double)n1, d1 = (double)n2;
-      const double Pr = fma(-b1, sg.re, b0), Pi = b1 * sg.im;     // c_0 - c_1 conj(s)
-      const double Nr = fma(-d1, sg.re, d0), Ni = d1 * sg.im;
-      const cd acc = {fma(delta.re, Pr, fma(-delta.im, Pi, -Nr)), fma(delta.re, Pi, fma(delta.im, Pr, -Ni))};
-      s = cmul(g, acc);
-      if (COUNT) {
-        rc.series_used += K;
-        if (route == ROUTE_CHEB) ++rc.n_cheb; else ++rc.n_moment;
-      }
-    }
+    if (o.route <= ROUTE_CHEB) s = series_finish<T, COUNT>(o, delta, p1, p2, n1, n2, rc);
   }
-  if (route >= ROUTE_NEAR) {
-    const cd eta = {__dadd_rn(0.25, delta.re), delta.im};
-    if (sizeof(T) == 8 || route == ROUTE_EXACT) {
-      ZetaDD z = {zeta.re, 0.0, zeta.im, zeta.im * zeta.im};
-      if (route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y.re, y.im, mur, mui);
-      s = angular_direct(eta, z, tb.mu0, tb.st, tb.stlo, tb.sw, tb.n_pairs);
-    } else {
-      s = angular_near<T>(eta, zeta, tb.mu0, tb.stT, tb.swT, tb.n_pairs);
-    }
-    if (COUNT) {
-      if (route == ROUTE_EXACT) { rc.exact_pairs += tb.n_pairs; ++rc.n_exact; }
-      else { rc.near_pairs += tb.n_pairs; ++rc.n_near; }
-    }
-  }
+  if (o.route >= ROUTE_NEAR) s = direct_route<T, COUNT>(tb, o.route, x, y, delta, zeta, mur, mui, rc);
   return s;
 }
 

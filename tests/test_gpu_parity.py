@@ -212,7 +212,9 @@ def test_route_counters(gf):
     # the nodes of the large-y tail take no route; the rest take exactly one
     assert 0 < c["near_nodes"] + series_nodes + c["exact_nodes"] < 0.6 * x.numel() * cfg["n_rad"]
     assert c["tails"] == x.numel()
-    assert c["near_pairs"] == c["near_nodes"] * n_pairs and c["exact_pairs"] == c["exact_nodes"] * n_pairs
+    # pairs are counted by loop (the NEAR lanes of a warp with an EXACT lane run the double-double loop too)
+    assert c["near_pairs"] + c["exact_pairs"] == (c["near_nodes"] + c["exact_nodes"]) * n_pairs
+    assert c["exact_pairs"] >= c["exact_nodes"] * n_pairs
     # each series triple needs 2..256 terms; a warp runs its longest series on all 32 lanes
     assert 2 * series_nodes <= c["series_terms_needed"] <= 256 * series_nodes
     assert c["series_terms_needed"] <= c["series_terms"] <= 256 * x.numel() * cfg["n_rad"]
