@@ -223,15 +223,20 @@ __device__ __forceinline__ void goertzel_pair(const typename Vec2<T>::type* __re
                                               T& p1, T& p2, T& n1, T& n2) {
   typedef typename Vec2<T>::type V2;
   p1 = p2 = n1 = n2 = (T)0;
-  const V2* c = tab + Kw;
+  // software pipeline: the coefficients of the next two terms are loaded while the current two are used (the
+  // last trip reads the two entries below the table, which exist in the staged block and are not used)
+  const V2* c = tab + Kw - 2;
+  V2 c1 = c[1], c0 = c[0];
 #pragma unroll(kGoertzelUnroll)
   for (int k = Kw; k > 0; k -= 2) {
     c -= 2;
-    const V2 c1 = c[1], c0 = c[0];
+    const V2 m1 = c[1], m0 = c[0];
     p2 = fma(r, p1, fma(ns, p2, c1.x));
     n2 = fma(r, n1, fma(ns, n2, c1.y));
     p1 = fma(r, p2, fma(ns, p1, c0.x));
     n1 = fma(r, n2, fma(ns, n1, c0.y));
+    c1 = m1;
+    c0 = m0;
   }
 }
 
