@@ -15,7 +15,10 @@ struct PoleTerm {
 };
 
 constexpr int kMaxTerms = 2;
-constexpr int kBlockThreads = 256;
+#ifndef GF_BLOCK_THREADS
+#define GF_BLOCK_THREADS 256
+#endif
+constexpr int kBlockThreads = GF_BLOCK_THREADS;
 constexpr int kKreqBins = 256;
 constexpr int kTailN = 32;  // terms of the large-y tail series (gf_eval.cu)
 

@@ -343,15 +343,17 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     double ai = qr >= 0.0 ? kk : copysign(h, qi);
     if (fma(wr, ar, wi * ai) < 0.0) { ar = -ar; ai = -ai; }
     const double Dr = fma(2.0, ar, wr), Di = fma(2.0, ai, wi);
-    const double in = rcp_fast(fma(Dr, Dr, Di * Di));   // 1/rho^2
+    const double rho2 = fma(Dr, Dr, Di * Di);
+    // terms needed at this rho (table made from the coefficients themselves, prep_series_kreq); taken from rho^2
+    // directly so that the look-up does not wait for the reciprocal.  zeta on [0,1] itself gives rho = 1 or NaN:
+    // the comparison fails, never CHEB
+    const float ell = 0.5f * lg2_ftz((float)rho2);     // log2(rho)
+    o.K = ell >= kEllLo ? tb.kreq[min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)] : 1 << 20;
+    const double in = rcp_fast(rho2);                  // 1/rho^2
     o.sg = {Dr * in, -Di * in};
     o.ns = -in;
     const double g2 = rm + rm;                   // 4/sqrt(w^2-1) = 2 conj(root)/|q|
     o.g = {ar * g2, -ai * g2};
-    // terms needed at this rho (table made from the coefficients themselves, prep_series_kreq).  zeta on [0,1]
-    // itself gives rho = 1 or NaN: the comparison fails, never CHEB
-    const float ell = -0.5f * lg2_ftz((float)in);     // log2(rho)
-    o.K = ell >= kEllLo ? tb.kreq[min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)] : 1 << 20;
     o.route = ROUTE_CHEB;
     if (!(o.K <= tb.kmc && 4 * o.K + kChebNodeCost < 8 * tb.n_pairs + kNearNodeCost)) {
       o.K = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
@@ -407,11 +409,11 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
                                         RouteCount& rc) {
   typedef typename Vec2<T>::type V2;
   const SeriesArg o = route_setup<T>(tb, zeta);
+  const V2* tab = o.route == ROUTE_CHEB ? tb.cheb : tb.mom;
   int Kw = __reduce_max_sync(0xffffffffu, o.K);
   Kw = min((Kw + 1) & ~1, tb.kmc);
   cd s = {0.0, 0.0};
   if (Kw > 0) {  // warp-uniform
-    const V2* tab = o.route == ROUTE_CHEB ? tb.cheb : tb.mom;
     T p1, p2, n1, n2;
     goertzel_pair<T>(tab, Kw, (T)(o.sg.re + o.sg.re), (T)o.ns, p1, p2, n1, n2);
     if (COUNT) rc.series_exec += Kw;
