@@ -36,7 +36,9 @@
 // the paper's eq. (18) for masses^2 = +-i/2, the Feynman-parameter form CF3 for
 // the rational propagator, G(0)=0, conjugation symmetry, cutoff independence,
 // line-swap symmetry, rule independence, exactness degree of the quadrature
-// rules, brute-force high-order quadrature.  Unpinned: values of RAY_ARC inside
+// rules, brute-force high-order quadrature; the paper's Kernels 3 and 4 (angular integral B of eq. (22) over
+// complex y; obstruction of the real y-axis by the cut) against the textbook angular integral, the scan
+// itself and the parabola of PAPER.md:270.  Unpinned: values of RAY_ARC inside
 // the wedge around the negative real axis and of REAL outside the parabola R2
 // (DESIGN.md "parity unpinned"), where no closed form applies.
 //
@@ -412,6 +414,90 @@ cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int
   return P.prefactor * cplx((double)gr, (double)gi);
 }
 
+// ---- paper Kernel 3 (Fig. 1): the angular integral B of eq. (22) for one x at a
+// complex y:  B(x, y) = sum_j w'_j [ D2(u_j) - D2(y) ] / D2(y),  u_j = x + y - 2 sqrt(x) sqrt(y) z_j.
+// For the massive line of the paper's example this is eq. (22)'s
+//   B = int dz sqrt(1-z^2) (-x + 2 sqrt(x) sqrt(y) z) / (x + y - 2 sqrt(x) sqrt(y) z + m2^2).
+// Plain loop over the angular nodes, every term and the sum in R.
+template <typename R>
+cplx angular_B(const Params& P, cplx x, cplx y, const double* z, const double* wz, int n_ang) {
+  typedef std::complex<R> C;
+  C xx((R)x.real(), (R)x.imag()), yy((R)y.real(), (R)y.imag());
+  C B2 = (R)2 * psqrt<R>(xx) * psqrt<R>(yy);
+  C D2y = prop<R>(P.line_pk, yy);
+  R sr = 0, si = 0;
+  for (int j = 0; j < n_ang; ++j) {
+    C d = xx - B2 * (R)z[j];
+    C f = prop_diff<R>(P.line_pk, yy, d) / D2y;
+    sr += (R)wz[j] * f.real();
+    si += (R)wz[j] * f.imag();
+  }
+  return cplx((double)sr, (double)si);
+}
+
+// ---- paper Kernel 4 (Fig. 2): does the branch cut that the angular integral induces in
+// the y-plane obstruct the original contour, the positive real y-axis up to Lambda^2?  The paper does not say
+// how its kernel decides (reading G19).  Here: the cut of a pole -mu of line 2 is the curve
+//   y(z) = k(z)^2,  k(z) = sqrt(x) z + i s(z),  s(z) = sqrt(x (1 - z^2) + mu),  -1 <= z <= 1       eq. (23)-(25)
+// (the second sign of eq. (24) is the same curve run backwards).  It is sampled at n_z equidistant z, s(z)
+// continued from sample to sample (the sign that keeps Re(s_k conj(s_{k-1})) >= 0; principal root at z = -1),
+// and a crossing is counted wherever Im y changes sign between neighbours (or is zero at the later one) and
+// the linearly interpolated Re y lies in (0, Lambda^2].  Every operation is a correctly rounded +, -, *, /
+// or sqrt in a fixed order, so that an integer decision is the same on any IEEE machine.
+struct CD { double re, im; };
+inline CD csqrt_rn(CD v) {   // principal square root from real operations only
+  const double m = std::sqrt(v.re * v.re + v.im * v.im);
+  const double h = std::sqrt(0.5 * (m + std::fabs(v.re)));
+  if (h == 0.0) return CD{0.0, 0.0};
+  const double k = v.im / (2.0 * h);
+  if (v.re >= 0.0) return CD{h, k};
+  return CD{std::fabs(k), std::copysign(h, v.im)};
+}
+int cut_crossings_one(CD x, CD mu, double cutoff2, int n_z) {
+  const CD sx = csqrt_rn(x);
+  int count = 0;
+  CD sprev{0.0, 0.0};
+  double yre_prev = 0.0, yim_prev = 0.0;
+  for (int k = 0; k < n_z; ++k) {
+    const double z = -1.0 + 2.0 * (double)k / (double)(n_z - 1);
+    const double omz2 = (1.0 - z) * (1.0 + z);
+    CD s = csqrt_rn(CD{x.re * omz2 + mu.re, x.im * omz2 + mu.im});
+    if (k > 0 && s.re * sprev.re + s.im * sprev.im < 0.0) { s.re = -s.re; s.im = -s.im; }
+    const double kre = sx.re * z - s.im, kim = sx.im * z + s.re;   // sqrt(x) z + i s
+    const double yre = kre * kre - kim * kim, yim = 2.0 * (kre * kim);
+    if (k > 0) {
+      const bool cross = (yim_prev < 0.0 && yim >= 0.0) || (yim_prev > 0.0 && yim <= 0.0);
+      if (cross) {
+        const double t = yim_prev / (yim_prev - yim);               // in (0, 1]
+        const double re0 = yre_prev + t * (yre - yre_prev);
+        if (re0 > 0.0 && re0 <= cutoff2) ++count;
+      }
+    }
+    sprev = s;
+    yre_prev = yre;
+    yim_prev = yim;
+  }
+  return count;
+}
+// all poles of line 2: one for a massive line (mu = m2^2), two for a rational one (the roots of Q(-mu) = 0)
+int cut_crossings(const Params& P, cplx x, int n_z) {
+  const Propagator& q = P.line_pk;
+  if (q.kind == PROP_MASSIVE) return cut_crossings_one(CD{x.real(), x.imag()}, CD{q.m2_re, q.m2_im}, P.cutoff2, n_z);
+  const double disc = q.a * q.a - 4.0 * q.b;
+  CD mu1, mu2;   // mu = -u_r, u_r = (-a +- sqrt(disc))/2
+  if (disc >= 0.0) {
+    const double r = std::sqrt(disc);
+    mu1 = CD{0.5 * (q.a - r), 0.0};
+    mu2 = CD{0.5 * (q.a + r), 0.0};
+  } else {
+    const double r = std::sqrt(-disc);
+    mu1 = CD{0.5 * q.a, -0.5 * r};
+    mu2 = CD{0.5 * q.a, 0.5 * r};
+  }
+  return cut_crossings_one(CD{x.real(), x.imag()}, mu1, P.cutoff2, n_z) +
+         cut_crossings_one(CD{x.real(), x.imag()}, mu2, P.cutoff2, n_z);
+}
+
 int check_params(const Params& P, int n_rad, int n_ang) {
   if (n_rad < 1 || n_ang < 1) return 2;
   if (!(P.cutoff2 > 0) || !(P.map_scale > 0)) return 2;
@@ -504,6 +590,33 @@ int gfo_contour_nodes(const void* params, double x_re, double x_im, const double
   }
   *n_out = (int)nodes.size();
   return pol;
+}
+
+// Kernel 3: B(x, y_k) for n complex y (interleaved re, im).  accum: 0 = double terms, 2 = long double terms.
+int gfo_eval_angular(const void* params, double x_re, double x_im, const double* ang_nodes, const double* ang_weights,
+                     int n_ang, const double* y, long long n, double* out, int accum) {
+  if (!params || !ang_nodes || !ang_weights || (!y && n) || (!out && n)) return 1;
+  if (n_ang < 1 || n < 0) return 2;
+  Params P;
+  std::memcpy(&P, params, sizeof(Params));
+  for (long long k = 0; k < n; ++k) {
+    cplx b = accum == 0 ? angular_B<double>(P, cplx(x_re, x_im), cplx(y[2 * k], y[2 * k + 1]), ang_nodes, ang_weights, n_ang)
+                        : angular_B<ld>(P, cplx(x_re, x_im), cplx(y[2 * k], y[2 * k + 1]), ang_nodes, ang_weights, n_ang);
+    out[2 * k] = b.real();
+    out[2 * k + 1] = b.imag();
+  }
+  return 0;
+}
+
+// Kernel 4: crossings of (0, Lambda^2] by the cut(s) of line 2, for n points x; out: n 32-bit integers.
+int gfo_cut_crossings(const void* params, const double* x, long long n, int n_z, int* out) {
+  if (!params || (!x && n) || (!out && n)) return 1;
+  if (n_z < 2 || n < 0) return 2;
+  Params P;
+  std::memcpy(&P, params, sizeof(Params));
+  if (!(P.cutoff2 > 0)) return 2;
+  for (long long k = 0; k < n; ++k) out[k] = cut_crossings(P, cplx(x[2 * k], x[2 * k + 1]), n_z);
+  return 0;
 }
 
 int gfo_params_size(void) { return (int)sizeof(Params); }

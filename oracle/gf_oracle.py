@@ -47,7 +47,8 @@ def build(force=False):
     if (not force and os.path.exists(_LIB)
             and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
         return _LIB
-    cmd = ["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-pthread", "-o", _LIB, _SRC, "-lquadmath"]
+    cmd = ["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-pthread", "-o", _LIB, _SRC,
+           "-lquadmath"]
     subprocess.run(cmd, check=True)
     return _LIB
 
@@ -157,3 +158,29 @@ def contour_nodes(params, x, rad_nodes, rad_weights, n_rad, n_ang):
     if pol < 0:
         raise ValueError("gfo_contour_nodes failed")
     return pol, y[:n.value].copy(), wy[:n.value].copy()
+
+
+def eval_angular(params, x, ang_nodes, ang_weights, y, extended=True):
+    """Paper Kernel 3: the angular integral B(x, y) of eq. (22) for one complex x at every complex y."""
+    yf = np.ascontiguousarray(np.asarray(y, dtype=np.complex128)).ravel()
+    out = np.empty_like(yf)
+    an = np.ascontiguousarray(ang_nodes, dtype=np.float64)
+    aw = np.ascontiguousarray(ang_weights, dtype=np.float64)
+    x = complex(x)
+    rc = lib().gfo_eval_angular(ctypes.byref(params), ctypes.c_double(x.real), ctypes.c_double(x.imag), _dp(an),
+                                _dp(aw), int(an.size), _dp(yf.view(np.float64)), ctypes.c_longlong(yf.size),
+                                _dp(out.view(np.float64)), 2 if extended else 0)
+    if rc:
+        raise ValueError("gfo_eval_angular failed: %d" % rc)
+    return out.reshape(np.shape(y))
+
+
+def cut_crossings(params, x, n_z):
+    """Paper Kernel 4: how often the cut(s) of line 2 cross (0, Lambda^2] of the real y-axis, per point of x."""
+    xf = np.ascontiguousarray(np.asarray(x, dtype=np.complex128)).ravel()
+    out = np.empty(xf.size, dtype=np.int32)
+    rc = lib().gfo_cut_crossings(ctypes.byref(params), _dp(xf.view(np.float64)), ctypes.c_longlong(xf.size),
+                                 int(n_z), out.ctypes.data_as(ctypes.POINTER(ctypes.c_int)))
+    if rc:
+        raise ValueError("gfo_cut_crossings failed: %d" % rc)
+    return out.reshape(np.shape(x))

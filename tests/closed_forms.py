@@ -55,3 +55,17 @@ def in_parabola_R2(x, m2=1.0, shrink=0.0):
     derived from eq. (23), PAPER.md:219; 'parabola-shaped region on the right', PAPER.md:270)."""
     x = complex(x)
     return x.real - shrink > x.imag ** 2 / (4 * m2) - m2
+
+
+def angular_B_massive(x, y, mu):
+    """Paper eq. (22), term B, in the continuum for a massive line 2 with mass^2 mu:
+       B = (y + mu) [ pi (A - r) / b^2 - (pi/2)/(y + mu) ],  A = x + y + mu, b = 2 sqrt(x) sqrt(y), r^2 = A^2 - b^2,
+    from the textbook integral  int_-1^1 sqrt(1-z^2)/(A - b z) dz = pi (A - r)/b^2  with the root r for which
+    |A - r| < |A + r| (the branch that decays like pi/(2A); it is analytic in A/b off [-1, 1], i.e. off the cut of
+    eq. (25))."""
+    x, y, mu = mp.mpc(x), mp.mpc(y), mp.mpc(mu)
+    A, b = x + y + mu, 2 * mp.sqrt(x) * mp.sqrt(y)
+    r = mp.sqrt(A * A - b * b)
+    if (mp.conj(A) * r).real < 0:
+        r = -r
+    return (y + mu) * (mp.pi * (A - r) / b ** 2 - mp.pi / 2 / (y + mu))

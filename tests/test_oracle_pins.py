@@ -406,3 +406,85 @@ def test_oracle_rejects_unsupported(oracle):
         oracle.eval_grid(oracle.make_params(BUB, RAT, 1e6, contour="thread"), rn, rw, 64, z, wz, xs)
     g, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e6), rn, rw, 64, z, wz, np.zeros(0, dtype=complex))
     assert g.size == 0
+
+
+# ---------------------------------------------------------------- paper Kernels 3 and 4
+@pytest.mark.parametrize("mu", [1.0, -0.5j])
+def test_kernel3_angular_integral_closed_form(oracle, mu):
+    """B(x, y) of eq. (22) with the Gauss rule of the measure against the textbook angular integral,
+    for the bubble and for the paper's line 2 (mass^2 -i/2), at complex y off the cut.  Catches a wrong sign of d,
+    a missing factor (y + mu), a wrong branch of sqrt(y)."""
+    P = oracle.make_params({"kind": "massive", "m2": 1.0}, {"kind": "massive", "m2": mu}, 1e6)
+    z, wz = oracle.make_quadrature("gauss_cheb2", 256, measure="sqrt1mz2")
+    for x in (1.0 + 2.0j, 0.3 - 0.2j, 2.5):
+        ys = np.array([0.3 + 0.2j, 2.0 - 1.0j, 5.0 + 0.5j, -2 + 6j, 10.0, 0.01, -4 - 4j])
+        B = oracle.eval_angular(P, x, z, wz, ys)
+        ref = np.array([complex(CF.angular_B_massive(x, y, mu)) for y in ys])
+        assert relerr(B, ref).max() < 1e-12, (x, relerr(B, ref))
+    # x = 0: the integrand vanishes identically (the factor d of eq. (20))
+    assert np.all(oracle.eval_angular(P, 0.0, z, wz, np.array([1.0 + 1j, 3.0])) == 0)
+
+
+def test_kernel3_is_the_inner_sum_of_the_scan(oracle):
+    """G(x) = c0 sum_i Wr_i y_i D1(y_i) D2(y_i) B(x, y_i): the scan rebuilt from Kernel 3 on the nodes of its own
+    contour (deformed ones included) -- ties B's normalisation to the pinned G, for a massive and a rational line 2."""
+    n_rad, n_ang = 64, 32
+    for lpk, contour in ((BUB, "real"), (RAT, "real"), (BUB, "ray_arc")):
+        P = oracle.make_params(BUB, lpk, 1e4, contour=contour)
+        rn, rw, z, wz = tables(oracle, n_rad, n_ang, "gauss_legendre")
+        for x in (0.5 + 0.2j, -3.0 + 1.5j):
+            _, y, wy = oracle.contour_nodes(P, x, rn, rw, n_rad, n_ang)
+            B = oracle.eval_angular(P, x, z, wz, y)
+            d1 = 1.0 / (y + 1.0)
+            d2 = 1.0 / (y + 1.0) if lpk is BUB else (y + RAT["M2"]) / (y * y + RAT["a"] * y + RAT["b"])
+            g = P.prefactor * np.sum(wy * y * d1 * d2 * B)
+            ref, _ = oracle.eval_grid(P, rn, rw, n_rad, z, wz, np.array([x]))
+            assert abs(g - ref[0]) <= 1e-13 * abs(ref[0])
+
+
+def test_kernel4_obstruction_is_the_parabola(oracle):
+    """The set where the cut leaves the positive real y-axis free is 'a parabola-shaped region on the right'
+    (PAPER.md:270): Re x > (Im x)^2/(4 m^2) - m^2 for a real mass (reading R2, from eq. (23)), and
+    Re x > (Im x)^2 - 1/4 for the paper's line 2 with mass^2 -i/2.  Away from the boundary by 1e-9 every point of
+    a grid must agree.  Catches a wrong branch continuation of eq. (25), a wrong sign test, an off-by-one in z."""
+    re, im = np.linspace(-6, 3, 91), np.linspace(-4, 4, 81)
+    X = re[None, :] + 1j * im[:, None]
+    for m2 in (1.0, 0.25):
+        P = oracle.make_params(BUB, {"kind": "massive", "m2": m2}, 1e6)
+        c = oracle.cut_crossings(P, X, 2001)
+        margin = X.real - (X.imag ** 2 / (4 * m2) - m2)
+        far = np.abs(margin) > 1e-9
+        assert np.array_equal((c == 0)[far], (margin > 0)[far])
+        assert set(np.unique(c)) <= {0, 1}
+    P = oracle.make_params({"kind": "massive", "m2": 0.5j}, {"kind": "massive", "m2": -0.5j}, 1e6)
+    c = oracle.cut_crossings(P, X, 2001)
+    margin = X.real - (X.imag ** 2 - 0.25)
+    far = np.abs(margin) > 1e-9
+    assert np.array_equal((c == 0)[far], (margin > 0)[far])
+
+
+def test_kernel4_respects_the_cutoff_and_counts_both_poles(oracle):
+    """A crossing beyond Lambda^2 does not obstruct [0, Lambda^2]; a rational line 2 has one cut per pole."""
+    x = np.array([-5.0 + 1.0j])
+    big = oracle.make_params(BUB, BUB, 1e6)
+    assert oracle.cut_crossings(big, x, 4001)[0] == 1
+    # where it crosses: y0 real with (x + y0 + 1)^2 = 4 x y0 t, some t in [0,1]; locate it by bisection on the count
+    lo, hi = 1e-3, 1e6
+    for _ in range(60):
+        mid = math.sqrt(lo * hi)
+        if oracle.cut_crossings(oracle.make_params(BUB, BUB, mid), x, 4001)[0]:
+            hi = mid
+        else:
+            lo = mid
+    y0 = hi
+    A = x[0] + y0 + 1.0
+    t = A * A / (4 * x[0] * y0)          # zeta at the crossing must lie on [0, 1]
+    assert abs(t.imag) < 1e-3 and -1e-3 < t.real < 1 + 1e-3
+    P = oracle.make_params(BUB, RAT, 1e6)
+    for xx in (-3.0 + 0.3j, 1.0 + 3.0j, 2.0 + 0.1j):
+        total = oracle.cut_crossings(P, np.array([xx]), 4001)[0]
+        parts = 0
+        for u, _ in CF.rational_poles(RAT["M2"], RAT["a"], RAT["b"]):
+            Pm = oracle.make_params(BUB, {"kind": "massive", "m2": complex(-u)}, 1e6)
+            parts += oracle.cut_crossings(Pm, np.array([xx]), 4001)[0]
+        assert total == parts
