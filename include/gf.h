@@ -164,6 +164,26 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
                       const double* h_ang_nodes, const double* h_ang_weights, int n_ang, const void* h_x,
                       long long n_points, void* h_out, void* stream);
 
+/* Paper Kernel 3 (Fig. 1): the angular integral B of eq. (22) for ONE x = (x_re, x_im) at
+ * n_y complex y (d_y, interleaved),
+ *     B(x, y) = sum_j w'_j [ D2(u_j) - D2(y) ] / D2(y),   u_j = x + y - 2 sqrt(x) sqrt(y) z_j,
+ * which for a massive line 2 is eq. (22)'s  int dz sqrt(1-z^2) (-x + 2 sqrt(x) sqrt(y) z)/(u + m2^2).  Only
+ * p->line_pk is used (line_k, cutoff2, contour play no part but must be valid); the angular rule as in
+ * gf_eval_grid.  d_out: n_y complex<double>.  x = 0 gives exactly 0; y = 0 is the limit value; where 4 x y
+ * overflows or underflows the entry is IEEE inf/NaN.  FP64 only.  Asynchronous on `stream`. */
+int gf_eval_angular(const gf_params* p, double x_re, double x_im, const double* d_ang_nodes,
+                    const double* d_ang_weights, int n_ang, const void* d_y, long long n_y, void* d_out, void* stream);
+
+/* Paper Kernel 4 (Fig. 2): for every x of d_x (n_points complex<double>), how often the branch
+ * cut(s) that the angular integral induces in the y-plane cross the original contour (0, Lambda^2] of the real
+ * y-axis; 0 means the contour "remains unharmed".  Procedure (reading G19; the paper does not give
+ * one): per pole -mu of line 2 the cut y(z) = (sqrt(x) z + i s(z))^2, s(z) = sqrt(x (1 - z^2) + mu) (eq. (23)-(25)),
+ * sampled at n_z equidistant z in [-1, 1] with s continued from sample to sample; a crossing is counted where
+ * Im y changes sign between neighbours and the linearly interpolated Re y is in (0, Lambda^2].  Every step is a
+ * correctly rounded real operation in a fixed order: the result is bit-identical to the oracle's.
+ * d_out: n_points 32-bit integers.  Asynchronous on `stream`. */
+int gf_cut_crossings(const gf_params* p, const void* d_x, long long n_points, int n_z, int* d_out, void* stream);
+
 /* The same evaluation, also counting the work by route for the roofline accounting.
  * d_counters: 9 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
  *   [0] pairs of the plain direct loop  [1] series terms EXECUTED (every lane of a warp runs its warp's longest

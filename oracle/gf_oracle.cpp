@@ -592,7 +592,9 @@ int gfo_contour_nodes(const void* params, double x_re, double x_im, const double
   return pol;
 }
 
-// Kernel 3: B(x, y_k) for n complex y (interleaved re, im).  accum: 0 = double terms, 2 = long double terms.
+// Kernel 3: B(x, y_k) for n complex y (interleaved re, im).  accum: 0 = double terms, 2 = long double terms,
+// 3 = binary128 terms (the +-z terms cancel by 2 sqrt(|y/x|) or 2 sqrt(|x/y|) and the leading moment by another
+// 1e7: at |y/x| = 1e6 even long double keeps only ten digits of B).
 int gfo_eval_angular(const void* params, double x_re, double x_im, const double* ang_nodes, const double* ang_weights,
                      int n_ang, const double* y, long long n, double* out, int accum) {
   if (!params || !ang_nodes || !ang_weights || (!y && n) || (!out && n)) return 1;
@@ -600,8 +602,10 @@ int gfo_eval_angular(const void* params, double x_re, double x_im, const double*
   Params P;
   std::memcpy(&P, params, sizeof(Params));
   for (long long k = 0; k < n; ++k) {
-    cplx b = accum == 0 ? angular_B<double>(P, cplx(x_re, x_im), cplx(y[2 * k], y[2 * k + 1]), ang_nodes, ang_weights, n_ang)
-                        : angular_B<ld>(P, cplx(x_re, x_im), cplx(y[2 * k], y[2 * k + 1]), ang_nodes, ang_weights, n_ang);
+    const cplx xx(x_re, x_im), yy(y[2 * k], y[2 * k + 1]);
+    cplx b = accum == 0   ? angular_B<double>(P, xx, yy, ang_nodes, ang_weights, n_ang)
+             : accum == 2 ? angular_B<ld>(P, xx, yy, ang_nodes, ang_weights, n_ang)
+                          : angular_B<__float128>(P, xx, yy, ang_nodes, ang_weights, n_ang);
     out[2 * k] = b.real();
     out[2 * k + 1] = b.imag();
   }

@@ -160,7 +160,7 @@ def contour_nodes(params, x, rad_nodes, rad_weights, n_rad, n_ang):
     return pol, y[:n.value].copy(), wy[:n.value].copy()
 
 
-def eval_angular(params, x, ang_nodes, ang_weights, y, extended=True):
+def eval_angular(params, x, ang_nodes, ang_weights, y, terms="long_double"):
     """Paper Kernel 3: the angular integral B(x, y) of eq. (22) for one complex x at every complex y."""
     yf = np.ascontiguousarray(np.asarray(y, dtype=np.complex128)).ravel()
     out = np.empty_like(yf)
@@ -169,7 +169,7 @@ def eval_angular(params, x, ang_nodes, ang_weights, y, extended=True):
     x = complex(x)
     rc = lib().gfo_eval_angular(ctypes.byref(params), ctypes.c_double(x.real), ctypes.c_double(x.imag), _dp(an),
                                 _dp(aw), int(an.size), _dp(yf.view(np.float64)), ctypes.c_longlong(yf.size),
-                                _dp(out.view(np.float64)), 2 if extended else 0)
+                                _dp(out.view(np.float64)), {"double": 0, "long_double": 2, "binary128": 3}[terms])
     if rc:
         raise ValueError("gfo_eval_angular failed: %d" % rc)
     return out.reshape(np.shape(y))

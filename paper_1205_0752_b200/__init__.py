@@ -69,6 +69,8 @@ _SIGNATURES = {
     "gf_eval_workspace_size": [ctypes.POINTER(gf_params), _int, _int],
     "gf_eval_prepare": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _vp],
     "gf_eval_grid_prepared": [ctypes.POINTER(gf_params), _int, _int, _vp, _vp, _ll, _vp, _vp, _vp],
+    "gf_eval_angular": [ctypes.POINTER(gf_params), _dbl, _dbl, _vp, _vp, _int, _vp, _ll, _vp, _vp],
+    "gf_cut_crossings": [ctypes.POINTER(gf_params), _vp, _ll, _int, _vp, _vp],
     "gf_eval_launch_info": [ctypes.POINTER(gf_params), _int, _int, _ll, ctypes.POINTER(gf_launch_info)],
     "gf_diag_fp64_peak": [_int, _int, _ll, _vp, _vp],
     "gf_diag_rcp_seed": [_vp, _vp, _ll, _vp],
@@ -279,6 +281,29 @@ def eval_grid_prepared(params, n_rad, n_ang, workspace, x, out=None, stream=None
     with torch.cuda.device(x.device):
         _check(lib().gf_eval_grid_prepared(ctypes.byref(params), n_rad, n_ang, workspace.data_ptr(), x.data_ptr(),
                                            x.numel(), out.data_ptr(), None, _stream(stream)))
+    return out
+
+
+def eval_angular(params, x, ang_nodes, ang_weights, y, out=None, stream=None):
+    """gf_eval_angular (paper Kernel 3): B(x, y) of eq. (22) for one complex x at every y (complex128 device tensor)."""
+    assert y.is_cuda and y.dtype == torch.complex128 and y.is_contiguous()
+    if out is None:
+        out = torch.empty_like(y)
+    x = complex(x)
+    with torch.cuda.device(y.device):
+        _check(lib().gf_eval_angular(ctypes.byref(params), x.real, x.imag, ang_nodes.data_ptr(), ang_weights.data_ptr(),
+                                     ang_nodes.numel(), y.data_ptr(), y.numel(), out.data_ptr(), _stream(stream)))
+    return out
+
+
+def cut_crossings(params, x, n_z, out=None, stream=None):
+    """gf_cut_crossings (paper Kernel 4): crossings of (0, Lambda^2] by the cut(s) of line 2, int32 per point of x."""
+    assert x.is_cuda and x.dtype == torch.complex128 and x.is_contiguous()
+    if out is None:
+        out = torch.empty(x.shape, dtype=torch.int32, device=x.device)
+    with torch.cuda.device(x.device):
+        _check(lib().gf_cut_crossings(ctypes.byref(params), x.data_ptr(), x.numel(), int(n_z), out.data_ptr(),
+                                      _stream(stream)))
     return out
 
 

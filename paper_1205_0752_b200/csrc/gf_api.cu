@@ -400,6 +400,31 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
   return rc ? rc : rc2;
 }
 
+int gf_eval_angular(const gf_params* p, double x_re, double x_im, const double* d_ang_nodes,
+                    const double* d_ang_weights, int n_ang, const void* d_y, long long n_y, void* d_out, void* stream) {
+  EvalArgs a;
+  int rc = build_args(p, 8, n_ang, n_y, &a);   // the radial order plays no part
+  if (rc) return rc;
+  if (!std::isfinite(x_re) || !std::isfinite(x_im)) { set_error("eval_angular: x is not finite"); return GF_ERR_ARG; }
+  if (!d_ang_nodes || !d_ang_weights) { set_error("eval_angular: null table pointer"); return GF_ERR_NULL; }
+  if (n_y > 0 && (!d_y || !d_out)) { set_error("eval_angular: null y/output pointer"); return GF_ERR_NULL; }
+  a.ang_nodes = d_ang_nodes;
+  a.ang_weights = d_ang_weights;
+  a.x = static_cast<const double2*>(d_y);
+  a.out = d_out;
+  return launch_angular(a, x_re, x_im, static_cast<cudaStream_t>(stream));
+}
+
+int gf_cut_crossings(const gf_params* p, const void* d_x, long long n_points, int n_z, int* d_out, void* stream) {
+  EvalArgs a;
+  int rc = build_args(p, 8, 2, n_points, &a);  // neither quadrature order plays a part
+  if (rc) return rc;
+  if (n_z < 2 || n_z > (1 << 24)) { set_error("cut_crossings: n_z=%d out of range [2, 2^24]", n_z); return GF_ERR_ARG; }
+  if (n_points > 0 && (!d_x || !d_out)) { set_error("cut_crossings: null grid/output pointer"); return GF_ERR_NULL; }
+  a.x = static_cast<const double2*>(d_x);
+  return launch_cut_crossings(a, n_z, d_out, static_cast<cudaStream_t>(stream));
+}
+
 int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_points, gf_launch_info* out) {
   if (!out) { set_error("eval_launch_info: out is null"); return GF_ERR_NULL; }
   EvalArgs a;

@@ -302,7 +302,9 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
   if (COUNT) flush_counters(rc, active, counters);
 }
 
-BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail) {
+}  // namespace
+
+BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail) {
   BlobLayout L;
   L.npad = (n_pairs + 3) & ~3;
   L.kmc = kKmc;
@@ -333,7 +335,6 @@ BlobLayout make_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyram
   return L;
 }
 
-}  // namespace
 
 // ---------------------------------------------------------------------------------------------
 int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
@@ -346,7 +347,7 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   plan->split_log2 = sl;
   const long long threads = a.n_points << sl;
   plan->grid_blocks = (threads + kBlockThreads - 1) / kBlockThreads;
-  plan->layout = make_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes, plan->shared_nodes);
+  plan->layout = make_blob_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes, plan->shared_nodes);
   plan->smem_bytes = 16 + (size_t)plan->layout.n_doubles * sizeof(double);
   if (plan->smem_bytes > 200 * 1024) {
     set_error("eval_grid: tables need %zu bytes of shared memory (limit 200 KiB): reduce n_rad/n_ang",

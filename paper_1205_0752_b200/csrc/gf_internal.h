@@ -101,6 +101,11 @@ int launch_contour(const EvalArgs& a, const LaunchPlan& plan, const double* blob
 int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d_nodes, int n, double* d_y,
                       cudaStream_t stream);
 
+// gf_cut.cu: the paper's Kernels 3 and 4 (a.x holds the y array / the x array, a.out the result)
+BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail);  // gf_eval.cu
+int launch_angular(const EvalArgs& a, double x_re, double x_im, cudaStream_t stream);
+int launch_cut_crossings(const EvalArgs& a, int n_z, int* d_out, cudaStream_t stream);
+
 // gf_diag.cu
 int launch_fp64_peak(int blocks, int threads, long long iters, double* d_sink, cudaStream_t stream);
 int launch_rcp_seed(const double* d_in, double* d_out, long long n, cudaStream_t stream);

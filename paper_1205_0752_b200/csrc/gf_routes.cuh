@@ -512,8 +512,8 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
       const double wT1 = j + 1 < a.n_pairs ? w1 * scratch[(size_t)(j + 1) * L.kmc + k] : 0.0;
       tau = dd_add_d(tau, wT0);
       tau1 = dd_add_d(tau1, wT1);
-      nu = dd_add(nu, two_prod(wT0, t0 - 0.25));
-      nu1 = dd_add(nu1, two_prod(wT1, t1 - 0.25));
+      nu = dd_add(nu, dd_mul_d(dd_add_d(two_sum(t0, -0.25), blob[L.off_tlo + j]), wT0));
+      nu1 = dd_add(nu1, dd_mul_d(dd_add_d(two_sum(t1, -0.25), blob[L.off_tlo + j + 1]), wT1));
     }
     tau = dd_add(tau, tau1);
     nu = dd_add(nu, nu1);
@@ -525,7 +525,8 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
           const double t = blob[L.off_t + j];
           const double wp = blob[L.off_w + j] * powi(t - 0.5, km);
           mo = dd_add_d(mo, wp);
-          no = dd_add(no, two_prod(wp, t - 0.25));
+          // t - 1/4 with t = hi + lo: b_0 = sum_j w_j (t_j - 1/4) is ~1e-8 of its terms (0 in the continuum)
+          no = dd_add(no, dd_mul_d(dd_add_d(two_sum(t, -0.25), blob[L.off_tlo + j]), wp));
         }
         s_cpart[c][0][km] = mo;
         s_cpart[c][1][km] = no;

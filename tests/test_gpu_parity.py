@@ -454,3 +454,49 @@ def test_runs_on_the_callers_stream(gf):
         g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
     s.synchronize()
     assert torch.equal(g.view(torch.float64), ref.view(torch.float64))
+
+
+# ------------------------------------------------------------------ paper Kernels 3 and 4
+@pytest.mark.parametrize("lines", ["bubble", "paper_example", "rational"])
+def test_kernel3_angular_integral_over_complex_y(gf, oracle, lines):
+    """B(x, y) of eq. (22) over a grid of complex y like the paper's Fig. 1 (box around the origin, cut and poles
+    inside), several x, against the oracle's plain sum in binary128 terms.  Ragged count (last CTA partial)."""
+    lk = {"kind": "massive", "m2": 1.0}
+    lpk = {"bubble": {"kind": "massive", "m2": 1.0}, "paper_example": {"kind": "massive", "m2": -0.5j},
+           "rational": {"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2}}[lines]
+    n_ang = 128
+    P = gf.make_params(lk, lpk, 1e6)
+    Po = oracle.make_params(lk, lpk, 1e6)
+    z, wz = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    zo, wzo = oracle.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    re, im = np.linspace(-12, 12, 97), np.linspace(-12, 12, 95)
+    ys = (re[None, :] + 1j * im[:, None]).ravel()[:-7]
+    ys = np.concatenate([ys, [0.0, 1e-9, 250.0 + 3e4j, 1e6]])
+    for x in (1.0 + 2.0j, -3.0 + 0.5j, 0.3 - 0.2j, -4.5, 2.0, 0.0):
+        B = gf.eval_angular(P, x, z, wz, torch.from_numpy(ys).cuda()).cpu().numpy()
+        ref = oracle.eval_angular(Po, x, zo, wzo, ys, terms="binary128")   # cancellation at |y/x| >> 1, << 1
+        e = relerr(B, ref)
+        # a y exactly on the cut (real x, real y here) makes single terms infinite in both; compare the rest
+        ok = np.isfinite(ref.view(np.float64)).reshape(-1, 2).all(axis=1) & (np.abs(ref) < 1e12)
+        assert ok.sum() > 0.99 * ys.size
+        assert e[ok].max() <= TOL64, (x, e[ok].max(), ys[ok][e[ok].argmax()])
+        if x == 0.0:
+            assert np.all(B == 0)
+
+
+@pytest.mark.parametrize("lines", ["bubble", "paper_example", "rational", "rational_real_poles"])
+def test_kernel4_cut_crossings_bit_exact(gf, oracle, lines):
+    """The obstruction map of Fig. 2 on a grid like the paper's (128 x 128 over [-5, 5]^2, plus config 2's box):
+    integer results identical to the oracle's."""
+    lk = {"kind": "massive", "m2": 1.0}
+    lpk = {"bubble": {"kind": "massive", "m2": 1.0}, "paper_example": {"kind": "massive", "m2": -0.5j},
+           "rational": {"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2},
+           "rational_real_poles": {"kind": "rational", "M2": 0.7, "a": 3.0, "b": 1.5}}[lines]
+    for cutoff2, box, n_z in ((1e6, (-5.0, 5.0, 128, -5.0, 5.0, 128), 1001), (30.0, (-10.0, 2.0, 97, -4.0, 4.0, 61), 257)):
+        P = gf.make_params(lk, lpk, cutoff2)
+        Po = oracle.make_params(lk, lpk, cutoff2)
+        x = gf.make_grid(*box)
+        c = gf.cut_crossings(P, x, n_z).cpu().numpy()
+        ref = oracle.cut_crossings(Po, x.cpu().numpy(), n_z)
+        assert c.dtype == np.int32 and np.array_equal(c, ref)
+        assert 0 < (c == 0).sum() < c.size     # both kinds of point occur
