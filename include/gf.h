@@ -28,7 +28,7 @@
  *     the real axis, Fortran order).
  *   - Errors: GF_ERR_NULL for a null pointer, GF_ERR_ARG for a value out of range,
  *     GF_ERR_UNSUPPORTED for a combination the method does not define (taylor_order != 0, a
- *     subtraction point other than 0, the THREAD contour with unequal or complex masses, a
+ *     subtraction point other than 0, a dimension other than 4 on a deformed contour, the THREAD contour with unequal or complex masses, a
  *     rational propagator with a double pole, precision 32 on a contour other than REAL), GF_ERR_CUDA when the CUDA runtime reports an
  *     error (no device, launch failure).  gf_last_error() describes the last failure of the
  *     calling thread.  A denominator that vanishes at a quadrature node yields IEEE inf/NaN in
@@ -94,6 +94,11 @@ typedef struct {
   int contour;           /* gf_contour */
   int precision;         /* 64: complex<double> output (the contract); 32: the FP32 comparison
                             variant, complex<float> output */
+  double dim;            /* space-time dimension d in [1, 8], 0 meaning 4 ("arbitrary dimensions by
+                            trivial modifications"): the radial measure becomes dy y^((d-2)/2); the angular measure
+                            (1-z^2)^((d-3)/2) is the caller's, in the angular weights (GF_MEASURE_PLAIN is d = 3).
+                            d != 4 on the REAL contour only.  Constants of the d-dimensional measure go into
+                            `prefactor` (d^dk = 1/2 y^((d-2)/2) dy dOmega_d). */
 } gf_params;
 
 /* Step 4 / Kernel 1: fill d_x[n_im][n_re] (complex<double>) with the

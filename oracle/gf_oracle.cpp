@@ -83,6 +83,9 @@ struct Params {
   double map_scale;    // s0 of the shifted-log radial map
   int contour;
   int precision;
+  double dim;          // space-time dimension d ("arbitrary dimensions by trivial modifications");
+                       // 0 means 4.  The radial measure is dy y^((d-2)/2) (d^dk = 1/2 y^((d-2)/2) dy dOmega_d);
+                       // the angular measure (1-z^2)^((d-3)/2) is in the caller's angular weights.
 };
 
 // ---- quadrature rules on [-1,1] ----------------------------
@@ -407,7 +410,9 @@ cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int
       si += (ACC)((R)wz[j] * f.imag());
     }
     C S((R)sr, (R)si);
-    C term = wy * y * S;                                       // dy y (...), eq. (14)
+    // dy y^((d-2)/2) (...): eq. (14) for d = 4; other d on the real contour only (y > 0, real power)
+    C term = (P.dim == 0 || P.dim == 4) ? wy * y * S
+                                          : wy * C((R)powq((__float128)nodes[i].y.real(), (__float128)(0.5 * (P.dim - 2))), (R)0) * S;
     gr += (ACC)term.real();
     gi += (ACC)term.imag();
   }
@@ -505,6 +510,8 @@ int check_params(const Params& P, int n_rad, int n_ang) {
   if (P.contour < 0 || P.contour > 3) return 2;
   if (P.contour != CONTOUR_REAL && n_rad % 8 != 0) return 2;
   if (P.contour == CONTOUR_THREAD && !thread_applicable(P)) return 3;
+  if (!(P.dim == 0 || (P.dim >= 1 && P.dim <= 8))) return 2;
+  if (!(P.dim == 0 || P.dim == 4) && P.contour != CONTOUR_REAL) return 3;
   return 0;
 }
 

@@ -95,6 +95,8 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   if (p->contour < GF_CONTOUR_REAL || p->contour > GF_CONTOUR_AUTO) { set_error("eval_grid: unknown contour %d", p->contour); return GF_ERR_ARG; }
   if (p->taylor_order != 0) { set_error("eval_grid: taylor_order %d unsupported (only t^0, eq. (13))", p->taylor_order); return GF_ERR_UNSUPPORTED; }
   if (p->sub_re != 0 || p->sub_im != 0) { set_error("eval_grid: subtraction point must be 0 (eq. (13))"); return GF_ERR_UNSUPPORTED; }
+  if (!(p->dim == 0 || (p->dim >= 1 && p->dim <= 8))) { set_error("eval_grid: dim=%g outside [1, 8] (0 = 4)", p->dim); return GF_ERR_ARG; }
+  if (!(p->dim == 0 || p->dim == 4) && p->contour != GF_CONTOUR_REAL) { set_error("eval_grid: a dimension other than 4 is supported on the REAL contour only"); return GF_ERR_UNSUPPORTED; }
   if (p->contour != GF_CONTOUR_REAL && n_rad % 8 != 0) { set_error("eval_grid: deformed contours need n_rad %% 8 == 0"); return GF_ERR_ARG; }
 
   *a = EvalArgs{};
@@ -106,6 +108,7 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   a->cutoff2 = p->cutoff2;
   a->s0 = p->map_scale;
   a->c0 = p->prefactor;
+  a->ypow = (p->dim == 0 || p->dim == 4) ? 1.0 : 0.5 * (p->dim - 2.0);
   log_ratio_dd(0.0, p->cutoff2, p->map_scale, &a->Llog_hi, &a->Llog_lo);  // REAL contour: [0, Lambda^2]
   a->contour = p->contour;
   a->th5 = 0.75 * 3.14159265358979323846;  // 3 pi/4, correctly rounded

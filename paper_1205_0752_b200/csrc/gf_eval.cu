@@ -100,7 +100,8 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
       const double Wr = ip < a.n_rad ? 0.5 * a.rad_weights[i] * a.Llog_hi * (y + a.s0) : 0.0;
       blob[L.off_y + ip] = y;
       blob[L.off_q4 + ip] = 0.25 / y;
-      const cd d1 = cscale(line_k_real(a.line_k, y), a.c0 * Wr * y);
+      // radial measure dy y^((d-2)/2): y itself in d = 4 (eq. (14)), pow otherwise
+      const cd d1 = cscale(line_k_real(a.line_k, y), a.c0 * Wr * (a.ypow == 1.0 ? y : pow(y, a.ypow)));
       for (int r = 0; r < a.n_terms; ++r) {
         const cd ic = cinv(cd{y + a.term[r].mu_re, a.term[r].mu_im});
         const cd pr = cmul(cmul(d1, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);

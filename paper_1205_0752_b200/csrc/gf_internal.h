@@ -36,6 +36,7 @@ struct EvalArgs {
   PoleTerm term[kMaxTerms];
   gf_propagator line_k;
   double cutoff2, s0, c0;
+  double ypow;         // radial measure dy y^ypow: (d - 2)/2, 1 in d = 4
   double Llog_hi, Llog_lo;  // ln((Lambda^2 + s0)/s0) as a double-double (host, binary128)
   double line2_scale;  // |m2^2| or the largest pole modulus: sizes the deformed contours
   int contour;         // gf_contour

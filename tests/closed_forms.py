@@ -69,3 +69,16 @@ def angular_B_massive(x, y, mu):
     if (mp.conj(A) * r).real < 0:
         r = -r
     return (y + mu) * (mp.pi * (A - r) / b ** 2 - mp.pi / 2 / (y + mu))
+
+
+def bubble_d3(x, m=1.0):
+    """Equal-mass bubble in d = 3, subtracted at x = 0, normalised int d^3k/(2 pi)^3:
+         G(x) = arctan(sqrt(x)/(2m)) / (4 pi sqrt(x)) - 1/(8 pi m)
+    (textbook; arctan w = ln((1 + i w)/(1 - i w))/(2i); even in sqrt(x); cut x <= -4 m^2 like CF1).  In the
+    variables of the scan: c0 = 1/(8 pi^2), radial measure dy y^(1/2), angular measure dz (d^3k = 1/2 y^(1/2) dy 2 pi dz)."""
+    x, m = mp.mpc(x), mp.mpf(m)
+    if x == 0:
+        return mp.mpc(0)
+    w = mp.sqrt(x) / (2 * m)
+    at = mp.log((1 + 1j * w) / (1 - 1j * w)) / 2j
+    return at / (4 * mp.pi * mp.sqrt(x)) - 1 / (8 * mp.pi * m)

@@ -500,3 +500,27 @@ def test_kernel4_cut_crossings_bit_exact(gf, oracle, lines):
         ref = oracle.cut_crossings(Po, x.cpu().numpy(), n_z)
         assert c.dtype == np.int32 and np.array_equal(c, ref)
         assert 0 < (c == 0).sum() < c.size     # both kinds of point occur
+
+
+# ------------------------------------------------------------------ other dimensions
+@pytest.mark.parametrize("dim,measure", [(3.0, "plain"), (2.0, "plain"), (3.5, "sqrt1mz2"), (5.0, "sqrt1mz2")])
+def test_other_dimensions(gf, oracle, dim, measure):
+    """Radial measure dy y^((d-2)/2); the angular measure is whatever the weights carry.  Parity on
+    config 1's grid and orders, every point; the deformed contours refuse d != 4."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    c0 = 1 / (8 * np.pi ** 2)
+    P = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=c0, dim=dim)
+    Po = oracle.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=c0, dim=dim)
+    rn, rw = gf.make_radial_tables("real", cfg["n_rad"], W.RADIAL_RULE)
+    z, wz = gf.make_quadrature(W.ANGULAR_RULE, cfg["n_ang"], measure=measure)
+    rno, rwo = oracle.make_quadrature(W.RADIAL_RULE, cfg["n_rad"])
+    zo, wzo = oracle.make_quadrature(W.ANGULAR_RULE, cfg["n_ang"], measure=measure)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
+    ref, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, oracle_grid(oracle, cfg), accum="extended")
+    assert relerr(g, ref).max() <= TOL64
+    Pd = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], contour="auto", dim=dim)
+    rnp, rwp = gf.make_radial_tables("auto", cfg["n_rad"], W.RADIAL_RULE)
+    with pytest.raises(gf.GfError) as e:
+        gf.eval_grid(Pd, rnp, rwp, cfg["n_rad"], z, wz, x)
+    assert e.value.status == 3
