@@ -83,6 +83,8 @@ struct Params {
   double map_scale;    // s0 of the shifted-log radial map
   int contour;
   int precision;
+  int routing;         // 0: the paper's eq. (19), lines carry k and p-k; 1: symmetric, lines carry k+p/2 and
+                       // k-p/2 (equal massive lines, real contour)
   double dim;          // space-time dimension d ("arbitrary dimensions by trivial modifications");
                        // 0 means 4.  The radial measure is dy y^((d-2)/2) (d^dk = 1/2 y^((d-2)/2) dy dOmega_d);
                        // the angular measure (1-z^2)^((d-3)/2) is in the caller's angular weights.
@@ -242,6 +244,21 @@ std::complex<R> prop_diff(const Propagator& P, std::complex<R> y, std::complex<R
   C Qu = u * u + (R)P.a * u + (R)P.b;
   C Qy = y * y + (R)P.a * y + (R)P.b;
   return -d * (u * y + (R)P.M2 * (u + y) + ((R)P.a * (R)P.M2 - (R)P.b)) / (Qu * Qy);
+}
+
+// Symmetric routing (shift invariance of eq. (4)): both lines 1/(q^2 + m2) with
+// q = k +- p/2, (k +- p/2)^2 = y + x/4 +- sqrt(x) sqrt(y) z, so
+//   F = 1/((c' + b z)(c' - b z)),  c' = y + x/4 + m2,  b = sqrt(x) sqrt(y),   F(x=0) = 1/c^2,  c = y + m2,
+//   F_sub = F - F(x=0) = [c^2 - c'^2 + b^2 z^2] / ((c' + b z)(c' - b z) c^2)
+//         = x [y z^2 - (2c + x/4)/4] / ((c' + b z)(c' - b z) c^2)
+// (numerator combined so that x is an explicit factor, like eq. (20): exactly 0 at x = 0).
+template <typename R>
+std::complex<R> fsub_symmetric(const Propagator& P, std::complex<R> x, std::complex<R> y, std::complex<R> b, R z) {
+  typedef std::complex<R> C;
+  C m2((R)P.m2_re, (R)P.m2_im);
+  C c = y + m2, cp = c + x / (R)4;
+  C num = x * (y * (z * z) - ((R)2 * c + x / (R)4) / (R)4);
+  return num / ((cp + b * z) * (cp - b * z) * c * c);
 }
 
 // scale of the singular structure of line 2 in the y-plane: |m2^2| for a
@@ -405,7 +422,8 @@ cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int
     ACC sr = 0, si = 0;
     for (int j = 0; j < n_ang; ++j) {
       C d = xx - B * (R)z[j];                                  // u - y
-      C f = D1 * prop_diff<R>(P.line_pk, y, d);                // F_sub, eq. (20)
+      C f = P.routing == 1 ? fsub_symmetric<R>(P.line_pk, xx, y, B / (R)2, (R)z[j])
+                           : D1 * prop_diff<R>(P.line_pk, y, d);   // F_sub, eq. (20)
       sr += (ACC)((R)wz[j] * f.real());
       si += (ACC)((R)wz[j] * f.imag());
     }
@@ -510,6 +528,10 @@ int check_params(const Params& P, int n_rad, int n_ang) {
   if (P.contour < 0 || P.contour > 3) return 2;
   if (P.contour != CONTOUR_REAL && n_rad % 8 != 0) return 2;
   if (P.contour == CONTOUR_THREAD && !thread_applicable(P)) return 3;
+  if (P.routing != 0 && P.routing != 1) return 2;
+  if (P.routing == 1 && !(P.contour == CONTOUR_REAL && P.line_k.kind == PROP_MASSIVE && P.line_pk.kind == PROP_MASSIVE &&
+                          P.line_k.m2_re == P.line_pk.m2_re && P.line_k.m2_im == P.line_pk.m2_im))
+    return 3;
   if (!(P.dim == 0 || (P.dim >= 1 && P.dim <= 8))) return 2;
   if (!(P.dim == 0 || P.dim == 4) && P.contour != CONTOUR_REAL) return 3;
   return 0;

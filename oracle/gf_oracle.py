@@ -39,7 +39,7 @@ class _Params(ctypes.Structure):
                 ("sub_re", ctypes.c_double), ("sub_im", ctypes.c_double),
                 ("taylor_order", ctypes.c_int), ("prefactor", ctypes.c_double),
                 ("map_scale", ctypes.c_double), ("contour", ctypes.c_int),
-                ("precision", ctypes.c_int), ("dim", ctypes.c_double)]
+                ("precision", ctypes.c_int), ("routing", ctypes.c_int), ("dim", ctypes.c_double)]
 
 
 def build(force=False):
@@ -79,7 +79,7 @@ def _prop(d):
 
 
 def make_params(line_k, line_pk, cutoff2, prefactor=2.0 / np.pi, map_scale=1.0, contour="real",
-                sub=0.0, taylor_order=0, precision=64, dim=4.0):
+                sub=0.0, taylor_order=0, precision=64, dim=4.0, routing="paper"):
     P = _Params()
     P.line_k, P.line_pk = _prop(line_k), _prop(line_pk)
     P.cutoff2 = float(cutoff2)
@@ -91,6 +91,7 @@ def make_params(line_k, line_pk, cutoff2, prefactor=2.0 / np.pi, map_scale=1.0, 
     P.contour = CONTOUR[contour]
     P.precision = int(precision)
     P.dim = float(dim)
+    P.routing = {"paper": 0, "symmetric": 1}[routing]
     return P
 
 

@@ -525,3 +525,42 @@ def test_dimension_argument_checks(oracle):
     g4, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e4, dim=4.0), rn, rw, 64, z, wz, np.array([1.0 + 1j]))
     g0, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e4, dim=0.0), rn, rw, 64, z, wz, np.array([1.0 + 1j]))
     assert g4[0] == g0[0]
+
+
+# ---------------------------------------------------------------- symmetric momentum routing
+def test_symmetric_routing_reaches_the_threshold_parabola(oracle):
+    """Lines carrying k + p/2 and k - p/2 (shift invariance of eq. (4)): the same G as CF1 up to
+    O(x/Lambda^2), and the REAL contour is now the continuation inside the parabola through the physical threshold,
+    Re x > (Im x)^2/(16 m^2) - 4 m^2 -- including points next to the negative axis between -m^2 and -4 m^2 where the
+    paper's routing fails.  Catches a wrong sign of the b z terms, a missing x/4, a subtraction not at x = 0."""
+    n_rad, n_ang, cutoff2 = 512, 256, 1e8
+    rn, rw = oracle.make_quadrature("gauss_legendre", n_rad)
+    z, wz = oracle.make_quadrature("gauss_cheb2", n_ang, measure="sqrt1mz2")
+    inside = np.array([0.5 + 0.2j, 1 + 2j, -3 + 0.002j, -3.9 + 0.002j, -3.5 + 0.5j, 2 - 4j, 1e-7])
+    outside = np.array([-8 + 4j, -6 + 1j])
+    ref_in = np.array([complex(CF.cf1(x)) for x in inside])
+    ref_out = np.array([complex(CF.cf1(x)) for x in outside])
+    Ps = oracle.make_params(BUB, BUB, cutoff2, routing="symmetric")
+    g, _ = oracle.eval_grid(Ps, rn, rw, n_rad, z, wz, inside)
+    assert relerr(g, ref_in).max() < 2e-7            # O(x/Lambda^2) + quadrature
+    g, _ = oracle.eval_grid(Ps, rn, rw, n_rad, z, wz, outside)
+    assert relerr(g, ref_out).min() > 1e-2           # outside the parabola REAL is another function
+    # the paper's routing fails at the points between the two parabolas
+    Pp = oracle.make_params(BUB, BUB, cutoff2)
+    g, _ = oracle.eval_grid(Pp, rn, rw, n_rad, z, wz, inside[2:5])
+    assert relerr(g, ref_in[2:5]).min() > 1e-3
+    # invariants: G(0) = 0 exactly, conjugation symmetry bitwise
+    g0, _ = oracle.eval_grid(Ps, rn, rw, n_rad, z, wz, np.array([0.0]))
+    assert g0[0] == 0
+    a, _ = oracle.eval_grid(Ps, rn, rw, n_rad, z, wz, inside[:6])
+    b, _ = oracle.eval_grid(Ps, rn, rw, n_rad, z, wz, np.conj(inside[:6]))
+    assert np.array_equal(b, np.conj(a))
+
+
+def test_symmetric_routing_argument_checks(oracle):
+    rn, rw, z, wz = tables(oracle, 64, 32)
+    for kw in (dict(line_pk={"kind": "massive", "m2": 2.0}), dict(line_pk=RAT), dict(contour="ray_arc")):
+        args = dict(line_k=BUB, line_pk=BUB, cutoff2=1e4, routing="symmetric")
+        args.update(kw)
+        with pytest.raises(ValueError):
+            oracle.eval_grid(oracle.make_params(**args), rn, rw, 64, z, wz, np.array([1.0]))
