@@ -94,6 +94,11 @@ typedef struct {
   int contour;           /* gf_contour */
   int precision;         /* 64: complex<double> output (the contract); 32: the FP32 comparison
                             variant, complex<float> output */
+  int routing;           /* 0: the paper's eq. (19), the lines carry k and p - k.  1: symmetric, the lines carry
+                            k + p/2 and k - p/2 (the integral is shift invariant, eq. (4)): equal massive
+                            lines and the REAL contour only; G agrees up to O(x/Lambda^2), and REAL is the
+                            continuation inside the parabola through the threshold, Re x > (Im x)^2/(16 m^2) - 4 m^2,
+                            instead of Re x > (Im x)^2/(4 m^2) - m^2 */
   double dim;            /* space-time dimension d in [1, 8], 0 meaning 4 ("arbitrary dimensions by
                             trivial modifications"): the radial measure becomes dy y^((d-2)/2); the angular measure
                             (1-z^2)^((d-3)/2) is the caller's, in the angular weights (GF_MEASURE_PLAIN is d = 3).

@@ -37,7 +37,7 @@ class gf_params(ctypes.Structure):
     _fields_ = [("line_k", gf_propagator), ("line_pk", gf_propagator), ("cutoff2", ctypes.c_double),
                 ("sub_re", ctypes.c_double), ("sub_im", ctypes.c_double), ("taylor_order", ctypes.c_int),
                 ("prefactor", ctypes.c_double), ("map_scale", ctypes.c_double), ("contour", ctypes.c_int),
-                ("precision", ctypes.c_int), ("dim", ctypes.c_double)]
+                ("precision", ctypes.c_int), ("routing", ctypes.c_int), ("dim", ctypes.c_double)]
 
 
 class gf_launch_info(ctypes.Structure):
@@ -128,7 +128,7 @@ def _prop(d):
 
 
 def make_params(line_k, line_pk, cutoff2, prefactor=2.0 / np.pi, map_scale=1.0, contour="real", sub=0.0,
-                taylor_order=0, precision=64, dim=4.0):
+                taylor_order=0, precision=64, dim=4.0, routing="paper"):
     """gf_params from plain Python values.  Propagators: {'kind': 'massive', 'm2': complex} or
     {'kind': 'rational', 'M2': .., 'a': .., 'b': ..}."""
     P = gf_params()
@@ -142,6 +142,7 @@ def make_params(line_k, line_pk, cutoff2, prefactor=2.0 / np.pi, map_scale=1.0, 
     P.contour = CONTOUR[contour] if isinstance(contour, str) else int(contour)
     P.precision = int(precision)
     P.dim = float(dim)
+    P.routing = {"paper": 0, "symmetric": 1}[routing] if isinstance(routing, str) else int(routing)
     return P
 
 

@@ -95,6 +95,12 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   if (p->contour < GF_CONTOUR_REAL || p->contour > GF_CONTOUR_AUTO) { set_error("eval_grid: unknown contour %d", p->contour); return GF_ERR_ARG; }
   if (p->taylor_order != 0) { set_error("eval_grid: taylor_order %d unsupported (only t^0, eq. (13))", p->taylor_order); return GF_ERR_UNSUPPORTED; }
   if (p->sub_re != 0 || p->sub_im != 0) { set_error("eval_grid: subtraction point must be 0 (eq. (13))"); return GF_ERR_UNSUPPORTED; }
+  if (p->routing != 0 && p->routing != 1) { set_error("eval_grid: unknown routing %d", p->routing); return GF_ERR_ARG; }
+  if (p->routing == 1 && !(p->contour == GF_CONTOUR_REAL && p->line_k.kind == GF_PROP_MASSIVE && p->line_pk.kind == GF_PROP_MASSIVE &&
+                           p->line_k.m2_re == p->line_pk.m2_re && p->line_k.m2_im == p->line_pk.m2_im)) {
+    set_error("eval_grid: symmetric routing needs two equal massive lines and the REAL contour");
+    return GF_ERR_UNSUPPORTED;
+  }
   if (!(p->dim == 0 || (p->dim >= 1 && p->dim <= 8))) { set_error("eval_grid: dim=%g outside [1, 8] (0 = 4)", p->dim); return GF_ERR_ARG; }
   if (!(p->dim == 0 || p->dim == 4) && p->contour != GF_CONTOUR_REAL) { set_error("eval_grid: a dimension other than 4 is supported on the REAL contour only"); return GF_ERR_UNSUPPORTED; }
   if (p->contour != GF_CONTOUR_REAL && n_rad % 8 != 0) { set_error("eval_grid: deformed contours need n_rad %% 8 == 0"); return GF_ERR_ARG; }
@@ -111,6 +117,7 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   a->ypow = (p->dim == 0 || p->dim == 4) ? 1.0 : 0.5 * (p->dim - 2.0);
   log_ratio_dd(0.0, p->cutoff2, p->map_scale, &a->Llog_hi, &a->Llog_lo);  // REAL contour: [0, Lambda^2]
   a->contour = p->contour;
+  a->routing = p->routing;
   a->th5 = 0.75 * 3.14159265358979323846;  // 3 pi/4, correctly rounded
   a->cos_th5 = std::cos(a->th5);
   a->sin_th5 = std::sin(a->th5);
@@ -409,6 +416,7 @@ int gf_eval_angular(const gf_params* p, double x_re, double x_im, const double* 
   int rc = build_args(p, 8, n_ang, n_y, &a);   // the radial order plays no part
   if (rc) return rc;
   if (!std::isfinite(x_re) || !std::isfinite(x_im)) { set_error("eval_angular: x is not finite"); return GF_ERR_ARG; }
+  if (p->routing != 0) { set_error("eval_angular: defined for the paper's routing (eq. (22)) only"); return GF_ERR_UNSUPPORTED; }
   if (!d_ang_nodes || !d_ang_weights) { set_error("eval_angular: null table pointer"); return GF_ERR_NULL; }
   if (n_y > 0 && (!d_y || !d_out)) { set_error("eval_angular: null y/output pointer"); return GF_ERR_NULL; }
   a.ang_nodes = d_ang_nodes;
@@ -422,6 +430,7 @@ int gf_cut_crossings(const gf_params* p, const void* d_x, long long n_points, in
   EvalArgs a;
   int rc = build_args(p, 8, 2, n_points, &a);  // neither quadrature order plays a part
   if (rc) return rc;
+  if (p->routing != 0) { set_error("cut_crossings: defined for the paper's routing (eq. (23)-(25)) only"); return GF_ERR_UNSUPPORTED; }
   if (n_z < 2 || n_z > (1 << 24)) { set_error("cut_crossings: n_z=%d out of range [2, 2^24]", n_z); return GF_ERR_ARG; }
   if (n_points > 0 && (!d_x || !d_out)) { set_error("cut_crossings: null grid/output pointer"); return GF_ERR_NULL; }
   a.x = static_cast<const double2*>(d_x);

@@ -101,7 +101,9 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
       blob[L.off_y + ip] = y;
       blob[L.off_q4 + ip] = 0.25 / y;
       // radial measure dy y^((d-2)/2): y itself in d = 4 (eq. (14)), pow otherwise
-      const cd d1 = cscale(line_k_real(a.line_k, y), a.c0 * Wr * (a.ypow == 1.0 ? y : pow(y, a.ypow)));
+      // symmetric routing: D1 D2 at x = 0 is 1/(y + mu)^2 for both lines together (line_k == line_pk, massive)
+      const cd d1 = cscale(a.routing == 1 ? cinv(cd{y + a.term[0].mu_re, a.term[0].mu_im}) : line_k_real(a.line_k, y),
+                           a.c0 * Wr * (a.ypow == 1.0 ? y : pow(y, a.ypow)));
       for (int r = 0; r < a.n_terms; ++r) {
         const cd ic = cinv(cd{y + a.term[r].mu_re, a.term[r].mu_im});
         const cd pr = cmul(cmul(d1, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);
@@ -224,13 +226,30 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
   // zeta = (x + mu + y)^2/(4 x y) = C1/y + C2 + C3 y with C1 = (x + mu)^2/(4x), C2 = (x + mu)/(2x), C3 = 1/(4x):
   // four DFMA per node-term.  Its absolute error is an ulp of the largest of the three terms, which is O(1)
   // wherever zeta is O(1) (the EXACT route recomputes zeta in double-double from x, y, mu anyway).
-  cd xm[NT], C1x4[NT], C2[NT];  // x + mu_r, 4 C1 (multiplies 1/(4y)), C2
-  const cd C3 = cscale(xinv, 0.25);
+  // Symmetric routing (gf_params.routing = 1; lines carry k + p/2 and k - p/2, equal masses): the folded sum is
+  // the same S with  zeta' = (y + x/4 + mu)^2/(x y) = zeta(x/4, y, mu)  and  eta' = 1/2 + (2 mu + x/4)/(4y),
+  // and the node prefactor is -c0 Wr y/(y + mu)^2 (made in the preparation kernel).
+  cd xm[NT], C1x4[NT], C2[NT], dA[NT];  // x + mu_r, 4 C1 (multiplies 1/(4y)), C2, delta = d0 + dA/(4y)
+  cd C3 = cscale(xinv, 0.25);
+  cd xz = x;                            // the "x" of zeta (the EXACT route recomputes zeta from it)
+  double d0 = 0.0;
+  if (a.routing == 1) {
+    xz = cscale(x, 0.25);
+    C3 = xinv;                          // 1/(4 (x/4))
+    d0 = 0.25;
+  }
 #pragma unroll
   for (int r = 0; r < NT; ++r) {
     xm[r] = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
-    C2[r] = cscale(cmul(xm[r], xinv), 0.5);
-    C1x4[r] = cscale(cmul(xm[r], C2[r]), 2.0);
+    dA[r] = xm[r];
+    cd az = xm[r], izx2 = cscale(xinv, 0.5);   // a = xz + mu, 1/(2 xz)
+    if (a.routing == 1) {
+      az = {xz.re + a.term[r].mu_re, xz.im + a.term[r].mu_im};
+      izx2 = cscale(xinv, 2.0);
+      dA[r] = {xz.re + 2.0 * a.term[r].mu_re, xz.im + 2.0 * a.term[r].mu_im};
+    }
+    C2[r] = cmul(az, izx2);
+    C1x4[r] = cscale(cmul(az, C2[r]), 2.0);
   }
 
   // where the tail series takes over: the first node with y_i >= Y0 = 4 (sqrt|x| + sqrt(|x| + |x + mu|))^2
@@ -265,9 +284,9 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
     const bool on = i0 + sub < i_end;                // past its own i_end a lane idles with weight 0
 #pragma unroll
     for (int r = 0; r < NT; ++r) {
-      const cd delta = cscale(xm[r], q4);            // eta - 1/4
+      const cd delta = {fma(dA[r].re, q4, d0), dA[r].im * q4};   // eta - 1/4
       const cd zeta = {fma(C1x4[r].re, q4, fma(C3.re, y, C2[r].re)), fma(C1x4[r].im, q4, fma(C3.im, y, C2[r].im))};
-      const cd s = node_term<T, COUNT>(tb, x, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc);
+      const cd s = node_term<T, COUNT>(tb, xz, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc);
       double2 pr = ppref[r * L.n_rad_pad];
       if (!on) pr = make_double2(0.0, 0.0);
       g_re = fma(pr.x, s.re, fma(-pr.y, s.im, g_re));
@@ -348,7 +367,8 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   plan->split_log2 = sl;
   const long long threads = a.n_points << sl;
   plan->grid_blocks = (threads + kBlockThreads - 1) / kBlockThreads;
-  plan->layout = make_blob_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes, plan->shared_nodes);
+  plan->layout = make_blob_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes,
+                                 plan->shared_nodes && a.routing == 0);   // the tail series is derived for the paper's routing
   plan->smem_bytes = 16 + (size_t)plan->layout.n_doubles * sizeof(double);
   if (plan->smem_bytes > 200 * 1024) {
     set_error("eval_grid: tables need %zu bytes of shared memory (limit 200 KiB): reduce n_rad/n_ang",

@@ -40,6 +40,7 @@ struct EvalArgs {
   double Llog_hi, Llog_lo;  // ln((Lambda^2 + s0)/s0) as a double-double (host, binary128)
   double line2_scale;  // |m2^2| or the largest pole modulus: sizes the deformed contours
   int contour;         // gf_contour
+  int routing;         // 0: eq. (19) (lines k, p-k); 1: symmetric (lines k + p/2, k - p/2)
   int thread_ok;       // THREAD applicable (equal real masses)
   double th5, cos_th5, sin_th5;  // 3 pi/4 and its cos, sin as the host's libm rounds them (far waypoint of THREAD)
   int split_log2;      // lanes per grid point = 1 << split_log2

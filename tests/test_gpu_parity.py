@@ -524,3 +524,58 @@ def test_other_dimensions(gf, oracle, dim, measure):
     with pytest.raises(gf.GfError) as e:
         gf.eval_grid(Pd, rnp, rwp, cfg["n_rad"], z, wz, x)
     assert e.value.status == 3
+
+
+# ------------------------------------------------------------------ symmetric momentum routing
+def test_symmetric_routing(gf, oracle):
+    """Lines carrying k + p/2 and k - p/2: parity on config 1 (every point) and on a sample of config 2, the FP32
+    variant, complex equal masses; and the closed form CF1 next to the negative axis between -m^2 and -4 m^2,
+    where the paper's routing on the REAL contour is not the continuation."""
+    for name, stride in (("cfg1_tiny", 1), ("cfg2_mid", 8)):
+        cfg = W.CONFIGS[name]
+        rn, rw = gf.make_radial_tables("real", cfg["n_rad"], W.RADIAL_RULE)
+        z, wz = gf.make_quadrature(W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
+        rno, rwo = oracle.make_quadrature(W.RADIAL_RULE, cfg["n_rad"])
+        zo, wzo = oracle.make_quadrature(W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
+        x = gpu_grid(gf, cfg)[::stride, ::stride].contiguous()
+        for m2 in (1.0, 0.7 - 0.4j):
+            line = {"kind": "massive", "m2": m2}
+            P = gf.make_params(line, line, cfg["cutoff2"], routing="symmetric")
+            Po = oracle.make_params(line, line, cfg["cutoff2"], routing="symmetric")
+            g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
+            ref, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, x.cpu().numpy(), accum="extended")
+            assert relerr(g, ref).max() <= TOL64, (name, m2, relerr(g, ref).max())
+        P32 = gf.make_params(line, line, cfg["cutoff2"], routing="symmetric", precision=32)
+        g32 = gf.eval_grid(P32, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy().astype(np.complex128)
+        assert relerr(g32, ref).max() <= TOL32
+    # closed form where only the symmetric routing reaches it (Gauss rule of the measure for a tight check)
+    from tests import closed_forms as CF
+    bub = {"kind": "massive", "m2": 1.0}
+    rn, rw = gf.make_radial_tables("real", 512, W.RADIAL_RULE)
+    z, wz = gf.make_quadrature("gauss_cheb2", 256, measure="sqrt1mz2")
+    xs = np.array([-3 + 0.002j, -3.9 + 0.002j, -3.5 + 0.5j, -2.0 - 0.01j])
+    ref = np.array([complex(CF.cf1(v)) for v in xs])
+    gs = gf.eval_grid(gf.make_params(bub, bub, 1e8, routing="symmetric"), rn, rw, 512, z, wz,
+                      torch.from_numpy(xs).cuda()).cpu().numpy()
+    gp = gf.eval_grid(gf.make_params(bub, bub, 1e8), rn, rw, 512, z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+    assert relerr(gs, ref).max() < 2e-7 and relerr(gp, ref).min() > 1e-3
+
+
+def test_symmetric_routing_refuses_what_it_does_not_define(gf):
+    cfg = W.CONFIGS["cfg1_tiny"]
+    rn, rw = gf.make_radial_tables("auto", cfg["n_rad"], W.RADIAL_RULE)
+    z, wz = gf.make_quadrature(W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
+    x = gpu_grid(gf, cfg)
+    bub = {"kind": "massive", "m2": 1.0}
+    for kw in (dict(line_pk={"kind": "massive", "m2": 2.0}), dict(contour="auto"),
+               dict(line_pk={"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2})):
+        args = dict(line_k=bub, line_pk=bub, cutoff2=1e4, routing="symmetric")
+        args.update(kw)
+        with pytest.raises(gf.GfError) as e:
+            gf.eval_grid(gf.make_params(**args), rn, rw, cfg["n_rad"], z, wz, x)
+        assert e.value.status == 3
+    P = gf.make_params(bub, bub, 1e4, routing="symmetric")
+    with pytest.raises(gf.GfError):
+        gf.cut_crossings(P, x, 65)
+    with pytest.raises(gf.GfError):
+        gf.eval_angular(P, 1.0 + 1j, z, wz, x)
