@@ -86,7 +86,7 @@ typedef enum { GF_SPACING_UNIFORM = 0, GF_SPACING_LOG_ABS_IM = 1 } gf_spacing;
 typedef struct {
   gf_propagator line_k;  /* D1(y): the line carrying k      (eq. (19)) */
   gf_propagator line_pk; /* D2(u): the line carrying p - k */
-  double cutoff2;        /* Lambda^2 > 0, upper limit of the radial integral */
+  double cutoff2;        /* Lambda^2 in (0, 1e60], upper limit of the radial integral */
   double sub_re, sub_im; /* subtraction point x0 of t^n; only 0 is supported (eq. (13)) */
   int taylor_order;      /* n of t^n; only 0 is supported (log-divergent integrals) */
   double prefactor;      /* c0; 1/(2 pi)^3 is eq. (14), 2/pi the rescaled eq. (21) */

@@ -88,7 +88,7 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   if ((rc = check_prop(p->line_pk, "line_pk"))) return rc;
   if (n_rad < 1 || n_ang < 1) { set_error("eval_grid: n_rad=%d, n_ang=%d must be >= 1", n_rad, n_ang); return GF_ERR_ARG; }
   if (n_points < 0) { set_error("eval_grid: n_points < 0"); return GF_ERR_ARG; }
-  if (!(p->cutoff2 > 0) || !std::isfinite(p->cutoff2)) { set_error("eval_grid: cutoff2 must be > 0"); return GF_ERR_ARG; }
+  if (!(p->cutoff2 > 0) || !(p->cutoff2 <= 1e60)) { set_error("eval_grid: cutoff2 must be in (0, 1e60]"); return GF_ERR_ARG; }
   if (!(p->map_scale > 0) || !std::isfinite(p->map_scale)) { set_error("eval_grid: map_scale must be > 0"); return GF_ERR_ARG; }
   if (!std::isfinite(p->prefactor)) { set_error("eval_grid: prefactor not finite"); return GF_ERR_ARG; }
   if (p->precision != 64 && p->precision != 32) { set_error("eval_grid: precision must be 64 or 32"); return GF_ERR_ARG; }

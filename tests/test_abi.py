@@ -78,6 +78,15 @@ def test_argument_errors_without_gpu(gf):
     assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 3  # UNSUPPORTED
     P = gf.make_params(bub, bub, -1.0)
     assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 2
+    for bad in (dict(cutoff2=1e61), dict(cutoff2=1e4, dim=9.0), dict(cutoff2=1e4, routing=2)):
+        P = gf.make_params(bub, bub, **bad)
+        assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 2, bad
+    for unsupported in (dict(dim=3.0, contour="auto"), dict(routing="symmetric", contour="ray_arc")):
+        P = gf.make_params(bub, bub, 1e4, **unsupported)
+        assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 3, unsupported
+    assert gf.lib().gf_eval_workspace_size(ctypes.byref(gf.make_params(bub, bub, 1e4)), 64, 32) > 0
+    assert gf.lib().gf_eval_workspace_size(ctypes.byref(gf.make_params(bub, bub, 1e4)), 0, 32) == -1
+    assert gf.lib().gf_trim_scratch() == 0
     P = gf.make_params(bub, {"kind": "massive", "m2": 2.0}, 1e4, contour="thread")
     assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 3
     assert L.gf_make_grid(0.0, 1.0, 4, 0.0, 1.0, 4, 0, 0.0, None, None) == 1
