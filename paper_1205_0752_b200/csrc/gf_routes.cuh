@@ -380,13 +380,14 @@ __device__ __forceinline__ cd series_finish(const SeriesArg& o, cd delta, T p1, 
 
 // The direct loop for a lane on the NEAR or EXACT route
 template <typename T, bool COUNT>
-__device__ __forceinline__ cd direct_route(const Tabs<T>& tb, int route, cd x, cd y, cd delta, cd zeta, double mur,
-                                           double mui, RouteCount& rc) {
+__device__ __forceinline__ cd direct_route(const Tabs<T>& tb, int route, bool warp_has_exact, cd x, cd y, cd delta,
+                                           cd zeta, double mur, double mui, RouteCount& rc) {
   cd s;
   const cd eta = {__dadd_rn(0.25, delta.re), delta.im};
   bool dd_loop = true;
-  if (sizeof(T) == 8 && !__any_sync(__activemask(), route == ROUTE_EXACT)) {
-    // no EXACT lane among the lanes here: the 8-instruction pair (zeta in double is accurate enough for NEAR)
+  if (sizeof(T) == 8 && !warp_has_exact) {
+    // no EXACT lane in this warp (voted by all 32 lanes before the routes diverge, so the choice of loop does
+    // not depend on how the hardware groups the lanes): the 8-instruction pair
     s = angular_near<T>(eta, zeta, tb.mu0, tb.stT, tb.swT, tb.n_pairs);
     dd_loop = false;
   } else if (sizeof(T) == 8 || route == ROUTE_EXACT) {
@@ -411,6 +412,7 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
   const SeriesArg o = route_setup<T>(tb, zeta);
   const V2* tab = o.route == ROUTE_CHEB ? tb.cheb : tb.mom;
   int Kw = __reduce_max_sync(0xffffffffu, o.K);
+  const bool warp_has_exact = __any_sync(0xffffffffu, o.route == ROUTE_EXACT);
   Kw = min((Kw + 1) & ~1, tb.kmc);
   cd s = {0.0, 0.0};
   if (Kw > 0) {  // warp-uniform
@@ -419,7 +421,7 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
     if (COUNT) rc.series_exec += Kw;
     if (o.route <= ROUTE_CHEB) s = series_finish<T, COUNT>(o, delta, p1, p2, n1, n2, rc);
   }
-  if (o.route >= ROUTE_NEAR) s = direct_route<T, COUNT>(tb, o.route, x, y, delta, zeta, mur, mui, rc);
+  if (o.route >= ROUTE_NEAR) s = direct_route<T, COUNT>(tb, o.route, warp_has_exact, x, y, delta, zeta, mur, mui, rc);
   return s;
 }
 
