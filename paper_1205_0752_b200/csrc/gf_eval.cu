@@ -109,6 +109,12 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
         const cd pr = cmul(cmul(d1, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);
         blob[L.off_pref + 2 * (r * L.n_rad_pad + ip)] = pr.re;
         blob[L.off_pref + 2 * (r * L.n_rad_pad + ip) + 1] = pr.im;
+        if (L.n_pref > a.n_terms) {   // symmetric routing, tail table 1: pref (1 + mu/y)/4
+          const cd f = {0.25 + a.term[0].mu_re * (0.25 / y), a.term[0].mu_im * (0.25 / y)};
+          const cd p2 = cmul(pr, f);
+          blob[L.off_pref + 2 * (a.n_terms * L.n_rad_pad + ip)] = p2.re;
+          blob[L.off_pref + 2 * (a.n_terms * L.n_rad_pad + ip) + 1] = p2.im;
+        }
       }
     }
   }
@@ -259,7 +265,10 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
     double Y0 = 0.0;
 #pragma unroll
     for (int r = 0; r < NT; ++r) {
-      const double q = sqrt(ax) + sqrt(ax + sqrt(fma(xm[r].re, xm[r].re, xm[r].im * xm[r].im)));
+      // symmetric routing: zeta' = zeta(x/4, y, mu), the same bound with x/4 and a' = x/4 + mu
+      const cd az = {xz.re + a.term[r].mu_re, xz.im + a.term[r].mu_im};
+      const double axz = a.routing == 1 ? 0.25 * ax : ax;
+      const double q = sqrt(axz) + sqrt(axz + sqrt(fma(az.re, az.re, az.im * az.im)));
       Y0 = fmax(Y0, 4.0 * q * q);
     }
     int lo = 0, hi = a.n_rad;
@@ -298,7 +307,10 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
     const double2* R = reinterpret_cast<const double2*>(blob + L.off_tail) + (size_t)i_end * kTailN;
 #pragma unroll
     for (int r = 0; r < NT; ++r) {
-      const cd tl = tail_series(sb + L.off_gam, R + (size_t)r * (a.n_rad + 1) * kTailN, x, xm[r], invy0);
+      const cd az = {xz.re + a.term[r].mu_re, xz.im + a.term[r].mu_im};   // x + mu, or x/4 + mu
+      cd tl = tail_series(sb + L.off_gam, R + (size_t)r * (a.n_rad + 1) * kTailN, xz, az, invy0);
+      if (L.off_gam2 >= 0)   // symmetric routing: S' = S(x/4, a') + (1 + mu/y)/4 sum_j w_j/(zeta' - t_j)
+        tl = cadd(tl, tail_series(sb + L.off_gam2, R + (size_t)NT * (a.n_rad + 1) * kTailN, xz, az, invy0));
       if (sub == 0) {
         g_re += tl.re;
         g_im += tl.im;
@@ -324,7 +336,7 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
 
 }  // namespace
 
-BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail) {
+BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail, bool sym) {
   BlobLayout L;
   L.npad = (n_pairs + 3) & ~3;
   L.kmc = kKmc;
@@ -339,18 +351,20 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
   L.n_rad_pad = (n_rad + 31) & ~31;
   L.off_y = take(L.n_rad_pad);
   L.off_q4 = take(L.n_rad_pad);
-  L.off_pref = take(2 * n_terms * L.n_rad_pad);
+  L.n_pref = n_terms + (sym && tail ? 1 : 0);
+  L.off_pref = take(2 * L.n_pref * L.n_rad_pad);
   // 2 float tables of npad entries = npad doubles; 2 float2 tables of kmc entries = 2 kmc doubles
   L.off_f32 = f32 ? take(L.npad + 2 * L.kmc) : -1;
   L.n_tab = pyramid ? n_rad + n_rad / 2 + n_rad / 4 + n_rad / 8 : 0;
   L.off_rt = pyramid ? take(L.n_tab) : -1;
   L.off_rw = pyramid ? take(L.n_tab) : -1;
   L.off_gam = tail ? take(kTailN * (kTailN + 1) / 2) : -1;
+  L.off_gam2 = tail && sym ? take(kTailN * (kTailN + 1) / 2) : -1;
   L.n_doubles = o;
-  L.off_tail = tail ? take(2 * n_terms * (n_rad + 1) * kTailN) : -1;
+  L.off_tail = tail ? take(2 * L.n_pref * (n_rad + 1) * kTailN) : -1;
   L.off_scratch = take(L.kmc * L.npad);
   L.off_scratch2 = tail ? take(2 * kTailN * n_rad) : -1;
-  L.off_scratch3 = tail ? take(kTailN * n_rad + 2 * kTailChunks * (2 * n_terms * kTailN + kTailN)) : -1;
+  L.off_scratch3 = tail ? take(kTailN * n_rad + 2 * kTailChunks * (2 * L.n_pref * kTailN + kTailN)) : -1;
   L.n_total = o;
   return L;
 }
@@ -368,7 +382,7 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   const long long threads = a.n_points << sl;
   plan->grid_blocks = (threads + kBlockThreads - 1) / kBlockThreads;
   plan->layout = make_blob_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes,
-                                 plan->shared_nodes && a.routing == 0);   // the tail series is derived for the paper's routing
+                                 plan->shared_nodes, a.routing == 1);
   plan->smem_bytes = 16 + (size_t)plan->layout.n_doubles * sizeof(double);
   if (plan->smem_bytes > 200 * 1024) {
     set_error("eval_grid: tables need %zu bytes of shared memory (limit 200 KiB): reduce n_rad/n_ang",

@@ -56,12 +56,14 @@ struct BlobLayout {
   int off_kreq;                 // int Kreq[kKreqBins]: Chebyshev terms needed per bin of log2(rho)
   int n_rad_pad;                // n_rad rounded up to 32: padding repeats the last node with prefactor 0
   int off_y, off_q4;            // radial nodes y_i, 1/(4 y_i), n_rad_pad each
-  int off_pref;                 // double2 pref[n_terms][n_rad_pad]
+  int n_pref;                   // rows of node prefactors: n_terms, + 1 for the symmetric routing's second tail table
+  int off_pref;                 // double2 pref[n_pref][n_rad_pad]
   int off_f32;                  // FP32 variant: float t[npad], w[npad], float2 mom[kmc], cheb[kmc]; or -1
   int off_rt, off_rw, n_tab;    // point-dependent contours: the radial rule pyramid (nodes, weights) or -1
   int n_doubles;                // doubles every CTA stages (even)
   int off_gam;                  // tail series: gamma_{n,k}, row n = 1..kTailN at n(n-1)/2, staged; or -1 (no tail)
-  int off_tail;                 // NOT staged (global): double2 Rhat[n_terms][n_rad + 1][kTailN]
+  int off_gam2;                 // symmetric routing: kappa_{n,k} = mu_k C(n+k, n-1-k), same shape; or -1
+  int off_tail;                 // NOT staged (global): double2 Rhat[n_pref][n_rad + 1][kTailN]
   int off_scratch;              // preparation-only scratch: T_k(s_j) [npad][kmc]; tail: q_i^n (hi, lo) [kTailN][n_rad] x 2
   int off_scratch2;
   int off_scratch3;             // tail: Q_c(i) [kTailN][n_rad], run starts (double-double)
@@ -104,7 +106,8 @@ int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d
                       cudaStream_t stream);
 
 // gf_cut.cu: the paper's Kernels 3 and 4 (a.x holds the y array / the x array, a.out the result)
-BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail);  // gf_eval.cu
+BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail,
+                            bool sym = false);  // gf_eval.cu
 int launch_angular(const EvalArgs& a, double x_re, double x_im, cudaStream_t stream);
 int launch_cut_crossings(const EvalArgs& a, int n_z, int* d_out, cudaStream_t stream);
 

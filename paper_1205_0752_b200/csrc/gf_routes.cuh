@@ -638,6 +638,7 @@ __device__ void prep_tail_gamma(const BlobLayout& L, double* blob, dd (*s_part)[
     const dd t1 = dd_mul(s_nu[k], dd_binom(n + k, n - 1 - k));
     const dd t2 = dd_scale2(dd_mul(s_mu[k], dd_binom(n + k - 1, n - 2 - k)), 0.25);
     blob[L.off_gam + e] = dd_neg(dd_add(t1, t2)).hi;
+    if (L.off_gam2 >= 0) blob[L.off_gam2 + e] = dd_mul(s_mu[k], dd_binom(n + k, n - 1 - k)).hi;   // kappa_{n,k}
   }
 }
 // phase C: thread per node i: q_i^n, n = 1..kTailN, in double-double into the scratch (hi, lo) [n][i]
@@ -664,13 +665,13 @@ __device__ void prep_tail_sums(const EvalArgs& a, const BlobLayout& L, double* b
   const double* qhi = blob + L.off_scratch2;
   const double* qlo = qhi + (size_t)kTailN * a.n_rad;
   double2* R = reinterpret_cast<double2*>(blob + L.off_tail);
-  const int n_items = 2 * a.n_terms * kTailN, CL = (a.n_rad + kTailChunks - 1) / kTailChunks;
+  const int n_items = 2 * L.n_pref * kTailN, CL = (a.n_rad + kTailChunks - 1) / kTailChunks;
   double* Qs = blob + L.off_scratch3;                                   // Q_c(i), [kTailN][n_rad]
   dd* Lstart = reinterpret_cast<dd*>(Qs + (size_t)kTailN * a.n_rad);    // [n_items][kTailChunks]
   dd* Qstart = Lstart + (size_t)n_items * kTailChunks;                  // [kTailN][kTailChunks]
   for (int w = threadIdx.x; w < n_items * kTailChunks; w += blockDim.x) {
     const int e = w % n_items, c = w / n_items;
-    const int part = e / (a.n_terms * kTailN), r = (e / kTailN) % a.n_terms, n = e % kTailN;
+    const int part = e / (L.n_pref * kTailN), r = (e / kTailN) % L.n_pref, n = e % kTailN;
     double* Rr = reinterpret_cast<double*>(R + (size_t)r * (a.n_rad + 1) * kTailN) + part;
     const bool owner = r == 0 && part == 0;
     if (c == 0) Rr[2 * ((size_t)a.n_rad * kTailN + n)] = 0.0;
@@ -690,7 +691,7 @@ __device__ void prep_tail_sums(const EvalArgs& a, const BlobLayout& L, double* b
   __syncthreads();
   for (int w = threadIdx.x; w < n_items * kTailChunks; w += blockDim.x) {
     const int e = w % n_items, c = w / n_items;
-    const int part = e / (a.n_terms * kTailN), r = (e / kTailN) % a.n_terms, n = e % kTailN;
+    const int part = e / (L.n_pref * kTailN), r = (e / kTailN) % L.n_pref, n = e % kTailN;
     double* Rr = reinterpret_cast<double*>(R + (size_t)r * (a.n_rad + 1) * kTailN) + part;
     dd carry = {0.0, 0.0};
     for (int cc = kTailChunks - 1; cc > c; --cc)
