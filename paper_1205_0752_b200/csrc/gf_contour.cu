@@ -126,11 +126,11 @@ __device__ int build_contour(const EvalArgs& a, int pol, double xr, double xi, S
 
 // D1(y) for complex y
 __device__ __forceinline__ cd line_k_complex(const gf_propagator& p, cd y) {
-  if (p.kind == GF_PROP_MASSIVE) return cinv(cd{y.re + p.m2_re, y.im + p.m2_im});
+  if (p.kind == GF_PROP_MASSIVE) return cinv_fast(cd{y.re + p.m2_re, y.im + p.m2_im});
   const cd ya = {y.re + p.a, y.im};
   cd den = cmul(y, ya);
   den.re += p.b;
-  return cmul(cd{y.re + p.M2, y.im}, cinv(den));
+  return cmul(cd{y.re + p.M2, y.im}, cinv_fast(den));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -227,7 +227,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
         wy = {__dmul_rn(-y.im, f), __dmul_rn(y.re, f)};  // i y dtheta
       }
       if (mirror) { y.im = -y.im; wy.im = -wy.im; }
-      q4 = cscale(cinv(y), 0.25);
+      q4 = cscale(cinv_fast(y), 0.25);
     }
     cd base = {0.0, 0.0};
     if (!table) base = cscale(cmul(cmul(wy, y), line_k_complex(a.line_k, y)), a.c0);
@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
         const double2 p2 = spref[r * L.n_rad_pad + i];
         pr = {p2.x, p2.y};
       } else {
-        const cd ic = cinv(cd{y.re + mur, y.im + mui});
+        const cd ic = cinv_fast(cd{y.re + mur, y.im + mui});
         pr = cmul(cmul(base, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);
       }
       if (!valid) pr = {0.0, 0.0};

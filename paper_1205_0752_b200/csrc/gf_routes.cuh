@@ -90,6 +90,13 @@ __device__ __forceinline__ double rsqrt_fast(double s) {
   return fma(r0, e * fma(0.375, e, 0.5), r0);            // r0 (1 + e/2 + 3 e^2/8)
 }
 
+// 1/a per radial node on the deformed contours: |a|^2 stays far inside the exponent range there
+// (|y| <= Lambda^2 <= 1e60, and a node or y + mu exactly 0 gives inf/NaN as the header says)
+__device__ __forceinline__ cd cinv_fast(cd a) {
+  const double in = rcp_fast(fma(a.re, a.re, a.im * a.im));
+  return {a.re * in, -a.im * in};
+}
+
 // ---- 1-D TMA: one bulk copy global -> shared, completion on an mbarrier ------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
