@@ -24,6 +24,10 @@ constexpr float kSeriesBits = GF_SERIES_BITS;    // series are cut where the dro
 #define GF_GOERTZEL_UNROLL 2
 #endif
 constexpr int kGoertzelUnroll = GF_GOERTZEL_UNROLL;   // trips of the series loop (2 terms each) unrolled
+#ifndef GF_NEAR_UNROLL
+#define GF_NEAR_UNROLL 1
+#endif
+constexpr int kNearUnroll = GF_NEAR_UNROLL;           // trips of the plain direct loop (4 pairs each) unrolled
 constexpr double kMomentMin = 4.5;    // MOMENT route when max(|Re zeta|, |Im zeta|) >= this: |zeta - 1/2| >= 4
 constexpr double kTau64 = 0x1p-8;     // EXACT route inside this distance of [0,1] (FP64)
 constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only good further away
@@ -202,7 +206,7 @@ __device__ __forceinline__ cd angular_near(cd eta, cd zeta, double mu0, const T*
   const T zi2 = (T)(zeta.im * zeta.im);
   T a0 = 0, a1 = 0, b0 = 0, b1 = 0;
   int j = 0;
-#pragma unroll 1
+#pragma unroll(kNearUnroll)
   for (; j + 4 <= n_pairs; j += 4) {
     const V2 t01 = *reinterpret_cast<const V2*>(st + j), t23 = *reinterpret_cast<const V2*>(st + j + 2);
     const V2 w01 = *reinterpret_cast<const V2*>(sw + j), w23 = *reinterpret_cast<const V2*>(sw + j + 2);
