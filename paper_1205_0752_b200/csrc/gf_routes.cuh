@@ -31,9 +31,6 @@ constexpr int kNearUnroll = GF_NEAR_UNROLL;           // trips of the plain dire
 constexpr double kMomentMin = 4.5;    // MOMENT route when max(|Re zeta|, |Im zeta|) >= this: |zeta - 1/2| >= 4
 constexpr double kTau64 = 0x1p-8;     // EXACT route inside this distance of [0,1] (FP64)
 constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only good further away
-// FP64-pipe instructions of the per-node code of each route (set-up + finish), used to pick the cheaper of
-// CHEB and NEAR; they only steer the choice, any value gives the same sum
-constexpr int kChebNodeCost = 76, kNearNodeCost = 24;
 // Kreq table: bins of log2(rho) from kEllLo in steps of kEllStep (the lower edge of a bin decides, so K is safe)
 constexpr float kEllLo = 0.235f, kEllStep = 0.02f;
 
@@ -366,7 +363,10 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     const double g2 = rm + rm;                   // 4/sqrt(w^2-1) = 2 conj(root)/|q|
     o.g = {ar * g2, -ai * g2};
     o.route = ROUTE_CHEB;
-    if (!(o.K <= tb.kmc && 4 * o.K + kChebNodeCost < 8 * tb.n_pairs + kNearNodeCost)) {
+    // CHEB whenever its series is short enough, whatever the direct loop would cost: next to [0,1] S is O(1), but
+    // further out S can be 1e-7 of mu0 (the rule nearly integrates eta - t to zero) and the direct form
+    // mu0 + (eta - zeta) C(zeta) would lose those digits; the series carry that cancellation in their tables
+    if (!(o.K <= tb.kmc)) {
       o.K = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
       o.route = (zeta.im * zeta.im < tb.tau * tb.tau && zeta.re > -tb.tau && zeta.re < 1.0 + tb.tau) ? ROUTE_EXACT
                                                                                                      : ROUTE_NEAR;
