@@ -138,7 +138,7 @@ def oracle_step(cfg, xs):
     return time.perf_counter() - t, used
 
 
-def cpu_baseline(cfg, stride=8):
+def cpu_baseline(cfg, stride=4):
     xs = oracle_sample(cfg, stride)
     dt, used = oracle_step(cfg, xs)
     return {"value": xs.size / dt, "unit": UNIT, "cores": used, "kind": "oracle",
