@@ -28,7 +28,8 @@ constexpr int kGoertzelUnroll = GF_GOERTZEL_UNROLL;   // trips of the series loo
 #define GF_NEAR_UNROLL 1
 #endif
 constexpr int kNearUnroll = GF_NEAR_UNROLL;           // trips of the plain direct loop (4 pairs each) unrolled
-constexpr double kMomentMin = 4.5;    // MOMENT route when max(|Re zeta|, |Im zeta|) >= this: |zeta - 1/2| >= 4
+// MOMENT route when max(|Re zeta|, |Im zeta|) >= 4.5 (then |zeta - 1/2| >= 4); the value is written out in
+// route_setup as the high word 0x40120000
 constexpr double kTau64 = 0x1p-8;     // EXACT route inside this distance of [0,1] (FP64)
 constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only good further away
 // Kreq table: bins of log2(rho) from kEllLo in steps of kEllStep (the lower edge of a bin decides, so K is safe)
@@ -329,7 +330,9 @@ struct SeriesArg {
 template <typename T>
 __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
   SeriesArg o;
-  if (fabs(zeta.re) >= kMomentMin || fabs(zeta.im) >= kMomentMin) {
+  // |Re zeta| or |Im zeta| >= 4.5, compared on the high words (4.5 = 0x40120000'00000000) to keep the test off the
+  // FP64 pipe; a NaN lands here too and stays a NaN
+  if (max(__double2hiint(zeta.re) & 0x7fffffff, __double2hiint(zeta.im) & 0x7fffffff) >= 0x40120000) {
     o.route = ROUTE_MOMENT;
     const double zc = zeta.re - 0.5;
     const double in = rcp_fast(fma(zc, zc, zeta.im * zeta.im));   // |zeta| < 2^500 (gf.h: domain)
@@ -347,9 +350,13 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     const double h2 = 0.5 * fma(n2, rm, fabs(qr));
     const double rh = rsqrt_fast(h2);
     const double h = h2 * rh, kk = 0.5 * qi * rh;
-    double ar = qr >= 0.0 ? h : fabs(kk);
-    double ai = qr >= 0.0 ? kk : copysign(h, qi);
-    if (fma(wr, ar, wi * ai) < 0.0) { ar = -ar; ai = -ai; }
+    // signs by integer operations on the high words (sign tests and negations would take FP64-pipe slots)
+    const bool qpos = __double2hiint(qr) >= 0;
+    double ar = qpos ? h : fabs(kk);
+    double ai = qpos ? kk : copysign(h, qi);
+    const int flip = __double2hiint(fma(wr, ar, wi * ai)) & 0x80000000;   // Re(conj(w) root) < 0: the other root
+    ar = __hiloint2double(__double2hiint(ar) ^ flip, __double2loint(ar));
+    ai = __hiloint2double(__double2hiint(ai) ^ flip, __double2loint(ai));
     const double Dr = fma(2.0, ar, wr), Di = fma(2.0, ai, wi);
     const double rho2 = fma(Dr, Dr, Di * Di);
     // terms needed at this rho (table made from the coefficients themselves, prep_series_kreq); taken from rho^2
