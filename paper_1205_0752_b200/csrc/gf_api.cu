@@ -453,7 +453,7 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
   out->series_terms_max = plan.layout.kmc;
   out->evals = (double)n_points * n_rad * n_ang;
   // FP64-pipe instructions per unit of each route, counted per SASS region in the ncu source page of
-  // eval_real_kernel<double, false, 1> (profiles/r01g_eval_ncu_full.md; DSETP not counted: no flops):
+  // eval_real_kernel<double, false, 1> (profiles/r01h_eval_ncu_full.md; DSETP not counted: no flops):
   //   pair of the plain direct loop 5 DFMA + 1 DMUL + 2 DADD, of the double-double loop 5 + 1 + 4;
   //   series term (P and N): 4 DFMA;
   //   every node-term: zeta, delta (5 DFMA + 3 DMUL + 1 DADD) and the accumulation into G (4 DFMA);
