@@ -180,7 +180,10 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
  * which for a massive line 2 is eq. (22)'s  int dz sqrt(1-z^2) (-x + 2 sqrt(x) sqrt(y) z)/(u + m2^2).  Only
  * p->line_pk is used (line_k, cutoff2, contour play no part but must be valid); the angular rule as in
  * gf_eval_grid.  d_out: n_y complex<double>.  x = 0 gives exactly 0; y = 0 is the limit value; where 4 x y
- * overflows or underflows the entry is IEEE inf/NaN.  FP64 only.  Asynchronous on `stream`. */
+ * overflows or underflows the entry is IEEE inf/NaN.  Accuracy: 1e-11 relative where |B| is of the order of the sum
+ * of the weights; where B is small by cancellation (|x|, |y| >> |m2|: the rule nearly integrates the numerator to
+ * zero) the error is absolute, about 1e-14 of the sum of the weights (2e-10 relative was the worst of 8 000 random
+ * (x, y, line 2, rule) against the oracle in binary128).  FP64 only.  Asynchronous on `stream`. */
 int gf_eval_angular(const gf_params* p, double x_re, double x_im, const double* d_ang_nodes,
                     const double* d_ang_weights, int n_ang, const void* d_y, long long n_y, void* d_out, void* stream);
 
