@@ -347,15 +347,16 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
 
   // x in, kernel, G out as a pipeline of chunks: copies in both directions overlap the evaluation
   // (pinned host buffers; with pageable ones the copies serialise but the result is the same)
-  const int kMaxChunks = 4;
+  const int kMaxChunks = 8;
   const long long min_chunk = 1 << 18;
   int n_chunks = (int)std::min<long long>(kMaxChunks, std::max<long long>(1, n_points / min_chunk));
-  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaStream_t s_in = nullptr, s_out = nullptr, s_k2 = nullptr;   // copies in / out, second compute stream
   cudaEvent_t ev_ready = nullptr, ev_in[kMaxChunks] = {}, ev_k[kMaxChunks] = {}, ev_done = nullptr;
   auto ok = [&](cudaError_t err, const char* what) { if (!rc) rc = check_cuda(err, what); };
   if (!rc && n_chunks > 1) {
     ok(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking), "cudaStreamCreate");
     ok(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking), "cudaStreamCreate");
+    ok(cudaStreamCreateWithFlags(&s_k2, cudaStreamNonBlocking), "cudaStreamCreate");
     ok(cudaEventCreateWithFlags(&ev_ready, cudaEventDisableTiming), "cudaEventCreate");
     ok(cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming), "cudaEventCreate");
     for (int c = 0; c < n_chunks; ++c) {
@@ -366,6 +367,7 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
       ok(cudaEventRecord(ev_ready, s), "cudaEventRecord");          // the scratch exists in stream order of s
       ok(cudaStreamWaitEvent(s_in, ev_ready, 0), "cudaStreamWaitEvent");
       ok(cudaStreamWaitEvent(s_out, ev_ready, 0), "cudaStreamWaitEvent");
+      ok(cudaStreamWaitEvent(s_k2, ev_ready, 0), "cudaStreamWaitEvent");
     }
   }
   for (int c = 0; c < n_chunks && !rc; ++c) {
@@ -373,21 +375,23 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
     // so the chunked result is bit-identical to gf_eval_grid's (the series loop runs to the warp's longest series)
     auto cut = [&](int k) { return k >= n_chunks ? n_points : (n_points * k / n_chunks) & ~(long long)(kBlockThreads - 1); };
     const long long p0 = cut(c), p1 = cut(c + 1), np = p1 - p0;
-    cudaStream_t sin = n_chunks > 1 ? s_in : s, sout = n_chunks > 1 ? s_out : s;
+    // odd chunks are evaluated on a second stream, so that the last, partly filled wave of CTAs of one chunk
+    // overlaps the first waves of the next
+    cudaStream_t sin = n_chunks > 1 ? s_in : s, sout = n_chunks > 1 ? s_out : s, sk = (c & 1) ? s_k2 : s;
     ok(cudaMemcpyAsync(d + off_x + (size_t)p0 * 16, static_cast<const char*>(h_x) + (size_t)p0 * 16, (size_t)np * 16,
                        cudaMemcpyHostToDevice, sin), "host->device copy (x)");
     if (n_chunks > 1) {
       ok(cudaEventRecord(ev_in[c], s_in), "cudaEventRecord");
-      ok(cudaStreamWaitEvent(s, ev_in[c], 0), "cudaStreamWaitEvent");
+      ok(cudaStreamWaitEvent(sk, ev_in[c], 0), "cudaStreamWaitEvent");
     }
     if (!rc) {
       a.x = reinterpret_cast<const double2*>(d + off_x) + p0;
       a.out = d + off_out + (size_t)p0 * out_elem;
       a.n_points = np;
-      rc = launch_prepared(a, p->precision, d_ws, nullptr, s);
+      rc = launch_prepared(a, p->precision, d_ws, nullptr, sk);
     }
     if (n_chunks > 1) {
-      ok(cudaEventRecord(ev_k[c], s), "cudaEventRecord");
+      ok(cudaEventRecord(ev_k[c], sk), "cudaEventRecord");
       ok(cudaStreamWaitEvent(s_out, ev_k[c], 0), "cudaStreamWaitEvent");
     }
     ok(cudaMemcpyAsync(static_cast<char*>(h_out) + (size_t)p0 * out_elem, d + off_out + (size_t)p0 * out_elem,
@@ -401,6 +405,7 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
   int rc2 = check_cuda(cudaStreamSynchronize(s), "stream synchronize");
   if (s_in) { cudaStreamSynchronize(s_in); cudaStreamDestroy(s_in); }
   if (s_out) { cudaStreamSynchronize(s_out); cudaStreamDestroy(s_out); }
+  if (s_k2) { cudaStreamSynchronize(s_k2); cudaStreamDestroy(s_k2); }
   if (ev_ready) cudaEventDestroy(ev_ready);
   if (ev_done) cudaEventDestroy(ev_done);
   for (int c = 0; c < kMaxChunks; ++c) {
