@@ -28,9 +28,11 @@
  *     the real axis, Fortran order).
  *   - Errors: GF_ERR_NULL for a null pointer, GF_ERR_ARG for a value out of range,
  *     GF_ERR_UNSUPPORTED for a combination the method does not define (taylor_order != 0, a
- *     subtraction point other than 0, a dimension other than 4 on a deformed contour, the THREAD contour with unequal or complex masses, a
- *     rational propagator with a double pole, precision 32 on a contour other than REAL), GF_ERR_CUDA when the CUDA runtime reports an
- *     error (no device, launch failure).  gf_last_error() describes the last failure of the
+ *     subtraction point other than 0, a dimension other than 4 or the symmetric routing on a
+ *     deformed contour, the symmetric routing with unequal or rational lines, the THREAD contour
+ *     with unequal or complex masses, a rational propagator with a double pole, precision 32 on a
+ *     contour other than REAL), GF_ERR_CUDA when the CUDA runtime reports an error (no device,
+ *     launch failure).  gf_last_error() describes the last failure of the
  *     calling thread.  A denominator that vanishes at a quadrature node yields IEEE inf/NaN in
  *     that output entry, not an error (the paper has no convention).
  */
