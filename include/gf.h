@@ -240,9 +240,13 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
  * gf_diag_fp64_peak: enqueue a kernel of `blocks` x `threads` threads, each running `iters` rounds of 8
  *   independent DFMA chains (16*iters flops per thread per round... see DESIGN.md); writes one double
  *   per thread to d_sink (blocks*threads doubles) so the work cannot be removed.
- * gf_diag_rcp_seed: for n doubles in d_in, writes the raw MUFU.RCP64H seed to d_out. */
+ * gf_diag_dfma_issue: the same launch shape and sink, 8 DFMA per thread and round as well, with the operand pattern
+ *   `mode` selects: 0 one varying register pair per DFMA (a = fma(a, m, c), m and c loop-invariant), 1 two varying
+ *   pairs, 2 three varying pairs (a_j = fma(a_j, b_j, c_j)), 3 the second-order recurrence of the series routes
+ *   (t = fma(ns, p2, c); p2 = fma(r, p1, t)) on four chains.  The ratio of the measured times is the issue cadence
+ *   of each pattern relative to the peak stream. */
 int gf_diag_fp64_peak(int blocks, int threads, long long iters, double* d_sink, void* stream);
-int gf_diag_rcp_seed(const double* d_in, double* d_out, long long n, void* stream);
+int gf_diag_dfma_issue(int mode, int blocks, int threads, long long iters, double* d_sink, void* stream);
 /* The radial nodes y_i = s0 expm1(u_i L), u_i = (t_i + 1)/2, L = ln((cutoff2 + s0)/s0), of the REAL contour
  * exactly as the evaluation kernel makes them (double-double, correctly rounded), for the n rule nodes in
  * d_nodes; tests compare them bit for bit with the oracle's. */
@@ -253,6 +257,9 @@ int gf_trim_scratch(void);
 
 const char* gf_last_error(void);
 const char* gf_version(void);
+/* Hash of the sources this binary was compiled from (paper_1205_0752_b200/build.py source_id()); the Python binding
+ * refuses a library whose id differs from that of the sources beside it.  "" when built by other means. */
+const char* gf_build_id(void);
 
 #ifdef __cplusplus
 }

@@ -73,11 +73,12 @@ _SIGNATURES = {
     "gf_cut_crossings": [ctypes.POINTER(gf_params), _vp, _ll, _int, _vp, _vp],
     "gf_eval_launch_info": [ctypes.POINTER(gf_params), _int, _int, _ll, ctypes.POINTER(gf_launch_info)],
     "gf_diag_fp64_peak": [_int, _int, _ll, _vp, _vp],
-    "gf_diag_rcp_seed": [_vp, _vp, _ll, _vp],
+    "gf_diag_dfma_issue": [_int, _int, _int, _ll, _vp, _vp],
     "gf_diag_radial_map": [_dbl, _dbl, _vp, _int, _vp, _vp],
     "gf_trim_scratch": [],
     "gf_last_error": [],
     "gf_version": [],
+    "gf_build_id": [],
 }
 
 
@@ -88,6 +89,10 @@ def lib():
         if not os.path.exists(LIB_PATH):
             raise RuntimeError("libgf_b200.so is missing: run `python -m paper_1205_0752_b200.build` "
                                "(nvcc, sm_100a).  There is no CPU fallback.")
+        from . import build as _build
+        if os.path.isdir(_build.CSRC) and _build.stale():
+            raise RuntimeError("libgf_b200.so was not built from the sources beside it (build id %r, sources %r): "
+                               "run `python -m paper_1205_0752_b200.build`" % (_build.built_id(), _build.source_id()))
         L = ctypes.CDLL(LIB_PATH)
         for name, args in _SIGNATURES.items():
             f = getattr(L, name)
@@ -97,6 +102,7 @@ def lib():
         L.gf_eval_workspace_size.restype = _ll
         L.gf_last_error.restype = ctypes.c_char_p
         L.gf_version.restype = ctypes.c_char_p
+        L.gf_build_id.restype = ctypes.c_char_p
         _lib = L
     return _lib
 
@@ -356,10 +362,8 @@ def diag_radial_map(cutoff2, map_scale, nodes, stream=None):
     return y
 
 
-def diag_rcp_seed(x, stream=None):
-    out = torch.empty_like(x)
-    _check(lib().gf_diag_rcp_seed(x.data_ptr(), out.data_ptr(), x.numel(), _stream(stream)))
-    return out
+def diag_dfma_issue(mode, blocks, threads, iters, sink, stream=None):
+    _check(lib().gf_diag_dfma_issue(mode, blocks, threads, iters, sink.data_ptr(), _stream(stream)))
 
 
 def trim_scratch():

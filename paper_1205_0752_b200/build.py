@@ -2,6 +2,7 @@
 
     python -m paper_1205_0752_b200.build [--force]
 """
+import hashlib
 import os
 import subprocess
 import sys
@@ -23,19 +24,41 @@ def _nvcc():
     return "nvcc"
 
 
-def stale():
+def source_id():
+    """Hash of every source and header the library is built from (and of the flags): compiled into the library as
+    gf_build_id(), so that a binary that does not belong to the sources beside it is refused at load time (file
+    times do not survive the copy to the GPU box; contents do)."""
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    for d in [os.path.join(CSRC, s) for s in SOURCES] + HEADERS:
+        h.update(os.path.basename(d).encode())
+        with open(d, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def built_id():
+    """The source hash recorded in the built library ('' if there is none or it predates gf_build_id)."""
     if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS
-    return any(os.path.getmtime(d) > t for d in deps)
+        return ""
+    import ctypes
+    try:
+        f = ctypes.CDLL(LIB).gf_build_id
+    except (OSError, AttributeError):
+        return ""
+    f.restype = ctypes.c_char_p
+    return f().decode()
+
+
+def stale():
+    return built_id() != source_id()
 
 
 def build(force=False, verbose=False):
     """Compile every CUDA source of the package into paper_1205_0752_b200/libgf_b200.so."""
     if not force and not stale():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("GF_NVCC_EXTRA", "").split() + ["-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB]
+    cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("GF_NVCC_EXTRA", "").split() + [
+        "-DGF_BUILD_ID=\"%s\"" % source_id(), "-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB]
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-lquadmath"]

@@ -181,7 +181,11 @@ int gf_trim_scratch(void) {
   return rc;
 }
 
-const char* gf_version(void) { return "gf_b200 0.1 (sm_100a)"; }
+const char* gf_version(void) { return "gf_b200 0.2 (sm_100a)"; }
+#ifndef GF_BUILD_ID
+#define GF_BUILD_ID ""
+#endif
+const char* gf_build_id(void) { return GF_BUILD_ID; }
 
 static int make_grid_rows(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,
                           int spacing, double im_abs_min, int row_first, int n_rows, void* d_x, void* stream) {
@@ -491,11 +495,10 @@ int gf_diag_radial_map(double cutoff2, double map_scale, const double* d_nodes, 
   return launch_radial_map(hi, lo, map_scale, d_nodes, n, d_y, static_cast<cudaStream_t>(stream));
 }
 
-int gf_diag_rcp_seed(const double* d_in, double* d_out, long long n, void* stream) {
-  if (!d_in || !d_out) { set_error("diag_rcp_seed: null pointer"); return GF_ERR_NULL; }
-  if (n < 0) { set_error("diag_rcp_seed: n < 0"); return GF_ERR_ARG; }
-  if (n == 0) return GF_OK;
-  return launch_rcp_seed(d_in, d_out, n, static_cast<cudaStream_t>(stream));
+int gf_diag_dfma_issue(int mode, int blocks, int threads, long long iters, double* d_sink, void* stream) {
+  if (!d_sink) { set_error("diag_dfma_issue: d_sink is null"); return GF_ERR_NULL; }
+  if (mode < 0 || mode > 3 || blocks < 1 || threads < 1 || threads > 1024 || iters < 0) { set_error("diag_dfma_issue: bad mode or launch shape"); return GF_ERR_ARG; }
+  return launch_dfma_issue(mode, blocks, threads, iters, d_sink, static_cast<cudaStream_t>(stream));
 }
 
 }  // extern "C"

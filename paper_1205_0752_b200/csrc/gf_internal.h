@@ -113,6 +113,6 @@ int launch_cut_crossings(const EvalArgs& a, int n_z, int* d_out, cudaStream_t st
 
 // gf_diag.cu
 int launch_fp64_peak(int blocks, int threads, long long iters, double* d_sink, cudaStream_t stream);
-int launch_rcp_seed(const double* d_in, double* d_out, long long n, cudaStream_t stream);
+int launch_dfma_issue(int mode, int blocks, int threads, long long iters, double* d_sink, cudaStream_t stream);
 
 }  // namespace gf
