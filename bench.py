@@ -128,11 +128,13 @@ def oracle_sample(cfg, stride):
 
 def oracle_step(cfg, xs):
     """One pass of the oracle over the sample: its own tables, then the triple loop (double accumulation,
-    the timed variant of oracle/gf_oracle.cpp).  Returns (seconds, threads used)."""
+    the timed variant of oracle/gf_oracle.cpp).  Returns (seconds, threads used, values)."""
     from oracle import gf_oracle as O
     t = time.perf_counter()
-    P = O.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE)
-    rn, rw = O.make_quadrature(W.RADIAL_RULE, cfg["n_rad"])
+    contour = cfg.get("contour", "real")
+    P = O.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
+                      contour=contour)
+    rn, rw = O.make_radial_pyramid(cfg["n_rad"], levels=1 if contour == "real" else 4, kind=W.RADIAL_RULE)
     z, wz = O.make_quadrature(W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
     g, used = O.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, xs, accum="double")
     return time.perf_counter() - t, used, g
@@ -168,7 +170,7 @@ def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return 0
-    cfg = dict(W.CONFIGS[args.workload], name=args.workload)
+    cfg = dict(W.CONFIGS[args.workload], name=args.workload, contour=args.contour)
     stride = 16
     from oracle import gf_oracle as O
     O.build()
@@ -197,13 +199,19 @@ def run_reference(args):
 
 
 def workload_config(cfg, world, rows_per_rank):
-    return {"workload": "%s: bubble m=1 once-subtracted at p^2=0, %dx%d grid over Re[%g,%g] Im[%g,%g], "
-                        "%d radial x %d angular Gauss-Legendre nodes, cutoff %g, REAL contour, complex128"
-                        % (cfg["name"], cfg["n_re"], rows_per_rank * world, cfg["re"][0], cfg["re"][1], cfg["im"][0],
-                           cfg["im"][1], cfg["n_rad"], cfg["n_ang"], cfg["cutoff2"]),
+    def line(p):
+        return ("1/(q^2+%g)" % p["m2"]) if p["kind"] == "massive" else "(q^2+%g)/(q^4+%g q^2+%g)" % (p["M2"], p["a"], p["b"])
+    return {"workload": "%s: lines %s and %s, once-subtracted at p^2=0, %dx%d grid over Re[%g,%g] Im[%g,%g]%s, "
+                        "%d radial x %d angular Gauss-Legendre nodes, cutoff %g, %s contour, complex128"
+                        % (cfg["name"], line(cfg["line_k"]), line(cfg["line_pk"]), cfg["n_re"], rows_per_rank * world,
+                           cfg["re"][0], cfg["re"][1], cfg["im"][0], cfg["im"][1],
+                           " (log-spaced |Im|)" if cfg["spacing"] != "uniform" else "", cfg["n_rad"], cfg["n_ang"],
+                           cfg["cutoff2"], cfg.get("contour", "real").upper()),
             "n_points": cfg["n_re"] * rows_per_rank * world, "n_rad": cfg["n_rad"], "n_ang": cfg["n_ang"],
+            "contour": cfg.get("contour", "real"),
             "parallelism": "rows x%d, no collective" % world,
-            "cache": "L2 flushed between steps (256 MiB write); x + G = 128 MiB per rank"}
+            "cache": "L2 flushed between steps (256 MiB write); x + G = %d MiB per rank"
+                     % (cfg["n_re"] * rows_per_rank * 32 >> 20)}
 
 
 # ------------------------------------------------------------------------------------- the CUDA arm
@@ -222,12 +230,14 @@ def run_ours(args):
 
     cfg = workload_for(args.workload, world)
     cfg["name"] = args.workload
+    cfg["contour"] = args.contour
     n_re, n_rows, n_rad, n_ang = cfg["n_re"], cfg["n_im"], cfg["n_rad"], cfg["n_ang"]
     row_first, rows_local = W.row_partition(cfg["n_im_global"], world, rank)
     assert rows_local == n_rows
     n_points_local = n_re * rows_local
+    contour = args.contour
     P = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
-                       contour="real", precision=64)
+                       contour=contour, precision=64)
     info = gf.launch_info(P, n_rad, n_ang, n_points_local)
 
     x = torch.empty((rows_local, n_re), dtype=torch.complex128, device=dev)
@@ -238,7 +248,7 @@ def run_ours(args):
     ev_k1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
 
     def step(k=None):
-        rn, rw = gf.make_radial_tables("real", n_rad, W.RADIAL_RULE)                    # a2
+        rn, rw = gf.make_radial_tables(contour, n_rad, W.RADIAL_RULE)                   # a2
         z, wz = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")           # a2
         gf.make_grid_rows(cfg["re"][0], cfg["re"][1], n_re, cfg["im"][0], cfg["im"][1], cfg["n_im_global"],
                           row_first, rows_local, spacing=cfg["spacing"], im_abs_min=cfg["im_abs_min"], out=x)  # a1
@@ -280,7 +290,7 @@ def run_ours(args):
 
     # ---- executed FP64 work of one launch: the kernel's own route counters (an untimed, counted launch
     #      with identical results) x the per-unit instruction counts of the SASS (gf_eval_launch_info)
-    rn_c, rw_c = gf.make_radial_tables("real", n_rad, W.RADIAL_RULE)
+    rn_c, rw_c = gf.make_radial_tables(contour, n_rad, W.RADIAL_RULE)
     z_c, wz_c = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
     out_c, counters = gf.eval_grid_counted(P, rn_c, rw_c, n_rad, z_c, wz_c, x)
     assert torch.equal(out_c.view(torch.float64), out.view(torch.float64)), "counted launch differs"
@@ -288,28 +298,30 @@ def run_ours(args):
     del out_c
 
     # ---- the FP32 comparison variant on the same scan (BASELINE.json configs[2]): untimed for `value`, own events
-    P32 = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
-                         contour="real", precision=32)
-    ws32 = gf.eval_prepare(P32, rn_c, rw_c, n_rad, z_c, wz_c)
-    out32 = torch.empty(x.shape, dtype=torch.complex64, device=dev)
-    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    for i in range(3):
-        if i == 2:
-            f0.record(stream)
-        gf.eval_grid_prepared(P32, n_rad, n_ang, ws32, x, out=out32)
-    f1.record(stream)
-    torch.cuda.synchronize()
-    ref64 = out.to(torch.complex128)
-    err32 = ((out32.to(torch.complex128) - ref64).abs() / ref64.abs().clamp_min(1e-300)).max().item()
-    fp32_variant = {"kernel_ms": f0.elapsed_time(f1), "max_rel_diff_vs_fp64": err32,
-                    "note": "series and NEAR loops in float, per-node set-up, EXACT lanes and the tail in FP64"}
-    out32_sample = out32[::4, ::4].cpu().numpy()   # compared with the oracle on the cpu_baseline sample below
-    del out32, ref64, ws32
+    fp32_variant, out32_sample = None, None
+    if contour == "real":
+        P32 = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
+                             contour="real", precision=32)
+        ws32 = gf.eval_prepare(P32, rn_c, rw_c, n_rad, z_c, wz_c)
+        out32 = torch.empty(x.shape, dtype=torch.complex64, device=dev)
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for i in range(3):
+            if i == 2:
+                f0.record(stream)
+            gf.eval_grid_prepared(P32, n_rad, n_ang, ws32, x, out=out32)
+        f1.record(stream)
+        torch.cuda.synchronize()
+        ref64 = out.to(torch.complex128)
+        err32 = ((out32.to(torch.complex128) - ref64).abs() / ref64.abs().clamp_min(1e-300)).max().item()
+        fp32_variant = {"kernel_ms": f0.elapsed_time(f1), "max_rel_diff_vs_fp64": err32,
+                        "note": "series and NEAR loops in float, per-node set-up, EXACT lanes and the tail in FP64"}
+        out32_sample = out32[::4, ::4].cpu().numpy()   # compared with the oracle on the cpu_baseline sample below
+        del out32, ref64, ws32
 
     # ---- e2e: the host-buffer entry point, copies inside the timed region
     xh = x.cpu().pin_memory()
     outh = torch.empty(xh.shape, dtype=torch.complex128).pin_memory()
-    rn_h, rw_h = gf.make_radial_tables_host("real", n_rad, W.RADIAL_RULE)
+    rn_h, rw_h = gf.make_radial_tables_host(contour, n_rad, W.RADIAL_RULE)
     z_h, wz_h = gf.make_quadrature_host(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
 
     def e2e_step():
@@ -327,7 +339,7 @@ def run_ours(args):
     barrier()
     e2e_ms = max_over_ranks(ee0.elapsed_time(ee1), world, dev)
     assert torch.equal(outh.view(torch.float64), out.cpu().view(torch.float64)), "e2e result differs from device path"
-    h2d = n_points_local * 16 + 8 * (2 * n_rad + 2 * n_ang)
+    h2d = n_points_local * 16 + 8 * (2 * rn_h.size + 2 * n_ang)
     d2h = n_points_local * 16
 
     # ---- the measured FP64-pipe peak at the clocks this run saw (8 independent DFMA chains per thread)
@@ -343,6 +355,21 @@ def run_ours(args):
         if i:
             best = min(best, a.elapsed_time(b))
     dfma_tflops = 2.0 * 8 * peak_iters * peak_blocks * peak_threads / (best * 1e-3) / 1e12
+
+    # ---- issue cadence of DFMA streams by operand pattern, relative to the peak stream (same shape and work)
+    dfma_issue = {}
+    for mode, name in ((0, "one_varying_pair"), (1, "two_varying_pairs"), (2, "three_varying_pairs"), (3, "goertzel_recurrence")):
+        best_m = float("inf")
+        for i in range(4):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            gf.diag_dfma_issue(mode, peak_blocks, peak_threads, peak_iters, sink)
+            b.record(stream)
+            torch.cuda.synchronize()
+            if i:
+                best_m = min(best_m, a.elapsed_time(b))
+        tf = 2.0 * 8 * peak_iters * peak_blocks * peak_threads / (best_m * 1e-3) / 1e12
+        dfma_issue[name] = {"tflops": tf, "cycles_per_warp_dfma_per_smsp": 2.0 * (2.0 * FP64_LANES_PER_SM * N_SM * 1.965e-3) / tf}
 
     if world > 1:
         torch.distributed.barrier()
@@ -364,7 +391,7 @@ def run_ours(args):
         "e2e": {"value": n_points_job * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
                 "h2d_bytes_per_step": h2d * world, "d2h_bytes_per_step": d2h * world},
         "gpu_launches": 3 * args.steps,  # make_grid, prep_real, eval_real per step (gf_eval_grid = the last two)
-        "launch": {"kernel": "eval_real_kernel<double>", "grid_blocks": info["grid_blocks"],
+        "launch": {"kernel": "eval_real_kernel<double>" if contour == "real" else "eval_contour_kernel", "grid_blocks": info["grid_blocks"],
                    "block_threads": info["block_threads"], "smem_bytes": info["smem_bytes"], "lanes_per_point": info["split"]},
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                      "frac": achieved / peak_nominal, "traffic": EVAL_KERNEL_DRAM_TRAFFIC_BYTES,
@@ -374,19 +401,22 @@ def run_ours(args):
                      "fp64_inst_per_launch": fp64_inst, "routes": counters,
                      "fp64_pipe_frac": fp64_inst / (kernel_ms * 1e-3) / (FP64_LANES_PER_SM * N_SM * sm_max * 1e6),
                      "kernel_share_of_step": kernel_ms * args.steps / ms_total},
-        "fp32_variant": fp32_variant,
+        "dfma_issue": dfma_issue,
         "clocks": clocks,
     }
+    if fp32_variant:
+        line["fp32_variant"] = fp32_variant
     if world == 1 and not args.no_cpu_baseline:
         from oracle import gf_oracle as O
         O.build()
         stride = 4
-        line["cpu_baseline"], g_oracle = cpu_baseline(dict(W.CONFIGS[args.workload], name=args.workload), stride)
+        line["cpu_baseline"], g_oracle = cpu_baseline(dict(W.CONFIGS[args.workload], name=args.workload, contour=contour), stride)
         line["parity_check"] = parity_check(out_host[::stride, ::stride], g_oracle, stride,
                                             "oracle/gf_oracle.cpp, double terms (the cpu_baseline leg's own values)")
-        p32 = parity_check(out32_sample, g_oracle, stride, "the same oracle values")
-        line["fp32_variant"]["max_rel_vs_oracle"] = p32["max_rel"]
-        line["fp32_variant"]["ok_1e-4"] = bool(p32["max_rel"] <= 1e-4)
+        if fp32_variant:
+            p32 = parity_check(out32_sample, g_oracle, stride, "the same oracle values")
+            fp32_variant["max_rel_vs_oracle"] = p32["max_rel"]
+            fp32_variant["ok_1e-4"] = bool(p32["max_rel"] <= 1e-4)
     print(json.dumps(line))
     if world > 1:
         torch.distributed.destroy_process_group()
@@ -400,6 +430,8 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", default="cfg3_production", choices=list(W.CONFIGS))
+    ap.add_argument("--contour", default="real", choices=["real", "ray_arc", "thread", "auto"],
+                    help="radial contour policy (the headline and the target are REAL; the others are reported)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)
     _, _, world = dist_env()

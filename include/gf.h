@@ -200,13 +200,14 @@ int gf_eval_angular(const gf_params* p, double x_re, double x_im, const double* 
 int gf_cut_crossings(const gf_params* p, const void* d_x, long long n_points, int n_z, int* d_out, void* stream);
 
 /* The same evaluation, also counting the work by route for the roofline accounting.
- * d_counters: 9 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
- *   [0] pairs of the plain direct loop  [1] series terms EXECUTED (every lane of a warp runs its warp's longest
- *   series)  [2] pairs of the double-double direct loop (EXACT lanes, and the NEAR lanes of their warps)
+ * d_counters: 10 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
+ *   [0] pairs of the plain direct loop  [1] series terms EXECUTED in FP64 (every lane of a warp runs its warp's
+ *   longest series; the FP64 kernel runs the high-order terms of a series, whose sum is below 2^-24 of the budget,
+ *   in FP32: those are counter [9])  [2] pairs of the double-double direct loop (EXACT lanes, and the NEAR lanes of their warps)
  *   [3] [4] [5] [6] (point, radial node, pole) triples taken by the NEAR / MOMENT / EXACT / CHEB
  *   route (the triples of the large-y tail are not among them)  [7] series terms NEEDED (the sum over series
- *   triples of their own K)  [8] tail series evaluated, one per (point, pole).  Results are identical to
- *   gf_eval_grid. */
+ *   triples of their own K)  [8] tail series evaluated, one per (point, pole)  [9] series terms executed in
+ *   FP32 by the FP64 kernel.  Results are identical to gf_eval_grid. */
 int gf_eval_grid_counted(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
                          const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
                          long long n_points, void* d_out, unsigned long long* d_counters, void* stream);

@@ -52,7 +52,7 @@ class gf_launch_info(ctypes.Structure):
 
 
 COUNTER_NAMES = ("near_pairs", "series_terms", "exact_pairs", "near_nodes", "moment_nodes", "exact_nodes",
-                 "cheb_nodes", "series_terms_needed", "tails")
+                 "cheb_nodes", "series_terms_needed", "tails", "series_terms_fp32")
 
 
 _lib = None

@@ -471,7 +471,7 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
   //   tail per (point, pole): 2 DFMA per coefficient (kTailN (kTailN + 1)), 8 + 9 per n, the per-point set-up.
   const bool f32 = p->precision == 32;
   out->near_pair_dfma = f32 ? 0 : 5; out->near_pair_other = f32 ? 0 : 3; out->near_pair_fp32 = f32 ? 5 : 0;
-  out->series_term_dfma = f32 ? 0 : 4; out->series_term_other = 0; out->series_term_fp32 = f32 ? 4 : 0;
+  out->series_term_dfma = f32 ? 0 : 4; out->series_term_other = 0; out->series_term_fp32 = 4;  // per term run in FP32 (counter [9]; the FP32 variant: counter [1])
   out->exact_pair_dfma = 5; out->exact_pair_other = 5;
   out->node_near_dfma = kNodeNearDfma; out->node_near_other = kNodeNearOther;
   out->node_moment_dfma = kNodeMomentDfma; out->node_moment_other = kNodeMomentOther;

@@ -189,7 +189,7 @@ __device__ __forceinline__ cd tail_series(const double* __restrict__ gam, const 
 // Evaluation, REAL contour.  counters (COUNT only): gf.h, gf_eval_grid_counted.
 // ---------------------------------------------------------------------------------------------
 #ifndef GF_MIN_BLOCKS
-#define GF_MIN_BLOCKS 3
+#define GF_MIN_BLOCKS 4
 #endif
 template <typename T, bool COUNT, int NT>
 __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
       const cd az = {xz.re + a.term[r].mu_re, xz.im + a.term[r].mu_im};
       const double axz = a.routing == 1 ? 0.25 * ax : ax;
       const double q = sqrt(axz) + sqrt(axz + sqrt(fma(az.re, az.re, az.im * az.im)));
-      Y0 = fmax(Y0, 4.0 * q * q);
+      Y0 = fmax(Y0, kTailFactor * q * q);
     }
     int lo = 0, hi = a.n_rad;
     while (lo < hi) {
@@ -353,8 +353,11 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
   L.off_q4 = take(L.n_rad_pad);
   L.n_pref = n_terms + (sym && tail ? 1 : 0);
   L.off_pref = take(2 * L.n_pref * L.n_rad_pad);
-  // 2 float tables of npad entries = npad doubles; 2 float2 tables of kmc entries = 2 kmc doubles
-  L.off_f32 = f32 ? take(L.npad + 2 * L.kmc) : -1;
+  // four entries of slack below the float2 series tables (the software-pipelined loop reads them on its last trip),
+  // then 2 float2 tables of kmc entries = 2 kmc doubles; FP32 variant: 2 float tables of npad entries = npad doubles
+  take(4);
+  L.off_sf = take(2 * L.kmc);
+  L.off_f32 = f32 ? take(L.npad) : -1;
   L.n_tab = pyramid ? n_rad + n_rad / 2 + n_rad / 4 + n_rad / 8 : 0;
   L.off_rt = pyramid ? take(L.n_tab) : -1;
   L.off_rw = pyramid ? take(L.n_tab) : -1;

@@ -20,7 +20,16 @@ constexpr int kMaxTerms = 2;
 #endif
 constexpr int kBlockThreads = GF_BLOCK_THREADS;
 constexpr int kKreqBins = 256;
-constexpr int kTailN = 32;  // terms of the large-y tail series (gf_eval.cu)
+#ifndef GF_TAIL_N
+#define GF_TAIL_N 32
+#endif
+#ifndef GF_TAIL_FACTOR
+#define GF_TAIL_FACTOR 4.0
+#endif
+constexpr int kTailN = GF_TAIL_N;  // terms of the large-y tail series (gf_eval.cu)
+// the tail takes over at y >= kTailFactor x (the extent of the cut in the y-plane); term n of its series is below
+// kTailFactor^-n there, and 4^-32 is 5e-20 (longer series with a lower threshold were measured slower: the series is one dependent chain per point)
+constexpr double kTailFactor = GF_TAIL_FACTOR;
 
 // Everything the evaluation kernel needs, passed by value as a __grid_constant__.
 struct EvalArgs {
@@ -58,7 +67,8 @@ struct BlobLayout {
   int off_y, off_q4;            // radial nodes y_i, 1/(4 y_i), n_rad_pad each
   int n_pref;                   // rows of node prefactors: n_terms, + 1 for the symmetric routing's second tail table
   int off_pref;                 // double2 pref[n_pref][n_rad_pad]
-  int off_f32;                  // FP32 variant: float t[npad], w[npad], float2 mom[kmc], cheb[kmc]; or -1
+  int off_sf;                   // float2 mom[kmc], cheb[kmc]: the series tables in float (high-order terms run in FP32)
+  int off_f32;                  // FP32 variant: float t[npad], w[npad]; or -1
   int off_rt, off_rw, n_tab;    // point-dependent contours: the radial rule pyramid (nodes, weights) or -1
   int n_doubles;                // doubles every CTA stages (even)
   int off_gam;                  // tail series: gamma_{n,k}, row n = 1..kTailN at n(n-1)/2, staged; or -1 (no tail)

@@ -137,7 +137,10 @@ struct Tabs {
   const double *st, *stlo, *sw;                   // folded angular rule
   const T *stT, *swT;                             // the same in the loop's type
   const typename Vec2<T>::type *mom, *cheb;       // series coefficients (P_k, N_k), kmc entries each
-  const int* kreq;                                // Chebyshev terms needed per bin of log2(rho)
+  uint32_t a_kreq;                                // shared-window address of kreq
+  uint32_t a_mom, a_momf;                         // shared-window addresses of the double2 / float2 series tables
+                                                  // (moment table first, the Chebyshev table kmc entries further)
+  const int* kreq;                                // Chebyshev terms needed per bin of log2(rho): K | K1 << 16
   double mu0;                                     // sum of the folded weights
   double tau;                                     // EXACT inside this distance of [0,1]
   int n_pairs, kmc;
@@ -157,9 +160,12 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
   } else {
     tb.stT = reinterpret_cast<const T*>(sb + L.off_f32);
     tb.swT = tb.stT + L.npad;
-    tb.mom = reinterpret_cast<const V2*>(tb.swT + L.npad);
+    tb.mom = reinterpret_cast<const V2*>(sb + L.off_sf);
     tb.cheb = tb.mom + L.kmc;
   }
+  tb.a_kreq = smem_u32(sb + L.off_kreq);
+  tb.a_mom = smem_u32(sb + L.off_mom);
+  tb.a_momf = smem_u32(sb + L.off_sf);
   tb.kreq = reinterpret_cast<const int*>(sb + L.off_kreq);
   tb.mu0 = sb[L.off_mom];  // a_0 of the moment series = sum of the folded weights
   tb.tau = sizeof(T) == 8 ? kTau64 : kTau32;
@@ -171,9 +177,9 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
 // Work counters of one thread (COUNT launches only)
 struct RouteCount {
   unsigned long long near_pairs = 0, series_exec = 0, exact_pairs = 0, n_near = 0, n_moment = 0, n_exact = 0,
-                     n_cheb = 0, series_used = 0, tails = 0;
+                     n_cheb = 0, series_used = 0, tails = 0, series_exec32 = 0;
 };
-constexpr int kNumCounters = 9;
+constexpr int kNumCounters = 10;
 
 // ---- NEAR: one folded angular pair: q = w/|zeta - t|^2 and the two sums ---------------------------
 __device__ __forceinline__ void pair_step(double zr, double zi2, double t, double w, double& u0, double& u1) {
@@ -227,25 +233,99 @@ __device__ __forceinline__ cd angular_near(cd eta, cd zeta, double mu0, const T*
 // tab[k], complex s, by the second-order (Goertzel) recurrence c_k = coef_k + r c_{k+1} - |s|^2 c_{k+2},
 // r = 2 Re s, run from k = Kw-1 down to 0 (Kw even): P(s) = c_0 - c_1 conj(s).  On return p1 = c_0,
 // p2 = c_1 (and n1, n2 for N).  Two real DFMA per coefficient instead of a complex multiply-add.
-template <typename T>
-__device__ __forceinline__ void goertzel_pair(const typename Vec2<T>::type* __restrict__ tab, int Kw, T r, T ns,
-                                              T& p1, T& p2, T& n1, T& n2) {
-  typedef typename Vec2<T>::type V2;
-  p1 = p2 = n1 = n2 = (T)0;
-  // software pipeline: the coefficients of the next two terms are loaded while the current two are used (the
-  // last trip reads the two entries below the table, which exist in the staged block and are not used)
-  const V2* c = tab + Kw - 2;
-  V2 c1 = c[1], c0 = c[0];
+// Coefficients k_hi-1 down to k_lo (both multiples of 4, k_hi >= k_lo) on top of the incoming state: on entry
+// p1 = c_{k_hi}, p2 = c_{k_hi+1} (zero to start a series), on return p1 = c_{k_lo}, p2 = c_{k_lo+1}.  Four terms per
+// trip, no remainder.  The tables are addressed by their 32-bit shared-window addresses (one register, no
+// generic-to-shared conversion per node).  With GF_PREFETCH64 the coefficients of the next trip are loaded while the
+// current four terms are used (the last trip then reads the four entries below its range, which exist in the staged
+// block and are not used): 16 more live registers for one load latency less per trip.
+#ifndef GF_PREFETCH64
+#define GF_PREFETCH64 0
+#endif
+__device__ __forceinline__ double2 lds_d2(uint32_t a) {
+  double2 v;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ float4 lds_f4(uint32_t a) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+  return v;
+}
+#ifndef GF_GOERTZEL_ORDER
+#define GF_GOERTZEL_ORDER 1
+#endif
+__device__ __forceinline__ void goertzel4(double r, double ns, double2 c3, double2 c2, double2 c1, double2 c0, double& p1,
+                                          double& p2, double& n1, double& n2) {
+#if GF_GOERTZEL_ORDER
+  // the four products with -|s|^2 of two terms first, then the four with r: runs of one loop-invariant multiplier
+  // (served by the operand-reuse cache) leave two register-file operands per DFMA, which issues every 2 cycles
+  // instead of 3.  Same operations, same values.
+  double t1 = fma(ns, p2, c3.x), u1 = fma(ns, n2, c3.y), t2 = fma(ns, p1, c2.x), u2 = fma(ns, n1, c2.y);
+  p2 = fma(r, p1, t1); n2 = fma(r, n1, u1); p1 = fma(r, p2, t2); n1 = fma(r, n2, u2);
+  t1 = fma(ns, p2, c1.x); u1 = fma(ns, n2, c1.y); t2 = fma(ns, p1, c0.x); u2 = fma(ns, n1, c0.y);
+  p2 = fma(r, p1, t1); n2 = fma(r, n1, u1); p1 = fma(r, p2, t2); n1 = fma(r, n2, u2);
+#else
+  p2 = fma(r, p1, fma(ns, p2, c3.x));
+  n2 = fma(r, n1, fma(ns, n2, c3.y));
+  p1 = fma(r, p2, fma(ns, p1, c2.x));
+  n1 = fma(r, n2, fma(ns, n1, c2.y));
+  p2 = fma(r, p1, fma(ns, p2, c1.x));
+  n2 = fma(r, n1, fma(ns, n2, c1.y));
+  p1 = fma(r, p2, fma(ns, p1, c0.x));
+  n1 = fma(r, n2, fma(ns, n1, c0.y));
+#endif
+}
+// tab: shared address of the double2 table's entry 0
+__device__ __forceinline__ void goertzel_range(uint32_t tab, int k_hi, int k_lo, double r, double ns, double& p1,
+                                               double& p2, double& n1, double& n2) {
+  uint32_t c = tab + 16u * (uint32_t)k_hi;
+#if GF_PREFETCH64
+  double2 c3 = lds_d2(c - 16), c2 = lds_d2(c - 32), c1 = lds_d2(c - 48), c0 = lds_d2(c - 64);
 #pragma unroll(kGoertzelUnroll)
-  for (int k = Kw; k > 0; k -= 2) {
-    c -= 2;
-    const V2 m1 = c[1], m0 = c[0];
-    p2 = fma(r, p1, fma(ns, p2, c1.x));
-    n2 = fma(r, n1, fma(ns, n2, c1.y));
-    p1 = fma(r, p2, fma(ns, p1, c0.x));
-    n1 = fma(r, n2, fma(ns, n1, c0.y));
-    c1 = m1;
-    c0 = m0;
+  for (int k = k_hi; k > k_lo; k -= 4) {
+    c -= 64;
+    const double2 m3 = lds_d2(c - 16), m2 = lds_d2(c - 32), m1 = lds_d2(c - 48), m0 = lds_d2(c - 64);
+    goertzel4(r, ns, c3, c2, c1, c0, p1, p2, n1, n2);
+    c3 = m3; c2 = m2; c1 = m1; c0 = m0;
+  }
+#else
+#pragma unroll 1
+  for (int k = k_hi; k > k_lo; k -= 4) {
+    const double2 c3 = lds_d2(c - 16), c2 = lds_d2(c - 32), c1 = lds_d2(c - 48), c0 = lds_d2(c - 64);
+    c -= 64;
+    goertzel4(r, ns, c3, c2, c1, c0, p1, p2, n1, n2);
+  }
+#endif
+}
+
+// The same recurrence in FP32 for both polynomials at once with the packed fused multiply-add of sm_100
+// (fma.rn.f32x2, SASS FFMA2): s1 = (p1, n1), s2 = (p2, n2); a coefficient pair (P_k, N_k) is one 64-bit operand.
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
+  unsigned long long ua, ub, uc, ud;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(b.x), "f"(b.y));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(uc) : "f"(c.x), "f"(c.y));
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ud) : "l"(ua), "l"(ub), "l"(uc));
+  float2 d;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(ud));
+  return d;
+}
+// tab: shared address of the float2 table's entry 0; the coefficients of the next trip are loaded one trip ahead
+__device__ __forceinline__ void goertzel_range_f32x2(uint32_t tab, int k_hi, int k_lo, float r, float ns, float2& s1,
+                                                     float2& s2) {
+  const float2 rr = {r, r}, nn = {ns, ns};
+  uint32_t c = tab + 8u * (uint32_t)k_hi;
+  float4 hi = lds_f4(c - 16), lo = lds_f4(c - 32);    // (tab[k-2], tab[k-1]), (tab[k-4], tab[k-3])
+#pragma unroll(kGoertzelUnroll)
+  for (int k = k_hi; k > k_lo; k -= 4) {
+    c -= 32;
+    const float4 mh = lds_f4(c - 16), ml = lds_f4(c - 32);
+    s2 = ffma2(rr, s1, ffma2(nn, s2, make_float2(hi.z, hi.w)));
+    s1 = ffma2(rr, s2, ffma2(nn, s1, make_float2(hi.x, hi.y)));
+    s2 = ffma2(rr, s1, ffma2(nn, s2, make_float2(lo.z, lo.w)));
+    s1 = ffma2(rr, s2, ffma2(nn, s1, make_float2(lo.x, lo.y)));
+    hi = mh; lo = ml;
   }
 }
 
@@ -324,7 +404,8 @@ __device__ __forceinline__ cd angular_direct(cd eta, ZetaDD z, double mu0, const
 struct SeriesArg {
   cd sg, g;     // series argument s and prefactor
   double ns;    // -|s|^2
-  int K, route;
+  int K, K1;    // terms needed; terms from K1 on may run in FP32 (their sum is below 2^-24 of the budget)
+  int route;
 };
 
 template <typename T>
@@ -340,7 +421,11 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     o.ns = -in;
     o.g = o.sg;
     // (|s|/2)^K <= 2^-kSeriesBits;  log2 |s|^2 <= -4 (-inf when it underflows in FP32: K = 2)
-    o.K = (int)(2.f * kSeriesBits * rcp_ftz(2.f - lg2_ftz((float)in))) + 2;
+    const float l2 = lg2_ftz((float)in), il = rcp_ftz(2.f - l2);
+    o.K = ((int)(2.f * kSeriesBits * il) + 5) & ~3;         // + 2, rounded up to whole trips of four terms
+    // FP32 from term K1 on: its rounding error 2^-24 A (|s|/2)^K1 (A <= 2.4 the recurrence's amplification) must stay
+    // below 2^-kSeriesBits of the first-order term b_1 s of N, the smallest S can be: (|s|/2)^K1 <= 2^-(kSeriesBits-14) |s|
+    o.K1 = min(((int)((2.f * (kSeriesBits - 14.f) - l2) * il) + 5) & ~3, o.K);
   } else {
     // root = sqrt(zeta (zeta - 1)) = sqrt(w^2 - 1)/2, sign such that |w + 2 root| >= 1
     const double zm = zeta.re - 1.0, wr = fma(2.0, zeta.re, -1.0), wi = zeta.im + zeta.im;
@@ -363,7 +448,12 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     // directly so that the look-up does not wait for the reciprocal.  zeta on [0,1] itself gives rho = 1 or NaN:
     // the comparison fails, never CHEB
     const float ell = 0.5f * lg2_ftz((float)rho2);     // log2(rho)
-    o.K = ell >= kEllLo ? tb.kreq[min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)] : 1 << 20;
+    int kq = 0xffff;
+    if (ell >= kEllLo)
+      asm volatile("ld.shared.s32 %0, [%1];" : "=r"(kq)
+                   : "r"(tb.a_kreq + 4u * (uint32_t)min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)));
+    o.K = kq & 0xffff;     // 0xffff: no usable series in this bin
+    o.K1 = kq >> 16;
     const double in = rcp_fast(rho2);                  // 1/rho^2
     o.sg = {Dr * in, -Di * in};
     o.ns = -in;
@@ -374,7 +464,7 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     // further out S can be 1e-7 of mu0 (the rule nearly integrates eta - t to zero) and the direct form
     // mu0 + (eta - zeta) C(zeta) would lose those digits; the series carry that cancellation in their tables
     if (!(o.K <= tb.kmc)) {
-      o.K = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
+      o.K = o.K1 = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
       o.route = (zeta.im * zeta.im < tb.tau * tb.tau && zeta.re > -tb.tau && zeta.re < 1.0 + tb.tau) ? ROUTE_EXACT
                                                                                                      : ROUTE_NEAR;
     }
@@ -383,9 +473,9 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
 }
 
 // S = g [delta P(s) - N(s)] from the recurrence's last two values of each polynomial
-template <typename T, bool COUNT>
-__device__ __forceinline__ cd series_finish(const SeriesArg& o, cd delta, T p1, T p2, T n1, T n2, RouteCount& rc) {
-  const double b0 = (double)p1, b1 = (double)p2, d0 = (double)n1, d1 = (double)n2;
+template <bool COUNT>
+__device__ __forceinline__ cd series_finish(const SeriesArg& o, cd delta, double b0, double b1, double d0, double d1,
+                                            RouteCount& rc) {
   const double Pr = fma(-b1, o.sg.re, b0), Pi = b1 * o.sg.im;     // c_0 - c_1 conj(s)
   const double Nr = fma(-d1, o.sg.re, d0), Ni = d1 * o.sg.im;
   const cd acc = {fma(delta.re, Pr, fma(-delta.im, Pi, -Nr)), fma(delta.re, Pi, fma(delta.im, Pr, -Ni))};
@@ -426,18 +516,22 @@ __device__ __forceinline__ cd direct_route(const Tabs<T>& tb, int route, bool wa
 template <typename T, bool COUNT>
 __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta, cd zeta, double mur, double mui,
                                         RouteCount& rc) {
-  typedef typename Vec2<T>::type V2;
   const SeriesArg o = route_setup<T>(tb, zeta);
-  const V2* tab = o.route == ROUTE_CHEB ? tb.cheb : tb.mom;
-  int Kw = __reduce_max_sync(0xffffffffu, o.K);
+  // every lane's K and K1 are multiples of 4 and at most kmc (route_setup): so are the warp's
+  const int Kw = __reduce_max_sync(0xffffffffu, o.K);
   const bool warp_has_exact = __any_sync(0xffffffffu, o.route == ROUTE_EXACT);
-  Kw = min((Kw + 1) & ~1, tb.kmc);
   cd s = {0.0, 0.0};
   if (Kw > 0) {  // warp-uniform
-    T p1, p2, n1, n2;
-    goertzel_pair<T>(tab, Kw, (T)(o.sg.re + o.sg.re), (T)o.ns, p1, p2, n1, n2);
-    if (COUNT) rc.series_exec += Kw;
-    if (o.route <= ROUTE_CHEB) s = series_finish<T, COUNT>(o, delta, p1, p2, n1, n2, rc);
+    // terms Kw-1 .. K1w run in FP32 on the FMA pipe (the warp's largest K1: every lane's own need is met), the
+    // recurrence's state is widened, and terms K1w-1 .. 0 run in FP64 (the FP32 variant: everything in FP32)
+    const int K1w = sizeof(T) == 8 ? __reduce_max_sync(0xffffffffu, o.K1) : 0;
+    const uint32_t tsel = o.route == ROUTE_CHEB ? (uint32_t)tb.kmc : 0u;   // the Chebyshev tables follow the moment tables
+    float2 s1 = {0.f, 0.f}, s2 = {0.f, 0.f};
+    goertzel_range_f32x2(tb.a_momf + 8u * tsel, Kw, K1w, (float)(o.sg.re + o.sg.re), (float)o.ns, s1, s2);
+    double p1 = (double)s1.x, n1 = (double)s1.y, p2 = (double)s2.x, n2 = (double)s2.y;
+    if (sizeof(T) == 8) goertzel_range(tb.a_mom + 16u * tsel, K1w, 0, o.sg.re + o.sg.re, o.ns, p1, p2, n1, n2);
+    if (COUNT) { rc.series_exec += sizeof(T) == 8 ? K1w : Kw; rc.series_exec32 += sizeof(T) == 8 ? Kw - K1w : 0; }
+    if (o.route <= ROUTE_CHEB) s = series_finish<COUNT>(o, delta, p1, p2, n1, n2, rc);
   }
   if (o.route >= ROUTE_NEAR) s = direct_route<T, COUNT>(tb, o.route, warp_has_exact, x, y, delta, zeta, mur, mui, rc);
   return s;
@@ -447,7 +541,7 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
 __device__ __forceinline__ void flush_counters(const RouteCount& rc, bool active, unsigned long long* counters) {
   unsigned long long v[kNumCounters] = {rc.near_pairs, rc.series_exec, rc.exact_pairs, rc.n_near,
                                         rc.n_moment,   rc.n_exact,     rc.n_cheb,      rc.series_used,
-                                        rc.tails};
+                                        rc.tails,      rc.series_exec32};
   for (int k = 0; k < kNumCounters; ++k) {
     if (!active) v[k] = 0;
     for (int o = 16; o; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
@@ -521,9 +615,8 @@ __device__ __forceinline__ double powi(double t, int k) {
 
 __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double* blob, dd (*s_cpart)[2][kMomTerms]) {
   const double* scratch = blob + L.off_scratch;
-  float2* momf = L.off_f32 >= 0 ? reinterpret_cast<float2*>(reinterpret_cast<float*>(blob + L.off_f32) + 2 * L.npad)
-                                : nullptr;
-  float2* chebf = momf ? momf + L.kmc : nullptr;
+  float2* momf = reinterpret_cast<float2*>(blob + L.off_sf);
+  float2* chebf = momf + L.kmc;
   for (int k = threadIdx.x; k < L.kmc; k += blockDim.x) {
     dd tau = {0.0, 0.0}, nu = {0.0, 0.0}, tau1 = {0.0, 0.0}, nu1 = {0.0, 0.0}, mo = {0.0, 0.0}, no = {0.0, 0.0};
     for (int j = 0; j < a.n_pairs; j += 2) {   // two independent accumulator chains (npad is even, padding has w = 0)
@@ -556,7 +649,7 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
     const double c0 = half * tau.hi, c1 = half * nu.hi;
     blob[L.off_cheb + 2 * k] = c0;
     blob[L.off_cheb + 2 * k + 1] = c1;
-    if (chebf) chebf[k] = make_float2((float)c0, (float)c1);
+    chebf[k] = make_float2((float)c0, (float)c1);
   }
   __syncthreads();
   for (int k = threadIdx.x; k < L.kmc; k += blockDim.x) {
@@ -569,7 +662,7 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
     const double m0 = mo.hi, m1 = no.hi;     // zero beyond kMomTerms
     blob[L.off_mom + 2 * k] = m0;
     blob[L.off_mom + 2 * k + 1] = m1;
-    if (momf) momf[k] = make_float2((float)m0, (float)m1);
+    momf[k] = make_float2((float)m0, (float)m1);
   }
 }
 
@@ -586,7 +679,7 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc 
   __syncthreads();
   for (int b = threadIdx.x; b < kKreqBins; b += blockDim.x) {
     const float ell = kEllLo + (float)b * kEllStep;
-    int K = 1 << 20;
+    int K = 0xffff, K1 = 0;
     if (ell * L.kmc >= 60.f) {
       K = 4;
       for (int j = L.kmc - 1; j >= 4; --j)
@@ -594,9 +687,20 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc 
           K = j + 1;
           break;
         }
-      K = (K + 3) & ~1;   // one spare term, even
+      K = (K + 4) & ~3;   // one spare term, whole trips of four terms (kmc is a multiple of 4)
+      // K1: from here on the terms may run in FP32.  A rounding error of the recurrence at step k acts like a
+      // perturbation of c_k by <= 4 2^-24 max_{j>=k}|c_j| / (1 - 1/rho)^2, and the perturbations sum like a geometric
+      // series: the FP32 phase costs <= 2^-22 max_{j>=K1} |c_j| rho^-j / (1 - 1/rho)^3, held below the truncation
+      // budget: |c_j| rho^-j <= 2^-(kSeriesBits - 20) (1 - 1/rho)^3 |c_0| for all j >= K1
+      const float thr = kSeriesBits - 20.f + 3.f * log2f(1.f / (1.f - exp2f(-ell)));
+      for (int j = L.kmc - 1; j >= 0; --j)
+        if (s_lc[j] - (float)j * ell > -thr) {
+          K1 = j + 1;
+          break;
+        }
+      K1 = min((K1 + 3) & ~3, K);
     }
-    kreq[b] = K;
+    kreq[b] = K | (K1 << 16);
   }
 }
 
@@ -607,17 +711,12 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc 
 //   Rhat_n(i0) = sum_{i >= i0} pref_i (y_i0 / y_i)^n by the downward recurrence
 //   Rhat_n(i) = pref_i + (y_i/y_{i+1})^n Rhat_n(i+1), the powers of q_i = y_i/y_{i+1} in double-double.
 // ---------------------------------------------------------------------------------------------
-__device__ dd dd_binom(int n, int k) {   // C(n, k) for n <= 63, exact: every partial product fits 64 bits
+__device__ dd dd_binom(int n, int k) {   // C(n, k) as a double-double (exact while it fits 106 bits)
   if (k < 0 || k > n) return {0.0, 0.0};
   if (k > n - k) k = n - k;
-  unsigned long long c = 1;
-  for (int i = 1; i <= k; ++i) {
-    const unsigned long long m = (unsigned long long)(n - k + i), d = (unsigned long long)i;
-    c = (c / d) * m + ((c % d) * m) / d;   // c m / d without forming c m (c m is divisible by d)
-  }
-  const double hi = (double)c;             // < 2^63; the remainder is exact in a double
-  const long long rem = (long long)c - (long long)hi;
-  return quick_two_sum(hi, (double)rem);
+  dd c = {1.0, 0.0};
+  for (int i = 1; i <= k; ++i) c = dd_div_d(dd_mul_d(c, (double)(n - k + i)), (double)i);   // stays an integer
+  return c;
 }
 
 // phase A (after prep_angular + __syncthreads): thread (k, c) sums chunk c of 8 of the nodes into s_part[c][k]

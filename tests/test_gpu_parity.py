@@ -245,9 +245,11 @@ def test_route_counters(gf):
     # pairs are counted by loop (the NEAR lanes of a warp with an EXACT lane run the double-double loop too)
     assert c["near_pairs"] + c["exact_pairs"] == (c["near_nodes"] + c["exact_nodes"]) * n_pairs
     assert c["exact_pairs"] >= c["exact_nodes"] * n_pairs
-    # each series triple needs 2..256 terms; a warp runs its longest series on all 32 lanes
-    assert 2 * series_nodes <= c["series_terms_needed"] <= 256 * series_nodes
-    assert c["series_terms_needed"] <= c["series_terms"] <= 256 * x.numel() * cfg["n_rad"]
+    # each series triple needs 4..256 terms; a warp runs its longest series on all 32 lanes, the high-order terms in
+    # FP32 (counter "series_terms_fp32"), the rest in FP64 ("series_terms")
+    assert 4 * series_nodes <= c["series_terms_needed"] <= 256 * series_nodes
+    assert c["series_terms_needed"] <= c["series_terms"] + c["series_terms_fp32"] <= 256 * x.numel() * cfg["n_rad"]
+    assert 0 < c["series_terms"] < c["series_terms_fp32"]
     assert 0 < c["exact_nodes"] < 0.2 * (c["near_nodes"] + c["exact_nodes"]) and c["cheb_nodes"] > c["near_nodes"]
 
 
