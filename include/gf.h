@@ -71,16 +71,35 @@ typedef struct {
  *   THREAD   polyline through the opening of the cut for Re x < -4 m^2 next to the negative
  *            axis, equal real masses only (analogue of the region-3/4 contours);
  *   AUTO     per-point choice among the three.
- * With sc = |m2^2| of line 2 (largest pole modulus for a rational line), phi = arg x:
- *   RAY_ARC  = ray r e^{i phi}, r in [0,R] shifted-log, n_rad/2 nodes; arc R e^{i theta}, theta: phi -> 0,
- *              n_rad/4; real [R, Lambda^2] shifted-log, n_rad/4; R = min(1.5 (sqrt|x| + sqrt(|x|+sc))^2, Lambda^2/2).
+ * Geometry (no angle is ever formed; every operation below is one correctly rounded +, -, *, /, sqrt in the order
+ * written, so the nodes are the same doubles on any IEEE machine).  sc = |m2^2| of line 2 (largest pole modulus for
+ * a rational line); dir = x/|x| with x scaled by a power of two first (two divisions); tau = tan(phi/4) of dir =
+ * (cos phi, sin phi) by half-angle formulas (ch = sqrt((1+c)/2), sh = (s/2)/ch for c >= 0, else sh = +-sqrt((1-c)/2),
+ * ch = (|s|/2)/|sh|; tau = sh/(1+ch)).  Ladder of contour radii: {2^k, 1.5 2^k}, starting one rung below the smallest
+ * rung >= 1.5 sc; rung(v) = the smallest rung >= v, or Lambda^2/2 when that rung is more than 64 rungs up the ladder
+ * or not below Lambda^2/2.
+ *   RAY_ARC  = ray r dir, r in [0,R] shifted-log, n_rad/2 nodes; arc y(v) = R ((1 + i tau v)/(1 - i tau v))^2,
+ *              v = 1 - u: 1 -> 0, with dy/du = -4 i tau y/(1 + tau^2 v^2), n_rad/4; real [R, Lambda^2] shifted-log,
+ *              n_rad/4; R = rung(1.5 (sqrt|x| + sqrt(|x|+sc))^2).
  *   THREAD   (Im x >= 0, mirrored otherwise; s = |x|, |A| = (sqrt s - m)^2, |B| = (sqrt s + m)^2, r0 = |x + m^2|)
- *              straight pieces 0 -> -m^2 + i(|A|-m^2)/2 -> (|A|+m^2)/2 e^{i phi} -> -(|A|+r0)/2 - i(r0-|A|)/2
- *              -> r0 e^{i phi} -> R e^{3 pi i/4}, arc to R, n_rad/8 nodes each; real [R, Lambda^2], n_rad/4;
- *              R = min(1.5 |B|, Lambda^2/2).
- *   AUTO     wedge W = {Re x < -sc, |Im x| n_ang sc < 5 |x|^2}: outside W RAY_ARC; inside W THREAD if it
- *              applies and Re x <= -4.1 sc, else REAL.
- * Every piece carries the Gauss-Legendre rule of its order from the pyramid of gf_radial_table_size(). */
+ *              straight pieces 0 -> -m^2 + i(|A|-m^2)/2 -> (|A|+m^2)/2 dir -> -(|A|+r0)/2 - i(r0-|A|)/2
+ *              -> r0 dir -> R e^{3 pi i/4} (the arc's v = 1 end with tau = tan(3 pi/16)), arc to R, n_rad/8 nodes
+ *              each; real [R, Lambda^2], n_rad/4; R = rung(1.5 |B|).
+ *   AUTO     with c2 = min over the poles -mu of line 2 of (Re sqrt(mu))^2 = (|mu| + Re mu)/2 and the parabola
+ *              P(c) = {Re x + c > 0, (Im x)^2 < 4 c (Re x + c)} (REAL is the continuation exactly inside P(c2),
+ *              PAPER.md:270), tested in this order:
+ *              1. x in P(c2/2): REAL (exact there and the cheapest);
+ *              2. Re x < 0, |Im x| n_rad < 80 |Re x| and x in P(c2): REAL (next to the negative axis the ray of
+ *                 RAY_ARC passes the pole of line 1 closer than the radial rule resolves);
+ *              3. x in the wedge W = {Re x < -sc, |Im x| n_ang sc < 5 |x|^2}: THREAD if it applies and
+ *                 Re x <= -4.1 sc, else REAL;
+ *              4. RAY_ARC.
+ *            Limitation: in case 3 with REAL (next to the negative axis between the parabola and -4.1 sc, e.g. the
+ *            strip -4 m^2 < Re x < -m^2 of the equal-mass bubble, and for lines THREAD does not apply to) the value
+ *            is bounded and reproducible but NOT the analytic continuation: no contour of this library reaches it.
+ * Every piece carries the Gauss-Legendre rule of its order from the pyramid of gf_radial_table_size().
+ * The restructured evaluation (pole sum, folded angular sum, series) needs propagators that are sums of simple
+ * poles, which MASSIVE and RATIONAL are; it does not extend to a general integrand F(x, y, z) of PAPER.md:43. */
 typedef enum { GF_CONTOUR_REAL = 0, GF_CONTOUR_RAY_ARC = 1, GF_CONTOUR_THREAD = 2, GF_CONTOUR_AUTO = 3 } gf_contour;
 
 typedef enum { GF_SPACING_UNIFORM = 0, GF_SPACING_LOG_ABS_IM = 1 } gf_spacing;
@@ -252,6 +271,14 @@ int gf_diag_dfma_issue(int mode, int blocks, int threads, long long iters, doubl
  * exactly as the evaluation kernel makes them (double-double, correctly rounded), for the n rule nodes in
  * d_nodes; tests compare them bit for bit with the oracle's. */
 int gf_diag_radial_map(double cutoff2, double map_scale, const double* d_nodes, int n, double* d_y, void* stream);
+/* The n_rad nodes of the contour of the one point x = (x_re, x_im) under a deformed policy (RAY_ARC, THREAD, AUTO)
+ * exactly as the evaluation kernel walks them, read from the workspace gf_eval_prepare() made for the same
+ * (p, rules, orders): d_policy[0] = the policy taken (gf_contour), d_y[g] = y_g, d_wy[g] = (rule weight) x dy/dt
+ * (complex<double>, n_rad each; the weights are re-derived and good to a few ulp).  Tests compare y bit for bit with
+ * the oracle's. */
+int gf_diag_contour_nodes(const gf_params* p, int n_rad, int n_ang, const void* d_workspace, const double* d_rad_nodes,
+                          const double* d_rad_weights, double x_re, double x_im, int* d_policy, void* d_y, void* d_wy,
+                          void* stream);
 
 /* Return the cached scratch of every device's pool to the driver (blocks still in use by enqueued work stay). */
 int gf_trim_scratch(void);

@@ -313,57 +313,123 @@ void seg_line(cplx a, cplx b, Rule R, std::vector<RNode>& out) {
   }
 }
 
-void seg_arc(double Rad, double th0, double th1, Rule R, std::vector<RNode>& out) {
+// Arc of the circle |y| = Rad from Rad e^{i phi} back to the real axis at Rad, tau = tan(phi/4), |tau| <= 1, in the
+// rational parametrisation  y(v) = Rad ((1 + i tau v)/(1 - i tau v))^2,  v = 1 - u  (angle 4 atan(tau v), so v = 1 is
+// the ray's end and v = 0 the real axis):  dy/du = -4 i tau y / (1 + tau^2 v^2).  Only + - * / occur, each rounded
+// once in the order written, so the nodes are the same doubles on any IEEE machine.
+void seg_arc(double Rad, double tau, Rule R, std::vector<RNode>& out) {
   for (int i = 0; i < R.n; ++i) {
     double u = 0.5 * (R.t[i] + 1.0);
-    double th = th0 + (th1 - th0) * u;
-    cplx y = Rad * cplx(std::cos(th), std::sin(th));
-    RNode nd = { y, cplx(0, 1) * y * ((th1 - th0) * 0.5 * R.w[i]) };
+    double v = 1.0 - u;
+    double tv = tau * v;
+    double t2 = tv * tv;
+    double n2 = 1.0 + t2;
+    double in2 = 1.0 / n2;                                  // the one division of the node
+    double gr = (1.0 - t2) * in2, gi = (2.0 * tv) * in2;    // g = (1 + i tau v)/(1 - i tau v)
+    double gr2 = gr * gr, gi2 = gi * gi;
+    double Er = gr2 - gi2, Ei = 2.0 * (gr * gi);            // g^2
+    double yr = Rad * Er, yi = Rad * Ei;
+    double f = ((2.0 * tau) * R.w[i]) * in2;
+    RNode nd = { cplx(yr, yi), cplx(f * yi, -(f * yr)) };
     out.push_back(nd);
   }
+}
+
+// The radius of a deformed contour is taken from the ladder {2^k, 1.5 2^k}: the smallest rung >= v.  (The library
+// keeps the radial nodes of every rung in tables made once per launch; the ladder is part of the contour's
+// definition, so it is restated here.)  rung index I: value(I) = 2^(I/2) for even I, 1.5 2^((I-1)/2) for odd I.
+int rung_index(double v) {
+  int e;
+  double m = std::frexp(v, &e);          // v = m 2^e, 0.5 <= m < 1
+  if (m == 0.5) return 2 * (e - 1);
+  if (m <= 0.75) return 2 * (e - 1) + 1;
+  return 2 * e;
+}
+const int kRungs = 64;   // rungs tabulated above the one below 1.5 sc; beyond them the radius is Lambda^2/2
+double contour_radius(double Rstar, double sc, double cutoff2) {
+  int I = rung_index(Rstar), I_lo = rung_index(1.5 * sc) - 1;
+  if (I < I_lo) I = I_lo;
+  double R = (I & 1) ? std::ldexp(1.5, (I - 1) >> 1) : std::ldexp(1.0, I >> 1);
+  if (I > I_lo + kRungs - 1 || !(R < 0.5 * cutoff2)) return 0.5 * cutoff2;
+  return R;
+}
+
+// direction x/|x| of the ray through x, each component one correctly rounded division (no angle is formed: through
+// atan2 and sincos the small component of the direction would inherit the ABSOLUTE error of the angle); x is first
+// scaled by a power of two so that no square underflows.  *ax: |x|.
+cplx ray_direction(cplx x, double* ax) {
+  double big = std::fmax(std::fabs(x.real()), std::fabs(x.imag()));
+  if (big == 0.0) { *ax = 0.0; return cplx(1.0, 0.0); }
+  int e;
+  std::frexp(big, &e);
+  double xr = std::ldexp(x.real(), -e), xi = std::ldexp(x.imag(), -e);
+  double as = std::sqrt(std::fma(xr, xr, xi * xi));
+  *ax = std::ldexp(as, e);
+  return cplx(xr / as, xi / as);
+}
+
+// tan(phi/4) of the direction (c, s) = (cos phi, sin phi), |phi| <= pi, by half-angle formulas without cancellation
+double tan_quarter(double c, double s) {
+  double ch, sh;   // cos(phi/2) >= 0, sin(phi/2)
+  if (c >= 0.0) {
+    ch = std::sqrt(0.5 * (1.0 + c));
+    sh = (0.5 * s) / ch;
+  } else {
+    sh = std::copysign(std::sqrt(0.5 * (1.0 - c)), s);
+    ch = (0.5 * std::fabs(s)) / std::fabs(sh);
+  }
+  return sh / (1.0 + ch);
 }
 
 void contour_real(const Params& P, const double* rn, const double* rw, int n_rad, std::vector<RNode>& out) {
   seg_logreal(0.0, P.cutoff2, P.map_scale, cplx(1, 0), level(rn, rw, n_rad, 0), out);
 }
 
+// RAY_ARC: generalises the paper's region-2/5 contour: ray along x, arc back to the real axis,
+// real tail.
 void contour_ray_arc(const Params& P, cplx x, const double* rn, const double* rw, int n_rad,
                      std::vector<RNode>& out) {
-  double ax = std::sqrt(std::fma(x.real(), x.real(), x.imag() * x.imag()));
-  double phi = std::atan2(x.imag(), x.real());
+  double ax;
+  cplx dir = ray_direction(x, &ax);
   double sc = line2_scale(P.line_pk);
   double q = std::sqrt(ax) + std::sqrt(ax + sc);
-  double Rad = std::fmin(1.5 * q * q, 0.5 * P.cutoff2);
-  cplx dir(std::cos(phi), std::sin(phi));
+  double Rad = contour_radius(1.5 * q * q, sc, P.cutoff2);
   seg_logreal(0.0, Rad, P.map_scale, dir, level(rn, rw, n_rad, 1), out);
-  seg_arc(Rad, phi, 0.0, level(rn, rw, n_rad, 2), out);
+  seg_arc(Rad, tan_quarter(dir.real(), dir.imag()), level(rn, rw, n_rad, 2), out);
   seg_logreal(Rad, P.cutoff2, P.map_scale, cplx(1, 0), level(rn, rw, n_rad, 2), out);
 }
 
 // THREAD: equal real masses, Re x < -4 m^2, near the negative axis.
+const double kTau5 = 0.66817863791929891999775768652308;   // tan(3 pi/16): the far waypoint sits at angle 3 pi/4
 void contour_thread(const Params& P, cplx x, const double* rn, const double* rw, int n_rad,
                     std::vector<RNode>& out) {
   bool mirror = x.imag() < 0;
   cplx xx = mirror ? std::conj(x) : x;
   double m2 = P.line_pk.m2_re, m = std::sqrt(m2);
-  double s = std::sqrt(std::fma(xx.real(), xx.real(), xx.imag() * xx.imag()));
-  double phi = std::atan2(xx.imag(), xx.real());
+  double s;
+  cplx e = ray_direction(xx, &s);
   double rs = std::sqrt(s);
   double Aa = (rs - m) * (rs - m), Bb = (rs + m) * (rs + m);
-  double r0 = std::abs(xx + m2);
-  cplx e(std::cos(phi), std::sin(phi));
+  double t = xx.real() + m2;
+  double r0 = std::sqrt(std::fma(t, t, xx.imag() * xx.imag()));   // |x + m^2|
   cplx W[6];
   W[0] = 0.0;
   W[1] = cplx(-m2, 0.5 * (Aa - m2));
-  W[2] = 0.5 * (Aa + m2) * e;
+  double h2 = 0.5 * (Aa + m2);
+  W[2] = cplx(h2 * e.real(), h2 * e.imag());
   W[3] = cplx(-0.5 * (Aa + r0), -0.5 * (r0 - Aa));
-  W[4] = r0 * e;
-  double Rad = std::fmin(1.5 * Bb, 0.5 * P.cutoff2);
-  double th5 = (double)(0.75L * kPi);
-  W[5] = Rad * cplx(std::cos(th5), std::sin(th5));
+  W[4] = cplx(r0 * e.real(), r0 * e.imag());
+  double Rad = contour_radius(1.5 * Bb, line2_scale(P.line_pk), P.cutoff2);
+  {   // W5 = Rad e^{3 pi i/4} as the arc's own v = 1 end
+    double t2 = kTau5 * kTau5, n2 = 1.0 + t2;
+    double in2 = 1.0 / n2;
+    double gr = (1.0 - t2) * in2, gi = (2.0 * kTau5) * in2;
+    double gr2 = gr * gr, gi2 = gi * gi;
+    W[5] = cplx(Rad * (gr2 - gi2), Rad * (2.0 * (gr * gi)));
+  }
   size_t first = out.size();
   for (int k = 0; k < 5; ++k) seg_line(W[k], W[k + 1], level(rn, rw, n_rad, 3), out);
-  seg_arc(Rad, th5, 0.0, level(rn, rw, n_rad, 3), out);
+  seg_arc(Rad, kTau5, level(rn, rw, n_rad, 3), out);
   seg_logreal(Rad, P.cutoff2, P.map_scale, cplx(1, 0), level(rn, rw, n_rad, 2), out);
   if (mirror)
     for (size_t k = first; k < out.size(); ++k) {
@@ -377,13 +443,42 @@ bool thread_applicable(const Params& P) {
          P.line_pk.m2_im == 0 && P.line_k.m2_re == P.line_pk.m2_re && P.line_pk.m2_re > 0;
 }
 
+// (Re sqrt(mu))^2 = (|mu| + Re mu)/2, the smallest over the poles -mu of line 2: the REAL contour is the continuation
+// exactly where |Im sqrt(x)| < Re sqrt(mu) for every pole (the cut (sqrt(x) z + i sqrt(x (1-z^2) + mu))^2 of eq. (25)
+// reaches the positive real y-axis when an end point (sqrt(x) +- i sqrt(mu))^2 becomes real), i.e. inside the parabola
+// Re x > (Im x)^2/(4 c2) - c2 -- for a real mass m the parabola of PAPER.md:270 with c2 = m^2.
+double parabola_c2(const Propagator& q) {
+  auto c2 = [](double mr, double mi) { return 0.5 * (std::sqrt(std::fma(mr, mr, mi * mi)) + mr); };
+  if (q.kind == PROP_MASSIVE) return c2(q.m2_re, q.m2_im);
+  double disc = q.a * q.a - 4.0 * q.b;
+  if (disc >= 0.0) {
+    double r = std::sqrt(disc);
+    return std::fmin(c2(0.5 * (q.a - r), 0.0), c2(0.5 * (q.a + r), 0.0));
+  }
+  return c2(0.5 * q.a, 0.5 * std::sqrt(-disc));
+}
+bool in_parabola(double xr, double xi, double cc) {
+  double t = xr + cc;
+  return t > 0.0 && xi * xi < (4.0 * cc) * t;
+}
+
 // AUTO: per-point choice, half-open tests exactly as DESIGN.md writes them.
-int auto_policy(const Params& P, cplx x, int n_ang) {
-  double sc = line2_scale(P.line_pk);
-  double ax2 = std::fma(x.real(), x.real(), x.imag() * x.imag());
-  bool wedge = (x.real() < -sc) && (std::fabs(x.imag()) * ((double)n_ang * sc) < 5.0 * ax2);
+//   1. inside the parabola of half the size (|Im sqrt x| < 0.71 Re sqrt mu): REAL, exact and the cheapest;
+//   2. next to the negative real axis (|Im x| n_rad < 80 |Re x|), where the ray of RAY_ARC passes the pole of line 1
+//      and the opening of the cut closer than the radial rule resolves: REAL as long as x is inside the parabola;
+//   3. in the wedge {Re x < -sc, |Im x| n_ang sc < 5 |x|^2}: THREAD where it applies and Re x <= -4.1 sc, else REAL
+//      (bounded and reproducible, but NOT the continuation: the documented limitation);
+//   4. RAY_ARC everywhere else.
+int auto_policy(const Params& P, cplx x, int n_rad, int n_ang) {
+  double sc = line2_scale(P.line_pk), c2 = parabola_c2(P.line_pk);
+  double xr = x.real(), xi = x.imag();
+  if (in_parabola(xr, xi, 0.5 * c2)) return CONTOUR_REAL;
+  bool near_axis = xr < 0.0 && std::fabs(xi) * (double)n_rad < 80.0 * std::fabs(xr);
+  if (near_axis && in_parabola(xr, xi, c2)) return CONTOUR_REAL;
+  double ax2 = std::fma(xr, xr, xi * xi);
+  bool wedge = (xr < -sc) && (std::fabs(xi) * ((double)n_ang * sc) < 5.0 * ax2);
   if (!wedge) return CONTOUR_RAY_ARC;
-  if (thread_applicable(P) && x.real() <= -4.1 * sc) return CONTOUR_THREAD;
+  if (thread_applicable(P) && xr <= -4.1 * sc) return CONTOUR_THREAD;
   return CONTOUR_REAL;
 }
 
@@ -406,7 +501,7 @@ cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int
                 const double* z, const double* wz, int n_ang, std::vector<RNode>& nodes) {
   typedef std::complex<R> C;
   nodes.clear();
-  int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, x, n_ang) : P.contour;
+  int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, x, n_rad, n_ang) : P.contour;
   if (pol == CONTOUR_REAL) contour_real(P, rn, rw, n_rad, nodes);
   else if (pol == CONTOUR_RAY_ARC) contour_ray_arc(P, x, rn, rw, n_rad, nodes);
   else contour_thread(P, x, rn, rw, n_rad, nodes);
@@ -609,7 +704,7 @@ int gfo_contour_nodes(const void* params, double x_re, double x_im, const double
   if (check_params(P, n_rad, n_ang)) return -1;
   cplx x(x_re, x_im);
   std::vector<RNode> nodes;
-  int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, x, n_ang) : P.contour;
+  int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, x, n_rad, n_ang) : P.contour;
   if (pol == CONTOUR_REAL) contour_real(P, rad_nodes, rad_weights, n_rad, nodes);
   else if (pol == CONTOUR_RAY_ARC) contour_ray_arc(P, x, rad_nodes, rad_weights, n_rad, nodes);
   else contour_thread(P, x, rad_nodes, rad_weights, n_rad, nodes);

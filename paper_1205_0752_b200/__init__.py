@@ -75,6 +75,7 @@ _SIGNATURES = {
     "gf_diag_fp64_peak": [_int, _int, _ll, _vp, _vp],
     "gf_diag_dfma_issue": [_int, _int, _int, _ll, _vp, _vp],
     "gf_diag_radial_map": [_dbl, _dbl, _vp, _int, _vp, _vp],
+    "gf_diag_contour_nodes": [ctypes.POINTER(gf_params), _int, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _vp, _vp, _vp],
     "gf_trim_scratch": [],
     "gf_last_error": [],
     "gf_version": [],
@@ -340,6 +341,23 @@ def eval_grid_host(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights
         raise GfError(4, "no CUDA device (no CPU fallback)")
     n_ang = int(ang_nodes.shape[0])
     n_points = int(np.prod(x.shape))
+    # the library reads and writes these buffers by size alone: check what it cannot
+    def _dt(a):
+        return str(a.dtype).replace("torch.", "")
+    need = radial_table_size(params.contour, n_rad)
+    if need < 0:
+        raise GfError(2, "bad contour / n_rad (deformed contours need n_rad % 8 == 0)")
+    for name, t, n in (("rad_nodes", rad_nodes, need), ("rad_weights", rad_weights, need), ("ang_nodes", ang_nodes, n_ang),
+                       ("ang_weights", ang_weights, n_ang)):
+        if _dt(t) != "float64" or int(np.prod(t.shape)) < n:
+            raise GfError(2, "eval_grid_host: %s must be float64 with at least %d entries" % (name, n))
+    if int(np.prod(ang_weights.shape)) != n_ang:
+        raise GfError(2, "eval_grid_host: ang_nodes and ang_weights differ in length")
+    odt = "complex64" if params.precision == 32 else "complex128"
+    if _dt(x) != "complex128":
+        raise GfError(2, "eval_grid_host: x must be complex128")
+    if _dt(out) != odt or int(np.prod(out.shape)) != n_points:
+        raise GfError(2, "eval_grid_host: out must be %s with %d entries" % (odt, n_points))
     _check(lib().gf_eval_grid_host(ctypes.byref(params), _host_ptr(rad_nodes), _host_ptr(rad_weights), n_rad,
                                    _host_ptr(ang_nodes), _host_ptr(ang_weights), n_ang, _host_ptr(x),
                                    n_points, _host_ptr(out), _stream(stream)))
@@ -360,6 +378,19 @@ def diag_radial_map(cutoff2, map_scale, nodes, stream=None):
     y = torch.empty_like(nodes)
     _check(lib().gf_diag_radial_map(cutoff2, map_scale, nodes.data_ptr(), nodes.numel(), y.data_ptr(), _stream(stream)))
     return y
+
+
+def diag_contour_nodes(params, n_rad, n_ang, workspace, rad_nodes, rad_weights, x, stream=None):
+    """gf_diag_contour_nodes: (policy, y, wy) of the one point x under a deformed policy, from a prepared workspace."""
+    x = complex(x)
+    y = torch.empty(n_rad, dtype=torch.complex128, device=workspace.device)
+    wy = torch.empty_like(y)
+    pol = torch.zeros(1, dtype=torch.int32, device=workspace.device)
+    with torch.cuda.device(workspace.device):
+        _check(lib().gf_diag_contour_nodes(ctypes.byref(params), n_rad, n_ang, workspace.data_ptr(), rad_nodes.data_ptr(),
+                                           rad_weights.data_ptr(), x.real, x.imag, pol.data_ptr(), y.data_ptr(),
+                                           wy.data_ptr(), _stream(stream)))
+    return int(pol.item()), y, wy
 
 
 def diag_dfma_issue(mode, blocks, threads, iters, sink, stream=None):

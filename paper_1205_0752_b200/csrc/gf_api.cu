@@ -80,6 +80,15 @@ int check_prop(const gf_propagator& p, const char* name) {
   return GF_OK;
 }
 
+// index of the smallest rung >= v of the ladder {2^k, 1.5 2^k}: rung I is 2^(I/2) for even I, 1.5 2^((I-1)/2) for odd I
+int rung_index(double v) {
+  int e;
+  const double m = std::frexp(v, &e);   // v = m 2^e, 0.5 <= m < 1
+  if (m == 0.5) return 2 * (e - 1);
+  if (m <= 0.75) return 2 * (e - 1) + 1;
+  return 2 * e;
+}
+
 // validate everything that does not need a pointer, and build the kernel arguments
 int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, EvalArgs* a) {
   if (!p) { set_error("eval_grid: params is null"); return GF_ERR_NULL; }
@@ -118,9 +127,6 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   log_ratio_dd(0.0, p->cutoff2, p->map_scale, &a->Llog_hi, &a->Llog_lo);  // REAL contour: [0, Lambda^2]
   a->contour = p->contour;
   a->routing = p->routing;
-  a->th5 = 0.75 * 3.14159265358979323846;  // 3 pi/4, correctly rounded
-  a->cos_th5 = std::cos(a->th5);
-  a->sin_th5 = std::sin(a->th5);
 
   // line 2 as a sum of simple poles R_r/(u + mu_r)
   const gf_propagator& q = p->line_pk;
@@ -148,6 +154,24 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   }
   a->thread_ok = p->line_k.kind == GF_PROP_MASSIVE && q.kind == GF_PROP_MASSIVE && p->line_k.m2_im == 0 &&
                  q.m2_im == 0 && p->line_k.m2_re == q.m2_re && q.m2_re > 0;
+  a->same_mass = p->line_k.kind == GF_PROP_MASSIVE && q.kind == GF_PROP_MASSIVE && p->line_k.m2_re == q.m2_re &&
+                 p->line_k.m2_im == q.m2_im;
+  // AUTO's parabola: (Re sqrt(mu))^2 = (|mu| + Re mu)/2, the smallest over the poles -mu of line 2 (gf.h, gf_contour)
+  {
+    auto c2 = [](double mr, double mi) { return 0.5 * (std::sqrt(std::fma(mr, mr, mi * mi)) + mr); };
+    if (q.kind == GF_PROP_MASSIVE) a->parab_c2 = c2(q.m2_re, q.m2_im);
+    else {
+      const double disc = q.a * q.a - 4.0 * q.b;
+      if (disc >= 0.0) {
+        const double r = std::sqrt(disc);
+        a->parab_c2 = std::fmin(c2(0.5 * (q.a - r), 0.0), c2(0.5 * (q.a + r), 0.0));
+      } else {
+        a->parab_c2 = c2(0.5 * q.a, 0.5 * std::sqrt(-disc));
+      }
+    }
+  }
+  // the ladder of contour radii {2^k, 1.5 2^k} starts one rung below the smallest rung >= 1.5 sc (gf.h, gf_contour)
+  a->rung_lo = rung_index(1.5 * a->line2_scale) - 1;
   if (p->contour == GF_CONTOUR_THREAD && !a->thread_ok) {
     set_error("eval_grid: the THREAD contour needs equal real positive masses on both lines");
     return GF_ERR_UNSUPPORTED;
@@ -493,6 +517,23 @@ int gf_diag_radial_map(double cutoff2, double map_scale, const double* d_nodes, 
   double hi, lo;
   log_ratio_dd(0.0, cutoff2, map_scale, &hi, &lo);
   return launch_radial_map(hi, lo, map_scale, d_nodes, n, d_y, static_cast<cudaStream_t>(stream));
+}
+
+int gf_diag_contour_nodes(const gf_params* p, int n_rad, int n_ang, const void* d_workspace, const double* d_rad_nodes,
+                          const double* d_rad_weights, double x_re, double x_im, int* d_policy, void* d_y, void* d_wy,
+                          void* stream) {
+  EvalArgs a;
+  int rc = build_args(p, n_rad, n_ang, 1, &a);
+  if (rc) return rc;
+  if (p->contour == GF_CONTOUR_REAL) { set_error("diag_contour_nodes: a deformed contour policy (or AUTO) is needed"); return GF_ERR_ARG; }
+  if (!d_workspace || !d_rad_nodes || !d_rad_weights || !d_policy || !d_y || !d_wy) { set_error("diag_contour_nodes: null pointer"); return GF_ERR_NULL; }
+  if (!std::isfinite(x_re) || !std::isfinite(x_im)) { set_error("diag_contour_nodes: x is not finite"); return GF_ERR_ARG; }
+  LaunchPlan plan;
+  if ((rc = plan_eval(a, p->precision, &plan))) return rc;
+  a.rad_nodes = d_rad_nodes;
+  a.rad_weights = d_rad_weights;
+  return launch_contour_nodes(a, plan, static_cast<const double*>(d_workspace), x_re, x_im, d_policy,
+                              static_cast<double2*>(d_y), static_cast<double2*>(d_wy), static_cast<cudaStream_t>(stream));
 }
 
 int gf_diag_dfma_issue(int mode, int blocks, int threads, long long iters, double* d_sink, void* stream) {

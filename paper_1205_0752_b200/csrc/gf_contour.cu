@@ -1,23 +1,28 @@
 // gf_contour.cu -- Step 3 inside Kernel 2: evaluation on radial contours
 // that depend on the grid point.  The paper's Kernel 2 picks one of four hand-made contours per thread
 // with an IF-THEN-ELSE on the region of x; here each thread builds its contour from x by one of the
-// policies of DESIGN.md "Contour policies" and walks its n_rad nodes:
+// policies of include/gf.h (gf_contour) and walks its nodes:
 //
 //   REAL     [0, Lambda^2], shifted-log map (nodes prepared once per launch, as in gf_eval.cu);
-//   RAY_ARC  ray y = r e^{i arg x}, r in [0,R] shifted-log (n_rad/2 nodes), arc R e^{i theta} back to the real
-//            axis (n_rad/4), real tail [R, Lambda^2] shifted-log (n_rad/4);  R = 1.5 (sqrt|x| + sqrt(|x|+sc))^2
-//            with sc the size of line 2's singular structure, capped at Lambda^2/2
-//            (generalises the paper's region-2/5 contour);
+//   RAY_ARC  ray y = r x/|x|, r in [0,R] shifted-log (n_rad/2 nodes), arc of |y| = R back to the real axis
+//            (n_rad/4), real tail [R, Lambda^2] shifted-log (n_rad/4);  R the smallest rung of the ladder
+//            {2^k, 1.5 2^k} above 1.5 (sqrt|x| + sqrt(|x|+sc))^2, sc the size of line 2's singular structure,
+//            Lambda^2/2 beyond the ladder (generalises the paper's region-2/5 contour);
 //   THREAD   equal real masses, next to the negative axis below -4 m^2: five straight pieces through
 //            the waypoints W0..W5 that pass the pole of line 1 and thread the opening of the cut at
-//            |x + m^2| e^{i arg x}, an arc from 3 pi/4 to 0 and the real tail (n_rad/8 nodes each, n_rad/4
+//            |x + m^2| x/|x|, an arc from 3 pi/4 to 0 and the real tail (n_rad/8 nodes each, n_rad/4
 //            on the tail); mirrored for Im x < 0 (the analogue of the region-3/4 polylines);
-//   AUTO     per point: RAY_ARC outside the wedge {Re x < -sc, |Im x| n_ang sc < 5 |x|^2}, inside it THREAD
-//            where it applies and Re x <= -4.1 sc, else REAL.
+//   AUTO     per point: REAL inside the parabola where it is the continuation, THREAD next to the cut, RAY_ARC
+//            elsewhere (auto_policy below).
 //
-// The geometry is written with the _rn intrinsics in the order DESIGN.md states it, so that region tests
-// and waypoints do not depend on contraction; sqrt is correctly rounded; atan2, sincos, hypot, log, expm1
-// are the device's (within 1-2 ulp; the sums are insensitive to that).
+// The geometry uses no angle: the direction of the ray is x/|x| by two correctly rounded divisions, arcs are the
+// rational parametrisation y = R ((1 + i tau v)/(1 - i tau v))^2, every operation is a +, -, *, /, sqrt written
+// with the _rn intrinsics in the order gf.h states, so the nodes are the same doubles as the oracle's on any IEEE
+// machine.  Because R comes from a ladder, the radial nodes of the ray and of the real tail do not depend on x
+// beyond the choice of the rung: a preparation kernel maps them once per launch (one CTA per rung, in
+// double-double, correctly rounded like the REAL contour's, reading G18) together with the tail's node
+// prefactors and its Rhat tables, so the large-y part of the real tail costs one tail series per point as on
+// the REAL contour (gf_routes.cuh, tail_series).
 // Per node the angular sum is the same folded sum S(eta, zeta) as on the REAL contour (gf_routes.cuh):
 // with complex y, eta = (x + y + mu)/(4y) and zeta = (x + y + mu)^2/(4xy) are simply complex.
 #include "gf_routes.cuh"
@@ -25,16 +30,8 @@
 namespace gf {
 namespace {
 
-enum { SEG_TABLE = 0, SEG_LOG = 1, SEG_LINE = 2, SEG_ARC = 3 };
-constexpr int kMaxSeg = 7;
-
-// One piece of a contour.  off/n: its Gauss-Legendre rule inside the pyramid; start: index of its first
-// node among the point's n_rad nodes.  p[]: LOG  a, L_hi, L_lo, dir.re, dir.im, a + s0;
-// LINE a.re, a.im, (b-a).re, (b-a).im;  ARC  R, theta0, theta1 - theta0.
-struct Seg {
-  int type, off, n, start;
-  double p[6];
-};
+// tan(3 pi/16): the far waypoint of THREAD sits at the angle 3 pi/4 = 4 atan(kTau5)
+constexpr double kTau5 = 0.66817863791929891999775768652308;
 
 // ln(v) for a double-double v >= 1: libm seed, one Newton step on exp in double-double
 __device__ dd dd_log(dd v) {
@@ -44,26 +41,80 @@ __device__ dd dd_log(dd v) {
   return quick_two_sum(l0, c.hi);
 }
 
-__device__ void seg_log(Seg& s, double a, double b, double s0, double dre, double dim, int off, int n) {
-  // L = ln((b + s0)/(a + s0)) (readings G3/G4)
-  const dd L = dd_log(dd_div(two_sum(b, s0), two_sum(a, s0)));
-  s.type = SEG_LOG; s.off = off; s.n = n;
-  s.p[0] = a; s.p[1] = L.hi; s.p[2] = L.lo; s.p[3] = dre; s.p[4] = dim; s.p[5] = __dadd_rn(a, s0);
+// ---- the ladder of contour radii -------------------------------------------------------------------
+__device__ __forceinline__ int rung_index_dev(double v) {
+  int e;
+  const double m = frexp(v, &e);   // v = m 2^e, 0.5 <= m < 1 (exact)
+  if (m == 0.5) return 2 * (e - 1);
+  if (m <= 0.75) return 2 * (e - 1) + 1;
+  return 2 * e;
 }
-__device__ void seg_line(Seg& s, cd a, cd b, int off, int n) {
-  s.type = SEG_LINE; s.off = off; s.n = n;
-  s.p[0] = a.re; s.p[1] = a.im; s.p[2] = __dadd_rn(b.re, -a.re); s.p[3] = __dadd_rn(b.im, -a.im);
-  s.p[4] = s.p[5] = 0.0;
-}
-__device__ void seg_arc(Seg& s, double R, double th0, double th1, int off, int n) {
-  s.type = SEG_ARC; s.off = off; s.n = n;
-  s.p[0] = R; s.p[1] = th0; s.p[2] = __dadd_rn(th1, -th0);
-  s.p[3] = s.p[4] = s.p[5] = 0.0;
+__device__ __forceinline__ double rung_value(int I) { return (I & 1) ? ldexp(1.5, (I - 1) >> 1) : ldexp(1.0, I >> 1); }
+// smallest rung >= Rstar (not below the first tabulated one); *row: its row in the rung tables
+__device__ __forceinline__ double contour_radius(const EvalArgs& a, double Rstar, int* row) {
+  int I = rung_index_dev(Rstar);
+  if (I < a.rung_lo) I = a.rung_lo;
+  const double R = rung_value(I);
+  if (I > a.rung_lo + kRungs - 1 || !(R < 0.5 * a.cutoff2)) {
+    *row = kRungs;
+    return 0.5 * a.cutoff2;
+  }
+  *row = I - a.rung_lo;
+  return R;
 }
 
-// AUTO's per-point choice; half-open tests exactly as DESIGN.md writes them
-__device__ int auto_policy(const EvalArgs& a, double xr, double xi) {
-  const double sc = a.line2_scale;
+// ---- the geometry of one point's contour ------------------------------------------------------------
+struct Geo {
+  int pol;           // GF_CONTOUR_REAL / RAY_ARC / THREAD
+  int mirror;        // THREAD for Im x < 0: conjugate every node
+  int row;           // row of the rung tables
+  double R;          // contour radius
+  double dre, dim;   // direction x/|x| of the ray (THREAD: of x mirrored into Im x >= 0)
+  double tau;        // arc: tan(phi/4)
+  double Aa, r0, m2; // THREAD: (sqrt|x| - m)^2, |x + m^2|, m^2
+};
+
+// x/|x| by correctly rounded operations, x scaled by a power of two first so that no square underflows; *ax = |x|
+__device__ __forceinline__ void ray_direction(double xr, double xi, double* dre, double* dim, double* ax) {
+  const double big = fmax(fabs(xr), fabs(xi));
+  if (big == 0.0) { *ax = 0.0; *dre = 1.0; *dim = 0.0; return; }
+  int e;
+  frexp(big, &e);
+  const double sr = ldexp(xr, -e), si = ldexp(xi, -e);
+  const double as = __dsqrt_rn(__fma_rn(sr, sr, __dmul_rn(si, si)));
+  *ax = ldexp(as, e);
+  *dre = __ddiv_rn(sr, as);
+  *dim = __ddiv_rn(si, as);
+}
+// tan(phi/4) of the direction (c, s) = (cos phi, sin phi), |phi| <= pi, by half-angle formulas without cancellation
+__device__ __forceinline__ double tan_quarter(double c, double s) {
+  double ch, sh;
+  if (c >= 0.0) {
+    ch = __dsqrt_rn(__dmul_rn(0.5, __dadd_rn(1.0, c)));
+    sh = __ddiv_rn(__dmul_rn(0.5, s), ch);
+  } else {
+    sh = copysign(__dsqrt_rn(__dmul_rn(0.5, __dadd_rn(1.0, -c))), s);
+    ch = __ddiv_rn(__dmul_rn(0.5, fabs(s)), fabs(sh));
+  }
+  return __ddiv_rn(sh, __dadd_rn(1.0, ch));
+}
+__device__ __forceinline__ bool in_parabola(double xr, double xi, double cc) {
+  const double t = __dadd_rn(xr, cc);
+  return t > 0.0 && __dmul_rn(xi, xi) < __dmul_rn(__dmul_rn(4.0, cc), t);
+}
+
+// AUTO's per-point choice; half-open tests exactly as gf.h writes them:
+//   1. inside the parabola of half the size (|Im sqrt x| < 0.71 Re sqrt mu): REAL, exact and the cheapest;
+//   2. next to the negative real axis (|Im x| n_rad < 80 |Re x|), where the ray of RAY_ARC passes the pole of line 1
+//      and the opening of the cut closer than the radial rule resolves: REAL as long as x is inside the parabola;
+//   3. in the wedge {Re x < -sc, |Im x| n_ang sc < 5 |x|^2}: THREAD where it applies and Re x <= -4.1 sc, else REAL
+//      (bounded and reproducible, NOT the continuation: the documented limitation);
+//   4. RAY_ARC everywhere else.
+__device__ __forceinline__ int auto_policy(const EvalArgs& a, double xr, double xi) {
+  const double sc = a.line2_scale, c2 = a.parab_c2;
+  if (in_parabola(xr, xi, __dmul_rn(0.5, c2))) return GF_CONTOUR_REAL;
+  const bool near_axis = xr < 0.0 && __dmul_rn(fabs(xi), (double)a.n_rad) < __dmul_rn(80.0, fabs(xr));
+  if (near_axis && in_parabola(xr, xi, c2)) return GF_CONTOUR_REAL;
   const double ax2 = __fma_rn(xr, xr, __dmul_rn(xi, xi));
   const bool wedge = (xr < -sc) && (__dmul_rn(fabs(xi), __dmul_rn((double)a.n_ang, sc)) < __dmul_rn(5.0, ax2));
   if (!wedge) return GF_CONTOUR_RAY_ARC;
@@ -71,57 +122,98 @@ __device__ int auto_policy(const EvalArgs& a, double xr, double xi) {
   return GF_CONTOUR_REAL;
 }
 
-// Build the segments of the point's contour; returns their number.  *mirror: conjugate every node.
-__device__ int build_contour(const EvalArgs& a, int pol, double xr, double xi, Seg* seg, bool* mirror) {
-  const int n = a.n_rad, o1 = n, o2 = n + n / 2, o3 = n + n / 2 + n / 4;
-  *mirror = false;
-  int ns = 0;
-  if (pol == GF_CONTOUR_REAL) {
-    seg[0].type = SEG_TABLE; seg[0].off = 0; seg[0].n = n;
-    ns = 1;
-  } else if (pol == GF_CONTOUR_RAY_ARC) {
-    const double ax = __dsqrt_rn(__fma_rn(xr, xr, __dmul_rn(xi, xi)));
-    const double phi = atan2(xi, xr);
+__device__ __forceinline__ Geo build_geo(const EvalArgs& a, double xr, double xi) {
+  Geo g = {};
+  g.pol = a.contour == GF_CONTOUR_AUTO ? auto_policy(a, xr, xi) : a.contour;
+  g.dre = 1.0;
+  if (g.pol == GF_CONTOUR_RAY_ARC) {
+    double ax;
+    ray_direction(xr, xi, &g.dre, &g.dim, &ax);
     const double q = __dadd_rn(__dsqrt_rn(ax), __dsqrt_rn(__dadd_rn(ax, a.line2_scale)));
-    const double R = fmin(__dmul_rn(__dmul_rn(1.5, q), q), 0.5 * a.cutoff2);
-    double sn, cs;
-    sincos(phi, &sn, &cs);
-    seg_log(seg[0], 0.0, R, a.s0, cs, sn, o1, n / 2);
-    seg_arc(seg[1], R, phi, 0.0, o2, n / 4);
-    seg_log(seg[2], R, a.cutoff2, a.s0, 1.0, 0.0, o2, n / 4);
-    ns = 3;
-  } else {
-    *mirror = xi < 0.0;
+    g.R = contour_radius(a, __dmul_rn(__dmul_rn(1.5, q), q), &g.row);
+    g.tau = tan_quarter(g.dre, g.dim);
+  } else if (g.pol == GF_CONTOUR_THREAD) {
+    g.mirror = xi < 0.0;
     const double yi = fabs(xi);
-    const double m2 = a.term[0].mu_re, m = __dsqrt_rn(m2);
-    const double s = __dsqrt_rn(__fma_rn(xr, xr, __dmul_rn(yi, yi)));
-    const double phi = atan2(yi, xr);
-    const double rs = __dsqrt_rn(s);
+    double s;
+    ray_direction(xr, yi, &g.dre, &g.dim, &s);
+    g.m2 = a.term[0].mu_re;
+    const double m = __dsqrt_rn(g.m2), rs = __dsqrt_rn(s);
     const double dm = __dadd_rn(rs, -m), dp = __dadd_rn(rs, m);
-    const double Aa = __dmul_rn(dm, dm), Bb = __dmul_rn(dp, dp);
-    const double r0 = hypot(__dadd_rn(xr, m2), yi);
-    double sn, cs;
-    sincos(phi, &sn, &cs);
-    cd W[6];
-    W[0] = {0.0, 0.0};
-    W[1] = {-m2, __dmul_rn(0.5, __dadd_rn(Aa, -m2))};
-    const double h2 = __dmul_rn(0.5, __dadd_rn(Aa, m2));
-    W[2] = {__dmul_rn(h2, cs), __dmul_rn(h2, sn)};
-    W[3] = {__dmul_rn(-0.5, __dadd_rn(Aa, r0)), __dmul_rn(-0.5, __dadd_rn(r0, -Aa))};
-    W[4] = {__dmul_rn(r0, cs), __dmul_rn(r0, sn)};
-    const double R = fmin(__dmul_rn(1.5, Bb), 0.5 * a.cutoff2);
-    W[5] = {__dmul_rn(R, a.cos_th5), __dmul_rn(R, a.sin_th5)};
-    for (int k = 0; k < 5; ++k) seg_line(seg[k], W[k], W[k + 1], o3, n / 8);
-    seg_arc(seg[5], R, a.th5, 0.0, o3, n / 8);
-    seg_log(seg[6], R, a.cutoff2, a.s0, 1.0, 0.0, o2, n / 4);
-    ns = 7;
+    g.Aa = __dmul_rn(dm, dm);
+    const double Bb = __dmul_rn(dp, dp);
+    const double t = __dadd_rn(xr, g.m2);
+    g.r0 = __dsqrt_rn(__fma_rn(t, t, __dmul_rn(yi, yi)));   // |x + m^2|
+    g.R = contour_radius(a, __dmul_rn(1.5, Bb), &g.row);
+    g.tau = kTau5;
   }
-  int start = 0;
-  for (int k = 0; k < ns; ++k) {
-    seg[k].start = start;
-    start += seg[k].n;
+  return g;
+}
+
+// the end of an arc of radius R at v = 1: R ((1 + i tau)/(1 - i tau))^2, in the arc's own arithmetic
+__device__ __forceinline__ cd arc_point(double R, double tv, double* in2_out) {
+  const double t2 = __dmul_rn(tv, tv);
+  const double n2 = __dadd_rn(1.0, t2);
+  const double in2 = __drcp_rn(n2);                                    // the one division of the node
+  const double gr = __dmul_rn(__dadd_rn(1.0, -t2), in2), gi = __dmul_rn(__dmul_rn(2.0, tv), in2);
+  const double gr2 = __dmul_rn(gr, gr), gi2 = __dmul_rn(gi, gi);
+  const double Er = __dadd_rn(gr2, -gi2), Ei = __dmul_rn(2.0, __dmul_rn(gr, gi));
+  *in2_out = in2;
+  return {__dmul_rn(R, Er), __dmul_rn(R, Ei)};
+}
+// waypoint W_k of THREAD (Im x >= 0 side), k = 0..5
+__device__ __forceinline__ cd thread_waypoint(const Geo& g, int k) {
+  switch (k) {
+    case 0: return {0.0, 0.0};
+    case 1: return {-g.m2, __dmul_rn(0.5, __dadd_rn(g.Aa, -g.m2))};
+    case 2: {
+      const double h2 = __dmul_rn(0.5, __dadd_rn(g.Aa, g.m2));
+      return {__dmul_rn(h2, g.dre), __dmul_rn(h2, g.dim)};
+    }
+    case 3: return {__dmul_rn(-0.5, __dadd_rn(g.Aa, g.r0)), __dmul_rn(-0.5, __dadd_rn(g.r0, -g.Aa))};
+    case 4: return {__dmul_rn(g.r0, g.dre), __dmul_rn(g.r0, g.dim)};
+    default: {
+      double in2;
+      return arc_point(g.R, kTau5, &in2);
+    }
   }
-  return ns;
+}
+
+// Where node g of the point's n_rad nodes lives.  type, index i inside its piece, and for LINE the piece k.
+enum { SEG_TABLE = 0, SEG_RAY = 1, SEG_LINE = 2, SEG_ARC = 3, SEG_TAIL = 4 };
+struct NodeAt {
+  int type, i, k, rule;   // rule: offset of the piece's Gauss-Legendre rule inside the staged levels 2 and 3
+};
+__device__ __forceinline__ NodeAt locate(int pol, int n_rad, int g) {
+  const int n2 = n_rad >> 1, n4 = n_rad >> 2, n8 = n_rad >> 3;
+  if (pol == GF_CONTOUR_REAL) return {SEG_TABLE, g, 0, 0};
+  if (pol == GF_CONTOUR_RAY_ARC) {
+    if (g < n2) return {SEG_RAY, g, 0, 0};
+    if (g < n2 + n4) return {SEG_ARC, g - n2, 0, 0};
+    return {SEG_TAIL, g - n2 - n4, 0, 0};
+  }
+  if (g < 5 * n8) { const int k = g / n8; return {SEG_LINE, g - k * n8, k, n4}; }
+  if (g < 6 * n8) return {SEG_ARC, g - 5 * n8, 0, n4};
+  return {SEG_TAIL, g - 6 * n8, 0, 0};
+}
+// index of the first node of the real tail piece
+__device__ __forceinline__ int tail_start(int pol, int n_rad) {
+  return pol == GF_CONTOUR_REAL ? 0 : n_rad - (n_rad >> 2);
+}
+
+// node of a straight piece a -> a + d and of an arc: y and (rule weight) x dy/dt
+__device__ __forceinline__ void line_node(cd a, cd d, double t, double w, cd* y, cd* wy) {
+  const double u = __dmul_rn(0.5, __dadd_rn(t, 1.0)), hw = __dmul_rn(0.5, w);
+  *y = {__dadd_rn(a.re, __dmul_rn(d.re, u)), __dadd_rn(a.im, __dmul_rn(d.im, u))};
+  *wy = {__dmul_rn(d.re, hw), __dmul_rn(d.im, hw)};
+}
+__device__ __forceinline__ void arc_node(double R, double tau, double t, double w, cd* y, cd* wy) {
+  const double u = __dmul_rn(0.5, __dadd_rn(t, 1.0));
+  const double v = __dadd_rn(1.0, -u);
+  double in2;
+  *y = arc_point(R, __dmul_rn(tau, v), &in2);
+  const double f = __dmul_rn(__dmul_rn(__dmul_rn(2.0, tau), w), in2);
+  *wy = {__dmul_rn(f, y->im), -__dmul_rn(f, y->re)};   // -i f y
 }
 
 // D1(y) for complex y
@@ -134,11 +226,67 @@ __device__ __forceinline__ cd line_k_complex(const gf_propagator& p, cd y) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// Rung tables (one CTA per row): the ray's and the real tail's nodes for the contour radius R_k, the tail's node
+// prefactors pref_{r,i} = c0 Wr_i y_i D1(y_i) (-R_r/(y_i + mu_r)) and its Rhat tables.  Rows whose radius is not
+// below Lambda^2/2 are never read and stay unwritten; the last row is R = Lambda^2/2.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) prep_rungs_kernel(const __grid_constant__ EvalArgs a,
+                                                         const __grid_constant__ BlobLayout L,
+                                                         double* __restrict__ blob) {
+  const int k = blockIdx.x;
+  double R = 0.5 * a.cutoff2;
+  if (k < kRungs) {
+    R = rung_value(a.rung_lo + k);
+    if (!(R < 0.5 * a.cutoff2)) return;
+  }
+  double* row = blob + L.off_rung + (long long)k * L.rung_stride;
+  const int n = a.n_rad, n2 = n >> 1, n4 = n >> 2;
+  // ray: r(u) = s0 expm1(u L), L = ln((R + s0)/s0), dr = (w/2) L (r + s0)            (level 1 of the pyramid)
+  const dd L1 = dd_log(dd_div_d(two_sum(R, a.s0), a.s0));
+  for (int i = threadIdx.x; i < n2; i += blockDim.x) {
+    const double t = a.rad_nodes[n + i], w = a.rad_weights[n + i];
+    const double r = radial_node(t, L1, a.s0);
+    const double dr = dd_mul(dd_mul_d(L1, 0.5 * w), two_sum(r, a.s0)).hi;
+    row[L.rg_r + i] = r;
+    row[L.rg_q4 + i] = 0.25 / r;
+    row[L.rg_w + i] = a.c0 * r * dr;
+  }
+  // real tail: y(u) = R + (R + s0) expm1(u L), L = ln((Lambda^2 + s0)/(R + s0))      (level 2)
+  const dd as = two_sum(R, a.s0);
+  const dd L2 = dd_log(dd_div(two_sum(a.cutoff2, a.s0), as));
+  for (int i = threadIdx.x; i < L.n4p; i += blockDim.x) {
+    const int ii = min(i, n4 - 1);
+    const double t = a.rad_nodes[n + n2 + ii], w = i < n4 ? a.rad_weights[n + n2 + ii] : 0.0;
+    const double u = 0.5 * (t + 1.0);
+    const double y = dd_add_d(dd_mul(as, dd_expm1(dd_mul_d(L2, u))), R).hi;
+    const double dy = dd_mul(dd_mul_d(L2, 0.5 * w), two_sum(y, a.s0)).hi;
+    row[L.rg_y + i] = y;
+    row[L.rg_yq4 + i] = 0.25 / y;
+    const cd d1 = cscale(line_k_real(a.line_k, y), a.c0 * dy * y);
+    for (int r = 0; r < a.n_terms; ++r) {
+      const cd ic = cinv(cd{y + a.term[r].mu_re, a.term[r].mu_im});
+      const cd pr = cmul(cmul(d1, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);
+      row[L.rg_pref + 2 * (r * L.n4p + i)] = pr.re;
+      row[L.rg_pref + 2 * (r * L.n4p + i) + 1] = pr.im;
+    }
+  }
+  __syncthreads();
+  const TailJob J = {n4, a.n_terms, L.n4p, row + L.rg_y, row + L.rg_pref, reinterpret_cast<double2*>(row + L.rg_tail),
+                     row + L.rg_s2, row + L.rg_s3};
+  prep_tail_powers(J);
+  __syncthreads();
+  prep_tail_sums(J);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Evaluation on point-dependent contours.  Same staging, lane split, routes, reductions and store as
 // eval_real_kernel; counters as there.
 // ---------------------------------------------------------------------------------------------
+#ifndef GF_CONTOUR_MIN_BLOCKS
+#define GF_CONTOUR_MIN_BLOCKS 2
+#endif
 template <bool COUNT>
-__global__ void __launch_bounds__(kBlockThreads, 2)
+__global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
     eval_contour_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                         const double* __restrict__ blob, unsigned long long* __restrict__ counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -150,9 +298,6 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   mbar_wait(bar, 0);
 
   const Tabs<double> tb = make_tabs<double>(sb, L, a.n_pairs);
-  const double* sy = sb + L.off_y;
-  const double* sq4 = sb + L.off_q4;
-  const double2* spref = reinterpret_cast<const double2*>(sb + L.off_pref);
   const double* srt = sb + L.off_rt;
   const double* srw = sb + L.off_rw;
   const bool bad_rule = sb[0] != 0.0;
@@ -180,58 +325,83 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   }
   const cd xinv = cinv(x);
 
-  Seg seg[kMaxSeg];
-  bool mirror;
-  const int pol = a.contour == GF_CONTOUR_AUTO ? auto_policy(a, x.re, x.im) : a.contour;
-  const int n_seg = build_contour(a, pol, x.re, x.im, seg, &mirror);
+  const Geo geo = build_geo(a, x.re, x.im);
+  const cd dir2 = {fma(geo.dre, geo.dre, -(geo.dim * geo.dim)), 2.0 * geo.dre * geo.dim};
+  // tables of the real nodes this point walks: the REAL contour's (policy REAL) or its rung's tail piece
+  const double* row = blob + L.off_rung + (long long)geo.row * L.rung_stride;
+  const bool real_pol = geo.pol == GF_CONTOUR_REAL;
+  const double* ty = real_pol ? blob + L.off_y : row + L.rg_y;
+  const double* tq4 = real_pol ? blob + L.off_q4 : row + L.rg_yq4;
+  const double2* tpref = reinterpret_cast<const double2*>(real_pol ? blob + L.off_pref : row + L.rg_pref);
+  const int tstride = real_pol ? L.n_rad_pad : L.n4p;
+  const int tn = real_pol ? a.n_rad : a.n_rad >> 2;
+  const int t0 = tail_start(geo.pol, a.n_rad);
+
+  // where the tail series takes over: the first real node with y >= Y0 = 4 (sqrt|x| + sqrt(|x| + |x + mu|))^2
+  int i_end;
+  {
+    const double ax = sqrt(fma(x.re, x.re, x.im * x.im));
+    double Y0 = 0.0;
+    for (int r = 0; r < a.n_terms; ++r) {
+      const cd az = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
+      const double q = sqrt(ax) + sqrt(ax + sqrt(fma(az.re, az.re, az.im * az.im)));
+      Y0 = fmax(Y0, kTailFactor * q * q);
+    }
+    int lo = 0, hi = tn;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (ty[mid] < Y0) lo = mid + 1; else hi = mid;
+    }
+    i_end = lo;
+  }
+  const int g_end = t0 + i_end;
+  const int g_stop = __reduce_max_sync(0xffffffffu, g_end);
 
   RouteCount rc;
   double g_re = 0.0, g_im = 0.0;
-  int ks = 0;
-  // warp-synchronous node loop (node_term is warp-collective): a lane past the last node repeats it with weight 0
+  int k_line = -1;           // the straight piece whose end points are in la, ld
+  cd la = {0.0, 0.0}, ld = {0.0, 0.0};
+  // warp-synchronous node loop (node_term is warp-collective): a lane past its last node repeats it with weight 0
 #pragma unroll 1
-  for (int g0 = 0; g0 < a.n_rad; g0 += S) {
-    const bool valid = g0 + sub < a.n_rad;
-    const int g = valid ? g0 + sub : a.n_rad - 1;
-    while (ks + 1 < n_seg && g >= seg[ks].start + seg[ks].n) ++ks;
-    const Seg& sg = seg[ks];
-    const int i = g - sg.start;
-    // ---- the node: y and (rule weight) x dy/dt
-    cd y, wy = {0.0, 0.0}, q4;
-    const bool table = sg.type == SEG_TABLE;
+  for (int g0 = 0; g0 < g_stop; g0 += S) {
+    const bool valid = g0 + sub < g_end;
+    const int g = valid ? g0 + sub : g_end - 1 + (g_end == 0);
+    const NodeAt at = locate(geo.pol, a.n_rad, g);
+    // ---- the node: y, 1/(4y), and the prefactor c0 (rule weight) dy/dt y D1(y) without the pole factors
+    cd y, q4, base = {0.0, 0.0};
+    const bool table = at.type == SEG_TABLE || at.type == SEG_TAIL;
     if (table) {
-      y = {sy[i], 0.0};
-      q4 = {sq4[i], 0.0};
+      y = {ty[at.i], 0.0};
+      q4 = {tq4[at.i], 0.0};
+    } else if (at.type == SEG_RAY) {
+      const double r = row[L.rg_r + at.i], q4r = row[L.rg_q4 + at.i], rw = row[L.rg_w + at.i];
+      y = {__dmul_rn(geo.dre, r), __dmul_rn(geo.dim, r)};
+      q4 = {geo.dre * q4r, -geo.dim * q4r};
+      base = {dir2.re * rw, dir2.im * rw};          // c0 wy y = c0 dir^2 r dr
     } else {
-      const double t = srt[sg.off + i], w = srw[sg.off + i];
-      const double u = __dmul_rn(0.5, __dadd_rn(t, 1.0));
-      if (sg.type == SEG_LOG) {
-        // r = a + (a + s0) expm1(u L), dr = (w/2) L (r + s0); L = L_hi + L_lo
-        const dd uL = dd_mul_d(dd{sg.p[1], sg.p[2]}, u);
-        const double e1 = expm1(uL.hi);
-        const double E = fma(uL.lo, e1 + 1.0, e1);
-        const double r = fma(sg.p[5], E, sg.p[0]);
-        const double dr = 0.5 * w * sg.p[1] * (r + a.s0);
-        y = {sg.p[3] * r, sg.p[4] * r};
-        wy = {sg.p[3] * dr, sg.p[4] * dr};
-      } else if (sg.type == SEG_LINE) {
-        const double hw = __dmul_rn(0.5, w);
-        y = {__dadd_rn(sg.p[0], __dmul_rn(sg.p[2], u)), __dadd_rn(sg.p[1], __dmul_rn(sg.p[3], u))};
-        wy = {__dmul_rn(sg.p[2], hw), __dmul_rn(sg.p[3], hw)};
+      const double t = srt[at.rule + at.i], w = srw[at.rule + at.i];
+      cd wy;
+      if (at.type == SEG_LINE) {
+        if (at.k != k_line) {
+          k_line = at.k;
+          la = thread_waypoint(geo, at.k);
+          const cd lb = thread_waypoint(geo, at.k + 1);
+          ld = {__dadd_rn(lb.re, -la.re), __dadd_rn(lb.im, -la.im)};
+        }
+        line_node(la, ld, t, w, &y, &wy);
       } else {
-        const double th = __dadd_rn(sg.p[1], __dmul_rn(sg.p[2], u));
-        double sn, cs;
-        sincos(th, &sn, &cs);
-        y = {__dmul_rn(sg.p[0], cs), __dmul_rn(sg.p[0], sn)};
-        const double f = __dmul_rn(__dmul_rn(sg.p[2], 0.5), w);
-        wy = {__dmul_rn(-y.im, f), __dmul_rn(y.re, f)};  // i y dtheta
+        arc_node(geo.R, geo.tau, t, w, &y, &wy);
       }
-      if (mirror) { y.im = -y.im; wy.im = -wy.im; }
+      if (geo.mirror) { y.im = -y.im; wy.im = -wy.im; }
       q4 = cscale(cinv_fast(y), 0.25);
+      base = cscale(cmul(wy, y), a.c0);
     }
-    cd base = {0.0, 0.0};
-    if (!table) base = cscale(cmul(cmul(wy, y), line_k_complex(a.line_k, y)), a.c0);
     const cd xq = cmul(xinv, q4);                    // 1/(4 x y)
+    cd ic0 = {0.0, 0.0};
+    if (!table) {
+      if (a.same_mass) ic0 = cinv_fast(cd{y.re + a.term[0].mu_re, y.im + a.term[0].mu_im});
+      base = cmul(base, a.same_mass ? ic0 : line_k_complex(a.line_k, y));
+    }
 #pragma unroll 1
     for (int r = 0; r < a.n_terms; ++r) {
       const double mur = a.term[r].mu_re, mui = a.term[r].mu_im;
@@ -242,15 +412,30 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
       const cd s = node_term<double, COUNT>(tb, x, y, delta, zeta, mur, mui, rc);
       cd pr;
       if (table) {
-        const double2 p2 = spref[r * L.n_rad_pad + i];
+        const double2 p2 = tpref[r * tstride + at.i];
         pr = {p2.x, p2.y};
       } else {
-        const cd ic = cinv_fast(cd{y.re + mur, y.im + mui});
+        const cd ic = a.same_mass ? ic0 : cinv_fast(cd{y.re + mur, y.im + mui});
         pr = cmul(cmul(base, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);
       }
       if (!valid) pr = {0.0, 0.0};
       g_re = fma(pr.re, s.re, fma(-pr.im, s.im, g_re));
       g_im = fma(pr.re, s.im, fma(pr.im, s.re, g_im));
+    }
+  }
+  // the large-y part of the real piece, all nodes from i_end on at once
+  if (__any_sync(0xffffffffu, i_end < tn)) {
+    const double invy0 = 4.0 * tq4[min(i_end, tn - 1)];
+    const double2* Rt = reinterpret_cast<const double2*>(real_pol ? blob + L.off_tail : row + L.rg_tail) +
+                        (size_t)i_end * kTailN;
+    for (int r = 0; r < a.n_terms; ++r) {
+      const cd az = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
+      const cd tl = tail_series(sb + L.off_gam, Rt + (size_t)r * (tn + 1) * kTailN, x, az, invy0);
+      if (sub == 0) {
+        g_re += tl.re;
+        g_im += tl.im;
+      }
+      if (COUNT) ++rc.tails;
     }
   }
   for (int o = 1; o < S; o <<= 1) {
@@ -265,6 +450,46 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
     reinterpret_cast<double2*>(a.out)[point] = make_double2(g_re, g_im);
   }
   if (COUNT) flush_counters(rc, active, counters);
+}
+
+// The nodes the evaluation kernel walks for one x, read from the same tables by the same code (diagnostic:
+// tests compare them with the oracle's bit for bit).  One thread per node; wy = (rule weight) x dy/dt.
+__global__ void contour_nodes_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
+                                     const double* __restrict__ blob, double xr, double xi, int* __restrict__ policy,
+                                     double2* __restrict__ out_y, double2* __restrict__ out_wy) {
+  const Geo geo = build_geo(a, xr, xi);
+  if (blockIdx.x == 0 && threadIdx.x == 0) *policy = geo.pol;
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= a.n_rad) return;
+  const double* row = blob + L.off_rung + (long long)geo.row * L.rung_stride;
+  const NodeAt at = locate(geo.pol, a.n_rad, g);
+  cd y, wy;
+  if (at.type == SEG_TABLE) {
+    y = {blob[L.off_y + at.i], 0.0};
+    wy = {0.5 * a.rad_weights[at.i] * a.Llog_hi * (y.re + a.s0), 0.0};
+  } else if (at.type == SEG_TAIL) {
+    y = {row[L.rg_y + at.i], 0.0};
+    // the row keeps pref, not the weight: recover (rule weight) dy/dt from the map itself
+    const dd L2 = dd_log(dd_div(two_sum(a.cutoff2, a.s0), two_sum(geo.R, a.s0)));
+    wy = {0.5 * a.rad_weights[a.n_rad + a.n_rad / 2 + at.i] * L2.hi * (y.re + a.s0), 0.0};
+  } else if (at.type == SEG_RAY) {
+    const double r = row[L.rg_r + at.i];
+    y = {__dmul_rn(geo.dre, r), __dmul_rn(geo.dim, r)};
+    const double dr = row[L.rg_w + at.i] / (a.c0 * r);
+    wy = {geo.dre * dr, geo.dim * dr};
+  } else {
+    const int lvl2 = a.n_rad + a.n_rad / 2;
+    const double t = a.rad_nodes[lvl2 + at.rule + at.i], w = a.rad_weights[lvl2 + at.rule + at.i];
+    if (at.type == SEG_LINE) {
+      const cd la = thread_waypoint(geo, at.k), lb = thread_waypoint(geo, at.k + 1);
+      line_node(la, cd{__dadd_rn(lb.re, -la.re), __dadd_rn(lb.im, -la.im)}, t, w, &y, &wy);
+    } else {
+      arc_node(geo.R, geo.tau, t, w, &y, &wy);
+    }
+  }
+  if (geo.mirror) { y.im = -y.im; wy.im = -wy.im; }
+  out_y[g] = make_double2(y.re, y.im);
+  out_wy[g] = make_double2(wy.re, wy.im);
 }
 
 template <bool COUNT>
@@ -286,6 +511,18 @@ int launch_contour(const EvalArgs& a, const LaunchPlan& plan, const double* blob
                    cudaStream_t stream) {
   return d_counters ? launch_contour_t<true>(a, plan, blob, d_counters, stream)
                     : launch_contour_t<false>(a, plan, blob, nullptr, stream);
+}
+
+int launch_prepare_rungs(const EvalArgs& a, const LaunchPlan& plan, double* blob, cudaStream_t stream) {
+  prep_rungs_kernel<<<plan.layout.n_rungs, 256, 0, stream>>>(a, plan.layout, blob);
+  return check_cuda(cudaGetLastError(), "rung preparation kernel launch");
+}
+
+int launch_contour_nodes(const EvalArgs& a, const LaunchPlan& plan, const double* blob, double x_re, double x_im,
+                         int* d_policy, double2* d_y, double2* d_wy, cudaStream_t stream) {
+  contour_nodes_kernel<<<(a.n_rad + 127) / 128, 128, 0, stream>>>(a, plan.layout, blob, x_re, x_im, d_policy, d_y,
+                                                                 d_wy);
+  return check_cuda(cudaGetLastError(), "contour_nodes launch");
 }
 
 }  // namespace gf

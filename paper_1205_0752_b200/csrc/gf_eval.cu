@@ -54,18 +54,6 @@
 namespace gf {
 namespace {
 
-// D1(y) for real y (REAL contour): massive 1/(y + m2) or rational (y + M2)/(y^2 + a y + b).
-__device__ __forceinline__ cd line_k_real(const gf_propagator& p, double y) {
-  if (p.kind == GF_PROP_MASSIVE) return cinv(cd{y + p.m2_re, p.m2_im});
-  return cd{(y + p.M2) / fma(y, y + p.a, p.b), 0.0};
-}
-
-// y = s0 expm1(u L) in double-double, rounded once (readings G3/G4, G18)
-__device__ __forceinline__ double radial_node(double t, dd Llog, double s0) {
-  const double u = 0.5 * (t + 1.0);
-  return dd_mul_d(dd_expm1(dd_mul_d(Llog, u)), s0).hi;
-}
-
 __global__ void radial_map_kernel(double Lhi, double Llo, double s0, const double* __restrict__ nodes, int n,
                                   double* __restrict__ y) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -118,71 +106,29 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
       }
     }
   }
-  if (L.off_rt >= 0)  // point-dependent contours: the rule pyramid as given ("n arrays")
+  if (L.off_rt >= 0) {  // point-dependent contours: levels 2 and 3 of the rule pyramid as given ("n arrays",
+                        // PAPER.md:150; levels 0 and 1 are mapped once per launch: REAL tables, rung tables)
+    const int lvl2 = a.n_rad + a.n_rad / 2;
     for (int i = threadIdx.x; i < L.n_tab; i += blockDim.x) {
-      blob[L.off_rt + i] = a.rad_nodes[i];
-      blob[L.off_rw + i] = a.rad_weights[i];
+      blob[L.off_rt + i] = a.rad_nodes[lvl2 + i];
+      blob[L.off_rw + i] = a.rad_weights[lvl2 + i];
     }
+  }
   __syncthreads();  // the T_k(s_j) matrix, the monomial moments and the radial tables are complete
   prep_series_sums(a, L, blob, s_cpart);
   __syncthreads();
   prep_series_kreq(L, blob, s_lc);
   if (L.off_gam >= 0) {
     prep_tail_gamma(L, blob, s_part, s_mu, s_nu);
-    prep_tail_powers(a, L, blob);
+    const TailJob J = real_tail_job(a, L, blob);
+    prep_tail_powers(J);
     __syncthreads();
-    prep_tail_sums(a, L, blob);
+    prep_tail_sums(J);
   }
   if (threadIdx.x == 0) {
     blob[0] = bad ? 1.0 : 0.0;
     blob[1] = 0.0;
   }
-}
-
-// ---------------------------------------------------------------------------------------------
-// Tail: all radial nodes with y_i >= Y0(x) at once.  With a = x + mu, eps = 1/y:
-//   S(x, y) = sum_k omega^(k+1) [delta mu_k - nu_k],  omega = 4 x eps/(1 + a eps)^2,  delta = a eps/4
-//           = sum_n eps^n X h_n(X, Z),   X = 4x, Z = -a,   h_n = sum_{k<n} gamma_{n,k} X^k Z^(n-1-k)
-// (binomial series of (1 + a eps)^(-2k-2); gamma_{n,k} in gf_routes.cuh).  The series converges absolutely,
-// term n below 4^-n, for y >= Y0 = 4 (sqrt|x| + sqrt(|x| + |a|))^2, so
-//   sum_{i >= i0} pref_i S(x, y_i) = X sum_n h_n sum_{i >= i0} pref_i y_i^-n = (X/y_i0) sum_n h_n(X/y_i0, Z/y_i0) Rhat_n(i0)
-// with the x-independent tables Rhat_n(i0) made once per launch.  h_n is a real-coefficient polynomial in the
-// ratio of X and Z (the smaller over the larger) and is evaluated by the same second-order recurrence as the
-// angular series.  A log-mapped radial rule has most of its nodes in this tail (about 60 % on the production
-// scan), and they cost kTailN (kTailN + 1) DFMA per point instead of a series each.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ cd tail_series(const double* __restrict__ gam, const double2* __restrict__ Rrow, cd x,
-                                          cd a, double invy0) {
-  const cd X = {4.0 * x.re * invy0, 4.0 * x.im * invy0}, Z = {-a.re * invy0, -a.im * invy0};
-  const double nX = fma(X.re, X.re, X.im * X.im), nZ = fma(Z.re, Z.re, Z.im * Z.im);
-  const bool fwd = nX <= nZ;                        // powers of X/Z, else of Z/X
-  const cd base = fwd ? Z : X, oth = fwd ? X : Z;
-  const double inb = 1.0 / (fwd ? nZ : nX);
-  const cd rho = {fma(oth.re, base.re, oth.im * base.im) * inb, fma(oth.im, base.re, -(oth.re * base.im)) * inb};
-  const double rr = rho.re + rho.re, ns = -fma(rho.re, rho.re, rho.im * rho.im);
-  cd pw = {1.0, 0.0}, acc = {0.0, 0.0};
-  const double* row = gam;
-#pragma unroll 1
-  for (int n = 1; n <= kTailN; ++n) {
-    double b0 = 0.0, b1 = 0.0;
-    const double* c = fwd ? row + n - 1 : row;      // highest power of the ratio first
-    const int step = fwd ? -1 : 1;
-    if (n & 1) {
-      b0 = *c;
-      c += step;
-    }
-#pragma unroll 2
-    for (int j = n >> 1; j > 0; --j, c += 2 * step) {   // two coefficients per trip, roles of b0, b1 alternate
-      b1 = fma(rr, b0, fma(ns, b1, c[0]));
-      b0 = fma(rr, b1, fma(ns, b0, c[step]));
-    }
-    const cd P = {fma(-b1, rho.re, b0), b1 * rho.im};   // c_0 - c_1 conj(rho)
-    const double2 R = Rrow[n - 1];
-    acc = cadd(acc, cmul(cmul(P, pw), cd{R.x, R.y}));
-    pw = cmul(pw, base);
-    row += n;
-  }
-  return cmul(X, acc);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -336,38 +282,64 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
 
 }  // namespace
 
+// pyramid: the layout of the deformed-contour kernel (gf_contour.cu).  It stages the angular rule, the series
+// tables, levels 2 and 3 of the radial pyramid and the tail's gamma table; the REAL node tables (read by the points
+// AUTO sends to REAL), every Rhat table and the rung tables stay in global memory.
 BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail, bool sym) {
-  BlobLayout L;
+  BlobLayout L = {};
   L.npad = (n_pairs + 3) & ~3;
   L.kmc = kKmc;
-  int o = 2;  // header
-  auto take = [&](int n) { int at = o; o += (n + 1) & ~1; return at; };
-  L.off_t = take(L.npad);
-  L.off_tlo = take(L.npad);
-  L.off_w = take(L.npad);
-  L.off_mom = take(2 * L.kmc);
-  L.off_cheb = take(2 * L.kmc);
-  L.off_kreq = take(kKreqBins / 2);
+  long long o = 2;  // header
+  auto take = [&](long long n) { long long at = o; o += (n + 1) & ~1LL; return at; };
+  L.off_t = (int)take(L.npad);
+  L.off_tlo = (int)take(L.npad);
+  L.off_w = (int)take(L.npad);
+  L.off_mom = (int)take(2 * L.kmc);
+  L.off_cheb = (int)take(2 * L.kmc);
+  L.off_kreq = (int)take(kKreqBins / 2);
   L.n_rad_pad = (n_rad + 31) & ~31;
-  L.off_y = take(L.n_rad_pad);
-  L.off_q4 = take(L.n_rad_pad);
   L.n_pref = n_terms + (sym && tail ? 1 : 0);
-  L.off_pref = take(2 * L.n_pref * L.n_rad_pad);
+  auto take_nodes = [&]() {
+    L.off_y = (int)take(L.n_rad_pad);
+    L.off_q4 = (int)take(L.n_rad_pad);
+    L.off_pref = (int)take(2 * L.n_pref * L.n_rad_pad);
+  };
+  if (!pyramid) take_nodes();
   // four entries of slack below the float2 series tables (the software-pipelined loop reads them on its last trip),
   // then 2 float2 tables of kmc entries = 2 kmc doubles; FP32 variant: 2 float tables of npad entries = npad doubles
   take(4);
-  L.off_sf = take(2 * L.kmc);
-  L.off_f32 = f32 ? take(L.npad) : -1;
-  L.n_tab = pyramid ? n_rad + n_rad / 2 + n_rad / 4 + n_rad / 8 : 0;
-  L.off_rt = pyramid ? take(L.n_tab) : -1;
-  L.off_rw = pyramid ? take(L.n_tab) : -1;
-  L.off_gam = tail ? take(kTailN * (kTailN + 1) / 2) : -1;
-  L.off_gam2 = tail && sym ? take(kTailN * (kTailN + 1) / 2) : -1;
-  L.n_doubles = o;
-  L.off_tail = tail ? take(2 * L.n_pref * (n_rad + 1) * kTailN) : -1;
-  L.off_scratch = take(L.kmc * L.npad);
-  L.off_scratch2 = tail ? take(2 * kTailN * n_rad) : -1;
-  L.off_scratch3 = tail ? take(kTailN * n_rad + 2 * kTailChunks * (2 * L.n_pref * kTailN + kTailN)) : -1;
+  L.off_sf = (int)take(2 * L.kmc);
+  L.off_f32 = f32 ? (int)take(L.npad) : -1;
+  L.n_tab = pyramid ? n_rad / 4 + n_rad / 8 : 0;
+  L.off_rt = pyramid ? (int)take(L.n_tab) : -1;
+  L.off_rw = pyramid ? (int)take(L.n_tab) : -1;
+  L.off_gam = tail ? (int)take(kTailN * (kTailN + 1) / 2) : -1;
+  L.off_gam2 = tail && sym ? (int)take(kTailN * (kTailN + 1) / 2) : -1;
+  L.n_doubles = (int)o;
+  if (pyramid) take_nodes();
+  L.off_tail = tail ? (int)take(2LL * L.n_pref * (n_rad + 1) * kTailN) : -1;
+  L.off_scratch = (int)take((long long)L.kmc * L.npad);
+  L.off_scratch2 = tail ? (int)take(2LL * kTailN * n_rad) : -1;
+  L.off_scratch3 = tail ? (int)take((long long)kTailN * n_rad + 2 * kTailChunks * (2 * L.n_pref * kTailN + kTailN)) : -1;
+  L.n_rungs = 0;
+  if (pyramid && tail) {
+    const int n2 = n_rad / 2, n4 = n_rad / 4;
+    L.n4p = (n4 + 1) & ~1;
+    long long ro = 0;
+    auto rtake = [&](long long n) { long long at = ro; ro += (n + 1) & ~1LL; return (int)at; };
+    L.rg_r = rtake(n2);
+    L.rg_q4 = rtake(n2);
+    L.rg_w = rtake(n2);
+    L.rg_y = rtake(L.n4p);
+    L.rg_yq4 = rtake(L.n4p);
+    L.rg_pref = rtake(2LL * n_terms * L.n4p);
+    L.rg_tail = rtake(2LL * n_terms * (n4 + 1) * kTailN);
+    L.rg_s2 = rtake(2LL * kTailN * n4);
+    L.rg_s3 = rtake((long long)kTailN * n4 + 2 * kTailChunks * (2 * n_terms * kTailN + kTailN));
+    L.rung_stride = ro;
+    L.n_rungs = kRungs + 1;
+    L.off_rung = take(ro * L.n_rungs);
+  }
   L.n_total = o;
   return L;
 }
@@ -384,8 +356,8 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   plan->split_log2 = sl;
   const long long threads = a.n_points << sl;
   plan->grid_blocks = (threads + kBlockThreads - 1) / kBlockThreads;
-  plan->layout = make_blob_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes,
-                                 plan->shared_nodes, a.routing == 1);
+  plan->layout = make_blob_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes, true,
+                                 a.routing == 1);
   plan->smem_bytes = 16 + (size_t)plan->layout.n_doubles * sizeof(double);
   if (plan->smem_bytes > 200 * 1024) {
     set_error("eval_grid: tables need %zu bytes of shared memory (limit 200 KiB): reduce n_rad/n_ang",
@@ -439,7 +411,8 @@ int launch_prepare(const EvalArgs& a, int precision, double* blob, cudaStream_t 
   if (rc) return rc;
   if ((rc = check_variant(plan, precision))) return rc;
   prep_real_kernel<<<1, 256, 0, stream>>>(a, plan.layout, blob);
-  return check_cuda(cudaGetLastError(), "prep kernel launch");
+  if ((rc = check_cuda(cudaGetLastError(), "prep kernel launch"))) return rc;
+  return plan.shared_nodes ? GF_OK : launch_prepare_rungs(a, plan, blob, stream);
 }
 
 // Evaluation alone, from tables made by launch_prepare with the same params, orders and precision.

@@ -51,7 +51,10 @@ struct EvalArgs {
   int contour;         // gf_contour
   int routing;         // 0: eq. (19) (lines k, p-k); 1: symmetric (lines k + p/2, k - p/2)
   int thread_ok;       // THREAD applicable (equal real masses)
-  double th5, cos_th5, sin_th5;  // 3 pi/4 and its cos, sin as the host's libm rounds them (far waypoint of THREAD)
+  int same_mass;       // line 1 is 1/(y + mu_0) with the one pole of line 2: D1(y)/(y + mu) = 1/(y + mu)^2
+  double parab_c2;     // (Re sqrt(mu))^2, the smallest over the poles of line 2: REAL is the continuation inside the
+                       // parabola Re x > (Im x)^2/(4 c2) - c2 (AUTO's first test)
+  int rung_lo;         // ladder index of the first tabulated contour radius (deformed contours)
   int split_log2;      // lanes per grid point = 1 << split_log2
 };
 
@@ -77,8 +80,20 @@ struct BlobLayout {
   int off_scratch;              // preparation-only scratch: T_k(s_j) [npad][kmc]; tail: q_i^n (hi, lo) [kTailN][n_rad] x 2
   int off_scratch2;
   int off_scratch3;             // tail: Q_c(i) [kTailN][n_rad], run starts (double-double)
-  int n_total;                  // doubles to allocate
+  // deformed contours: one row of tables per contour radius R_k of the ladder (kRungs rungs + the cap Lambda^2/2),
+  // NOT staged.  Row k starts at off_rung + k rung_stride; inside a row (offsets in doubles):
+  //   rg_r, rg_q4 [n_rad/2]            ray |y| = r_i in [0, R_k] (shifted-log, correctly rounded), 1/(4 r_i)
+  //   rg_w [n_rad/2]                   c0 r_i dr_i  (dr_i = rule weight x dr/dt)
+  //   rg_y, rg_yq4 [n4p]               real tail y_i in [R_k, Lambda^2], 1/(4 y_i)     (n4p = n_rad/4 rounded up to even)
+  //   rg_pref double2 [n_terms][n4p]   node prefactors of the tail, as off_pref
+  //   rg_tail double2 [n_terms][n_rad/4 + 1][kTailN]   Rhat of the tail segment
+  //   rg_s2, rg_s3                     preparation-only scratch of the row
+  long long off_rung, rung_stride;
+  int n_rungs;                  // rows (kRungs + 1) or 0
+  int n4p, rg_r, rg_q4, rg_w, rg_y, rg_yq4, rg_pref, rg_tail, rg_s2, rg_s3;
+  long long n_total;            // doubles to allocate
 };
+constexpr int kRungs = 64;      // tabulated contour radii above the first (deformed contours); then Lambda^2/2
 
 struct LaunchPlan {
   int block_threads;
@@ -112,12 +127,15 @@ int launch_prepared(const EvalArgs& a, int precision, const double* blob, unsign
 // gf_contour.cu: evaluation kernel for contours that depend on the grid point (RAY_ARC, THREAD, AUTO)
 int launch_contour(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* d_counters,
                    cudaStream_t stream);
+int launch_prepare_rungs(const EvalArgs& a, const LaunchPlan& plan, double* blob, cudaStream_t stream);
+int launch_contour_nodes(const EvalArgs& a, const LaunchPlan& plan, const double* blob, double x_re, double x_im,
+                         int* d_policy, double2* d_y, double2* d_wy, cudaStream_t stream);
 int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d_nodes, int n, double* d_y,
                       cudaStream_t stream);
 
 // gf_cut.cu: the paper's Kernels 3 and 4 (a.x holds the y array / the x array, a.out the result)
 BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail,
-                            bool sym = false);  // gf_eval.cu
+                            bool sym = false);  // gf_eval.cu; pyramid: the layout of the deformed-contour kernel
 int launch_angular(const EvalArgs& a, double x_re, double x_im, cudaStream_t stream);
 int launch_cut_crossings(const EvalArgs& a, int n_z, int* d_out, cudaStream_t stream);
 

@@ -758,17 +758,27 @@ __device__ void prep_tail_gamma(const BlobLayout& L, double* blob, dd (*s_part)[
     if (L.off_gam2 >= 0) blob[L.off_gam2 + e] = dd_mul(s_mu[k], dd_binom(n + k, n - 1 - k)).hi;   // kappa_{n,k}
   }
 }
+// One set of Rhat tables: the n real nodes y[0..n) (ascending) with prefactors pref[r][i] = (re, im) at
+// pref[2 (r stride + i)], r < n_pref; out: double2 R[n_pref][n + 1][kTailN]; s2, s3: scratch of 2 kTailN n and
+// kTailN n + 2 kTailChunks (2 n_pref kTailN + kTailN) doubles.
+struct TailJob {
+  int n, n_pref, stride;
+  const double* y;
+  const double* pref;
+  double2* R;
+  double *s2, *s3;
+};
 // phase C: thread per node i: q_i^n, n = 1..kTailN, in double-double into the scratch (hi, lo) [n][i]
-__device__ void prep_tail_powers(const EvalArgs& a, const BlobLayout& L, double* blob) {
-  double* qhi = blob + L.off_scratch2;
-  double* qlo = qhi + (size_t)kTailN * a.n_rad;
-  for (int i = threadIdx.x; i < a.n_rad; i += blockDim.x) {
+__device__ void prep_tail_powers(const TailJob& J) {
+  double* qhi = J.s2;
+  double* qlo = qhi + (size_t)kTailN * J.n;
+  for (int i = threadIdx.x; i < J.n; i += blockDim.x) {
     dd q = {1.0, 0.0};
-    if (i + 1 < a.n_rad) q = dd_div(dd{blob[L.off_y + i], 0.0}, dd{blob[L.off_y + i + 1], 0.0});
+    if (i + 1 < J.n) q = dd_div(dd{J.y[i], 0.0}, dd{J.y[i + 1], 0.0});
     dd p = q;
     for (int n = 0; n < kTailN; ++n) {
-      qhi[(size_t)n * a.n_rad + i] = p.hi;
-      qlo[(size_t)n * a.n_rad + i] = p.lo;
+      qhi[(size_t)n * J.n + i] = p.hi;
+      qlo[(size_t)n * J.n + i] = p.lo;
       p = dd_mul(p, q);
     }
   }
@@ -778,28 +788,28 @@ __device__ void prep_tail_powers(const EvalArgs& a, const BlobLayout& L, double*
 // each run from 0 (L_c(i)) with the run's product of q (Q_c(i)); pass 2 folds the runs above c into the carry
 // Rhat(end of run c) in double-double and completes Rhat(i) = L_c(i) + Q_c(i) carry.
 constexpr int kTailChunks = 8;
-__device__ void prep_tail_sums(const EvalArgs& a, const BlobLayout& L, double* blob) {
-  const double* qhi = blob + L.off_scratch2;
-  const double* qlo = qhi + (size_t)kTailN * a.n_rad;
-  double2* R = reinterpret_cast<double2*>(blob + L.off_tail);
-  const int n_items = 2 * L.n_pref * kTailN, CL = (a.n_rad + kTailChunks - 1) / kTailChunks;
-  double* Qs = blob + L.off_scratch3;                                   // Q_c(i), [kTailN][n_rad]
-  dd* Lstart = reinterpret_cast<dd*>(Qs + (size_t)kTailN * a.n_rad);    // [n_items][kTailChunks]
-  dd* Qstart = Lstart + (size_t)n_items * kTailChunks;                  // [kTailN][kTailChunks]
+__device__ void prep_tail_sums(const TailJob& J) {
+  const double* qhi = J.s2;
+  const double* qlo = qhi + (size_t)kTailN * J.n;
+  double2* R = J.R;
+  const int n_items = 2 * J.n_pref * kTailN, CL = (J.n + kTailChunks - 1) / kTailChunks;
+  double* Qs = J.s3;                                                   // Q_c(i), [kTailN][n]
+  dd* Lstart = reinterpret_cast<dd*>(Qs + (size_t)kTailN * J.n);       // [n_items][kTailChunks]
+  dd* Qstart = Lstart + (size_t)n_items * kTailChunks;                 // [kTailN][kTailChunks]
   for (int w = threadIdx.x; w < n_items * kTailChunks; w += blockDim.x) {
     const int e = w % n_items, c = w / n_items;
-    const int part = e / (L.n_pref * kTailN), r = (e / kTailN) % L.n_pref, n = e % kTailN;
-    double* Rr = reinterpret_cast<double*>(R + (size_t)r * (a.n_rad + 1) * kTailN) + part;
+    const int part = e / (J.n_pref * kTailN), r = (e / kTailN) % J.n_pref, n = e % kTailN;
+    double* Rr = reinterpret_cast<double*>(R + (size_t)r * (J.n + 1) * kTailN) + part;
     const bool owner = r == 0 && part == 0;
-    if (c == 0) Rr[2 * ((size_t)a.n_rad * kTailN + n)] = 0.0;
+    if (c == 0) Rr[2 * ((size_t)J.n * kTailN + n)] = 0.0;
     dd acc = {0.0, 0.0}, Q = {1.0, 0.0};
-    for (int i = min((c + 1) * CL, a.n_rad) - 1; i >= c * CL; --i) {
-      const dd q = {qhi[(size_t)n * a.n_rad + i], qlo[(size_t)n * a.n_rad + i]};
-      acc = dd_add_d(dd_mul(acc, q), blob[L.off_pref + 2 * (r * L.n_rad_pad + i) + part]);
+    for (int i = min((c + 1) * CL, J.n) - 1; i >= c * CL; --i) {
+      const dd q = {qhi[(size_t)n * J.n + i], qlo[(size_t)n * J.n + i]};
+      acc = dd_add_d(dd_mul(acc, q), J.pref[2 * (r * J.stride + i) + part]);
       Rr[2 * ((size_t)i * kTailN + n)] = acc.hi;
       if (owner) {
         Q = dd_mul(Q, q);
-        Qs[(size_t)n * a.n_rad + i] = Q.hi;
+        Qs[(size_t)n * J.n + i] = Q.hi;
       }
     }
     Lstart[(size_t)e * kTailChunks + c] = acc;
@@ -808,18 +818,83 @@ __device__ void prep_tail_sums(const EvalArgs& a, const BlobLayout& L, double* b
   __syncthreads();
   for (int w = threadIdx.x; w < n_items * kTailChunks; w += blockDim.x) {
     const int e = w % n_items, c = w / n_items;
-    const int part = e / (L.n_pref * kTailN), r = (e / kTailN) % L.n_pref, n = e % kTailN;
-    double* Rr = reinterpret_cast<double*>(R + (size_t)r * (a.n_rad + 1) * kTailN) + part;
+    const int part = e / (J.n_pref * kTailN), r = (e / kTailN) % J.n_pref, n = e % kTailN;
+    double* Rr = reinterpret_cast<double*>(R + (size_t)r * (J.n + 1) * kTailN) + part;
     dd carry = {0.0, 0.0};
     for (int cc = kTailChunks - 1; cc > c; --cc)
       carry = dd_add(Lstart[(size_t)e * kTailChunks + cc], dd_mul(Qstart[(size_t)n * kTailChunks + cc], carry));
     if (carry.hi != 0.0 || carry.lo != 0.0)
-      for (int i = min((c + 1) * CL, a.n_rad) - 1; i >= c * CL; --i) {
+      for (int i = min((c + 1) * CL, J.n) - 1; i >= c * CL; --i) {
         const size_t at = 2 * ((size_t)i * kTailN + n);
-        Rr[at] = dd_add_d(dd_mul_d(carry, Qs[(size_t)n * a.n_rad + i]), Rr[at]).hi;
+        Rr[at] = dd_add_d(dd_mul_d(carry, Qs[(size_t)n * J.n + i]), Rr[at]).hi;
       }
   }
 }
+// the REAL contour's job: all n_rad nodes of the prepared block
+__device__ __forceinline__ TailJob real_tail_job(const EvalArgs& a, const BlobLayout& L, double* blob) {
+  return TailJob{a.n_rad, L.n_pref, L.n_rad_pad, blob + L.off_y, blob + L.off_pref,
+                 reinterpret_cast<double2*>(blob + L.off_tail), blob + L.off_scratch2, blob + L.off_scratch3};
+}
+
+// D1(y) for real y (REAL contour): massive 1/(y + m2) or rational (y + M2)/(y^2 + a y + b).
+__device__ __forceinline__ cd line_k_real(const gf_propagator& p, double y) {
+  if (p.kind == GF_PROP_MASSIVE) return cinv(cd{y + p.m2_re, p.m2_im});
+  return cd{(y + p.M2) / fma(y, y + p.a, p.b), 0.0};
+}
+
+// y = s0 expm1(u L) in double-double, rounded once (readings G3/G4, G18)
+__device__ __forceinline__ double radial_node(double t, dd Llog, double s0) {
+  const double u = 0.5 * (t + 1.0);
+  return dd_mul_d(dd_expm1(dd_mul_d(Llog, u)), s0).hi;
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// Tail: all radial nodes with y_i >= Y0(x) at once.  With a = x + mu, eps = 1/y:
+//   S(x, y) = sum_k omega^(k+1) [delta mu_k - nu_k],  omega = 4 x eps/(1 + a eps)^2,  delta = a eps/4
+//           = sum_n eps^n X h_n(X, Z),   X = 4x, Z = -a,   h_n = sum_{k<n} gamma_{n,k} X^k Z^(n-1-k)
+// (binomial series of (1 + a eps)^(-2k-2); gamma_{n,k} in gf_routes.cuh).  The series converges absolutely,
+// term n below 4^-n, for y >= Y0 = 4 (sqrt|x| + sqrt(|x| + |a|))^2, so
+//   sum_{i >= i0} pref_i S(x, y_i) = X sum_n h_n sum_{i >= i0} pref_i y_i^-n = (X/y_i0) sum_n h_n(X/y_i0, Z/y_i0) Rhat_n(i0)
+// with the x-independent tables Rhat_n(i0) made once per launch.  h_n is a real-coefficient polynomial in the
+// ratio of X and Z (the smaller over the larger) and is evaluated by the same second-order recurrence as the
+// angular series.  A log-mapped radial rule has most of its nodes in this tail (about 60 % on the production
+// scan), and they cost kTailN (kTailN + 1) DFMA per point instead of a series each.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ cd tail_series(const double* __restrict__ gam, const double2* __restrict__ Rrow, cd x,
+                                          cd a, double invy0) {
+  const cd X = {4.0 * x.re * invy0, 4.0 * x.im * invy0}, Z = {-a.re * invy0, -a.im * invy0};
+  const double nX = fma(X.re, X.re, X.im * X.im), nZ = fma(Z.re, Z.re, Z.im * Z.im);
+  const bool fwd = nX <= nZ;                        // powers of X/Z, else of Z/X
+  const cd base = fwd ? Z : X, oth = fwd ? X : Z;
+  const double inb = 1.0 / (fwd ? nZ : nX);
+  const cd rho = {fma(oth.re, base.re, oth.im * base.im) * inb, fma(oth.im, base.re, -(oth.re * base.im)) * inb};
+  const double rr = rho.re + rho.re, ns = -fma(rho.re, rho.re, rho.im * rho.im);
+  cd pw = {1.0, 0.0}, acc = {0.0, 0.0};
+  const double* row = gam;
+#pragma unroll 1
+  for (int n = 1; n <= kTailN; ++n) {
+    double b0 = 0.0, b1 = 0.0;
+    const double* c = fwd ? row + n - 1 : row;      // highest power of the ratio first
+    const int step = fwd ? -1 : 1;
+    if (n & 1) {
+      b0 = *c;
+      c += step;
+    }
+#pragma unroll 2
+    for (int j = n >> 1; j > 0; --j, c += 2 * step) {   // two coefficients per trip, roles of b0, b1 alternate
+      b1 = fma(rr, b0, fma(ns, b1, c[0]));
+      b0 = fma(rr, b1, fma(ns, b0, c[step]));
+    }
+    const cd P = {fma(-b1, rho.re, b0), b1 * rho.im};   // c_0 - c_1 conj(rho)
+    const double2 R = Rrow[n - 1];
+    acc = cadd(acc, cmul(cmul(P, pw), cd{R.x, R.y}));
+    pw = cmul(pw, base);
+    row += n;
+  }
+  return cmul(X, acc);
+}
+
 
 }  // namespace
 }  // namespace gf

@@ -368,13 +368,79 @@ def test_contour_geometry(oracle):
 
 
 def test_auto_policy_regions(oracle):
+    """AUTO's four tests in their order (include/gf.h, gf_contour), on both sides of each boundary."""
     rn, rw = oracle.make_radial_pyramid(64)
     P = oracle.make_params(BUB, BUB, 1e6, contour="auto")
     pol = lambda x: oracle.contour_nodes(P, x, rn, rw, 64, 128)[0]
-    assert pol(1 + 1j) == 1 and pol(-3 + 2j) == 1        # RAY_ARC outside the wedge
-    assert pol(-6 + 0.01j) == 2 and pol(-6 - 0.01j) == 2  # THREAD near the cut
-    assert pol(-3 + 0.01j) == 0                           # REAL in the strip -4.1 < Re x < -1
-    assert pol(-0.5 + 0.001j) == 1                        # Re x >= -m^2: not in the wedge
+    assert pol(1 + 1j) == 0 and pol(2 + 2.2j) == 0         # 1. inside the half-size parabola Re x > (Im x)^2/2 - 1/2: REAL
+    assert pol(2 + 2.3j) == 1 and pol(0 + 1.1j) == 1      #    just outside it: RAY_ARC
+    assert pol(-0.5 + 0.001j) == 0 and pol(-0.9 - 0.01j) == 0   # 2. next to the negative axis inside the parabola: REAL
+    assert pol(-0.5 + 0.7j) == 1                           #    |Im x| n_rad >= 80 |Re x|: not "next to the axis"
+    assert pol(-3 + 2j) == 1                               # 4. RAY_ARC outside the wedge
+    assert pol(-6 + 0.01j) == 2 and pol(-6 - 0.01j) == 2   # 3. THREAD near the cut
+    assert pol(-3 + 0.01j) == 0                            #    REAL in the strip -4.1 < Re x < -1 (the limitation)
+    # a line THREAD does not apply to: REAL inside the wedge
+    Pr = oracle.make_params(BUB, RAT, 1e6, contour="auto")
+    assert oracle.contour_nodes(Pr, -6 + 0.01j, rn, rw, 64, 128)[0] == 0
+
+
+def test_auto_is_the_continuation_where_the_header_says(oracle):
+    """AUTO against the closed form CF1 over the analytic region of config 2's box (no test pinned AUTO):
+    REAL inside the parabola is exact to the quadrature; RAY_ARC and THREAD reproduce CF1 away from the negative
+    axis; the one region that is NOT the continuation is case 3 with REAL (the strip next to the negative axis
+    between the parabola and -4.1 m^2), exactly as include/gf.h states."""
+    n_rad, n_ang = 256, 128
+    re, im = np.linspace(-10, 2, 49), np.linspace(-4, 4, 33)
+    xs = (re[None, :] + 1j * im[:, None]).ravel()
+    xs = xs[xs.imag != 0]
+    P = oracle.make_params(BUB, BUB, 1e6, contour="auto")
+    rn, rw = oracle.make_radial_pyramid(n_rad, levels=4)
+    z, wz = oracle.make_quadrature("gauss_cheb2", n_ang, measure="sqrt1mz2")
+    g, _ = oracle.eval_grid(P, rn, rw, n_rad, z, wz, xs)
+    err = relerr(g, [complex(CF.cf1(v)) for v in xs])
+    pol = np.array([oracle.contour_nodes(P, v, rn, rw, n_rad, n_ang)[0] for v in xs])
+    inside = np.array([CF.in_parabola_R2(v) for v in xs])
+    assert (pol == 0).sum() > 100 and (pol == 1).sum() > 900 and (pol == 2).sum() > 300
+    assert err[(pol == 0) & inside].max() < 1e-10                       # REAL where it is the continuation
+    strip = (pol == 0) & ~inside                                        # the documented limitation
+    assert strip.sum() > 0 and np.all((xs[strip].real < -1) & (xs[strip].real > -4.1) & (np.abs(xs[strip].imag) <= 0.5))
+    assert err[strip].min() > 0.5
+    far = np.abs(xs.imag) >= 0.5                                        # rays and threads away from the axis
+    assert err[(pol == 1) & far].max() < 2e-3 and err[(pol == 2)].max() < 3e-2
+    assert np.median(err[pol == 1]) < 1e-8
+    # the three points ADVICE r1 lists (x = -0.5, -0.5 + 0.0078i, -0.5 + 0.03i: RAY_ARC was off by 2 ... 5e3 there)
+    xa = np.array([-0.5 + 1e-9j, -0.5 + 0.0078j, -0.5 + 0.03j])
+    ga, _ = oracle.eval_grid(P, rn, rw, n_rad, z, wz, xa)
+    assert relerr(ga, [complex(CF.cf1(v)) for v in xa]).max() < 1e-9
+
+
+def test_contour_ladder_and_arc(oracle):
+    """The radius of a deformed contour is the smallest rung of {2^k, 1.5 2^k} above 1.5 (sqrt|x| + sqrt(|x|+sc))^2
+    (Lambda^2/2 beyond the ladder), the ray runs along x/|x|, and the rational arc ends where the ray ends and on
+    the real axis, at the angles 4 atan(tau v) (compared with the angle form it replaces)."""
+    rn, rw = oracle.make_radial_pyramid(256)
+    P = oracle.make_params(BUB, BUB, 1e6, contour="ray_arc")
+    rungs = sorted([2.0 ** k for k in range(-4, 22)] + [1.5 * 2.0 ** k for k in range(-4, 22)])
+    for x in [-3 + 2j, 1e-3 + 1e-3j, 40 - 90j, -7 + 1e-7j, 0.2 - 0.1j, 2500 + 1j]:
+        _, y, wy = oracle.contour_nodes(P, x, rn, rw, 256, 128)
+        q = math.sqrt(abs(x)) + math.sqrt(abs(x) + 1.0)
+        want = min(r for r in rungs if r >= 1.5 * q * q * (1 - 1e-15))
+        R = abs(y[128])
+        assert abs(R - want) <= 2e-15 * want, (x, R, want)
+        assert np.max(np.abs(y[:128] / np.abs(y[:128]) - x / abs(x))) < 4e-16          # the ray's direction
+        th = np.angle(y[128:192])
+        u = 0.5 * (rn[256 + 128:256 + 192] + 1.0)
+        tau = math.tan(np.angle(x) / 4)
+        assert np.max(np.abs(th - 4 * np.arctan(tau * (1 - u)))) < 1e-14               # arc: theta = 4 atan(tau v), v = 1 - u
+        dth = -4 * tau / (1 + (tau * (1 - u)) ** 2)                                     # d theta/du
+        assert np.max(np.abs(wy[128:192] / (1j * y[128:192] * dth * 0.5 * rw[256 + 128:256 + 192]) - 1)) < 1e-14
+        assert np.max(np.abs(np.abs(y[128:192]) / want - 1)) < 2e-15
+        assert y[192].real > want and np.all(np.diff(y[192:].real) > 0)                    # real tail starts at R
+        assert abs(np.sum(wy) - 1e6) / 1e6 < 1e-9
+    # beyond the ladder / the cutoff: Lambda^2/2
+    P2 = oracle.make_params(BUB, BUB, 30.0, contour="ray_arc")
+    _, y, _ = oracle.contour_nodes(P2, -6 + 2j, rn, rw, 256, 128)
+    assert abs(abs(y[128]) - 15.0) < 1e-14
 
 
 def test_thread_contour_and_discontinuity(oracle):
