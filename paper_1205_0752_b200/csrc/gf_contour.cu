@@ -192,7 +192,10 @@ __device__ __forceinline__ NodeAt locate(int pol, int n_rad, int g) {
     if (g < n2 + n4) return {SEG_ARC, g - n2, 0, 0};
     return {SEG_TAIL, g - n2 - n4, 0, 0};
   }
-  if (g < 5 * n8) { const int k = g / n8; return {SEG_LINE, g - k * n8, k, n4}; }
+  if (g < 5 * n8) {
+    const int k = (g >= n8) + (g >= 2 * n8) + (g >= 3 * n8) + (g >= 4 * n8);   // g / n8 without the division
+    return {SEG_LINE, g - k * n8, k, n4};
+  }
   if (g < 6 * n8) return {SEG_ARC, g - 5 * n8, 0, n4};
   return {SEG_TAIL, g - 6 * n8, 0, 0};
 }
@@ -283,9 +286,9 @@ __global__ void __launch_bounds__(256) prep_rungs_kernel(const __grid_constant__
 // eval_real_kernel; counters as there.
 // ---------------------------------------------------------------------------------------------
 #ifndef GF_CONTOUR_MIN_BLOCKS
-#define GF_CONTOUR_MIN_BLOCKS 2
+#define GF_CONTOUR_MIN_BLOCKS 4
 #endif
-template <bool COUNT>
+template <bool COUNT, int NT>
 __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
     eval_contour_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                         const double* __restrict__ blob, unsigned long long* __restrict__ counters) {
@@ -327,6 +330,17 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
 
   const Geo geo = build_geo(a, x.re, x.im);
   const cd dir2 = {fma(geo.dre, geo.dre, -(geo.dim * geo.dim)), 2.0 * geo.dre * geo.dim};
+  // One pole (NT == 1): on a piece y = dir r with real r from a table (the ray; dir = 1 on the real pieces)
+  //   zeta = (x + mu + y)^2/(4 x y) = Z1/(4r) + C2 + Z3 r,  Z1 = (x + mu)^2/x conj(dir), C2 = (x + mu)/(2x), Z3 = dir/(4x)
+  //   delta = (x + mu)/(4y) = Dc/(4r),  Dc = (x + mu) conj(dir)
+  // as on the REAL contour (four DFMA instead of three complex products); zdir: the direction the constants are for.
+  cd Z1 = {0.0, 0.0}, C2 = {0.0, 0.0}, Z3 = {0.0, 0.0}, Dc = {0.0, 0.0}, C1x4 = {0.0, 0.0};
+  int zdir = -1;   // -1 not set, 0 dir = 1, 1 dir = geo.d
+  if (NT == 1) {
+    const cd xm0 = {x.re + a.term[0].mu_re, x.im + a.term[0].mu_im};
+    C2 = cmul(xm0, cscale(xinv, 0.5));
+    C1x4 = cscale(cmul(xm0, C2), 2.0);
+  }
   // tables of the real nodes this point walks: the REAL contour's (policy REAL) or its rung's tail piece
   const double* row = blob + L.off_rung + (long long)geo.row * L.rung_stride;
   const bool real_pol = geo.pol == GF_CONTOUR_REAL;
@@ -342,7 +356,8 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
   {
     const double ax = sqrt(fma(x.re, x.re, x.im * x.im));
     double Y0 = 0.0;
-    for (int r = 0; r < a.n_terms; ++r) {
+#pragma unroll
+    for (int r = 0; r < NT; ++r) {
       const cd az = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
       const double q = sqrt(ax) + sqrt(ax + sqrt(fma(az.re, az.re, az.im * az.im)));
       Y0 = fmax(Y0, kTailFactor * q * q);
@@ -396,19 +411,39 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
       q4 = cscale(cinv_fast(y), 0.25);
       base = cscale(cmul(wy, y), a.c0);
     }
-    const cd xq = cmul(xinv, q4);                    // 1/(4 x y)
+    const bool affine = NT == 1 && (table || at.type == SEG_RAY);
+    cd xq = {0.0, 0.0};
+    if (affine) {
+      const int want = at.type == SEG_RAY;
+      if (zdir != want) {   // once per piece
+        zdir = want;
+        const cd d = want ? cd{geo.dre, geo.dim} : cd{1.0, 0.0}, dc = {d.re, -d.im};
+        Z1 = cmul(C1x4, dc);
+        Z3 = cscale(cmul(xinv, d), 0.25);
+        Dc = cmul(cd{x.re + a.term[0].mu_re, x.im + a.term[0].mu_im}, dc);
+      }
+    } else {
+      xq = cmul(xinv, q4);                           // 1/(4 x y)
+    }
     cd ic0 = {0.0, 0.0};
     if (!table) {
       if (a.same_mass) ic0 = cinv_fast(cd{y.re + a.term[0].mu_re, y.im + a.term[0].mu_im});
       base = cmul(base, a.same_mass ? ic0 : line_k_complex(a.line_k, y));
     }
-#pragma unroll 1
-    for (int r = 0; r < a.n_terms; ++r) {
+#pragma unroll
+    for (int r = 0; r < NT; ++r) {
       const double mur = a.term[r].mu_re, mui = a.term[r].mu_im;
-      const cd xm = {x.re + mur, x.im + mui};
-      const cd A = {xm.re + y.re, xm.im + y.im};
-      const cd delta = cmul(xm, q4);                 // eta - 1/4
-      const cd zeta = cmul(csqr(A), xq);
+      cd delta, zeta;
+      if (affine) {
+        const double q4r = table ? q4.re : row[L.rg_q4 + at.i], rr = table ? y.re : row[L.rg_r + at.i];
+        delta = {Dc.re * q4r, Dc.im * q4r};
+        zeta = {fma(Z1.re, q4r, fma(Z3.re, rr, C2.re)), fma(Z1.im, q4r, fma(Z3.im, rr, C2.im))};
+      } else {
+        const cd xm = {x.re + mur, x.im + mui};
+        const cd A = {xm.re + y.re, xm.im + y.im};
+        delta = cmul(xm, q4);                        // eta - 1/4
+        zeta = cmul(csqr(A), xq);
+      }
       const cd s = node_term<double, COUNT>(tb, x, y, delta, zeta, mur, mui, rc);
       cd pr;
       if (table) {
@@ -416,7 +451,9 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
         pr = {p2.x, p2.y};
       } else {
         const cd ic = a.same_mass ? ic0 : cinv_fast(cd{y.re + mur, y.im + mui});
-        pr = cmul(cmul(base, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);
+        // a massive line 2 is its one pole with residue 1
+        pr = NT == 1 ? cd{-base.re, -base.im} : cmul(base, cd{-a.term[r].R_re, -a.term[r].R_im});
+        pr = cmul(pr, ic);
       }
       if (!valid) pr = {0.0, 0.0};
       g_re = fma(pr.re, s.re, fma(-pr.im, s.im, g_re));
@@ -428,7 +465,8 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
     const double invy0 = 4.0 * tq4[min(i_end, tn - 1)];
     const double2* Rt = reinterpret_cast<const double2*>(real_pol ? blob + L.off_tail : row + L.rg_tail) +
                         (size_t)i_end * kTailN;
-    for (int r = 0; r < a.n_terms; ++r) {
+#pragma unroll
+    for (int r = 0; r < NT; ++r) {
       const cd az = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
       const cd tl = tail_series(sb + L.off_gam, Rt + (size_t)r * (tn + 1) * kTailN, x, az, invy0);
       if (sub == 0) {
@@ -492,10 +530,10 @@ __global__ void contour_nodes_kernel(const __grid_constant__ EvalArgs a, const _
   out_wy[g] = make_double2(wy.re, wy.im);
 }
 
-template <bool COUNT>
+template <bool COUNT, int NT>
 int launch_contour_t(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
                      cudaStream_t stream) {
-  auto kern = eval_contour_kernel<COUNT>;
+  auto kern = eval_contour_kernel<COUNT, NT>;
   if (plan.smem_bytes > 48 * 1024) {
     int rc = check_cuda(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes),
                         "cudaFuncSetAttribute(max dynamic shared memory)");
@@ -509,8 +547,11 @@ int launch_contour_t(const EvalArgs& a, const LaunchPlan& plan, const double* bl
 
 int launch_contour(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* d_counters,
                    cudaStream_t stream) {
-  return d_counters ? launch_contour_t<true>(a, plan, blob, d_counters, stream)
-                    : launch_contour_t<false>(a, plan, blob, nullptr, stream);
+  if (a.n_terms == 1)
+    return d_counters ? launch_contour_t<true, 1>(a, plan, blob, d_counters, stream)
+                      : launch_contour_t<false, 1>(a, plan, blob, nullptr, stream);
+  return d_counters ? launch_contour_t<true, 2>(a, plan, blob, d_counters, stream)
+                    : launch_contour_t<false, 2>(a, plan, blob, nullptr, stream);
 }
 
 int launch_prepare_rungs(const EvalArgs& a, const LaunchPlan& plan, double* blob, cudaStream_t stream) {
