@@ -38,7 +38,10 @@
 // line-swap symmetry, rule independence, exactness degree of the quadrature
 // rules, brute-force high-order quadrature; the paper's Kernels 3 and 4 (angular integral B of eq. (22) over
 // complex y; obstruction of the real y-axis by the cut) against the textbook angular integral, the scan
-// itself and the parabola of PAPER.md:270.  Unpinned: values of RAY_ARC inside
+// itself and the parabola of PAPER.md:270; the Taylor subtraction of order n > 0 (eq. (12),(13)) against the
+// definition itself (F minus its Taylor polynomial in p, differentiated numerically at 100+ digits), the closed form
+// CF1 minus its first n Taylor terms, CF3 minus x CF3'(0), G_n = O(x^(n+1)); the rules of the d-dimensional angular
+// measure (Gauss-Chebyshev of the first kind included) against B(k+1/2, (d-1)/2).  Unpinned: values of RAY_ARC inside
 // the wedge around the negative real axis and of REAL outside the parabola R2
 // (DESIGN.md "parity unpinned"), where no closed form applies.
 //
@@ -61,7 +64,7 @@ typedef long double ld;
 const long double kPi = 3.14159265358979323846264338327950288L;
 
 // ---- enums (values are part of the oracle's own C interface) -------------
-enum { QUAD_GAUSS_LEGENDRE = 0, QUAD_GAUSS_CHEB2 = 1, QUAD_TANH_SINH = 2 };
+enum { QUAD_GAUSS_LEGENDRE = 0, QUAD_GAUSS_CHEB2 = 1, QUAD_TANH_SINH = 2, QUAD_GAUSS_CHEB1 = 3 };
 enum { MEASURE_PLAIN = 0, MEASURE_SQRT1MZ2 = 1 };
 enum { PROP_MASSIVE = 0, PROP_RATIONAL = 1 };
 enum { CONTOUR_REAL = 0, CONTOUR_RAY_ARC = 1, CONTOUR_THREAD = 2, CONTOUR_AUTO = 3 };
@@ -131,23 +134,43 @@ void gauss_legendre(int n, double* x, double* w) {
   if (n % 2 == 1) x[n / 2] = 0.0;
 }
 
-int make_quadrature(int kind, int n, double step, int measure, double* x, double* w) {
+// Rules for the angular measure (1 - z^2)^alpha dz, alpha = (d-3)/2 in d dimensions (eq. (5),(9) for d = 4: alpha =
+// 1/2; "arbitrary dimensions by trivial modifications"; Gauss-Legendre, Gauss-Chebyshev "of
+// the first and second kind ... depending on the dimension", tanh-sinh).  The Gauss-Chebyshev rules are the exact Gauss
+// rules of d = 2 (first kind, weight (1-z^2)^(-1/2)) and d = 4 (second kind, weight (1-z^2)^(1/2)); for another
+// alpha the remaining power of (1 - z^2) = sin^2(theta) is put into the weights, as for Gauss-Legendre and tanh-sinh.
+int make_quadrature_alpha(int kind, int n, double step, long double alpha, double* x, double* w) {
   if (n < 1 || !x || !w) return 1;
   if (kind == QUAD_GAUSS_LEGENDRE) {
     gauss_legendre(n, x, w);
-    if (measure == MEASURE_SQRT1MZ2)
+    if (alpha == 0.5L)
       for (int j = 0; j < n; ++j) w[j] *= std::sqrt((1.0 - x[j]) * (1.0 + x[j]));
+    else if (alpha != 0)
+      for (int j = 0; j < n; ++j) w[j] = (double)((ld)w[j] * std::pow(((ld)1 - (ld)x[j]) * ((ld)1 + (ld)x[j]), alpha));
     return 0;
   }
   if (kind == QUAD_GAUSS_CHEB2) {
     // Gauss-Chebyshev, 2nd kind: exact Gauss rule for the weight sqrt(1-z^2)
-    // (Abramowitz-Stegun 25.4.40; the paper's check rule).
+    // (Abramowitz-Stegun 25.4.40; the paper's check rule): z_j = cos(j pi/(n+1)),
+    // w_j = pi/(n+1) sin^2(theta_j); for the weight (1-z^2)^alpha: pi/(n+1) sin^(2 alpha + 1)(theta_j).
     for (int j = 0; j < n; ++j) {
       ld th = (ld)kPi * (ld)(n - j) / (ld)(n + 1);  // ascending z
-      ld s = std::sin(th);
+      ld sn = std::sin(th);
       x[j] = (double)std::cos(th);
-      ld ww = (ld)kPi / (ld)(n + 1) * s * s;  // includes sqrt(1-z^2)
-      w[j] = (double)(measure == MEASURE_SQRT1MZ2 ? ww : ww / s);
+      ld ww = (ld)kPi / (ld)(n + 1) * sn * sn;  // includes sqrt(1-z^2)
+      w[j] = (double)(alpha == 0.5L ? ww : alpha == 0 ? ww / sn : ww * std::pow(sn, 2 * alpha - 1));
+    }
+    if (n % 2 == 1) x[n / 2] = 0.0;
+    return 0;
+  }
+  if (kind == QUAD_GAUSS_CHEB1) {
+    // Gauss-Chebyshev, 1st kind: exact Gauss rule for the weight 1/sqrt(1-z^2) (Abramowitz-Stegun 25.4.38):
+    // z_j = cos((2j-1) pi/(2n)), w_j = pi/n; for the weight (1-z^2)^alpha: pi/n sin^(2 alpha + 1)(theta_j).
+    for (int j = 0; j < n; ++j) {
+      ld th = (ld)kPi * (ld)(2 * (n - j) - 1) / (ld)(2 * n);  // ascending z
+      ld sn = std::sin(th);
+      x[j] = (double)std::cos(th);
+      w[j] = (double)((ld)kPi / (ld)n * std::pow(sn, 2 * alpha + 1));
     }
     if (n % 2 == 1) x[n / 2] = 0.0;
     return 0;
@@ -163,13 +186,18 @@ int make_quadrature(int kind, int n, double step, int measure, double* x, double
       ld ch = std::cosh(a);
       x[j] = (double)std::tanh(a);
       ld ww = 0.5L * (ld)kPi * h * std::cosh(k * h) / (ch * ch);
-      // sqrt(1 - tanh^2) = sech, computed without cancellation
-      w[j] = (double)(measure == MEASURE_SQRT1MZ2 ? ww / ch : ww);
+      // 1 - tanh^2 = sech^2, computed without cancellation
+      w[j] = (double)(alpha == 0.5L ? ww / ch : alpha == 0 ? ww : ww * std::pow(1 / ch, 2 * alpha));
     }
     if (n % 2 == 1) x[n / 2] = 0.0;
     return 0;
   }
   return 2;
+}
+
+int make_quadrature(int kind, int n, double step, int measure, double* x, double* w) {
+  if (measure != MEASURE_PLAIN && measure != MEASURE_SQRT1MZ2) return 2;
+  return make_quadrature_alpha(kind, n, step, measure == MEASURE_SQRT1MZ2 ? 0.5L : 0.0L, x, w);
 }
 
 // ---- Step 4 / Kernel 1: the grid ------------------
@@ -244,6 +272,72 @@ std::complex<R> prop_diff(const Propagator& P, std::complex<R> y, std::complex<R
   C Qu = u * u + (R)P.a * u + (R)P.b;
   C Qy = y * y + (R)P.a * y + (R)P.b;
   return -d * (u * y + (R)P.M2 * (u + y) + ((R)P.a * (R)P.M2 - (R)P.b)) / (Qu * Qy);
+}
+
+// ---- Taylor subtraction of order n > 0 (eq. (12),(13)) ---------------------------------------
+// Reading G20: eq. (13)'s "x = 0" is p = 0 -- eq. (20) sets the scalar product sqrt(x) sqrt(y) z to zero
+// together with x -- so t^n is the BPHZ Taylor operator in the external momentum p_mu, and a power x^i of eq. (13)
+// is the order 2i in p.  With p -> eps p,  F(eps) = D1(y) D2(y + eps^2 x + eps bz),  bz = -2 sqrt(x) sqrt(y) z, and
+//   t^n F = the Taylor polynomial of F(eps) of degree 2n, at eps = 1
+//         = D1(y) sum_{m=0}^{2n} t_m sum_{l <= m, m + l <= 2n} C(m,l) x^l bz^(m-l),     t_m = D2^(m)(y)/m!
+// (d^m = (x + bz)^m = sum_l C(m,l) x^l bz^(m-l) has the order m + l in p).  The odd orders are odd in z and cancel
+// under a symmetric angular rule; n = 0 gives t^0 F = D1(y) D2(y), eq. (20).
+//
+// t_m, m = 0..M, by Leibniz' rule on Q f = N (f = D2 = N/Q):  Q t_m = N_m - Q' t_{m-1} - (Q''/2) t_{m-2},
+// N_0 = N(y), N_1 = N'(y), N_m = 0 beyond (N is linear or constant).
+const int kMaxTaylor = 4;
+template <typename R>
+void prop_taylor(const Propagator& P, std::complex<R> y, int M, std::complex<R>* t) {
+  typedef std::complex<R> C;
+  if (P.kind == PROP_MASSIVE) {   // N = 1, Q = y + m2
+    C Q = y + C((R)P.m2_re, (R)P.m2_im);
+    t[0] = C(1) / Q;
+    for (int m = 1; m <= M; ++m) t[m] = -t[m - 1] / Q;
+    return;
+  }
+  C Q = y * y + (R)P.a * y + (R)P.b, Q1 = (R)2 * y + (R)P.a;   // Q''/2 = 1
+  t[0] = (y + (R)P.M2) / Q;
+  if (M >= 1) t[1] = (C(1) - Q1 * t[0]) / Q;
+  for (int m = 2; m <= M; ++m) t[m] = -(Q1 * t[m - 1] + t[m - 2]) / Q;
+}
+
+// D2(u) - [Taylor polynomial of D2 of degree 2n in p], u = y + d, d = x + bz, in a combined form (like eq. (20) for
+// n = 0: every term carries its full power of p explicitly, no difference of nearly equal numbers is formed):
+//   D2(y + d) - sum_{m <= M} t_m d^m = -d^(M+1) [Q' t_M + (Q''/2)(t_{M-1} + t_M d)] / Q(u)        (M = 2n >= 2)
+// (multiply by Q(u) = Q + Q' d + (Q''/2) d^2: the coefficients of d^0..d^M cancel identically, those of d^(M+1) and
+// d^(M+2) remain), plus the terms of sum_{m <= M} t_m d^m whose order in p exceeds 2n, which t^n does not subtract:
+//   sum_{m = n+1}^{2n} t_m sum_{l = 2n-m+1}^{m} C(m,l) x^l bz^(m-l).
+template <typename R>
+std::complex<R> prop_diff_taylor(const Propagator& P, std::complex<R> y, std::complex<R> x, std::complex<R> bz, int n) {
+  typedef std::complex<R> C;
+  const int M = 2 * n;
+  C t[2 * kMaxTaylor + 1];
+  prop_taylor<R>(P, y, M, t);
+  C d = x + bz, u = y + d;
+  C dM1 = d;
+  for (int k = 0; k < M; ++k) dM1 *= d;   // d^(M+1)
+  C rem;
+  if (P.kind == PROP_MASSIVE) {
+    rem = -dM1 * t[M] / (u + C((R)P.m2_re, (R)P.m2_im));
+  } else {
+    C Qu = u * u + (R)P.a * u + (R)P.b, Q1 = (R)2 * y + (R)P.a;
+    rem = -dM1 * (Q1 * t[M] + t[M - 1] + t[M] * d) / Qu;
+  }
+  C extra = 0;
+  for (int m = n + 1; m <= M; ++m) {
+    R binom = 1;                         // C(m, l), starting at l = 0
+    C xl = 1;                            // x^l
+    for (int l = 0; l <= m; ++l) {
+      if (l >= M - m + 1) {
+        C bp = 1;
+        for (int k = 0; k < m - l; ++k) bp *= bz;
+        extra += t[m] * binom * xl * bp;
+      }
+      binom = binom * (R)(m - l) / (R)(l + 1);
+      xl *= x;
+    }
+  }
+  return rem + extra;
 }
 
 // Symmetric routing (shift invariance of eq. (4)): both lines 1/(q^2 + m2) with
@@ -518,7 +612,8 @@ cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int
     for (int j = 0; j < n_ang; ++j) {
       C d = xx - B * (R)z[j];                                  // u - y
       C f = P.routing == 1 ? fsub_symmetric<R>(P.line_pk, xx, y, B / (R)2, (R)z[j])
-                           : D1 * prop_diff<R>(P.line_pk, y, d);   // F_sub, eq. (20)
+            : P.taylor_order == 0 ? D1 * prop_diff<R>(P.line_pk, y, d)   // F_sub, eq. (20)
+                                  : D1 * prop_diff_taylor<R>(P.line_pk, y, xx, -(B * (R)z[j]), P.taylor_order);   // eq. (12),(13)
       sr += (ACC)((R)wz[j] * f.real());
       si += (ACC)((R)wz[j] * f.imag());
     }
@@ -619,7 +714,8 @@ int cut_crossings(const Params& P, cplx x, int n_z) {
 int check_params(const Params& P, int n_rad, int n_ang) {
   if (n_rad < 1 || n_ang < 1) return 2;
   if (!(P.cutoff2 > 0) || !(P.map_scale > 0)) return 2;
-  if (P.taylor_order != 0 || P.sub_re != 0 || P.sub_im != 0) return 3;
+  if (P.taylor_order < 0 || P.taylor_order > kMaxTaylor || P.sub_re != 0 || P.sub_im != 0) return 3;
+  if (P.taylor_order != 0 && P.routing != 0) return 3;
   if (P.contour < 0 || P.contour > 3) return 2;
   if (P.contour != CONTOUR_REAL && n_rad % 8 != 0) return 2;
   if (P.contour == CONTOUR_THREAD && !thread_applicable(P)) return 3;
@@ -638,6 +734,12 @@ extern "C" {
 
 int gfo_make_quadrature(int kind, int n, double step, int measure, double* nodes, double* weights) {
   return make_quadrature(kind, n, step, measure, nodes, weights);
+}
+
+// the rule for the angular measure (1 - z^2)^((dim-3)/2) dz of dim space-time dimensions
+int gfo_make_quadrature_dim(int kind, int n, double step, double dim, double* nodes, double* weights) {
+  if (!(dim >= 1 && dim <= 8)) return 2;
+  return make_quadrature_alpha(kind, n, step, ((long double)dim - 3) / 2, nodes, weights);
 }
 
 int gfo_make_grid(double re_min, double re_max, int n_re, double im_min, double im_max, int n_im,

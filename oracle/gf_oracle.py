@@ -18,7 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "gf_oracle.cpp")
 _LIB = os.path.join(_HERE, "libgf_oracle.so")
 
-QUAD = {"gauss_legendre": 0, "gauss_cheb2": 1, "tanh_sinh": 2}
+QUAD = {"gauss_legendre": 0, "gauss_cheb2": 1, "tanh_sinh": 2, "gauss_cheb1": 3}
 MEASURE = {"plain": 0, "sqrt1mz2": 1}
 PROP = {"massive": 0, "rational": 1}
 CONTOUR = {"real": 0, "ray_arc": 1, "thread": 2, "auto": 3}
@@ -102,6 +102,16 @@ def make_quadrature(kind, n, step=0.0, measure="plain"):
                                    _dp(x), _dp(w))
     if rc:
         raise ValueError("gfo_make_quadrature failed: %d" % rc)
+    return x, w
+
+
+def make_quadrature_dim(kind, n, dim, step=0.0):
+    """The rule for the angular measure (1 - z^2)^((dim-3)/2) dz of `dim` space-time dimensions."""
+    x = np.empty(n, dtype=np.float64)
+    w = np.empty(n, dtype=np.float64)
+    rc = lib().gfo_make_quadrature_dim(QUAD[kind], int(n), ctypes.c_double(step), ctypes.c_double(dim), _dp(x), _dp(w))
+    if rc:
+        raise ValueError("gfo_make_quadrature_dim failed: %d" % rc)
     return x, w
 
 

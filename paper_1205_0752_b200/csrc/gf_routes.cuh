@@ -28,8 +28,10 @@ constexpr int kGoertzelUnroll = GF_GOERTZEL_UNROLL;   // trips of the series loo
 #define GF_NEAR_UNROLL 1
 #endif
 constexpr int kNearUnroll = GF_NEAR_UNROLL;           // trips of the plain direct loop (4 pairs each) unrolled
-// MOMENT route when max(|Re zeta|, |Im zeta|) >= 4.5 (then |zeta - 1/2| >= 4); the value is written out in
-// route_setup as the high word 0x40120000
+// MOMENT route when max(|Re zeta|, |Im zeta|) >= 4.5 (then |zeta - 1/2| >= 4), compared on the high words
+#ifndef GF_MOMENT_HIWORD
+#define GF_MOMENT_HIWORD 0x40120000
+#endif
 constexpr double kTau64 = 0x1p-8;     // EXACT route inside this distance of [0,1] (FP64)
 constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only good further away
 // Kreq table: bins of log2(rho) from kEllLo in steps of kEllStep (the lower edge of a bin decides, so K is safe)
@@ -413,7 +415,7 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
   SeriesArg o;
   // |Re zeta| or |Im zeta| >= 4.5, compared on the high words (4.5 = 0x40120000'00000000) to keep the test off the
   // FP64 pipe; a NaN lands here too and stays a NaN
-  if (max(__double2hiint(zeta.re) & 0x7fffffff, __double2hiint(zeta.im) & 0x7fffffff) >= 0x40120000) {
+  if (max(__double2hiint(zeta.re) & 0x7fffffff, __double2hiint(zeta.im) & 0x7fffffff) >= GF_MOMENT_HIWORD) {
     o.route = ROUTE_MOMENT;
     const double zc = zeta.re - 0.5;
     const double in = rcp_fast(fma(zc, zc, zeta.im * zeta.im));   // |zeta| < 2^500 (gf.h: domain)

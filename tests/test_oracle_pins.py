@@ -336,6 +336,25 @@ def test_parity_variant_rounding_error_is_negligible(oracle, x):
     assert relerr(gq, [ref])[0] < 1e-15
 
 
+@pytest.mark.parametrize("case", ["rational_real", "rational_ray_arc", "bubble_ray_arc", "bubble_thread",
+                                  "bubble_ray_arc_near_axis"])
+def test_parity_variants_on_rational_lines_and_deformed_contours(oracle, case):
+    """The same check off the REAL contour and for a rational line 2: the `extended` and `quad` term variants share
+    one template with the massive REAL case, these instances of it are pinned to the 60-digit sum of the definition
+    too (complex nodes, the rational form of prop_diff)."""
+    lp, contour, x = {"rational_real": (RAT, "real", -2.0 + 3.0j), "rational_ray_arc": (RAT, "ray_arc", -1.5 + 2.5j),
+                      "bubble_ray_arc": (BUB, "ray_arc", 2.0 - 4.0j), "bubble_thread": (BUB, "thread", -6.0 + 1e-3j),
+                      "bubble_ray_arc_near_axis": (BUB, "ray_arc", -3.0 + 0.05j)}[case]
+    P = oracle.make_params(BUB, lp, 1e4, contour=contour)
+    rn, rw = oracle.make_radial_pyramid(32, levels=4)
+    z, wz = oracle.make_quadrature("gauss_cheb2", 33, measure="sqrt1mz2")
+    ref = MPR.finite_sum(oracle, P, x, rn, rw, 32, z, wz, digits=60)
+    g, _ = oracle.eval_grid(P, rn, rw, 32, z, wz, np.array([x]), accum="extended")
+    assert relerr(g, [ref])[0] < 1e-13, (g, ref)
+    gq, _ = oracle.eval_grid(P, rn, rw, 32, z, wz, np.array([x]), accum="quad")
+    assert relerr(gq, [ref])[0] < 1e-15, (gq, ref)
+
+
 # ---------------------------------------------------------------- contours (a3)
 def test_real_contour_fails_outside_parabola(oracle):
     """R2: outside the parabola the REAL sum is NOT the continuation."""
@@ -465,7 +484,7 @@ def test_oracle_rejects_unsupported(oracle):
     rn, rw, z, wz = tables(oracle, 64, 32)
     xs = np.array([1 + 1j])
     with pytest.raises(ValueError):
-        oracle.eval_grid(oracle.make_params(BUB, BUB, 1e6, taylor_order=1), rn, rw, 64, z, wz, xs)
+        oracle.eval_grid(oracle.make_params(BUB, BUB, 1e6, taylor_order=5), rn, rw, 64, z, wz, xs)
     with pytest.raises(ValueError):
         oracle.eval_grid(oracle.make_params(BUB, BUB, -1.0), rn, rw, 64, z, wz, xs)
     with pytest.raises(ValueError):
@@ -489,6 +508,31 @@ def test_kernel3_angular_integral_closed_form(oracle, mu):
         assert relerr(B, ref).max() < 1e-12, (x, relerr(B, ref))
     # x = 0: the integrand vanishes identically (the factor d of eq. (20))
     assert np.all(oracle.eval_angular(P, 0.0, z, wz, np.array([1.0 + 1j, 3.0])) == 0)
+
+
+def test_kernel3_binary128_variant_at_large_ratio(oracle):
+    """The binary128 term variant (the reference Kernel 3's GPU parity uses) where the other variants run out of digits:
+    |y/x| = 1e6 and 1e-6, where the +-z terms cancel by 2 sqrt(|y/x|) and the leading moment by another 1e7.  Against
+    the definition sum_j w'_j [D2(u_j) - D2(y)]/D2(y) on the same tables at 60 digits, and (looser: the tables are
+    rounded to double, which moves a sum that cancels by 1e12) against the textbook angular integral."""
+    P = oracle.make_params(BUB, BUB, 1e6)
+    z, wz = oracle.make_quadrature("gauss_cheb2", 512, measure="sqrt1mz2")
+    for x, ys in ((1.0 + 0.5j, np.array([1e6 + 2e5j, -3e5 + 1e6j])), (2e5 - 1e6j, np.array([1.0 + 0.3j, 0.2 - 0.9j]))):
+        B = oracle.eval_angular(P, x, z, wz, ys, terms="binary128")
+        with mp.workdps(60):
+            ref, cf = [], []
+            for y in ys:
+                xm, ym = mp.mpc(x), mp.mpc(complex(y))
+                b2 = 2 * mp.sqrt(xm) * mp.sqrt(ym)
+                D2 = lambda u: 1 / (u + 1)
+                ref.append(complex(mp.fsum(mp.mpf(float(w)) * (D2(xm + ym - b2 * mp.mpf(float(t))) - D2(ym)) / D2(ym)
+                                           for t, w in zip(z, wz))))
+                cf.append(complex(CF.angular_B_massive(x, y, 1.0)))
+        assert relerr(B, ref).max() < 1e-15, (x, relerr(B, ref))
+        assert relerr(B, cf).max() < 1e-8, (x, relerr(B, cf))
+        if abs(x) < 10:   # |y/x| = 1e6: the double variant is not good enough there, which is why binary128 exists
+            Bd = oracle.eval_angular(P, x, z, wz, ys, terms="double")
+            assert relerr(Bd, ref).max() > 1e-9
 
 
 def test_kernel3_is_the_inner_sum_of_the_scan(oracle):
@@ -515,7 +559,7 @@ def test_kernel4_obstruction_is_the_parabola(oracle):
     a grid must agree.  Catches a wrong branch continuation of eq. (25), a wrong sign test, an off-by-one in z."""
     re, im = np.linspace(-6, 3, 91), np.linspace(-4, 4, 81)
     X = re[None, :] + 1j * im[:, None]
-    for m2 in (1.0, 0.25):
+    for m2 in (1.0, 0.25, 2.5):
         P = oracle.make_params(BUB, {"kind": "massive", "m2": m2}, 1e6)
         c = oracle.cut_crossings(P, X, 2001)
         margin = X.real - (X.imag ** 2 / (4 * m2) - m2)
@@ -630,3 +674,145 @@ def test_symmetric_routing_argument_checks(oracle):
         args.update(kw)
         with pytest.raises(ValueError):
             oracle.eval_grid(oracle.make_params(**args), rn, rw, 64, z, wz, np.array([1.0]))
+
+
+# ---------------------------------------------------------------- rules of other dimensions
+def _angular_moment(alpha, k):
+    """int_-1^1 (1-z^2)^alpha z^(2k) dz = B(k + 1/2, alpha + 1)."""
+    return float(mp.beta(mp.mpf(k) + mp.mpf(1) / 2, mp.mpf(alpha) + 1))
+
+
+@pytest.mark.parametrize("n", [1, 2, 7, 32, 129])
+def test_cheb1_is_the_gauss_rule_of_d2(oracle, n):
+    """Gauss-Chebyshev of the first kind (A-S 25.4.38): z_j = cos((2j-1) pi/2n), weights pi/n, exact for
+    int (1-z^2)^(-1/2) z^(2k) dz = pi (2k)!/(4^k k!^2) up to degree 2n-1.  Catches second-kind nodes, a wrong weight."""
+    z, w = oracle.make_quadrature_dim("gauss_cheb1", n, 2.0)
+    assert np.allclose(w, math.pi / n, rtol=2e-15)
+    assert np.array_equal(z, -z[::-1]) and (np.all(np.diff(z) > 0) or n == 1)
+    assert abs(z[-1] - math.cos(math.pi / (2 * n))) < 2e-16
+    for k in range(0, min(n, 12)):
+        exact = math.pi * math.factorial(2 * k) / (4 ** k * math.factorial(k) ** 2)
+        assert abs(np.sum(w * z ** (2 * k)) - exact) < 4e-15 * exact * max(1, n / 8)
+    if 2 <= n <= 32:   # a Gauss rule of n nodes: degree 2n is off by exactly -pi 2^(1-2n) (sum_j T_2n(z_j) pi/n = -pi)
+        exact = math.pi * math.factorial(2 * n) / (4 ** n * math.factorial(n) ** 2)
+        assert abs((np.sum(w * z ** (2 * n)) - exact) / (-math.pi * 2.0 ** (1 - 2 * n)) - 1) < 1e-3 * 4.0 ** max(0, n - 20)
+
+
+@pytest.mark.parametrize("dim", [2.0, 3.0, 3.5, 4.0, 5.0, 6.0])
+@pytest.mark.parametrize("kind", ["gauss_legendre", "gauss_cheb1", "gauss_cheb2", "tanh_sinh"])
+def test_rules_of_the_d_dimensional_angular_measure(oracle, kind, dim):
+    """make_quadrature_dim integrates (1-z^2)^((d-3)/2) z^(2k) dz = B(k+1/2, (d-1)/2): exactly (to rounding) for the
+    Gauss rule of that measure (Legendre d=3, Chebyshev-1 d=2, Chebyshev-2 d=4), within the rule's error otherwise.
+    d = 3 and d = 4 reproduce the tables of make_quadrature bit for bit."""
+    alpha = (dim - 3) / 2
+    n = 97 if kind == "tanh_sinh" else 64
+    z, w = oracle.make_quadrature_dim(kind, n, dim)
+    # the Gauss rule of the measure, and the Chebyshev rules wherever the remaining power of sin(theta) is even (the
+    # midpoint / trapezoid rule in theta is then exact for the cosine polynomial; Chebyshev-2 has no end nodes, so it
+    # needs at least sin^2)
+    exact_rule = {("gauss_legendre", 3.0), ("gauss_cheb1", 2.0), ("gauss_cheb1", 4.0), ("gauss_cheb1", 6.0),
+                  ("gauss_cheb2", 4.0), ("gauss_cheb2", 6.0)}
+    for k in range(6):
+        ref = _angular_moment(alpha, k)
+        err = abs(np.sum(w * z ** (2 * k)) - ref) / ref
+        if (kind, dim) in exact_rule:
+            assert err < 1e-14, (k, err)          # polynomial x natural weight: exact
+        elif kind == "tanh_sinh":
+            assert err < (1e-10 if alpha >= 0 else 2e-5), (k, err)   # end-point singularity z^2-1 at d = 2
+        else:
+            assert err < (0.1 if alpha < 0 else 5e-3), (k, err)   # algebraic convergence where the weight is not smooth
+    if dim in (3.0, 4.0) and kind != "gauss_cheb1":
+        z0, w0 = oracle.make_quadrature(kind, n, measure="plain" if dim == 3.0 else "sqrt1mz2")
+        assert np.array_equal(z, z0) and np.array_equal(w, w0)
+    assert np.allclose(z, -z[::-1], rtol=0, atol=3e-16) and np.allclose(w, w[::-1], rtol=1e-14, atol=0)
+
+
+def test_dimension_2_bubble_with_the_cheb1_rule(oracle):
+    """d = 2 through the rule of its own measure: the angular integral int (1-z^2)^(-1/2)/(A - b z) dz = pi/sqrt(A^2-b^2)
+    is reproduced by Chebyshev-1 to rounding where Gauss-Legendre with the weight folded in is off by 1e-3 (the rule,
+    not the measure, is what the dimension changes: PAPER.md:138)."""
+    A, b = 3.0, 1.0
+    z, w = oracle.make_quadrature_dim("gauss_cheb1", 32, 2.0)
+    assert abs(np.sum(w / (A - b * z)) - math.pi / math.sqrt(A * A - b * b)) < 1e-14
+    zg, wg = oracle.make_quadrature_dim("gauss_legendre", 32, 2.0)
+    assert 1e-4 < abs(np.sum(wg / (A - b * zg)) - math.pi / math.sqrt(A * A - b * b)) < 1e-1
+
+
+# ---------------------------------------------------------------- Taylor subtraction of order n (eq. (12),(13))
+@pytest.mark.parametrize("n", [1, 2, 3])
+@pytest.mark.parametrize("lines", ["bubble", "unequal_complex", "rational"])
+def test_taylor_order_matches_the_definition(oracle, n, lines):
+    """(1 - t^n) F with t^n of eq. (13) read as the Taylor operator in p (reading G20): the oracle's
+    combined form against the definition itself -- F minus its Taylor polynomial, differentiated numerically at 100+
+    digits (tests/mp_reference.py) -- on small rules.  Catches a wrong binomial, a dropped or extra term of the
+    polynomial, a wrong remainder, for massive and rational lines."""
+    lk, lp = {"bubble": (BUB, BUB), "unequal_complex": ({"kind": "massive", "m2": 0.5j}, {"kind": "massive", "m2": 2 - 0.5j}),
+              "rational": (BUB, RAT)}[lines]
+    P = oracle.make_params(lk, lp, 1e4, taylor_order=n)
+    rn, rw = oracle.make_quadrature("gauss_legendre", 12)
+    z, wz = oracle.make_quadrature("gauss_cheb2", 9, measure="sqrt1mz2")
+    for x in (0.5 + 0.2j, -2.0 + 1.5j, 3e-3 - 1e-3j, 40.0 + 9j):
+        ref = MPR.finite_sum(oracle, P, x, rn, rw, 12, z, wz, digits=60)
+        g, _ = oracle.eval_grid(P, rn, rw, 12, z, wz, np.array([x]), accum="quad")
+        assert relerr(g, [ref])[0] < 1e-15, (x, g, ref)
+        g, _ = oracle.eval_grid(P, rn, rw, 12, z, wz, np.array([x]), accum="extended")
+        assert relerr(g, [ref])[0] < 2e-13, (x, g, ref)
+
+
+@pytest.mark.parametrize("n", [1, 2])
+def test_taylor_order_closed_form_of_the_bubble(oracle, n):
+    """Subtracting t^n under the integral removes the first n Taylor coefficients of G: with CF1's series
+    -tau/6 + tau^2/60 - ..., G_1 = CF1 + x/(6 m^2), G_2 = G_1 - x^2/(60 m^4).  Catches a wrong sign or
+    order of the subtracted terms; the tight tolerance needs the Gauss rule of the measure."""
+    xs = [0.5 + 0.2j, 1 + 2j, 3.0, -0.5 + 0.3j, 0.05 - 0.02j]
+    g = G(oracle, xs, cutoff2=1e6, n_rad=256, n_ang=128, taylor_order=n)
+    with mp.workdps(40):
+        ref = [CF.cf1(x) + mp.mpc(x) / 6 - (mp.mpc(x) ** 2 / 60 if n == 2 else 0) for x in xs]
+        ref = [complex(r) for r in ref]
+    assert np.max(relerr(g, ref)) < 3e-12
+
+
+def test_taylor_order_rational_line_against_cf3(oracle):
+    """Config 4's lines: G_1(x) = CF3(x) - x CF3'(0), the derivative of the Feynman-parameter form taken numerically."""
+    xs = [0.5 + 0.2j, 1 + 1j]
+    g = G(oracle, xs, line_k=BUB, line_pk=RAT, cutoff2=1e6, n_rad=256, n_ang=128, taylor_order=1)
+    with mp.workdps(30):
+        d0 = mp.diff(lambda t: CF.cf3_rational(t, 1.0, 2.0, 0.5, 1.2), 0, h=mp.mpf("1e-8"))
+        ref = [complex(CF.cf3_rational(x, 1.0, 2.0, 0.5, 1.2) - mp.mpc(x) * d0) for x in xs]
+    assert np.max(relerr(g, ref)) < 1e-10
+
+
+def test_taylor_order_invariants_and_cutoff(oracle):
+    """G_n(0) = 0 exactly and G_n = O(x^(n+1)) (G_1/x^2 -> 1/60 m^4); conjugation symmetry bitwise; the cutoff error of
+    G_1 falls at least as fast as order 0's Lambda^-4 (BPHZ ensures cut-off independence)."""
+    rn, rw, z, wz = tables(oracle, 256, 128, ang="gauss_cheb2", levels=1)
+    P1 = oracle.make_params(BUB, BUB, 1e6, taylor_order=1)
+    g, _ = oracle.eval_grid(P1, rn, rw, 256, z, wz, np.array([0.0, 1e-4, 1e-4j]), accum="extended")
+    assert g[0] == 0
+    assert abs(g[1] / 1e-8 - 1 / 60) < 1e-5 and abs(g[2] / -1e-8 - 1 / 60) < 1e-5
+    xs = np.array([0.7 - 1.1j, -3 + 0.5j, 2e-3 + 1e-3j])
+    a, _ = oracle.eval_grid(P1, rn, rw, 256, z, wz, xs)
+    b, _ = oracle.eval_grid(P1, rn, rw, 256, z, wz, np.conj(xs))
+    assert np.array_equal(b, np.conj(a))
+    x = np.array([0.5 + 0.2j])
+    ref = complex(CF.cf1(x[0])) + x[0] / 6
+    err = []
+    for c2 in (1e2, 1e3, 1e4):
+        Pc = oracle.make_params(BUB, BUB, c2, taylor_order=1)
+        gc, _ = oracle.eval_grid(Pc, rn, rw, 256, z, wz, x)
+        err.append(abs(gc[0] - ref))
+    p1, p2 = math.log10(err[0] / err[1]), math.log10(err[1] / err[2])
+    assert p1 > 1.9 and p2 > 1.9, (err, p1, p2)   # error ~ Lambda^-4 or faster: two decades per decade of Lambda^2
+
+
+def test_taylor_order_argument_checks(oracle):
+    rn, rw, z, wz = tables(oracle, 64, 32)
+    for kw in (dict(taylor_order=-1), dict(taylor_order=5), dict(taylor_order=1, routing="symmetric"), dict(sub=1.0)):
+        args = dict(line_k=BUB, line_pk=BUB, cutoff2=1e4)
+        args.update(kw)
+        with pytest.raises(ValueError):
+            oracle.eval_grid(oracle.make_params(**args), rn, rw, 64, z, wz, np.array([1.0]))
+    # order 0 through the new code path selector is the old value, bit for bit
+    g0, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e4, taylor_order=0), rn, rw, 64, z, wz, np.array([1.0 + 1j]))
+    g1, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e4, taylor_order=1), rn, rw, 64, z, wz, np.array([1.0 + 1j]))
+    assert g0[0] != g1[0] and abs(g1[0] - (g0[0] + (1 + 1j) / 6)) < 1e-3
