@@ -27,7 +27,8 @@
  *   - Grids are stored [n_im][n_re], the real index fastest (the paper's X(M,N) with M along
  *     the real axis, Fortran order).
  *   - Errors: GF_ERR_NULL for a null pointer, GF_ERR_ARG for a value out of range,
- *     GF_ERR_UNSUPPORTED for a combination the method does not define (taylor_order != 0, a
+ *     GF_ERR_UNSUPPORTED for a combination the method does not define or that is not built (taylor_order outside
+ *     [0, 4], taylor_order > 0 off the REAL contour, with the symmetric routing or with precision 32, a
  *     subtraction point other than 0, a dimension other than 4 or the symmetric routing on a
  *     deformed contour, the symmetric routing with unequal or rational lines, the THREAD contour
  *     with unequal or complex masses, a rational propagator with a double pole, precision 32 on a
@@ -48,7 +49,8 @@ typedef enum { GF_OK = 0, GF_ERR_NULL = 1, GF_ERR_ARG = 2, GF_ERR_UNSUPPORTED = 
 /* Quadrature rules on [-1,1]: Gauss-Legendre (the paper's radial rule, and the
  * angular rule of BASELINE.json's configs), Gauss-Chebyshev of the 2nd kind (the paper's check
  * rule; the exact Gauss rule for the d=4 angular measure), tanh-sinh (the paper's angular rule). */
-typedef enum { GF_QUAD_GAUSS_LEGENDRE = 0, GF_QUAD_GAUSS_CHEB2 = 1, GF_QUAD_TANH_SINH = 2 } gf_quad_kind;
+typedef enum { GF_QUAD_GAUSS_LEGENDRE = 0, GF_QUAD_GAUSS_CHEB2 = 1, GF_QUAD_TANH_SINH = 2,
+               GF_QUAD_GAUSS_CHEB1 = 3 /* first kind: the exact Gauss rule of the d = 2 angular measure */ } gf_quad_kind;
 
 /* Which measure the returned weights integrate against: dz (radial rules), or the d=4
  * hyperspherical angular measure sqrt(1-z^2) dz of eq. (9)/(11). */
@@ -109,7 +111,12 @@ typedef struct {
   gf_propagator line_pk; /* D2(u): the line carrying p - k */
   double cutoff2;        /* Lambda^2 in (0, 1e60], upper limit of the radial integral */
   double sub_re, sub_im; /* subtraction point x0 of t^n; only 0 is supported (eq. (13)) */
-  int taylor_order;      /* n of t^n; only 0 is supported (log-divergent integrals) */
+  int taylor_order;      /* n of the Taylor subtraction t^n of eq. (12),(13), 0 <= n <= 4.  0 is the
+                            paper's worked example (log-divergent integrals).  "x = 0" in eq. (13) is
+                            p = 0 (eq. (20) sets the scalar product to zero with x): t^n is the Taylor operator in the
+                            external momentum, x^i standing for the order 2i in p, so (1 - t^n) F is F minus every
+                            term of its expansion in p up to the order 2n and G_n = G - sum_{i<=n} x^i G^(i)(0)/i! =
+                            O(x^(n+1)).  n > 0: REAL contour, the paper's routing, precision 64 (any dim) */
   double prefactor;      /* c0; 1/(2 pi)^3 is eq. (14), 2/pi the rescaled eq. (21) */
   double map_scale;      /* s0 > 0 of the shifted-log radial map y(u) = a + (a+s0) expm1(u L) */
   int contour;           /* gf_contour */
@@ -122,7 +129,8 @@ typedef struct {
                             instead of Re x > (Im x)^2/(4 m^2) - m^2 */
   double dim;            /* space-time dimension d in [1, 8], 0 meaning 4 ("arbitrary dimensions by
                             trivial modifications"): the radial measure becomes dy y^((d-2)/2); the angular measure
-                            (1-z^2)^((d-3)/2) is the caller's, in the angular weights (GF_MEASURE_PLAIN is d = 3).
+                            (1-z^2)^((d-3)/2) is the caller's, in the angular weights (gf_make_quadrature_dim makes them;
+                            GF_MEASURE_PLAIN is d = 3).
                             d != 4 on the REAL contour only.  Constants of the d-dimensional measure go into
                             `prefactor` (d^dk = 1/2 y^((d-2)/2) dy dOmega_d). */
 } gf_params;
@@ -154,6 +162,16 @@ int gf_make_quadrature(int kind, int n, double step, int measure, double* d_node
 
 /* The same tables into HOST arrays (no CUDA call is made). */
 int gf_make_quadrature_host(int kind, int n, double step, int measure, double* h_nodes, double* h_weights);
+
+/* The angular rule of `dim` space-time dimensions ("arbitrary dimensions by trivial modifications"): nodes
+ * of rule `kind` and weights that integrate against (1 - z^2)^((dim-3)/2) dz, dim in [1, 8] -- what gf_params.dim
+ * expects in the angular weights.  The paper uses "Gauss-Chebyshev ... polynomials of the first and second kind ...
+ * depending on the dimension": GF_QUAD_GAUSS_CHEB1 is the exact Gauss rule of dim = 2 (z_j =
+ * cos((2j-1) pi/2n), weights pi/n), GF_QUAD_GAUSS_CHEB2 of dim = 4, GF_QUAD_GAUSS_LEGENDRE of dim = 3; for another dim
+ * the remaining power of (1 - z^2) = sin^2(theta) goes into the weights.  dim = 3 and dim = 4 give the tables of
+ * gf_make_quadrature with GF_MEASURE_PLAIN and GF_MEASURE_SQRT1MZ2 bit for bit.  Otherwise as gf_make_quadrature. */
+int gf_make_quadrature_dim(int kind, int n, double step, double dim, double* d_nodes, double* d_weights, void* stream);
+int gf_make_quadrature_dim_host(int kind, int n, double step, double dim, double* h_nodes, double* h_weights);
 
 /* Doubles needed for the radial tables of a contour policy: n_rad for REAL; for the other policies
  * the pyramid n_rad + n_rad/2 + n_rad/4 + n_rad/8 (rules of those orders back to back -- the paper's

@@ -14,7 +14,7 @@ import torch
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libgf_b200.so")
 
-QUAD = {"gauss_legendre": 0, "gauss_cheb2": 1, "tanh_sinh": 2}
+QUAD = {"gauss_legendre": 0, "gauss_cheb2": 1, "tanh_sinh": 2, "gauss_cheb1": 3}
 MEASURE = {"plain": 0, "sqrt1mz2": 1}
 PROP = {"massive": 0, "rational": 1}
 CONTOUR = {"real": 0, "ray_arc": 1, "thread": 2, "auto": 3}
@@ -62,6 +62,8 @@ _SIGNATURES = {
     "gf_make_grid_rows": [_dbl, _dbl, _int, _dbl, _dbl, _int, _int, _dbl, _int, _int, _vp, _vp],
     "gf_make_quadrature": [_int, _int, _dbl, _int, _vp, _vp, _vp],
     "gf_make_quadrature_host": [_int, _int, _dbl, _int, _vp, _vp],
+    "gf_make_quadrature_dim": [_int, _int, _dbl, _dbl, _vp, _vp, _vp],
+    "gf_make_quadrature_dim_host": [_int, _int, _dbl, _dbl, _vp, _vp],
     "gf_radial_table_size": [_int, _int],
     "gf_eval_grid": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
     "gf_eval_grid_counted": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp, _vp],
@@ -192,6 +194,25 @@ def make_quadrature_host(kind, n, step=0.0, measure="plain"):
     weights = np.empty(n, dtype=np.float64)
     _check(lib().gf_make_quadrature_host(QUAD[kind], n, step, MEASURE[measure], nodes.ctypes.data,
                                          weights.ctypes.data))
+    return nodes, weights
+
+
+def make_quadrature_dim(kind, n, dim, step=0.0, device=None, stream=None):
+    """gf_make_quadrature_dim: the rule for the angular measure (1 - z^2)^((dim-3)/2) dz, on the device."""
+    dev = _device(device)
+    nodes = torch.empty(n, dtype=torch.float64, device=dev)
+    weights = torch.empty(n, dtype=torch.float64, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib().gf_make_quadrature_dim(QUAD[kind], n, step, float(dim), nodes.data_ptr(), weights.data_ptr(),
+                                            _stream(stream)))
+    return nodes, weights
+
+
+def make_quadrature_dim_host(kind, n, dim, step=0.0):
+    """gf_make_quadrature_dim_host: the same tables as numpy arrays (no CUDA call)."""
+    nodes = np.empty(n, dtype=np.float64)
+    weights = np.empty(n, dtype=np.float64)
+    _check(lib().gf_make_quadrature_dim_host(QUAD[kind], n, step, float(dim), nodes.ctypes.data, weights.ctypes.data))
     return nodes, weights
 
 

@@ -102,7 +102,11 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   if (!std::isfinite(p->prefactor)) { set_error("eval_grid: prefactor not finite"); return GF_ERR_ARG; }
   if (p->precision != 64 && p->precision != 32) { set_error("eval_grid: precision must be 64 or 32"); return GF_ERR_ARG; }
   if (p->contour < GF_CONTOUR_REAL || p->contour > GF_CONTOUR_AUTO) { set_error("eval_grid: unknown contour %d", p->contour); return GF_ERR_ARG; }
-  if (p->taylor_order != 0) { set_error("eval_grid: taylor_order %d unsupported (only t^0, eq. (13))", p->taylor_order); return GF_ERR_UNSUPPORTED; }
+  if (p->taylor_order < 0 || p->taylor_order > kMaxTaylor) { set_error("eval_grid: taylor_order %d outside [0, %d] (eq. (13))", p->taylor_order, kMaxTaylor); return GF_ERR_UNSUPPORTED; }
+  if (p->taylor_order > 0 && (p->contour != GF_CONTOUR_REAL || p->routing != 0 || p->precision != 64)) {
+    set_error("eval_grid: taylor_order > 0 is built for the REAL contour, the paper's routing and precision 64");
+    return GF_ERR_UNSUPPORTED;
+  }
   if (p->sub_re != 0 || p->sub_im != 0) { set_error("eval_grid: subtraction point must be 0 (eq. (13))"); return GF_ERR_UNSUPPORTED; }
   if (p->routing != 0 && p->routing != 1) { set_error("eval_grid: unknown routing %d", p->routing); return GF_ERR_ARG; }
   if (p->routing == 1 && !(p->contour == GF_CONTOUR_REAL && p->line_k.kind == GF_PROP_MASSIVE && p->line_pk.kind == GF_PROP_MASSIVE &&
@@ -127,6 +131,7 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   log_ratio_dd(0.0, p->cutoff2, p->map_scale, &a->Llog_hi, &a->Llog_lo);  // REAL contour: [0, Lambda^2]
   a->contour = p->contour;
   a->routing = p->routing;
+  a->taylor_order = p->taylor_order;
 
   // line 2 as a sum of simple poles R_r/(u + mu_r)
   const gf_propagator& q = p->line_pk;
@@ -260,6 +265,21 @@ int gf_make_quadrature(int kind, int n, double step, int measure, double* d_node
   if (rc) return rc;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   // pageable source: the runtime stages the data before returning, so x, w may go out of scope
+  if ((rc = check_cuda(cudaMemcpyAsync(d_nodes, x.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy nodes"))) return rc;
+  return check_cuda(cudaMemcpyAsync(d_weights, w.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy weights");
+}
+
+int gf_make_quadrature_dim_host(int kind, int n, double step, double dim, double* h_nodes, double* h_weights) {
+  return make_rule_dim_host(kind, n, step, dim, h_nodes, h_weights);
+}
+
+int gf_make_quadrature_dim(int kind, int n, double step, double dim, double* d_nodes, double* d_weights, void* stream) {
+  if (!d_nodes || !d_weights) { set_error("make_quadrature_dim: null device pointer"); return GF_ERR_NULL; }
+  if (n < 1 || n > (1 << 20)) { set_error("make_quadrature_dim: n=%d out of range", n); return GF_ERR_ARG; }
+  std::vector<double> x(n), w(n);
+  int rc = make_rule_dim_host(kind, n, step, dim, x.data(), w.data());
+  if (rc) return rc;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
   if ((rc = check_cuda(cudaMemcpyAsync(d_nodes, x.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy nodes"))) return rc;
   return check_cuda(cudaMemcpyAsync(d_weights, w.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy weights");
 }
@@ -485,6 +505,13 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
   out->n_terms = a.n_terms;
   out->series_terms_max = plan.layout.kmc;
   out->evals = (double)n_points * n_rad * n_ang;
+  if (a.taylor_order > 0) {   // gf_taylor.cu has no instruction model: launch shape only, the per-unit counts stay 0
+    out->near_pair_dfma = out->near_pair_other = out->near_pair_fp32 = out->series_term_dfma = out->series_term_other =
+        out->series_term_fp32 = out->exact_pair_dfma = out->exact_pair_other = out->node_near_dfma = out->node_near_other =
+            out->node_moment_dfma = out->node_moment_other = out->node_cheb_dfma = out->node_cheb_other =
+                out->node_exact_dfma = out->node_exact_other = out->tail_dfma = out->tail_other = 0.0;
+    return GF_OK;
+  }
   // FP64-pipe instructions per unit of each route, counted per SASS region in the ncu source page of
   // eval_real_kernel<double, false, 1> (profiles/r01h_eval_ncu_full.md; DSETP not counted: no flops):
   //   pair of the plain direct loop 5 DFMA + 1 DMUL + 2 DADD, of the double-double loop 5 + 1 + 4;

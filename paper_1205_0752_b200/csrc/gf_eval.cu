@@ -117,7 +117,7 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
   __syncthreads();  // the T_k(s_j) matrix, the monomial moments and the radial tables are complete
   prep_series_sums(a, L, blob, s_cpart);
   __syncthreads();
-  prep_series_kreq(L, blob, s_lc);
+  prep_series_kreq(L, blob, s_lc, blob + L.off_cheb, 2);
   if (L.off_gam >= 0) {
     prep_tail_gamma(L, blob, s_part, s_mu, s_nu);
     const TailJob J = real_tail_job(a, L, blob);
@@ -347,6 +347,7 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
 
 // ---------------------------------------------------------------------------------------------
 int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
+  if (a.taylor_order > 0) return plan_taylor(a, plan);
   plan->block_threads = kBlockThreads;
   plan->shared_nodes = (a.contour == GF_CONTOUR_REAL);
   // lanes per point: enough threads for >= 2 CTAs on each of the 148 SMs, at most a warp
@@ -410,6 +411,7 @@ int launch_prepare(const EvalArgs& a, int precision, double* blob, cudaStream_t 
   int rc = plan_eval(a, precision, &plan);
   if (rc) return rc;
   if ((rc = check_variant(plan, precision))) return rc;
+  if (a.taylor_order > 0) return launch_taylor_prepare(a, plan, blob, stream);
   prep_real_kernel<<<1, 256, 0, stream>>>(a, plan.layout, blob);
   if ((rc = check_cuda(cudaGetLastError(), "prep kernel launch"))) return rc;
   return plan.shared_nodes ? GF_OK : launch_prepare_rungs(a, plan, blob, stream);
@@ -425,6 +427,10 @@ int launch_prepared(const EvalArgs& a_in, int precision, const double* blob, uns
   if ((rc = check_variant(plan, precision))) return rc;
   EvalArgs a = a_in;
   a.split_log2 = plan.split_log2;
+  if (a.taylor_order > 0) {
+    if (d_counters) { set_error("eval_grid_counted: the route counters exist for taylor_order 0 only"); return GF_ERR_UNSUPPORTED; }
+    return launch_taylor(a, plan, blob, stream);
+  }
   if (!plan.shared_nodes) return launch_contour(a, plan, blob, d_counters, stream);
   if (d_counters)
     return precision == 32 ? launch_real<float, true>(a, plan, blob, d_counters, stream)

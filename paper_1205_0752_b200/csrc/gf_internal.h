@@ -15,6 +15,7 @@ struct PoleTerm {
 };
 
 constexpr int kMaxTerms = 2;
+constexpr int kMaxTaylor = 4;   // largest order n of the Taylor subtraction t^n (gf_taylor.cu)
 #ifndef GF_BLOCK_THREADS
 #define GF_BLOCK_THREADS 256
 #endif
@@ -56,6 +57,7 @@ struct EvalArgs {
                        // parabola Re x > (Im x)^2/(4 c2) - c2 (AUTO's first test)
   int rung_lo;         // ladder index of the first tabulated contour radius (deformed contours)
   int split_log2;      // lanes per grid point = 1 << split_log2
+  int taylor_order;    // n of the Taylor subtraction t^n (eq. (13)); n > 0 runs gf_taylor.cu
 };
 
 // Offsets (in doubles) of the prepared tables, as the preparation kernel writes them and every CTA of the
@@ -92,6 +94,8 @@ struct BlobLayout {
   int n_rungs;                  // rows (kRungs + 1) or 0
   int n4p, rg_r, rg_q4, rg_w, rg_y, rg_yq4, rg_pref, rg_tail, rg_s2, rg_s3;
   long long n_total;            // doubles to allocate
+  // Taylor order n > 0 (gf_taylor.cu): n_poly = n + 2 series tables per family, [k][n_poly], and 1/(y_i + mu_r)
+  int n_poly, off_momA, off_chebA, off_ic;
 };
 constexpr int kRungs = 64;      // tabulated contour radii above the first (deformed contours); then Lambda^2/2
 
@@ -111,6 +115,7 @@ int scratch_alloc(void** ptr, size_t bytes, cudaStream_t stream);  // from the l
 
 // gf_tables.cpp
 int make_rule_host(int kind, int n, double step, int measure, double* nodes, double* weights);
+int make_rule_dim_host(int kind, int n, double step, double dim, double* nodes, double* weights);
 void log_ratio_dd(double a, double b, double s0, double* hi, double* lo);  // ln((b+s0)/(a+s0)), binary128 -> (hi, lo)
 
 // gf_grid.cu
@@ -132,6 +137,11 @@ int launch_contour_nodes(const EvalArgs& a, const LaunchPlan& plan, const double
                          int* d_policy, double2* d_y, double2* d_wy, cudaStream_t stream);
 int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d_nodes, int n, double* d_y,
                       cudaStream_t stream);
+
+// gf_taylor.cu: Taylor subtraction of order n > 0 on the REAL contour
+int plan_taylor(const EvalArgs& a, LaunchPlan* plan);
+int launch_taylor_prepare(const EvalArgs& a, const LaunchPlan& plan, double* blob, cudaStream_t stream);
+int launch_taylor(const EvalArgs& a, const LaunchPlan& plan, const double* blob, cudaStream_t stream);
 
 // gf_cut.cu: the paper's Kernels 3 and 4 (a.x holds the y array / the x array, a.out the result)
 BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail,

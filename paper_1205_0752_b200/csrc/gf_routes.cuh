@@ -673,11 +673,18 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
 // j >= K, c_j the larger of the two coefficients.  For a rule that integrates the measure well the c_j beyond
 // the first few are the rule's defect (~1e-7), so far fewer terms are needed than rho^-K <= 2^-60 asks for.
 // Coefficients beyond kmc are not known: a bin is usable only if rho^-kmc <= 2^-60.
-__device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc /* [kKmc] shared */) {
+// coef: the Chebyshev tables, n_poly coefficients per k ([k][n_poly]); c_j is the largest of them in modulus.
+__device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc /* [kKmc] shared */, const double* coef,
+                                 int n_poly) {
   int* kreq = reinterpret_cast<int*>(blob + L.off_kreq);
-  const double c00 = fmax(fabs(blob[L.off_cheb]), fabs(blob[L.off_cheb + 1]));
+  auto cmax = [&](int j) {
+    double m = 0.0;
+    for (int q = 0; q < n_poly; ++q) m = fmax(m, fabs(coef[j * n_poly + q]));
+    return m;
+  };
+  const double c00 = cmax(0);
   for (int j = threadIdx.x; j < L.kmc; j += blockDim.x)   // log2 |c_j / c_0|, rounded up a little (c = 0: -inf)
-    s_lc[j] = (float)log2(fmax(fabs(blob[L.off_cheb + 2 * j]), fabs(blob[L.off_cheb + 2 * j + 1])) / c00) + 1e-3f;
+    s_lc[j] = (float)log2(cmax(j) / c00) + 1e-3f;
   __syncthreads();
   for (int b = threadIdx.x; b < kKreqBins; b += blockDim.x) {
     const float ell = kEllLo + (float)b * kEllStep;

@@ -151,22 +151,22 @@ void log_ratio_dd(double a, double b, double s0, double* hi, double* lo) {
   *lo = (double)(L - (__float128)*hi);
 }
 
-int make_rule_host(int kind, int n, double step, int measure, double* nodes, double* weights) {
+// Rule `kind` for the angular measure (1 - z^2)^alpha dz (alpha = (d-3)/2 in d dimensions; alpha = 0 is
+// the plain rule, 1/2 the d = 4 measure of eq. (9)).  Mirrored halves: exactly symmetric.
+static int make_rule_alpha(int kind, int n, double step, real alpha, double* nodes, double* weights) {
   if (!nodes || !weights) { set_error("make_quadrature: null table pointer"); return GF_ERR_NULL; }
   if (n < 1 || n > (1 << 20)) { set_error("make_quadrature: n=%d out of range [1, 2^20]", n); return GF_ERR_ARG; }
-  if (measure != GF_MEASURE_PLAIN && measure != GF_MEASURE_SQRT1MZ2) {
-    set_error("make_quadrature: unknown measure %d", measure);
-    return GF_ERR_ARG;
-  }
   if (!(step >= 0) || !std::isfinite(step)) { set_error("make_quadrature: step must be >= 0"); return GF_ERR_ARG; }
-  const bool ang = measure == GF_MEASURE_SQRT1MZ2;
+  // sin(theta)^(2 alpha + 1 - e): the power of sin left over after the rule's own weight sin^e
+  auto spow = [&](real s, real e) { const real p = 2 * alpha + 1 - e; return p == 0 ? (real)1 : p == 1 ? s : p == 2 ? s * s : powl(s, p); };
   switch (kind) {
     case GF_QUAD_GAUSS_LEGENDRE: {
       gauss_legendre(n, nodes, weights);
-      if (ang)
+      if (alpha != 0)
         for (int j = 0; j < n; ++j) {
           real z = nodes[j];
-          weights[j] = (double)((real)weights[j] * sqrtl((1 - z) * (1 + z)));
+          const real om = (1 - z) * (1 + z);
+          weights[j] = (double)((real)weights[j] * (alpha == 0.5L ? sqrtl(om) : powl(om, alpha)));
         }
       return GF_OK;
     }
@@ -175,7 +175,7 @@ int make_rule_host(int kind, int n, double step, int measure, double* nodes, dou
       for (int j = 0; j < n / 2; ++j) {
         real th = PI * (real)(j + 1) / (real)(n + 1);  // largest z first
         real s = sinl(th), c = cosl(th);
-        real wt = PI / (real)(n + 1) * s * (ang ? s : 1.0L);
+        real wt = PI / (real)(n + 1) * s * spow(s, 1);
         nodes[n - 1 - j] = (double)c;
         nodes[j] = -(double)c;
         weights[n - 1 - j] = weights[j] = (double)wt;
@@ -186,6 +186,22 @@ int make_rule_host(int kind, int n, double step, int measure, double* nodes, dou
       }
       return GF_OK;
     }
+    case GF_QUAD_GAUSS_CHEB1: {
+      // z_j = cos((2j-1) pi/(2n)), w_j = pi/n for the weight 1/sqrt(1-z^2) (A-S 25.4.38): the Gauss rule of d = 2
+      for (int j = 0; j < n / 2; ++j) {
+        real th = PI * (real)(2 * j + 1) / (real)(2 * n);  // largest z first
+        real s = sinl(th), c = cosl(th);
+        real wt = PI / (real)n * spow(s, 0);
+        nodes[n - 1 - j] = (double)c;
+        nodes[j] = -(double)c;
+        weights[n - 1 - j] = weights[j] = (double)wt;
+      }
+      if (n & 1) {
+        nodes[n / 2] = 0.0;
+        weights[n / 2] = (double)(PI / (real)n);
+      }
+      return GF_OK;
+    }
     case GF_QUAD_TANH_SINH: {
       // Takahasi-Mori (ref. [19]); default step: reading G8 of DESIGN.md
       real h = step > 0 ? (real)step : (n > 1 ? 5.8L / (real)(n - 1) : 1.0L);
@@ -193,7 +209,8 @@ int make_rule_host(int kind, int n, double step, int measure, double* nodes, dou
         real k = (real)(n - 1) / 2 - (real)j;  // k >= 0, largest first
         real arg = 0.5L * PI * sinhl(k * h);
         real sech = 1 / coshl(arg);
-        real wt = 0.5L * PI * h * coshl(k * h) * sech * sech * (ang ? sech : 1.0L);
+        // (1 - z^2)^alpha = sech^(2 alpha)
+        real wt = 0.5L * PI * h * coshl(k * h) * sech * sech * (alpha == 0 ? (real)1 : alpha == 0.5L ? sech : powl(sech, 2 * alpha));
         real z = tanhl(arg);
         nodes[n - 1 - j] = (double)z;
         nodes[j] = -(double)z;
@@ -206,6 +223,19 @@ int make_rule_host(int kind, int n, double step, int measure, double* nodes, dou
       set_error("make_quadrature: unknown rule kind %d", kind);
       return GF_ERR_ARG;
   }
+}
+
+int make_rule_host(int kind, int n, double step, int measure, double* nodes, double* weights) {
+  if (measure != GF_MEASURE_PLAIN && measure != GF_MEASURE_SQRT1MZ2) {
+    set_error("make_quadrature: unknown measure %d", measure);
+    return GF_ERR_ARG;
+  }
+  return make_rule_alpha(kind, n, step, measure == GF_MEASURE_SQRT1MZ2 ? 0.5L : 0.0L, nodes, weights);
+}
+
+int make_rule_dim_host(int kind, int n, double step, double dim, double* nodes, double* weights) {
+  if (!(dim >= 1 && dim <= 8)) { set_error("make_quadrature_dim: dim=%g outside [1, 8]", dim); return GF_ERR_ARG; }
+  return make_rule_alpha(kind, n, step, ((real)dim - 3) / 2, nodes, weights);
 }
 
 }  // namespace gf

@@ -64,6 +64,29 @@ def test_host_quadrature_is_symmetric_and_exact(gf):
     assert abs(np.sum(w) - np.pi / 2) < 1e-11
 
 
+def test_host_rules_of_the_d_dimensional_measure(gf):
+    """gf_make_quadrature_dim_host (no CUDA call): exact moments B(k+1/2, (d-1)/2) for the Gauss rule of each measure
+    (Chebyshev-1 d = 2, Legendre d = 3, Chebyshev-2 d = 4: PAPER.md:138), d = 3 / 4 identical to the fixed measures,
+    exactly mirrored tables, argument errors.  The GPU tests compare the same tables with the oracle's."""
+    from math import gamma, pi
+    for kind, dim in (("gauss_cheb1", 2.0), ("gauss_legendre", 3.0), ("gauss_cheb2", 4.0), ("gauss_cheb1", 6.0)):
+        z, w = gf.make_quadrature_dim_host(kind, 24, dim)
+        assert np.array_equal(z, -z[::-1]) and np.array_equal(w, w[::-1]) and np.all(np.diff(z) > 0)
+        for k in range(8):
+            ref = gamma(k + 0.5) * gamma((dim - 1) / 2) / gamma(k + dim / 2)
+            assert abs(np.sum(w * z ** (2 * k)) - ref) < 4e-15 * ref * 4, (kind, dim, k)
+    z, w = gf.make_quadrature_dim_host("gauss_cheb1", 5, 2.0)
+    assert np.allclose(w, pi / 5, rtol=1e-15) and abs(z[-1] - np.cos(pi / 10)) < 2e-16
+    for kind in ("gauss_legendre", "gauss_cheb2", "tanh_sinh"):
+        for dim, meas in ((3.0, "plain"), (4.0, "sqrt1mz2")):
+            a, b = gf.make_quadrature_dim_host(kind, 33, dim), gf.make_quadrature_host(kind, 33, measure=meas)
+            assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    for bad in (0.5, 9.0, float("nan")):
+        with pytest.raises(gf.GfError) as e:
+            gf.make_quadrature_dim_host("gauss_legendre", 8, bad)
+        assert e.value.status == 2
+
+
 def test_argument_errors_without_gpu(gf):
     L = gf.lib()
     bub = {"kind": "massive", "m2": 1.0}
@@ -74,7 +97,10 @@ def test_argument_errors_without_gpu(gf):
     assert L.gf_eval_launch_info(None, 64, 32, 4096, ctypes.byref(info)) == 1          # GF_ERR_NULL
     assert L.gf_eval_launch_info(ctypes.byref(P), 0, 32, 4096, ctypes.byref(info)) == 2  # GF_ERR_ARG
     assert b"n_rad" in L.gf_last_error()
-    P.taylor_order = 1
+    P.taylor_order = 1   # eq. (13) with n = 1: its own kernel, no per-route instruction model
+    assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 0
+    assert info.grid_blocks > 0 and info.series_term_dfma == 0
+    P.taylor_order = 5
     assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 3  # UNSUPPORTED
     P = gf.make_params(bub, bub, -1.0)
     assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 2

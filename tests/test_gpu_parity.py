@@ -99,6 +99,20 @@ def test_tables_match_oracle(gf, oracle, kind, n, measure):
     assert np.array_equal(xh, xg) and np.array_equal(wh, wg)
 
 
+@pytest.mark.parametrize("kind", ["gauss_legendre", "gauss_cheb1", "gauss_cheb2", "tanh_sinh"])
+@pytest.mark.parametrize("dim", [2.0, 3.0, 3.5, 4.0, 5.0])
+def test_tables_of_the_d_dimensional_measure_match_oracle(gf, oracle, kind, dim):
+    """gf_make_quadrature_dim (Gauss-Chebyshev of the first kind included) against the oracle's own
+    generator: nodes to 4 eps, weights to 64 ulp."""
+    for n in (1, 2, 31, 32, 49, 256):
+        z, w = gf.make_quadrature_dim(kind, n, dim)
+        zo, wo = oracle.make_quadrature_dim(kind, n, dim)
+        z, w = z.cpu().numpy(), w.cpu().numpy()
+        assert np.abs(z - zo).max() <= 4 * np.finfo(float).eps
+        assert (np.abs(w - wo) / np.abs(wo)).max() <= 64 * np.finfo(float).eps
+        assert np.array_equal(z, -z[::-1]) and np.array_equal(w, w[::-1])
+
+
 def test_radial_map_bit_identical(gf, oracle):
     """The REAL contour's nodes y_i = s0 expm1(u_i L): kernel (double-double) vs oracle (binary128), bit
     for bit -- next to a singularity of the integrand a 1-ulp difference of y_i moves G by more than
@@ -572,6 +586,44 @@ def test_kernel4_cut_crossings_bit_exact(gf, oracle, lines):
 
 
 # ------------------------------------------------------------------ other dimensions
+def test_kernel4_obstruction_is_the_parabola_on_the_gpu(gf):
+    """gf_cut_crossings against the statement of the paper itself, not against the oracle's procedure (which it
+    shares by construction, reading G19): the contour 'remains unharmed' exactly inside the parabola of PAPER.md:270,
+    Re x > (Im x)^2/(4 m^2) - m^2 for a real mass (three masses) and Re x > (Im x)^2 - 1/4 for the paper's mass^2 -i/2."""
+    re, im = np.linspace(-6, 3, 91), np.linspace(-4, 4, 81)
+    X = re[None, :] + 1j * im[:, None]
+    xd = torch.from_numpy(np.ascontiguousarray(X)).cuda()
+    bub = {"kind": "massive", "m2": 1.0}
+    for m2 in (1.0, 0.25, 2.5):
+        P = gf.make_params(bub, {"kind": "massive", "m2": m2}, 1e6)
+        c = gf.cut_crossings(P, xd, 2001).cpu().numpy()
+        margin = X.real - (X.imag ** 2 / (4 * m2) - m2)
+        far = np.abs(margin) > 1e-9
+        assert np.array_equal((c == 0)[far], (margin > 0)[far])
+        assert set(np.unique(c)) <= {0, 1}
+    P = gf.make_params({"kind": "massive", "m2": 0.5j}, {"kind": "massive", "m2": -0.5j}, 1e6)
+    c = gf.cut_crossings(P, xd, 2001).cpu().numpy()
+    margin = X.real - (X.imag ** 2 - 0.25)
+    far = np.abs(margin) > 1e-9
+    assert np.array_equal((c == 0)[far], (margin > 0)[far])
+
+
+def test_dimension_2_through_the_abi_alone(gf, oracle):
+    """d = 2 with the paper's rule for it (Gauss-Chebyshev of the first kind) made by
+    gf_make_quadrature_dim: no table comes from outside the library.  Parity with the oracle on its own tables."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    xs = oracle_grid(oracle, cfg)[::3, ::3].ravel()
+    P = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=1 / (4 * np.pi), dim=2.0)
+    rn, rw = gf.make_radial_tables("real", cfg["n_rad"], W.RADIAL_RULE)
+    z, wz = gf.make_quadrature_dim("gauss_cheb1", 33, 2.0)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+    Po = oracle.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=1 / (4 * np.pi), dim=2.0)
+    rno, rwo = oracle.make_quadrature(W.RADIAL_RULE, cfg["n_rad"])
+    zo, wzo = oracle.make_quadrature_dim("gauss_cheb1", 33, 2.0)
+    ref, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, xs, accum="extended")
+    assert relerr(g, ref).max() <= TOL64
+
+
 @pytest.mark.parametrize("dim,measure", [(3.0, "plain"), (2.0, "plain"), (3.5, "sqrt1mz2"), (5.0, "sqrt1mz2")])
 def test_other_dimensions(gf, oracle, dim, measure):
     """Radial measure dy y^((d-2)/2); the angular measure is whatever the weights carry.  Parity on
@@ -698,3 +750,138 @@ def test_random_parameter_sets(gf, oracle):
         assert e <= TOL64, (trial, e, lk, lpk, cutoff2, s0, n_rad, n_ang, ang, routing, dim, xs[relerr(g, ref).argmax()])
         worst = max(worst, e)
     print("worst relative error over 300 random parameter sets: %.2e" % worst)
+
+
+# ------------------------------------------------------------------ Taylor subtraction of order n > 0 (eq. (12),(13))
+def _taylor_pair(gf, oracle, lk, lp, cutoff2, n, **kw):
+    return (gf.make_params(lk, lp, cutoff2, taylor_order=n, **kw), oracle.make_params(lk, lp, cutoff2, taylor_order=n, **kw))
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4])
+def test_taylor_order_cfg1_every_point(gf, oracle, n):
+    """(1 - t^n) F: config 1's grid and orders, every point, 1e-11 against the
+    oracle's parity variant.  The kernel's form (remainder of the +-z pair as a rational function of x, Chebyshev U_2i
+    polynomials, moment tables of the measures w t^a) shares nothing with the oracle's (Taylor coefficients of D2,
+    remainder in d)."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    P, Po = _taylor_pair(gf, oracle, cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], n)
+    _, rn, rw, z, wz = gpu_setup(gf, cfg)
+    _, rno, rwo, zo, wzo = oracle_setup(oracle, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, gpu_grid(gf, cfg)).cpu().numpy()
+    ref, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, oracle_grid(oracle, cfg), accum="extended")
+    e = relerr(g, ref)
+    assert e.max() <= TOL64, (n, e.max(), oracle_grid(oracle, cfg).ravel()[e.argmax()])
+
+
+@pytest.mark.parametrize("n", [1, 2])
+def test_taylor_order_cfg2_sampled(gf, oracle, n):
+    """Config 2 (512x512 points, 256x128 nodes) at full size on the GPU, every 4th index in each direction compared."""
+    cfg = W.CONFIGS["cfg2_mid"]
+    P, Po = _taylor_pair(gf, oracle, cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], n)
+    _, rn, rw, z, wz = gpu_setup(gf, cfg)
+    _, rno, rwo, zo, wzo = oracle_setup(oracle, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, gpu_grid(gf, cfg)).cpu().numpy()[::4, ::4]
+    ref, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, oracle_grid(oracle, cfg)[::4, ::4], accum="extended")
+    e = relerr(g, ref)
+    assert e.max() <= TOL64, (n, e.max())
+
+
+@pytest.mark.parametrize("lines", ["rational", "complex_masses", "unequal", "rational_k"])
+def test_taylor_order_other_propagators(gf, oracle, lines):
+    bub = {"kind": "massive", "m2": 1.0}
+    rat = {"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2}
+    lk, lp = {"rational": (bub, rat), "complex_masses": ({"kind": "massive", "m2": 0.5j}, {"kind": "massive", "m2": -0.5j}),
+              "unequal": ({"kind": "massive", "m2": 0.3}, {"kind": "massive", "m2": 2.5}), "rational_k": (rat, bub)}[lines]
+    cfg = W.CONFIGS["cfg1_tiny"]
+    n_rad, n_ang = 96, 48
+    rn, rw = gf.make_radial_tables("real", n_rad, W.RADIAL_RULE)
+    z, wz = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    rno, rwo = oracle.make_quadrature(W.RADIAL_RULE, n_rad)
+    zo, wzo = oracle.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    xs = oracle_grid(oracle, cfg)[::2, ::2].ravel()
+    for n in (1, 2):
+        P, Po = _taylor_pair(gf, oracle, lk, lp, 1e5, n)
+        g = gf.eval_grid(P, rn, rw, n_rad, z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+        ref, _ = oracle.eval_grid(Po, rno, rwo, n_rad, zo, wzo, xs, accum="extended")
+        e = relerr(g, ref)
+        assert e.max() <= TOL64, (lines, n, e.max(), xs[e.argmax()])
+
+
+def test_taylor_order_degenerate_points_rules_and_splits(gf, oracle):
+    """x = 0 (exactly 0), tiny and huge |x|, points on the cut side; odd / tiny rules; every lane split (1 .. 4097
+    points); the host path; d = 3."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    xs = np.array([0, 1e-20 + 1e-20j, 1e-12, -1e-9j, 1e-5 + 1e-5j, 3e-3, 1.0, -0.5, 1j, -1j, -3.9 + 1e-3j,
+                   -0.999 + 0.01j, 250.0 + 1j, 1e6 + 3e5j, -1e6 + 1j, 1e12j, -5 + 2j, -5 - 2j], dtype=np.complex128)
+    for n in (1, 2):
+        P, Po = _taylor_pair(gf, oracle, cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], n)
+        _, rn, rw, z, wz = gpu_setup(gf, cfg)
+        _, rno, rwo, zo, wzo = oracle_setup(oracle, cfg)
+        g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+        ref, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, xs, accum="quad")
+        assert g[0] == 0 and ref[0] == 0
+        e = relerr(g, ref)
+        assert e.max() <= TOL64, (n, e.max(), xs[e.argmax()])
+        # below |x| ~ 1e-30 the oracle cannot form the plain sum (its header); there G_n(x) = c x^(n+1) (1 + O(x)) ties
+        # the values to the one at 1e-20 (1 + i), which the oracle covers; where x^(n+1) underflows the result is 0
+        tiny = np.array([1e-100 + 1e-100j, 1e-140 - 1e-140j, 1e-200 + 1e-200j], dtype=np.complex128)
+        gt = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, torch.from_numpy(tiny).cuda()).cpu().numpy()
+        for xt, v in zip(tiny, gt):
+            expect = g[1] * (xt / xs[1]) ** (n + 1)
+            if abs(expect) > 1e-290:
+                assert abs(v - expect) <= 1e-11 * abs(expect), (n, xt, v, expect)
+            else:
+                assert abs(v) <= 1e-290
+    P, Po = _taylor_pair(gf, oracle, cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], 1)
+    grid = oracle_grid(oracle, cfg).ravel()
+    for ang, n_ang, n_rad in (("gauss_cheb2", 33, 7), ("tanh_sinh", 49, 64), ("gauss_legendre", 1, 3), ("gauss_legendre", 2, 100)):
+        rn, rw = gf.make_radial_tables("real", n_rad, W.RADIAL_RULE)
+        z, wz = gf.make_quadrature(ang, n_ang, measure="sqrt1mz2")
+        rno, rwo = oracle.make_quadrature(W.RADIAL_RULE, n_rad)
+        zo, wzo = oracle.make_quadrature(ang, n_ang, measure="sqrt1mz2")
+        x = grid[::37]
+        g = gf.eval_grid(P, rn, rw, n_rad, z, wz, torch.from_numpy(x).cuda()).cpu().numpy()
+        ref, _ = oracle.eval_grid(Po, rno, rwo, n_rad, zo, wzo, x, accum="extended")
+        assert relerr(g, ref).max() <= (TOL64 if n_rad > 3 else 1e-9), (ang, n_ang, n_rad, relerr(g, ref).max())
+    _, rn, rw, z, wz = gpu_setup(gf, cfg)
+    _, rno, rwo, zo, wzo = oracle_setup(oracle, cfg)
+    ref_all, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, grid, accum="extended")
+    for n_points in (1, 31, 257, 4096):
+        g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, torch.from_numpy(grid[:n_points].copy()).cuda()).cpu().numpy()
+        assert relerr(g, ref_all[:n_points]).max() <= TOL64, n_points
+    # the host entry point runs the same kernels
+    rnh, rwh = gf.make_radial_tables_host("real", cfg["n_rad"], W.RADIAL_RULE)
+    zh, wzh = gf.make_quadrature_host(W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
+    out = np.empty(grid.size, dtype=np.complex128)
+    gf.eval_grid_host(P, rnh, rwh, cfg["n_rad"], zh, wzh, grid, out)
+    assert relerr(out, ref_all).max() <= TOL64
+    # d = 3 (radial measure y^(1/2), plain angular measure)
+    P3, Po3 = _taylor_pair(gf, oracle, cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], 1, dim=3.0, prefactor=1 / (8 * np.pi ** 2))
+    z3, wz3 = gf.make_quadrature_dim(W.ANGULAR_RULE, cfg["n_ang"], 3.0)
+    zo3, wzo3 = oracle.make_quadrature_dim(W.ANGULAR_RULE, cfg["n_ang"], 3.0)
+    g = gf.eval_grid(P3, rn, rw, cfg["n_rad"], z3, wz3, torch.from_numpy(grid[::5].copy()).cuda()).cpu().numpy()
+    ref, _ = oracle.eval_grid(Po3, rno, rwo, cfg["n_rad"], zo3, wzo3, grid[::5], accum="extended")
+    assert relerr(g, ref).max() <= TOL64
+
+
+def test_taylor_order_reaches_the_closed_form_and_refuses_the_rest(gf):
+    """G_1 = CF1 + x/(6 m^2), G_2 = G_1 - x^2/(60 m^4) on the GPU with the Gauss rule of the measure; combinations that
+    are not built are GF_ERR_UNSUPPORTED, not a wrong number."""
+    from tests import closed_forms as CF
+    import mpmath as mp
+    bub = {"kind": "massive", "m2": 1.0}
+    rn, rw = gf.make_radial_tables("real", 256, W.RADIAL_RULE)
+    z, wz = gf.make_quadrature("gauss_cheb2", 128, measure="sqrt1mz2")
+    xs = np.array([0.5 + 0.2j, 1 + 2j, 3.0, -0.5 + 0.3j, 0.05 - 0.02j])
+    for n in (1, 2):
+        g = gf.eval_grid(gf.make_params(bub, bub, 1e6, taylor_order=n), rn, rw, 256, z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+        with mp.workdps(40):
+            ref = [complex(CF.cf1(x) + mp.mpc(x) / 6 - (mp.mpc(x) ** 2 / 60 if n == 2 else 0)) for x in xs]
+        assert relerr(g, ref).max() < 3e-12
+    x = torch.from_numpy(xs).cuda()
+    rnp, rwp = gf.make_radial_tables("auto", 256, W.RADIAL_RULE)
+    for kw, tabs in ((dict(taylor_order=5), (rn, rw)), (dict(taylor_order=-1), (rn, rw)), (dict(taylor_order=1, contour="auto"), (rnp, rwp)),
+                     (dict(taylor_order=1, routing="symmetric"), (rn, rw)), (dict(taylor_order=1, precision=32), (rn, rw))):
+        with pytest.raises(gf.GfError) as e:
+            gf.eval_grid(gf.make_params(bub, bub, 1e6, **kw), tabs[0], tabs[1], 256, z, wz, x)
+        assert e.value.status == 3, kw
