@@ -301,6 +301,13 @@ void prop_taylor(const Propagator& P, std::complex<R> y, int M, std::complex<R>*
   for (int m = 2; m <= M; ++m) t[m] = -(Q1 * t[m - 1] + t[m - 2]) / Q;
 }
 
+// squared distance from y to the nearest pole of the propagator (selects between two equal forms below)
+double pole_distance2(const Propagator& P, std::complex<double> y) {
+  if (P.kind == PROP_MASSIVE) return std::norm(y + std::complex<double>(P.m2_re, P.m2_im));
+  std::complex<double> sq = std::sqrt(std::complex<double>(P.a * P.a - 4.0 * P.b, 0.0));
+  return std::fmin(std::norm(y - 0.5 * (-P.a + sq)), std::norm(y - 0.5 * (-P.a - sq)));
+}
+
 // D2(u) - [Taylor polynomial of D2 of degree 2n in p], u = y + d, d = x + bz, in a combined form (like eq. (20) for
 // n = 0: every term carries its full power of p explicitly, no difference of nearly equal numbers is formed):
 //   D2(y + d) - sum_{m <= M} t_m d^m = -d^(M+1) [Q' t_M + (Q''/2)(t_{M-1} + t_M d)] / Q(u)        (M = 2n >= 2)
@@ -314,6 +321,26 @@ std::complex<R> prop_diff_taylor(const Propagator& P, std::complex<R> y, std::co
   C t[2 * kMaxTaylor + 1];
   prop_taylor<R>(P, y, M, t);
   C d = x + bz, u = y + d;
+  // Where |d| is not small against the distance from y to the nearest pole of D2 (|c| for a massive line) the
+  // polynomial is the larger part of F_sub and the definition itself, D2(u) minus the polynomial, is well
+  // conditioned; the combined form below would cancel by (d/c)^(n+1) there (its pieces are of the orders 2n+1 and
+  // above in d/c, the result of the order 2n).  Both are the same number; each is used where it is accurate (the
+  // test only selects the form, its own accuracy plays no part).
+  if ((R)4 * std::norm(d) > (R)pole_distance2(P, std::complex<double>((double)y.real(), (double)y.imag()))) {
+    C poly = 0;
+    for (int m = 0; m <= M; ++m) {
+      R binom = 1;
+      C xl = 1;
+      for (int l = 0; l <= m && m + l <= M; ++l) {
+        C bp = 1;
+        for (int k = 0; k < m - l; ++k) bp *= bz;
+        poly += t[m] * binom * xl * bp;
+        binom = binom * (R)(m - l) / (R)(l + 1);
+        xl *= x;
+      }
+    }
+    return prop<R>(P, u) - poly;
+  }
   C dM1 = d;
   for (int k = 0; k < M; ++k) dM1 *= d;   // d^(M+1)
   C rem;
@@ -752,7 +779,9 @@ int gfo_make_grid(double re_min, double re_max, int n_re, double im_min, double 
 // is << 1e-11 at every point (reading G18): long double terms and sums, and binary128 (libquadmath)
 // terms and sums where |x| < 2^-10 -- there the +-z terms, each O(sqrt|x y|), cancel to O(|x|), which
 // costs even long double a factor 2 sqrt(y/|x|) (measured against a 60-digit evaluation of the same
-// sum: 7e-9 at |x| = 1e-16); 3 = binary128 everywhere (slow; checks variant 2).
+// sum: 7e-9 at |x| = 1e-16); with a Taylor order n > 0 below |x| = 2^-4 (the angular sum of the order-(2n+2) terms
+// cancels by a further y/mu at large y: 1.7e-12 was measured at |x| = 1.5e-3, mu = 0.013 with long double terms);
+// 3 = binary128 everywhere (slow; checks variant 2).
 // n_threads <= 0: hardware concurrency.
 // Returns 0 on success; fills *threads_used.
 int gfo_eval_grid(const void* params, const double* rad_nodes, const double* rad_weights, int n_rad,
@@ -779,7 +808,7 @@ int gfo_eval_grid(const void* params, const double* rad_nodes, const double* rad
                    ? eval_point<ld, double>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
                : accum == 1
                    ? eval_point<double, double>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
-               : (accum == 2 && std::fmax(std::fabs(xx.real()), std::fabs(xx.imag())) >= 0x1p-10)
+               : (accum == 2 && std::fmax(std::fabs(xx.real()), std::fabs(xx.imag())) >= (P.taylor_order > 0 ? 0x1p-4 : 0x1p-10))
                    ? eval_point<ld, ld>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, n_ang, nodes)
                    : eval_point<__float128, __float128>(P, xx, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights,
                                                         n_ang, nodes);

@@ -1,5 +1,7 @@
 // gf_api.cu -- the C ABI of include/gf.h: argument validation, host-side preparation (pole
 // decomposition of line 2, launch plan) and kernel launches.  No torch types, no exceptions.
+#include <quadmath.h>
+
 #include <algorithm>
 #include <cmath>
 #include <complex>
@@ -89,6 +91,35 @@ int rung_index(double v) {
   return 2 * e;
 }
 
+// The roots u_1 = (-a + sqrt(a^2-4b))/2, u_2 = (-a - sqrt(a^2-4b))/2 of u^2 + a u + b and the residues
+// R_r = (u_r + M2)/(u_r - u_s) of (u + M2)/(u^2 + a u + b), in binary128 (the smaller real root from b/q: no
+// cancellation), returned as poles -mu_r with mu_r split into hi + lo.
+void rational_poles(double M2, double a, double b, PoleTerm* t) {
+  const __float128 A = a, B = b, disc = A * A - 4 * B;
+  __float128 ur[2], ui[2] = {0, 0};
+  if (disc >= 0) {
+    const __float128 sq = sqrtq(disc);
+    if (A >= 0) { ur[1] = -(A + sq) / 2; ur[0] = ur[1] != 0 ? B / ur[1] : (__float128)0; }
+    else { ur[0] = (sq - A) / 2; ur[1] = B / ur[0]; }
+  } else {
+    ur[0] = ur[1] = -A / 2;
+    ui[0] = sqrtq(-disc) / 2;
+    ui[1] = -ui[0];
+  }
+  for (int r = 0; r < 2; ++r) {
+    const int s = 1 - r;
+    // R_r = (u_r + M2)/(u_r - u_s)
+    const __float128 nr = ur[r] + (__float128)M2, ni = ui[r], dr = ur[r] - ur[s], di = ui[r] - ui[s];
+    const __float128 dn = dr * dr + di * di;
+    t[r].R_re = (double)((nr * dr + ni * di) / dn);
+    t[r].R_im = (double)((ni * dr - nr * di) / dn);
+    t[r].mu_re = (double)(-ur[r]);
+    t[r].mu_re_lo = (double)(-ur[r] - (__float128)t[r].mu_re);
+    t[r].mu_im = (double)(-ui[r]);
+    t[r].mu_im_lo = (double)(-ui[r] - (__float128)t[r].mu_im);
+  }
+}
+
 // validate everything that does not need a pointer, and build the kernel arguments
 int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, EvalArgs* a) {
   if (!p) { set_error("eval_grid: params is null"); return GF_ERR_NULL; }
@@ -137,7 +168,7 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   const gf_propagator& q = p->line_pk;
   if (q.kind == GF_PROP_MASSIVE) {
     a->n_terms = 1;
-    a->term[0] = PoleTerm{1.0, 0.0, q.m2_re, q.m2_im};
+    a->term[0] = PoleTerm{1.0, 0.0, q.m2_re, q.m2_im, 0.0, 0.0};
     a->line2_scale = std::hypot(q.m2_re, q.m2_im);
   } else {
     const double disc = q.a * q.a - 4.0 * q.b;
@@ -145,18 +176,14 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
       set_error("line_pk: rational propagator with a double pole (a^2 = 4b) is unsupported");
       return GF_ERR_UNSUPPORTED;
     }
-    typedef std::complex<double> C;
-    const C sq = std::sqrt(C(disc, 0.0));
-    const C u1 = 0.5 * (-q.a + sq), u2 = 0.5 * (-q.a - sq);
-    const C R1 = (u1 + q.M2) / (u1 - u2), R2 = (u2 + q.M2) / (u2 - u1);
     a->n_terms = 2;
-    a->term[0] = PoleTerm{R1.real(), R1.imag(), -u1.real(), -u1.imag()};
-    a->term[1] = PoleTerm{R2.real(), R2.imag(), -u2.real(), -u2.imag()};
+    rational_poles(q.M2, q.a, q.b, a->term);
     // size of the singular structure of line 2 in the y-plane, the largest pole modulus: sqrt(b) for a
     // complex-conjugate pair (|u_r|^2 = b), else max |(-a +- sqrt(disc))/2|
     a->line2_scale = disc < 0 ? std::sqrt(q.b)
                               : std::fmax(std::fabs(-q.a + std::sqrt(disc)), std::fabs(-q.a - std::sqrt(disc))) / 2.0;
   }
+  if (p->line_k.kind == GF_PROP_RATIONAL) rational_poles(p->line_k.M2, p->line_k.a, p->line_k.b, a->kroot);
   a->thread_ok = p->line_k.kind == GF_PROP_MASSIVE && q.kind == GF_PROP_MASSIVE && p->line_k.m2_im == 0 &&
                  q.m2_im == 0 && p->line_k.m2_re == q.m2_re && q.m2_re > 0;
   a->same_mass = p->line_k.kind == GF_PROP_MASSIVE && q.kind == GF_PROP_MASSIVE && p->line_k.m2_re == q.m2_re &&

@@ -219,12 +219,16 @@ __device__ __forceinline__ void arc_node(double R, double tau, double t, double 
   *wy = {__dmul_rn(f, y->im), -__dmul_rn(f, y->re)};   // -i f y
 }
 
-// D1(y) for complex y
-__device__ __forceinline__ cd line_k_complex(const gf_propagator& p, cd y) {
+// y + mu with mu = hi + lo: accurate to an ulp of itself next to the pole y = -mu
+__device__ __forceinline__ cd y_plus_mu(cd y, const PoleTerm& t) {
+  return {(y.re + t.mu_re) + t.mu_re_lo, (y.im + t.mu_im) + t.mu_im_lo};
+}
+// D1(y) for complex y; a rational line through its factored denominator (y + nu_1)(y + nu_2), which stays accurate
+// where the contour passes next to a root
+__device__ __forceinline__ cd line_k_complex(const EvalArgs& a, cd y) {
+  const gf_propagator& p = a.line_k;
   if (p.kind == GF_PROP_MASSIVE) return cinv_fast(cd{y.re + p.m2_re, y.im + p.m2_im});
-  const cd ya = {y.re + p.a, y.im};
-  cd den = cmul(y, ya);
-  den.re += p.b;
+  const cd den = cmul(y_plus_mu(y, a.kroot[0]), y_plus_mu(y, a.kroot[1]));
   return cmul(cd{y.re + p.M2, y.im}, cinv_fast(den));
 }
 
@@ -336,10 +340,15 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
   // as on the REAL contour (four DFMA instead of three complex products); zdir: the direction the constants are for.
   cd Z1 = {0.0, 0.0}, C2 = {0.0, 0.0}, Z3 = {0.0, 0.0}, Dc = {0.0, 0.0}, C1x4 = {0.0, 0.0};
   int zdir = -1;   // -1 not set, 0 dir = 1, 1 dir = geo.d
+  // The three terms are of the size |C2| = |x + mu|/|2x| each, and on the ray (y along x) they can cancel to a zeta
+  // next to [0,1]: the form is used only where |C2| <= 8, which keeps its absolute error below 1e-15 (for |x| << |mu|
+  // the product form below, accurate to an ulp of zeta itself, is taken instead).
+  bool affine_ok = false;
   if (NT == 1) {
     const cd xm0 = {x.re + a.term[0].mu_re, x.im + a.term[0].mu_im};
     C2 = cmul(xm0, cscale(xinv, 0.5));
     C1x4 = cscale(cmul(xm0, C2), 2.0);
+    affine_ok = fma(C2.re, C2.re, C2.im * C2.im) <= 64.0;
   }
   // tables of the real nodes this point walks: the REAL contour's (policy REAL) or its rung's tail piece
   const double* row = blob + L.off_rung + (long long)geo.row * L.rung_stride;
@@ -411,7 +420,7 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
       q4 = cscale(cinv_fast(y), 0.25);
       base = cscale(cmul(wy, y), a.c0);
     }
-    const bool affine = NT == 1 && (table || at.type == SEG_RAY);
+    const bool affine = NT == 1 && affine_ok && (table || at.type == SEG_RAY);
     cd xq = {0.0, 0.0};
     if (affine) {
       const int want = at.type == SEG_RAY;
@@ -427,8 +436,8 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
     }
     cd ic0 = {0.0, 0.0};
     if (!table) {
-      if (a.same_mass) ic0 = cinv_fast(cd{y.re + a.term[0].mu_re, y.im + a.term[0].mu_im});
-      base = cmul(base, a.same_mass ? ic0 : line_k_complex(a.line_k, y));
+      if (a.same_mass) ic0 = cinv_fast(y_plus_mu(y, a.term[0]));
+      base = cmul(base, a.same_mass ? ic0 : line_k_complex(a, y));
     }
 #pragma unroll
     for (int r = 0; r < NT; ++r) {
@@ -444,13 +453,13 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
         delta = cmul(xm, q4);                        // eta - 1/4
         zeta = cmul(csqr(A), xq);
       }
-      const cd s = node_term<double, COUNT>(tb, x, y, delta, zeta, mur, mui, rc);
+      const cd s = node_term<double, COUNT>(tb, x, y, delta, zeta, mur, mui, rc, a.term[r].mu_re_lo, a.term[r].mu_im_lo);
       cd pr;
       if (table) {
         const double2 p2 = tpref[r * tstride + at.i];
         pr = {p2.x, p2.y};
       } else {
-        const cd ic = a.same_mass ? ic0 : cinv_fast(cd{y.re + mur, y.im + mui});
+        const cd ic = a.same_mass ? ic0 : cinv_fast(y_plus_mu(y, a.term[r]));
         // a massive line 2 is its one pole with residue 1
         pr = NT == 1 ? cd{-base.re, -base.im} : cmul(base, cd{-a.term[r].R_re, -a.term[r].R_im});
         pr = cmul(pr, ic);

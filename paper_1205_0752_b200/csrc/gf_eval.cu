@@ -241,7 +241,8 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
     for (int r = 0; r < NT; ++r) {
       const cd delta = {fma(dA[r].re, q4, d0), dA[r].im * q4};   // eta - 1/4
       const cd zeta = {fma(C1x4[r].re, q4, fma(C3.re, y, C2[r].re)), fma(C1x4[r].im, q4, fma(C3.im, y, C2[r].im))};
-      const cd s = node_term<T, COUNT>(tb, xz, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc);
+      const cd s = node_term<T, COUNT>(tb, xz, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc,
+                                       a.term[r].mu_re_lo, a.term[r].mu_im_lo);
       double2 pr = ppref[r * L.n_rad_pad];
       if (!on) pr = make_double2(0.0, 0.0);
       g_re = fma(pr.x, s.re, fma(-pr.y, s.im, g_re));

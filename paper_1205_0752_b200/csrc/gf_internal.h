@@ -12,6 +12,9 @@ namespace gf {
 struct PoleTerm {
   double R_re, R_im;
   double mu_re, mu_im;
+  double mu_re_lo, mu_im_lo;   // mu = (mu_re + mu_re_lo) + i (mu_im + mu_im_lo): the roots of a rational line are made
+                               // in binary128 on the host; where a deformed contour passes next to the pole of D2(y)
+                               // at y = -mu, y + mu must be accurate to an ulp of ITSELF (reading G18)
 };
 
 constexpr int kMaxTerms = 2;
@@ -45,6 +48,8 @@ struct EvalArgs {
   int n_terms;
   PoleTerm term[kMaxTerms];
   gf_propagator line_k;
+  PoleTerm kroot[2];   // rational line 1: y^2 + a y + b = (y + nu_1)(y + nu_2), nu in mu_re.. (deformed contours
+                       // evaluate the denominator in this form: accurate next to a root)
   double cutoff2, s0, c0;
   double ypow;         // radial measure dy y^ypow: (d - 2)/2, 1 in d = 4
   double Llog_hi, Llog_lo;  // ln((Lambda^2 + s0)/s0) as a double-double (host, binary128)

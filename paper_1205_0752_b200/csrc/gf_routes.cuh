@@ -335,8 +335,9 @@ __device__ __forceinline__ void goertzel_range_f32x2(uint32_t tab, int k_hi, int
 struct ZetaDD {
   double re_hi, re_lo, im, im2;   // Re zeta = hi + lo, Im zeta, (Im zeta)^2
 };
-__device__ __noinline__ ZetaDD zeta_dd(double xr, double xi, double yr, double yi, double mur, double mui) {
-  const dd Ar = dd_add_d(two_sum(xr, mur), yr), Ai = dd_add_d(two_sum(xi, mui), yi);
+__device__ __noinline__ ZetaDD zeta_dd(double xr, double xi, double yr, double yi, double mur, double mui,
+                                       double mur_lo = 0.0, double mui_lo = 0.0) {
+  const dd Ar = dd_add_d(dd_add_d(two_sum(xr, mur), yr), mur_lo), Ai = dd_add_d(dd_add_d(two_sum(xi, mui), yi), mui_lo);
   const dd A2r = dd_add(dd_mul(Ar, Ar), dd_neg(dd_mul(Ai, Ai)));
   const dd A2i = dd_scale2(dd_mul(Ar, Ai), 2.0);
   // den = 4 x y;  zeta = A^2 conj(den) / |den|^2
@@ -491,7 +492,8 @@ __device__ __forceinline__ cd series_finish(const SeriesArg& o, cd delta, double
 // The direct loop for a lane on the NEAR or EXACT route
 template <typename T, bool COUNT>
 __device__ __forceinline__ cd direct_route(const Tabs<T>& tb, int route, bool warp_has_exact, cd x, cd y, cd delta,
-                                           cd zeta, double mur, double mui, RouteCount& rc) {
+                                           cd zeta, double mur, double mui, RouteCount& rc, double mur_lo = 0.0,
+                                           double mui_lo = 0.0) {
   cd s;
   const cd eta = {__dadd_rn(0.25, delta.re), delta.im};
   bool dd_loop = true;
@@ -502,7 +504,7 @@ __device__ __forceinline__ cd direct_route(const Tabs<T>& tb, int route, bool wa
     dd_loop = false;
   } else if (sizeof(T) == 8 || route == ROUTE_EXACT) {
     ZetaDD z = {zeta.re, 0.0, zeta.im, zeta.im * zeta.im};
-    if (route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y.re, y.im, mur, mui);
+    if (route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y.re, y.im, mur, mui, mur_lo, mui_lo);
     s = angular_direct(eta, z, tb.mu0, tb.st, tb.stlo, tb.sw, tb.n_pairs);
   } else {
     s = angular_near<T>(eta, zeta, tb.mu0, tb.stT, tb.swT, tb.n_pairs);
@@ -517,7 +519,7 @@ __device__ __forceinline__ cd direct_route(const Tabs<T>& tb, int route, bool wa
 
 template <typename T, bool COUNT>
 __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta, cd zeta, double mur, double mui,
-                                        RouteCount& rc) {
+                                        RouteCount& rc, double mur_lo = 0.0, double mui_lo = 0.0) {
   const SeriesArg o = route_setup<T>(tb, zeta);
   // every lane's K and K1 are multiples of 4 and at most kmc (route_setup): so are the warp's
   const int Kw = __reduce_max_sync(0xffffffffu, o.K);
@@ -535,7 +537,8 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
     if (COUNT) { rc.series_exec += sizeof(T) == 8 ? K1w : Kw; rc.series_exec32 += sizeof(T) == 8 ? Kw - K1w : 0; }
     if (o.route <= ROUTE_CHEB) s = series_finish<COUNT>(o, delta, p1, p2, n1, n2, rc);
   }
-  if (o.route >= ROUTE_NEAR) s = direct_route<T, COUNT>(tb, o.route, warp_has_exact, x, y, delta, zeta, mur, mui, rc);
+  if (o.route >= ROUTE_NEAR)
+    s = direct_route<T, COUNT>(tb, o.route, warp_has_exact, x, y, delta, zeta, mur, mui, rc, mur_lo, mui_lo);
   return s;
 }
 

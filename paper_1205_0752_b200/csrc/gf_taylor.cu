@@ -230,7 +230,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
         s = cmul(o.g, acc);
       } else {
         ZetaDD z = {zeta.re, 0.0, zeta.im, zeta.im * zeta.im};
-        if (o.route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y, 0.0, a.term[r].mu_re, a.term[r].mu_im);
+        if (o.route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y, 0.0, a.term[r].mu_re, a.term[r].mu_im, a.term[r].mu_re_lo, a.term[r].mu_im_lo);
         double u0 = 0.0, ua = 0.0, v0 = 0.0, va = 0.0;
         int j = 0;
 #pragma unroll 1

@@ -751,7 +751,7 @@ def test_taylor_order_matches_the_definition(oracle, n, lines):
     P = oracle.make_params(lk, lp, 1e4, taylor_order=n)
     rn, rw = oracle.make_quadrature("gauss_legendre", 12)
     z, wz = oracle.make_quadrature("gauss_cheb2", 9, measure="sqrt1mz2")
-    for x in (0.5 + 0.2j, -2.0 + 1.5j, 3e-3 - 1e-3j, 40.0 + 9j):
+    for x in (0.5 + 0.2j, -2.0 + 1.5j, 3e-3 - 1e-3j, 40.0 + 9j, -2.8e4 + 9.4e3j):   # the last: |x| >> y, m^2
         ref = MPR.finite_sum(oracle, P, x, rn, rw, 12, z, wz, digits=60)
         g, _ = oracle.eval_grid(P, rn, rw, 12, z, wz, np.array([x]), accum="quad")
         assert relerr(g, [ref])[0] < 1e-15, (x, g, ref)
