@@ -135,7 +135,7 @@ def oracle_step(cfg, xs):
     P = O.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
                       contour=contour)
     rn, rw = O.make_radial_pyramid(cfg["n_rad"], levels=1 if contour == "real" else 4, kind=W.RADIAL_RULE)
-    z, wz = O.make_quadrature(W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
+    z, wz = O.make_quadrature(cfg.get("ang", W.ANGULAR_RULE), cfg["n_ang"], measure="sqrt1mz2")
     g, used = O.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, xs, accum="double")
     return time.perf_counter() - t, used, g
 
@@ -200,13 +200,14 @@ def run_reference(args):
 
 def workload_config(cfg, world, rows_per_rank):
     def line(p):
-        return ("1/(q^2+%g)" % p["m2"]) if p["kind"] == "massive" else "(q^2+%g)/(q^4+%g q^2+%g)" % (p["M2"], p["a"], p["b"])
+        m2 = complex(p.get("m2", 0.0))
+        return ("1/(q^2+%s)" % (("%g" % m2.real) if m2.imag == 0 else "(%g%+gi)" % (m2.real, m2.imag))) if p["kind"] == "massive" else "(q^2+%g)/(q^4+%g q^2+%g)" % (p["M2"], p["a"], p["b"])
     return {"workload": "%s: lines %s and %s, once-subtracted at p^2=0, %dx%d grid over Re[%g,%g] Im[%g,%g]%s, "
-                        "%d radial x %d angular Gauss-Legendre nodes, cutoff %g, %s contour, complex128"
+                        "%d radial Gauss-Legendre x %d angular %s nodes, cutoff %g, %s contour, complex128"
                         % (cfg["name"], line(cfg["line_k"]), line(cfg["line_pk"]), cfg["n_re"], rows_per_rank * world,
                            cfg["re"][0], cfg["re"][1], cfg["im"][0], cfg["im"][1],
                            " (log-spaced |Im|)" if cfg["spacing"] != "uniform" else "", cfg["n_rad"], cfg["n_ang"],
-                           cfg["cutoff2"], cfg.get("contour", "real").upper()),
+                           cfg.get("ang", W.ANGULAR_RULE), cfg["cutoff2"], cfg.get("contour", "real").upper()),
             "n_points": cfg["n_re"] * rows_per_rank * world, "n_rad": cfg["n_rad"], "n_ang": cfg["n_ang"],
             "contour": cfg.get("contour", "real"),
             "parallelism": "rows x%d, no collective" % world,
@@ -236,6 +237,7 @@ def run_ours(args):
     assert rows_local == n_rows
     n_points_local = n_re * rows_local
     contour = args.contour
+    ang_rule = cfg.get("ang", W.ANGULAR_RULE)
     P = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
                        contour=contour, precision=64)
     info = gf.launch_info(P, n_rad, n_ang, n_points_local)
@@ -249,7 +251,7 @@ def run_ours(args):
 
     def step(k=None):
         rn, rw = gf.make_radial_tables(contour, n_rad, W.RADIAL_RULE)                   # a2
-        z, wz = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")           # a2
+        z, wz = gf.make_quadrature(ang_rule, n_ang, measure="sqrt1mz2")           # a2
         gf.make_grid_rows(cfg["re"][0], cfg["re"][1], n_re, cfg["im"][0], cfg["im"][1], cfg["n_im_global"],
                           row_first, rows_local, spacing=cfg["spacing"], im_abs_min=cfg["im_abs_min"], out=x)  # a1
         ws = gf.eval_prepare(P, rn, rw, n_rad, z, wz)                                    # a3: x-independent set-up
@@ -291,7 +293,7 @@ def run_ours(args):
     # ---- executed FP64 work of one launch: the kernel's own route counters (an untimed, counted launch
     #      with identical results) x the per-unit instruction counts of the SASS (gf_eval_launch_info)
     rn_c, rw_c = gf.make_radial_tables(contour, n_rad, W.RADIAL_RULE)
-    z_c, wz_c = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    z_c, wz_c = gf.make_quadrature(ang_rule, n_ang, measure="sqrt1mz2")
     out_c, counters = gf.eval_grid_counted(P, rn_c, rw_c, n_rad, z_c, wz_c, x)
     assert torch.equal(out_c.view(torch.float64), out.view(torch.float64)), "counted launch differs"
     fp64_inst, fp64_flops = gf.executed_fp64(info, counters)
@@ -322,7 +324,7 @@ def run_ours(args):
     xh = x.cpu().pin_memory()
     outh = torch.empty(xh.shape, dtype=torch.complex128).pin_memory()
     rn_h, rw_h = gf.make_radial_tables_host(contour, n_rad, W.RADIAL_RULE)
-    z_h, wz_h = gf.make_quadrature_host(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    z_h, wz_h = gf.make_quadrature_host(ang_rule, n_ang, measure="sqrt1mz2")
 
     def e2e_step():
         gf.eval_grid_host(P, rn_h, rw_h, n_rad, z_h, wz_h, xh, outh)   # synchronises before returning

@@ -46,6 +46,13 @@ CONFIGS = {
         line_k=_BUBBLE, line_pk=_BUBBLE, cutoff2=1e6,
         n_re=4096, n_im=256, re=(-10.0, -3.0), im=(-1e-3, 1e-3), spacing="log_abs_im",
         im_abs_min=1e-6, n_rad=1024, n_ang=512),
+    # not a BASELINE.json config: a scan of the size the paper itself ran (its worked example, masses^2 +-i/2,
+    # eq. (19); 128 x 128 points, ngl = 64 radial Gauss-Legendre and ndbl = 49 tanh-sinh nodes: PAPER.md:150,158,276),
+    # kept to show what preparation and launch overheads cost on small grids (bench.py --workload paper_scan_128)
+    "paper_scan_128": dict(
+        line_k={"kind": "massive", "m2": 0.5j}, line_pk={"kind": "massive", "m2": -0.5j}, cutoff2=1e6,
+        n_re=128, n_im=128, re=(-2.0, 2.0), im=(-2.0, 2.0), spacing="uniform", im_abs_min=0.0,
+        n_rad=64, n_ang=49, ang="tanh_sinh"),
 }
 
 PREFACTOR = 2.0 / np.pi   # c0 of eq. (21): 16 pi^2 / (2 pi)^3

@@ -36,6 +36,13 @@
  *     launch failure).  gf_last_error() describes the last failure of the
  *     calling thread.  A denominator that vanishes at a quadrature node yields IEEE inf/NaN in
  *     that output entry, not an error (the paper has no convention).
+ *   - Bad input that only a kernel can see (tables in DEVICE memory: an angular rule that is not symmetric, radial
+ *     nodes that are not ascending strictly inside (-1,1); a workspace that was prepared for other parameters): the
+ *     kernel fills every output of that call with NaN and leaves a code in a mapped host word of the device; the
+ *     NEXT call of gf_eval_grid / _counted / _host, gf_eval_prepare, gf_eval_grid_prepared or gf_eval_angular on
+ *     that device (after the kernel has run) does nothing, returns GF_ERR_ARG and names the cause, once.
+ *     gf_eval_grid_host checks its (host) tables before it launches anything and reports what its own kernels found
+ *     before it returns.
  */
 #ifndef GF_B200_H_
 #define GF_B200_H_
@@ -180,11 +187,12 @@ long long gf_radial_table_size(int contour, int n_rad);
 
 /* Step 5 / Kernel 2: G at every point of d_x.
  *   d_rad_nodes/d_rad_weights  radial rule(s), measure PLAIN, gf_radial_table_size() doubles each;
- *                              nodes strictly inside (-1,1)
+ *                              nodes ascending, strictly inside (-1,1) (every level of the pyramid; the tail series
+ *                              and its binary search rely on the order)
  *   d_ang_nodes/d_ang_weights  angular rule of n_ang nodes whose weights include the measure
  *                              sqrt(1-z^2) (GF_MEASURE_SQRT1MZ2).  The rule must be symmetric
  *                              (z[n-1-j] = -z[j], equal weights): the kernel folds +-z pairs.  A rule
- *                              that is not makes every output NaN.
+ *                              that is not makes every output NaN (and see "Bad input" above).
  *   d_x      n_points complex<double>
  *   d_out    n_points complex<double> (precision 64) or complex<float> (precision 32; REAL contour only)
  * Domain: x = 0 gives exactly 0; |x| up to 1e100.  Asynchronous on `stream`; n_points = 0 is a no-op. */
@@ -197,7 +205,8 @@ int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_
  * depend on x (folded angular rule, series coefficients, radial nodes and prefactors, tail tables) into the
  * caller's DEVICE workspace of gf_eval_workspace_size() bytes (256-byte aligned; -1 on a bad argument; it does not
  * depend on the number of points).  gf_eval_grid_prepared evaluates d_x from such a workspace; params, n_rad and
- * n_ang must be the ones it was prepared with (not checked).  d_counters may be NULL (else as in
+ * n_ang must be the ones it was prepared with: the workspace header carries a hash of them, and the kernels read
+ * nothing else from a workspace whose hash differs (outputs NaN, "Bad input" above).  d_counters may be NULL (else as in
  * gf_eval_grid_counted).  gf_eval_grid == workspace from cudaMallocAsync + these two + cudaFreeAsync. */
 long long gf_eval_workspace_size(const gf_params* p, int n_rad, int n_ang);
 int gf_eval_prepare(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,

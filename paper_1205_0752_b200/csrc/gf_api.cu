@@ -7,6 +7,7 @@
 #include <complex>
 #include <cstdarg>
 #include <cstdio>
+#include <exception>
 #include <mutex>
 #include <vector>
 
@@ -62,7 +63,77 @@ int scratch_alloc(void** ptr, size_t bytes, cudaStream_t stream) {
   return check_cuda(cudaMallocFromPoolAsync(ptr, bytes, pool, stream), "cudaMallocFromPoolAsync(scratch)");
 }
 
+// One mapped host word per device that kernels report bad input to (an asymmetric angular rule, radial tables that are
+// not ascending inside (-1,1), a workspace prepared for other parameters): zero-copy, so reading it needs no
+// synchronisation.  Allocated on first use, kept for the life of the process (4 bytes of pinned host memory).
+static int* g_status[64] = {};
+
+static int status_word(int** word) {
+  int dev = 0;
+  int rc = check_cuda(cudaGetDevice(&dev), "cudaGetDevice");
+  if (rc) return rc;
+  if (dev < 0 || dev >= 64) { set_error("device ordinal %d out of range", dev); return GF_ERR_CUDA; }
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  if (!g_status[dev]) {
+    int* h = nullptr;
+    if ((rc = check_cuda(cudaHostAlloc(reinterpret_cast<void**>(&h), sizeof(int), cudaHostAllocMapped), "cudaHostAlloc(status word)"))) return rc;
+    *h = 0;
+    g_status[dev] = h;
+  }
+  *word = g_status[dev];
+  return GF_OK;
+}
+
+int attach_status(EvalArgs* a) {
+  int* h = nullptr;
+  int rc = status_word(&h);
+  if (rc) return rc;
+  int* d = nullptr;
+  if ((rc = check_cuda(cudaHostGetDevicePointer(reinterpret_cast<void**>(&d), h, 0), "cudaHostGetDevicePointer(status word)"))) return rc;
+  a->status = d;
+  return GF_OK;
+}
+
+int take_status(const char* where) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return GF_OK; }
+  int* h;
+  {
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    h = g_status[dev];
+  }
+  if (!h) return GF_OK;
+  const int code = __atomic_exchange_n(h, 0, __ATOMIC_ACQ_REL);
+  if (!code) return GF_OK;
+  set_error("%s: a kernel of this device was given bad input:%s%s%s", where,
+            (code & kStatusAsymmetricRule) ? " an angular rule that is not symmetric (z[n-1-j] = -z[j], equal weights);" : "",
+            (code & kStatusRadialNodes) ? " radial nodes that are not ascending strictly inside (-1,1);" : "",
+            (code & kStatusWorkspace) ? " a workspace prepared with other parameters, orders or precision;" : "");
+  return GF_ERR_ARG;
+}
+
 namespace {
+
+// FNV-1a over the parameter block and the orders -> a double in [1, 2) (EvalArgs::ws_tag)
+double workspace_tag(const gf_params* p, int n_rad, int n_ang) {
+  unsigned long long h = 1469598103934665603ULL;
+  auto mix = [&](const void* ptr, size_t n) {
+    const unsigned char* b = static_cast<const unsigned char*>(ptr);
+    for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ULL; }
+  };
+  // field by field: the struct's padding bytes are not the caller's to define
+  const gf_propagator* pr[2] = {&p->line_k, &p->line_pk};
+  for (int k = 0; k < 2; ++k) {
+    mix(&pr[k]->kind, sizeof(int)); mix(&pr[k]->m2_re, sizeof(double)); mix(&pr[k]->m2_im, sizeof(double));
+    mix(&pr[k]->M2, sizeof(double)); mix(&pr[k]->a, sizeof(double)); mix(&pr[k]->b, sizeof(double));
+  }
+  mix(&p->cutoff2, sizeof(double)); mix(&p->sub_re, sizeof(double)); mix(&p->sub_im, sizeof(double));
+  mix(&p->taylor_order, sizeof(int)); mix(&p->prefactor, sizeof(double)); mix(&p->map_scale, sizeof(double));
+  mix(&p->contour, sizeof(int)); mix(&p->precision, sizeof(int)); mix(&p->routing, sizeof(int)); mix(&p->dim, sizeof(double));
+  const int extra[3] = {n_rad, n_ang, kLayoutVersion};
+  mix(extra, sizeof(extra));
+  return 1.0 + (double)(h >> 12) * 0x1p-52;
+}
 
 // per (point, node, pole) FP64-pipe instructions of each route's set-up + finish (SASS of eval_real_kernel<double>)
 constexpr double kNodeNearDfma = 12, kNodeNearOther = 13, kNodeMomentDfma = 21, kNodeMomentOther = 13,
@@ -163,6 +234,7 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   a->contour = p->contour;
   a->routing = p->routing;
   a->taylor_order = p->taylor_order;
+  a->ws_tag = workspace_tag(p, n_rad, n_ang);
 
   // line 2 as a sum of simple poles R_r/(u + mu_r)
   const gf_propagator& q = p->line_pk;
@@ -223,6 +295,19 @@ long long radial_table_size(int contour, int n_rad) {
 
 using namespace gf;
 
+// gf_tables.cpp allocates (std::vector) and may start threads: nothing may propagate across the C ABI
+template <typename F>
+static int no_throw(const char* what, F&& f) {
+  try {
+    return f();
+  } catch (const std::exception& e) {
+    set_error("%s: %s", what, e.what());
+  } catch (...) {
+    set_error("%s: unknown C++ exception", what);
+  }
+  return GF_ERR_ARG;
+}
+
 extern "C" {
 
 const char* gf_last_error(void) { return g_err; }
@@ -281,34 +366,38 @@ int gf_make_grid_rows(double re_min, double re_max, int n_re, double im_min, dou
 }
 
 int gf_make_quadrature_host(int kind, int n, double step, int measure, double* h_nodes, double* h_weights) {
-  return make_rule_host(kind, n, step, measure, h_nodes, h_weights);
+  return no_throw("make_quadrature_host", [&] { return make_rule_host(kind, n, step, measure, h_nodes, h_weights); });
 }
 
 int gf_make_quadrature(int kind, int n, double step, int measure, double* d_nodes, double* d_weights, void* stream) {
   if (!d_nodes || !d_weights) { set_error("make_quadrature: null device pointer"); return GF_ERR_NULL; }
   if (n < 1 || n > (1 << 20)) { set_error("make_quadrature: n=%d out of range", n); return GF_ERR_ARG; }
-  std::vector<double> x(n), w(n);
-  int rc = make_rule_host(kind, n, step, measure, x.data(), w.data());
-  if (rc) return rc;
-  cudaStream_t s = static_cast<cudaStream_t>(stream);
-  // pageable source: the runtime stages the data before returning, so x, w may go out of scope
-  if ((rc = check_cuda(cudaMemcpyAsync(d_nodes, x.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy nodes"))) return rc;
-  return check_cuda(cudaMemcpyAsync(d_weights, w.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy weights");
+  return no_throw("make_quadrature", [&] {
+    std::vector<double> x(n), w(n);
+    int rc = make_rule_host(kind, n, step, measure, x.data(), w.data());
+    if (rc) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    // pageable source: the runtime stages the data before returning, so x, w may go out of scope
+    if ((rc = check_cuda(cudaMemcpyAsync(d_nodes, x.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy nodes"))) return rc;
+    return check_cuda(cudaMemcpyAsync(d_weights, w.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy weights");
+  });
 }
 
 int gf_make_quadrature_dim_host(int kind, int n, double step, double dim, double* h_nodes, double* h_weights) {
-  return make_rule_dim_host(kind, n, step, dim, h_nodes, h_weights);
+  return no_throw("make_quadrature_dim_host", [&] { return make_rule_dim_host(kind, n, step, dim, h_nodes, h_weights); });
 }
 
 int gf_make_quadrature_dim(int kind, int n, double step, double dim, double* d_nodes, double* d_weights, void* stream) {
   if (!d_nodes || !d_weights) { set_error("make_quadrature_dim: null device pointer"); return GF_ERR_NULL; }
   if (n < 1 || n > (1 << 20)) { set_error("make_quadrature_dim: n=%d out of range", n); return GF_ERR_ARG; }
-  std::vector<double> x(n), w(n);
-  int rc = make_rule_dim_host(kind, n, step, dim, x.data(), w.data());
-  if (rc) return rc;
-  cudaStream_t s = static_cast<cudaStream_t>(stream);
-  if ((rc = check_cuda(cudaMemcpyAsync(d_nodes, x.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy nodes"))) return rc;
-  return check_cuda(cudaMemcpyAsync(d_weights, w.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy weights");
+  return no_throw("make_quadrature_dim", [&] {
+    std::vector<double> x(n), w(n);
+    int rc = make_rule_dim_host(kind, n, step, dim, x.data(), w.data());
+    if (rc) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if ((rc = check_cuda(cudaMemcpyAsync(d_nodes, x.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy nodes"))) return rc;
+    return check_cuda(cudaMemcpyAsync(d_weights, w.data(), sizeof(double) * n, cudaMemcpyHostToDevice, s), "copy weights");
+  });
 }
 
 long long gf_radial_table_size(int contour, int n_rad) { return radial_table_size(contour, n_rad); }
@@ -321,6 +410,7 @@ static int eval_grid_impl(const gf_params* p, const double* d_rad_nodes, const d
   if (rc) return rc;
   if (!d_rad_nodes || !d_rad_weights || !d_ang_nodes || !d_ang_weights) { set_error("eval_grid: null table pointer"); return GF_ERR_NULL; }
   if (n_points > 0 && (!d_x || !d_out)) { set_error("eval_grid: null grid/output pointer"); return GF_ERR_NULL; }
+  if ((rc = take_status("eval_grid")) || (rc = attach_status(&a))) return rc;
   a.rad_nodes = d_rad_nodes;
   a.rad_weights = d_rad_weights;
   a.ang_nodes = d_ang_nodes;
@@ -361,6 +451,7 @@ int gf_eval_prepare(const gf_params* p, const double* d_rad_nodes, const double*
   if (rc) return rc;
   if (!d_rad_nodes || !d_rad_weights || !d_ang_nodes || !d_ang_weights) { set_error("eval_prepare: null table pointer"); return GF_ERR_NULL; }
   if (!d_workspace) { set_error("eval_prepare: d_workspace is null"); return GF_ERR_NULL; }
+  if ((rc = take_status("eval_prepare")) || (rc = attach_status(&a))) return rc;
   a.rad_nodes = d_rad_nodes;
   a.rad_weights = d_rad_weights;
   a.ang_nodes = d_ang_nodes;
@@ -375,6 +466,7 @@ int gf_eval_grid_prepared(const gf_params* p, int n_rad, int n_ang, const void* 
   if (rc) return rc;
   if (!d_workspace) { set_error("eval_grid_prepared: d_workspace is null"); return GF_ERR_NULL; }
   if (n_points > 0 && (!d_x || !d_out)) { set_error("eval_grid_prepared: null grid/output pointer"); return GF_ERR_NULL; }
+  if ((rc = take_status("eval_grid_prepared")) || (rc = attach_status(&a))) return rc;
   a.x = static_cast<const double2*>(d_x);
   a.out = d_out;
   return launch_prepared(a, p->precision, static_cast<const double*>(d_workspace), d_counters,
@@ -389,7 +481,28 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
   if (rc) return rc;
   if (!h_rad_nodes || !h_rad_weights || !h_ang_nodes || !h_ang_weights) { set_error("eval_grid_host: null table pointer"); return GF_ERR_NULL; }
   if (n_points > 0 && (!h_x || !h_out)) { set_error("eval_grid_host: null grid/output pointer"); return GF_ERR_NULL; }
+  // the tables are in host memory here: what the kernels can only answer with NaN (gf_eval_grid) is an error code
+  for (int j = 0; j < (n_ang + 1) / 2; ++j) {
+    const int jm = n_ang - 1 - j;
+    const double zp = h_ang_nodes[jm], zm = h_ang_nodes[j], wp = h_ang_weights[jm], wm = h_ang_weights[j];
+    const double tol = 16.0 * 2.220446049250313e-16;
+    const bool ok = jm == j ? std::fabs(zp) <= 1e-15
+                            : (std::fabs(zp + zm) <= tol * std::fabs(zp) && std::fabs(wp - wm) <= tol * std::fabs(wp));
+    if (!ok) { set_error("eval_grid_host: the angular rule is not symmetric at node %d (z[n-1-j] = -z[j], equal weights)", j); return GF_ERR_ARG; }
+  }
+  {
+    int off = 0, n = n_rad;
+    for (int l = 0; l < (p->contour == GF_CONTOUR_REAL ? 1 : 4); ++l, off += n, n >>= 1)
+      for (int i = 0; i < n; ++i) {
+        const double t = h_rad_nodes[off + i];
+        if (!(t > -1.0 && t < 1.0) || (i > 0 && !(t > h_rad_nodes[off + i - 1]))) {
+          set_error("eval_grid_host: radial nodes must be ascending strictly inside (-1,1) (level %d, node %d)", l, i);
+          return GF_ERR_ARG;
+        }
+      }
+  }
   if (n_points == 0) return GF_OK;
+  if ((rc = take_status("eval_grid_host")) || (rc = attach_status(&a))) return rc;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const size_t n_radtab = (size_t)radial_table_size(p->contour, n_rad);
   const size_t out_elem = p->precision == 32 ? 8 : 16;
@@ -472,12 +585,19 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
     ok(cudaMemcpyAsync(static_cast<char*>(h_out) + (size_t)p0 * out_elem, d + off_out + (size_t)p0 * out_elem,
                        (size_t)np * out_elem, cudaMemcpyDeviceToHost, sout), "device->host copy");
   }
-  if (n_chunks > 1 && ev_done && s_out) {
+  if (rc) {
+    // a call failed part-way: work already enqueued on the side streams has no event edge to s, so drain them before
+    // the scratch goes back to the pool
+    if (s_in) cudaStreamSynchronize(s_in);
+    if (s_k2) cudaStreamSynchronize(s_k2);
+    if (s_out) cudaStreamSynchronize(s_out);
+  } else if (n_chunks > 1 && ev_done && s_out) {
     cudaEventRecord(ev_done, s_out);
     cudaStreamWaitEvent(s, ev_done, 0);   // the scratch is freed in stream order of s after the last copy out
   }
   cudaFreeAsync(d, s);
   int rc2 = check_cuda(cudaStreamSynchronize(s), "stream synchronize");
+  if (!rc && !rc2) rc2 = take_status("eval_grid_host");   // the call has synchronised: report what its kernels found
   if (s_in) { cudaStreamSynchronize(s_in); cudaStreamDestroy(s_in); }
   if (s_out) { cudaStreamSynchronize(s_out); cudaStreamDestroy(s_out); }
   if (s_k2) { cudaStreamSynchronize(s_k2); cudaStreamDestroy(s_k2); }
@@ -499,6 +619,7 @@ int gf_eval_angular(const gf_params* p, double x_re, double x_im, const double* 
   if (p->routing != 0) { set_error("eval_angular: defined for the paper's routing (eq. (22)) only"); return GF_ERR_UNSUPPORTED; }
   if (!d_ang_nodes || !d_ang_weights) { set_error("eval_angular: null table pointer"); return GF_ERR_NULL; }
   if (n_y > 0 && (!d_y || !d_out)) { set_error("eval_angular: null y/output pointer"); return GF_ERR_NULL; }
+  if ((rc = take_status("eval_angular")) || (rc = attach_status(&a))) return rc;
   a.ang_nodes = d_ang_nodes;
   a.ang_weights = d_ang_weights;
   a.x = static_cast<const double2*>(d_y);
@@ -581,6 +702,7 @@ int gf_diag_contour_nodes(const gf_params* p, int n_rad, int n_ang, const void* 
   if (rc) return rc;
   if (p->contour == GF_CONTOUR_REAL) { set_error("diag_contour_nodes: a deformed contour policy (or AUTO) is needed"); return GF_ERR_ARG; }
   if (!d_workspace || !d_rad_nodes || !d_rad_weights || !d_policy || !d_y || !d_wy) { set_error("diag_contour_nodes: null pointer"); return GF_ERR_NULL; }
+  if ((rc = attach_status(&a))) return rc;
   if (!std::isfinite(x_re) || !std::isfinite(x_im)) { set_error("diag_contour_nodes: x is not finite"); return GF_ERR_ARG; }
   LaunchPlan plan;
   if ((rc = plan_eval(a, p->precision, &plan))) return rc;

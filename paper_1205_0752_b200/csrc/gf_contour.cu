@@ -299,6 +299,12 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
   extern __shared__ __align__(128) unsigned char smem_raw[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
   double* sb = reinterpret_cast<double*>(smem_raw + 16);
+  if (!workspace_matches(a, blob)) {   // prepared for other parameters or orders: refuse it before reading a table
+    const long long pt = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> a.split_log2;
+    if (pt < a.n_points) reinterpret_cast<double2*>(a.out)[pt] = make_double2(nan(""), nan(""));
+    if (blockIdx.x == 0 && threadIdx.x == 0) report_status(a.status, kStatusWorkspace);
+    return;
+  }
   if (threadIdx.x == 0) mbar_init(bar, 1);
   __syncthreads();
   if (threadIdx.x == 0) bulk_load(sb, blob, (uint32_t)(L.n_doubles * sizeof(double)), bar);

@@ -34,8 +34,9 @@ __global__ void __launch_bounds__(256) prep_angular_only_kernel(const __grid_con
   __syncthreads();
   prep_series_kreq(L, blob, s_lc, blob + L.off_cheb, 2);
   if (threadIdx.x == 0) {
-    blob[0] = bad ? 1.0 : 0.0;
-    blob[1] = 0.0;
+    blob[0] = (double)bad;
+    blob[1] = a.ws_tag;
+    if (bad) report_status(a.status, bad);
   }
 }
 

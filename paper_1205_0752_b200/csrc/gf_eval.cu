@@ -75,6 +75,7 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
   if (threadIdx.x == 0) bad = 0;
   __syncthreads();
   prep_angular(a, L, blob, &bad);
+  check_radial_tables(a, &bad);
   __syncthreads();  // t, w written by this CTA are visible to it
   prep_series_T(a, L, blob);
   if (L.off_gam >= 0) prep_tail_moments(a, L, blob, s_part);
@@ -126,8 +127,9 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
     prep_tail_sums(J);
   }
   if (threadIdx.x == 0) {
-    blob[0] = bad ? 1.0 : 0.0;
-    blob[1] = 0.0;
+    blob[0] = (double)bad;
+    blob[1] = a.ws_tag;
+    if (bad) report_status(a.status, bad);
   }
 }
 
@@ -144,6 +146,15 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
   extern __shared__ __align__(128) unsigned char smem_raw[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
   double* sb = reinterpret_cast<double*>(smem_raw + 16);
+  if (!workspace_matches(a, blob)) {   // prepared for other parameters or orders: refuse it before reading a table
+    const long long pt = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> a.split_log2;
+    if (pt < a.n_points) {
+      if (sizeof(T) == 8) reinterpret_cast<double2*>(a.out)[pt] = make_double2(nan(""), nan(""));
+      else reinterpret_cast<float2*>(a.out)[pt] = make_float2(nanf(""), nanf(""));
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) report_status(a.status, kStatusWorkspace);
+    return;
+  }
   if (threadIdx.x == 0) mbar_init(bar, 1);
   __syncthreads();
   if (threadIdx.x == 0) bulk_load(sb, blob, (uint32_t)(L.n_doubles * sizeof(double)), bar);

@@ -63,7 +63,13 @@ struct EvalArgs {
   int rung_lo;         // ladder index of the first tabulated contour radius (deformed contours)
   int split_log2;      // lanes per grid point = 1 << split_log2
   int taylor_order;    // n of the Taylor subtraction t^n (eq. (13)); n > 0 runs gf_taylor.cu
+  int* status;         // mapped host word the kernels report bad input to (gf.h "Errors"); may be null
+  double ws_tag;       // hash of (params, orders, layout version) as a double in [1, 2): the preparation kernel writes
+                       // it into the workspace header, the evaluation kernels refuse a workspace that carries another
 };
+// codes a kernel leaves in *status (the next API call of the device returns GF_ERR_ARG and describes it)
+enum { kStatusAsymmetricRule = 1, kStatusRadialNodes = 2, kStatusWorkspace = 4 };
+constexpr int kLayoutVersion = 7;   // bump when a BlobLayout or the meaning of a table changes
 
 // Offsets (in doubles) of the prepared tables, as the preparation kernel writes them and every CTA of the
 // evaluation kernel copies them to shared memory (one 16-byte header first).
@@ -117,6 +123,8 @@ struct LaunchPlan {
 void set_error(const char* fmt, ...);
 int check_cuda(cudaError_t e, const char* what);
 int scratch_alloc(void** ptr, size_t bytes, cudaStream_t stream);  // from the library's own stream-ordered pool
+int attach_status(EvalArgs* a);   // a->status = the current device's status word (allocated on first use)
+int take_status(const char* where);   // GF_ERR_ARG (and the word cleared) if a kernel of the current device reported bad input
 
 // gf_tables.cpp
 int make_rule_host(int kind, int n, double step, int measure, double* nodes, double* weights);

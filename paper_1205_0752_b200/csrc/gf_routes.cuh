@@ -126,6 +126,31 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
   }
 }
 
+// bad input found by a kernel: leave a code in the mapped host word (gf_internal.h), read by the next API call
+__device__ __forceinline__ void report_status(int* status, int code) {
+  if (status) {
+    atomicOr_system(status, code);
+    __threadfence_system();
+  }
+}
+// the header of a prepared workspace: [0] != 0: bad tables (every output NaN), [1] = EvalArgs::ws_tag
+__device__ __forceinline__ bool workspace_matches(const EvalArgs& a, const double* __restrict__ blob) {
+  return __ldg(blob + 1) == a.ws_tag;
+}
+// radial tables (every level of the pyramid a deformed contour uses): strictly inside (-1,1) and ascending
+__device__ void check_radial_tables(const EvalArgs& a, int* bad) {
+  const int levels = a.contour == GF_CONTOUR_REAL ? 1 : 4;
+  int off = 0, n = a.n_rad;
+  for (int l = 0; l < levels; ++l) {
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      const double t = a.rad_nodes[off + i];
+      if (!(t > -1.0 && t < 1.0) || (i > 0 && !(t > a.rad_nodes[off + i - 1]))) atomicOr(bad, kStatusRadialNodes);
+    }
+    off += n;
+    n >>= 1;
+  }
+}
+
 template <typename T>
 struct Vec2;
 template <>
@@ -568,7 +593,7 @@ __device__ void prep_angular(const EvalArgs& a, const BlobLayout& L, double* blo
       const double tol = 16.0 * DBL_EPSILON;
       const bool ok = (jm == j) ? (fabs(zp) <= 1e-15)
                                 : (fabs(zp + zm) <= tol * fabs(zp) && fabs(wp - wm) <= tol * fabs(wp));
-      if (!ok) atomicExch(bad, 1);
+      if (!ok) atomicOr(bad, kStatusAsymmetricRule);
       const dd tt = two_prod(zp, zp);
       t = tt.hi;
       tlo = tt.lo;

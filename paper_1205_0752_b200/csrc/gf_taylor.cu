@@ -54,6 +54,7 @@ __global__ void __launch_bounds__(256) prep_taylor_kernel(const __grid_constant_
   if (threadIdx.x == 0) bad = 0;
   __syncthreads();
   prep_angular(a, L, blob, &bad);
+  check_radial_tables(a, &bad);
   __syncthreads();
   prep_series_T(a, L, blob);
   {
@@ -111,8 +112,9 @@ __global__ void __launch_bounds__(256) prep_taylor_kernel(const __grid_constant_
   __syncthreads();
   prep_series_kreq(L, blob, s_lc, blob + L.off_chebA, NA);
   if (threadIdx.x == 0) {
-    blob[0] = bad ? 1.0 : 0.0;
-    blob[1] = 0.0;
+    blob[0] = (double)bad;
+    blob[1] = a.ws_tag;
+    if (bad) report_status(a.status, bad);
   }
 }
 
@@ -127,6 +129,12 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   extern __shared__ __align__(128) unsigned char smem_raw[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
   double* sb = reinterpret_cast<double*>(smem_raw + 16);
+  if (!workspace_matches(a, blob)) {   // prepared for other parameters or orders: refuse it before reading a table
+    const long long pt = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> a.split_log2;
+    if (pt < a.n_points) reinterpret_cast<double2*>(a.out)[pt] = make_double2(nan(""), nan(""));
+    if (blockIdx.x == 0 && threadIdx.x == 0) report_status(a.status, kStatusWorkspace);
+    return;
+  }
   if (threadIdx.x == 0) mbar_init(bar, 1);
   __syncthreads();
   if (threadIdx.x == 0) bulk_load(sb, blob, (uint32_t)(L.n_doubles * sizeof(double)), bar);

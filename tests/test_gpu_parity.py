@@ -362,13 +362,82 @@ def test_other_propagators(gf, oracle, lines):
     assert e.max() <= TOL64, e.max()
 
 
-def test_asymmetric_rule_is_rejected_with_nan(gf):
+def test_bad_tables_are_reported(gf):
+    """Tables live in device memory, so gf_eval_grid can only find out inside its kernels: every output becomes NaN
+    and the NEXT call on the device returns GF_ERR_ARG naming the cause (include/gf.h "Errors"); the call after that
+    is clean again.  gf_eval_grid_host sees the tables on the host and refuses them at once."""
     cfg = W.CONFIGS["cfg1_tiny"]
+    x = gpu_grid(gf, cfg)
+    for contour in ("real", "auto"):
+        P, rn, rw, z, wz = gpu_setup(gf, cfg, contour=contour)
+        z2 = z.clone()
+        z2[3] += 1e-3                        # angular rule no longer symmetric
+        rn2 = rn.clone()
+        rn2[5], rn2[6] = rn[6].item(), rn[5].item()   # radial nodes no longer ascending
+        for tabs, word in (((rn, rw, z2, wz), "symmetric"), ((rn2, rw, z, wz), "ascending")):
+            g = gf.eval_grid(P, tabs[0], tabs[1], cfg["n_rad"], tabs[2], tabs[3], x)
+            torch.cuda.synchronize()
+            assert torch.isnan(g.real).all(), (contour, word)
+            with pytest.raises(gf.GfError) as e:
+                gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+            assert e.value.status == 2 and word in str(e.value), str(e.value)
+            g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)   # reported once, then clean
+            torch.cuda.synchronize()
+            assert torch.isfinite(g.real).all()
+    # the Taylor-order kernel has the same checks
+    P1 = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], taylor_order=1)
     P, rn, rw, z, wz = gpu_setup(gf, cfg)
     z2 = z.clone()
     z2[3] += 1e-3
-    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z2, wz, gpu_grid(gf, cfg))
+    g = gf.eval_grid(P1, rn, rw, cfg["n_rad"], z2, wz, x)
+    torch.cuda.synchronize()
     assert torch.isnan(g.real).all()
+    with pytest.raises(gf.GfError):
+        gf.eval_grid(P1, rn, rw, cfg["n_rad"], z, wz, x)
+    # host entry point: an error code, nothing launched
+    rnh, rwh = gf.make_radial_tables_host("real", cfg["n_rad"], W.RADIAL_RULE)
+    zh, wzh = gf.make_quadrature_host(W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
+    xh, out = x.cpu().numpy(), np.empty(x.numel(), dtype=np.complex128)
+    zb = zh.copy()
+    zb[3] += 1e-3
+    rb = rnh.copy()
+    rb[[5, 6]] = rb[[6, 5]]
+    for tabs in ((rnh, rwh, zb, wzh), (rb, rwh, zh, wzh)):
+        with pytest.raises(gf.GfError) as e:
+            gf.eval_grid_host(P, tabs[0], tabs[1], cfg["n_rad"], tabs[2], tabs[3], xh, out)
+        assert e.value.status == 2
+    gf.eval_grid_host(P, rnh, rwh, cfg["n_rad"], zh, wzh, xh, out)
+    assert np.isfinite(out).all()
+
+
+def test_a_workspace_of_other_parameters_is_refused(gf):
+    """gf_eval_grid_prepared with a workspace prepared for another mass, other orders, another precision or another
+    contour: the workspace header carries a hash of what it was made for, the kernels read no table from a workspace
+    that is not theirs (outputs NaN) and the next call returns GF_ERR_ARG."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    x = gpu_grid(gf, cfg)
+    P, rn, rw, z, wz = gpu_setup(gf, cfg)
+    ws = gf.eval_prepare(P, rn, rw, cfg["n_rad"], z, wz)
+    good = gf.eval_grid_prepared(P, cfg["n_rad"], cfg["n_ang"], ws, x)
+    torch.cuda.synchronize()
+    assert torch.isfinite(good.real).all()
+    other_mass = gf.make_params({"kind": "massive", "m2": 1.5}, cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE)
+    p32 = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE, precision=32)
+    t1 = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE, taylor_order=1)
+    auto = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE, contour="auto")
+    big = torch.zeros(max(ws.numel(), 1 << 24), dtype=torch.uint8, device="cuda")   # the callee may expect a larger one
+    big[:ws.numel()] = ws
+    for Pbad, n_rad, n_ang in ((other_mass, cfg["n_rad"], cfg["n_ang"]), (P, cfg["n_rad"] // 2, cfg["n_ang"]),
+                               (P, cfg["n_rad"], cfg["n_ang"] - 2), (p32, cfg["n_rad"], cfg["n_ang"]),
+                               (t1, cfg["n_rad"], cfg["n_ang"]), (auto, cfg["n_rad"], cfg["n_ang"])):
+        g = gf.eval_grid_prepared(Pbad, n_rad, n_ang, big, x)
+        torch.cuda.synchronize()
+        assert torch.isnan(g.real).all()
+        with pytest.raises(gf.GfError) as e:
+            gf.eval_grid_prepared(P, cfg["n_rad"], cfg["n_ang"], ws, x)
+        assert e.value.status == 2 and "workspace" in str(e.value)
+    again = gf.eval_grid_prepared(P, cfg["n_rad"], cfg["n_ang"], ws, x)
+    assert torch.equal(torch.view_as_real(again), torch.view_as_real(good))
 
 
 # ------------------------------------------------------------------ a3: contours that depend on the point
