@@ -246,14 +246,16 @@ int gf_eval_angular(const gf_params* p, double x_re, double x_im, const double* 
 int gf_cut_crossings(const gf_params* p, const void* d_x, long long n_points, int n_z, int* d_out, void* stream);
 
 /* The same evaluation, also counting the work by route for the roofline accounting.
- * d_counters: 10 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
+ * d_counters: 12 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
  *   [0] pairs of the plain direct loop  [1] series terms EXECUTED in FP64 (every lane of a warp runs its warp's
  *   longest series; the FP64 kernel runs the high-order terms of a series, whose sum is below 2^-24 of the budget,
  *   in FP32: those are counter [9])  [2] pairs of the double-double direct loop (EXACT lanes, and the NEAR lanes of their warps)
  *   [3] [4] [5] [6] (point, radial node, pole) triples taken by the NEAR / MOMENT / EXACT / CHEB
  *   route (the triples of the large-y tail are not among them)  [7] series terms NEEDED (the sum over series
  *   triples of their own K)  [8] tail series evaluated, one per (point, pole)  [9] series terms executed in
- *   FP32 by the FP64 kernel.  Results are identical to gf_eval_grid. */
+ *   FP32 by the FP64 kernel  [10] far blocks of the angular rule summed by their own series on the NEAR / EXACT
+ *   routes (rules of 64 and more folded pairs are split into blocks of 32; counters [0] and [2] then count only the
+ *   pairs of the blocks next to zeta)  [11] terms of those block series.  Results are identical to gf_eval_grid. */
 int gf_eval_grid_counted(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
                          const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
                          long long n_points, void* d_out, unsigned long long* d_counters, void* stream);
@@ -280,6 +282,8 @@ typedef struct {
   double node_cheb_dfma, node_cheb_other;
   double node_exact_dfma, node_exact_other;
   double tail_dfma, tail_other;                                   /* per tail series (point, pole) */
+  double blk_series_dfma, blk_series_other;                       /* per far block: set-up + finish of its series */
+  double blk_term_dfma, blk_term_other;                           /* per term of a block series */
 } gf_launch_info;
 int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_points, gf_launch_info* out);
 

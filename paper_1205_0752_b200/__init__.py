@@ -48,11 +48,12 @@ class gf_launch_info(ctypes.Structure):
             "near_pair_dfma", "near_pair_other", "near_pair_fp32", "series_term_dfma", "series_term_other",
             "series_term_fp32", "exact_pair_dfma", "exact_pair_other", "node_near_dfma", "node_near_other",
             "node_moment_dfma", "node_moment_other", "node_cheb_dfma", "node_cheb_other", "node_exact_dfma",
-            "node_exact_other", "tail_dfma", "tail_other")]
+            "node_exact_other", "tail_dfma", "tail_other", "blk_series_dfma", "blk_series_other", "blk_term_dfma",
+            "blk_term_other")]
 
 
 COUNTER_NAMES = ("near_pairs", "series_terms", "exact_pairs", "near_nodes", "moment_nodes", "exact_nodes",
-                 "cheb_nodes", "series_terms_needed", "tails", "series_terms_fp32")
+                 "cheb_nodes", "series_terms_needed", "tails", "series_terms_fp32", "block_series", "block_series_terms")
 
 
 _lib = None
@@ -341,7 +342,8 @@ def executed_fp64(info, counters):
     """(FP64-pipe thread-instructions, flops with FMA = 2) of one launch from its route counters."""
     units = (("near_pair", "near_pairs"), ("series_term", "series_terms"), ("exact_pair", "exact_pairs"),
              ("node_near", "near_nodes"), ("node_moment", "moment_nodes"), ("node_exact", "exact_nodes"),
-             ("node_cheb", "cheb_nodes"), ("tail", "tails"))
+             ("node_cheb", "cheb_nodes"), ("tail", "tails"), ("blk_series", "block_series"),
+             ("blk_term", "block_series_terms"))
     inst = sum((info[u + "_dfma"] + info[u + "_other"]) * counters[c] for u, c in units)
     flops = sum((2 * info[u + "_dfma"] + info[u + "_other"]) * counters[c] for u, c in units)
     return float(inst), float(flops)

@@ -658,6 +658,7 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
         out->series_term_fp32 = out->exact_pair_dfma = out->exact_pair_other = out->node_near_dfma = out->node_near_other =
             out->node_moment_dfma = out->node_moment_other = out->node_cheb_dfma = out->node_cheb_other =
                 out->node_exact_dfma = out->node_exact_other = out->tail_dfma = out->tail_other = 0.0;
+    out->blk_series_dfma = out->blk_series_other = out->blk_term_dfma = out->blk_term_other = 0.0;
     return GF_OK;
   }
   // FP64-pipe instructions per unit of each route, counted per SASS region in the ncu source page of
@@ -677,6 +678,10 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
   out->node_cheb_dfma = kNodeChebDfma; out->node_cheb_other = kNodeChebOther;
   out->node_exact_dfma = kNodeNearDfma + 29; out->node_exact_other = kNodeNearOther + 217;
   out->tail_dfma = kTailN * (kTailN + 1) + 8.0 * kTailN + 45; out->tail_other = 9.0 * kTailN + 34;
+  // a far block of a split rule (angular_blocked): w', its complex square root, s, the finish: 27 DFMA + 24 DMUL/DADD;
+  // 2 DFMA per term of its series
+  out->blk_series_dfma = 27; out->blk_series_other = 24;
+  out->blk_term_dfma = 2; out->blk_term_other = 0;
   return GF_OK;
 }
 

@@ -292,7 +292,7 @@ __global__ void __launch_bounds__(256) prep_rungs_kernel(const __grid_constant__
 #ifndef GF_CONTOUR_MIN_BLOCKS
 #define GF_CONTOUR_MIN_BLOCKS 4
 #endif
-template <bool COUNT, int NT>
+template <bool COUNT, int NT, bool BLK>
 __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
     eval_contour_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                         const double* __restrict__ blob, unsigned long long* __restrict__ counters) {
@@ -459,7 +459,7 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
         delta = cmul(xm, q4);                        // eta - 1/4
         zeta = cmul(csqr(A), xq);
       }
-      const cd s = node_term<double, COUNT>(tb, x, y, delta, zeta, mur, mui, rc, a.term[r].mu_re_lo, a.term[r].mu_im_lo);
+      const cd s = node_term<double, COUNT, BLK>(tb, x, y, delta, zeta, mur, mui, rc, a.term[r].mu_re_lo, a.term[r].mu_im_lo);
       cd pr;
       if (table) {
         const double2 p2 = tpref[r * tstride + at.i];
@@ -545,10 +545,10 @@ __global__ void contour_nodes_kernel(const __grid_constant__ EvalArgs a, const _
   out_wy[g] = make_double2(wy.re, wy.im);
 }
 
-template <bool COUNT, int NT>
+template <bool COUNT, int NT, bool BLK>
 int launch_contour_t(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
                      cudaStream_t stream) {
-  auto kern = eval_contour_kernel<COUNT, NT>;
+  auto kern = eval_contour_kernel<COUNT, NT, BLK>;
   if (plan.smem_bytes > 48 * 1024) {
     int rc = check_cuda(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes),
                         "cudaFuncSetAttribute(max dynamic shared memory)");
@@ -562,11 +562,17 @@ int launch_contour_t(const EvalArgs& a, const LaunchPlan& plan, const double* bl
 
 int launch_contour(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* d_counters,
                    cudaStream_t stream) {
-  if (a.n_terms == 1)
-    return d_counters ? launch_contour_t<true, 1>(a, plan, blob, d_counters, stream)
-                      : launch_contour_t<false, 1>(a, plan, blob, nullptr, stream);
-  return d_counters ? launch_contour_t<true, 2>(a, plan, blob, d_counters, stream)
-                    : launch_contour_t<false, 2>(a, plan, blob, nullptr, stream);
+  const bool blk = plan.layout.n_blk > 0;
+  if (a.n_terms == 1) {
+    if (d_counters) return blk ? launch_contour_t<true, 1, true>(a, plan, blob, d_counters, stream)
+                               : launch_contour_t<true, 1, false>(a, plan, blob, d_counters, stream);
+    return blk ? launch_contour_t<false, 1, true>(a, plan, blob, nullptr, stream)
+               : launch_contour_t<false, 1, false>(a, plan, blob, nullptr, stream);
+  }
+  if (d_counters) return blk ? launch_contour_t<true, 2, true>(a, plan, blob, d_counters, stream)
+                             : launch_contour_t<true, 2, false>(a, plan, blob, d_counters, stream);
+  return blk ? launch_contour_t<false, 2, true>(a, plan, blob, nullptr, stream)
+             : launch_contour_t<false, 2, false>(a, plan, blob, nullptr, stream);
 }
 
 int launch_prepare_rungs(const EvalArgs& a, const LaunchPlan& plan, double* blob, cudaStream_t stream) {

@@ -77,6 +77,7 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
   prep_angular(a, L, blob, &bad);
   check_radial_tables(a, &bad);
   __syncthreads();  // t, w written by this CTA are visible to it
+  prep_blocks(a, L, blob);
   prep_series_T(a, L, blob);
   if (L.off_gam >= 0) prep_tail_moments(a, L, blob, s_part);
   {
@@ -139,7 +140,7 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
 #ifndef GF_MIN_BLOCKS
 #define GF_MIN_BLOCKS 4
 #endif
-template <typename T, bool COUNT, int NT>
+template <typename T, bool COUNT, int NT, bool BLK>
 __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
     eval_real_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                      const double* __restrict__ blob, unsigned long long* __restrict__ counters) {
@@ -252,8 +253,8 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
     for (int r = 0; r < NT; ++r) {
       const cd delta = {fma(dA[r].re, q4, d0), dA[r].im * q4};   // eta - 1/4
       const cd zeta = {fma(C1x4[r].re, q4, fma(C3.re, y, C2[r].re)), fma(C1x4[r].im, q4, fma(C3.im, y, C2[r].im))};
-      const cd s = node_term<T, COUNT>(tb, xz, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc,
-                                       a.term[r].mu_re_lo, a.term[r].mu_im_lo);
+      // (the lo parts of a rational line's poles matter where a contour passes next to y = -mu: not on the real axis)
+      const cd s = node_term<T, COUNT, BLK>(tb, xz, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc);
       double2 pr = ppref[r * L.n_rad_pad];
       if (!on) pr = make_double2(0.0, 0.0);
       g_re = fma(pr.x, s.re, fma(-pr.y, s.im, g_re));
@@ -327,6 +328,9 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
   L.off_rw = pyramid ? (int)take(L.n_tab) : -1;
   L.off_gam = tail ? (int)take(kTailN * (kTailN + 1) / 2) : -1;
   L.off_gam2 = tail && sym ? (int)take(kTailN * (kTailN + 1) / 2) : -1;
+  L.n_blk = n_pairs >= kBlkMinPairs ? (n_pairs + kBlkPairs - 1) / kBlkPairs : 0;
+  L.off_blk = L.n_blk ? (int)take(2 * L.n_blk) : -1;
+  L.off_blkM = L.n_blk ? (int)take((long long)L.n_blk * kBlkTerms) : -1;
   L.n_doubles = (int)o;
   if (pyramid) take_nodes();
   L.off_tail = tail ? (int)take(2LL * L.n_pref * (n_rad + 1) * kTailN) : -1;
@@ -384,10 +388,10 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   return GF_OK;
 }
 
-template <typename T, bool COUNT, int NT>
+template <typename T, bool COUNT, int NT, bool BLK>
 static int launch_real_nt(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
                           cudaStream_t stream) {
-  auto kern = eval_real_kernel<T, COUNT, NT>;
+  auto kern = eval_real_kernel<T, COUNT, NT, BLK>;
   if (plan.smem_bytes > 48 * 1024) {
     int rc = check_cuda(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes),
                         "cudaFuncSetAttribute(max dynamic shared memory)");
@@ -399,8 +403,12 @@ static int launch_real_nt(const EvalArgs& a, const LaunchPlan& plan, const doubl
 template <typename T, bool COUNT>
 static int launch_real(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
                        cudaStream_t stream) {
-  return a.n_terms == 1 ? launch_real_nt<T, COUNT, 1>(a, plan, blob, counters, stream)
-                        : launch_real_nt<T, COUNT, 2>(a, plan, blob, counters, stream);
+  const bool blk = sizeof(T) == 8 && plan.layout.n_blk > 0;
+  if (a.n_terms == 1)
+    return blk ? launch_real_nt<T, COUNT, 1, true>(a, plan, blob, counters, stream)
+               : launch_real_nt<T, COUNT, 1, false>(a, plan, blob, counters, stream);
+  return blk ? launch_real_nt<T, COUNT, 2, true>(a, plan, blob, counters, stream)
+             : launch_real_nt<T, COUNT, 2, false>(a, plan, blob, counters, stream);
 }
 
 int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d_nodes, int n, double* d_y,

@@ -69,7 +69,7 @@ struct EvalArgs {
 };
 // codes a kernel leaves in *status (the next API call of the device returns GF_ERR_ARG and describes it)
 enum { kStatusAsymmetricRule = 1, kStatusRadialNodes = 2, kStatusWorkspace = 4 };
-constexpr int kLayoutVersion = 7;   // bump when a BlobLayout or the meaning of a table changes
+constexpr int kLayoutVersion = 8;   // bump when a BlobLayout or the meaning of a table changes
 
 // Offsets (in doubles) of the prepared tables, as the preparation kernel writes them and every CTA of the
 // evaluation kernel copies them to shared memory (one 16-byte header first).
@@ -107,6 +107,9 @@ struct BlobLayout {
   long long n_total;            // doubles to allocate
   // Taylor order n > 0 (gf_taylor.cu): n_poly = n + 2 series tables per family, [k][n_poly], and 1/(y_i + mu_r)
   int n_poly, off_momA, off_chebA, off_ic;
+  // blocks of the folded rule for the direct routes (gf_routes.cuh, angular_blocked), staged: n_blk x (c, 1/h) and
+  // n_blk x kBlkTerms Chebyshev moments; n_blk = 0: the rule is not split
+  int n_blk, off_blk, off_blkM;
 };
 constexpr int kRungs = 64;      // tabulated contour radii above the first (deformed contours); then Lambda^2/2
 

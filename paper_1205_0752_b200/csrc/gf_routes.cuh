@@ -20,6 +20,11 @@ constexpr int kMomTerms = 32;         // genuine coefficients of the centred-mom
 #define GF_SERIES_BITS 50
 #endif
 constexpr float kSeriesBits = GF_SERIES_BITS;    // series are cut where the dropped terms are below 2^-50 of the leading one
+// extra bits of error the FP32 phase of a series may cost over the truncation budget 2^-kSeriesBits (0: none)
+#ifndef GF_FP32_SLACK_BITS
+#define GF_FP32_SLACK_BITS 0
+#endif
+constexpr float kFp32Slack = GF_FP32_SLACK_BITS;
 #ifndef GF_GOERTZEL_UNROLL
 #define GF_GOERTZEL_UNROLL 2
 #endif
@@ -36,6 +41,19 @@ constexpr double kTau64 = 0x1p-8;     // EXACT route inside this distance of [0,
 constexpr double kTau32 = 0x1p-4;     // the FP32 variant's NEAR loop is only good further away
 // Kreq table: bins of log2(rho) from kEllLo in steps of kEllStep (the lower edge of a bin decides, so K is safe)
 constexpr float kEllLo = 0.235f, kEllStep = 0.02f;
+
+// Blocks of the folded rule for the direct routes (angular_blocked): kBlkPairs consecutive pairs each; a block that is
+// far from zeta (ellipse parameter of ITS interval rho_b^2 >= kBlkRho2Min) is summed by its own Chebyshev series of at
+// most kBlkTerms terms instead of pair by pair.  K_b = 112/log2(rho_b^2) + 1: dropped terms below 2^-56 rho-scaled.
+#ifndef GF_BLK_TERMS
+#define GF_BLK_TERMS 32
+#endif
+constexpr int kBlkPairs = 32, kBlkTerms = GF_BLK_TERMS;
+#ifndef GF_BLK_MIN_PAIRS
+#define GF_BLK_MIN_PAIRS 192   // measured: 128 pairs (4 blocks) break even, 256 pairs gain 9 to 17 %
+#endif
+constexpr int kBlkMinPairs = GF_BLK_MIN_PAIRS;   // rules with fewer folded pairs are not split
+constexpr float kBlkRho2Min = GF_BLK_TERMS == 32 ? 12.3f : GF_BLK_TERMS == 48 ? 5.3f : 3.5f;   // 2^(112/(kBlkTerms - 1))
 
 enum { ROUTE_MOMENT = 0, ROUTE_CHEB = 1, ROUTE_NEAR = 2, ROUTE_EXACT = 3 };
 
@@ -171,6 +189,9 @@ struct Tabs {
   double mu0;                                     // sum of the folded weights
   double tau;                                     // EXACT inside this distance of [0,1]
   int n_pairs, kmc;
+  int n_blk;                                      // blocks of the folded rule (0: not split)
+  const double2* blk;                             // per block: centre c_b and 1/h_b of its interval [c - h, c + h]
+  const double* blkM;                             // per block: M_k = sum'_{j in b} w_j T_k((t_j - c)/h), kBlkTerms each
 };
 template <typename T>
 __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout& L, int n_pairs) {
@@ -198,15 +219,18 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
   tb.tau = sizeof(T) == 8 ? kTau64 : kTau32;
   tb.n_pairs = n_pairs;
   tb.kmc = L.kmc;
+  tb.n_blk = L.n_blk;
+  tb.blk = reinterpret_cast<const double2*>(sb + (L.n_blk ? L.off_blk : 0));
+  tb.blkM = sb + (L.n_blk ? L.off_blkM : 0);
   return tb;
 }
 
 // Work counters of one thread (COUNT launches only)
 struct RouteCount {
   unsigned long long near_pairs = 0, series_exec = 0, exact_pairs = 0, n_near = 0, n_moment = 0, n_exact = 0,
-                     n_cheb = 0, series_used = 0, tails = 0, series_exec32 = 0;
+                     n_cheb = 0, series_used = 0, tails = 0, series_exec32 = 0, blk_series = 0, blk_terms = 0;
 };
-constexpr int kNumCounters = 10;
+constexpr int kNumCounters = 12;
 
 // ---- NEAR: one folded angular pair: q = w/|zeta - t|^2 and the two sums ---------------------------
 __device__ __forceinline__ void pair_step(double zr, double zi2, double t, double w, double& u0, double& u1) {
@@ -414,6 +438,85 @@ __device__ __forceinline__ cd angular_direct(cd eta, ZetaDD z, double mu0, const
   return {mu0 + fma(dr, cr, -(di * ci)), fma(dr, ci, di * cr)};
 }
 
+// The direct routes on a rule split into blocks (FP64 kernel, n_pairs >= kBlkMinPairs): C(zeta) = sum_j w_j/(zeta - t_j)
+// block by block.  For block b with interval [c - h, c + h]: w' = (zeta - c)/h, root = sqrt(w'^2 - 1) on the branch
+// |w' + root| >= 1, s = 1/(w' + root) (|s| = 1/rho_b), and
+//     sum_{j in b} w_j/(zeta - t_j) = (1/h) (2/root) sum'_k M_k s^k          (M_k: the block's Chebyshev moments)
+// wherever rho_b^2 >= kBlkRho2Min (K_b <= kBlkTerms terms, one real-coefficient polynomial: 2 DFMA per term); the
+// blocks next to zeta are summed pair by pair as before (DD: with zeta and t_j in double-double, the EXACT form).
+// S = mu0 + (eta - zeta) C(zeta).  Near [0,1] a node-term costs its own block (and at times a neighbour) instead of
+// every pair of the rule.
+#ifndef GF_BLK_INLINE
+#define GF_BLK_INLINE 1   // measured: as a called function 3 to 10 % slower on every config
+#endif
+template <bool DD, bool COUNT>
+#if GF_BLK_INLINE
+__device__ __forceinline__
+#else
+__device__ __noinline__
+#endif
+cd angular_blocked(cd eta, ZetaDD z, const Tabs<double>& tb, RouteCount& rc) {
+  double u0 = 0.0, u1 = 0.0, v0 = 0.0, v1 = 0.0;   // direct sums: U0 = sum q_j; U1 = sum q_j a_j (DD) or sum q_j t_j
+  cd far = {0.0, 0.0};
+#pragma unroll 1
+  for (int b = 0; b < tb.n_blk; ++b) {
+    const double2 ch = tb.blk[b];
+    const double wr = (z.re_hi - ch.x) * ch.y, wi = z.im * ch.y;
+    const double qr = fma(wr, wr, -fma(wi, wi, 1.0)), qi = 2.0 * wr * wi;   // w'^2 - 1
+    const double n2 = fma(qr, qr, qi * qi);
+    const double rm = rsqrt_fast(n2);                                      // 1/|q| = 1/|root|^2
+    const double h2 = 0.5 * fma(n2, rm, fabs(qr));
+    const double rh = rsqrt_fast(h2);
+    const double h = h2 * rh, kk = 0.5 * qi * rh;
+    double ar = qr >= 0.0 ? h : fabs(kk), ai = qr >= 0.0 ? kk : copysign(h, qi);
+    if (fma(wr, ar, wi * ai) < 0.0) { ar = -ar; ai = -ai; }
+    const double Dr = wr + ar, Di = wi + ai;
+    const double rho2 = fma(Dr, Dr, Di * Di);
+    if ((float)rho2 >= kBlkRho2Min) {       // false for NaN (zeta on an end point of the block's interval): direct
+      const double in = rcp_fast(rho2);
+      const double sr = Dr * in, si = -Di * in, rr = sr + sr, ns = -in;
+      const int K = min((int)(112.f * rcp_ftz(lg2_ftz((float)rho2))) + 1, kBlkTerms);
+      const double* M = tb.blkM + b * kBlkTerms;
+      double p1 = 0.0, p2 = 0.0;
+#pragma unroll 1
+      for (int k = K - 1; k >= 0; --k) {
+        const double t = fma(rr, p1, fma(ns, p2, M[k]));
+        p2 = p1;
+        p1 = t;
+      }
+      const cd P = {fma(-p2, sr, p1), p2 * si};          // c_0 - c_1 conj(s)
+      const double g2 = 2.0 * ch.y * rm;                 // (1/h) 2/root = (2/h) conj(root)/|root|^2
+      far = cadd(far, cmul(cd{ar * g2, -ai * g2}, P));
+      if (COUNT) { ++rc.blk_series; rc.blk_terms += K; }
+    } else {
+      const int j0 = b * kBlkPairs, j1 = min(j0 + kBlkPairs, tb.n_pairs);
+      int j = j0;
+#pragma unroll 1
+      for (; j + 2 <= j1; j += 2) {
+        if (DD) {
+          direct_step(z.re_hi, z.re_lo, z.im2, tb.st[j], tb.stlo[j], tb.sw[j], u0, u1);
+          direct_step(z.re_hi, z.re_lo, z.im2, tb.st[j + 1], tb.stlo[j + 1], tb.sw[j + 1], v0, v1);
+        } else {
+          pair_step(z.re_hi, z.im2, tb.st[j], tb.sw[j], u0, u1);
+          pair_step(z.re_hi, z.im2, tb.st[j + 1], tb.sw[j + 1], v0, v1);
+        }
+      }
+      if (j < j1) {
+        if (DD) direct_step(z.re_hi, z.re_lo, z.im2, tb.st[j], tb.stlo[j], tb.sw[j], u0, u1);
+        else pair_step(z.re_hi, z.im2, tb.st[j], tb.sw[j], u0, u1);
+      }
+      if (COUNT) { if (DD) rc.exact_pairs += j1 - j0; else rc.near_pairs += j1 - j0; }
+    }
+  }
+  u0 += v0;
+  u1 += v1;
+  // sum over the direct blocks of w_j/(zeta - t_j): U1 - i Im U0 (DD: U1 = sum q a), conj(zeta) U0 - U1 otherwise
+  const cd Cd = DD ? cd{u1, -z.im * u0} : cd{fma(z.re_hi, u0, -u1), -z.im * u0};
+  const cd C = cadd(Cd, far);
+  const double dr = (eta.re - z.re_hi) - z.re_lo, di = eta.im - z.im;
+  return {tb.mu0 + fma(dr, C.re, -(di * C.im)), fma(dr, C.im, di * C.re)};
+}
+
 // ---------------------------------------------------------------------------------------------
 // One (point, radial node, pole): S(delta, zeta) by the route zeta selects.  delta = eta - 1/4.
 // WARP-COLLECTIVE: all 32 lanes must call it together (the series loop runs to the warp's longest
@@ -453,7 +556,7 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     o.K = ((int)(2.f * kSeriesBits * il) + 5) & ~3;         // + 2, rounded up to whole trips of four terms
     // FP32 from term K1 on: its rounding error 2^-24 A (|s|/2)^K1 (A <= 2.4 the recurrence's amplification) must stay
     // below 2^-kSeriesBits of the first-order term b_1 s of N, the smallest S can be: (|s|/2)^K1 <= 2^-(kSeriesBits-14) |s|
-    o.K1 = min(((int)((2.f * (kSeriesBits - 14.f) - l2) * il) + 5) & ~3, o.K);
+    o.K1 = min(((int)((2.f * (kSeriesBits - 14.f - kFp32Slack) - l2) * il) + 5) & ~3, o.K);
   } else {
     // root = sqrt(zeta (zeta - 1)) = sqrt(w^2 - 1)/2, sign such that |w + 2 root| >= 1
     const double zm = zeta.re - 1.0, wr = fma(2.0, zeta.re, -1.0), wi = zeta.im + zeta.im;
@@ -515,13 +618,22 @@ __device__ __forceinline__ cd series_finish(const SeriesArg& o, cd delta, double
 }
 
 // The direct loop for a lane on the NEAR or EXACT route
-template <typename T, bool COUNT>
+template <typename T, bool COUNT, bool BLK>
 __device__ __forceinline__ cd direct_route(const Tabs<T>& tb, int route, bool warp_has_exact, cd x, cd y, cd delta,
                                            cd zeta, double mur, double mui, RouteCount& rc, double mur_lo = 0.0,
                                            double mui_lo = 0.0) {
   cd s;
   const cd eta = {__dadd_rn(0.25, delta.re), delta.im};
   bool dd_loop = true;
+  if (BLK && sizeof(T) == 8 && tb.n_blk > 0) {
+    // the rule is split into blocks: far blocks by their own short series, the blocks next to zeta pair by pair
+    ZetaDD z = {zeta.re, 0.0, zeta.im, zeta.im * zeta.im};
+    if (route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y.re, y.im, mur, mui, mur_lo, mui_lo);
+    const Tabs<double>& tbd = reinterpret_cast<const Tabs<double>&>(tb);
+    s = warp_has_exact ? angular_blocked<true, COUNT>(eta, z, tbd, rc) : angular_blocked<false, COUNT>(eta, z, tbd, rc);
+    if (COUNT) { if (route == ROUTE_EXACT) ++rc.n_exact; else ++rc.n_near; }
+    return s;
+  }
   if (sizeof(T) == 8 && !warp_has_exact) {
     // no EXACT lane in this warp (voted by all 32 lanes before the routes diverge, so the choice of loop does
     // not depend on how the hardware groups the lanes): the 8-instruction pair
@@ -542,7 +654,9 @@ __device__ __forceinline__ cd direct_route(const Tabs<T>& tb, int route, bool wa
   return s;
 }
 
-template <typename T, bool COUNT>
+// BLK: the kernel instantiation that carries the blocked direct routes (launched for rules of kBlkMinPairs and more
+// folded pairs; the other instantiation does not pay their registers)
+template <typename T, bool COUNT, bool BLK = false>
 __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta, cd zeta, double mur, double mui,
                                         RouteCount& rc, double mur_lo = 0.0, double mui_lo = 0.0) {
   const SeriesArg o = route_setup<T>(tb, zeta);
@@ -563,15 +677,15 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
     if (o.route <= ROUTE_CHEB) s = series_finish<COUNT>(o, delta, p1, p2, n1, n2, rc);
   }
   if (o.route >= ROUTE_NEAR)
-    s = direct_route<T, COUNT>(tb, o.route, warp_has_exact, x, y, delta, zeta, mur, mui, rc, mur_lo, mui_lo);
+    s = direct_route<T, COUNT, BLK>(tb, o.route, warp_has_exact, x, y, delta, zeta, mur, mui, rc, mur_lo, mui_lo);
   return s;
 }
 
 // Add this thread's counters to the launch's (one atomic per warp and counter)
 __device__ __forceinline__ void flush_counters(const RouteCount& rc, bool active, unsigned long long* counters) {
-  unsigned long long v[kNumCounters] = {rc.near_pairs, rc.series_exec, rc.exact_pairs, rc.n_near,
-                                        rc.n_moment,   rc.n_exact,     rc.n_cheb,      rc.series_used,
-                                        rc.tails,      rc.series_exec32};
+  unsigned long long v[kNumCounters] = {rc.near_pairs, rc.series_exec, rc.exact_pairs,   rc.n_near,
+                                        rc.n_moment,   rc.n_exact,     rc.n_cheb,        rc.series_used,
+                                        rc.tails,      rc.series_exec32, rc.blk_series,  rc.blk_terms};
   for (int k = 0; k < kNumCounters; ++k) {
     if (!active) v[k] = 0;
     for (int o = 16; o; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
@@ -629,6 +743,39 @@ __device__ void prep_series_T(const EvalArgs& a, const BlobLayout& L, double* bl
       Tm = Tk;
       Tk = Tn;
       row[k] = Tn.hi;
+    }
+  }
+}
+
+// Block tables of the folded rule (call after prep_angular and a __syncthreads()): per block its interval
+// [c - h, c + h] (the extreme t of its pairs) as (c, 1/h), and M_k = sum'_{j in b} w_j T_k(tau_j), tau_j = (t_j - c)/h,
+// k < kBlkTerms (k = 0 halved), T_k by the three-term recurrence and the sums in double-double.  One thread per (b, k).
+__device__ void prep_blocks(const EvalArgs& a, const BlobLayout& L, double* blob) {
+  for (int e = threadIdx.x; e < L.n_blk * kBlkTerms; e += blockDim.x) {
+    const int b = e / kBlkTerms, k = e % kBlkTerms;
+    const int j0 = b * kBlkPairs, j1 = min(j0 + kBlkPairs, a.n_pairs);
+    double tmin = blob[L.off_t + j0], tmax = tmin;
+    for (int j = j0 + 1; j < j1; ++j) {
+      tmin = fmin(tmin, blob[L.off_t + j]);
+      tmax = fmax(tmax, blob[L.off_t + j]);
+    }
+    const double c = 0.5 * (tmin + tmax), ih = 1.0 / fmax(0.5 * (tmax - tmin), 1e-12);
+    dd acc = {0.0, 0.0};
+    for (int j = j0; j < j1; ++j) {
+      const dd tau = dd_mul_d(dd_add_d(dd{blob[L.off_t + j], blob[L.off_tlo + j]}, -c), ih);
+      const dd twot = dd_scale2(tau, 2.0);
+      dd Tm = {1.0, 0.0}, Tk = tau;       // T_0, T_1
+      for (int q = 2; q <= k; ++q) {
+        const dd Tn = dd_add(dd_mul(twot, Tk), dd_neg(Tm));
+        Tm = Tk;
+        Tk = Tn;
+      }
+      acc = dd_add(acc, dd_mul_d(k == 0 ? dd{1.0, 0.0} : Tk, blob[L.off_w + j]));
+    }
+    blob[L.off_blkM + b * kBlkTerms + k] = (k == 0 ? 0.5 : 1.0) * acc.hi;
+    if (k == 0) {
+      blob[L.off_blk + 2 * b] = c;
+      blob[L.off_blk + 2 * b + 1] = ih;
     }
   }
 }
@@ -729,7 +876,7 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc 
       // perturbation of c_k by <= 4 2^-24 max_{j>=k}|c_j| / (1 - 1/rho)^2, and the perturbations sum like a geometric
       // series: the FP32 phase costs <= 2^-22 max_{j>=K1} |c_j| rho^-j / (1 - 1/rho)^3, held below the truncation
       // budget: |c_j| rho^-j <= 2^-(kSeriesBits - 20) (1 - 1/rho)^3 |c_0| for all j >= K1
-      const float thr = kSeriesBits - 20.f + 3.f * log2f(1.f / (1.f - exp2f(-ell)));
+      const float thr = kSeriesBits - 20.f - kFp32Slack + 3.f * log2f(1.f / (1.f - exp2f(-ell)));
       for (int j = L.kmc - 1; j >= 0; --j)
         if (s_lc[j] - (float)j * ell > -thr) {
           K1 = j + 1;

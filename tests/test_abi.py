@@ -47,7 +47,7 @@ def test_struct_layout_matches_header(gf):
     # gf_params: 2 propagators of (int, 5 doubles) + 3 doubles + int + 2 doubles + 3 ints + 1 double, natural alignment
     assert ctypes.sizeof(gf.gf_propagator) == 48
     assert ctypes.sizeof(gf.gf_params) == 2 * 48 + 3 * 8 + 8 + 2 * 8 + 8 + 8 + 8
-    assert ctypes.sizeof(gf.gf_launch_info) == 40 + 8 + 18 * 8
+    assert ctypes.sizeof(gf.gf_launch_info) == 40 + 8 + 22 * 8
 
 
 def test_host_quadrature_is_symmetric_and_exact(gf):

@@ -282,27 +282,40 @@ def test_ragged_point_counts(gf, oracle, n_points):
 
 
 def test_route_counters(gf):
-    """Every (point, node, pole) triple takes exactly one route; the counted call returns the same G."""
-    cfg = W.CONFIGS["cfg2_mid"]
-    P, rn, rw, z, wz = gpu_setup(gf, cfg)
-    x = gpu_grid(gf, cfg)
-    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
-    g2, c = gf.eval_grid_counted(P, rn, rw, cfg["n_rad"], z, wz, x)
-    assert torch.equal(g.view(torch.float64), g2.view(torch.float64))
-    n_pairs = cfg["n_ang"] // 2
-    series_nodes = c["moment_nodes"] + c["cheb_nodes"]
-    # the nodes of the large-y tail take no route; the rest take exactly one
-    assert 0 < c["near_nodes"] + series_nodes + c["exact_nodes"] < 0.6 * x.numel() * cfg["n_rad"]
-    assert c["tails"] == x.numel()
-    # pairs are counted by loop (the NEAR lanes of a warp with an EXACT lane run the double-double loop too)
-    assert c["near_pairs"] + c["exact_pairs"] == (c["near_nodes"] + c["exact_nodes"]) * n_pairs
-    assert c["exact_pairs"] >= c["exact_nodes"] * n_pairs
-    # each series triple needs 4..256 terms; a warp runs its longest series on all 32 lanes, the high-order terms in
-    # FP32 (counter "series_terms_fp32"), the rest in FP64 ("series_terms")
-    assert 4 * series_nodes <= c["series_terms_needed"] <= 256 * series_nodes
-    assert c["series_terms_needed"] <= c["series_terms"] + c["series_terms_fp32"] <= 256 * x.numel() * cfg["n_rad"]
-    assert c["series_terms"] > 0 and c["series_terms_fp32"] > 0
-    assert 0 < c["exact_nodes"] < 0.2 * (c["near_nodes"] + c["exact_nodes"]) and c["cheb_nodes"] > c["near_nodes"]
+    """Every (point, node, pole) triple takes exactly one route; the counted call returns the same G.  Config 2's rule
+    (64 folded pairs) is not split; a rule of 256 folded pairs is split into 8 blocks of 32, and a direct node-term
+    then takes every block exactly one way: pair by pair, or by the block's own series where it is far from zeta."""
+    for name, n_ang in (("cfg2_mid", None), ("cfg1_tiny", 512)):
+        cfg = dict(W.CONFIGS[name])
+        if n_ang:
+            cfg["n_ang"] = n_ang
+        P, rn, rw, z, wz = gpu_setup(gf, cfg)
+        x = gpu_grid(gf, cfg)
+        g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+        g2, c = gf.eval_grid_counted(P, rn, rw, cfg["n_rad"], z, wz, x)
+        assert torch.equal(g.view(torch.float64), g2.view(torch.float64))
+        n_pairs = cfg["n_ang"] // 2
+        series_nodes = c["moment_nodes"] + c["cheb_nodes"]
+        direct_nodes = c["near_nodes"] + c["exact_nodes"]
+        # the nodes of the large-y tail take no route; the rest take exactly one
+        assert 0 < direct_nodes + series_nodes < 0.8 * x.numel() * cfg["n_rad"]
+        assert c["tails"] % x.numel() == 0 and c["tails"] >= x.numel()   # one per (point, pole) and lane sharing the point
+        # pairs are counted by loop (the NEAR lanes of a warp with an EXACT lane run the double-double loop too)
+        assert c["near_pairs"] + c["exact_pairs"] + 32 * c["block_series"] == direct_nodes * n_pairs
+        if n_pairs < 192:
+            assert c["block_series"] == 0 and c["block_series_terms"] == 0
+            assert c["exact_pairs"] >= c["exact_nodes"] * n_pairs
+        else:
+            n_blk = (n_pairs + 31) // 32
+            assert c["near_pairs"] + c["exact_pairs"] >= direct_nodes * 32            # at least its own block
+            assert 0 < c["block_series"] <= (n_blk - 1) * direct_nodes
+            assert c["block_series"] <= c["block_series_terms"] <= 32 * c["block_series"]
+        # each series triple needs 4..256 terms; a warp runs its longest series on all 32 lanes, the high-order terms
+        # in FP32 (counter "series_terms_fp32"), the rest in FP64 ("series_terms")
+        assert 4 * series_nodes <= c["series_terms_needed"] <= 256 * series_nodes
+        assert c["series_terms_needed"] <= c["series_terms"] + c["series_terms_fp32"] <= 256 * x.numel() * cfg["n_rad"]
+        assert c["series_terms"] > 0 and c["series_terms_fp32"] > 0
+        assert 0 < c["exact_nodes"] < 0.5 * direct_nodes and c["cheb_nodes"] > c["near_nodes"]
 
 
 def test_empty_input(gf):
