@@ -28,7 +28,7 @@
  *     the real axis, Fortran order).
  *   - Errors: GF_ERR_NULL for a null pointer, GF_ERR_ARG for a value out of range,
  *     GF_ERR_UNSUPPORTED for a combination the method does not define or that is not built (taylor_order outside
- *     [0, 4], taylor_order > 0 off the REAL contour, with the symmetric routing or with precision 32, a
+ *     [0, 4], taylor_order > 0 with the symmetric routing or with precision 32, a
  *     subtraction point other than 0, a dimension other than 4 or the symmetric routing on a
  *     deformed contour, the symmetric routing with unequal or rational lines, the THREAD contour
  *     with unequal or complex masses, a rational propagator with a double pole, precision 32 on a
@@ -123,7 +123,7 @@ typedef struct {
                             p = 0 (eq. (20) sets the scalar product to zero with x): t^n is the Taylor operator in the
                             external momentum, x^i standing for the order 2i in p, so (1 - t^n) F is F minus every
                             term of its expansion in p up to the order 2n and G_n = G - sum_{i<=n} x^i G^(i)(0)/i! =
-                            O(x^(n+1)).  n > 0: REAL contour, the paper's routing, precision 64 (any dim) */
+                            O(x^(n+1)).  n > 0: any contour policy, the paper's routing, precision 64 (any dim on REAL) */
   double prefactor;      /* c0; 1/(2 pi)^3 is eq. (14), 2/pi the rescaled eq. (21) */
   double map_scale;      /* s0 > 0 of the shifted-log radial map y(u) = a + (a+s0) expm1(u L) */
   int contour;           /* gf_contour */

@@ -12,7 +12,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libgf_b200.so")
 SOURCES = ["gf_api.cu", "gf_eval.cu", "gf_contour.cu", "gf_taylor.cu", "gf_cut.cu", "gf_grid.cu", "gf_diag.cu", "gf_tables.cpp"]
-HEADERS = [os.path.join(CSRC, "gf_internal.h"), os.path.join(CSRC, "gf_routes.cuh"), os.path.join(CSRC, "gf_dd.cuh"), os.path.join(ROOT, "include", "gf.h")]
+HEADERS = [os.path.join(CSRC, "gf_internal.h"), os.path.join(CSRC, "gf_routes.cuh"), os.path.join(CSRC, "gf_dd.cuh"), os.path.join(CSRC, "gf_geometry.cuh"), os.path.join(ROOT, "include", "gf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--threads", "4"]
 

@@ -205,8 +205,8 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   if (p->precision != 64 && p->precision != 32) { set_error("eval_grid: precision must be 64 or 32"); return GF_ERR_ARG; }
   if (p->contour < GF_CONTOUR_REAL || p->contour > GF_CONTOUR_AUTO) { set_error("eval_grid: unknown contour %d", p->contour); return GF_ERR_ARG; }
   if (p->taylor_order < 0 || p->taylor_order > kMaxTaylor) { set_error("eval_grid: taylor_order %d outside [0, %d] (eq. (13))", p->taylor_order, kMaxTaylor); return GF_ERR_UNSUPPORTED; }
-  if (p->taylor_order > 0 && (p->contour != GF_CONTOUR_REAL || p->routing != 0 || p->precision != 64)) {
-    set_error("eval_grid: taylor_order > 0 is built for the REAL contour, the paper's routing and precision 64");
+  if (p->taylor_order > 0 && (p->routing != 0 || p->precision != 64)) {
+    set_error("eval_grid: taylor_order > 0 is built for the paper's routing and precision 64");
     return GF_ERR_UNSUPPORTED;
   }
   if (p->sub_re != 0 || p->sub_im != 0) { set_error("eval_grid: subtraction point must be 0 (eq. (13))"); return GF_ERR_UNSUPPORTED; }

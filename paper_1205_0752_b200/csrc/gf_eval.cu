@@ -118,8 +118,11 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
   }
   __syncthreads();  // the T_k(s_j) matrix, the monomial moments and the radial tables are complete
   prep_series_sums(a, L, blob, s_cpart);
+  if (L.n_poly) prep_series_A(a, L, blob);
   __syncthreads();
-  prep_series_kreq(L, blob, s_lc, blob + L.off_cheb, 2);
+  // Kreq from the tables the evaluation kernel will run: order 0's two, or the n + 2 of a Taylor order
+  if (L.n_poly) prep_series_kreq(L, blob, s_lc, blob + L.off_chebA, L.n_poly);
+  else prep_series_kreq(L, blob, s_lc, blob + L.off_cheb, 2);
   if (L.off_gam >= 0) {
     prep_tail_gamma(L, blob, s_part, s_mu, s_nu);
     const TailJob J = real_tail_job(a, L, blob);
@@ -298,7 +301,8 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
 // pyramid: the layout of the deformed-contour kernel (gf_contour.cu).  It stages the angular rule, the series
 // tables, levels 2 and 3 of the radial pyramid and the tail's gamma table; the REAL node tables (read by the points
 // AUTO sends to REAL), every Rhat table and the rung tables stay in global memory.
-BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail, bool sym) {
+BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail, bool sym,
+                            int taylor_order) {
   BlobLayout L = {};
   L.npad = (n_pairs + 3) & ~3;
   L.kmc = kKmc;
@@ -328,6 +332,11 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
   L.off_rw = pyramid ? (int)take(L.n_tab) : -1;
   L.off_gam = tail ? (int)take(kTailN * (kTailN + 1) / 2) : -1;
   L.off_gam2 = tail && sym ? (int)take(kTailN * (kTailN + 1) / 2) : -1;
+  // Taylor order n > 0 on a deformed contour (gf_taylor.cu): the n + 2 series tables per family, staged
+  L.n_poly = taylor_order > 0 ? taylor_order + 2 : 0;
+  L.off_momA = L.n_poly ? (int)take((long long)kMomTerms * L.n_poly) : -1;
+  L.off_chebA = L.n_poly ? (int)take((long long)L.kmc * L.n_poly) : -1;
+  L.off_ic = -1;
   L.n_blk = n_pairs >= kBlkMinPairs ? (n_pairs + kBlkPairs - 1) / kBlkPairs : 0;
   L.off_blk = L.n_blk ? (int)take(2 * L.n_blk) : -1;
   L.off_blkM = L.n_blk ? (int)take((long long)L.n_blk * kBlkTerms) : -1;
@@ -363,7 +372,7 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
 
 // ---------------------------------------------------------------------------------------------
 int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
-  if (a.taylor_order > 0) return plan_taylor(a, plan);
+  if (a.taylor_order > 0 && a.contour == GF_CONTOUR_REAL) return plan_taylor(a, plan);
   plan->block_threads = kBlockThreads;
   plan->shared_nodes = (a.contour == GF_CONTOUR_REAL);
   // lanes per point: enough threads for >= 2 CTAs on each of the 148 SMs, at most a warp
@@ -374,7 +383,7 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   const long long threads = a.n_points << sl;
   plan->grid_blocks = (threads + kBlockThreads - 1) / kBlockThreads;
   plan->layout = make_blob_layout(a.n_rad, a.n_pairs, a.n_terms, precision == 32, !plan->shared_nodes, true,
-                                 a.routing == 1);
+                                 a.routing == 1, a.taylor_order);
   plan->smem_bytes = 16 + (size_t)plan->layout.n_doubles * sizeof(double);
   if (plan->smem_bytes > 200 * 1024) {
     set_error("eval_grid: tables need %zu bytes of shared memory (limit 200 KiB): reduce n_rad/n_ang",
@@ -431,7 +440,7 @@ int launch_prepare(const EvalArgs& a, int precision, double* blob, cudaStream_t 
   int rc = plan_eval(a, precision, &plan);
   if (rc) return rc;
   if ((rc = check_variant(plan, precision))) return rc;
-  if (a.taylor_order > 0) return launch_taylor_prepare(a, plan, blob, stream);
+  if (a.taylor_order > 0 && plan.shared_nodes) return launch_taylor_prepare(a, plan, blob, stream);
   prep_real_kernel<<<1, 256, 0, stream>>>(a, plan.layout, blob);
   if ((rc = check_cuda(cudaGetLastError(), "prep kernel launch"))) return rc;
   return plan.shared_nodes ? GF_OK : launch_prepare_rungs(a, plan, blob, stream);

@@ -161,7 +161,7 @@ int launch_taylor(const EvalArgs& a, const LaunchPlan& plan, const double* blob,
 
 // gf_cut.cu: the paper's Kernels 3 and 4 (a.x holds the y array / the x array, a.out the result)
 BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool pyramid, bool tail,
-                            bool sym = false);  // gf_eval.cu; pyramid: the layout of the deformed-contour kernel
+                            bool sym = false, int taylor_order = 0);  // gf_eval.cu; pyramid: the layout of the deformed-contour kernel
 int launch_angular(const EvalArgs& a, double x_re, double x_im, cudaStream_t stream);
 int launch_cut_crossings(const EvalArgs& a, int n_z, int* d_out, cudaStream_t stream);
 

@@ -843,6 +843,44 @@ __device__ void prep_series_sums(const EvalArgs& a, const BlobLayout& L, double*
   }
 }
 
+// Taylor orders n > 0 (gf_taylor.cu): the n + 2 series tables per family, the moments of the measures w_j t_j^q,
+//   momA[k][q] = sum_j w_j t_j^q (t_j - 1/2)^k (k < kMomTerms),  chebA[k][q] = sum'_j w_j t_j^q T_k(2 t_j - 1) (k < kmc),
+// in double-double (call after prep_series_T and a __syncthreads(): the T_k matrix is in the scratch).
+__device__ void prep_series_A(const EvalArgs& a, const BlobLayout& L, double* blob) {
+  const int NA = L.n_poly;
+  const double* scratch = blob + L.off_scratch;
+  for (int k = threadIdx.x; k < L.kmc; k += blockDim.x) {
+    dd ch[kMaxTaylor + 2], mo[kMaxTaylor + 2];
+    for (int q = 0; q < NA; ++q) ch[q] = mo[q] = dd{0.0, 0.0};
+    for (int j = 0; j < a.n_pairs; ++j) {
+      const dd t = {blob[L.off_t + j], blob[L.off_tlo + j]};
+      const double w = blob[L.off_w + j];
+      const double wT = w * scratch[(size_t)j * L.kmc + k];
+      dd cp = {0.0, 0.0};                   // w (t - 1/2)^k, k < kMomTerms
+      if (k < kMomTerms) {
+        const dd c = dd_add_d(t, -0.5);
+        dd p = {1.0, 0.0}, b = c;
+        for (int ex = k; ex; ex >>= 1) {
+          if (ex & 1) p = dd_mul(p, b);
+          b = dd_mul(b, b);
+        }
+        cp = dd_mul_d(p, w);
+      }
+      dd ta = {1.0, 0.0};                   // t^q
+      for (int q = 0; q < NA; ++q) {
+        ch[q] = dd_add(ch[q], dd_mul_d(ta, wT));
+        if (k < kMomTerms) mo[q] = dd_add(mo[q], dd_mul(ta, cp));
+        ta = dd_mul(ta, t);
+      }
+    }
+    const double half = k == 0 ? 0.5 : 1.0;   // sum': the k = 0 term of a Chebyshev series is halved
+    for (int q = 0; q < NA; ++q) {
+      blob[L.off_chebA + k * NA + q] = half * ch[q].hi;
+      if (k < kMomTerms) blob[L.off_momA + k * NA + q] = mo[q].hi;
+    }
+  }
+}
+
 // Kreq[b]: the number of Chebyshev terms after which every dropped term is below 2^-(kSeriesBits+2) of the leading
 // coefficient when log2(rho) >= kEllLo + b kEllStep: the smallest K with |c_j| rho^-j <= 2^-(kSeriesBits+2) |c_0| for all
 // j >= K, c_j the larger of the two coefficients.  For a rule that integrates the measure well the c_j beyond
@@ -1045,6 +1083,9 @@ __device__ __forceinline__ double radial_node(double t, dd Llog, double s0) {
 // angular series.  A log-mapped radial rule has most of its nodes in this tail (about 60 % on the production
 // scan), and they cost kTailN (kTailN + 1) DFMA per point instead of a series each.
 // ---------------------------------------------------------------------------------------------
+#ifndef GF_TAIL_ILP
+#define GF_TAIL_ILP 1
+#endif
 __device__ __forceinline__ cd tail_series(const double* __restrict__ gam, const double2* __restrict__ Rrow, cd x,
                                           cd a, double invy0) {
   const cd X = {4.0 * x.re * invy0, 4.0 * x.im * invy0}, Z = {-a.re * invy0, -a.im * invy0};
@@ -1056,6 +1097,39 @@ __device__ __forceinline__ cd tail_series(const double* __restrict__ gam, const 
   const double rr = rho.re + rho.re, ns = -fma(rho.re, rho.re, rho.im * rho.im);
   cd pw = {1.0, 0.0}, acc = {0.0, 0.0};
   const double* row = gam;
+#if GF_TAIL_ILP
+  // rows n and n + 1 together (kTailN is even): two independent recurrences, so that the one dependent chain per point
+  // that the series is does not wait on its own latency.  Row n holds the n coefficients of h_n, highest power of the
+  // ratio first when read from its end (fwd) or from its start.
+  static_assert(kTailN % 2 == 0, "the tail series takes its rows in pairs");
+  const int step = fwd ? -1 : 1;
+  const cd base2 = csqr(base);
+#pragma unroll 1
+  for (int n = 1; n <= kTailN; n += 2) {
+    const double* rowB = row + n;                       // row n + 1
+    const double* cA = fwd ? row + n - 1 : row;
+    const double* cB = fwd ? rowB + n : rowB;
+    double a0 = 0.0, a1 = 0.0, b1 = 0.0;
+    double b0 = *cB;                                    // row n + 1 is one coefficient longer
+    cB += step;
+#pragma unroll 2
+    for (int j = 0; j < n; ++j, cA += step, cB += step) {
+      const double ta = fma(rr, a0, fma(ns, a1, *cA));
+      const double tb = fma(rr, b0, fma(ns, b1, *cB));
+      a1 = a0; a0 = ta;
+      b1 = b0; b0 = tb;
+    }
+    const cd PA = {fma(-a1, rho.re, a0), a1 * rho.im};   // c_0 - c_1 conj(rho)
+    const cd PB = {fma(-b1, rho.re, b0), b1 * rho.im};
+    const double2 RA = Rrow[n - 1], RB = Rrow[n];
+    // acc += pw [PA RA + base PB RB]
+    const cd tB = cmul(cmul(PB, base), cd{RB.x, RB.y});
+    const cd tA = cmul(PA, cd{RA.x, RA.y});
+    acc = cadd(acc, cmul(pw, cadd(tA, tB)));
+    pw = cmul(pw, base2);
+    row += 2 * n + 1;
+  }
+#else
 #pragma unroll 1
   for (int n = 1; n <= kTailN; ++n) {
     double b0 = 0.0, b1 = 0.0;
@@ -1076,6 +1150,7 @@ __device__ __forceinline__ cd tail_series(const double* __restrict__ gam, const 
     pw = cmul(pw, base);
     row += n;
   }
+#endif
   return cmul(X, acc);
 }
 

@@ -26,6 +26,7 @@
 // terms; x^(n+1) is an explicit factor, so G_n(0) = 0 and small |x| keeps full accuracy.
 // One thread per grid point (or 1/S of its radial nodes), no warp-collective step, no tail series: every radial node
 // takes a route (far nodes need 4 to 8 series terms).
+#include "gf_geometry.cuh"
 #include "gf_routes.cuh"
 
 namespace gf {
@@ -40,6 +41,99 @@ __host__ __device__ constexpr double psi_coef(int i, int k) {
   if (r > n - r) r = n - r;
   for (int q = 1; q <= r; ++q) c = c * (double)(n - r + q) / (double)q;   // small integers: exact
   return ((i - k) & 1) ? -c : c;
+}
+
+// The staged tables one node-term needs
+struct TaylorTabs {
+  Tabs<double> tb;              // a_kreq, kmc, tau (route_setup)
+  const double *st, *stlo, *sw; // folded rule
+  const double *momA, *chebA;   // n + 2 series tables per family, [k][n + 2]
+  int n_pairs;
+};
+__device__ __forceinline__ TaylorTabs make_taylor_tabs(const double* sb, const BlobLayout& L, int n_pairs) {
+  TaylorTabs t = {};
+  t.tb.a_kreq = smem_u32(sb + L.off_kreq);
+  t.tb.kmc = L.kmc;
+  t.tb.tau = kTau64;
+  t.st = sb + L.off_t;
+  t.stlo = sb + L.off_tlo;
+  t.sw = sb + L.off_w;
+  t.momA = sb + L.off_momA;
+  t.chebA = sb + L.off_chebA;
+  t.n_pairs = n_pairs;
+  return t;
+}
+
+// xi^n S_n for one (point, radial node, pole): S_n = sum_j w_j Pi(t_j)/(zeta - t_j) by the route zeta selects (header).
+// y may be complex (deformed contours); pole: mu = hi + lo.
+template <int N>
+__device__ __forceinline__ cd taylor_node(const TaylorTabs& T, cd x, cd y, cd xi, cd kap, cd zeta, const PoleTerm& pole) {
+  constexpr int NA = N + 2;
+  const SeriesArg o = route_setup<double>(T.tb, zeta);
+  cd pi[NA];
+  {
+    cd kp = {1.0, 0.0};
+#pragma unroll
+    for (int q = 0; q < NA; ++q) {
+      pi[q] = cmul(kp, cd{fma(-xi.re, psi_coef(N, q), psi_coef(N + 1, q)), -xi.im * psi_coef(N, q)});
+      kp = cmul(kp, kap);
+    }
+  }
+  cd s;
+  if (o.route <= ROUTE_CHEB) {
+    const double* tab = o.route == ROUTE_CHEB ? T.chebA : T.momA;
+    const double rr = o.sg.re + o.sg.re, ns = o.ns;
+    double p1[NA], p2[NA];
+#pragma unroll
+    for (int q = 0; q < NA; ++q) p1[q] = p2[q] = 0.0;
+#pragma unroll 1
+    for (int k = o.K - 1; k >= 0; --k) {
+      const double* c = tab + k * NA;
+#pragma unroll
+      for (int q = 0; q < NA; ++q) {
+        const double b = fma(rr, p1[q], fma(ns, p2[q], c[q]));
+        p2[q] = p1[q];
+        p1[q] = b;
+      }
+    }
+    cd acc = {0.0, 0.0};
+#pragma unroll
+    for (int q = 0; q < NA; ++q) {
+      const cd P = {fma(-p2[q], o.sg.re, p1[q]), p2[q] * o.sg.im};   // c_0 - c_1 conj(s)
+      acc = cadd(acc, cmul(pi[q], P));
+    }
+    s = cmul(o.g, acc);
+  } else {
+    ZetaDD z = {zeta.re, 0.0, zeta.im, zeta.im * zeta.im};
+    if (o.route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y.re, y.im, pole.mu_re, pole.mu_im, pole.mu_re_lo, pole.mu_im_lo);
+    double u0 = 0.0, ua = 0.0, v0 = 0.0, va = 0.0;
+    int j = 0;
+#pragma unroll 1
+    for (; j + 2 <= T.n_pairs; j += 2) {
+      direct_step(z.re_hi, z.re_lo, z.im2, T.st[j], T.stlo[j], T.sw[j], u0, ua);
+      direct_step(z.re_hi, z.re_lo, z.im2, T.st[j + 1], T.stlo[j + 1], T.sw[j + 1], v0, va);
+    }
+    if (j < T.n_pairs) direct_step(z.re_hi, z.re_lo, z.im2, T.st[j], T.stlo[j], T.sw[j], u0, ua);
+    u0 += v0;
+    ua += va;
+    const cd C = {ua, -z.im * u0};                   // sum_j w_j/(zeta - t_j)
+    const cd zt = {z.re_hi, z.im};
+    cd Pz = pi[NA - 1], h = {T.momA[0], 0.0}, qs = cmul(pi[1], h);   // momA[q] = m^(q)_0 = sum_j w_j t_j^q
+#pragma unroll
+    for (int q = NA - 2; q >= 0; --q) Pz = cadd(cmul(Pz, zt), pi[q]);
+#pragma unroll
+    for (int q = 2; q < NA; ++q) {                   // h_q = sum_{b<q} mu_b zeta^(q-1-b)
+      h = cmul(h, zt);
+      h.re += T.momA[q - 1];
+      qs = cadd(qs, cmul(pi[q], h));
+    }
+    const cd PC = cmul(Pz, C);
+    s = {PC.re - qs.re, PC.im - qs.im};
+  }
+  cd xn = xi;
+#pragma unroll
+  for (int q = 1; q < N; ++q) xn = cmul(xn, xi);     // xi^n
+  return cmul(xn, s);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -77,40 +171,9 @@ __global__ void __launch_bounds__(256) prep_taylor_kernel(const __grid_constant_
     }
   }
   __syncthreads();
-  const int NA = L.n_poly;
-  const double* scratch = blob + L.off_scratch;
-  for (int k = threadIdx.x; k < L.kmc; k += blockDim.x) {
-    dd ch[kMaxTaylor + 2], mo[kMaxTaylor + 2];
-    for (int q = 0; q < NA; ++q) ch[q] = mo[q] = dd{0.0, 0.0};
-    for (int j = 0; j < a.n_pairs; ++j) {
-      const dd t = {blob[L.off_t + j], blob[L.off_tlo + j]};
-      const double w = blob[L.off_w + j];
-      const double wT = w * scratch[(size_t)j * L.kmc + k];
-      dd cp = {0.0, 0.0};                   // w (t - 1/2)^k, k < kMomTerms
-      if (k < kMomTerms) {
-        const dd c = dd_add_d(t, -0.5);
-        dd p = {1.0, 0.0}, b = c;
-        for (int ex = k; ex; ex >>= 1) {
-          if (ex & 1) p = dd_mul(p, b);
-          b = dd_mul(b, b);
-        }
-        cp = dd_mul_d(p, w);
-      }
-      dd ta = {1.0, 0.0};                   // t^q
-      for (int q = 0; q < NA; ++q) {
-        ch[q] = dd_add(ch[q], dd_mul_d(ta, wT));
-        if (k < kMomTerms) mo[q] = dd_add(mo[q], dd_mul(ta, cp));
-        ta = dd_mul(ta, t);
-      }
-    }
-    const double half = k == 0 ? 0.5 : 1.0;   // sum': the k = 0 term of a Chebyshev series is halved
-    for (int q = 0; q < NA; ++q) {
-      blob[L.off_chebA + k * NA + q] = half * ch[q].hi;
-      if (k < kMomTerms) blob[L.off_momA + k * NA + q] = mo[q].hi;
-    }
-  }
+  prep_series_A(a, L, blob);
   __syncthreads();
-  prep_series_kreq(L, blob, s_lc, blob + L.off_chebA, NA);
+  prep_series_kreq(L, blob, s_lc, blob + L.off_chebA, L.n_poly);
   if (threadIdx.x == 0) {
     blob[0] = (double)bad;
     blob[1] = a.ws_tag;
@@ -125,7 +188,6 @@ template <int N, int NT>
 __global__ void __launch_bounds__(kBlockThreads, 2)
     eval_taylor_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                        const double* __restrict__ blob) {
-  constexpr int NA = N + 2;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
   double* sb = reinterpret_cast<double*>(smem_raw + 16);
@@ -140,15 +202,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   if (threadIdx.x == 0) bulk_load(sb, blob, (uint32_t)(L.n_doubles * sizeof(double)), bar);
   mbar_wait(bar, 0);
 
-  Tabs<double> tb = {};
-  tb.a_kreq = smem_u32(sb + L.off_kreq);
-  tb.kmc = L.kmc;
-  tb.tau = kTau64;
-  const double* st = sb + L.off_t;
-  const double* stlo = sb + L.off_tlo;
-  const double* sw = sb + L.off_w;
-  const double* momA = sb + L.off_momA;
-  const double* chebA = sb + L.off_chebA;
+  const TaylorTabs T = make_taylor_tabs(sb, L, a.n_pairs);
   const bool bad_rule = sb[0] != 0.0;
 
   const int S = 1 << a.split_log2;
@@ -182,14 +236,6 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
     C2[r] = cmul(xm, cscale(xinv, 0.5));
     C1x4[r] = cscale(cmul(xm, C2[r]), 2.0);
   }
-  double e1[NA], e0[NA], mu[NA];
-#pragma unroll
-  for (int q = 0; q < NA; ++q) {
-    e1[q] = psi_coef(N + 1, q);
-    e0[q] = psi_coef(N, q);
-    mu[q] = momA[q];            // m^(q)_0 = sum_j w_j t_j^q
-  }
-
   double g_re = 0.0, g_im = 0.0;
 #pragma unroll 1
   for (int i = sub; i < a.n_rad; i += S) {
@@ -202,71 +248,130 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
       const cd xi = cmul(x, ic);                       // x/c
       const cd kap = cscale(ic, 4.0 * y);              // 4y/c
       const cd zeta = {fma(C1x4[r].re, q4, fma(C3.re, y, C2[r].re)), fma(C1x4[r].im, q4, fma(C3.im, y, C2[r].im))};
-      const SeriesArg o = route_setup<double>(tb, zeta);
-      cd pi[NA];
-      {
-        cd kp = {1.0, 0.0};
-#pragma unroll
-        for (int q = 0; q < NA; ++q) {
-          pi[q] = cmul(kp, cd{fma(-xi.re, e0[q], e1[q]), -xi.im * e0[q]});
-          kp = cmul(kp, kap);
-        }
-      }
-      cd s;
-      if (o.route <= ROUTE_CHEB) {
-        const double* tab = o.route == ROUTE_CHEB ? chebA : momA;
-        const double rr = o.sg.re + o.sg.re, ns = o.ns;
-        double p1[NA], p2[NA];
-#pragma unroll
-        for (int q = 0; q < NA; ++q) p1[q] = p2[q] = 0.0;
+      const cd term = cmul(cd{prv.x, prv.y}, taylor_node<N>(T, x, cd{y, 0.0}, xi, kap, zeta, a.term[r]));
+      g_re += term.re;
+      g_im += term.im;
+    }
+  }
+  for (int o = 1; o < S; o <<= 1) {
+    g_re += __shfl_xor_sync(0xffffffffu, g_re, o);
+    g_im += __shfl_xor_sync(0xffffffffu, g_im, o);
+  }
+  if (active && sub == 0) {
+    if (is_zero) { g_re = 0.0; g_im = 0.0; }
+    g_re *= out_scale;
+    g_im *= out_scale;
+    if (bad_rule) { g_re = nan(""); g_im = nan(""); }
+    reinterpret_cast<double2*>(a.out)[point] = make_double2(g_re, g_im);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The same on the point-dependent contours (RAY_ARC, THREAD, AUTO; gf_geometry.cuh): the thread walks the n_rad nodes
+// of its point's contour (tables of gf_contour.cu's preparation: the REAL nodes, the ray's and the real tail's nodes
+// of the point's rung; lines and arcs from the staged rules) and sends every node through taylor_node with complex y.
+// Node weight: c0 (rule weight x dy/dt) y D1(y) R_r/(4y).  No tail series: the real tail's nodes take a route each.
+// ---------------------------------------------------------------------------------------------
+template <int N, int NT>
+__global__ void __launch_bounds__(kBlockThreads, 2)
+    eval_taylor_contour_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
+                               const double* __restrict__ blob) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
+  double* sb = reinterpret_cast<double*>(smem_raw + 16);
+  if (!workspace_matches(a, blob)) {
+    const long long pt = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> a.split_log2;
+    if (pt < a.n_points) reinterpret_cast<double2*>(a.out)[pt] = make_double2(nan(""), nan(""));
+    if (blockIdx.x == 0 && threadIdx.x == 0) report_status(a.status, kStatusWorkspace);
+    return;
+  }
+  if (threadIdx.x == 0) mbar_init(bar, 1);
+  __syncthreads();
+  if (threadIdx.x == 0) bulk_load(sb, blob, (uint32_t)(L.n_doubles * sizeof(double)), bar);
+  mbar_wait(bar, 0);
+  const TaylorTabs T = make_taylor_tabs(sb, L, a.n_pairs);
+  const double* srt = sb + L.off_rt;
+  const double* srw = sb + L.off_rw;
+  const bool bad_rule = sb[0] != 0.0;
+
+  const int S = 1 << a.split_log2;
+  const long long gtid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  const long long point = gtid >> a.split_log2;
+  const int sub = (int)(gtid & (S - 1));
+  const bool active = point < a.n_points;
+  cd x = {1.0, 0.0};
+  if (active) {
+    const double2 xv = a.x[point];
+    x = {xv.x, xv.y};
+  }
+  const bool is_zero = (x.re == 0.0 && x.im == 0.0);
+  double out_scale = 1.0;
+  const double xmax = fmax(fabs(x.re), fabs(x.im));
+  if (is_zero) x = {1.0, 0.0};
+  else if (xmax < 0x1p-200) {
+    const int k = -200 - ilogb(xmax);
+    x = {scalbn(x.re, k), scalbn(x.im, k)};
+    out_scale = scalbn(1.0, -k * (N + 1));
+  }
+  const cd xinv = cinv(x);
+  const Geo geo = build_geo(a, x.re, x.im);
+  const cd dir2 = {fma(geo.dre, geo.dre, -(geo.dim * geo.dim)), 2.0 * geo.dre * geo.dim};
+  const double* row = blob + L.off_rung + (long long)geo.row * L.rung_stride;
+  const bool real_pol = geo.pol == GF_CONTOUR_REAL;
+  const double* ty = real_pol ? blob + L.off_y : row + L.rg_y;
+  const double* tq4 = real_pol ? blob + L.off_q4 : row + L.rg_yq4;
+  const double2* tpref = reinterpret_cast<const double2*>(real_pol ? blob + L.off_pref : row + L.rg_pref);
+  const int tstride = real_pol ? L.n_rad_pad : L.n4p;
+
+  double g_re = 0.0, g_im = 0.0;
 #pragma unroll 1
-        for (int k = o.K - 1; k >= 0; --k) {
-          const double* c = tab + k * NA;
-#pragma unroll
-          for (int q = 0; q < NA; ++q) {
-            const double b = fma(rr, p1[q], fma(ns, p2[q], c[q]));
-            p2[q] = p1[q];
-            p1[q] = b;
-          }
-        }
-        cd acc = {0.0, 0.0};
-#pragma unroll
-        for (int q = 0; q < NA; ++q) {
-          const cd P = {fma(-p2[q], o.sg.re, p1[q]), p2[q] * o.sg.im};   // c_0 - c_1 conj(s)
-          acc = cadd(acc, cmul(pi[q], P));
-        }
-        s = cmul(o.g, acc);
+  for (int g = sub; g < a.n_rad; g += S) {
+    const NodeAt at = locate(geo.pol, a.n_rad, g);
+    const bool table = at.type == SEG_TABLE || at.type == SEG_TAIL;
+    cd y, q4, W = {0.0, 0.0};
+    if (table) {
+      y = {ty[at.i], 0.0};
+      q4 = {tq4[at.i], 0.0};
+    } else {
+      cd base;
+      if (at.type == SEG_RAY) {
+        const double r = row[L.rg_r + at.i], q4r = row[L.rg_q4 + at.i], rw = row[L.rg_w + at.i];
+        y = {__dmul_rn(geo.dre, r), __dmul_rn(geo.dim, r)};
+        q4 = {geo.dre * q4r, -geo.dim * q4r};
+        base = {dir2.re * rw, dir2.im * rw};          // c0 wy y = c0 dir^2 r dr
       } else {
-        ZetaDD z = {zeta.re, 0.0, zeta.im, zeta.im * zeta.im};
-        if (o.route == ROUTE_EXACT) z = zeta_dd(x.re, x.im, y, 0.0, a.term[r].mu_re, a.term[r].mu_im, a.term[r].mu_re_lo, a.term[r].mu_im_lo);
-        double u0 = 0.0, ua = 0.0, v0 = 0.0, va = 0.0;
-        int j = 0;
-#pragma unroll 1
-        for (; j + 2 <= a.n_pairs; j += 2) {
-          direct_step(z.re_hi, z.re_lo, z.im2, st[j], stlo[j], sw[j], u0, ua);
-          direct_step(z.re_hi, z.re_lo, z.im2, st[j + 1], stlo[j + 1], sw[j + 1], v0, va);
+        const double t = srt[at.rule + at.i], w = srw[at.rule + at.i];
+        cd wy;
+        if (at.type == SEG_LINE) {
+          const cd la = thread_waypoint(geo, at.k), lb = thread_waypoint(geo, at.k + 1);
+          line_node(la, cd{__dadd_rn(lb.re, -la.re), __dadd_rn(lb.im, -la.im)}, t, w, &y, &wy);
+        } else {
+          arc_node(geo.R, geo.tau, t, w, &y, &wy);
         }
-        if (j < a.n_pairs) direct_step(z.re_hi, z.re_lo, z.im2, st[j], stlo[j], sw[j], u0, ua);
-        u0 += v0;
-        ua += va;
-        const cd C = {ua, -z.im * u0};                   // sum_j w_j/(zeta - t_j)
-        const cd zt = {z.re_hi, z.im};
-        cd Pz = pi[NA - 1], h = {mu[0], 0.0}, qs = cmul(pi[1], h);
-#pragma unroll
-        for (int q = NA - 2; q >= 0; --q) Pz = cadd(cmul(Pz, zt), pi[q]);
-#pragma unroll
-        for (int q = 2; q < NA; ++q) {                   // h_q = sum_{b<q} mu_b zeta^(q-1-b)
-          h = cmul(h, zt);
-          h.re += mu[q - 1];
-          qs = cadd(qs, cmul(pi[q], h));
-        }
-        const cd PC = cmul(Pz, C);
-        s = {PC.re - qs.re, PC.im - qs.im};
+        if (geo.mirror) { y.im = -y.im; wy.im = -wy.im; }
+        q4 = cscale(cinv_fast(y), 0.25);
+        base = cscale(cmul(wy, y), a.c0);
       }
-      cd xn = xi;
+      W = cmul(cmul(base, line_k_complex(a, y)), q4);   // c0 wy y D1(y)/(4y)
+    }
+    const cd xq = cmul(xinv, q4);                       // 1/(4 x y)
 #pragma unroll
-      for (int q = 1; q < N; ++q) xn = cmul(xn, xi);     // xi^n
-      const cd term = cmul(cmul(cd{prv.x, prv.y}, xn), s);
+    for (int r = 0; r < NT; ++r) {
+      const cd c = y_plus_mu(y, a.term[r]);
+      const cd ic = cinv_fast(c);
+      cd Wr;
+      if (table) {   // the tables keep pref = c0 Wr y D1 (-R_r/(y + mu_r)):  W R_r/(4y) = -pref (y + mu_r)/(4y)
+        const double2 p2 = tpref[r * tstride + at.i];
+        Wr = cmul(cmul(cd{-p2.x, -p2.y}, c), q4);
+      } else {
+        Wr = NT == 1 ? W : cmul(W, cd{a.term[r].R_re, a.term[r].R_im});
+      }
+      const cd xi = cmul(x, ic);
+      const cd kap = cscale(cmul(y, ic), 4.0);
+      const cd xm = {x.re + a.term[r].mu_re, x.im + a.term[r].mu_im};
+      const cd A = {xm.re + y.re, xm.im + y.im};
+      const cd zeta = cmul(csqr(A), xq);
+      const cd term = cmul(Wr, taylor_node<N>(T, x, y, xi, kap, zeta, a.term[r]));
       g_re += term.re;
       g_im += term.im;
     }
@@ -324,6 +429,8 @@ int launch_taylor_n(const EvalArgs& a, const LaunchPlan& plan, const double* blo
     kern<<<(unsigned)plan.grid_blocks, plan.block_threads, plan.smem_bytes, stream>>>(a, plan.layout, blob);
     return check_cuda(cudaGetLastError(), "taylor kernel launch");
   };
+  if (!plan.shared_nodes)   // a point-dependent contour
+    return a.n_terms == 1 ? launch(eval_taylor_contour_kernel<N, 1>) : launch(eval_taylor_contour_kernel<N, 2>);
   return a.n_terms == 1 ? launch(eval_taylor_kernel<N, 1>) : launch(eval_taylor_kernel<N, 2>);
 }
 

@@ -1102,8 +1102,83 @@ def test_taylor_order_reaches_the_closed_form_and_refuses_the_rest(gf):
         assert relerr(g, ref).max() < 3e-12
     x = torch.from_numpy(xs).cuda()
     rnp, rwp = gf.make_radial_tables("auto", 256, W.RADIAL_RULE)
-    for kw, tabs in ((dict(taylor_order=5), (rn, rw)), (dict(taylor_order=-1), (rn, rw)), (dict(taylor_order=1, contour="auto"), (rnp, rwp)),
+    for kw, tabs in ((dict(taylor_order=5), (rn, rw)), (dict(taylor_order=-1), (rn, rw)), (dict(taylor_order=5, contour="auto"), (rnp, rwp)),
                      (dict(taylor_order=1, routing="symmetric"), (rn, rw)), (dict(taylor_order=1, precision=32), (rn, rw))):
         with pytest.raises(gf.GfError) as e:
             gf.eval_grid(gf.make_params(bub, bub, 1e6, **kw), tabs[0], tabs[1], 256, z, wz, x)
         assert e.value.status == 3, kw
+
+
+@pytest.mark.parametrize("contour,over", [
+    ("ray_arc", {}), ("auto", {}),
+    ("thread", {"re": (-5.0, -4.2), "im": (-0.5, 0.5)}),
+])
+@pytest.mark.parametrize("n", [1, 2])
+def test_taylor_order_on_deformed_contours(gf, oracle, contour, over, n):
+    """(1 - t^n) F on the point-dependent contours (Step 2 and Step 3 of the paper together): config
+    1's orders, every point of its grid (THREAD: of the part of the plane it is made for), 1e-11 against the oracle."""
+    cfg = dict(W.CONFIGS["cfg1_tiny"])
+    cfg.update(over)
+    P = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
+                       contour=contour, taylor_order=n)
+    Po = oracle.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
+                            contour=contour, taylor_order=n)
+    _, rn, rw, z, wz = gpu_setup(gf, cfg, contour=contour)
+    _, rno, rwo, zo, wzo = oracle_setup(oracle, cfg, contour=contour)
+    x = gpu_grid(gf, cfg)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
+    xs = oracle_grid(oracle, cfg)
+    ref, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, xs, accum="extended")
+    # bound relative to the largest of |G_0| .. |G_n| (DESIGN.md "Tolerances"): on a deformed contour the nodes of the
+    # ray cancel in G_n at small |x| (the oracle's own double-term variant is 2.7e-11 off at x = -0.048 - 0.032i, n = 2)
+    scale = np.abs(ref)
+    for lower in range(n):
+        Pl = oracle.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=W.PREFACTOR, map_scale=W.MAP_SCALE,
+                                contour=contour, taylor_order=lower)
+        gl, _ = oracle.eval_grid(Pl, rno, rwo, cfg["n_rad"], zo, wzo, xs, accum="extended")
+        scale = np.maximum(scale, np.abs(gl))
+    e = np.abs(g - ref) / np.where(scale == 0, 1.0, scale)
+    assert e.max() <= TOL64, (contour, n, e.max(), xs.ravel()[e.argmax()])
+    assert np.quantile(relerr(g, ref), 0.99) <= TOL64      # and plainly relative at all but the worst-conditioned points
+
+
+def test_taylor_order_on_deformed_contours_other_lines_and_the_continuation(gf, oracle):
+    """Rational and complex-mass lines under AUTO with n = 1 (parity), lane splits and the host path; and the point of
+    it: outside the parabola, where the REAL contour is not the continuation, RAY_ARC with n = 1 reaches the closed
+    form CF1 + x/(6 m^2)."""
+    from tests import closed_forms as CF
+    bub = {"kind": "massive", "m2": 1.0}
+    rat = {"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2}
+    cfg = W.CONFIGS["cfg1_tiny"]
+    n_rad, n_ang = 64, 48
+    rn, rw = gf.make_radial_tables("auto", n_rad, W.RADIAL_RULE)
+    z, wz = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    rno, rwo = oracle.make_radial_pyramid(n_rad, levels=4)
+    zo, wzo = oracle.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    xs = oracle_grid(oracle, cfg)[::2, ::2].ravel()
+    for lk, lp in ((bub, rat), ({"kind": "massive", "m2": 0.5j}, {"kind": "massive", "m2": -0.5j}), (rat, bub)):
+        P = gf.make_params(lk, lp, 1e5, contour="auto", taylor_order=1)
+        Po = oracle.make_params(lk, lp, 1e5, contour="auto", taylor_order=1)
+        ref, _ = oracle.eval_grid(Po, rno, rwo, n_rad, zo, wzo, xs, accum="extended")
+        for n_points in (xs.size, 33, 1):
+            g = gf.eval_grid(P, rn, rw, n_rad, z, wz, torch.from_numpy(xs[:n_points].copy()).cuda()).cpu().numpy()
+            e = relerr(g, ref[:n_points])
+            assert e.max() <= TOL64, (lk, lp, n_points, e.max(), xs[e.argmax()])
+    rnh, rwh = gf.make_radial_tables_host("auto", n_rad, W.RADIAL_RULE)
+    zh, wzh = gf.make_quadrature_host(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    out = np.empty(xs.size, dtype=np.complex128)
+    gf.eval_grid_host(P, rnh, rwh, n_rad, zh, wzh, xs, out)
+    assert relerr(out, ref).max() <= TOL64
+    # the continuation: points outside the parabola Re x > (Im x)^2/4 - 1
+    import mpmath as mp
+    rn, rw = gf.make_radial_tables("ray_arc", 256, W.RADIAL_RULE)
+    z, wz = gf.make_quadrature("gauss_cheb2", 128, measure="sqrt1mz2")
+    pts = np.array([2 - 4j, -3 + 2j, -8 + 4j])
+    g = gf.eval_grid(gf.make_params(bub, bub, 1e6, contour="ray_arc", taylor_order=1), rn, rw, 256, z, wz,
+                     torch.from_numpy(pts).cuda()).cpu().numpy()
+    with mp.workdps(30):
+        ref = [complex(CF.cf1(v) + mp.mpc(v) / 6) for v in pts]
+    assert relerr(g, ref).max() < 1e-9
+    rnr, rwr = gf.make_radial_tables("real", 256, W.RADIAL_RULE)
+    gr = gf.eval_grid(gf.make_params(bub, bub, 1e6, taylor_order=1), rnr, rwr, 256, z, wz, torch.from_numpy(pts).cuda()).cpu().numpy()
+    assert relerr(gr, ref).min() > 1e-3
