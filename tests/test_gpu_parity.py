@@ -974,6 +974,39 @@ def test_random_parameter_sets_taylor(gf, oracle):
           % (worst, worst_at, plain))
 
 
+def test_random_parameter_sets_taylor_contours(gf, oracle):
+    """Seeded random problems with a Taylor order 1..2 on RAY_ARC / AUTO: the bound of test_random_parameter_sets_taylor
+    (1e-11 of the largest of |G_0| .. |G_n|)."""
+    rng = np.random.default_rng(W.PARITY_SEED + 4)
+    worst, worst_at = 0.0, None
+    for trial in range(120):
+        contour = ["ray_arc", "auto"][trial % 2]
+        lk, lpk = _random_lines(rng, int(rng.integers(0, 6)))
+        order = int(rng.integers(1, 3))
+        cutoff2, s0 = 10 ** rng.uniform(2, 8), 10 ** rng.uniform(-2, 1)
+        n_rad, n_ang = int(rng.choice([16, 64, 128])), int(rng.choice([17, 32, 64, 129]))
+        ang = str(rng.choice(["gauss_legendre", "gauss_cheb2", "tanh_sinh"]))
+        n = int(rng.choice([1, 5, 33, 200]))
+        xs = (rng.normal(size=n) + 1j * rng.normal(size=n)) * 10 ** rng.uniform(-3, 2.5)
+        rn, rw = gf.make_radial_tables(contour, n_rad)
+        z, wz = gf.make_quadrature(ang, n_ang, measure="sqrt1mz2")
+        rno, rwo = oracle.make_radial_pyramid(n_rad, levels=4)
+        zo, wzo = oracle.make_quadrature(ang, n_ang, measure="sqrt1mz2")
+        P = gf.make_params(lk, lpk, cutoff2, map_scale=s0, taylor_order=order, contour=contour)
+        g = gf.eval_grid(P, rn, rw, n_rad, z, wz, torch.from_numpy(xs).cuda()).cpu().numpy()
+        scale, ref = None, None
+        for o in range(order + 1):
+            Po = oracle.make_params(lk, lpk, cutoff2, map_scale=s0, taylor_order=o, contour=contour)
+            ref, _ = oracle.eval_grid(Po, rno, rwo, n_rad, zo, wzo, xs, accum="extended")
+            scale = np.abs(ref) if scale is None else np.maximum(scale, np.abs(ref))
+        ok = np.isfinite(ref)
+        e = (np.abs(g - ref) / np.where(scale == 0, 1.0, scale))[ok]
+        if e.size and e.max() > worst:
+            worst, worst_at = e.max(), (trial, contour, order, lk, lpk, cutoff2, s0, n_rad, n_ang, ang, xs[ok][e.argmax()])
+        assert e.size == 0 or e.max() <= TOL64, "%r" % ((e.max(), trial, contour, order, lk, lpk, cutoff2, s0, n_rad, n_ang, ang, xs[ok][e.argmax()]),)
+    print("worst error over 120 random Taylor-order problems on deformed contours: %.2e of max(|G_0|..|G_n|) at %s" % (worst, worst_at))
+
+
 # ------------------------------------------------------------------ Taylor subtraction of order n > 0 (eq. (12),(13))
 def _taylor_pair(gf, oracle, lk, lp, cutoff2, n, **kw):
     return (gf.make_params(lk, lp, cutoff2, taylor_order=n, **kw), oracle.make_params(lk, lp, cutoff2, taylor_order=n, **kw))
