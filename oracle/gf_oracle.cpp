@@ -395,7 +395,9 @@ double line2_scale(const Propagator& P) {
 
 // ---- contours (Step 3; the IF-THEN-ELSE of Kernel 2,
 //      PAPER.md:162,310).  DESIGN.md "Contour policies" states each one. -----
-struct RNode { cplx y; cplx wy; };  // node and (rule weight) x dy/dt
+// node, (rule weight) x dy/dt, and arg y continued along the contour from its start at y = 0 (used only for the
+// measure y^((d-2)/2) of d != 4: the branch of the power follows the contour, reading G21 of DESIGN.md)
+struct RNode { cplx y; cplx wy; double arg; };
 
 struct Rule { const double* t; const double* w; int n; };
 
@@ -421,15 +423,20 @@ void seg_logreal(double a, double b, double s0, cplx dir, Rule R, std::vector<RN
     double u = 0.5 * (R.t[i] + 1.0);
     double r = (double)((__float128)a + as * expm1q((__float128)u * L));
     double dr = (double)((__float128)(0.5 * R.w[i]) * L * ((__float128)r + (__float128)s0));
-    RNode nd = { dir * r, dir * dr };
+    RNode nd = { dir * r, dir * dr, std::atan2(dir.imag(), dir.real()) };   // a ray from 0: arg y = arg dir
     out.push_back(nd);
   }
 }
 
-void seg_line(cplx a, cplx b, Rule R, std::vector<RNode>& out) {
+// lower: the piece dips below the negative real axis (THREAD's pieces W2 -> W3 -> W4, which pass under the inward
+// tail of the cut): there arg y runs past pi, so a node with Im y < 0 has arg y = atan2 + 2 pi
+void seg_line(cplx a, cplx b, Rule R, std::vector<RNode>& out, bool lower = false) {
   for (int i = 0; i < R.n; ++i) {
     double u = 0.5 * (R.t[i] + 1.0);
-    RNode nd = { a + (b - a) * u, (b - a) * (0.5 * R.w[i]) };
+    cplx y = a + (b - a) * u;
+    double arg = std::atan2(y.imag(), y.real());
+    if (lower && y.imag() < 0) arg += 2.0 * (double)kPi;
+    RNode nd = { y, (b - a) * (0.5 * R.w[i]), arg };
     out.push_back(nd);
   }
 }
@@ -451,7 +458,7 @@ void seg_arc(double Rad, double tau, Rule R, std::vector<RNode>& out) {
     double Er = gr2 - gi2, Ei = 2.0 * (gr * gi);            // g^2
     double yr = Rad * Er, yi = Rad * Ei;
     double f = ((2.0 * tau) * R.w[i]) * in2;
-    RNode nd = { cplx(yr, yi), cplx(f * yi, -(f * yr)) };
+    RNode nd = { cplx(yr, yi), cplx(f * yi, -(f * yr)), 4.0 * std::atan(tv) };   // y = Rad g^2, arg g = 2 atan(tau v)
     out.push_back(nd);
   }
 }
@@ -549,13 +556,14 @@ void contour_thread(const Params& P, cplx x, const double* rn, const double* rw,
     W[5] = cplx(Rad * (gr2 - gi2), Rad * (2.0 * (gr * gi)));
   }
   size_t first = out.size();
-  for (int k = 0; k < 5; ++k) seg_line(W[k], W[k + 1], level(rn, rw, n_rad, 3), out);
+  for (int k = 0; k < 5; ++k) seg_line(W[k], W[k + 1], level(rn, rw, n_rad, 3), out, k == 2 || k == 3);
   seg_arc(Rad, kTau5, level(rn, rw, n_rad, 3), out);
   seg_logreal(Rad, P.cutoff2, P.map_scale, cplx(1, 0), level(rn, rw, n_rad, 2), out);
   if (mirror)
     for (size_t k = first; k < out.size(); ++k) {
       out[k].y = std::conj(out[k].y);
       out[k].wy = std::conj(out[k].wy);
+      out[k].arg = -out[k].arg;
     }
 }
 
@@ -645,9 +653,17 @@ cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int
       si += (ACC)((R)wz[j] * f.imag());
     }
     C S((R)sr, (R)si);
-    // dy y^((d-2)/2) (...): eq. (14) for d = 4; other d on the real contour only (y > 0, real power)
-    C term = (P.dim == 0 || P.dim == 4) ? wy * y * S
-                                          : wy * C((R)powq((__float128)nodes[i].y.real(), (__float128)(0.5 * (P.dim - 2))), (R)0) * S;
+    // dy y^((d-2)/2) (...): eq. (14) for d = 4; otherwise the power on the branch continued along the contour from
+    // y = 0: |y|^p e^(i p arg y) with the node's continued argument (p real; on the real axis arg = 0)
+    C term;
+    if (P.dim == 0 || P.dim == 4) {
+      term = wy * y * S;
+    } else {
+      const __float128 p = 0.5 * ((__float128)P.dim - 2);
+      const __float128 mag = powq(hypotq((__float128)nodes[i].y.real(), (__float128)nodes[i].y.imag()), p);
+      const __float128 ang = p * (__float128)nodes[i].arg;
+      term = wy * C((R)(mag * cosq(ang)), (R)(mag * sinq(ang))) * S;
+    }
     gr += (ACC)term.real();
     gi += (ACC)term.imag();
   }
@@ -751,7 +767,6 @@ int check_params(const Params& P, int n_rad, int n_ang) {
                           P.line_k.m2_re == P.line_pk.m2_re && P.line_k.m2_im == P.line_pk.m2_im))
     return 3;
   if (!(P.dim == 0 || (P.dim >= 1 && P.dim <= 8))) return 2;
-  if (!(P.dim == 0 || P.dim == 4) && P.contour != CONTOUR_REAL) return 3;
   return 0;
 }
 

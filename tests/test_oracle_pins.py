@@ -626,12 +626,42 @@ def test_dimension_3_bubble_closed_form(oracle):
     assert relerr(g4, ref).min() > 0.1
 
 
+def test_dimension_3_on_the_deformed_contours(oracle):
+    """y^((d-2)/2) at complex y, on the branch continued along the contour from y = 0 (reading G21): with it RAY_ARC and
+    AUTO reach the d = 3 closed form outside the parabola where the REAL contour is off by 20-180 %, and THREAD reaches
+    it below -4 m^2 next to the cut, where its pieces W2 -> W3 -> W4 dip under the negative real axis and arg y runs
+    past pi (a principal-branch power there flips the sign of those pieces: O(1) error).  Catches a wrong branch, a
+    missing power on a piece, the d = 4 measure left in a table."""
+    z, wz = oracle.make_quadrature("gauss_legendre", 64, measure="plain")
+    c0 = 1 / (8 * np.pi ** 2)
+    xs = np.array([2 - 4j, -3 + 2j, 0.5 + 0.2j, -0.5 + 0.3j])
+    ref = np.array([complex(CF.bubble_d3(x)) for x in xs])
+    rn, rw = oracle.make_radial_pyramid(512, levels=4)
+    for contour in ("ray_arc", "auto"):
+        g, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e8, prefactor=c0, dim=3.0, contour=contour), rn, rw, 512, z, wz, xs)
+        assert relerr(g, ref).max() < 1e-6, (contour, relerr(g, ref))
+    g, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e8, prefactor=c0, dim=3.0), rn, rw, 512, z, wz, xs[:2])
+    assert relerr(g, ref[:2]).min() > 0.1                      # REAL is not the continuation there
+    zt, wzt = oracle.make_quadrature("gauss_legendre", 256, measure="plain")
+    xt = np.array([-6 + 1j, -6 - 1j, -8 + 0.5j])
+    reft = np.array([complex(CF.bubble_d3(x)) for x in xt])
+    gt, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e8, prefactor=c0, dim=3.0, contour="thread"), rn, rw, 512, zt, wzt, xt)
+    assert relerr(gt, reft).max() < 2e-3, relerr(gt, reft)
+    assert np.allclose(gt[1], np.conj(gt[0]), rtol=1e-13)
+    # d = 5 (p = 3/2): no closed form at hand; the contour must not matter where both are the continuation
+    P5r = oracle.make_params(BUB, BUB, 1e6, prefactor=c0, dim=5.0, taylor_order=1)
+    P5c = oracle.make_params(BUB, BUB, 1e6, prefactor=c0, dim=5.0, taylor_order=1, contour="ray_arc")
+    z5, wz5 = oracle.make_quadrature_dim("gauss_legendre", 128, 5.0)
+    xin = np.array([0.5 + 0.2j, 1.0 + 0.5j])
+    a, _ = oracle.eval_grid(P5r, rn, rw, 512, z5, wz5, xin)
+    b, _ = oracle.eval_grid(P5c, rn, rw, 512, z5, wz5, xin)
+    assert relerr(b, a).max() < 1e-4, relerr(b, a)
+
+
 def test_dimension_argument_checks(oracle):
     rn, rw, z, wz = tables(oracle, 64, 32)
     with pytest.raises(ValueError):
         oracle.eval_grid(oracle.make_params(BUB, BUB, 1e4, dim=0.5), rn, rw, 64, z, wz, np.array([1.0]))
-    with pytest.raises(ValueError):   # other dimensions on the real contour only (y^((d-2)/2) needs y > 0)
-        oracle.eval_grid(oracle.make_params(BUB, BUB, 1e4, dim=3.0, contour="ray_arc"), rn, rw, 64, z, wz, np.array([1.0]))
     g4, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e4, dim=4.0), rn, rw, 64, z, wz, np.array([1.0 + 1j]))
     g0, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e4, dim=0.0), rn, rw, 64, z, wz, np.array([1.0 + 1j]))
     assert g4[0] == g0[0]
