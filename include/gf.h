@@ -29,7 +29,7 @@
  *   - Errors: GF_ERR_NULL for a null pointer, GF_ERR_ARG for a value out of range,
  *     GF_ERR_UNSUPPORTED for a combination the method does not define or that is not built (taylor_order outside
  *     [0, 4], taylor_order > 0 with the symmetric routing or with precision 32, a
- *     subtraction point other than 0, a dimension other than 4 or the symmetric routing on a
+ *     subtraction point other than 0, the symmetric routing on a
  *     deformed contour, the symmetric routing with unequal or rational lines, the THREAD contour
  *     with unequal or complex masses, a rational propagator with a double pole, precision 32 on a
  *     contour other than REAL), GF_ERR_CUDA when the CUDA runtime reports an error (no device,
@@ -138,7 +138,9 @@ typedef struct {
                             trivial modifications"): the radial measure becomes dy y^((d-2)/2); the angular measure
                             (1-z^2)^((d-3)/2) is the caller's, in the angular weights (gf_make_quadrature_dim makes them;
                             GF_MEASURE_PLAIN is d = 3).
-                            d != 4 on the REAL contour only.  Constants of the d-dimensional measure go into
+                            On a deformed contour y^((d-2)/2) is taken on the branch continued along the contour
+                            from y = 0 (|y|^p e^(i p arg y), arg y = arg x on the ray, running past pi on THREAD's
+                            pieces under the negative real axis).  Constants of the d-dimensional measure go into
                             `prefactor` (d^dk = 1/2 y^((d-2)/2) dy dOmega_d). */
 } gf_params;
 

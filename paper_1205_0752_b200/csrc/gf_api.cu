@@ -217,7 +217,6 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
     return GF_ERR_UNSUPPORTED;
   }
   if (!(p->dim == 0 || (p->dim >= 1 && p->dim <= 8))) { set_error("eval_grid: dim=%g outside [1, 8] (0 = 4)", p->dim); return GF_ERR_ARG; }
-  if (!(p->dim == 0 || p->dim == 4) && p->contour != GF_CONTOUR_REAL) { set_error("eval_grid: a dimension other than 4 is supported on the REAL contour only"); return GF_ERR_UNSUPPORTED; }
   if (p->contour != GF_CONTOUR_REAL && n_rad % 8 != 0) { set_error("eval_grid: deformed contours need n_rad %% 8 == 0"); return GF_ERR_ARG; }
 
   *a = EvalArgs{};

@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(256) prep_rungs_kernel(const __grid_constant__
     const double dr = dd_mul(dd_mul_d(L1, 0.5 * w), two_sum(r, a.s0)).hi;
     row[L.rg_r + i] = r;
     row[L.rg_q4 + i] = 0.25 / r;
-    row[L.rg_w + i] = a.c0 * r * dr;
+    row[L.rg_w + i] = a.c0 * (a.ypow == 1.0 ? r : pow(r, a.ypow)) * dr;   // c0 r^p dr, p = (d-2)/2
   }
   // real tail: y(u) = R + (R + s0) expm1(u L), L = ln((Lambda^2 + s0)/(R + s0))      (level 2)
   const dd as = two_sum(R, a.s0);
@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(256) prep_rungs_kernel(const __grid_constant__
     const double dy = dd_mul(dd_mul_d(L2, 0.5 * w), two_sum(y, a.s0)).hi;
     row[L.rg_y + i] = y;
     row[L.rg_yq4 + i] = 0.25 / y;
-    const cd d1 = cscale(line_k_real(a.line_k, y), a.c0 * dy * y);
+    const cd d1 = cscale(line_k_real(a.line_k, y), a.c0 * dy * (a.ypow == 1.0 ? y : pow(y, a.ypow)));
     for (int r = 0; r < a.n_terms; ++r) {
       const cd ic = cinv(cd{y + a.term[r].mu_re, a.term[r].mu_im});
       const cd pr = cmul(cmul(d1, cd{-a.term[r].R_re, -a.term[r].R_im}), ic);
@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
   const cd xinv = cinv(x);
 
   const Geo geo = build_geo(a, x.re, x.im);
-  const cd dir2 = {fma(geo.dre, geo.dre, -(geo.dim * geo.dim)), 2.0 * geo.dre * geo.dim};
+  const cd dir2 = ray_measure_dir(a, geo);   // dir^2 in d = 4
   // One pole (NT == 1): on a piece y = dir r with real r from a table (the ray; dir = 1 on the real pieces)
   //   zeta = (x + mu + y)^2/(4 x y) = Z1/(4r) + C2 + Z3 r,  Z1 = (x + mu)^2/x conj(dir), C2 = (x + mu)/(2x), Z3 = dir/(4x)
   //   delta = (x + mu)/(4y) = Dc/(4r),  Dc = (x + mu) conj(dir)
@@ -221,9 +221,9 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
       } else {
         arc_node(geo.R, geo.tau, t, w, &y, &wy);
       }
-      if (geo.mirror) { y.im = -y.im; wy.im = -wy.im; }
+      base = measure_base(a, geo, at.type, at.k, t, y, wy);
+      if (geo.mirror) { y.im = -y.im; wy.im = -wy.im; base.im = -base.im; }
       q4 = cscale(cinv_fast(y), 0.25);
-      base = cscale(cmul(wy, y), a.c0);
     }
     const bool affine = NT == 1 && affine_ok && (table || at.type == SEG_RAY);
     cd xq = {0.0, 0.0};

@@ -203,6 +203,36 @@ __device__ __forceinline__ void arc_node(double R, double tau, double t, double 
 __device__ __forceinline__ cd y_plus_mu(cd y, const PoleTerm& t) {
   return {(y.re + t.mu_re) + t.mu_re_lo, (y.im + t.mu_im) + t.mu_im_lo};
 }
+// Other dimensions (gf_params.dim): the radial measure y^p, p = (d-2)/2, at complex y, on the branch continued along the
+// contour from y = 0 (reading G21): |y|^p e^(i p arg y) with the continued argument of the node --
+// arg dir on the ray, 4 atan(tau v) on an arc, atan2 on a straight piece, plus 2 pi below the negative real axis on
+// THREAD's pieces W2 -> W3 -> W4 (which pass under the inward tail of the cut), negated for the mirrored contour.
+__device__ __forceinline__ cd cpow_arg(cd y, double arg, double p) {
+  const double mag = exp(0.5 * p * log(fma(y.re, y.re, y.im * y.im)));
+  double sn, cs;
+  sincos(p * arg, &sn, &cs);
+  return {mag * cs, mag * sn};
+}
+// c0 (rule weight x dy/dt) y^p for a node of a straight piece (k: THREAD's piece) or of an arc, before mirroring
+__device__ __forceinline__ cd measure_base(const EvalArgs& a, const Geo& geo, int seg_type, int k, double t, cd y, cd wy) {
+  if (a.ypow == 1.0) return cscale(cmul(wy, y), a.c0);
+  double arg;
+  if (seg_type == SEG_ARC) {
+    arg = 4.0 * atan(geo.tau * (1.0 - 0.5 * (t + 1.0)));
+  } else {
+    arg = atan2(y.im, y.re);
+    if ((k == 2 || k == 3) && y.im < 0.0) arg += 6.283185307179586476925;
+  }
+  return cscale(cmul(wy, cpow_arg(y, arg, a.ypow)), a.c0);
+}
+// the direction factor of the ray's nodes: dy y^p = dir^(p+1) r^p dr
+__device__ __forceinline__ cd ray_measure_dir(const EvalArgs& a, const Geo& geo) {
+  if (a.ypow == 1.0) return {fma(geo.dre, geo.dre, -(geo.dim * geo.dim)), 2.0 * geo.dre * geo.dim};
+  double sn, cs;
+  sincos((a.ypow + 1.0) * atan2(geo.dim, geo.dre), &sn, &cs);
+  return {cs, sn};
+}
+
 // D1(y) for complex y; a rational line through its factored denominator (y + nu_1)(y + nu_2), which stays accurate
 // where the contour passes next to a root
 __device__ __forceinline__ cd line_k_complex(const EvalArgs& a, cd y) {

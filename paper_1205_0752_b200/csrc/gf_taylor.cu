@@ -315,7 +315,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
   }
   const cd xinv = cinv(x);
   const Geo geo = build_geo(a, x.re, x.im);
-  const cd dir2 = {fma(geo.dre, geo.dre, -(geo.dim * geo.dim)), 2.0 * geo.dre * geo.dim};
+  const cd dir2 = ray_measure_dir(a, geo);   // dir^2 in d = 4
   const double* row = blob + L.off_rung + (long long)geo.row * L.rung_stride;
   const bool real_pol = geo.pol == GF_CONTOUR_REAL;
   const double* ty = real_pol ? blob + L.off_y : row + L.rg_y;
@@ -348,9 +348,9 @@ __global__ void __launch_bounds__(kBlockThreads, 2)
         } else {
           arc_node(geo.R, geo.tau, t, w, &y, &wy);
         }
-        if (geo.mirror) { y.im = -y.im; wy.im = -wy.im; }
+        base = measure_base(a, geo, at.type, at.k, t, y, wy);
+        if (geo.mirror) { y.im = -y.im; wy.im = -wy.im; base.im = -base.im; }
         q4 = cscale(cinv_fast(y), 0.25);
-        base = cscale(cmul(wy, y), a.c0);
       }
       W = cmul(cmul(base, line_k_complex(a, y)), q4);   // c0 wy y D1(y)/(4y)
     }

@@ -722,11 +722,50 @@ def test_other_dimensions(gf, oracle, dim, measure):
     g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x).cpu().numpy()
     ref, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, oracle_grid(oracle, cfg), accum="extended")
     assert relerr(g, ref).max() <= TOL64
-    Pd = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], contour="auto", dim=dim)
-    rnp, rwp = gf.make_radial_tables("auto", cfg["n_rad"], W.RADIAL_RULE)
-    with pytest.raises(gf.GfError) as e:
-        gf.eval_grid(Pd, rnp, rwp, cfg["n_rad"], z, wz, x)
-    assert e.value.status == 3
+
+
+@pytest.mark.parametrize("contour,over", [
+    ("ray_arc", {}), ("auto", {}),
+    ("thread", {"re": (-5.0, -4.2), "im": (-0.5, 0.5)}),
+])
+@pytest.mark.parametrize("dim,order", [(3.0, 0), (3.5, 0), (5.0, 1), (2.0, 0)])
+def test_other_dimensions_on_deformed_contours(gf, oracle, contour, over, dim, order):
+    """y^((d-2)/2) at complex y on the branch continued along the contour (reading G21; PAPER.md:41 with Step 3): config
+    1's orders, every point, every policy, order 0 and (d = 5) order 1.  The power is a smooth factor of the node
+    weight: each side takes it with its own libm."""
+    cfg = dict(W.CONFIGS["cfg1_tiny"])
+    cfg.update(over)
+    c0 = 1 / (8 * np.pi ** 2)
+    kw = dict(prefactor=c0, dim=dim, contour=contour, taylor_order=order)
+    P = gf.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], **kw)
+    Po = oracle.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], **kw)
+    rn, rw = gf.make_radial_tables(contour, cfg["n_rad"], W.RADIAL_RULE)
+    z, wz = gf.make_quadrature_dim(W.ANGULAR_RULE, cfg["n_ang"], dim)
+    rno, rwo = oracle.make_radial_pyramid(cfg["n_rad"], levels=4)
+    zo, wzo = oracle.make_quadrature_dim(W.ANGULAR_RULE, cfg["n_ang"], dim)
+    g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, gpu_grid(gf, cfg)).cpu().numpy()
+    xs = oracle_grid(oracle, cfg)
+    ref, _ = oracle.eval_grid(Po, rno, rwo, cfg["n_rad"], zo, wzo, xs, accum="extended")
+    scale = np.abs(ref)
+    if order:   # Taylor order: bound relative to the largest of |G_0| .. |G_n| (DESIGN.md "Tolerances")
+        P0 = oracle.make_params(cfg["line_k"], cfg["line_pk"], cfg["cutoff2"], prefactor=c0, dim=dim, contour=contour)
+        g0, _ = oracle.eval_grid(P0, rno, rwo, cfg["n_rad"], zo, wzo, xs, accum="extended")
+        scale = np.maximum(scale, np.abs(g0))
+    e = np.abs(g - ref) / np.where(scale == 0, 1.0, scale)
+    assert e.max() <= TOL64, (contour, dim, e.max(), xs.ravel()[e.argmax()])
+
+
+def test_dimension_3_reaches_the_closed_form_on_ray_arc(gf):
+    """d = 3 outside the parabola: arctan(sqrt(x)/2m)/(4 pi sqrt x) - 1/(8 pi m) through RAY_ARC on the GPU."""
+    from tests import closed_forms as CF
+    bub = {"kind": "massive", "m2": 1.0}
+    xs = np.array([2 - 4j, -3 + 2j, 0.5 + 0.2j])
+    ref = np.array([complex(CF.bubble_d3(v)) for v in xs])
+    rn, rw = gf.make_radial_tables("ray_arc", 512, W.RADIAL_RULE)
+    z, wz = gf.make_quadrature_dim("gauss_legendre", 64, 3.0)
+    g = gf.eval_grid(gf.make_params(bub, bub, 1e8, prefactor=1 / (8 * np.pi ** 2), dim=3.0, contour="ray_arc"), rn, rw, 512, z, wz,
+                     torch.from_numpy(xs).cuda()).cpu().numpy()
+    assert relerr(g, ref).max() < 1e-6
 
 
 # ------------------------------------------------------------------ symmetric momentum routing (SURVEY 8(f) item 1)
