@@ -611,6 +611,20 @@ int auto_policy(const Params& P, cplx x, int n_rad, int n_ang) {
   return CONTOUR_REAL;
 }
 
+// The contour of the point x under the policy of P.  Symmetric routing (lines k + p/2, k - p/2): the zeros of the
+// denominators are (y + x/4 + m^2)^2 = x y z^2, i.e. the cut of the paper's routing at the external momentum x/4
+// (zeta(x/4, y, m^2) in [0,1]), and the pole of the subtracted term sits at y = -m^2 as before: the policies are applied
+// to x/4 (region tests, contour radius, direction and waypoints) and the integrand is taken at x.
+int build_contour(const Params& P, cplx x, const double* rn, const double* rw, int n_rad, int n_ang,
+                  std::vector<RNode>& nodes) {
+  cplx xg = P.routing == 1 ? cplx(0.25 * x.real(), 0.25 * x.imag()) : x;
+  int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, xg, n_rad, n_ang) : P.contour;
+  if (pol == CONTOUR_REAL) contour_real(P, rn, rw, n_rad, nodes);
+  else if (pol == CONTOUR_RAY_ARC) contour_ray_arc(P, xg, rn, rw, n_rad, nodes);
+  else contour_thread(P, xg, rn, rw, n_rad, nodes);
+  return pol;
+}
+
 // principal square root in the term type (libstdc++ has no std::sqrt for complex<__float128>)
 template <typename R>
 std::complex<R> psqrt(std::complex<R> v) { return std::sqrt(v); }
@@ -630,10 +644,7 @@ cplx eval_point(const Params& P, cplx x, const double* rn, const double* rw, int
                 const double* z, const double* wz, int n_ang, std::vector<RNode>& nodes) {
   typedef std::complex<R> C;
   nodes.clear();
-  int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, x, n_rad, n_ang) : P.contour;
-  if (pol == CONTOUR_REAL) contour_real(P, rn, rw, n_rad, nodes);
-  else if (pol == CONTOUR_RAY_ARC) contour_ray_arc(P, x, rn, rw, n_rad, nodes);
-  else contour_thread(P, x, rn, rw, n_rad, nodes);
+  build_contour(P, x, rn, rw, n_rad, n_ang, nodes);
 
   C xx((R)x.real(), (R)x.imag());
   C sx = psqrt<R>(xx);  // principal branch
@@ -763,7 +774,7 @@ int check_params(const Params& P, int n_rad, int n_ang) {
   if (P.contour != CONTOUR_REAL && n_rad % 8 != 0) return 2;
   if (P.contour == CONTOUR_THREAD && !thread_applicable(P)) return 3;
   if (P.routing != 0 && P.routing != 1) return 2;
-  if (P.routing == 1 && !(P.contour == CONTOUR_REAL && P.line_k.kind == PROP_MASSIVE && P.line_pk.kind == PROP_MASSIVE &&
+  if (P.routing == 1 && !(P.line_k.kind == PROP_MASSIVE && P.line_pk.kind == PROP_MASSIVE &&
                           P.line_k.m2_re == P.line_pk.m2_re && P.line_k.m2_im == P.line_pk.m2_im))
     return 3;
   if (!(P.dim == 0 || (P.dim >= 1 && P.dim <= 8))) return 2;
@@ -850,10 +861,7 @@ int gfo_contour_nodes(const void* params, double x_re, double x_im, const double
   if (check_params(P, n_rad, n_ang)) return -1;
   cplx x(x_re, x_im);
   std::vector<RNode> nodes;
-  int pol = P.contour == CONTOUR_AUTO ? auto_policy(P, x, n_rad, n_ang) : P.contour;
-  if (pol == CONTOUR_REAL) contour_real(P, rad_nodes, rad_weights, n_rad, nodes);
-  else if (pol == CONTOUR_RAY_ARC) contour_ray_arc(P, x, rad_nodes, rad_weights, n_rad, nodes);
-  else contour_thread(P, x, rad_nodes, rad_weights, n_rad, nodes);
+  int pol = build_contour(P, x, rad_nodes, rad_weights, n_rad, n_ang, nodes);
   for (size_t i = 0; i < nodes.size(); ++i) {
     y[2 * i] = nodes[i].y.real(); y[2 * i + 1] = nodes[i].y.imag();
     wy[2 * i] = nodes[i].wy.real(); wy[2 * i + 1] = nodes[i].wy.imag();

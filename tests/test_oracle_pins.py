@@ -697,9 +697,36 @@ def test_symmetric_routing_reaches_the_threshold_parabola(oracle):
     assert np.array_equal(b, np.conj(a))
 
 
+def test_symmetric_routing_on_the_deformed_contours(oracle):
+    """The cut of the symmetric routing is the cut of the paper's routing at x/4 ((y + x/4 + m^2)^2 = x y z^2), so the
+    contour policies applied to x/4 continue it: RAY_ARC and AUTO reach CF1 outside the threshold parabola
+    Re x > (Im x)^2/16m^2 - 4m^2 where the REAL contour is off by 50 % and more; THREAD (for Re x/4 <= -4.1 m^2) gives
+    the discontinuity across the cut.  Catches contours built from x instead of x/4, a policy test on the wrong variable."""
+    rn, rw = oracle.make_radial_pyramid(512, levels=4)
+    z, wz = oracle.make_quadrature("gauss_cheb2", 256, measure="sqrt1mz2")
+    xs = np.array([0.5 + 0.2j, -3 + 0.5j, -8 + 4j, -6 + 1j, 2 - 9j, -20 + 12j])
+    ref = np.array([complex(CF.cf1(x)) for x in xs])
+    for contour in ("ray_arc", "auto"):
+        g, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e8, routing="symmetric", contour=contour), rn, rw, 512, z, wz, xs)
+        assert relerr(g, ref).max() < 1e-7, (contour, relerr(g, ref))
+    g, _ = oracle.eval_grid(oracle.make_params(BUB, BUB, 1e8, routing="symmetric"), rn, rw, 512, z, wz, xs[[2, 3, 5]])
+    assert relerr(g, ref[[2, 3, 5]]).min() > 0.3
+    # the policy is applied to x/4: the nodes of x under the symmetric routing are the nodes of x/4 under the paper's
+    Ps = oracle.make_params(BUB, BUB, 1e8, routing="symmetric", contour="auto")
+    Pp = oracle.make_params(BUB, BUB, 1e8, contour="auto")
+    for x in (-8 + 4j, -30 + 0.5j, 0.5 + 0.2j):
+        ps, ys, ws = oracle.contour_nodes(Ps, x, rn, rw, 512, 256)
+        pp, yp, wp = oracle.contour_nodes(Pp, x / 4, rn, rw, 512, 256)
+        assert ps == pp and np.array_equal(ys, yp) and np.array_equal(ws, wp)
+    # next to the cut below the threshold: THREAD through AUTO, Im G = -+ pi sqrt(1 - 4/s) within its accuracy
+    gp, gm = oracle.eval_grid(Ps, rn, rw, 512, z, wz, np.array([-30 + 0.05j, -30 - 0.05j]))[0]
+    disc = math.pi * math.sqrt(1 - 4 / 30)
+    assert abs(gp.imag / -disc - 1) < 0.2 and abs(gm.imag / disc - 1) < 0.2 and gm == np.conj(gp)
+
+
 def test_symmetric_routing_argument_checks(oracle):
     rn, rw, z, wz = tables(oracle, 64, 32)
-    for kw in (dict(line_pk={"kind": "massive", "m2": 2.0}), dict(line_pk=RAT), dict(contour="ray_arc")):
+    for kw in (dict(line_pk={"kind": "massive", "m2": 2.0}), dict(line_pk=RAT), dict(taylor_order=1)):
         args = dict(line_k=BUB, line_pk=BUB, cutoff2=1e4, routing="symmetric")
         args.update(kw)
         with pytest.raises(ValueError):
