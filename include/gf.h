@@ -29,8 +29,7 @@
  *   - Errors: GF_ERR_NULL for a null pointer, GF_ERR_ARG for a value out of range,
  *     GF_ERR_UNSUPPORTED for a combination the method does not define or that is not built (taylor_order outside
  *     [0, 4], taylor_order > 0 with the symmetric routing or with precision 32, a
- *     subtraction point other than 0, the symmetric routing on a
- *     deformed contour, the symmetric routing with unequal or rational lines, the THREAD contour
+ *     subtraction point other than 0, the symmetric routing with unequal or rational lines, the THREAD contour
  *     with unequal or complex masses, a rational propagator with a double pole, precision 32 on a
  *     contour other than REAL), GF_ERR_CUDA when the CUDA runtime reports an error (no device,
  *     launch failure).  gf_last_error() describes the last failure of the
@@ -131,9 +130,10 @@ typedef struct {
                             variant, complex<float> output */
   int routing;           /* 0: the paper's eq. (19), the lines carry k and p - k.  1: symmetric, the lines carry
                             k + p/2 and k - p/2 (the integral is shift invariant, eq. (4)): equal massive
-                            lines and the REAL contour only; G agrees up to O(x/Lambda^2), and REAL is the
+                            lines only, taylor_order 0; G agrees up to O(x/Lambda^2), and REAL is the
                             continuation inside the parabola through the threshold, Re x > (Im x)^2/(16 m^2) - 4 m^2,
-                            instead of Re x > (Im x)^2/(4 m^2) - m^2 */
+                            instead of Re x > (Im x)^2/(4 m^2) - m^2.  Its cut in the y-plane is the paper
+                            routing's at x/4, so the deformed contours (RAY_ARC, THREAD, AUTO) are those of x/4 */
   double dim;            /* space-time dimension d in [1, 8], 0 meaning 4 ("arbitrary dimensions by
                             trivial modifications"): the radial measure becomes dy y^((d-2)/2); the angular measure
                             (1-z^2)^((d-3)/2) is the caller's, in the angular weights (gf_make_quadrature_dim makes them;

@@ -211,9 +211,9 @@ int build_args(const gf_params* p, int n_rad, int n_ang, long long n_points, Eva
   }
   if (p->sub_re != 0 || p->sub_im != 0) { set_error("eval_grid: subtraction point must be 0 (eq. (13))"); return GF_ERR_UNSUPPORTED; }
   if (p->routing != 0 && p->routing != 1) { set_error("eval_grid: unknown routing %d", p->routing); return GF_ERR_ARG; }
-  if (p->routing == 1 && !(p->contour == GF_CONTOUR_REAL && p->line_k.kind == GF_PROP_MASSIVE && p->line_pk.kind == GF_PROP_MASSIVE &&
+  if (p->routing == 1 && !(p->line_k.kind == GF_PROP_MASSIVE && p->line_pk.kind == GF_PROP_MASSIVE &&
                            p->line_k.m2_re == p->line_pk.m2_re && p->line_k.m2_im == p->line_pk.m2_im)) {
-    set_error("eval_grid: symmetric routing needs two equal massive lines and the REAL contour");
+    set_error("eval_grid: symmetric routing needs two equal massive lines");
     return GF_ERR_UNSUPPORTED;
   }
   if (!(p->dim == 0 || (p->dim >= 1 && p->dim <= 8))) { set_error("eval_grid: dim=%g outside [1, 8] (0 = 4)", p->dim); return GF_ERR_ARG; }

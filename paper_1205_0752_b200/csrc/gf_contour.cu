@@ -135,6 +135,12 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
     x = {scalbn(x.re, k), scalbn(x.im, k)};
     out_scale = scalbn(1.0, -k);
   }
+  // Symmetric routing (lines k + p/2, k - p/2; equal massive lines): the folded sum is S(eta', zeta') with
+  // zeta' = zeta(x/4, y, mu) and eta' = 1/2 + (2 mu + x/4)/(4y), the node prefactor -c0 wy y/(y + mu)^2 as for equal masses,
+  // and the cut is the paper routing's at x/4: from here on x IS x/4 (geometry, policy, zeta); only delta differs.
+  const bool sym = a.routing == 1;
+  if (sym) x = cscale(x, 0.25);
+  const double d0 = sym ? 0.25 : 0.0, dmu = sym ? 2.0 : 1.0;   // delta = d0 + (x + dmu mu)/(4y)
   const cd xinv = cinv(x);
 
   const Geo geo = build_geo(a, x.re, x.im);
@@ -181,7 +187,7 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
       const int mid = (lo + hi) >> 1;
       if (ty[mid] < Y0) lo = mid + 1; else hi = mid;
     }
-    i_end = lo;
+    i_end = sym ? tn : lo;   // (the symmetric routing's tail needs a second table pair: its real nodes take routes)
   }
   const int g_end = t0 + i_end;
   const int g_stop = __reduce_max_sync(0xffffffffu, g_end);
@@ -234,7 +240,7 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
         const cd d = want ? cd{geo.dre, geo.dim} : cd{1.0, 0.0}, dc = {d.re, -d.im};
         Z1 = cmul(C1x4, dc);
         Z3 = cscale(cmul(xinv, d), 0.25);
-        Dc = cmul(cd{x.re + a.term[0].mu_re, x.im + a.term[0].mu_im}, dc);
+        Dc = cmul(cd{fma(dmu, a.term[0].mu_re, x.re), fma(dmu, a.term[0].mu_im, x.im)}, dc);
       }
     } else {
       xq = cmul(xinv, q4);                           // 1/(4 x y)
@@ -250,12 +256,13 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
       cd delta, zeta;
       if (affine) {
         const double q4r = table ? q4.re : row[L.rg_q4 + at.i], rr = table ? y.re : row[L.rg_r + at.i];
-        delta = {Dc.re * q4r, Dc.im * q4r};
+        delta = {fma(Dc.re, q4r, d0), Dc.im * q4r};
         zeta = {fma(Z1.re, q4r, fma(Z3.re, rr, C2.re)), fma(Z1.im, q4r, fma(Z3.im, rr, C2.im))};
       } else {
         const cd xm = {x.re + mur, x.im + mui};
         const cd A = {xm.re + y.re, xm.im + y.im};
-        delta = cmul(xm, q4);                        // eta - 1/4
+        delta = cmul(cd{fma(dmu, mur, x.re), fma(dmu, mui, x.im)}, q4);   // eta - 1/4
+        delta.re += d0;
         zeta = cmul(csqr(A), xq);
       }
       const cd s = node_term<double, COUNT, BLK>(tb, x, y, delta, zeta, mur, mui, rc, a.term[r].mu_re_lo, a.term[r].mu_im_lo);
@@ -309,7 +316,8 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
 __global__ void contour_nodes_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                                      const double* __restrict__ blob, double xr, double xi, int* __restrict__ policy,
                                      double2* __restrict__ out_y, double2* __restrict__ out_wy) {
-  const Geo geo = build_geo(a, xr, xi);
+  const double f = a.routing == 1 ? 0.25 : 1.0;   // symmetric routing: the contour of x/4 (exact scaling)
+  const Geo geo = build_geo(a, f * xr, f * xi);
   if (blockIdx.x == 0 && threadIdx.x == 0) *policy = geo.pol;
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= a.n_rad) return;

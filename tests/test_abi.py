@@ -107,7 +107,7 @@ def test_argument_errors_without_gpu(gf):
     for bad in (dict(cutoff2=1e61), dict(cutoff2=1e4, dim=9.0), dict(cutoff2=1e4, routing=2)):
         P = gf.make_params(bub, bub, **bad)
         assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 2, bad
-    for unsupported in (dict(routing="symmetric", contour="ray_arc"), dict(routing="symmetric", taylor_order=1)):
+    for unsupported in (dict(routing="symmetric", taylor_order=1), dict(taylor_order=1, precision=32), dict(sub=0.5)):
         P = gf.make_params(bub, bub, 1e4, **unsupported)
         assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 3, unsupported
     assert gf.lib().gf_eval_workspace_size(ctypes.byref(gf.make_params(bub, bub, 1e4)), 64, 32) > 0

@@ -803,13 +803,50 @@ def test_symmetric_routing(gf, oracle):
     assert relerr(gs, ref).max() < 2e-7 and relerr(gp, ref).min() > 1e-3
 
 
+@pytest.mark.parametrize("contour,box", [("ray_arc", (-40.0, 4.0, -14.0, 14.0)), ("auto", (-40.0, 4.0, -14.0, 14.0)),
+                                         ("thread", (-40.0, -17.0, -2.0, 2.0))])
+def test_symmetric_routing_on_deformed_contours(gf, oracle, contour, box):
+    """The symmetric routing under RAY_ARC / AUTO / THREAD (the policies applied to x/4: its cut is the paper routing's
+    there): parity on a 48 x 48 grid that reaches beyond the threshold parabola, real and complex equal masses; the
+    nodes bit-identical to the oracle's; CF1 beyond the parabola."""
+    n_rad, n_ang = 64, 32
+    rn, rw = gf.make_radial_tables(contour, n_rad, W.RADIAL_RULE)
+    z, wz = gf.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    rno, rwo = oracle.make_radial_pyramid(n_rad, levels=4)
+    zo, wzo = oracle.make_quadrature(W.ANGULAR_RULE, n_ang, measure="sqrt1mz2")
+    x = gf.make_grid(box[0], box[1], 48, box[2], box[3], 48)
+    xs = oracle.make_grid(box[0], box[1], 48, box[2], box[3], 48)
+    for m2 in ((1.0,) if contour == "thread" else (1.0, 0.7 - 0.4j)):
+        line = {"kind": "massive", "m2": m2}
+        P = gf.make_params(line, line, 1e5, routing="symmetric", contour=contour)
+        Po = oracle.make_params(line, line, 1e5, routing="symmetric", contour=contour)
+        g = gf.eval_grid(P, rn, rw, n_rad, z, wz, x).cpu().numpy()
+        ref, _ = oracle.eval_grid(Po, rno, rwo, n_rad, zo, wzo, xs, accum="extended")
+        e = relerr(g, ref)
+        assert e.max() <= TOL64, (contour, m2, e.max(), xs.ravel()[e.argmax()])
+    ws = gf.eval_prepare(P, rn, rw, n_rad, z, wz)
+    for xv in (xs.ravel()[5], xs.ravel()[1200], -30 + 0.5j):
+        pol, y, wy = gf.diag_contour_nodes(P, n_rad, n_ang, ws, rn, rw, xv)
+        polo, yo, wyo = oracle.contour_nodes(Po, xv, rno, rwo, n_rad, n_ang)
+        assert pol == polo and np.array_equal(y.cpu().numpy().view(np.float64), yo.view(np.float64))
+    if contour != "thread":
+        from tests import closed_forms as CF
+        bub = {"kind": "massive", "m2": 1.0}
+        rnb, rwb = gf.make_radial_tables(contour, 512, W.RADIAL_RULE)
+        zb, wzb = gf.make_quadrature("gauss_cheb2", 256, measure="sqrt1mz2")
+        pts = np.array([-8 + 4j, -6 + 1j, -20 + 12j])      # outside Re x > (Im x)^2/16 - 4
+        gb = gf.eval_grid(gf.make_params(bub, bub, 1e8, routing="symmetric", contour=contour), rnb, rwb, 512, zb, wzb,
+                          torch.from_numpy(pts).cuda()).cpu().numpy()
+        assert relerr(gb, [complex(CF.cf1(v)) for v in pts]).max() < 1e-7
+
+
 def test_symmetric_routing_refuses_what_it_does_not_define(gf):
     cfg = W.CONFIGS["cfg1_tiny"]
     rn, rw = gf.make_radial_tables("auto", cfg["n_rad"], W.RADIAL_RULE)
     z, wz = gf.make_quadrature(W.ANGULAR_RULE, cfg["n_ang"], measure="sqrt1mz2")
     x = gpu_grid(gf, cfg)
     bub = {"kind": "massive", "m2": 1.0}
-    for kw in (dict(line_pk={"kind": "massive", "m2": 2.0}), dict(contour="auto"),
+    for kw in (dict(line_pk={"kind": "massive", "m2": 2.0}), dict(taylor_order=1),
                dict(line_pk={"kind": "rational", "M2": 2.0, "a": 0.5, "b": 1.2})):
         args = dict(line_k=bub, line_pk=bub, cutoff2=1e4, routing="symmetric")
         args.update(kw)
