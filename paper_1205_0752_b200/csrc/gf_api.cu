@@ -321,7 +321,7 @@ int gf_trim_scratch(void) {
   return rc;
 }
 
-const char* gf_version(void) { return "gf_b200 0.2 (sm_100a)"; }
+const char* gf_version(void) { return "gf_b200 0.3 (sm_100a)"; }
 #ifndef GF_BUILD_ID
 #define GF_BUILD_ID ""
 #endif
