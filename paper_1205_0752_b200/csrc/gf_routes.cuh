@@ -17,7 +17,7 @@ namespace {
 constexpr int kKmc = 256;             // series coefficients staged per table (even)
 constexpr int kMomTerms = 32;         // genuine coefficients of the centred-moment series (zero beyond)
 #ifndef GF_SERIES_BITS
-#define GF_SERIES_BITS 50
+#define GF_SERIES_BITS 46
 #endif
 constexpr float kSeriesBits = GF_SERIES_BITS;    // series are cut where the dropped terms are below 2^-50 of the leading one
 // extra bits of error the FP32 phase of a series may cost over the truncation budget 2^-kSeriesBits (0: none)
@@ -25,6 +25,13 @@ constexpr float kSeriesBits = GF_SERIES_BITS;    // series are cut where the dro
 #define GF_FP32_SLACK_BITS 0
 #endif
 constexpr float kFp32Slack = GF_FP32_SLACK_BITS;
+// the centred-moment series (far nodes, at most 20 terms) is cut four bits later than the Chebyshev series: where
+// |x| >> the masses on a deformed contour its leading terms cancel in S and the truncation shows (measured: 1.2e-11
+// at 46 bits on a ray next to the negative axis, 3e-12 at 50)
+#ifndef GF_MOMENT_BITS
+#define GF_MOMENT_BITS (GF_SERIES_BITS + 4)
+#endif
+constexpr float kMomentBits = GF_MOMENT_BITS;
 #ifndef GF_GOERTZEL_UNROLL
 #define GF_GOERTZEL_UNROLL 2
 #endif
@@ -553,10 +560,10 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     o.g = o.sg;
     // (|s|/2)^K <= 2^-kSeriesBits;  log2 |s|^2 <= -4 (-inf when it underflows in FP32: K = 2)
     const float l2 = lg2_ftz((float)in), il = rcp_ftz(2.f - l2);
-    o.K = ((int)(2.f * kSeriesBits * il) + 5) & ~3;         // + 2, rounded up to whole trips of four terms
+    o.K = ((int)(2.f * kMomentBits * il) + 5) & ~3;         // + 2, rounded up to whole trips of four terms
     // FP32 from term K1 on: its rounding error 2^-24 A (|s|/2)^K1 (A <= 2.4 the recurrence's amplification) must stay
     // below 2^-kSeriesBits of the first-order term b_1 s of N, the smallest S can be: (|s|/2)^K1 <= 2^-(kSeriesBits-14) |s|
-    o.K1 = min(((int)((2.f * (kSeriesBits - 14.f - kFp32Slack) - l2) * il) + 5) & ~3, o.K);
+    o.K1 = min(((int)((2.f * (kMomentBits - 14.f - kFp32Slack) - l2) * il) + 5) & ~3, o.K);
   } else {
     // root = sqrt(zeta (zeta - 1)) = sqrt(w^2 - 1)/2, sign such that |w + 2 root| >= 1
     const double zm = zeta.re - 1.0, wr = fma(2.0, zeta.re, -1.0), wi = zeta.im + zeta.im;
@@ -904,8 +911,11 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc 
     int K = 0xffff, K1 = 0;
     if (ell * L.kmc >= 60.f) {
       K = 4;
+      // the dropped terms sum like a geometric series: the bound is on |c_j| rho^-j / (1 - 1/rho), so that a slowly
+      // converging series next to [0,1] (rho -> 1.18: a factor 6.5) is cut as safely as a fast one
+      const float geo = log2f(1.f / (1.f - exp2f(-ell)));
       for (int j = L.kmc - 1; j >= 4; --j)
-        if (s_lc[j] - (float)j * ell > -kSeriesBits - 2.f) {
+        if (s_lc[j] - (float)j * ell + geo > -kSeriesBits - 2.f) {
           K = j + 1;
           break;
         }
@@ -914,7 +924,7 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc 
       // perturbation of c_k by <= 4 2^-24 max_{j>=k}|c_j| / (1 - 1/rho)^2, and the perturbations sum like a geometric
       // series: the FP32 phase costs <= 2^-22 max_{j>=K1} |c_j| rho^-j / (1 - 1/rho)^3, held below the truncation
       // budget: |c_j| rho^-j <= 2^-(kSeriesBits - 20) (1 - 1/rho)^3 |c_0| for all j >= K1
-      const float thr = kSeriesBits - 20.f - kFp32Slack + 3.f * log2f(1.f / (1.f - exp2f(-ell)));
+      const float thr = kSeriesBits - 20.f - kFp32Slack + 3.f * geo;
       for (int j = L.kmc - 1; j >= 0; --j)
         if (s_lc[j] - (float)j * ell > -thr) {
           K1 = j + 1;
