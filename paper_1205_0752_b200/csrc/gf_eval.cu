@@ -337,7 +337,7 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
   L.off_momA = L.n_poly ? (int)take((long long)kMomTerms * L.n_poly) : -1;
   L.off_chebA = L.n_poly ? (int)take((long long)L.kmc * L.n_poly) : -1;
   L.off_ic = -1;
-  L.n_blk = n_pairs >= kBlkMinPairs ? (n_pairs + kBlkPairs - 1) / kBlkPairs : 0;
+  L.n_blk = n_pairs >= (pyramid ? kBlkMinPairsContour : kBlkMinPairs) ? (n_pairs + kBlkPairs - 1) / kBlkPairs : 0;
   L.off_blk = L.n_blk ? (int)take(2 * L.n_blk) : -1;
   L.off_blkM = L.n_blk ? (int)take((long long)L.n_blk * kBlkTerms) : -1;
   L.n_doubles = (int)o;

@@ -53,14 +53,18 @@ constexpr float kEllLo = 0.235f, kEllStep = 0.02f;
 // far from zeta (ellipse parameter of ITS interval rho_b^2 >= kBlkRho2Min) is summed by its own Chebyshev series of at
 // most kBlkTerms terms instead of pair by pair.  K_b = 112/log2(rho_b^2) + 1: dropped terms below 2^-56 rho-scaled.
 #ifndef GF_BLK_TERMS
-#define GF_BLK_TERMS 32
+#define GF_BLK_TERMS 64
 #endif
 constexpr int kBlkPairs = 32, kBlkTerms = GF_BLK_TERMS;
 #ifndef GF_BLK_MIN_PAIRS
-#define GF_BLK_MIN_PAIRS 192   // measured: 128 pairs (4 blocks) break even, 256 pairs gain 9 to 17 %
+#define GF_BLK_MIN_PAIRS 128           // REAL contour
 #endif
-constexpr int kBlkMinPairs = GF_BLK_MIN_PAIRS;   // rules with fewer folded pairs are not split
+#ifndef GF_BLK_MIN_PAIRS_CONTOUR
+#define GF_BLK_MIN_PAIRS_CONTOUR 192   // deformed contours (measured: 128 pairs lose 4 % there, 256 gain 15 %)
+#endif
+constexpr int kBlkMinPairs = GF_BLK_MIN_PAIRS, kBlkMinPairsContour = GF_BLK_MIN_PAIRS_CONTOUR;   // smaller rules are not split
 constexpr float kBlkRho2Min = GF_BLK_TERMS == 32 ? 12.3f : GF_BLK_TERMS == 48 ? 5.3f : 3.5f;   // 2^(112/(kBlkTerms - 1))
+static_assert(GF_BLK_TERMS == 32 || GF_BLK_TERMS == 48 || GF_BLK_TERMS == 64, "block series of 32, 48 or 64 terms");
 
 enum { ROUTE_MOMENT = 0, ROUTE_CHEB = 1, ROUTE_NEAR = 2, ROUTE_EXACT = 3 };
 
@@ -482,14 +486,18 @@ cd angular_blocked(cd eta, ZetaDD z, const Tabs<double>& tb, RouteCount& rc) {
     if ((float)rho2 >= kBlkRho2Min) {       // false for NaN (zeta on an end point of the block's interval): direct
       const double in = rcp_fast(rho2);
       const double sr = Dr * in, si = -Di * in, rr = sr + sr, ns = -in;
-      const int K = min((int)(112.f * rcp_ftz(lg2_ftz((float)rho2))) + 1, kBlkTerms);
-      const double* M = tb.blkM + b * kBlkTerms;
+      // whole trips of four terms (the table holds kBlkTerms, a multiple of 4; extra terms are below the cut)
+      const int K = min(((int)(112.f * rcp_ftz(lg2_ftz((float)rho2))) + 4) & ~3, kBlkTerms);
+      const double2* M2 = reinterpret_cast<const double2*>(tb.blkM + b * kBlkTerms) + (K >> 1);
       double p1 = 0.0, p2 = 0.0;
 #pragma unroll 1
-      for (int k = K - 1; k >= 0; --k) {
-        const double t = fma(rr, p1, fma(ns, p2, M[k]));
-        p2 = p1;
-        p1 = t;
+      for (int k = K; k > 0; k -= 4) {
+        M2 -= 2;
+        const double2 c23 = M2[1], c01 = M2[0];
+        p2 = fma(rr, p1, fma(ns, p2, c23.y));
+        p1 = fma(rr, p2, fma(ns, p1, c23.x));
+        p2 = fma(rr, p1, fma(ns, p2, c01.y));
+        p1 = fma(rr, p2, fma(ns, p1, c01.x));
       }
       const cd P = {fma(-p2, sr, p1), p2 * si};          // c_0 - c_1 conj(s)
       const double g2 = 2.0 * ch.y * rm;                 // (1/h) 2/root = (2/h) conj(root)/|root|^2
