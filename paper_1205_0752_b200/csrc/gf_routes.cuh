@@ -62,6 +62,10 @@ constexpr int kBlkPairs = 32, kBlkTerms = GF_BLK_TERMS;
 #ifndef GF_BLK_MIN_PAIRS_CONTOUR
 #define GF_BLK_MIN_PAIRS_CONTOUR 192   // deformed contours (measured: 128 pairs lose 4 % there, 256 gain 15 %)
 #endif
+#ifndef GF_BLK_CHEB_CAP
+#define GF_BLK_CHEB_CAP 256
+#endif
+constexpr int kBlkChebCap = GF_BLK_CHEB_CAP;   // with a split rule, Chebyshev series longer than this go to the direct route
 constexpr int kBlkMinPairs = GF_BLK_MIN_PAIRS, kBlkMinPairsContour = GF_BLK_MIN_PAIRS_CONTOUR;   // smaller rules are not split
 constexpr float kBlkRho2Min = GF_BLK_TERMS == 32 ? 12.3f : GF_BLK_TERMS == 48 ? 5.3f : 3.5f;   // 2^(112/(kBlkTerms - 1))
 static_assert(GF_BLK_TERMS == 32 || GF_BLK_TERMS == 48 || GF_BLK_TERMS == 64, "block series of 32, 48 or 64 terms");
@@ -200,6 +204,8 @@ struct Tabs {
   double mu0;                                     // sum of the folded weights
   double tau;                                     // EXACT inside this distance of [0,1]
   int n_pairs, kmc;
+  int kcap;                                       // longest Chebyshev series taken (kmc, or less where the split rule's
+                                                  // direct route is cheaper than a long series)
   int n_blk;                                      // blocks of the folded rule (0: not split)
   const double2* blk;                             // per block: centre c_b and 1/h_b of its interval [c - h, c + h]
   const double* blkM;                             // per block: M_k = sum'_{j in b} w_j T_k((t_j - c)/h), kBlkTerms each
@@ -231,6 +237,7 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
   tb.n_pairs = n_pairs;
   tb.kmc = L.kmc;
   tb.n_blk = L.n_blk;
+  tb.kcap = (sizeof(T) == 8 && L.n_blk > 0) ? min(L.kmc, kBlkChebCap) : L.kmc;
   tb.blk = reinterpret_cast<const double2*>(sb + (L.n_blk ? L.off_blk : 0));
   tb.blkM = sb + (L.n_blk ? L.off_blkM : 0);
   return tb;
@@ -609,7 +616,7 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     // CHEB whenever its series is short enough, whatever the direct loop would cost: next to [0,1] S is O(1), but
     // further out S can be 1e-7 of mu0 (the rule nearly integrates eta - t to zero) and the direct form
     // mu0 + (eta - zeta) C(zeta) would lose those digits; the series carry that cancellation in their tables
-    if (!(o.K <= tb.kmc)) {
+    if (!(o.K <= tb.kcap)) {
       o.K = o.K1 = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
       o.route = (zeta.im * zeta.im < tb.tau * tb.tau && zeta.re > -tb.tau && zeta.re < 1.0 + tb.tau) ? ROUTE_EXACT
                                                                                                      : ROUTE_NEAR;

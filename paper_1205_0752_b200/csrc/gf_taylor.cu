@@ -54,6 +54,7 @@ __device__ __forceinline__ TaylorTabs make_taylor_tabs(const double* sb, const B
   TaylorTabs t = {};
   t.tb.a_kreq = smem_u32(sb + L.off_kreq);
   t.tb.kmc = L.kmc;
+  t.tb.kcap = L.kmc;
   t.tb.tau = kTau64;
   t.st = sb + L.off_t;
   t.stlo = sb + L.off_tlo;
