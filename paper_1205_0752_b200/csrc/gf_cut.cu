@@ -28,9 +28,10 @@ __global__ void __launch_bounds__(256) prep_angular_only_kernel(const __grid_con
   __syncthreads();
   prep_angular(a, L, blob, &bad);
   __syncthreads();
-  prep_blocks(a, L, blob);
+  prep_blocks_T(a, L, blob);
   prep_series_T(a, L, blob);
   __syncthreads();
+  prep_blocks_sums(a, L, blob);
   prep_series_sums(a, L, blob, s_cpart);
   __syncthreads();
   prep_series_kreq(L, blob, s_lc, blob + L.off_cheb, 2);

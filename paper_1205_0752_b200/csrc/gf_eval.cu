@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
   prep_angular(a, L, blob, &bad);
   check_radial_tables(a, &bad);
   __syncthreads();  // t, w written by this CTA are visible to it
-  prep_blocks(a, L, blob);
+  prep_blocks_T(a, L, blob);
   prep_series_T(a, L, blob);
   if (L.off_gam >= 0) prep_tail_moments(a, L, blob, s_part);
   {
@@ -117,6 +117,7 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
     }
   }
   __syncthreads();  // the T_k(s_j) matrix, the monomial moments and the radial tables are complete
+  prep_blocks_sums(a, L, blob);
   prep_series_sums(a, L, blob, s_cpart);
   if (L.n_poly) prep_series_A(a, L, blob);
   __syncthreads();
@@ -344,6 +345,7 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
   if (pyramid) take_nodes();
   L.off_tail = tail ? (int)take(2LL * L.n_pref * (n_rad + 1) * kTailN) : -1;
   L.off_scratch = (int)take((long long)L.kmc * L.npad);
+  L.off_blkS = L.n_blk ? take(2LL * kBlkTerms * L.npad) : -1;
   L.off_scratch2 = tail ? (int)take(2LL * kTailN * n_rad) : -1;
   L.off_scratch3 = tail ? (int)take((long long)kTailN * n_rad + 2 * kTailChunks * (2 * L.n_pref * kTailN + kTailN)) : -1;
   L.n_rungs = 0;

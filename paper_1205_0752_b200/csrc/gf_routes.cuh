@@ -769,33 +769,60 @@ __device__ void prep_series_T(const EvalArgs& a, const BlobLayout& L, double* bl
   }
 }
 
-// Block tables of the folded rule (call after prep_angular and a __syncthreads()): per block its interval
-// [c - h, c + h] (the extreme t of its pairs) as (c, 1/h), and M_k = sum'_{j in b} w_j T_k(tau_j), tau_j = (t_j - c)/h,
-// k < kBlkTerms (k = 0 halved), T_k by the three-term recurrence and the sums in double-double.  One thread per (b, k).
-__device__ void prep_blocks(const EvalArgs& a, const BlobLayout& L, double* blob) {
+// Block tables of the folded rule, in two phases (both after prep_angular and a __syncthreads(), with another one
+// between them): per block its interval [c - h, c + h] (the extreme t of its pairs) as (c, 1/h), and
+// M_k = sum'_{j in b} w_j T_k(tau_j), tau_j = (t_j - c)/h, k < kBlkTerms (k = 0 halved).
+//   phase 1 (prep_blocks_T): one thread per pair j runs the three-term recurrence once, in double-double, and leaves
+//            w_j T_k(tau_j) (hi, lo) in the scratch [j][k];
+//   phase 2 (prep_blocks_sums): one thread per (b, k) adds its block's 32 entries in double-double.
+__device__ __forceinline__ void block_interval(const BlobLayout& L, const double* blob, int b, int n_pairs, double* c,
+                                               double* ih) {
+  const int j0 = b * kBlkPairs, j1 = min(j0 + kBlkPairs, n_pairs);
+  double tmin = blob[L.off_t + j0], tmax = tmin;
+  for (int j = j0 + 1; j < j1; ++j) {
+    tmin = fmin(tmin, blob[L.off_t + j]);
+    tmax = fmax(tmax, blob[L.off_t + j]);
+  }
+  *c = 0.5 * (tmin + tmax);
+  *ih = 1.0 / fmax(0.5 * (tmax - tmin), 1e-12);
+}
+__device__ void prep_blocks_T(const EvalArgs& a, const BlobLayout& L, double* blob) {
+  if (L.n_blk == 0) return;
+  double2* S = reinterpret_cast<double2*>(blob + L.off_blkS);
+  for (int j = threadIdx.x; j < a.n_pairs; j += blockDim.x) {
+    double c, ih;
+    block_interval(L, blob, j / kBlkPairs, a.n_pairs, &c, &ih);
+    const double w = blob[L.off_w + j];
+    const dd tau = dd_mul_d(dd_add_d(dd{blob[L.off_t + j], blob[L.off_tlo + j]}, -c), ih);
+    const dd twot = dd_scale2(tau, 2.0);
+    dd Tm = {1.0, 0.0}, Tk = tau;       // T_0, T_1
+    double2* row = S + (size_t)j * kBlkTerms;
+    row[0] = make_double2(w, 0.0);
+    const dd w1 = dd_mul_d(Tk, w);
+    row[1] = make_double2(w1.hi, w1.lo);
+    for (int q = 2; q < kBlkTerms; ++q) {
+      const dd Tn = dd_add(dd_mul(twot, Tk), dd_neg(Tm));
+      Tm = Tk;
+      Tk = Tn;
+      const dd wq = dd_mul_d(Tk, w);
+      row[q] = make_double2(wq.hi, wq.lo);
+    }
+  }
+}
+__device__ void prep_blocks_sums(const EvalArgs& a, const BlobLayout& L, double* blob) {
+  const double2* S = reinterpret_cast<const double2*>(blob + L.off_blkS);
   for (int e = threadIdx.x; e < L.n_blk * kBlkTerms; e += blockDim.x) {
     const int b = e / kBlkTerms, k = e % kBlkTerms;
     const int j0 = b * kBlkPairs, j1 = min(j0 + kBlkPairs, a.n_pairs);
-    double tmin = blob[L.off_t + j0], tmax = tmin;
-    for (int j = j0 + 1; j < j1; ++j) {
-      tmin = fmin(tmin, blob[L.off_t + j]);
-      tmax = fmax(tmax, blob[L.off_t + j]);
-    }
-    const double c = 0.5 * (tmin + tmax), ih = 1.0 / fmax(0.5 * (tmax - tmin), 1e-12);
     dd acc = {0.0, 0.0};
     for (int j = j0; j < j1; ++j) {
-      const dd tau = dd_mul_d(dd_add_d(dd{blob[L.off_t + j], blob[L.off_tlo + j]}, -c), ih);
-      const dd twot = dd_scale2(tau, 2.0);
-      dd Tm = {1.0, 0.0}, Tk = tau;       // T_0, T_1
-      for (int q = 2; q <= k; ++q) {
-        const dd Tn = dd_add(dd_mul(twot, Tk), dd_neg(Tm));
-        Tm = Tk;
-        Tk = Tn;
-      }
-      acc = dd_add(acc, dd_mul_d(k == 0 ? dd{1.0, 0.0} : Tk, blob[L.off_w + j]));
+      const double2 v = S[(size_t)j * kBlkTerms + k];
+      acc = dd_add(acc, dd{v.x, v.y});
     }
     blob[L.off_blkM + b * kBlkTerms + k] = (k == 0 ? 0.5 : 1.0) * acc.hi;
     if (k == 0) {
+      double c, ih;
+      block_interval(L, blob, b, a.n_pairs, &c, &ih);
       blob[L.off_blk + 2 * b] = c;
       blob[L.off_blk + 2 * b + 1] = ih;
     }

@@ -415,6 +415,7 @@ BlobLayout make_taylor_layout(int n_rad, int n_pairs, int n_terms, int order) {
   L.off_mom = L.off_cheb = L.off_sf = -1;
   L.n_blk = 0;
   L.off_blk = L.off_blkM = -1;
+  L.off_blkS = -1;
   L.n_total = o;
   return L;
 }
