@@ -318,6 +318,36 @@ def test_route_counters(gf):
         assert 0 < c["exact_nodes"] < 0.5 * direct_nodes and c["cheb_nodes"] > c["near_nodes"]
 
 
+@pytest.mark.parametrize("ang,n_ang", [("gauss_cheb2", 256), ("tanh_sinh", 385), ("gauss_legendre", 300),
+                                       ("tanh_sinh", 512), ("gauss_cheb1", 257)])
+@pytest.mark.parametrize("contour", ["real", "auto"])
+def test_split_rule_other_rules(gf, oracle, ang, n_ang, contour):
+    """The direct routes on a split rule (blocks of 32 folded pairs, far blocks by their own series) with rules whose
+    nodes cluster differently from Gauss-Legendre's, odd orders, a ragged last block and unequal masses, on config 1's
+    grid (every 3rd index): parity at 1e-11 on the REAL contour (rules of 128 and more pairs are split) and under AUTO
+    (192 and more)."""
+    cfg = W.CONFIGS["cfg1_tiny"]
+    n_rad = 64
+    lk, lp = {"kind": "massive", "m2": 1.0}, {"kind": "massive", "m2": 0.6}
+    P = gf.make_params(lk, lp, cfg["cutoff2"], contour=contour)
+    Po = oracle.make_params(lk, lp, cfg["cutoff2"], contour=contour)
+    rn, rw = gf.make_radial_tables(contour, n_rad, W.RADIAL_RULE)
+    rno, rwo = oracle.make_radial_pyramid(n_rad, levels=4)
+    if ang == "gauss_cheb1":   # the d = 2 rule with the d = 4 weight put into it: any symmetric rule is a legal input
+        z, wz = gf.make_quadrature_dim(ang, n_ang, 4.0)
+        zo, wzo = oracle.make_quadrature_dim(ang, n_ang, 4.0)
+    else:
+        z, wz = gf.make_quadrature(ang, n_ang, measure="sqrt1mz2")
+        zo, wzo = oracle.make_quadrature(ang, n_ang, measure="sqrt1mz2")
+    xs = np.ascontiguousarray(oracle_grid(oracle, cfg)[::3, ::3]).ravel()
+    g, c = gf.eval_grid_counted(P, rn, rw, n_rad, z, wz, torch.from_numpy(xs).cuda())
+    if contour == "real" or (n_ang + 1) // 2 >= 192:
+        assert c["block_series"] > 0
+    ref, _ = oracle.eval_grid(Po, rno, rwo, n_rad, zo, wzo, xs, accum="extended")
+    e = relerr(g.cpu().numpy(), ref)
+    assert e.max() <= TOL64, (ang, n_ang, contour, e.max(), xs[e.argmax()])
+
+
 def test_empty_input(gf):
     cfg = W.CONFIGS["cfg1_tiny"]
     P, rn, rw, z, wz = gpu_setup(gf, cfg)
