@@ -248,7 +248,7 @@ int gf_eval_angular(const gf_params* p, double x_re, double x_im, const double* 
 int gf_cut_crossings(const gf_params* p, const void* d_x, long long n_points, int n_z, int* d_out, void* stream);
 
 /* The same evaluation, also counting the work by route for the roofline accounting.
- * d_counters: 12 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
+ * d_counters: 13 unsigned 64-bit DEVICE counters the kernel ADDS to (zero them first):
  *   [0] pairs of the plain direct loop  [1] series terms EXECUTED in FP64 (every lane of a warp runs its warp's
  *   longest series; the FP64 kernel runs the high-order terms of a series, whose sum is below 2^-24 of the budget,
  *   in FP32: those are counter [9])  [2] pairs of the double-double direct loop (EXACT lanes, and the NEAR lanes of their warps)
@@ -256,8 +256,10 @@ int gf_cut_crossings(const gf_params* p, const void* d_x, long long n_points, in
  *   route (the triples of the large-y tail are not among them)  [7] series terms NEEDED (the sum over series
  *   triples of their own K)  [8] tail series evaluated, one per (point, pole)  [9] series terms executed in
  *   FP32 by the FP64 kernel  [10] far blocks of the angular rule summed by their own series on the NEAR / EXACT
- *   routes (rules of 64 and more folded pairs are split into blocks of 32; counters [0] and [2] then count only the
- *   pairs of the blocks next to zeta)  [11] terms of those block series.  Results are identical to gf_eval_grid. */
+ *   routes (rules of 128 and more folded pairs, 192 on the deformed contours, are split into a binary tree of blocks
+ *   whose leaves hold 32 pairs; counters [0] and [2] then count only the pairs of the leaves next to zeta)  [11] terms
+ *   of those block series  [12] leaves covered by them (a block of level l covers 2^l).  Results are identical to
+ *   gf_eval_grid. */
 int gf_eval_grid_counted(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
                          const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
                          long long n_points, void* d_out, unsigned long long* d_counters, void* stream);

@@ -53,7 +53,8 @@ class gf_launch_info(ctypes.Structure):
 
 
 COUNTER_NAMES = ("near_pairs", "series_terms", "exact_pairs", "near_nodes", "moment_nodes", "exact_nodes",
-                 "cheb_nodes", "series_terms_needed", "tails", "series_terms_fp32", "block_series", "block_series_terms")
+                 "cheb_nodes", "series_terms_needed", "tails", "series_terms_fp32", "block_series", "block_series_terms",
+                 "block_series_leaves")
 
 
 _lib = None

@@ -339,13 +339,22 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
   L.off_chebA = L.n_poly ? (int)take((long long)L.kmc * L.n_poly) : -1;
   L.off_ic = -1;
   L.n_blk = n_pairs >= (pyramid ? kBlkMinPairsContour : kBlkMinPairs) ? (n_pairs + kBlkPairs - 1) / kBlkPairs : 0;
-  L.off_blk = L.n_blk ? (int)take(2 * L.n_blk) : -1;
-  L.off_blkM = L.n_blk ? (int)take((long long)L.n_blk * kBlkTerms) : -1;
+  L.n_lev = 0;
+  L.n_blk_all = 0;
+  for (int l = 0, n = L.n_blk; l < kBlkMaxLev && n > 0; ++l) {   // levels up to the one that has a single block
+    L.lev_off[l] = L.n_blk_all;
+    L.n_blk_all += n;
+    L.n_lev = l + 1;
+    if (n == 1) break;
+    n = (n + 1) / 2;
+  }
+  L.off_blk = L.n_blk ? (int)take(2 * L.n_blk_all) : -1;
+  L.off_blkM = L.n_blk ? (int)take((long long)L.n_blk_all * kBlkTerms) : -1;
   L.n_doubles = (int)o;
   if (pyramid) take_nodes();
   L.off_tail = tail ? (int)take(2LL * L.n_pref * (n_rad + 1) * kTailN) : -1;
   L.off_scratch = (int)take((long long)L.kmc * L.npad);
-  L.off_blkS = L.n_blk ? take(2LL * kBlkTerms * L.npad) : -1;
+  L.off_blkS = L.n_blk ? take(2LL * kBlkTerms * L.npad * L.n_lev) : -1;
   L.off_scratch2 = tail ? (int)take(2LL * kTailN * n_rad) : -1;
   L.off_scratch3 = tail ? (int)take((long long)kTailN * n_rad + 2 * kTailChunks * (2 * L.n_pref * kTailN + kTailN)) : -1;
   L.n_rungs = 0;

@@ -18,6 +18,7 @@ struct PoleTerm {
 };
 
 constexpr int kMaxTerms = 2;
+constexpr int kBlkMaxLev = 4;    // levels of the tree of blocks of a split angular rule (gf_routes.cuh)
 constexpr int kMaxTaylor = 4;   // largest order n of the Taylor subtraction t^n (gf_taylor.cu)
 #ifndef GF_BLOCK_THREADS
 #define GF_BLOCK_THREADS 256
@@ -69,7 +70,7 @@ struct EvalArgs {
 };
 // codes a kernel leaves in *status (the next API call of the device returns GF_ERR_ARG and describes it)
 enum { kStatusAsymmetricRule = 1, kStatusRadialNodes = 2, kStatusWorkspace = 4 };
-constexpr int kLayoutVersion = 9;   // bump when a BlobLayout or the meaning of a table changes
+constexpr int kLayoutVersion = 10;   // bump when a BlobLayout or the meaning of a table changes
 
 // Offsets (in doubles) of the prepared tables, as the preparation kernel writes them and every CTA of the
 // evaluation kernel copies them to shared memory (one 16-byte header first).
@@ -110,7 +111,10 @@ struct BlobLayout {
   // blocks of the folded rule for the direct routes (gf_routes.cuh, angular_blocked), staged: n_blk x (c, 1/h) and
   // n_blk x kBlkTerms Chebyshev moments; n_blk = 0: the rule is not split
   int n_blk, off_blk, off_blkM;
-  long long off_blkS;           // preparation-only scratch of the block tables: double2 [n_pairs][kBlkTerms]
+  // the blocks form a binary tree: level l joins 2^l leaves (kBlkPairs 2^l pairs); lev_off[l] = index of level l's first
+  // block in the tables, n_lev levels, n_blk_all blocks over all levels (tables: n_blk_all entries)
+  int n_lev, n_blk_all, lev_off[kBlkMaxLev];
+  long long off_blkS;           // preparation-only scratch of the block tables: double2 [n_lev][n_pairs][kBlkTerms]
 };
 constexpr int kRungs = 64;      // tabulated contour radii above the first (deformed contours); then Lambda^2/2
 

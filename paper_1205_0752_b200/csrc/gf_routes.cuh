@@ -69,6 +69,8 @@ constexpr int kBlkChebCap = GF_BLK_CHEB_CAP;   // with a split rule, Chebyshev s
 constexpr int kBlkMinPairs = GF_BLK_MIN_PAIRS, kBlkMinPairsContour = GF_BLK_MIN_PAIRS_CONTOUR;   // smaller rules are not split
 constexpr float kBlkRho2Min = GF_BLK_TERMS == 32 ? 12.3f : GF_BLK_TERMS == 48 ? 5.3f : 3.5f;   // 2^(112/(kBlkTerms - 1))
 static_assert(GF_BLK_TERMS == 32 || GF_BLK_TERMS == 48 || GF_BLK_TERMS == 64, "block series of 32, 48 or 64 terms");
+// |w'|^2 beyond which a block is far: the squared semi-major axis of the ellipse rho^2 = kBlkRho2Min, (R + 2 + 1/R)/4
+constexpr double kBlkFarW2 = (kBlkRho2Min + 2.0 + 1.0 / kBlkRho2Min) / 4.0;
 
 enum { ROUTE_MOMENT = 0, ROUTE_CHEB = 1, ROUTE_NEAR = 2, ROUTE_EXACT = 3 };
 
@@ -206,7 +208,9 @@ struct Tabs {
   int n_pairs, kmc;
   int kcap;                                       // longest Chebyshev series taken (kmc, or less where the split rule's
                                                   // direct route is cheaper than a long series)
-  int n_blk;                                      // blocks of the folded rule (0: not split)
+  int n_blk;                                      // leaf blocks of the folded rule (0: not split)
+  int n_lev;                                      // levels of the tree of blocks
+  unsigned long long lev_pack;                    // level l's blocks start at table index (lev_pack >> 16 l) & 0xffff
   const double2* blk;                             // per block: centre c_b and 1/h_b of its interval [c - h, c + h]
   const double* blkM;                             // per block: M_k = sum'_{j in b} w_j T_k((t_j - c)/h), kBlkTerms each
 };
@@ -237,6 +241,10 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
   tb.n_pairs = n_pairs;
   tb.kmc = L.kmc;
   tb.n_blk = L.n_blk;
+  tb.n_lev = L.n_lev;
+  tb.lev_pack = 0;
+#pragma unroll
+  for (int l = 0; l < kBlkMaxLev; ++l) tb.lev_pack |= (unsigned long long)(L.lev_off[l] & 0xffff) << (16 * l);
   tb.kcap = (sizeof(T) == 8 && L.n_blk > 0) ? min(L.kmc, kBlkChebCap) : L.kmc;
   tb.blk = reinterpret_cast<const double2*>(sb + (L.n_blk ? L.off_blk : 0));
   tb.blkM = sb + (L.n_blk ? L.off_blkM : 0);
@@ -246,9 +254,10 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
 // Work counters of one thread (COUNT launches only)
 struct RouteCount {
   unsigned long long near_pairs = 0, series_exec = 0, exact_pairs = 0, n_near = 0, n_moment = 0, n_exact = 0,
-                     n_cheb = 0, series_used = 0, tails = 0, series_exec32 = 0, blk_series = 0, blk_terms = 0;
+                     n_cheb = 0, series_used = 0, tails = 0, series_exec32 = 0, blk_series = 0, blk_terms = 0,
+                     blk_leaves = 0;
 };
-constexpr int kNumCounters = 12;
+constexpr int kNumCounters = 13;
 
 // ---- NEAR: one folded angular pair: q = w/|zeta - t|^2 and the two sums ---------------------------
 __device__ __forceinline__ void pair_step(double zr, double zi2, double t, double w, double& u0, double& u1) {
@@ -476,26 +485,41 @@ __device__ __noinline__
 cd angular_blocked(cd eta, ZetaDD z, const Tabs<double>& tb, RouteCount& rc) {
   double u0 = 0.0, u1 = 0.0, v0 = 0.0, v1 = 0.0;   // direct sums: U0 = sum q_j; U1 = sum q_j a_j (DD) or sum q_j t_j
   cd far = {0.0, 0.0};
+  // The blocks form a binary tree (level l joins 2^l leaves).  Walk the leaves from the left; at leaf b try the
+  // largest block that starts there, then its left descendants: a block is taken by its series if |w'|^2 >= kBlkFarW2
+  // (w' outside the disk that contains the ellipse rho_b^2 = kBlkRho2Min, so its series needs <= kBlkTerms terms);
+  // a leaf that is not far is summed pair by pair.  A NaN fails the test: direct.
+  int b = 0;
 #pragma unroll 1
-  for (int b = 0; b < tb.n_blk; ++b) {
-    const double2 ch = tb.blk[b];
-    const double wr = (z.re_hi - ch.x) * ch.y, wi = z.im * ch.y;
-    const double qr = fma(wr, wr, -fma(wi, wi, 1.0)), qi = 2.0 * wr * wi;   // w'^2 - 1
-    const double n2 = fma(qr, qr, qi * qi);
-    const double rm = rsqrt_fast(n2);                                      // 1/|q| = 1/|root|^2
-    const double h2 = 0.5 * fma(n2, rm, fabs(qr));
-    const double rh = rsqrt_fast(h2);
-    const double h = h2 * rh, kk = 0.5 * qi * rh;
-    double ar = qr >= 0.0 ? h : fabs(kk), ai = qr >= 0.0 ? kk : copysign(h, qi);
-    if (fma(wr, ar, wi * ai) < 0.0) { ar = -ar; ai = -ai; }
-    const double Dr = wr + ar, Di = wi + ai;
-    const double rho2 = fma(Dr, Dr, Di * Di);
-    if ((float)rho2 >= kBlkRho2Min) {       // false for NaN (zeta on an end point of the block's interval): direct
+  while (b < tb.n_blk) {
+    int l = min(tb.n_lev - 1, b ? __ffs(b) - 1 : kBlkMaxLev - 1), idx = 0;
+    double wr = 0.0, wi = 0.0, ih = 0.0;
+    bool is_far = false;
+#pragma unroll 1
+    for (; l >= 0; --l) {
+      idx = (int)((tb.lev_pack >> (16 * l)) & 0xffffu) + (b >> l);
+      const double2 ch = tb.blk[idx];
+      ih = ch.y;
+      wr = (z.re_hi - ch.x) * ih;
+      wi = z.im * ih;
+      if (fma(wr, wr, wi * wi) >= kBlkFarW2) { is_far = true; break; }
+    }
+    if (is_far) {
+      const double qr = fma(wr, wr, -fma(wi, wi, 1.0)), qi = 2.0 * wr * wi;   // w'^2 - 1
+      const double n2 = fma(qr, qr, qi * qi);
+      const double rm = rsqrt_fast(n2);                                      // 1/|q| = 1/|root|^2
+      const double h2 = 0.5 * fma(n2, rm, fabs(qr));
+      const double rh = rsqrt_fast(h2);
+      const double h = h2 * rh, kk = 0.5 * qi * rh;
+      double ar = qr >= 0.0 ? h : fabs(kk), ai = qr >= 0.0 ? kk : copysign(h, qi);
+      if (fma(wr, ar, wi * ai) < 0.0) { ar = -ar; ai = -ai; }
+      const double Dr = wr + ar, Di = wi + ai;
+      const double rho2 = fma(Dr, Dr, Di * Di);
       const double in = rcp_fast(rho2);
       const double sr = Dr * in, si = -Di * in, rr = sr + sr, ns = -in;
       // whole trips of four terms (the table holds kBlkTerms, a multiple of 4; extra terms are below the cut)
       const int K = min(((int)(112.f * rcp_ftz(lg2_ftz((float)rho2))) + 4) & ~3, kBlkTerms);
-      const double2* M2 = reinterpret_cast<const double2*>(tb.blkM + b * kBlkTerms) + (K >> 1);
+      const double2* M2 = reinterpret_cast<const double2*>(tb.blkM + idx * kBlkTerms) + (K >> 1);
       double p1 = 0.0, p2 = 0.0;
 #pragma unroll 1
       for (int k = K; k > 0; k -= 4) {
@@ -507,9 +531,10 @@ cd angular_blocked(cd eta, ZetaDD z, const Tabs<double>& tb, RouteCount& rc) {
         p1 = fma(rr, p2, fma(ns, p1, c01.x));
       }
       const cd P = {fma(-p2, sr, p1), p2 * si};          // c_0 - c_1 conj(s)
-      const double g2 = 2.0 * ch.y * rm;                 // (1/h) 2/root = (2/h) conj(root)/|root|^2
+      const double g2 = 2.0 * ih * rm;                   // (1/h) 2/root = (2/h) conj(root)/|root|^2
       far = cadd(far, cmul(cd{ar * g2, -ai * g2}, P));
-      if (COUNT) { ++rc.blk_series; rc.blk_terms += K; }
+      if (COUNT) { ++rc.blk_series; rc.blk_terms += K; rc.blk_leaves += 1 << l; }
+      b += 1 << l;
     } else {
       const int j0 = b * kBlkPairs, j1 = min(j0 + kBlkPairs, tb.n_pairs);
       int j = j0;
@@ -528,6 +553,7 @@ cd angular_blocked(cd eta, ZetaDD z, const Tabs<double>& tb, RouteCount& rc) {
         else pair_step(z.re_hi, z.im2, tb.st[j], tb.sw[j], u0, u1);
       }
       if (COUNT) { if (DD) rc.exact_pairs += j1 - j0; else rc.near_pairs += j1 - j0; }
+      ++b;
     }
   }
   u0 += v0;
@@ -707,7 +733,8 @@ __device__ __forceinline__ cd node_term(const Tabs<T>& tb, cd x, cd y, cd delta,
 __device__ __forceinline__ void flush_counters(const RouteCount& rc, bool active, unsigned long long* counters) {
   unsigned long long v[kNumCounters] = {rc.near_pairs, rc.series_exec, rc.exact_pairs,   rc.n_near,
                                         rc.n_moment,   rc.n_exact,     rc.n_cheb,        rc.series_used,
-                                        rc.tails,      rc.series_exec32, rc.blk_series,  rc.blk_terms};
+                                        rc.tails,      rc.series_exec32, rc.blk_series,  rc.blk_terms,
+                                        rc.blk_leaves};
   for (int k = 0; k < kNumCounters; ++k) {
     if (!active) v[k] = 0;
     for (int o = 16; o; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
@@ -775,9 +802,11 @@ __device__ void prep_series_T(const EvalArgs& a, const BlobLayout& L, double* bl
 //   phase 1 (prep_blocks_T): one thread per pair j runs the three-term recurrence once, in double-double, and leaves
 //            w_j T_k(tau_j) (hi, lo) in the scratch [j][k];
 //   phase 2 (prep_blocks_sums): one thread per (b, k) adds its block's 32 entries in double-double.
-__device__ __forceinline__ void block_interval(const BlobLayout& L, const double* blob, int b, int n_pairs, double* c,
-                                               double* ih) {
-  const int j0 = b * kBlkPairs, j1 = min(j0 + kBlkPairs, n_pairs);
+// block i of level l covers the pairs [i 2^l kBlkPairs, (i + 1) 2^l kBlkPairs) of the rule
+__device__ __forceinline__ void block_interval(const BlobLayout& L, const double* blob, int l, int i, int n_pairs,
+                                               double* c, double* ih) {
+  const int span = kBlkPairs << l;
+  const int j0 = i * span, j1 = min(j0 + span, n_pairs);
   double tmin = blob[L.off_t + j0], tmax = tmin;
   for (int j = j0 + 1; j < j1; ++j) {
     tmin = fmin(tmin, blob[L.off_t + j]);
@@ -789,14 +818,15 @@ __device__ __forceinline__ void block_interval(const BlobLayout& L, const double
 __device__ void prep_blocks_T(const EvalArgs& a, const BlobLayout& L, double* blob) {
   if (L.n_blk == 0) return;
   double2* S = reinterpret_cast<double2*>(blob + L.off_blkS);
-  for (int j = threadIdx.x; j < a.n_pairs; j += blockDim.x) {
+  for (int e = threadIdx.x; e < a.n_pairs * L.n_lev; e += blockDim.x) {
+    const int l = e / a.n_pairs, j = e % a.n_pairs;
     double c, ih;
-    block_interval(L, blob, j / kBlkPairs, a.n_pairs, &c, &ih);
+    block_interval(L, blob, l, j / (kBlkPairs << l), a.n_pairs, &c, &ih);
     const double w = blob[L.off_w + j];
     const dd tau = dd_mul_d(dd_add_d(dd{blob[L.off_t + j], blob[L.off_tlo + j]}, -c), ih);
     const dd twot = dd_scale2(tau, 2.0);
     dd Tm = {1.0, 0.0}, Tk = tau;       // T_0, T_1
-    double2* row = S + (size_t)j * kBlkTerms;
+    double2* row = S + ((size_t)l * a.n_pairs + j) * kBlkTerms;
     row[0] = make_double2(w, 0.0);
     const dd w1 = dd_mul_d(Tk, w);
     row[1] = make_double2(w1.hi, w1.lo);
@@ -811,20 +841,23 @@ __device__ void prep_blocks_T(const EvalArgs& a, const BlobLayout& L, double* bl
 }
 __device__ void prep_blocks_sums(const EvalArgs& a, const BlobLayout& L, double* blob) {
   const double2* S = reinterpret_cast<const double2*>(blob + L.off_blkS);
-  for (int e = threadIdx.x; e < L.n_blk * kBlkTerms; e += blockDim.x) {
-    const int b = e / kBlkTerms, k = e % kBlkTerms;
-    const int j0 = b * kBlkPairs, j1 = min(j0 + kBlkPairs, a.n_pairs);
+  for (int e = threadIdx.x; e < L.n_blk_all * kBlkTerms; e += blockDim.x) {
+    const int idx = e / kBlkTerms, k = e % kBlkTerms;
+    int l = 0;
+    while (l + 1 < L.n_lev && idx >= L.lev_off[l + 1]) ++l;
+    const int i = idx - L.lev_off[l], span = kBlkPairs << l;
+    const int j0 = i * span, j1 = min(j0 + span, a.n_pairs);
     dd acc = {0.0, 0.0};
     for (int j = j0; j < j1; ++j) {
-      const double2 v = S[(size_t)j * kBlkTerms + k];
+      const double2 v = S[((size_t)l * a.n_pairs + j) * kBlkTerms + k];
       acc = dd_add(acc, dd{v.x, v.y});
     }
-    blob[L.off_blkM + b * kBlkTerms + k] = (k == 0 ? 0.5 : 1.0) * acc.hi;
+    blob[L.off_blkM + idx * kBlkTerms + k] = (k == 0 ? 0.5 : 1.0) * acc.hi;
     if (k == 0) {
       double c, ih;
-      block_interval(L, blob, b, a.n_pairs, &c, &ih);
-      blob[L.off_blk + 2 * b] = c;
-      blob[L.off_blk + 2 * b + 1] = ih;
+      block_interval(L, blob, l, i, a.n_pairs, &c, &ih);
+      blob[L.off_blk + 2 * idx] = c;
+      blob[L.off_blk + 2 * idx + 1] = ih;
     }
   }
 }

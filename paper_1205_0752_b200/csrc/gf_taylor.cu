@@ -413,7 +413,7 @@ BlobLayout make_taylor_layout(int n_rad, int n_pairs, int n_terms, int order) {
   L.off_scratch = take((long long)L.kmc * L.npad);
   L.off_f32 = L.off_rt = L.off_rw = L.off_gam = L.off_gam2 = L.off_tail = L.off_scratch2 = L.off_scratch3 = -1;
   L.off_mom = L.off_cheb = L.off_sf = -1;
-  L.n_blk = 0;
+  L.n_blk = L.n_lev = L.n_blk_all = 0;
   L.off_blk = L.off_blkM = -1;
   L.off_blkS = -1;
   L.n_total = o;

@@ -301,15 +301,16 @@ def test_route_counters(gf):
         assert 0 < direct_nodes + series_nodes < 0.8 * x.numel() * cfg["n_rad"]
         assert c["tails"] % x.numel() == 0 and c["tails"] >= x.numel()   # one per (point, pole) and lane sharing the point
         # pairs are counted by loop (the NEAR lanes of a warp with an EXACT lane run the double-double loop too)
-        assert c["near_pairs"] + c["exact_pairs"] + 32 * c["block_series"] == direct_nodes * n_pairs
+        assert c["near_pairs"] + c["exact_pairs"] + 32 * c["block_series_leaves"] == direct_nodes * n_pairs
         if n_pairs < 128:
-            assert c["block_series"] == 0 and c["block_series_terms"] == 0
+            assert c["block_series"] == 0 and c["block_series_terms"] == 0 and c["block_series_leaves"] == 0
             assert c["exact_pairs"] >= c["exact_nodes"] * n_pairs
         else:
             n_blk = (n_pairs + 31) // 32
             # (a zeta just outside the outermost node is far from EVERY block in units of the block's width: no pair)
             assert 0 < c["near_pairs"] + c["exact_pairs"] and 0 < c["block_series"] <= n_blk * direct_nodes
             assert c["block_series"] <= c["block_series_terms"] <= 64 * c["block_series"]
+            assert c["block_series"] <= c["block_series_leaves"] <= n_blk * direct_nodes   # a block of level l covers 2^l leaves
         # each series triple needs 4..256 terms; a warp runs its longest series on all 32 lanes, the high-order terms
         # in FP32 (counter "series_terms_fp32"), the rest in FP64 ("series_terms")
         assert 4 * series_nodes <= c["series_terms_needed"] <= 256 * series_nodes
