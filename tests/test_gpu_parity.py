@@ -320,11 +320,12 @@ def test_route_counters(gf):
 
 
 @pytest.mark.parametrize("ang,n_ang", [("gauss_cheb2", 256), ("tanh_sinh", 385), ("gauss_legendre", 300),
-                                       ("tanh_sinh", 512), ("gauss_cheb1", 257)])
+                                       ("tanh_sinh", 512), ("gauss_cheb1", 257), ("gauss_legendre", 1100)])
 @pytest.mark.parametrize("contour", ["real", "auto"])
 def test_split_rule_other_rules(gf, oracle, ang, n_ang, contour):
-    """The direct routes on a split rule (blocks of 32 folded pairs, far blocks by their own series) with rules whose
-    nodes cluster differently from Gauss-Legendre's, odd orders, a ragged last block and unequal masses, on config 1's
+    """The direct routes on a split rule (a binary tree of blocks over leaves of 32 folded pairs, far blocks by their own
+    series) with rules whose nodes cluster differently from Gauss-Legendre's, odd orders, ragged last blocks on every
+    level (1100 nodes: 18 leaves under 9, 5 and 3 blocks) and unequal masses, on config 1's
     grid (every 3rd index): parity at 1e-11 on the REAL contour (rules of 128 and more pairs are split) and under AUTO
     (192 and more)."""
     cfg = W.CONFIGS["cfg1_tiny"]
