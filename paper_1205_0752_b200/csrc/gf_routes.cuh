@@ -204,7 +204,6 @@ struct Tabs {
                                                   // (moment table first, the Chebyshev table kmc entries further)
   const int* kreq;                                // Chebyshev terms needed per bin of log2(rho): K | K1 << 16
   double mu0;                                     // sum of the folded weights
-  double tau;                                     // EXACT inside this distance of [0,1]
   int n_pairs, kmc;
   int kcap;                                       // longest Chebyshev series taken (kmc, or less where the split rule's
                                                   // direct route is cheaper than a long series)
@@ -237,7 +236,6 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
   tb.a_momf = smem_u32(sb + L.off_sf);
   tb.kreq = reinterpret_cast<const int*>(sb + L.off_kreq);
   tb.mu0 = sb[L.off_mom];  // a_0 of the moment series = sum of the folded weights
-  tb.tau = sizeof(T) == 8 ? kTau64 : kTau32;
   tb.n_pairs = n_pairs;
   tb.kmc = L.kmc;
   tb.n_blk = L.n_blk;
@@ -580,6 +578,9 @@ cd angular_blocked(cd eta, ZetaDD z, const Tabs<double>& tb, RouteCount& rc) {
 //   EXACT   zeta within tau of [0,1];   NEAR  the rest (zeta close to [0,1], or few angular nodes).
 // ---------------------------------------------------------------------------------------------
 // The series argument of one (point, radial node, pole), as route_setup leaves it
+#ifndef GF_CHEB_DIRECT_S
+#define GF_CHEB_DIRECT_S 1
+#endif
 struct SeriesArg {
   cd sg, g;     // series argument s and prefactor
   double ns;    // -|s|^2
@@ -616,11 +617,26 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     const double h = h2 * rh, kk = 0.5 * qi * rh;
     // signs by integer operations on the high words (sign tests and negations would take FP64-pipe slots)
     const bool qpos = __double2hiint(qr) >= 0;
-    double ar = qpos ? h : fabs(kk);
+    double ar = qpos ? h : __hiloint2double(__double2hiint(kk) & 0x7fffffff, __double2loint(kk));   // |kk|
     double ai = qpos ? kk : copysign(h, qi);
     const int flip = __double2hiint(fma(wr, ar, wi * ai)) & 0x80000000;   // Re(conj(w) root) < 0: the other root
     ar = __hiloint2double(__double2hiint(ar) ^ flip, __double2loint(ar));
     ai = __hiloint2double(__double2hiint(ai) ^ flip, __double2loint(ai));
+#if GF_CHEB_DIRECT_S
+    // s = 1/(w + 2 root) = w - 2 root exactly ((w + 2 root)(w - 2 root) = w^2 - (w^2 - 1)): no reciprocal.  The
+    // difference cancels |w|/|s| <= 2 |w|^2 of its operands' digits; |w| < 14 on this route (MOMENT beyond)
+    const double sr = fma(-2.0, ar, wr), si = fma(-2.0, ai, wi);
+    const double ns = fma(-sr, sr, -(si * si));        // -|s|^2 = -1/rho^2
+    const float ell = -0.5f * lg2_ftz(fabsf((float)ns));   // log2(rho)
+    int kq = 0xffff;
+    if (ell >= kEllLo)
+      asm volatile("ld.shared.s32 %0, [%1];" : "=r"(kq)
+                   : "r"(tb.a_kreq + 4u * (uint32_t)min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)));
+    o.K = kq & 0xffff;     // 0xffff: no usable series in this bin
+    o.K1 = kq >> 16;
+    o.sg = {sr, si};
+    o.ns = ns;
+#else
     const double Dr = fma(2.0, ar, wr), Di = fma(2.0, ai, wi);
     const double rho2 = fma(Dr, Dr, Di * Di);
     // terms needed at this rho (table made from the coefficients themselves, prep_series_kreq); taken from rho^2
@@ -636,6 +652,7 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     const double in = rcp_fast(rho2);                  // 1/rho^2
     o.sg = {Dr * in, -Di * in};
     o.ns = -in;
+#endif
     const double g2 = rm + rm;                   // 4/sqrt(w^2-1) = 2 conj(root)/|q|
     o.g = {ar * g2, -ai * g2};
     o.route = ROUTE_CHEB;
@@ -644,8 +661,12 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     // mu0 + (eta - zeta) C(zeta) would lose those digits; the series carry that cancellation in their tables
     if (!(o.K <= tb.kcap)) {
       o.K = o.K1 = 0;   // sg, ns stay as they are: this lane idles through the series loop and its result is dropped
-      o.route = (zeta.im * zeta.im < tb.tau * tb.tau && zeta.re > -tb.tau && zeta.re < 1.0 + tb.tau) ? ROUTE_EXACT
-                                                                                                     : ROUTE_NEAR;
+      // |Im zeta| < tau and -tau < Re zeta < 1 + tau on the high words: tau and 1 + tau have a zero low word (tau a
+      // power of two >= 2^-20), so a < c is hi(a) < hi(c) exactly; a NaN compares as a large number (NEAR, as before)
+      constexpr double tau = sizeof(T) == 8 ? kTau64 : kTau32;
+      const int th = __double2hiint(tau), oh = __double2hiint(1.0 + tau);
+      const int zih = __double2hiint(zeta.im) & 0x7fffffff, zrh = __double2hiint(zeta.re);
+      o.route = (zih < th && (zrh >= 0 ? zrh < oh : (zrh & 0x7fffffff) < th)) ? ROUTE_EXACT : ROUTE_NEAR;
     }
   }
   return o;

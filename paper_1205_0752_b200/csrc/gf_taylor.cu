@@ -45,7 +45,7 @@ __host__ __device__ constexpr double psi_coef(int i, int k) {
 
 // The staged tables one node-term needs
 struct TaylorTabs {
-  Tabs<double> tb;              // a_kreq, kmc, tau (route_setup)
+  Tabs<double> tb;              // a_kreq, kmc (route_setup)
   const double *st, *stlo, *sw; // folded rule
   const double *momA, *chebA;   // n + 2 series tables per family, [k][n + 2]
   int n_pairs;
@@ -55,7 +55,6 @@ __device__ __forceinline__ TaylorTabs make_taylor_tabs(const double* sb, const B
   t.tb.a_kreq = smem_u32(sb + L.off_kreq);
   t.tb.kmc = L.kmc;
   t.tb.kcap = L.kmc;
-  t.tb.tau = kTau64;
   t.st = sb + L.off_t;
   t.stlo = sb + L.off_tlo;
   t.sw = sb + L.off_w;
