@@ -144,7 +144,9 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
 #ifndef GF_MIN_BLOCKS
 #define GF_MIN_BLOCKS 4
 #endif
-template <typename T, bool COUNT, int NT, bool BLK>
+// SPLIT = false: one thread per point known at compile time (the node pointers are then warp-uniform: no lane
+// registers, nothing of the node loop's bookkeeping in local memory)
+template <typename T, bool COUNT, int NT, bool BLK, bool SPLIT>
 __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
     eval_real_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                      const double* __restrict__ blob, unsigned long long* __restrict__ counters) {
@@ -168,10 +170,10 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
   const Tabs<T> tb = make_tabs<T>(sb, L, a.n_pairs);
   const bool bad_rule = sb[0] != 0.0;
 
-  const int S = 1 << a.split_log2;
+  const int S = SPLIT ? 1 << a.split_log2 : 1;
   const long long gtid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  const long long point = gtid >> a.split_log2;
-  const int sub = (int)(gtid & (S - 1));
+  const long long point = SPLIT ? gtid >> a.split_log2 : gtid;
+  const int sub = SPLIT ? (int)(gtid & (S - 1)) : 0;
   const bool active = point < a.n_points;
 
   cd x = {1.0, 0.0};
@@ -408,10 +410,10 @@ int plan_eval(const EvalArgs& a, int precision, LaunchPlan* plan) {
   return GF_OK;
 }
 
-template <typename T, bool COUNT, int NT, bool BLK>
-static int launch_real_nt(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
-                          cudaStream_t stream) {
-  auto kern = eval_real_kernel<T, COUNT, NT, BLK>;
+template <typename T, bool COUNT, int NT, bool BLK, bool SPLIT>
+static int launch_real_kern(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
+                            cudaStream_t stream) {
+  auto kern = eval_real_kernel<T, COUNT, NT, BLK, SPLIT>;
   if (plan.smem_bytes > 48 * 1024) {
     int rc = check_cuda(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes),
                         "cudaFuncSetAttribute(max dynamic shared memory)");
@@ -420,15 +422,24 @@ static int launch_real_nt(const EvalArgs& a, const LaunchPlan& plan, const doubl
   kern<<<(unsigned)plan.grid_blocks, plan.block_threads, plan.smem_bytes, stream>>>(a, plan.layout, blob, counters);
   return check_cuda(cudaGetLastError(), "eval kernel launch");
 }
+// the kernel instantiation for this launch: the unsplit one exists for the timed FP64 kernels only, the blocked one
+// for FP64 only
+template <typename T, bool COUNT, int NT, bool BLK>
+static int launch_real_nt(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
+                          cudaStream_t stream) {
+  if constexpr (!COUNT && sizeof(T) == 8)
+    if (a.split_log2 == 0) return launch_real_kern<T, COUNT, NT, BLK, false>(a, plan, blob, counters, stream);
+  return launch_real_kern<T, COUNT, NT, BLK, true>(a, plan, blob, counters, stream);
+}
 template <typename T, bool COUNT>
 static int launch_real(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
                        cudaStream_t stream) {
-  const bool blk = sizeof(T) == 8 && plan.layout.n_blk > 0;
-  if (a.n_terms == 1)
-    return blk ? launch_real_nt<T, COUNT, 1, true>(a, plan, blob, counters, stream)
-               : launch_real_nt<T, COUNT, 1, false>(a, plan, blob, counters, stream);
-  return blk ? launch_real_nt<T, COUNT, 2, true>(a, plan, blob, counters, stream)
-             : launch_real_nt<T, COUNT, 2, false>(a, plan, blob, counters, stream);
+  if constexpr (sizeof(T) == 8)
+    if (plan.layout.n_blk > 0)
+      return a.n_terms == 1 ? launch_real_nt<T, COUNT, 1, true>(a, plan, blob, counters, stream)
+                            : launch_real_nt<T, COUNT, 2, true>(a, plan, blob, counters, stream);
+  return a.n_terms == 1 ? launch_real_nt<T, COUNT, 1, false>(a, plan, blob, counters, stream)
+                        : launch_real_nt<T, COUNT, 2, false>(a, plan, blob, counters, stream);
 }
 
 int launch_radial_map(double Llog_hi, double Llog_lo, double s0, const double* d_nodes, int n, double* d_y,
