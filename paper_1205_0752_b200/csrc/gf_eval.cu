@@ -61,26 +61,52 @@ __global__ void radial_map_kernel(double Lhi, double Llo, double s0, const doubl
 }
 
 // ---------------------------------------------------------------------------------------------
-// Preparation (one CTA): everything that does not depend on x, for the REAL contour.
-//   header [0] = 1.0 if the angular rule is not symmetric;  t, t_lo, w (folded rule);  series coefficients
-//   mom[k], cheb[k];  y_i, 1/(4 y_i);  pref_{r,i} = c0 Wr_i y_i D1(y_i) (-R_r/(y_i + mu_r)).
+// Preparation: everything that does not depend on x, for the REAL contour.
+//   header [0] = status bits of the tables;  t, t_lo, w (folded rule);  series coefficients mom[k], cheb[k], Kreq;
+//   block tables of a split rule;  y_i, 1/(4 y_i);  pref_{r,i} = c0 Wr_i y_i D1(y_i) (-R_r/(y_i + mu_r));  the
+//   tail's gamma and Rhat tables.
+// Three CTAs with one role each, nothing exchanged between them (each folds the angular rule for itself: the same
+// values to the same places): 0 the series tables and the checks, 1 the radial tables and the tail's, 2 the block
+// tables.  Their chains of dependent double-double steps run side by side instead of one after the other.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ EvalArgs a,
-                                                        const __grid_constant__ BlobLayout L,
-                                                        double* __restrict__ blob) {
+constexpr int kPrepThreads = 512, kPrepRoles = 3;
+__global__ void __launch_bounds__(kPrepThreads) prep_real_kernel(const __grid_constant__ EvalArgs a,
+                                                                 const __grid_constant__ BlobLayout L,
+                                                                 double* __restrict__ blob) {
   __shared__ int bad;
   __shared__ dd s_mu[kTailN], s_nu[kTailN], s_part[8][2][kTailN];
   __shared__ float s_lc[kKmc];
   __shared__ dd s_cpart[8][2][kMomTerms];
+  const int role = blockIdx.x;
   if (threadIdx.x == 0) bad = 0;
   __syncthreads();
   prep_angular(a, L, blob, &bad);
-  check_radial_tables(a, &bad);
+  if (role == 0) check_radial_tables(a, &bad);
   __syncthreads();  // t, w written by this CTA are visible to it
-  prep_blocks_T(a, L, blob);
-  prep_series_T(a, L, blob);
-  if (L.off_gam >= 0) prep_tail_moments(a, L, blob, s_part);
-  {
+  if (role == 0) {
+    prep_series_T(a, L, blob);
+    if (L.off_rt >= 0) {  // point-dependent contours: levels 2 and 3 of the rule pyramid as given ("n arrays",
+                          // PAPER.md:150; levels 0 and 1 are mapped once per launch: REAL tables, rung tables)
+      const int lvl2 = a.n_rad + a.n_rad / 2;
+      for (int i = threadIdx.x; i < L.n_tab; i += blockDim.x) {
+        blob[L.off_rt + i] = a.rad_nodes[lvl2 + i];
+        blob[L.off_rw + i] = a.rad_weights[lvl2 + i];
+      }
+    }
+    __syncthreads();  // the T_k(s_j) matrix is complete
+    prep_series_sums(a, L, blob, s_cpart);
+    if (L.n_poly) prep_series_A(a, L, blob);
+    __syncthreads();
+    // Kreq from the tables the evaluation kernel will run: order 0's two, or the n + 2 of a Taylor order
+    if (L.n_poly) prep_series_kreq(L, blob, s_lc, blob + L.off_chebA, L.n_poly);
+    else prep_series_kreq(L, blob, s_lc, blob + L.off_cheb, 2);
+    if (threadIdx.x == 0) {
+      blob[0] = (double)bad;
+      blob[1] = a.ws_tag;
+      if (bad) report_status(a.status, bad);
+    }
+  } else if (role == 1) {
+    if (L.off_gam >= 0) prep_tail_moments(a, L, blob, s_part);
     // shifted-log map of [0, Lambda^2] (readings G3/G4): y(u) = s0 expm1(u L), dy/du = L (y + s0),
     // L = ln((Lambda^2 + s0)/s0) as a double-double from the host; y_i correctly rounded.
     const dd Llog = {a.Llog_hi, a.Llog_lo};
@@ -107,34 +133,18 @@ __global__ void __launch_bounds__(256) prep_real_kernel(const __grid_constant__ 
         }
       }
     }
-  }
-  if (L.off_rt >= 0) {  // point-dependent contours: levels 2 and 3 of the rule pyramid as given ("n arrays",
-                        // PAPER.md:150; levels 0 and 1 are mapped once per launch: REAL tables, rung tables)
-    const int lvl2 = a.n_rad + a.n_rad / 2;
-    for (int i = threadIdx.x; i < L.n_tab; i += blockDim.x) {
-      blob[L.off_rt + i] = a.rad_nodes[lvl2 + i];
-      blob[L.off_rw + i] = a.rad_weights[lvl2 + i];
+    __syncthreads();  // the monomial moments and the radial tables are complete
+    if (L.off_gam >= 0) {
+      prep_tail_gamma(L, blob, s_part, s_mu, s_nu);
+      const TailJob J = real_tail_job(a, L, blob);
+      prep_tail_powers(J);
+      __syncthreads();
+      prep_tail_sums(J);
     }
-  }
-  __syncthreads();  // the T_k(s_j) matrix, the monomial moments and the radial tables are complete
-  prep_blocks_sums(a, L, blob);
-  prep_series_sums(a, L, blob, s_cpart);
-  if (L.n_poly) prep_series_A(a, L, blob);
-  __syncthreads();
-  // Kreq from the tables the evaluation kernel will run: order 0's two, or the n + 2 of a Taylor order
-  if (L.n_poly) prep_series_kreq(L, blob, s_lc, blob + L.off_chebA, L.n_poly);
-  else prep_series_kreq(L, blob, s_lc, blob + L.off_cheb, 2);
-  if (L.off_gam >= 0) {
-    prep_tail_gamma(L, blob, s_part, s_mu, s_nu);
-    const TailJob J = real_tail_job(a, L, blob);
-    prep_tail_powers(J);
+  } else {
+    prep_blocks_T(a, L, blob);
     __syncthreads();
-    prep_tail_sums(J);
-  }
-  if (threadIdx.x == 0) {
-    blob[0] = (double)bad;
-    blob[1] = a.ws_tag;
-    if (bad) report_status(a.status, bad);
+    prep_blocks_sums(a, L, blob);
   }
 }
 
@@ -463,7 +473,7 @@ int launch_prepare(const EvalArgs& a, int precision, double* blob, cudaStream_t 
   if (rc) return rc;
   if ((rc = check_variant(plan, precision))) return rc;
   if (a.taylor_order > 0 && plan.shared_nodes) return launch_taylor_prepare(a, plan, blob, stream);
-  prep_real_kernel<<<1, 256, 0, stream>>>(a, plan.layout, blob);
+  prep_real_kernel<<<kPrepRoles, kPrepThreads, 0, stream>>>(a, plan.layout, blob);
   if ((rc = check_cuda(cudaGetLastError(), "prep kernel launch"))) return rc;
   return plan.shared_nodes ? GF_OK : launch_prepare_rungs(a, plan, blob, stream);
 }
