@@ -65,11 +65,12 @@ __global__ void radial_map_kernel(double Lhi, double Llo, double s0, const doubl
 //   header [0] = status bits of the tables;  t, t_lo, w (folded rule);  series coefficients mom[k], cheb[k], Kreq;
 //   block tables of a split rule;  y_i, 1/(4 y_i);  pref_{r,i} = c0 Wr_i y_i D1(y_i) (-R_r/(y_i + mu_r));  the
 //   tail's gamma and Rhat tables.
-// Three CTAs with one role each, nothing exchanged between them (each folds the angular rule for itself: the same
-// values to the same places): 0 the series tables and the checks, 1 the radial tables and the tail's, 2 the block
-// tables.  Their chains of dependent double-double steps run side by side instead of one after the other.
+// Four CTAs with one role each, nothing exchanged between them (each folds the angular rule for itself: the same
+// values to the same places): 0 the series tables and the checks, 1 the radial tables and the tail's Rhat, 2 the
+// block tables, 3 the tail's gamma.  Their chains of dependent double-double steps run side by side instead of one
+// after the other.
 // ---------------------------------------------------------------------------------------------
-constexpr int kPrepThreads = 512, kPrepRoles = 3;
+constexpr int kPrepThreads = 1024, kPrepRoles = 4;
 __global__ void __launch_bounds__(kPrepThreads) prep_real_kernel(const __grid_constant__ EvalArgs a,
                                                                  const __grid_constant__ BlobLayout L,
                                                                  double* __restrict__ blob) {
@@ -80,7 +81,7 @@ __global__ void __launch_bounds__(kPrepThreads) prep_real_kernel(const __grid_co
   const int role = blockIdx.x;
   if (threadIdx.x == 0) bad = 0;
   __syncthreads();
-  prep_angular(a, L, blob, &bad);
+  if (role != 1) prep_angular(a, L, blob, &bad);   // (role 1 reads nothing of the angular rule)
   if (role == 0) check_radial_tables(a, &bad);
   __syncthreads();  // t, w written by this CTA are visible to it
   if (role == 0) {
@@ -106,7 +107,6 @@ __global__ void __launch_bounds__(kPrepThreads) prep_real_kernel(const __grid_co
       if (bad) report_status(a.status, bad);
     }
   } else if (role == 1) {
-    if (L.off_gam >= 0) prep_tail_moments(a, L, blob, s_part);
     // shifted-log map of [0, Lambda^2] (readings G3/G4): y(u) = s0 expm1(u L), dy/du = L (y + s0),
     // L = ln((Lambda^2 + s0)/s0) as a double-double from the host; y_i correctly rounded.
     const dd Llog = {a.Llog_hi, a.Llog_lo};
@@ -133,18 +133,21 @@ __global__ void __launch_bounds__(kPrepThreads) prep_real_kernel(const __grid_co
         }
       }
     }
-    __syncthreads();  // the monomial moments and the radial tables are complete
+    __syncthreads();  // the radial tables are complete
     if (L.off_gam >= 0) {
-      prep_tail_gamma(L, blob, s_part, s_mu, s_nu);
       const TailJob J = real_tail_job(a, L, blob);
       prep_tail_powers(J);
       __syncthreads();
       prep_tail_sums(J);
     }
-  } else {
+  } else if (role == 2) {
     prep_blocks_T(a, L, blob);
     __syncthreads();
     prep_blocks_sums(a, L, blob);
+  } else if (L.off_gam >= 0) {
+    prep_tail_moments(a, L, blob, s_part);
+    __syncthreads();  // the monomial moments are complete
+    prep_tail_gamma(L, blob, s_part, s_mu, s_nu);
   }
 }
 

@@ -1101,17 +1101,16 @@ struct TailJob {
   double2* R;
   double *s2, *s3;
 };
-// phase C: thread per node i: q_i^n, n = 1..kTailN, in double-double into the scratch (hi, lo) [n][i]
+// phase C: thread per node i: q_i^n, n = 1..kTailN, in double-double into the scratch as (hi, lo) [i][n] (n fastest:
+// phase D's warps hold 32 consecutive n of one node)
 __device__ void prep_tail_powers(const TailJob& J) {
-  double* qhi = J.s2;
-  double* qlo = qhi + (size_t)kTailN * J.n;
+  double2* q2 = reinterpret_cast<double2*>(J.s2);
   for (int i = threadIdx.x; i < J.n; i += blockDim.x) {
     dd q = {1.0, 0.0};
     if (i + 1 < J.n) q = dd_div(dd{J.y[i], 0.0}, dd{J.y[i + 1], 0.0});
     dd p = q;
     for (int n = 0; n < kTailN; ++n) {
-      qhi[(size_t)n * J.n + i] = p.hi;
-      qlo[(size_t)n * J.n + i] = p.lo;
+      q2[(size_t)i * kTailN + n] = make_double2(p.hi, p.lo);
       p = dd_mul(p, q);
     }
   }
@@ -1120,15 +1119,14 @@ __device__ void prep_tail_powers(const TailJob& J) {
 // threads share it: item = (pole r, power n + 1, real / imaginary part), run c.  Pass 1 runs the recurrence inside
 // each run from 0 (L_c(i)) with the run's product of q (Q_c(i)); pass 2 folds the runs above c into the carry
 // Rhat(end of run c) in double-double and completes Rhat(i) = L_c(i) + Q_c(i) carry.
-constexpr int kTailChunks = 8;
+constexpr int kTailChunks = 16;
 __device__ void prep_tail_sums(const TailJob& J) {
-  const double* qhi = J.s2;
-  const double* qlo = qhi + (size_t)kTailN * J.n;
+  const double2* q2 = reinterpret_cast<const double2*>(J.s2);
   double2* R = J.R;
   const int n_items = 2 * J.n_pref * kTailN, CL = (J.n + kTailChunks - 1) / kTailChunks;
-  double* Qs = J.s3;                                                   // Q_c(i), [kTailN][n]
-  dd* Lstart = reinterpret_cast<dd*>(Qs + (size_t)kTailN * J.n);       // [n_items][kTailChunks]
-  dd* Qstart = Lstart + (size_t)n_items * kTailChunks;                 // [kTailN][kTailChunks]
+  double* Qs = J.s3;                                                   // Q_c(i), [n][kTailN]
+  dd* Lstart = reinterpret_cast<dd*>(Qs + (size_t)kTailN * J.n);       // [kTailChunks][n_items]
+  dd* Qstart = Lstart + (size_t)n_items * kTailChunks;                 // [kTailChunks][kTailN]
   for (int w = threadIdx.x; w < n_items * kTailChunks; w += blockDim.x) {
     const int e = w % n_items, c = w / n_items;
     const int part = e / (J.n_pref * kTailN), r = (e / kTailN) % J.n_pref, n = e % kTailN;
@@ -1136,17 +1134,31 @@ __device__ void prep_tail_sums(const TailJob& J) {
     const bool owner = r == 0 && part == 0;
     if (c == 0) Rr[2 * ((size_t)J.n * kTailN + n)] = 0.0;
     dd acc = {0.0, 0.0}, Q = {1.0, 0.0};
-    for (int i = min((c + 1) * CL, J.n) - 1; i >= c * CL; --i) {
-      const dd q = {qhi[(size_t)n * J.n + i], qlo[(size_t)n * J.n + i]};
-      acc = dd_add_d(dd_mul(acc, q), J.pref[2 * (r * J.stride + i) + part]);
+    // the next node's operands are fetched before this node's result is stored (the stores could alias the loads
+    // as far as the compiler knows: without this every step would wait a whole L2 round trip)
+    const int i_hi = min((c + 1) * CL, J.n) - 1, i_lo = c * CL;
+    double2 nq = make_double2(0.0, 0.0);
+    double np = 0.0;
+    if (i_hi >= i_lo) {
+      nq = q2[(size_t)i_hi * kTailN + n];
+      np = J.pref[2 * (r * J.stride + i_hi) + part];
+    }
+    for (int i = i_hi; i >= i_lo; --i) {
+      const dd q = {nq.x, nq.y};
+      const double pf = np;
+      if (i > i_lo) {
+        nq = q2[(size_t)(i - 1) * kTailN + n];
+        np = J.pref[2 * (r * J.stride + i - 1) + part];
+      }
+      acc = dd_add_d(dd_mul(acc, q), pf);
       Rr[2 * ((size_t)i * kTailN + n)] = acc.hi;
       if (owner) {
         Q = dd_mul(Q, q);
-        Qs[(size_t)n * J.n + i] = Q.hi;
+        Qs[(size_t)i * kTailN + n] = Q.hi;
       }
     }
-    Lstart[(size_t)e * kTailChunks + c] = acc;
-    if (owner) Qstart[(size_t)n * kTailChunks + c] = Q;
+    Lstart[(size_t)c * n_items + e] = acc;
+    if (owner) Qstart[(size_t)c * kTailN + n] = Q;
   }
   __syncthreads();
   for (int w = threadIdx.x; w < n_items * kTailChunks; w += blockDim.x) {
@@ -1155,12 +1167,22 @@ __device__ void prep_tail_sums(const TailJob& J) {
     double* Rr = reinterpret_cast<double*>(R + (size_t)r * (J.n + 1) * kTailN) + part;
     dd carry = {0.0, 0.0};
     for (int cc = kTailChunks - 1; cc > c; --cc)
-      carry = dd_add(Lstart[(size_t)e * kTailChunks + cc], dd_mul(Qstart[(size_t)n * kTailChunks + cc], carry));
-    if (carry.hi != 0.0 || carry.lo != 0.0)
-      for (int i = min((c + 1) * CL, J.n) - 1; i >= c * CL; --i) {
-        const size_t at = 2 * ((size_t)i * kTailN + n);
-        Rr[at] = dd_add_d(dd_mul_d(carry, Qs[(size_t)n * J.n + i]), Rr[at]).hi;
+      carry = dd_add(Lstart[(size_t)cc * n_items + e], dd_mul(Qstart[(size_t)cc * kTailN + n], carry));
+    if (carry.hi != 0.0 || carry.lo != 0.0) {
+      const int i_hi = min((c + 1) * CL, J.n) - 1, i_lo = c * CL;
+      for (int ib = i_hi; ib >= i_lo; ib -= 4) {   // four independent nodes: loads first, then the stores
+        double qv[4], rv[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          if (ib - u >= i_lo) {
+            qv[u] = Qs[(size_t)(ib - u) * kTailN + n];
+            rv[u] = Rr[2 * ((size_t)(ib - u) * kTailN + n)];
+          }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          if (ib - u >= i_lo) Rr[2 * ((size_t)(ib - u) * kTailN + n)] = dd_add_d(dd_mul_d(carry, qv[u]), rv[u]).hi;
       }
+    }
   }
 }
 // the REAL contour's job: all n_rad nodes of the prepared block
