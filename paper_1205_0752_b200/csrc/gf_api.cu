@@ -136,8 +136,8 @@ double workspace_tag(const gf_params* p, int n_rad, int n_ang) {
 }
 
 // per (point, node, pole) FP64-pipe instructions of each route's set-up + finish (SASS of eval_real_kernel<double>)
-constexpr double kNodeNearDfma = 12, kNodeNearOther = 13, kNodeMomentDfma = 21, kNodeMomentOther = 13,
-                 kNodeChebDfma = 34, kNodeChebOther = 33;
+constexpr double kNodeNearDfma = 12, kNodeNearOther = 13, kNodeMomentDfma = 21, kNodeMomentOther = 15,
+                 kNodeChebDfma = 31, kNodeChebOther = 28;
 
 bool finite_prop(const gf_propagator& p) {
   return std::isfinite(p.m2_re) && std::isfinite(p.m2_im) && std::isfinite(p.M2) && std::isfinite(p.a) &&
@@ -661,11 +661,12 @@ int gf_eval_launch_info(const gf_params* p, int n_rad, int n_ang, long long n_po
     return GF_OK;
   }
   // FP64-pipe instructions per unit of each route, counted per SASS region in the ncu source page of
-  // eval_real_kernel<double, false, 1> (profiles/r01h_eval_ncu_full.md; DSETP not counted: no flops):
+  // eval_real_kernel<double, false, 1, true, false> (profiles/r02c_eval_ncu_full.md; DSETP not counted: no flops):
   //   pair of the plain direct loop 5 DFMA + 1 DMUL + 2 DADD, of the double-double loop 5 + 1 + 4;
   //   series term (P and N): 4 DFMA;
   //   every node-term: zeta, delta (5 DFMA + 3 DMUL + 1 DADD) and the accumulation into G (4 DFMA);
-  //   MOMENT adds 4 + 5 (set-up) and 8 + 4 (finish), CHEB 17 + 25 and 8 + 4, the direct loops 3 + 9,
+  //   MOMENT adds 4 + 5 (set-up) and 8 + 4 (finish), CHEB 14 + 18 and 8 + 4, both 2 DADD (2 Re s at the head of the
+  //   FP32 and of the FP64 phase of the series loop), the direct loops 3 + 9,
   //   EXACT lanes the double-double zeta (29 + 217);
   //   tail per (point, pole): 2 DFMA per coefficient (kTailN (kTailN + 1)), 8 + 9 per n, the per-point set-up.
   const bool f32 = p->precision == 32;

@@ -43,6 +43,7 @@
 //  * One thread owns one grid point (or 1/S of its radial nodes when the grid is too small to fill 148
 //    SMs; the S lanes are merged with warp shuffles); the node loop is warp-synchronous (the series loop
 //    of node_term runs to the warp's longest series); results leave as coalesced 16-byte stores.
+#include <cstdlib>
 #include <cfloat>
 #include <cmath>
 #include <cstdint>
@@ -324,12 +325,19 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
   L.kmc = kKmc;
   long long o = 2;  // header
   auto take = [&](long long n) { long long at = o; o += (n + 1) & ~1LL; return at; };
-  L.off_t = (int)take(L.npad);
-  L.off_tlo = (int)take(L.npad);
-  L.off_w = (int)take(L.npad);
+  // the tables every node-term reads come first, at offsets known at compile time (kOffMom ... kOffSf: the kernels
+  // address them as one base plus immediates); four entries of slack below the float2 series tables (the
+  // software-pipelined loop reads them on its last trip), 2 float2 tables of kmc entries = 2 kmc doubles
   L.off_mom = (int)take(2 * L.kmc);
   L.off_cheb = (int)take(2 * L.kmc);
   L.off_kreq = (int)take(kKreqBins / 2);
+  take(4);
+  L.off_sf = (int)take(2 * L.kmc);
+  static_assert(kOffSf % 2 == 0, "float2 tables must be 16-byte aligned");
+  if (L.off_mom != kOffMom || L.off_cheb != kOffCheb || L.off_kreq != kOffKreq || L.off_sf != kOffSf) abort();
+  L.off_t = (int)take(L.npad);
+  L.off_tlo = (int)take(L.npad);
+  L.off_w = (int)take(L.npad);
   L.n_rad_pad = (n_rad + 31) & ~31;
   L.n_pref = n_terms + (sym && tail ? 1 : 0);
   auto take_nodes = [&]() {
@@ -338,10 +346,7 @@ BlobLayout make_blob_layout(int n_rad, int n_pairs, int n_terms, bool f32, bool 
     L.off_pref = (int)take(2 * L.n_pref * L.n_rad_pad);
   };
   if (!pyramid) take_nodes();
-  // four entries of slack below the float2 series tables (the software-pipelined loop reads them on its last trip),
-  // then 2 float2 tables of kmc entries = 2 kmc doubles; FP32 variant: 2 float tables of npad entries = npad doubles
-  take(4);
-  L.off_sf = (int)take(2 * L.kmc);
+  // FP32 variant: 2 float tables of npad entries = npad doubles
   L.off_f32 = f32 ? (int)take(L.npad) : -1;
   L.n_tab = pyramid ? n_rad / 4 + n_rad / 8 : 0;
   L.off_rt = pyramid ? (int)take(L.n_tab) : -1;

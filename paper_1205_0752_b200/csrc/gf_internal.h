@@ -70,7 +70,7 @@ struct EvalArgs {
 };
 // codes a kernel leaves in *status (the next API call of the device returns GF_ERR_ARG and describes it)
 enum { kStatusAsymmetricRule = 1, kStatusRadialNodes = 2, kStatusWorkspace = 4 };
-constexpr int kLayoutVersion = 11;   // bump when a BlobLayout or the meaning of a table changes
+constexpr int kLayoutVersion = 12;   // bump when a BlobLayout or the meaning of a table changes
 
 // Offsets (in doubles) of the prepared tables, as the preparation kernel writes them and every CTA of the
 // evaluation kernel copies them to shared memory (one 16-byte header first).

@@ -15,6 +15,9 @@ namespace gf {
 namespace {
 
 constexpr int kKmc = 256;             // series coefficients staged per table (even)
+// fixed places of the series tables in the staged block, in doubles (make_blob_layout)
+constexpr int kOffMom = 2, kOffCheb = kOffMom + 2 * kKmc, kOffKreq = kOffCheb + 2 * kKmc,
+              kOffSf = kOffKreq + kKreqBins / 2 + 4;
 constexpr int kMomTerms = 32;         // genuine coefficients of the centred-moment series (zero beyond)
 #ifndef GF_SERIES_BITS
 #define GF_SERIES_BITS 46
@@ -231,11 +234,12 @@ __device__ __forceinline__ Tabs<T> make_tabs(const double* sb, const BlobLayout&
     tb.mom = reinterpret_cast<const V2*>(sb + L.off_sf);
     tb.cheb = tb.mom + L.kmc;
   }
-  tb.a_kreq = smem_u32(sb + L.off_kreq);
-  tb.a_mom = smem_u32(sb + L.off_mom);
-  tb.a_momf = smem_u32(sb + L.off_sf);
-  tb.kreq = reinterpret_cast<const int*>(sb + L.off_kreq);
-  tb.mu0 = sb[L.off_mom];  // a_0 of the moment series = sum of the folded weights
+  const uint32_t base = smem_u32(sb);   // one base, immediates from the fixed layout
+  tb.a_kreq = base + 8u * kOffKreq;
+  tb.a_mom = base + 8u * kOffMom;
+  tb.a_momf = base + 8u * kOffSf;
+  tb.kreq = reinterpret_cast<const int*>(sb + kOffKreq);
+  tb.mu0 = sb[kOffMom];  // a_0 of the moment series = sum of the folded weights
   tb.n_pairs = n_pairs;
   tb.kmc = L.kmc;
   tb.n_blk = L.n_blk;
