@@ -202,6 +202,24 @@ int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_
                  const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
                  long long n_points, void* d_out, void* stream);
 
+/* gf_eval_grid for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the same arguments, the same kernels, the same results, but the workspace of the prepared tables
+ * is a static device array of GF_STATIC_WORKSPACE_BYTES inside the library instead of stream-ordered scratch.  It calls
+ * no cudaMalloc, cudaFree, memory-pool or host-allocation routine.
+ *   Limit: parameters and orders whose gf_eval_workspace_size() exceeds GF_STATIC_WORKSPACE_BYTES are refused with
+ *          GF_ERR_ARG and a message that names both sizes (the configs of this repository need 0.2 to 26 MiB).
+ *   Cost:  every GPU that loads the library holds the array until the process exits.
+ *   Sharing: every call on a device uses the same array, which keeps the last call's tables (each call rewrites all
+ *          it reads and resets the header first).  Calls that OVERLAP on the GPU (two streams, two host threads) race on
+ *          it: issue them on one stream, or order them with events.  Other devices have their own copy.
+ *   Errors: as gf_eval_grid, except that bad TABLES (an asymmetric angular rule, radial nodes out of order) show as NaN
+ *          results only: this entry point does not use the mapped status word of "Bad input" above (it would have to
+ *          allocate it).  precision 32 / 64, every contour policy, routing, dim and taylor_order as gf_eval_grid. */
+#define GF_STATIC_WORKSPACE_BYTES (32ll << 20)
+int gf_eval_grid_static(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                        const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
+                        long long n_points, void* d_out, void* stream);
+
 /* The two halves of gf_eval_grid, for callers that evaluate several grids with the same parameters and rules
  * (and for benchmarks that time the evaluation kernel alone).  gf_eval_prepare makes every table that does not
  * depend on x (folded angular rule, series coefficients, radial nodes and prefactors, tail tables) into the

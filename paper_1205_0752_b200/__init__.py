@@ -68,6 +68,7 @@ _SIGNATURES = {
     "gf_make_quadrature_dim_host": [_int, _int, _dbl, _dbl, _vp, _vp],
     "gf_radial_table_size": [_int, _int],
     "gf_eval_grid": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
+    "gf_eval_grid_static": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
     "gf_eval_grid_counted": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp, _vp],
     "gf_eval_grid_host": [ctypes.POINTER(gf_params), _vp, _vp, _int, _vp, _vp, _int, _vp, _ll, _vp, _vp],
     "gf_eval_workspace_size": [ctypes.POINTER(gf_params), _int, _int],
@@ -274,6 +275,21 @@ def eval_grid(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, 
         _check(lib().gf_eval_grid(ctypes.byref(params), rad_nodes.data_ptr(), rad_weights.data_ptr(), n_rad,
                                   ang_nodes.data_ptr(), ang_weights.data_ptr(), ang_nodes.numel(),
                                   x.data_ptr(), x.numel(), out.data_ptr(), _stream(stream)))
+    return out
+
+
+STATIC_WORKSPACE_BYTES = 32 << 20   # GF_STATIC_WORKSPACE_BYTES of include/gf.h
+
+
+def eval_grid_static(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out=None, stream=None):
+    """gf_eval_grid_static: gf_eval_grid with the library's static device workspace (no allocation inside the
+    library; pass `out` to allocate nothing here either).  Refuses workspaces beyond STATIC_WORKSPACE_BYTES; calls that
+    overlap on the GPU race on the workspace (include/gf.h)."""
+    out = _eval_checks(params, rad_nodes, rad_weights, n_rad, ang_nodes, ang_weights, x, out)
+    with torch.cuda.device(x.device):
+        _check(lib().gf_eval_grid_static(ctypes.byref(params), rad_nodes.data_ptr(), rad_weights.data_ptr(), n_rad,
+                                         ang_nodes.data_ptr(), ang_weights.data_ptr(), ang_nodes.numel(),
+                                         x.data_ptr(), x.numel(), out.data_ptr(), _stream(stream)))
     return out
 
 

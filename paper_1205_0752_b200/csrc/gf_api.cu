@@ -724,3 +724,77 @@ int gf_diag_dfma_issue(int mode, int blocks, int threads, long long iters, doubl
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// gf_eval_grid_static: gf_eval_grid for callers that cannot allocate (code under CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc).  The workspace of the prepared tables is a file-scope device array of
+// GF_STATIC_WORKSPACE_BYTES that every GPU loading this library holds until the process exits; the entry point calls
+// no cudaMalloc / cudaFree / pool routine and no mapped host word (status = NULL: bad tables show as NaN results only).
+// In host code the array's NAME is a host-side stand-in, not a device address: the address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_static_workspace[GF_STATIC_WORKSPACE_BYTES / sizeof(double)];
+
+// Device code may name the array directly.  The header (status bits of the tables, hash tag) is what a kernel reads
+// first from a workspace: it starts every call at zero, whatever the last call left there.
+static __global__ void static_workspace_reset_kernel() {
+  g_static_workspace[0] = 0.0;
+  g_static_workspace[1] = 0.0;
+}
+
+static double* g_static_ptr[64] = {};
+static std::mutex g_static_mutex;
+
+static int static_workspace(double** ptr) {
+  int dev = 0;
+  int rc = check_cuda(cudaGetDevice(&dev), "cudaGetDevice");
+  if (rc) return rc;
+  if (dev < 0 || dev >= 64) { set_error("device ordinal %d out of range", dev); return GF_ERR_CUDA; }
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_ptr[dev]) {
+    double* d = nullptr;
+    if ((rc = check_cuda(cudaGetSymbolAddress(reinterpret_cast<void**>(&d), g_static_workspace),
+                         "cudaGetSymbolAddress(static workspace)")))
+      return rc;
+    if (!d) { set_error("eval_grid_static: the static workspace has no device address"); return GF_ERR_CUDA; }
+    g_static_ptr[dev] = d;
+  }
+  *ptr = g_static_ptr[dev];
+  return GF_OK;
+}
+
+extern "C" int gf_eval_grid_static(const gf_params* p, const double* d_rad_nodes, const double* d_rad_weights, int n_rad,
+                                   const double* d_ang_nodes, const double* d_ang_weights, int n_ang, const void* d_x,
+                                   long long n_points, void* d_out, void* stream) {
+  return no_throw("eval_grid_static", [&] {
+    EvalArgs a;
+    int rc = build_args(p, n_rad, n_ang, n_points, &a);
+    if (rc) return rc;
+    if (!d_rad_nodes || !d_rad_weights || !d_ang_nodes || !d_ang_weights) { set_error("eval_grid_static: null table pointer"); return (int)GF_ERR_NULL; }
+    if (n_points > 0 && (!d_x || !d_out)) { set_error("eval_grid_static: null grid/output pointer"); return (int)GF_ERR_NULL; }
+    LaunchPlan plan;
+    if ((rc = plan_eval(a, p->precision, &plan))) return rc;
+    const long long need = (long long)plan.layout.n_total * (long long)sizeof(double);
+    if (need > (long long)GF_STATIC_WORKSPACE_BYTES) {
+      set_error("eval_grid_static: these parameters and orders need a workspace of %lld bytes; the static workspace "
+                "holds GF_STATIC_WORKSPACE_BYTES = %lld (use gf_eval_grid, or gf_eval_prepare with a workspace of the caller's)",
+                need, (long long)GF_STATIC_WORKSPACE_BYTES);
+      return (int)GF_ERR_ARG;
+    }
+    if (n_points == 0) return (int)GF_OK;
+    double* blob = nullptr;
+    if ((rc = static_workspace(&blob))) return rc;
+    a.status = nullptr;
+    a.rad_nodes = d_rad_nodes;
+    a.rad_weights = d_rad_weights;
+    a.ang_nodes = d_ang_nodes;
+    a.ang_weights = d_ang_weights;
+    a.x = static_cast<const double2*>(d_x);
+    a.out = d_out;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    static_workspace_reset_kernel<<<1, 1, 0, s>>>();
+    if ((rc = check_cuda(cudaGetLastError(), "static workspace reset launch"))) return rc;
+    if ((rc = launch_prepare(a, p->precision, blob, s))) return rc;
+    return launch_prepared(a, p->precision, blob, nullptr, s);
+  });
+}
