@@ -275,10 +275,11 @@ __global__ void __launch_bounds__(kBlockThreads, GF_MIN_BLOCKS)
       const cd zeta = {fma(C1x4[r].re, q4, fma(C3.re, y, C2[r].re)), fma(C1x4[r].im, q4, fma(C3.im, y, C2[r].im))};
       // (the lo parts of a rational line's poles matter where a contour passes next to y = -mu: not on the real axis)
       const cd s = node_term<T, COUNT, BLK>(tb, xz, cd{y, 0.0}, delta, zeta, a.term[r].mu_re, a.term[r].mu_im, rc);
-      double2 pr = ppref[r * L.n_rad_pad];
-      if (!on) pr = make_double2(0.0, 0.0);
-      g_re = fma(pr.x, s.re, fma(-pr.y, s.im, g_re));
-      g_im = fma(pr.x, s.im, fma(pr.y, s.re, g_im));
+      const double2 pr = ppref[r * L.n_rad_pad];
+      if (on) {   // (four predicated DFMA; an idle lane's s may be anything)
+        g_re = fma(pr.x, s.re, fma(-pr.y, s.im, g_re));
+        g_im = fma(pr.x, s.im, fma(pr.y, s.re, g_im));
+      }
     }
   }
   if (L.off_gam >= 0 && __any_sync(0xffffffffu, i_end < a.n_rad)) {

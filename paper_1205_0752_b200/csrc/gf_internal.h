@@ -70,7 +70,7 @@ struct EvalArgs {
 };
 // codes a kernel leaves in *status (the next API call of the device returns GF_ERR_ARG and describes it)
 enum { kStatusAsymmetricRule = 1, kStatusRadialNodes = 2, kStatusWorkspace = 4 };
-constexpr int kLayoutVersion = 12;   // bump when a BlobLayout or the meaning of a table changes
+constexpr int kLayoutVersion = 13;   // bump when a BlobLayout or the meaning of a table changes
 
 // Offsets (in doubles) of the prepared tables, as the preparation kernel writes them and every CTA of the
 // evaluation kernel copies them to shared memory (one 16-byte header first).
@@ -79,7 +79,7 @@ struct BlobLayout {
   int kmc;                      // series coefficients k = 0 .. kmc-1 (even)
   int off_t, off_tlo, off_w;    // folded angular rule: t = z^2 (hi, lo), weight
   int off_mom, off_cheb;        // double2 (P_k, N_k)[kmc]: centred-moment series, Chebyshev series
-  int off_kreq;                 // int Kreq[kKreqBins]: Chebyshev terms needed per bin of log2(rho)
+  int off_kreq;                 // int Kreq[kKreqBins]: entry 0 "no series", entry 1 + b the Chebyshev terms needed in bin b of log2(rho)
   int n_rad_pad;                // n_rad rounded up to 32: padding repeats the last node with prefactor 0
   int off_y, off_q4;            // radial nodes y_i, 1/(4 y_i), n_rad_pad each
   int n_pref;                   // rows of node prefactors: n_terms, + 1 for the symmetric routing's second tail table

@@ -587,9 +587,6 @@ cd angular_blocked(cd eta, ZetaDD z, const Tabs<double>& tb, RouteCount& rc) {
 //   EXACT   zeta within tau of [0,1];   NEAR  the rest (zeta close to [0,1], or few angular nodes).
 // ---------------------------------------------------------------------------------------------
 // The series argument of one (point, radial node, pole), as route_setup leaves it
-#ifndef GF_CHEB_DIRECT_S
-#define GF_CHEB_DIRECT_S 1
-#endif
 struct SeriesArg {
   cd sg, g;     // series argument s and prefactor
   double ns;    // -|s|^2
@@ -631,37 +628,22 @@ __device__ __forceinline__ SeriesArg route_setup(const Tabs<T>& tb, cd zeta) {
     const int flip = __double2hiint(fma(wr, ar, wi * ai)) & 0x80000000;   // Re(conj(w) root) < 0: the other root
     ar = __hiloint2double(__double2hiint(ar) ^ flip, __double2loint(ar));
     ai = __hiloint2double(__double2hiint(ai) ^ flip, __double2loint(ai));
-#if GF_CHEB_DIRECT_S
     // s = 1/(w + 2 root) = w - 2 root exactly ((w + 2 root)(w - 2 root) = w^2 - (w^2 - 1)): no reciprocal.  The
     // difference cancels |w|/|s| <= 2 |w|^2 of its operands' digits; |w| < 14 on this route (MOMENT beyond)
     const double sr = fma(-2.0, ar, wr), si = fma(-2.0, ai, wi);
     const double ns = fma(-sr, sr, -(si * si));        // -|s|^2 = -1/rho^2
-    const float ell = -0.5f * lg2_ftz(fabsf((float)ns));   // log2(rho)
-    int kq = 0xffff;
-    if (ell >= kEllLo)
-      asm volatile("ld.shared.s32 %0, [%1];" : "=r"(kq)
-                   : "r"(tb.a_kreq + 4u * (uint32_t)min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)));
+    // terms needed at this rho (table made from the coefficients themselves, prep_series_kreq): entry 0 says "no usable
+    // series" (log2 rho below kEllLo; zeta on [0,1] itself gives rho = 1 or NaN: entry 0 too), entry 1 + b is bin b.
+    // index = floor((log2 rho - kEllLo)/kEllStep) + 1 by one FFMA from log2 |s|^2 and a conversion rounding down
+    // (a NaN converts to 0), clamped: no comparison, no branch
+    const float fidx = fmaf(lg2_ftz(fabsf((float)ns)), -0.5f / kEllStep, 1.f - kEllLo / kEllStep);
+    int kq;
+    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(kq)
+                 : "r"(tb.a_kreq + 4u * (uint32_t)min(max(__float2int_rd(fidx), 0), kKreqBins - 1)));
     o.K = kq & 0xffff;     // 0xffff: no usable series in this bin
     o.K1 = kq >> 16;
     o.sg = {sr, si};
     o.ns = ns;
-#else
-    const double Dr = fma(2.0, ar, wr), Di = fma(2.0, ai, wi);
-    const double rho2 = fma(Dr, Dr, Di * Di);
-    // terms needed at this rho (table made from the coefficients themselves, prep_series_kreq); taken from rho^2
-    // directly so that the look-up does not wait for the reciprocal.  zeta on [0,1] itself gives rho = 1 or NaN:
-    // the comparison fails, never CHEB
-    const float ell = 0.5f * lg2_ftz((float)rho2);     // log2(rho)
-    int kq = 0xffff;
-    if (ell >= kEllLo)
-      asm volatile("ld.shared.s32 %0, [%1];" : "=r"(kq)
-                   : "r"(tb.a_kreq + 4u * (uint32_t)min((int)((ell - kEllLo) * (1.f / kEllStep)), kKreqBins - 1)));
-    o.K = kq & 0xffff;     // 0xffff: no usable series in this bin
-    o.K1 = kq >> 16;
-    const double in = rcp_fast(rho2);                  // 1/rho^2
-    o.sg = {Dr * in, -Di * in};
-    o.ns = -in;
-#endif
     const double g2 = rm + rm;                   // 4/sqrt(w^2-1) = 2 conj(root)/|q|
     o.g = {ar * g2, -ai * g2};
     o.route = ROUTE_CHEB;
@@ -1011,7 +993,8 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc 
   for (int j = threadIdx.x; j < L.kmc; j += blockDim.x)   // log2 |c_j / c_0|, rounded up a little (c = 0: -inf)
     s_lc[j] = (float)log2(cmax(j) / c00) + 1e-3f;
   __syncthreads();
-  for (int b = threadIdx.x; b < kKreqBins; b += blockDim.x) {
+  if (threadIdx.x == 0) kreq[0] = 0xffff;   // entry 0: log2(rho) below kEllLo, no usable series (route_setup)
+  for (int b = threadIdx.x; b < kKreqBins - 1; b += blockDim.x) {
     const float ell = kEllLo + (float)b * kEllStep;
     int K = 0xffff, K1 = 0;
     if (ell * L.kmc >= 60.f) {
@@ -1037,7 +1020,7 @@ __device__ void prep_series_kreq(const BlobLayout& L, double* blob, float* s_lc 
         }
       K1 = min((K1 + 3) & ~3, K);
     }
-    kreq[b] = K | (K1 << 16);
+    kreq[b + 1] = K | (K1 << 16);
   }
 }
 
