@@ -91,7 +91,9 @@ __global__ void __launch_bounds__(256) prep_rungs_kernel(const __grid_constant__
 #ifndef GF_CONTOUR_MIN_BLOCKS
 #define GF_CONTOUR_MIN_BLOCKS 4
 #endif
-template <bool COUNT, int NT, bool BLK>
+// POL >= 0: every point of the launch walks this policy (an explicit gf_params.contour), known at compile time: the
+// other policies' code and registers are gone; POL = -1: the policy is each point's own (AUTO)
+template <bool COUNT, int NT, bool BLK, int POL>
 __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
     eval_contour_kernel(const __grid_constant__ EvalArgs a, const __grid_constant__ BlobLayout L,
                         const double* __restrict__ blob, unsigned long long* __restrict__ counters) {
@@ -143,7 +145,8 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
   const double d0 = sym ? 0.25 : 0.0, dmu = sym ? 2.0 : 1.0;   // delta = d0 + (x + dmu mu)/(4y)
   const cd xinv = cinv(x);
 
-  const Geo geo = build_geo(a, x.re, x.im);
+  const Geo geo = build_geo(a, x.re, x.im, POL);
+  const int pol = POL >= 0 ? POL : geo.pol;
   const cd dir2 = ray_measure_dir(a, geo);   // dir^2 in d = 4
   // One pole (NT == 1): on a piece y = dir r with real r from a table (the ray; dir = 1 on the real pieces)
   //   zeta = (x + mu + y)^2/(4 x y) = Z1/(4r) + C2 + Z3 r,  Z1 = (x + mu)^2/x conj(dir), C2 = (x + mu)/(2x), Z3 = dir/(4x)
@@ -163,13 +166,13 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
   }
   // tables of the real nodes this point walks: the REAL contour's (policy REAL) or its rung's tail piece
   const double* row = blob + L.off_rung + (long long)geo.row * L.rung_stride;
-  const bool real_pol = geo.pol == GF_CONTOUR_REAL;
+  const bool real_pol = pol == GF_CONTOUR_REAL;
   const double* ty = real_pol ? blob + L.off_y : row + L.rg_y;
   const double* tq4 = real_pol ? blob + L.off_q4 : row + L.rg_yq4;
   const double2* tpref = reinterpret_cast<const double2*>(real_pol ? blob + L.off_pref : row + L.rg_pref);
   const int tstride = real_pol ? L.n_rad_pad : L.n4p;
   const int tn = real_pol ? a.n_rad : a.n_rad >> 2;
-  const int t0 = tail_start(geo.pol, a.n_rad);
+  const int t0 = tail_start(pol, a.n_rad);
 
   // where the tail series takes over: the first real node with y >= Y0 = 4 (sqrt|x| + sqrt(|x| + |x + mu|))^2
   int i_end;
@@ -201,7 +204,7 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
   for (int g0 = 0; g0 < g_stop; g0 += S) {
     const bool valid = g0 + sub < g_end;
     const int g = valid ? g0 + sub : g_end - 1 + (g_end == 0);
-    const NodeAt at = locate(geo.pol, a.n_rad, g);
+    const NodeAt at = locate(pol, a.n_rad, g);
     // ---- the node: y, 1/(4y), and the prefactor c0 (rule weight) dy/dt y D1(y) without the pole factors
     cd y, q4, base = {0.0, 0.0};
     const bool table = at.type == SEG_TABLE || at.type == SEG_TAIL;
@@ -276,9 +279,10 @@ __global__ void __launch_bounds__(kBlockThreads, GF_CONTOUR_MIN_BLOCKS)
         pr = NT == 1 ? cd{-base.re, -base.im} : cmul(base, cd{-a.term[r].R_re, -a.term[r].R_im});
         pr = cmul(pr, ic);
       }
-      if (!valid) pr = {0.0, 0.0};
-      g_re = fma(pr.re, s.re, fma(-pr.im, s.im, g_re));
-      g_im = fma(pr.re, s.im, fma(pr.im, s.re, g_im));
+      if (valid) {   // (four predicated DFMA)
+        g_re = fma(pr.re, s.re, fma(-pr.im, s.im, g_re));
+        g_im = fma(pr.re, s.im, fma(pr.im, s.re, g_im));
+      }
     }
   }
   // the large-y part of the real piece, all nodes from i_end on at once
@@ -352,10 +356,10 @@ __global__ void contour_nodes_kernel(const __grid_constant__ EvalArgs a, const _
   out_wy[g] = make_double2(wy.re, wy.im);
 }
 
-template <bool COUNT, int NT, bool BLK>
-int launch_contour_t(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
-                     cudaStream_t stream) {
-  auto kern = eval_contour_kernel<COUNT, NT, BLK>;
+template <bool COUNT, int NT, bool BLK, int POL>
+int launch_contour_kern(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
+                        cudaStream_t stream) {
+  auto kern = eval_contour_kernel<COUNT, NT, BLK, POL>;
   if (plan.smem_bytes > 48 * 1024) {
     int rc = check_cuda(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes),
                         "cudaFuncSetAttribute(max dynamic shared memory)");
@@ -363,6 +367,17 @@ int launch_contour_t(const EvalArgs& a, const LaunchPlan& plan, const double* bl
   }
   kern<<<(unsigned)plan.grid_blocks, plan.block_threads, plan.smem_bytes, stream>>>(a, plan.layout, blob, counters);
   return check_cuda(cudaGetLastError(), "contour kernel launch");
+}
+
+// the instantiations for one policy exist for the timed kernels only
+template <bool COUNT, int NT, bool BLK>
+int launch_contour_t(const EvalArgs& a, const LaunchPlan& plan, const double* blob, unsigned long long* counters,
+                     cudaStream_t stream) {
+  if constexpr (!COUNT) {
+    if (a.contour == GF_CONTOUR_RAY_ARC) return launch_contour_kern<COUNT, NT, BLK, GF_CONTOUR_RAY_ARC>(a, plan, blob, counters, stream);
+    if (a.contour == GF_CONTOUR_THREAD) return launch_contour_kern<COUNT, NT, BLK, GF_CONTOUR_THREAD>(a, plan, blob, counters, stream);
+  }
+  return launch_contour_kern<COUNT, NT, BLK, -1>(a, plan, blob, counters, stream);
 }
 
 }  // namespace

@@ -102,9 +102,10 @@ __device__ __forceinline__ int auto_policy(const EvalArgs& a, double xr, double 
   return GF_CONTOUR_REAL;
 }
 
-__device__ __forceinline__ Geo build_geo(const EvalArgs& a, double xr, double xi) {
+// force_pol >= 0: the policy is known to the caller at compile time (a kernel instantiated for one policy)
+__device__ __forceinline__ Geo build_geo(const EvalArgs& a, double xr, double xi, int force_pol = -1) {
   Geo g = {};
-  g.pol = a.contour == GF_CONTOUR_AUTO ? auto_policy(a, xr, xi) : a.contour;
+  g.pol = force_pol >= 0 ? force_pol : a.contour == GF_CONTOUR_AUTO ? auto_policy(a, xr, xi) : a.contour;
   g.dre = 1.0;
   if (g.pol == GF_CONTOUR_RAY_ARC) {
     double ax;
