@@ -44,6 +44,8 @@ constexpr int kGoertzelUnroll = GF_GOERTZEL_UNROLL;   // trips of the series loo
 #endif
 constexpr int kNearUnroll = GF_NEAR_UNROLL;           // trips of the plain direct loop (4 pairs each) unrolled
 // MOMENT route when max(|Re zeta|, |Im zeta|) >= 4.5 (then |zeta - 1/2| >= 4), compared on the high words
+// (measured again with the cheaper CHEB set-up: from 6 or 8 the cfg3 kernel is 0.5 / 0.75 % faster, but CHEB's s = w - 2 root
+// loses 2 |w|^2 of its digits and the worst case of the random deformed-contour problems goes 3.2e-12 -> 5.8e-12: not taken)
 #ifndef GF_MOMENT_HIWORD
 #define GF_MOMENT_HIWORD 0x40120000
 #endif
