@@ -41,7 +41,7 @@ FP64_LANES_PER_SM = 64
 N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of one eval kernel launch on cfg3 (profiles/, ncu --set full);
 # None until a capture is committed
-EVAL_KERNEL_DRAM_TRAFFIC_BYTES = 102.7e6  # profiles/r02c_eval_ncu_full.md: 67.6 MB read + 35.1 MB written (134 MB algorithmic: x in, G out)
+EVAL_KERNEL_DRAM_TRAFFIC_BYTES = 102.9e6  # profiles/r02c_eval_ncu_full.md: 67.9 MB read + 34.9 MB written (134 MB algorithmic: x in, G out)
 
 
 def dist_env():
