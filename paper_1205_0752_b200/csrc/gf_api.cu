@@ -560,7 +560,7 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
   for (int c = 0; c < n_chunks && !rc; ++c) {
     // boundaries on multiples of the CTA size: every warp holds the same points as in one launch over all of x,
     // so the chunked result is bit-identical to gf_eval_grid's (the series loop runs to the warp's longest series)
-    auto cut = [&](int k) { return k >= n_chunks ? n_points : (n_points * k / n_chunks) & ~(long long)(kBlockThreads - 1); };
+    auto cut = [&](int k) { return k >= n_chunks ? n_points : (n_points * k / n_chunks) / kBlockThreads * kBlockThreads; };
     const long long p0 = cut(c), p1 = cut(c + 1), np = p1 - p0;
     // odd chunks are evaluated on a second stream, so that the last, partly filled wave of CTAs of one chunk
     // overlaps the first waves of the next
