@@ -281,6 +281,26 @@ def test_ragged_point_counts(gf, oracle, n_points):
     assert relerr(g[keep], ref).max() <= TOL64
 
 
+def test_kernel_instantiations_agree_bit_for_bit(gf):
+    """The timed launches run kernels instantiated for the case at hand (one thread per point known at compile time; an
+    explicit contour policy known at compile time); the counted launch runs the general kernel.  Same arithmetic in the
+    same order: identical results."""
+    cfg = W.CONFIGS["cfg2_mid"]   # one thread per point
+    x = gpu_grid(gf, cfg)
+    for contour in ("real", "ray_arc", "thread", "auto"):
+        P, rn, rw, z, wz = gpu_setup(gf, cfg, contour=contour)
+        g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+        g2, _ = gf.eval_grid_counted(P, rn, rw, cfg["n_rad"], z, wz, x)
+        assert torch.equal(g.view(torch.float64), g2.view(torch.float64)), contour
+    cfg = W.CONFIGS["cfg1_tiny"]  # several lanes per point: the general kernel either way, here for the policies
+    x = gpu_grid(gf, cfg)
+    for contour in ("ray_arc", "thread"):
+        P, rn, rw, z, wz = gpu_setup(gf, cfg, contour=contour)
+        g = gf.eval_grid(P, rn, rw, cfg["n_rad"], z, wz, x)
+        g2, _ = gf.eval_grid_counted(P, rn, rw, cfg["n_rad"], z, wz, x)
+        assert torch.equal(g.view(torch.float64), g2.view(torch.float64)), contour
+
+
 def test_route_counters(gf):
     """Every (point, node, pole) triple takes exactly one route; the counted call returns the same G.  Config 2's rule
     (64 folded pairs) is not split (rules of 128 and more are); a rule of 256 folded pairs is split into 8 blocks of 32, and a direct node-term
