@@ -560,7 +560,14 @@ int gf_eval_grid_host(const gf_params* p, const double* h_rad_nodes, const doubl
   for (int c = 0; c < n_chunks && !rc; ++c) {
     // boundaries on multiples of the CTA size: every warp holds the same points as in one launch over all of x,
     // so the chunked result is bit-identical to gf_eval_grid's (the series loop runs to the warp's longest series)
-    auto cut = [&](int k) { return k >= n_chunks ? n_points : (n_points * k / n_chunks) / kBlockThreads * kBlockThreads; };
+    // With the full eight chunks the first and the last are small (1/32 of the points, then 3/32, the middle four 6/32
+    // each): the copy in of the first chunk and the copy out of the last are the only ones nothing overlaps
+    static const int kRamp[kMaxChunks + 1] = {0, 1, 4, 10, 16, 22, 28, 31, 32};
+    auto cut = [&](int k) {
+      if (k >= n_chunks) return n_points;
+      const long long at = n_chunks == kMaxChunks ? n_points * kRamp[k] / 32 : n_points * k / n_chunks;
+      return at / kBlockThreads * kBlockThreads;
+    };
     const long long p0 = cut(c), p1 = cut(c + 1), np = p1 - p0;
     // odd chunks are evaluated on a second stream, so that the last, partly filled wave of CTAs of one chunk
     // overlaps the first waves of the next
