@@ -209,6 +209,8 @@ int gf_eval_grid(const gf_params* p, const double* d_rad_nodes, const double* d_
  *   Limit: parameters and orders whose gf_eval_workspace_size() exceeds GF_STATIC_WORKSPACE_BYTES are refused with
  *          GF_ERR_ARG and a message that names both sizes (the configs of this repository need 0.2 to 26 MiB).
  *   Cost:  every GPU that loads the library holds the array until the process exits.
+ *   First call: looks up the array's device address (cudaGetSymbolAddress, once per device) and may set a kernel's
+ *          shared-memory attribute; make one call per device outside a stream capture before capturing calls.
  *   Sharing: every call on a device uses the same array, which keeps the last call's tables (each call rewrites all
  *          it reads and resets the header first).  Calls that OVERLAP on the GPU (two streams, two host threads) race on
  *          it: issue them on one stream, or order them with events.  Other devices have their own copy.
