@@ -117,6 +117,18 @@ def test_argument_errors_without_gpu(gf):
     assert L.gf_eval_launch_info(ctypes.byref(P), 64, 32, 4096, ctypes.byref(info)) == 3
     assert L.gf_make_grid(0.0, 1.0, 4, 0.0, 1.0, 4, 0, 0.0, None, None) == 1
     assert L.gf_make_quadrature_host(9, 4, 0.0, 0, None, None) != 0
+    # gf_eval_grid_static checks its arguments and the size of the workspace before any CUDA call
+    P = gf.make_params(bub, bub, 1e4)
+    assert L.gf_eval_grid_static(ctypes.byref(P), None, None, 64, None, None, 32, None, 0, None, None) == 1
+    assert L.gf_eval_grid_static(None, None, None, 64, None, None, 32, None, 0, None, None) == 1
+    buf = (ctypes.c_double * 4)()
+    ptr = ctypes.addressof(buf)   # never dereferenced on the paths below
+    assert L.gf_eval_grid_static(ctypes.byref(P), ptr, ptr, 0, ptr, ptr, 32, ptr, 2, ptr, None) == 2
+    Pa = gf.make_params(bub, bub, 1e4, contour="auto")
+    need = L.gf_eval_workspace_size(ctypes.byref(Pa), 2048, 32)
+    assert need > gf.STATIC_WORKSPACE_BYTES
+    assert L.gf_eval_grid_static(ctypes.byref(Pa), ptr, ptr, 2048, ptr, ptr, 32, ptr, 2, ptr, None) == 2
+    assert b"GF_STATIC_WORKSPACE_BYTES" in L.gf_last_error() and str(need).encode() in L.gf_last_error()
     assert gf.radial_table_size("real", 64) == 64
     assert gf.radial_table_size("auto", 64) == 64 + 32 + 16 + 8
     assert gf.radial_table_size("auto", 63) == -1
